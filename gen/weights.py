@@ -1,0 +1,120 @@
+"""Seeded weights and the WMW1 weight-file writer (format: include/wm.h).
+
+Draw order (one Generator(PCG64(weight_seed))):
+  embedding (E, W_p, b_p | Tbl), transition (W1, b1, W2, b2[, gamma, beta] | W_g, W_r, W_h),
+  scorer layers first to last (W, b each).
+Matrices ~ N(0, 1/fan_in) (variance), tables ~ N(0,1), biases ~ N(0, 1/fan_in) of their layer,
+gamma = 1 + 0.1 N(0,1), beta = 0.1 N(0,1).  bf16 configs: every tensor is rounded to the nearest-even
+bf16 value and stored as fp32 (S14), so every consumer sees identical weights.
+"""
+from __future__ import annotations
+
+import struct
+from typing import Dict, List
+
+import numpy as np
+
+from .configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, DTYPE_BF16, EMBED_LINEAR, EMBED_BUCKET)
+
+MAGIC = b"WMW1"
+VERSION = 1
+MAX_SCORER_HIDDEN = 6
+
+
+def round_to_bf16(x: np.ndarray) -> np.ndarray:
+    """Round fp32 values to the nearest-even bf16 value, returned as fp32."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    u = x.view(np.uint32).astype(np.uint64)
+    u = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
+    return u.astype(np.uint32).view(np.float32).reshape(x.shape)
+
+
+def tensor_order(cfg: WMConfig) -> List[str]:
+    """Names of the tensors in file order."""
+    names: List[str] = []
+    if cfg.embed == EMBED_LINEAR:
+        names += ["E", "W_p", "b_p"]
+    else:
+        names += ["Tbl"]
+    if cfg.kind in (KIND_MLP, KIND_MLP_LN):
+        names += ["W1", "b1", "W2", "b2"]
+        if cfg.kind == KIND_MLP_LN:
+            names += ["gamma", "beta"]
+    else:
+        names += ["W_g", "W_r", "W_h"]
+    for i in range(len(cfg.scorer_widths) + 1):
+        names += [f"Ws{i}", f"bs{i}"]
+    return names
+
+
+def tensor_shapes(cfg: WMConfig) -> Dict[str, tuple]:
+    d, da, hid = cfg.d, cfg.d_a, cfg.hidden
+    sh: Dict[str, tuple] = {}
+    if cfg.embed == EMBED_LINEAR:
+        sh["E"] = (cfg.n_types, da)
+        sh["W_p"] = (da, cfg.P)
+        sh["b_p"] = (da,)
+    else:
+        sh["Tbl"] = (cfg.n_types * cfg.P * cfg.n_buckets, da)
+    if cfg.kind in (KIND_MLP, KIND_MLP_LN):
+        sh["W1"] = (hid, d + da)
+        sh["b1"] = (hid,)
+        sh["W2"] = (d, hid)
+        sh["b2"] = (d,)
+        if cfg.kind == KIND_MLP_LN:
+            sh["gamma"] = (d,)
+            sh["beta"] = (d,)
+    else:
+        for n in ("W_g", "W_r", "W_h"):
+            sh[n] = (d, d + da)
+    dims = (cfg.scorer_in,) + tuple(cfg.scorer_widths) + (1,)
+    for i, (a, b) in enumerate(zip(dims[:-1], dims[1:])):
+        sh[f"Ws{i}"] = (b, a)
+        sh[f"bs{i}"] = (b,)
+    return sh
+
+
+def make_weights(cfg: WMConfig) -> Dict[str, np.ndarray]:
+    rng = np.random.Generator(np.random.PCG64(cfg.weight_seed))
+    shapes = tensor_shapes(cfg)
+    w: Dict[str, np.ndarray] = {}
+    for name in tensor_order(cfg):
+        shp = shapes[name]
+        if name in ("E", "Tbl"):
+            t = rng.standard_normal(shp)
+        elif name == "gamma":
+            t = 1.0 + 0.1 * rng.standard_normal(shp)
+        elif name == "beta":
+            t = 0.1 * rng.standard_normal(shp)
+        elif len(shp) == 2:
+            t = rng.standard_normal(shp) / np.sqrt(shp[1])
+        else:  # bias of the layer drawn just before it
+            fan_in = shapes[_matrix_of(name)][1]
+            t = rng.standard_normal(shp) / np.sqrt(fan_in)
+        t = t.astype(np.float32)
+        if cfg.dtype == DTYPE_BF16:
+            t = round_to_bf16(t)
+        w[name] = t
+    return w
+
+
+def _matrix_of(bias: str) -> str:
+    return {"b_p": "W_p", "b1": "W1", "b2": "W2"}.get(bias, "Ws" + bias[2:])
+
+
+def header_bytes(cfg: WMConfig) -> bytes:
+    widths = list(cfg.scorer_widths) + [0] * (MAX_SCORER_HIDDEN - len(cfg.scorer_widths))
+    return MAGIC + struct.pack(
+        "<12I%dIf" % MAX_SCORER_HIDDEN,
+        VERSION, cfg.kind, cfg.dtype, cfg.embed, cfg.d, cfg.d_a, cfg.hidden, cfg.n_types, cfg.P,
+        cfg.n_buckets, cfg.H, len(cfg.scorer_widths) + 1, *widths, cfg.ln_eps)
+
+
+def write_weight_file(path: str, cfg: WMConfig, weights: Dict[str, np.ndarray]) -> None:
+    shapes = tensor_shapes(cfg)
+    with open(path, "wb") as f:
+        f.write(header_bytes(cfg))
+        for name in tensor_order(cfg):
+            t = np.ascontiguousarray(weights[name], dtype="<f4")
+            assert t.shape == shapes[name], (name, t.shape, shapes[name])
+            f.write(t.tobytes())

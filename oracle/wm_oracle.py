@@ -1,0 +1,363 @@
+"""Float64 CPU oracle for the batched candidate evaluator.  TEST INFRASTRUCTURE ONLY.
+
+What it computes is the plain definition (no approximation in the method, so no algorithm to follow):
+
+    z_0 = init_states[s]                                   PAPER.md:215 ("initial tensor-program state of the task")
+    z_t = F(z_{t-1}, a_t),  t = 1..len                     PAPER.md:68-71 Eq.1, :162 Eq.8, :166 (recurrent rollout)
+    steps with t > len leave z unchanged                   PAPER.md:176 Eq.11 (rollout mask m_t)
+    phi = mean_t a_t (0 if len = 0)                        PAPER.md:186 (action features; BASELINE.json cfg 1 form)
+    y   = G([z_T ; phi ; h])                               PAPER.md:122 Eq.3, :188 Eq.12
+    top-k per subgraph by (score desc, index asc)
+
+with the network shapes BASELINE.json's configs bind (F = residual MLP [+LayerNorm] or GRU-style gate,
+G = MLP, embedding = table + Linear(log2 params) or bucketed table); readings S1..S23 in DESIGN.md §3.
+
+Everything is numpy float64; weights arrive as the dict gen.make_weights() returns (or read_weight_file()).
+Two implementations: `rollout_score_vec` (loop over t, matmul over one subgraph's candidates, np.where
+mask) and `rollout_score_scalar` (pure per-candidate python loops, math.erf) — the second pins the first.
+
+Pins (tests/test_oracle_pins.py): P1..P13 of SURVEY.md §8(c) — hand-expanded 2x3 MLP step and GRU step
+(values in tests/golden/), closed forms, torch float64 library cross-checks, scalar-vs-vector brute
+force, top-k vs full sort.  The paper prints no worked numeric example of this path, so the composition
+at full size rests on those pins: beyond them, parity unpinned.
+"""
+from __future__ import annotations
+
+import math
+import struct
+from typing import Dict, Optional, Tuple
+
+import numpy as np
+from scipy.special import erf as _erf
+
+KIND_MLP, KIND_MLP_LN, KIND_GRU = 0, 1, 2
+EMBED_LINEAR, EMBED_BUCKET = 0, 1
+F64 = np.float64
+
+
+# ----------------------------------------------------------------------------- pieces
+
+def gelu(x: np.ndarray) -> np.ndarray:
+    """Exact GELU x*Phi(x) (S5)."""
+    x = np.asarray(x, dtype=F64)
+    return 0.5 * x * (1.0 + _erf(x / math.sqrt(2.0)))
+
+
+def layer_norm(v: np.ndarray, gamma: np.ndarray, beta: np.ndarray, eps: float) -> np.ndarray:
+    """LayerNorm over the last axis, population variance (S6; PAPER.md:164 'finally normalized')."""
+    v = np.asarray(v, dtype=F64)
+    mean = v.mean(axis=-1, keepdims=True)
+    var = ((v - mean) ** 2).mean(axis=-1, keepdims=True)
+    return gamma * (v - mean) / np.sqrt(var + eps) + beta
+
+
+def embed_linear(ids: np.ndarray, params: np.ndarray, E, W_p, b_p) -> np.ndarray:
+    """a = E[id] + W_p @ log2(p) + b_p   (configs 1-4; north_star 'token-id gather plus projection')."""
+    lp = np.log2(np.asarray(params, dtype=F64))
+    return np.asarray(E, F64)[ids] + lp @ np.asarray(W_p, F64).T + np.asarray(b_p, F64)
+
+
+def bucket_index(p: int, n_buckets: int) -> int:
+    """Quarter-octave bucket min(n_b-1, floor(4*log2 p)) in exact integer arithmetic (S10)."""
+    return min(n_buckets - 1, (int(p) ** 4).bit_length() - 1)
+
+
+def embed_bucket(ids: np.ndarray, params: np.ndarray, Tbl, P: int, n_buckets: int) -> np.ndarray:
+    """a = sum_j Tbl[(id*P + j)*n_b + bucket(p_j)]   (config 5, S10)."""
+    ids = np.asarray(ids)
+    params = np.asarray(params)
+    Tbl = np.asarray(Tbl, F64)
+    flat_p = params.reshape(-1, P)
+    flat_id = ids.reshape(-1)
+    out = np.zeros((flat_id.shape[0], Tbl.shape[1]), dtype=F64)
+    bk = np.array([[bucket_index(int(p), n_buckets) for p in row] for row in flat_p], dtype=np.int64) \
+        if flat_p.size < 4096 else _bucket_vec(flat_p, n_buckets)
+    for j in range(P):
+        out += Tbl[(flat_id.astype(np.int64) * P + j) * n_buckets + bk[:, j]]
+    return out.reshape(ids.shape + (Tbl.shape[1],))
+
+
+def _bucket_vec(p: np.ndarray, n_buckets: int) -> np.ndarray:
+    """Vectorised bucket_index: p^4 < 2^63 for p <= 32767, bit_length via exact integer compares."""
+    p4 = p.astype(np.int64) ** 4
+    bl = np.zeros(p4.shape, dtype=np.int64)
+    for b in range(1, 63):
+        bl += (p4 >= (np.int64(1) << np.int64(b))).astype(np.int64)
+    return np.minimum(n_buckets - 1, bl)
+
+
+def step_mlp(z, a, W1, b1, W2, b2, gamma=None, beta=None, eps: float = 1e-5) -> np.ndarray:
+    """z' = z + W2 gelu(W1 [z;a] + b1) + b2, then LayerNorm if gamma is given (cfg 1 / cfg 2-4)."""
+    x = np.concatenate([z, a], axis=-1)
+    u = x @ np.asarray(W1, F64).T + np.asarray(b1, F64)
+    v = z + gelu(u) @ np.asarray(W2, F64).T + np.asarray(b2, F64)
+    if gamma is None:
+        return v
+    return layer_norm(v, np.asarray(gamma, F64), np.asarray(beta, F64), eps)
+
+
+def _sigmoid(x):
+    return 1.0 / (1.0 + np.exp(-x))
+
+
+def step_gru(z, a, W_g, W_r, W_h) -> np.ndarray:
+    """g=s(W_g[z;a]); r=s(W_r[z;a]); z'=(1-g) z + g tanh(W_h [r*z; a])   (cfg 5)."""
+    x = np.concatenate([z, a], axis=-1)
+    g = _sigmoid(x @ np.asarray(W_g, F64).T)
+    r = _sigmoid(x @ np.asarray(W_r, F64).T)
+    h = np.tanh(np.concatenate([r * z, a], axis=-1) @ np.asarray(W_h, F64).T)
+    return (1.0 - g) * z + g * h
+
+
+def scorer(x: np.ndarray, w: Dict[str, np.ndarray], n_layers: int) -> np.ndarray:
+    """G as an MLP: hidden linears followed by GELU, last linear plain (S8). Returns [...]."""
+    for i in range(n_layers):
+        x = x @ np.asarray(w[f"Ws{i}"], F64).T + np.asarray(w[f"bs{i}"], F64)
+        if i + 1 < n_layers:
+            x = gelu(x)
+    return x[..., 0]
+
+
+def _n_scorer_layers(w) -> int:
+    n = 0
+    while f"Ws{n}" in w:
+        n += 1
+    return n
+
+
+def _kind(w) -> int:
+    if "W_g" in w:
+        return KIND_GRU
+    return KIND_MLP_LN if "gamma" in w else KIND_MLP
+
+
+def _embed(w, ids, params, P, n_buckets):
+    if "Tbl" in w:
+        return embed_bucket(ids, params, w["Tbl"], P, n_buckets)
+    return embed_linear(ids, params, w["E"], w["W_p"], w["b_p"])
+
+
+def _step(w, z, a, eps):
+    k = _kind(w)
+    if k == KIND_GRU:
+        return step_gru(z, a, w["W_g"], w["W_r"], w["W_h"])
+    if k == KIND_MLP_LN:
+        return step_mlp(z, a, w["W1"], w["b1"], w["W2"], w["b2"], w["gamma"], w["beta"], eps)
+    return step_mlp(z, a, w["W1"], w["b1"], w["W2"], w["b2"])
+
+
+# ----------------------------------------------------------------------------- the path
+
+def rollout_score_vec(w: Dict[str, np.ndarray], init_states, action_ids, action_params, lengths, hw_feats,
+                      subgraph_offsets: Optional[np.ndarray], n_buckets: int = 0, ln_eps: float = 1e-5,
+                      return_latent: bool = False):
+    """Scores [B] float64.  subgraph_offsets None => per-candidate init_states [B,d] / hw_feats [B,H] (S1/S2)."""
+    ids = np.asarray(action_ids)
+    par = np.asarray(action_params)
+    lens = np.asarray(lengths).astype(np.int64)
+    B, T = ids.shape
+    P = par.shape[2]
+    z0 = np.asarray(init_states, F64)
+    hw = np.asarray(hw_feats, F64)
+    nl = _n_scorer_layers(w)
+    if subgraph_offsets is None:
+        segs = [(i, i + 1, i) for i in range(B)] if B else []
+        # one block over all candidates is the same computation; keep per-candidate rows together
+        segs = [(0, B, None)] if B else []
+    else:
+        off = np.asarray(subgraph_offsets).astype(np.int64)
+        segs = [(int(off[s]), int(off[s + 1]), s) for s in range(len(off) - 1)]
+    scores = np.zeros(B, dtype=F64)
+    lat = np.zeros((B, z0.shape[1]), dtype=F64) if return_latent else None
+    da = (w["Tbl"] if "Tbl" in w else w["E"]).shape[1]
+    for lo, hi, s in segs:
+        n = hi - lo
+        if n <= 0:
+            continue
+        z = z0[lo:hi].copy() if s is None else np.repeat(z0[s][None, :], n, axis=0)
+        h = hw[lo:hi] if s is None else np.repeat(hw[s][None, :], n, axis=0)
+        ln = lens[lo:hi]
+        asum = np.zeros((n, da), dtype=F64)
+        for t in range(int(ln.max()) if n else 0):
+            act = ln > t                               # rollout mask m_t
+            idx = np.nonzero(act)[0]
+            if idx.size == 0:
+                break
+            a = _embed(w, ids[lo:hi][idx, t], par[lo:hi][idx, t, :], P, n_buckets)
+            asum[idx] += a
+            z[idx] = _step(w, z[idx], a, ln_eps)       # masked rows keep z unchanged
+        phi = np.where(ln[:, None] > 0, asum / np.maximum(ln, 1)[:, None], 0.0)
+        scores[lo:hi] = scorer(np.concatenate([z, phi, h], axis=-1), w, nl)
+        if return_latent:
+            lat[lo:hi] = z
+    return (scores, lat) if return_latent else scores
+
+
+def rollout_score_scalar(w, init_states, action_ids, action_params, lengths, hw_feats, subgraph_offsets,
+                         n_buckets: int = 0, ln_eps: float = 1e-5) -> np.ndarray:
+    """Pure-python per-candidate loops (tiny inputs only); independent of the vector code above."""
+    W = {k: np.asarray(v, F64).tolist() for k, v in w.items()}
+    ids = np.asarray(action_ids).tolist()
+    par = np.asarray(action_params).tolist()
+    lens = [int(x) for x in np.asarray(lengths)]
+    z0 = np.asarray(init_states, F64).tolist()
+    hw = np.asarray(hw_feats, F64).tolist()
+    B = len(lens)
+    seg_of = list(range(B))
+    if subgraph_offsets is not None:
+        off = [int(x) for x in subgraph_offsets]
+        for s in range(len(off) - 1):
+            for b in range(off[s], off[s + 1]):
+                seg_of[b] = s
+    kind = _kind(w)
+    P = len(par[0][0]) if B and len(par[0]) else 0
+
+    def mv(M, x):
+        return [sum(mij * xj for mij, xj in zip(row, x)) for row in M]
+
+    def gelu1(x):
+        return 0.5 * x * (1.0 + math.erf(x / math.sqrt(2.0)))
+
+    def sig(x):
+        return 1.0 / (1.0 + math.exp(-x))
+
+    out = []
+    for b in range(B):
+        s = seg_of[b]
+        z = list(z0[s])
+        d = len(z)
+        da = len(W["Tbl"][0]) if "Tbl" in W else len(W["E"][0])
+        asum = [0.0] * da
+        for t in range(lens[b]):
+            if "Tbl" in W:
+                a = [0.0] * da
+                for j in range(P):
+                    row = W["Tbl"][(ids[b][t] * P + j) * n_buckets + bucket_index(par[b][t][j], n_buckets)]
+                    a = [x + y for x, y in zip(a, row)]
+            else:
+                lp = [math.log2(p) for p in par[b][t]]
+                a = [e + q + c for e, q, c in zip(W["E"][ids[b][t]], mv(W["W_p"], lp), W["b_p"])]
+            asum = [x + y for x, y in zip(asum, a)]
+            if kind == KIND_GRU:
+                x = z + a
+                g = [sig(u) for u in mv(W["W_g"], x)]
+                r = [sig(u) for u in mv(W["W_r"], x)]
+                hcand = [math.tanh(u) for u in mv(W["W_h"], [ri * zi for ri, zi in zip(r, z)] + a)]
+                z = [(1.0 - gi) * zi + gi * hi for gi, zi, hi in zip(g, z, hcand)]
+            else:
+                u = [ui + bi for ui, bi in zip(mv(W["W1"], z + a), W["b1"])]
+                hdn = [gelu1(ui) for ui in u]
+                v = [zi + wi + bi for zi, wi, bi in zip(z, mv(W["W2"], hdn), W["b2"])]
+                if kind == KIND_MLP_LN:
+                    m = sum(v) / d
+                    var = sum((vi - m) ** 2 for vi in v) / d
+                    z = [g_ * (vi - m) / math.sqrt(var + ln_eps) + b_
+                         for g_, vi, b_ in zip(W["gamma"], v, W["beta"])]
+                else:
+                    z = v
+        phi = [x / lens[b] for x in asum] if lens[b] > 0 else [0.0] * da
+        x = z + phi + list(hw[s])
+        nl = _n_scorer_layers(w)
+        for i in range(nl):
+            x = [ui + bi for ui, bi in zip(mv(W[f"Ws{i}"], x), W[f"bs{i}"])]
+            if i + 1 < nl:
+                x = [gelu1(ui) for ui in x]
+        out.append(x[0])
+    return np.array(out, dtype=F64)
+
+
+def topk_segments(scores, subgraph_offsets, k: int) -> np.ndarray:
+    """idx_out [S,k] int32: per segment the first min(k,n_s) candidates of the order (score desc, index asc),
+    global indices, -1 fill (S16).  -0.0 == +0.0; NaN ranks below every number (ties by index)."""
+    sc = np.asarray(scores)
+    off = [int(x) for x in subgraph_offsets]
+    S = len(off) - 1
+    out = np.full((S, k), -1, dtype=np.int32)
+    for s in range(S):
+        items = []
+        for i in range(off[s], off[s + 1]):
+            v = float(sc[i])
+            key = (1, 0.0) if math.isnan(v) else (0, -(v + 0.0))
+            items.append((key, i))
+        items.sort()
+        for j, (_, i) in enumerate(items[:k]):
+            out[s, j] = i
+    return out
+
+
+# ----------------------------------------------------------------------------- metrics (S15)
+
+def score_error(y_gpu, y_ref, subgraph_offsets) -> float:
+    """max_b |y - yref| / max(|yref|, RMS_s(yref))  (S15: relative error with a per-subgraph RMS floor)."""
+    y_gpu = np.asarray(y_gpu, F64)
+    y_ref = np.asarray(y_ref, F64)
+    if y_ref.size == 0:
+        return 0.0
+    floor = np.zeros_like(y_ref)
+    if subgraph_offsets is None:
+        floor[:] = math.sqrt(float(np.mean(y_ref ** 2)))
+    else:
+        off = [int(x) for x in subgraph_offsets]
+        for s in range(len(off) - 1):
+            seg = y_ref[off[s]:off[s + 1]]
+            if seg.size:
+                floor[off[s]:off[s + 1]] = math.sqrt(float(np.mean(seg ** 2)))
+    den = np.maximum(np.abs(y_ref), floor)
+    den = np.where(den == 0.0, 1.0, den)
+    return float(np.max(np.abs(y_gpu - y_ref) / den))
+
+
+def topk_overlap(idx_a, idx_b) -> Tuple[float, float]:
+    """(mean, min) over segments of |A ∩ B| / |B valid|  (S15)."""
+    vals = []
+    for ra, rb in zip(np.asarray(idx_a), np.asarray(idx_b)):
+        sb = set(int(x) for x in rb if x >= 0)
+        if not sb:
+            continue
+        sa = set(int(x) for x in ra if x >= 0)
+        vals.append(len(sa & sb) / len(sb))
+    if not vals:
+        return 1.0, 1.0
+    return float(np.mean(vals)), float(np.min(vals))
+
+
+# ----------------------------------------------------------------------------- weight file (own reader)
+
+def read_weight_file(path: str):
+    """Independent reader of the WMW1 format (include/wm.h). Returns (header dict, weights dict)."""
+    with open(path, "rb") as f:
+        raw = f.read()
+    if raw[:4] != b"WMW1":
+        raise ValueError("bad magic")
+    vals = struct.unpack_from("<12I6If", raw, 4)
+    (version, kind, dtype, embed, d, d_a, hidden, n_types, P, n_buckets, H, n_lin) = vals[:12]
+    widths = [x for x in vals[12:18]][: n_lin - 1]
+    eps = vals[18]
+    hdr = dict(version=version, kind=kind, dtype=dtype, embed=embed, d=d, d_a=d_a, hidden=hidden,
+               n_types=n_types, P=P, n_buckets=n_buckets, H=H, n_scorer_layers=n_lin,
+               scorer_widths=widths, ln_eps=eps)
+    pos = 4 + struct.calcsize("<12I6If")
+    w = {}
+
+    def take(name, *shape):
+        nonlocal pos
+        n = int(np.prod(shape))
+        w[name] = np.frombuffer(raw, dtype="<f4", count=n, offset=pos).reshape(shape).copy()
+        pos += 4 * n
+
+    if embed == EMBED_LINEAR:
+        take("E", n_types, d_a); take("W_p", d_a, P); take("b_p", d_a)
+    else:
+        take("Tbl", n_types * P * n_buckets, d_a)
+    if kind in (KIND_MLP, KIND_MLP_LN):
+        take("W1", hidden, d + d_a); take("b1", hidden); take("W2", d, hidden); take("b2", d)
+        if kind == KIND_MLP_LN:
+            take("gamma", d); take("beta", d)
+    else:
+        take("W_g", d, d + d_a); take("W_r", d, d + d_a); take("W_h", d, d + d_a)
+    dims = [d + d_a + H] + widths + [1]
+    for i in range(n_lin):
+        take(f"Ws{i}", dims[i + 1], dims[i]); take(f"bs{i}", dims[i + 1])
+    if pos != len(raw):
+        raise ValueError("trailing bytes in weight file")
+    return hdr, w

@@ -1,0 +1,30 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box via gpurun)")
+
+
+def read_golden(name):
+    """Parse tests/golden/<name>: '#' comments, then 'key v0 v1 ...' lines -> dict of float lists."""
+    out = {}
+    with open(os.path.join(ROOT, "tests", "golden", name)) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            parts = line.split()
+            out.setdefault(parts[0], []).append([float(x) for x in parts[1:]])
+    return {k: (v[0] if len(v) == 1 else v) for k, v in out.items()}
+
+
+@pytest.fixture(scope="session")
+def golden():
+    return read_golden

@@ -1,0 +1,332 @@
+"""Pins for the float64 oracle.  CPU only.
+
+Each pin checks the oracle against something other than itself: hand-expanded fixtures under
+tests/golden/, closed forms, torch float64 library routines, brute force (scalar loops) and the
+invariants BASELINE.json's north_star lists.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import gen
+import oracle
+from gen.configs import WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, DTYPE_FP32, EMBED_LINEAR, EMBED_BUCKET
+
+
+def tiny_cfg(kind=KIND_MLP_LN, embed=EMBED_LINEAR, S=3, n=7, T=5, d=6, da=4, hid=8, H=3, widths=(5, 4),
+             number=9, len_lo=0):
+    return WMConfig("tiny", number, kind, DTYPE_FP32, embed, S=S, per_subgraph=n, T_max=T,
+                    len_dist="uniform", len_lo=len_lo, len_hi=T, n_types=5, P=3,
+                    param_dist="loguniform", param_hi=1024, n_buckets=40 if embed == EMBED_BUCKET else 0,
+                    d=d, d_a=da, hidden=0 if kind == KIND_GRU else hid, H=H, scorer_widths=widths, k=3)
+
+
+def run_vec(cfg, w, b, **kw):
+    return oracle.rollout_score_vec(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.hw_feats,
+                                    b.subgraph_offsets, n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps, **kw)
+
+
+ALL_KINDS = [(KIND_MLP, EMBED_LINEAR), (KIND_MLP_LN, EMBED_LINEAR), (KIND_GRU, EMBED_BUCKET),
+             (KIND_GRU, EMBED_LINEAR), (KIND_MLP_LN, EMBED_BUCKET)]
+
+
+# ---- P4 / P5 / P6 / P11: hand-expanded fixtures ---------------------------------------------------
+
+def test_p4_mlp_step_hand_expanded(golden):
+    g = golden("p4_mlp_step.txt")
+    z = np.array([[1.0, 2.0]]); a = np.array([[3.0]])
+    W1 = [[1, 0, -1], [2, 1, 0]]; b1 = [0.5, -1.0]; W2 = [[1, 1], [0, 2]]; b2 = [0.25, -0.5]
+    np.testing.assert_allclose(oracle.gelu(np.array(g["u"])), g["gelu"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(oracle.step_mlp(z, a, W1, b1, W2, b2)[0], g["z_next"], rtol=0, atol=1e-14)
+    out = oracle.step_mlp(z, a, W1, b1, W2, b2, gamma=np.ones(2), beta=np.zeros(2), eps=1e-5)[0]
+    np.testing.assert_allclose(out, g["z_next_ln"], rtol=0, atol=1e-13)
+    # a transposed W1 or a dropped bias must fail: sanity that the fixture discriminates
+    bad = oracle.step_mlp(z, a, W1, [0.0, 0.0], W2, b2)[0]
+    assert np.abs(bad - np.array(g["z_next"])).max() > 1e-2
+
+
+def test_p5_layernorm_closed_form(golden):
+    g = golden("p5_layernorm.txt")
+    x = np.array([1.0, 2.0, 3.0, 4.0])
+    np.testing.assert_allclose(oracle.layer_norm(x, 1.0, 0.0, 0.0), g["eps0"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(oracle.layer_norm(x, 1.0, 0.0, 1e-5), g["eps1e-5"], rtol=0, atol=1e-15)
+
+
+def test_p6_gru_step_hand_expanded(golden):
+    g = golden("p6_gru_step.txt")
+    z = np.array([[1.0, -2.0]]); a = np.array([[0.5]])
+    W_g = [[1, 0, 2], [0, 1, -2]]; W_r = [[0, 1, 0], [1, 0, 0]]; W_h = [[1, 1, 1], [1, -1, 2]]
+    np.testing.assert_allclose(oracle.step_gru(z, a, W_g, W_r, W_h)[0], g["z_next"], rtol=0, atol=1e-14)
+
+
+def test_p11_bucket_function(golden):
+    g = golden("p11_buckets.txt")
+    for p, bk in g.items():
+        assert oracle.bucket_index(int(p), 40) == int(bk[0])
+    # integer formula equals floor(4*log2 p) wherever floating point is unambiguous, for all p in 1..1024
+    for p in range(1, 1025):
+        x = 4 * math.log2(p)
+        if abs(x - round(x)) > 1e-9:
+            assert oracle.bucket_index(p, 40) == min(39, math.floor(x))
+        else:
+            assert oracle.bucket_index(p, 40) == min(39, round(x))
+    ps = np.arange(1, 1025).reshape(-1, 1)
+    vec = oracle.wm_oracle._bucket_vec(ps, 40)[:, 0]
+    assert all(int(vec[i]) == oracle.bucket_index(i + 1, 40) for i in range(1024))
+
+
+# ---- P1 / P2 / P3 / P13: invariants -----------------------------------------------------------------
+
+@pytest.mark.parametrize("kind,embed", ALL_KINDS)
+def test_p1_zero_length_returns_initial_state(kind, embed):
+    cfg = tiny_cfg(kind, embed)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    b.lengths[:] = 0
+    y, lat = run_vec(cfg, w, b, return_latent=True)
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    np.testing.assert_array_equal(lat, b.init_states[seg].astype(np.float64))
+    x = np.concatenate([b.init_states[seg], np.zeros((cfg.B, cfg.d_a)), b.hw_feats[seg]], -1).astype(np.float64)
+    np.testing.assert_allclose(y, oracle.scorer(x, w, len(cfg.scorer_widths) + 1), rtol=0, atol=0)
+
+
+@pytest.mark.parametrize("kind,embed", ALL_KINDS)
+def test_p2_padding_invariance(kind, embed):
+    cfg = tiny_cfg(kind, embed)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg, sentinel_padding=True)
+    y1 = run_vec(cfg, w, b)
+    b2 = gen.make_inputs(cfg, sentinel_padding=False)       # padding holds ordinary random draws instead
+    assert (b2.action_ids != b.action_ids).any()
+    y2 = run_vec(cfg, w, b2)
+    np.testing.assert_array_equal(y1, y2)                  # bit-identical
+
+
+@pytest.mark.parametrize("kind,embed", ALL_KINDS)
+def test_p3_permutation_equivariance_and_subgraph_move(kind, embed):
+    cfg = tiny_cfg(kind, embed)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    y = run_vec(cfg, w, b)
+    rng = np.random.default_rng(5)
+    n = cfg.per_subgraph
+    perm = np.concatenate([s * n + rng.permutation(n) for s in range(cfg.S)])
+    yp = oracle.rollout_score_vec(w, b.init_states, b.action_ids[perm], b.action_params[perm], b.lengths[perm],
+                                  b.hw_feats, b.subgraph_offsets, n_buckets=cfg.n_buckets)
+    np.testing.assert_allclose(yp, y[perm], rtol=0, atol=1e-13)
+    # two subgraphs with equal z0/hw: a candidate scores the same in either
+    z0 = b.init_states.copy(); hw = b.hw_feats.copy()
+    z0[1] = z0[0]; hw[1] = hw[0]
+    ids = b.action_ids.copy(); par = b.action_params.copy(); ln = b.lengths.copy()
+    ids[n] = ids[0]; par[n] = par[0]; ln[n] = ln[0]
+    ym = oracle.rollout_score_vec(w, z0, ids, par, ln, hw, b.subgraph_offsets, n_buckets=cfg.n_buckets)
+    assert abs(ym[n] - ym[0]) < 1e-13
+
+
+@pytest.mark.parametrize("kind,embed", ALL_KINDS)
+def test_p13_batch_independence_and_per_candidate_mode(kind, embed):
+    cfg = tiny_cfg(kind, embed)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    y = run_vec(cfg, w, b)
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    for i in (0, 5, cfg.B - 1):
+        yi = oracle.rollout_score_vec(w, b.init_states[seg[i]][None], b.action_ids[i:i + 1],
+                                      b.action_params[i:i + 1], b.lengths[i:i + 1], b.hw_feats[seg[i]][None],
+                                      np.array([0, 1]), n_buckets=cfg.n_buckets)
+        assert abs(yi[0] - y[i]) < 1e-13
+    ypc = oracle.rollout_score_vec(w, b.init_states[seg], b.action_ids, b.action_params, b.lengths,
+                                   b.hw_feats[seg], None, n_buckets=cfg.n_buckets)
+    np.testing.assert_allclose(ypc, y, rtol=0, atol=1e-13)
+
+
+# ---- P7: closed forms ---------------------------------------------------------------------------------
+
+def test_p7_closed_forms():
+    cfg = tiny_cfg(KIND_MLP, len_lo=1)
+    b = gen.make_inputs(cfg)
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    z0 = b.init_states[seg].astype(np.float64)
+    # (a) W1 = 0, no LN: z_T = z_0 + T (W2 gelu(b1) + b2)
+    w = gen.make_weights(cfg); w["W1"] = np.zeros_like(w["W1"])
+    _, lat = run_vec(cfg, w, b, return_latent=True)
+    inc = w["W2"].astype(np.float64) @ oracle.gelu(w["b1"].astype(np.float64)) + w["b2"]
+    np.testing.assert_allclose(lat, z0 + b.lengths[:, None] * inc[None, :], rtol=0, atol=1e-12)
+    # (b) W2 = 0, b2 = 0, no LN: z_T = z_0
+    w = gen.make_weights(cfg); w["W2"] = np.zeros_like(w["W2"]); w["b2"] = np.zeros_like(w["b2"])
+    _, lat = run_vec(cfg, w, b, return_latent=True)
+    np.testing.assert_array_equal(lat, z0)
+    # (c) same with LN, gamma=1, beta=0, eps=0: z_T = LN(z_0) for any T >= 1 (idempotent)
+    cfg2 = tiny_cfg(KIND_MLP_LN, len_lo=1)
+    w = gen.make_weights(cfg2); w["W2"] = np.zeros_like(w["W2"]); w["b2"] = np.zeros_like(w["b2"])
+    w["gamma"] = np.ones_like(w["gamma"]); w["beta"] = np.zeros_like(w["beta"])
+    b2 = gen.make_inputs(cfg2)
+    lat = oracle.rollout_score_vec(w, b2.init_states, b2.action_ids, b2.action_params, b2.lengths, b2.hw_feats,
+                                   b2.subgraph_offsets, ln_eps=0.0, return_latent=True)[1]
+    z0b = b2.init_states[seg].astype(np.float64)
+    ref = (z0b - z0b.mean(-1, keepdims=True)) / z0b.std(-1, keepdims=True)
+    np.testing.assert_allclose(lat, ref, rtol=0, atol=1e-12)
+    # (d) GRU, all weights 0: g = 1/2, h = 0 => z_T = z_0 / 2^T
+    cfg3 = tiny_cfg(KIND_GRU, EMBED_BUCKET, len_lo=1)
+    w = gen.make_weights(cfg3)
+    for nme in ("W_g", "W_r", "W_h"):
+        w[nme] = np.zeros_like(w[nme])
+    b3 = gen.make_inputs(cfg3)
+    _, lat = run_vec(cfg3, w, b3, return_latent=True)
+    z0c = b3.init_states[seg].astype(np.float64)
+    np.testing.assert_allclose(lat, z0c / (2.0 ** b3.lengths)[:, None], rtol=0, atol=1e-15)
+    # (e) GRU, W_h = 0: one step is (1-g) z
+    w = gen.make_weights(cfg3); w["W_h"] = np.zeros_like(w["W_h"])
+    z = np.array([[0.3, -1.2, 0.5, 2.0, -0.1, 0.7]]); a = np.array([[1.0, -1.0, 0.5, 0.25]])
+    g = 1 / (1 + np.exp(-(np.concatenate([z, a], -1) @ w["W_g"].astype(np.float64).T)))
+    np.testing.assert_allclose(oracle.step_gru(z, a, w["W_g"], w["W_r"], w["W_h"]), (1 - g) * z, atol=1e-15)
+
+
+# ---- P8: library cross-checks (torch float64 CPU) ---------------------------------------------------------
+
+def test_p8_library_cross_checks():
+    rng = np.random.default_rng(0)
+    x = rng.standard_normal((37, 19)) * 3
+    t = torch.from_numpy(x)
+    np.testing.assert_allclose(oracle.gelu(x), torch.nn.functional.gelu(t, approximate="none").numpy(),
+                               rtol=0, atol=1e-14)
+    gam = rng.standard_normal(19); bet = rng.standard_normal(19)
+    ref = torch.nn.functional.layer_norm(t, (19,), torch.from_numpy(gam), torch.from_numpy(bet), 1e-5).numpy()
+    np.testing.assert_allclose(oracle.layer_norm(x, gam, bet, 1e-5), ref, rtol=0, atol=1e-13)
+    # whole MLP+LN step and GRU step against torch linear algebra
+    d, da, hid = 19, 7, 23
+    z = rng.standard_normal((11, d)); a = rng.standard_normal((11, da))
+    W1 = rng.standard_normal((hid, d + da)); b1 = rng.standard_normal(hid)
+    W2 = rng.standard_normal((d, hid)); b2 = rng.standard_normal(d)
+    tz, ta = torch.from_numpy(z), torch.from_numpy(a)
+    F = torch.nn.functional
+    tv = tz + F.linear(F.gelu(F.linear(torch.cat([tz, ta], -1), torch.from_numpy(W1), torch.from_numpy(b1))),
+                       torch.from_numpy(W2), torch.from_numpy(b2))
+    np.testing.assert_allclose(oracle.step_mlp(z, a, W1, b1, W2, b2), tv.numpy(), rtol=0, atol=1e-12)
+    tln = F.layer_norm(tv, (d,), torch.from_numpy(gam), torch.from_numpy(bet), 1e-5)
+    np.testing.assert_allclose(oracle.step_mlp(z, a, W1, b1, W2, b2, gam, bet, 1e-5), tln.numpy(), atol=1e-12)
+    Wg, Wr, Wh = (rng.standard_normal((d, d + da)) for _ in range(3))
+    x_ = torch.cat([tz, ta], -1)
+    g = torch.sigmoid(F.linear(x_, torch.from_numpy(Wg))); r = torch.sigmoid(F.linear(x_, torch.from_numpy(Wr)))
+    h = torch.tanh(F.linear(torch.cat([r * tz, ta], -1), torch.from_numpy(Wh)))
+    np.testing.assert_allclose(oracle.step_gru(z, a, Wg, Wr, Wh), ((1 - g) * tz + g * h).numpy(), atol=1e-13)
+    # embedding against torch.nn.functional.embedding + linear
+    E = rng.standard_normal((5, da)); Wp = rng.standard_normal((da, 3)); bp = rng.standard_normal(da)
+    ids = rng.integers(0, 5, 11); par = rng.integers(1, 1025, (11, 3))
+    ref = F.embedding(torch.from_numpy(ids), torch.from_numpy(E)) + \
+        F.linear(torch.log2(torch.from_numpy(par).double()), torch.from_numpy(Wp), torch.from_numpy(bp))
+    np.testing.assert_allclose(oracle.embed_linear(ids, par, E, Wp, bp), ref.numpy(), atol=1e-13)
+    # bucketed embedding against an embedding_bag-style torch gather
+    Tbl = rng.standard_normal((5 * 3 * 40, da))
+    bk = torch.clamp(torch.floor(4 * torch.log2(torch.from_numpy(par).double()) + 1e-9), max=39).long()
+    idx = (torch.from_numpy(ids)[:, None] * 3 + torch.arange(3)[None]) * 40 + bk
+    ref = F.embedding(idx, torch.from_numpy(Tbl)).sum(1)
+    np.testing.assert_allclose(oracle.embed_bucket(ids, par, Tbl, 3, 40), ref.numpy(), atol=1e-13)
+
+
+# ---- P9: brute force --------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("kind,embed", ALL_KINDS)
+def test_p9_scalar_vs_vector(kind, embed):
+    cfg = tiny_cfg(kind, embed)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    yv = run_vec(cfg, w, b)
+    ys = oracle.rollout_score_scalar(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.hw_feats,
+                                     b.subgraph_offsets, n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps)
+    np.testing.assert_allclose(yv, ys, rtol=0, atol=1e-12)
+
+
+def test_p9_cfg1_scalar_vs_vector():
+    cfg = gen.get_config(1)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    yv = run_vec(cfg, w, b)
+    ys = oracle.rollout_score_scalar(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.hw_feats,
+                                     b.subgraph_offsets)
+    np.testing.assert_allclose(yv, ys, rtol=0, atol=1e-11)
+
+
+# ---- P10: top-k -------------------------------------------------------------------------------------------
+
+def test_p10_topk_matches_full_sort():
+    rng = np.random.default_rng(3)
+    sc = rng.integers(-3, 4, 50).astype(np.float32)           # many duplicates
+    sc[7] = -0.0; sc[9] = 0.0; sc[11] = np.nan; sc[40] = np.nan; sc[13] = np.inf; sc[14] = -np.inf
+    off = np.array([0, 0, 20, 23, 50], dtype=np.int32)         # empty, normal, n_s < k, normal
+    k = 5
+    out = oracle.topk_segments(sc, off, k)
+    assert out.shape == (4, 5)
+    assert (out[0] == -1).all()
+    t = torch.from_numpy(sc.astype(np.float64))
+    t = torch.where(torch.isnan(t), torch.full_like(t, -float("inf")), t)   # NaN lowest (after -inf by index)
+    for s in range(1, 4):
+        lo, hi = off[s], off[s + 1]
+        seg = t[lo:hi]
+        order = torch.sort(-seg, stable=True).indices.numpy() + lo           # stable => index asc on ties
+        # -inf vs NaN: NaN must come after real -inf
+        order = sorted(order, key=lambda i: (1 if math.isnan(sc[i]) else 0, -(t[i].item()), i))
+        exp = list(order[:k]) + [-1] * max(0, k - (hi - lo))
+        assert list(out[s]) == exp[:k]
+    assert list(oracle.topk_segments(np.array([0.0, -0.0, 0.0], np.float32), [0, 3], 3)[0]) == [0, 1, 2]
+    assert list(oracle.topk_segments(np.array([1.0, 1.0, 1.0, 1.0], np.float32), [0, 4], 2)[0]) == [0, 1]
+    # against torch.topk where scores are distinct
+    x = rng.standard_normal(200).astype(np.float32)
+    ref = torch.topk(torch.from_numpy(x), 17).indices.numpy()
+    assert list(oracle.topk_segments(x, [0, 200], 17)[0]) == list(ref)
+
+
+# ---- P12: shared-prefix reuse equals from-scratch ---------------------------------------------------------------
+
+def test_p12_prefix_reuse_equals_scratch():
+    cfg = gen.get_config(4).scaled(S=1, per_subgraph=64)
+    cfg = WMConfig(**{**cfg.__dict__, "d": 8, "d_a": 4, "hidden": 12, "H": 3, "scorer_widths": (6, 5)})
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    y = run_vec(cfg, w, b)
+    # children 0..63 share parent 0's prefix up to their cut; roll the common prefix (min cut = 16) once
+    c = 16
+    assert (b.action_ids[:, :c] == b.action_ids[0, :c]).all()
+    _, zc = oracle.rollout_score_vec(w, b.init_states, b.action_ids[:1, :c], b.action_params[:1, :c],
+                                     np.array([c]), b.hw_feats, np.array([0, 1]), return_latent=True)
+    # continue every child from the shared latent in per-candidate mode; phi needs the whole sequence, so
+    # compare terminal latents (the quantity prefix reuse shares)
+    _, lat_full = run_vec(cfg, w, b, return_latent=True)
+    _, lat_sfx = oracle.rollout_score_vec(w, np.repeat(zc, 64, 0), b.action_ids[:, c:], b.action_params[:, c:],
+                                          b.lengths - c, np.repeat(b.hw_feats, 64, 0), None, return_latent=True)
+    np.testing.assert_allclose(lat_sfx, lat_full, rtol=0, atol=1e-12)
+    assert np.isfinite(y).all()
+
+
+# ---- generator / file format ----------------------------------------------------------------------------------
+
+def test_weight_file_roundtrip(tmp_path):
+    for n in (1, 2, 5):
+        cfg = gen.get_config(n)
+        if n != 1:
+            cfg = WMConfig(**{**cfg.__dict__, "d": 16, "d_a": 8, "hidden": 0 if n == 5 else 24,
+                              "scorer_widths": (12, 10)})
+        w = gen.make_weights(cfg)
+        p = str(tmp_path / f"w{n}.bin")
+        gen.write_weight_file(p, cfg, w)
+        hdr, w2 = oracle.read_weight_file(p)
+        assert hdr["d"] == cfg.d and hdr["kind"] == cfg.kind and hdr["P"] == cfg.P
+        assert list(w2.keys()) == gen.tensor_order(cfg)
+        for kname in w:
+            np.testing.assert_array_equal(w[kname], w2[kname])
+        if n != 1:   # bf16 configs: stored values are bf16-representable
+            for v in w.values():
+                assert (v.view(np.uint32) & 0xFFFF == 0).all()
+
+
+def test_generator_recipe():
+    c2 = gen.get_config(2); b = gen.make_inputs(c2)
+    assert b.lengths.min() == 8 and b.lengths.max() == 32 and b.action_ids.shape == (32768, 32)
+    valid = np.arange(32)[None, :] < b.lengths[:, None]
+    assert b.action_ids[valid].min() == 0 and b.action_ids[valid].max() == 31
+    assert b.action_params[valid].min() == 1 and b.action_params[valid].max() <= 1024
+    assert set(np.unique(b.action_ids[~valid])) <= {-2**31, 2**31 - 1}
+    c3 = gen.get_config(3).scaled(S=8); b3 = gen.make_inputs(c3)
+    assert b3.lengths.min() >= 4 and b3.lengths.max() <= 48 and abs(b3.lengths.mean() - 17.14) < 0.6
+    c4 = gen.get_config(4).scaled(S=1, per_subgraph=128); b4 = gen.make_inputs(c4)
+    assert (b4.lengths == 32).all()
+    assert (b4.action_ids[:64, :16] == b4.action_ids[0, :16]).all()          # 64 children share >= 16 steps
+    assert (b4.action_ids[64:128, :16] == b4.action_ids[64, :16]).all()
+    assert (b4.action_ids[0, :16] != b4.action_ids[64, :16]).any()
+    b_again = gen.make_inputs(c2)
+    np.testing.assert_array_equal(b.action_params, b_again.action_params)       # seeded
