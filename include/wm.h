@@ -1,0 +1,161 @@
+/* wm.h — C ABI of the batched candidate evaluator (B200 / sm_100a).
+ *
+ * What the library computes (arxiv/paper_2606_09312, citations are PAPER.md:<line>):
+ *
+ *   z_0 = init_states[s]                       the task's initial latent program state
+ *   z_t = F(z_{t-1}, a_t),  t = 1..len         action-conditioned transition, applied
+ *                                              recurrently                               PAPER.md:68-71 Eq.1, :162 Eq.8, :166
+ *   steps t > len leave z unchanged            rollout mask m_t                          PAPER.md:176 Eq.11
+ *   phi = mean_t a_t (0 when len = 0)          action features
+ *   y   = G([z_T ; phi ; h])                   ranking score                             PAPER.md:122 Eq.3, :188 Eq.12
+ *   top-k per subgraph, (score desc, idx asc)  candidates prioritised for measurement
+ *
+ * F, G and the action embedding take the parametrisations BASELINE.json's configs bind:
+ *   embedding  a = E[id] + W_p log2(p) + b_p            (EMBED_LINEAR)
+ *              a = sum_j Tbl[(id*P + j)*n_b + bucket(p_j)], bucket(p)=min(n_b-1, floor(4 log2 p)) (EMBED_BUCKET)
+ *   F (MLP)    z' = z + W2 gelu(W1 [z;a] + b1) + b2     (KIND_MLP; KIND_MLP_LN adds LayerNorm(z'), eps in header)
+ *   F (GRU)    g = s(W_g[z;a]); r = s(W_r[z;a]); z' = (1-g) z + g tanh(W_h [r*z ; a])   (KIND_GRU)
+ *   G          MLP, hidden linears followed by exact (erf) GELU, last linear plain.
+ *
+ * Conventions
+ *   - Every array argument of wm_rollout_score / wm_topk is a DEVICE pointer owned by the caller (any
+ *     allocator; the tests use torch).  The library never frees or retains them.  wm_score_topk_host takes
+ *     HOST pointers (pinned or pageable) and does the copies itself.
+ *   - Calls enqueue work on `cuda_stream` (a cudaStream_t cast to void*; NULL = the legacy default stream) and
+ *     return without synchronising, except wm_load_weights, wm_check, wm_free and wm_score_topk_host.
+ *   - Return value: WM_OK (0) or a negative WM_ERR_* code; wm_last_error() then returns a thread-local,
+ *     NUL-terminated message.  No exceptions, no aborts.
+ *   - Data-dependent faults (len outside [0,T_max]; type id outside [0,n_types) or a parameter < 1 at a valid
+ *     position t < len) cannot be seen by the host without a sync: kernels clamp the value so every access
+ *     stays in bounds and OR a bit into a device flag word that wm_check() reads.  Padding positions
+ *     (t >= len) may hold anything and are never read.
+ *   - One ctx may be used from several streams concurrently: each call takes a private slice of the
+ *     workspace (a small pool keyed by stream).
+ */
+#ifndef WM_H_
+#define WM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WM_OK               0
+#define WM_ERR_ARG         -1   /* null pointer, negative size, k <= 0, k > WM_MAX_K, T_max > WM_MAX_T        */
+#define WM_ERR_IO          -2   /* weight file cannot be opened / read                                        */
+#define WM_ERR_FORMAT      -3   /* bad magic, version, header field or file size                              */
+#define WM_ERR_CUDA        -4   /* a CUDA runtime call failed (message carries cudaGetErrorString)            */
+#define WM_ERR_UNSUPPORTED -5   /* header describes a model no kernel in this build handles                   */
+
+#define WM_MAX_T   256          /* largest T_max accepted                                                     */
+#define WM_MAX_K   1024         /* largest k accepted by wm_topk                                              */
+
+/* bits of the device fault word returned by wm_check() */
+#define WM_FAULT_LEN    1u      /* a length was outside [0, T_max] (clamped)                                  */
+#define WM_FAULT_TYPE   2u      /* an action type id at a valid position was outside [0, n_types) (clamped)   */
+#define WM_FAULT_PARAM  4u      /* an action parameter at a valid position was < 1 (treated as 1)             */
+
+/* values of wm_info.kind / dtype / embed (the weight-file header fields) */
+#define WM_KIND_MLP     0
+#define WM_KIND_MLP_LN  1
+#define WM_KIND_GRU     2
+#define WM_DTYPE_FP32   0
+#define WM_DTYPE_BF16   1
+#define WM_EMBED_LINEAR 0
+#define WM_EMBED_BUCKET 1
+
+/* wm_set_option keys */
+#define WM_OPT_PATH      1      /* 0 = auto (default), 1 = force the fp32 CUDA-core kernel, 2 = force tcgen05  */
+#define WM_OPT_SORT      2      /* 1 = bucket candidates by length before tiling (default), 0 = input order    */
+
+typedef struct wm_ctx wm_ctx;   /* opaque: device weights (all layouts the kernels need) + workspace pool      */
+
+typedef struct wm_info {        /* model hyper-parameters, as read from the weight-file header                 */
+    int32_t kind, dtype, embed;
+    int32_t d, d_a, hidden, n_types, P, n_buckets, H;
+    int32_t n_scorer_layers;    /* number of linears of G                                                      */
+    int32_t scorer_widths[6];   /* hidden widths of G (n_scorer_layers-1 used)                                 */
+    float   ln_eps;
+    int32_t path;               /* kernel the auto policy picks for this model: 1 = fp32 CUDA-core, 2 = tcgen05 */
+} wm_info;
+
+/* Read a WMW1 weight file (format below), convert to the kernels' layouts and copy to `device`.
+ *   path     host path, NUL-terminated.
+ *   device   CUDA device ordinal.
+ *   ctx_out  receives the context (caller frees with wm_free).
+ * File format (little-endian): "WMW1", then uint32 version(=1), kind, dtype, embed, d, d_a, hidden, n_types, P,
+ * n_buckets, H, n_scorer_layers, uint32 scorer_widths[6], float ln_eps (80 bytes in all), then fp32 tensors,
+ * row-major, in this order:
+ *   EMBED_LINEAR: E[n_types,d_a], W_p[d_a,P], b_p[d_a]        EMBED_BUCKET: Tbl[n_types*P*n_buckets, d_a]
+ *   MLP / MLP_LN: W1[hidden,d+d_a], b1[hidden], W2[d,hidden], b2[d] (, gamma[d], beta[d])
+ *   GRU:          W_g[d,d+d_a], W_r[d,d+d_a], W_h[d,d+d_a]
+ *   G:            for each linear i: Ws_i[out_i,in_i], bs_i[out_i];  in_0 = d+d_a+H, out_last = 1
+ * With dtype = bf16 every stored value is already bf16-representable (BASELINE.json cfg 2-5: "bf16 weights with
+ * fp32 accumulate"); the tcgen05 path then runs bf16 x bf16 -> fp32 MMAs with an fp32 latent.
+ * Errors: WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_UNSUPPORTED, WM_ERR_CUDA.  Synchronous. */
+int wm_load_weights(const char* path, int device, wm_ctx** ctx_out);
+
+/* Free a context (device weights, workspace).  Synchronises the device.  NULL is a no-op. */
+void wm_free(wm_ctx* ctx);
+
+/* Copy the model description out of a context. */
+int wm_get_info(const wm_ctx* ctx, wm_info* info_out);
+
+/* Set a WM_OPT_* option; returns WM_ERR_ARG for an unknown key or value, WM_ERR_UNSUPPORTED when the forced
+ * path cannot run this model. */
+int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value);
+
+/* Roll every candidate's action sequence through F from its subgraph's initial latent, then score it with G
+ * (Eq.1/8/12).  Steps a0-a6 of DESIGN.md §1.
+ *   init_states       [S, d]  fp32 row-major, one z_0 per subgraph        ([B, d] when subgraph_offsets == NULL)
+ *   action_ids        [B, T_max] int32, entries at t >= lengths[b] ignored
+ *   action_params     [B, T_max, P] int32, >= 1 at valid positions
+ *   lengths           [B] int32, 0 <= len <= T_max
+ *   hw_feats          [S, H]  fp32, one h per subgraph                    ([B, H] when subgraph_offsets == NULL)
+ *   scores_out        [B] fp32, written in the original candidate order
+ *   subgraph_offsets  [S+1] int32 CSR, offsets[0] = 0, offsets[S] = B, non-decreasing (empty segments allowed);
+ *                     NULL selects per-candidate mode and S is ignored
+ *   B, S, T_max       sizes; B = 0 is a no-op.  P, d, H come from the weight file.
+ *   cuda_stream       stream to enqueue on
+ * Errors: WM_ERR_ARG (null pointer with B > 0, B < 0, S < 0, T_max < 0 or > WM_MAX_T), WM_ERR_CUDA. */
+int wm_rollout_score(wm_ctx* ctx,
+                     const float* init_states, const int32_t* action_ids, const int32_t* action_params,
+                     const int32_t* lengths, const float* hw_feats, float* scores_out,
+                     const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream);
+
+/* Per subgraph segment [offsets[s], offsets[s+1]) select the k largest scores, ordered by
+ * (score descending, index ascending).  -0.0 == +0.0; NaN ranks below every number (ties by index).
+ *   scores            [offsets[S]] fp32
+ *   subgraph_offsets  [S+1] int32 CSR (device)
+ *   idx_out           [S, k] int32: GLOBAL candidate indices; rows of segments with fewer than k candidates
+ *                     are padded with -1
+ * Needs no context.  Errors: WM_ERR_ARG (null pointer with S > 0, S < 0, k <= 0, k > WM_MAX_K), WM_ERR_CUDA. */
+int wm_topk(const float* scores, const int32_t* subgraph_offsets, int32_t S, int32_t k, int32_t* idx_out,
+            void* cuda_stream);
+
+/* Synchronise `cuda_stream` and return the OR of the WM_FAULT_* bits raised since the last wm_check on this
+ * ctx (>= 0), or a negative error code.  Resets the word. */
+int wm_check(wm_ctx* ctx, void* cuda_stream);
+
+/* End-to-end convenience entry: same computation as wm_rollout_score followed by wm_topk, with HOST buffers.
+ * Copies the inputs host->device into ctx-owned staging, runs both steps on `cuda_stream`, copies scores
+ * ([B] fp32, may be NULL to skip) and idx ([S,k] int32) back, and synchronises the stream before returning.
+ * subgraph_offsets must be non-NULL (top-k needs segments).  Used by bench.py's e2e leg. */
+int wm_score_topk_host(wm_ctx* ctx,
+                       const float* init_states, const int32_t* action_ids, const int32_t* action_params,
+                       const int32_t* lengths, const float* hw_feats, const int32_t* subgraph_offsets,
+                       int64_t B, int32_t S, int32_t T_max, int32_t k,
+                       float* scores_out, int32_t* idx_out, void* cuda_stream);
+
+/* Number of kernels the library launched on behalf of this ctx since it was created (bench.py's
+ * gpu_launches); wm_topk's launches are counted in a process-wide counter returned when ctx == NULL. */
+int64_t wm_launch_count(const wm_ctx* ctx);
+
+/* Message for the last nonzero status returned on this thread ("" if none). */
+const char* wm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WM_H_ */

@@ -1,0 +1,155 @@
+"""paper_2606_09312_b200 — thin Python binding of the C-ABI library (include/wm.h).
+
+Argument marshalling only: every step of the hot path runs in the library's CUDA kernels.  The functions
+keep the ABI's names (`wm_load_weights`, `wm_rollout_score`, `wm_topk`, ...).  PyTorch is used for device
+memory and streams.  There is no CPU fallback: if libwm.so is missing or does not load, importing the
+binding's functions raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libwm.so")
+
+WM_OK, WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_CUDA, WM_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
+WM_MAX_T, WM_MAX_K = 256, 1024
+WM_FAULT_LEN, WM_FAULT_TYPE, WM_FAULT_PARAM = 1, 2, 4
+WM_OPT_PATH, WM_OPT_SORT = 1, 2
+PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
+
+# every symbol include/wm.h declares
+ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
+               "wm_check", "wm_score_topk_host", "wm_launch_count", "wm_last_error")
+
+
+class WmInfo(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("dtype", ctypes.c_int32), ("embed", ctypes.c_int32),
+                ("d", ctypes.c_int32), ("d_a", ctypes.c_int32), ("hidden", ctypes.c_int32),
+                ("n_types", ctypes.c_int32), ("P", ctypes.c_int32), ("n_buckets", ctypes.c_int32),
+                ("H", ctypes.c_int32), ("n_scorer_layers", ctypes.c_int32),
+                ("scorer_widths", ctypes.c_int32 * 6), ("ln_eps", ctypes.c_float), ("path", ctypes.c_int32)]
+
+
+class WmError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"wm error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libwm.so (built by paper_2606_09312_b200.build).  Fails loudly when it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2606_09312_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    L.wm_load_weights.argtypes = [ctypes.c_char_p, ctypes.c_int, ctypes.POINTER(vp)]
+    L.wm_load_weights.restype = ctypes.c_int
+    L.wm_free.argtypes = [vp]
+    L.wm_free.restype = None
+    L.wm_get_info.argtypes = [vp, ctypes.POINTER(WmInfo)]
+    L.wm_get_info.restype = ctypes.c_int
+    L.wm_set_option.argtypes = [vp, i32, i32]
+    L.wm_set_option.restype = ctypes.c_int
+    L.wm_rollout_score.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, vp]
+    L.wm_rollout_score.restype = ctypes.c_int
+    L.wm_topk.argtypes = [vp, vp, i32, i32, vp, vp]
+    L.wm_topk.restype = ctypes.c_int
+    L.wm_check.argtypes = [vp, vp]
+    L.wm_check.restype = ctypes.c_int
+    L.wm_score_topk_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp, vp, vp]
+    L.wm_score_topk_host.restype = ctypes.c_int
+    L.wm_launch_count.argtypes = [vp]
+    L.wm_launch_count.restype = i64
+    L.wm_last_error.argtypes = []
+    L.wm_last_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int) -> int:
+    if rc < 0:
+        raise WmError(rc, lib().wm_last_error().decode("utf-8", "replace"))
+    return rc
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream=None) -> Optional[int]:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream or None
+
+
+def wm_last_error() -> str:
+    return lib().wm_last_error().decode("utf-8", "replace")
+
+
+def wm_load_weights(path: str, device: int = 0) -> int:
+    """-> ctx handle (int).  include/wm.h: wm_load_weights."""
+    ctx = ctypes.c_void_p()
+    _check(lib().wm_load_weights(os.fsencode(path), int(device), ctypes.byref(ctx)))
+    return ctx.value
+
+
+def wm_free(ctx: int) -> None:
+    lib().wm_free(ctx)
+
+
+def wm_get_info(ctx: int) -> WmInfo:
+    info = WmInfo()
+    _check(lib().wm_get_info(ctx, ctypes.byref(info)))
+    return info
+
+
+def wm_set_option(ctx: int, key: int, value: int) -> None:
+    _check(lib().wm_set_option(ctx, key, value))
+
+
+def wm_rollout_score(ctx: int, init_states, action_ids, action_params, lengths, hw_feats, scores_out,
+                     subgraph_offsets=None, stream=None) -> None:
+    """Device tensors in, scores_out ([B] fp32, device) written asynchronously on the stream.
+    Sizes are read from the tensors: B = lengths.numel(), T_max = action_ids.shape[1],
+    S = subgraph_offsets.numel() - 1 (0 in per-candidate mode)."""
+    B = int(lengths.numel())
+    T_max = int(action_ids.shape[1]) if action_ids is not None and action_ids.dim() == 2 else 0
+    S = int(subgraph_offsets.numel()) - 1 if subgraph_offsets is not None else 0
+    _check(lib().wm_rollout_score(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
+                                  _ptr(hw_feats), _ptr(scores_out), _ptr(subgraph_offsets), B, S, T_max,
+                                  _stream(stream)))
+
+
+def wm_topk(scores, subgraph_offsets, k: int, idx_out, stream=None) -> None:
+    """idx_out [S, k] int32 (device) written asynchronously on the stream."""
+    S = int(subgraph_offsets.numel()) - 1
+    _check(lib().wm_topk(_ptr(scores), _ptr(subgraph_offsets), S, int(k), _ptr(idx_out), _stream(stream)))
+
+
+def wm_check(ctx: int, stream=None) -> int:
+    return _check(lib().wm_check(ctx, _stream(stream)))
+
+
+def wm_score_topk_host(ctx: int, init_states, action_ids, action_params, lengths, hw_feats, subgraph_offsets,
+                       k: int, scores_out, idx_out, stream=None) -> None:
+    """HOST tensors (CPU, contiguous; pinned for speed) in and out; synchronous.  include/wm.h."""
+    B = int(lengths.numel())
+    T_max = int(action_ids.shape[1]) if action_ids.dim() == 2 else 0
+    S = int(subgraph_offsets.numel()) - 1
+    _check(lib().wm_score_topk_host(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
+                                    _ptr(hw_feats), _ptr(subgraph_offsets), B, S, T_max, int(k),
+                                    _ptr(scores_out), _ptr(idx_out), _stream(stream)))
+
+
+def wm_launch_count(ctx: Optional[int]) -> int:
+    return int(lib().wm_launch_count(ctx))

@@ -1,0 +1,451 @@
+// The C ABI (include/wm.h): weight loading, context/workspace management, argument validation and dispatch.
+// No arithmetic of the method lives here; see wm_bucket.cu (a0), wm_generic.cu / wm_tc.cu (a1-a6), wm_topk.cu (a7).
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "wm_internal.h"
+
+namespace wm {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int64_t topk_launches();
+
+namespace {
+
+struct Header {
+    uint32_t version, kind, dtype, embed, d, d_a, hidden, n_types, P, n_buckets, H, n_lin;
+    uint32_t widths[6];
+    float ln_eps;
+};
+static_assert(sizeof(Header) == 76, "WMW1 header is 4 + 76 bytes");
+
+struct HostTensor {
+    std::string name;
+    int rows = 0, cols = 0;   // vectors: rows = n, cols = 1
+    std::vector<float> v;
+};
+
+int upload(wm_ctx* ctx, const std::vector<float>& h, float** out) {
+    void* p = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&p, h.size() * sizeof(float) + 16));
+    ctx->allocs.push_back(p);
+    WM_CUDA_TRY(cudaMemcpy(p, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
+    *out = static_cast<float*>(p);
+    return WM_OK;
+}
+
+std::vector<float> transposed(const HostTensor& t) {
+    std::vector<float> o(t.v.size());
+    for (int r = 0; r < t.rows; ++r)
+        for (int c = 0; c < t.cols; ++c) o[(size_t)c * t.rows + r] = t.v[(size_t)r * t.cols + c];
+    return o;
+}
+
+Workspace* acquire_ws(wm_ctx* ctx, cudaStream_t st) {
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    for (Workspace* w : ctx->pool)
+        if (w->stream == st) return w;
+    Workspace* w = new Workspace();
+    w->stream = st;
+    if (cudaMalloc(&w->counters, sizeof(int32_t) * kCounterInts) != cudaSuccess) {
+        delete w;
+        return nullptr;
+    }
+    ctx->pool.push_back(w);
+    return w;
+}
+
+int ensure_perm(Workspace* ws, int64_t B, cudaStream_t st) {
+    if (ws->perm_cap >= B) return WM_OK;
+    // growing frees the old buffer: work already queued on this stream may still read it
+    if (ws->perm) {
+        WM_CUDA_TRY(cudaStreamSynchronize(st));
+        WM_CUDA_TRY(cudaFree(ws->perm));
+        ws->perm = nullptr;
+        ws->perm_cap = 0;
+    }
+    const int64_t cap = B + B / 4 + 1024;
+    WM_CUDA_TRY(cudaMalloc(&ws->perm, sizeof(int32_t) * cap));
+    ws->perm_cap = cap;
+    return WM_OK;
+}
+
+int pick_path(const wm_ctx* ctx) {
+    if (ctx->opt_path == 1) return 1;
+    if (ctx->opt_path == 2) return 2;
+    return tc_supported(ctx) ? 2 : 1;
+}
+
+}  // namespace
+}  // namespace wm
+
+using namespace wm;
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+const char* wm_last_error(void) { return g_err; }
+
+int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
+    if (!path || !ctx_out) {
+        set_error("wm_load_weights: null argument");
+        return WM_ERR_ARG;
+    }
+    *ctx_out = nullptr;
+    FILE* f = fopen(path, "rb");
+    if (!f) {
+        set_error("wm_load_weights: cannot open '%s'", path);
+        return WM_ERR_IO;
+    }
+    char magic[4];
+    Header h;
+    if (fread(magic, 1, 4, f) != 4 || fread(&h, sizeof(h), 1, f) != 1) {
+        fclose(f);
+        set_error("wm_load_weights: file shorter than the header");
+        return WM_ERR_FORMAT;
+    }
+    if (memcmp(magic, "WMW1", 4) != 0 || h.version != 1) {
+        fclose(f);
+        set_error("wm_load_weights: bad magic or version");
+        return WM_ERR_FORMAT;
+    }
+    const bool mlp = h.kind == WM_KIND_MLP || h.kind == WM_KIND_MLP_LN;
+    if (h.kind > 2 || h.dtype > 1 || h.embed > 1 || h.d == 0 || h.d_a == 0 || h.n_types == 0 || h.P == 0 ||
+        h.d > 65536 || h.d_a > 65536 || h.hidden > 65536 || h.P > 64 || h.H > 65536 || h.n_types > (1u << 20) ||
+        h.n_lin < 1 || h.n_lin > 7 || (mlp && h.hidden == 0) || (h.embed == WM_EMBED_BUCKET && h.n_buckets == 0) ||
+        h.n_buckets > 4096 || !(h.ln_eps >= 0.0f)) {
+        fclose(f);
+        set_error("wm_load_weights: header field out of range");
+        return WM_ERR_FORMAT;
+    }
+    for (uint32_t i = 0; i + 1 < h.n_lin; ++i)
+        if (h.widths[i] == 0 || h.widths[i] > 65536) {
+            fclose(f);
+            set_error("wm_load_weights: scorer width out of range");
+            return WM_ERR_FORMAT;
+        }
+
+    // tensor list in file order
+    std::vector<HostTensor> ts;
+    auto add = [&](const char* name, int rows, int cols) {
+        HostTensor t;
+        t.name = name;
+        t.rows = rows;
+        t.cols = cols;
+        ts.push_back(t);
+    };
+    const int d = h.d, da = h.d_a, hid = h.hidden;
+    if (h.embed == WM_EMBED_LINEAR) {
+        add("E", h.n_types, da); add("W_p", da, h.P); add("b_p", da, 1);
+    } else {
+        add("Tbl", h.n_types * h.P * h.n_buckets, da);
+    }
+    if (mlp) {
+        add("W1", hid, d + da); add("b1", hid, 1); add("W2", d, hid); add("b2", d, 1);
+        if (h.kind == WM_KIND_MLP_LN) { add("gamma", d, 1); add("beta", d, 1); }
+    } else {
+        add("W_g", d, d + da); add("W_r", d, d + da); add("W_h", d, d + da);
+    }
+    int sdim[kMaxScorerLinears + 1] = {};
+    sdim[0] = d + da + h.H;
+    for (uint32_t i = 0; i + 1 < h.n_lin; ++i) sdim[i + 1] = h.widths[i];
+    sdim[h.n_lin] = 1;
+    for (uint32_t i = 0; i < h.n_lin; ++i) {
+        char nm[16];
+        snprintf(nm, sizeof(nm), "Ws%u", i); add(nm, sdim[i + 1], sdim[i]);
+        snprintf(nm, sizeof(nm), "bs%u", i); add(nm, sdim[i + 1], 1);
+    }
+    for (HostTensor& t : ts) {
+        t.v.resize((size_t)t.rows * t.cols);
+        if (fread(t.v.data(), sizeof(float), t.v.size(), f) != t.v.size()) {
+            fclose(f);
+            set_error("wm_load_weights: file truncated in tensor %s", t.name.c_str());
+            return WM_ERR_FORMAT;
+        }
+    }
+    char extra;
+    const bool trailing = fread(&extra, 1, 1, f) == 1;
+    fclose(f);
+    if (trailing) {
+        set_error("wm_load_weights: trailing bytes after the last tensor");
+        return WM_ERR_FORMAT;
+    }
+
+    WM_CUDA_TRY(cudaSetDevice(device));
+    wm_ctx* ctx = new wm_ctx();
+    ctx->device = device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+        delete ctx;
+        set_error("wm_load_weights: cudaGetDeviceProperties failed");
+        return WM_ERR_CUDA;
+    }
+    ctx->n_sms = prop.multiProcessorCount;
+    ctx->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    Model& m = ctx->m;
+    m.kind = h.kind; m.dtype = h.dtype; m.embed = h.embed; m.d = d; m.d_a = da; m.hidden = hid;
+    m.n_types = h.n_types; m.P = h.P; m.n_buckets = h.n_buckets; m.H = h.H; m.n_lin = h.n_lin;
+    for (int i = 0; i <= kMaxScorerLinears; ++i) m.sdim[i] = sdim[i];
+    m.ln_eps = h.ln_eps;
+
+    int rc = WM_OK;
+    auto find = [&](const std::string& n) -> const HostTensor* {
+        for (const HostTensor& t : ts)
+            if (t.name == n) return &t;
+        return nullptr;
+    };
+    auto up = [&](const char* n, float** dst, bool transpose) {
+        const HostTensor* t = find(n);
+        if (!t || rc != WM_OK) return;
+        rc = transpose ? upload(ctx, transposed(*t), dst) : upload(ctx, t->v, dst);
+    };
+    up("E", &m.E, false); up("W_p", &m.WpT, true); up("b_p", &m.bp, false); up("Tbl", &m.Tbl, false);
+    up("W1", &m.W1t, true); up("b1", &m.b1, false); up("W2", &m.W2t, true); up("b2", &m.b2, false);
+    up("gamma", &m.gamma, false); up("beta", &m.beta, false);
+    up("W_g", &m.Wgt, true); up("W_r", &m.Wrt, true); up("W_h", &m.Wht, true);
+    for (int i = 0; i < m.n_lin; ++i) {
+        char nm[16];
+        snprintf(nm, sizeof(nm), "Ws%d", i); up(nm, &m.Wst[i], true);
+        snprintf(nm, sizeof(nm), "bs%d", i); up(nm, &m.bs[i], false);
+    }
+    if (rc == WM_OK) {
+        void* p = nullptr;
+        if (cudaMalloc(&p, 16) != cudaSuccess || cudaMemset(p, 0, 16) != cudaSuccess) {
+            set_error("wm_load_weights: cannot allocate the fault word");
+            rc = WM_ERR_CUDA;
+        } else {
+            ctx->allocs.push_back(p);
+            ctx->fault = static_cast<uint32_t*>(p);
+        }
+    }
+    if (rc == WM_OK) {
+        std::vector<std::vector<float>> hv;
+        std::vector<std::string> names;
+        for (HostTensor& t : ts) {
+            names.push_back(t.name);
+            hv.push_back(std::move(t.v));
+        }
+        rc = tc_prepare(ctx, hv, names);
+    }
+    if (rc == WM_OK && !generic_supported(ctx) && !tc_supported(ctx)) {
+        set_error("wm_load_weights: no kernel in this build handles this model (too wide for shared memory)");
+        rc = WM_ERR_UNSUPPORTED;
+    }
+    if (rc != WM_OK) {
+        wm_free(ctx);
+        return rc;
+    }
+    *ctx_out = ctx;
+    return WM_OK;
+}
+
+void wm_free(wm_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    for (Workspace* w : ctx->pool) {
+        if (w->perm) cudaFree(w->perm);
+        if (w->counters) cudaFree(w->counters);
+        if (w->stage) cudaFree(w->stage);
+        delete w;
+    }
+    for (void* p : ctx->allocs) cudaFree(p);
+    delete ctx;
+}
+
+int wm_get_info(const wm_ctx* ctx, wm_info* o) {
+    if (!ctx || !o) {
+        set_error("wm_get_info: null argument");
+        return WM_ERR_ARG;
+    }
+    const Model& m = ctx->m;
+    o->kind = m.kind; o->dtype = m.dtype; o->embed = m.embed; o->d = m.d; o->d_a = m.d_a; o->hidden = m.hidden;
+    o->n_types = m.n_types; o->P = m.P; o->n_buckets = m.n_buckets; o->H = m.H; o->n_scorer_layers = m.n_lin;
+    for (int i = 0; i < 6; ++i) o->scorer_widths[i] = (i + 1 < m.n_lin) ? m.sdim[i + 1] : 0;
+    o->ln_eps = m.ln_eps;
+    o->path = tc_supported(ctx) ? 2 : 1;
+    return WM_OK;
+}
+
+int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value) {
+    if (!ctx) {
+        set_error("wm_set_option: null ctx");
+        return WM_ERR_ARG;
+    }
+    if (key == WM_OPT_PATH) {
+        if (value < 0 || value > 2) {
+            set_error("wm_set_option: WM_OPT_PATH takes 0, 1 or 2");
+            return WM_ERR_ARG;
+        }
+        if (value == 2 && !tc_supported(ctx)) {
+            set_error("wm_set_option: the tcgen05 path does not handle this model");
+            return WM_ERR_UNSUPPORTED;
+        }
+        if (value == 1 && !generic_supported(ctx)) {
+            set_error("wm_set_option: the fp32 path does not handle this model");
+            return WM_ERR_UNSUPPORTED;
+        }
+        ctx->opt_path = value;
+        return WM_OK;
+    }
+    if (key == WM_OPT_SORT) {
+        if (value < 0 || value > 1) {
+            set_error("wm_set_option: WM_OPT_SORT takes 0 or 1");
+            return WM_ERR_ARG;
+        }
+        ctx->opt_sort = value;
+        return WM_OK;
+    }
+    set_error("wm_set_option: unknown key %d", key);
+    return WM_ERR_ARG;
+}
+
+int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* action_ids, const int32_t* action_params,
+                     const int32_t* lengths, const float* hw_feats, float* scores_out,
+                     const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream) {
+    if (!ctx) {
+        set_error("wm_rollout_score: null ctx");
+        return WM_ERR_ARG;
+    }
+    if (B < 0 || B > 0x7fffffffLL || S < 0 || T_max < 0 || T_max > WM_MAX_T) {
+        set_error("wm_rollout_score: size out of range (B=%lld S=%d T_max=%d)", (long long)B, S, T_max);
+        return WM_ERR_ARG;
+    }
+    if (B == 0) return WM_OK;
+    if (!init_states || !lengths || !scores_out || (ctx->m.H > 0 && !hw_feats) ||
+        (T_max > 0 && (!action_ids || !action_params)) || (subgraph_offsets && S < 1)) {
+        set_error("wm_rollout_score: null pointer (or S < 1 with offsets) for a non-empty batch");
+        return WM_ERR_ARG;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    WM_CUDA_TRY(cudaSetDevice(ctx->device));
+    Workspace* ws = acquire_ws(ctx, st);
+    if (!ws) {
+        set_error("wm_rollout_score: cannot allocate workspace");
+        return WM_ERR_CUDA;
+    }
+    CallArgs a;
+    a.init_states = init_states; a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
+    a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets; a.perm = nullptr;
+    a.B = B; a.S = S; a.T_max = T_max; a.fault = ctx->fault;
+    if (ctx->opt_sort) {
+        int rc = ensure_perm(ws, B, st);
+        if (rc != WM_OK) return rc;
+        rc = launch_length_bucketing(ctx, ws, lengths, B, T_max, st);
+        if (rc != WM_OK) return rc;
+        a.perm = ws->perm;
+    }
+    if (pick_path(ctx) == 2) return launch_tc(ctx, ws, a, st);
+    return launch_generic(ctx, a, st);
+}
+
+int wm_topk(const float* scores, const int32_t* subgraph_offsets, int32_t S, int32_t k, int32_t* idx_out,
+            void* cuda_stream) {
+    if (S < 0 || k <= 0 || k > WM_MAX_K) {
+        set_error("wm_topk: size out of range (S=%d k=%d)", S, k);
+        return WM_ERR_ARG;
+    }
+    if (S == 0) return WM_OK;
+    if (!scores || !subgraph_offsets || !idx_out) {
+        set_error("wm_topk: null pointer");
+        return WM_ERR_ARG;
+    }
+    return launch_topk(scores, subgraph_offsets, S, k, idx_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int wm_check(wm_ctx* ctx, void* cuda_stream) {
+    if (!ctx) {
+        set_error("wm_check: null ctx");
+        return WM_ERR_ARG;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    WM_CUDA_TRY(cudaSetDevice(ctx->device));
+    uint32_t word = 0;
+    WM_CUDA_TRY(cudaMemcpyAsync(&word, ctx->fault, sizeof(word), cudaMemcpyDeviceToHost, st));
+    WM_CUDA_TRY(cudaMemsetAsync(ctx->fault, 0, sizeof(word), st));
+    WM_CUDA_TRY(cudaStreamSynchronize(st));
+    return (int)(word & 0x7fffffffu);
+}
+
+int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* action_ids,
+                       const int32_t* action_params, const int32_t* lengths, const float* hw_feats,
+                       const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
+                       float* scores_out, int32_t* idx_out, void* cuda_stream) {
+    if (!ctx) {
+        set_error("wm_score_topk_host: null ctx");
+        return WM_ERR_ARG;
+    }
+    if (B < 0 || B > 0x7fffffffLL || S < 1 || T_max < 0 || T_max > WM_MAX_T || k <= 0 || k > WM_MAX_K ||
+        !subgraph_offsets || !idx_out || !init_states || !lengths || (ctx->m.H > 0 && !hw_feats) ||
+        (B > 0 && T_max > 0 && (!action_ids || !action_params))) {
+        set_error("wm_score_topk_host: bad argument");
+        return WM_ERR_ARG;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    WM_CUDA_TRY(cudaSetDevice(ctx->device));
+    Workspace* ws = acquire_ws(ctx, st);
+    if (!ws) {
+        set_error("wm_score_topk_host: cannot allocate workspace");
+        return WM_ERR_CUDA;
+    }
+    const Model& m = ctx->m;
+    auto up16 = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    const size_t b_z0 = up16((size_t)S * m.d * 4), b_hw = up16((size_t)S * m.H * 4);
+    const size_t b_ids = up16((size_t)B * T_max * 4), b_par = up16((size_t)B * T_max * m.P * 4);
+    const size_t b_len = up16((size_t)B * 4), b_off = up16((size_t)(S + 1) * 4);
+    const size_t b_sc = up16((size_t)B * 4), b_idx = up16((size_t)S * k * 4);
+    const size_t need = b_z0 + b_hw + b_ids + b_par + b_len + b_off + b_sc + b_idx;
+    if (ws->stage_cap < need) {
+        if (ws->stage) {
+            WM_CUDA_TRY(cudaStreamSynchronize(st));
+            WM_CUDA_TRY(cudaFree(ws->stage));
+            ws->stage = nullptr;
+            ws->stage_cap = 0;
+        }
+        WM_CUDA_TRY(cudaMalloc(&ws->stage, need));
+        ws->stage_cap = need;
+    }
+    char* p = static_cast<char*>(ws->stage);
+    float* dz0 = (float*)p; p += b_z0;
+    float* dhw = (float*)p; p += b_hw;
+    int32_t* dids = (int32_t*)p; p += b_ids;
+    int32_t* dpar = (int32_t*)p; p += b_par;
+    int32_t* dlen = (int32_t*)p; p += b_len;
+    int32_t* doff = (int32_t*)p; p += b_off;
+    float* dsc = (float*)p; p += b_sc;
+    int32_t* didx = (int32_t*)p;
+    const auto H2D = cudaMemcpyHostToDevice;
+    WM_CUDA_TRY(cudaMemcpyAsync(dz0, init_states, (size_t)S * m.d * 4, H2D, st));
+    if (m.H) WM_CUDA_TRY(cudaMemcpyAsync(dhw, hw_feats, (size_t)S * m.H * 4, H2D, st));
+    if (B && T_max) {
+        WM_CUDA_TRY(cudaMemcpyAsync(dids, action_ids, (size_t)B * T_max * 4, H2D, st));
+        WM_CUDA_TRY(cudaMemcpyAsync(dpar, action_params, (size_t)B * T_max * m.P * 4, H2D, st));
+    }
+    if (B) WM_CUDA_TRY(cudaMemcpyAsync(dlen, lengths, (size_t)B * 4, H2D, st));
+    WM_CUDA_TRY(cudaMemcpyAsync(doff, subgraph_offsets, (size_t)(S + 1) * 4, H2D, st));
+    int rc = wm_rollout_score(ctx, dz0, dids, dpar, dlen, dhw, dsc, doff, B, S, T_max, cuda_stream);
+    if (rc != WM_OK) return rc;
+    rc = wm_topk(dsc, doff, S, k, didx, cuda_stream);
+    if (rc != WM_OK) return rc;
+    if (scores_out && B) WM_CUDA_TRY(cudaMemcpyAsync(scores_out, dsc, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    WM_CUDA_TRY(cudaMemcpyAsync(idx_out, didx, (size_t)S * k * 4, cudaMemcpyDeviceToHost, st));
+    WM_CUDA_TRY(cudaStreamSynchronize(st));
+    return WM_OK;
+}
+
+int64_t wm_launch_count(const wm_ctx* ctx) {
+    if (!ctx) return topk_launches();
+    return ctx->launches.load();
+}
+
+}  // extern "C"
+#pragma GCC visibility pop

@@ -1,0 +1,387 @@
+// K2-fp32: the whole hot path (a1-a6 of DESIGN.md §1) on fp32 CUDA cores, for every model kind.
+//
+// It is the kernel of record for cfg 1 (fp32, 1e-4 tolerance: TF32/bf16 tensor cores cannot meet it) and the
+// fallback for the bf16 models the tcgen05 kernel (wm_tc.cu) does not cover yet.  One CTA owns a tile of R
+// candidates; all activations of the tile live in shared memory TRANSPOSED ([feature][row], rows contiguous)
+// so that (a) a thread that owns one output unit reads the R inputs of a feature as float4 broadcasts and
+// (b) element-wise phases map lanes to rows and never bank-conflict.  Weights are read through the read-only
+// path from their [in][out] (transposed at load time) layout: consecutive threads -> consecutive addresses.
+//
+// PAPER.md:162 Eq.8 / :166 (recurrent rollout), :176 (mask), :186-188 Eq.12 (features + score).
+#include <math_constants.h>
+
+#include "wm_internal.h"
+
+namespace wm {
+
+struct GenericParams {
+    int kind, embed, d, da, hidden, n_types, P, n_buckets, H, n_lin;
+    int sdim[kMaxScorerLinears + 1];
+    int maxw;        // rows of buffer Hb
+    int alt_rows;    // rows of the region that holds V, AS, Y (and the scorer's second ping-pong buffer)
+    float ln_eps;
+    const float *E, *WpT, *bp, *Tbl;
+    const float *W1t, *b1, *W2t, *b2, *gamma, *beta;
+    const float *Wgt, *Wrt, *Wht;
+    const float* Wst[kMaxScorerLinears];
+    const float* bs[kMaxScorerLinears];
+    CallArgs a;
+    int n_tiles;
+};
+
+enum { ACT_NONE = 0, ACT_GELU = 1, ACT_SIGMOID = 2, ACT_TANH = 3 };
+
+__device__ __forceinline__ float gelu_erf(float x) { return 0.5f * x * (1.0f + erff(x * 0.70710678118654752440f)); }
+__device__ __forceinline__ float sigmoidf_(float x) { return 1.0f / (1.0f + expf(-x)); }
+
+template <int ACT>
+__device__ __forceinline__ float apply_act(float x) {
+    if (ACT == ACT_GELU) return gelu_erf(x);
+    if (ACT == ACT_SIGMOID) return sigmoidf_(x);
+    if (ACT == ACT_TANH) return tanhf(x);
+    return x;
+}
+
+// outT[n][r] = act(bias[n] + sum_k Wt[k][n] * inT[k][r]),  n < N, r < R.  inT/outT in shared memory.
+template <int R, int ACT>
+__device__ void linear_T(const float* __restrict__ Wt, const float* __restrict__ bias, const float* inT, int K,
+                         int N, float* outT) {
+    for (int n = threadIdx.x; n < N; n += blockDim.x) {
+        float acc[R];
+        const float b = bias ? __ldg(bias + n) : 0.0f;
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = b;
+        const float* wp = Wt + n;
+        int k = 0;
+        for (; k + 4 <= K; k += 4) {
+            float w[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) w[u] = __ldg(wp + (size_t)(k + u) * N);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float4* xv = reinterpret_cast<const float4*>(inT + (size_t)(k + u) * R);
+#pragma unroll
+                for (int q = 0; q < R / 4; ++q) {
+                    float4 x = xv[q];
+                    acc[4 * q + 0] = fmaf(w[u], x.x, acc[4 * q + 0]);
+                    acc[4 * q + 1] = fmaf(w[u], x.y, acc[4 * q + 1]);
+                    acc[4 * q + 2] = fmaf(w[u], x.z, acc[4 * q + 2]);
+                    acc[4 * q + 3] = fmaf(w[u], x.w, acc[4 * q + 3]);
+                }
+            }
+        }
+        for (; k < K; ++k) {
+            const float w = __ldg(wp + (size_t)k * N);
+            const float4* xv = reinterpret_cast<const float4*>(inT + (size_t)k * R);
+#pragma unroll
+            for (int q = 0; q < R / 4; ++q) {
+                float4 x = xv[q];
+                acc[4 * q + 0] = fmaf(w, x.x, acc[4 * q + 0]);
+                acc[4 * q + 1] = fmaf(w, x.y, acc[4 * q + 1]);
+                acc[4 * q + 2] = fmaf(w, x.z, acc[4 * q + 2]);
+                acc[4 * q + 3] = fmaf(w, x.w, acc[4 * q + 3]);
+            }
+        }
+        float4* ov = reinterpret_cast<float4*>(outT + (size_t)n * R);
+#pragma unroll
+        for (int q = 0; q < R / 4; ++q) {
+            float4 o;
+            o.x = apply_act<ACT>(acc[4 * q + 0]);
+            o.y = apply_act<ACT>(acc[4 * q + 1]);
+            o.z = apply_act<ACT>(acc[4 * q + 2]);
+            o.w = apply_act<ACT>(acc[4 * q + 3]);
+            ov[q] = o;
+        }
+    }
+}
+
+__device__ __forceinline__ int find_segment(const int32_t* __restrict__ off, int S, int cand) {
+    // largest s with off[s] <= cand (empty segments have off[s] == off[s+1]; pick the one that contains cand)
+    int lo = 0, hi = S;  // invariant: off[lo] <= cand < off[hi]
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(off + mid) <= cand) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+constexpr int kGenericThreads = 256;
+
+template <int R>
+__global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const GenericParams p) {
+    extern __shared__ __align__(16) float smem[];
+    const int d = p.d, da = p.da, H = p.H, P = p.P;
+    const int K1 = d + da;
+    float* X = smem;                                   // [(d+da+H)][R]  rows: z | a (phi) | hw
+    float* Hb = X + (size_t)(K1 + H) * R;              // [maxw][R]
+    float* ALT = Hb + (size_t)p.maxw * R;              // [alt_rows][R]: V | AS | Y   (scorer: ping-pong buffer)
+    float* V = ALT;                                    // [d][R]
+    float* AS = V + (size_t)d * R;                     // [da][R]
+    float* Y = AS + (size_t)da * R;                    // [(d+da)][R], GRU only
+    float* LP = ALT + (size_t)p.alt_rows * R;          // [R][P] log2(param) or bucket index (as int bits)
+    float* RED = LP + (size_t)R * P;                   // [G][R] reduction scratch, G = threads / R
+    int* meta = reinterpret_cast<int*>(RED + kGenericThreads);   // cand[R], len[R], seg[R], id[R], tile_len
+    int* m_cand = meta;
+    int* m_len = meta + R;
+    int* m_seg = meta + 2 * R;
+    int* m_id = meta + 3 * R;
+    int* m_tile_len = meta + 4 * R;
+
+    const int tid = threadIdx.x;
+    const int r_of = tid % R;
+    const int g_of = tid / R;
+    constexpr int G = kGenericThreads / R;
+    const CallArgs& a = p.a;
+
+    for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+        __syncthreads();
+        if (tid == 0) *m_tile_len = 0;
+        __syncthreads();
+        if (tid < R) {
+            const int64_t i = (int64_t)tile * R + tid;
+            int cand = -1, len = 0, seg = 0;
+            if (i < a.B) {
+                cand = a.perm ? __ldg(a.perm + i) : (int)i;
+                len = __ldg(a.lengths + cand);
+                if (len < 0 || len > a.T_max) {
+                    atomicOr(a.fault, WM_FAULT_LEN);
+                    len = len < 0 ? 0 : a.T_max;
+                }
+                seg = a.offsets ? find_segment(a.offsets, a.S, cand) : cand;
+            }
+            m_cand[tid] = cand;
+            m_len[tid] = len;
+            m_seg[tid] = seg;
+            atomicMax(m_tile_len, len);
+        }
+        __syncthreads();
+        const int tile_len = *m_tile_len;
+        // z_0 and the running action sum
+        for (int e = tid; e < d * R; e += kGenericThreads) {
+            const int r = e % R, j = e / R;   // lanes over rows: conflict-free store; global read strided but tiny
+            X[(size_t)j * R + r] = m_cand[r] >= 0 ? __ldg(a.init_states + (size_t)m_seg[r] * d + j) : 0.0f;
+        }
+        for (int e = tid; e < da * R; e += kGenericThreads) AS[e] = 0.0f;
+        __syncthreads();
+
+        for (int t = 0; t < tile_len; ++t) {
+            // ---- a1: action embedding of step t (rows with t >= len get a = 0 and touch no input)
+            if (tid < R) {
+                int id = 0;
+                if (t < m_len[tid]) {
+                    id = __ldg(a.action_ids + (size_t)m_cand[tid] * a.T_max + t);
+                    if (id < 0 || id >= p.n_types) {
+                        atomicOr(a.fault, WM_FAULT_TYPE);
+                        id = id < 0 ? 0 : p.n_types - 1;
+                    }
+                }
+                m_id[tid] = id;
+            }
+            for (int e = tid; e < R * P; e += kGenericThreads) {
+                const int r = e / P, j = e % P;
+                float v = 0.0f;
+                if (t < m_len[r]) {
+                    int prm = __ldg(a.action_params + ((size_t)m_cand[r] * a.T_max + t) * P + j);
+                    if (prm < 1) {
+                        atomicOr(a.fault, WM_FAULT_PARAM);
+                        prm = 1;
+                    }
+                    if (p.embed == WM_EMBED_LINEAR) {
+                        v = log2f((float)prm);
+                    } else {
+                        // bucket(p) = min(n_b-1, floor(4 log2 p)) = bit_length(p^4)-1, exact in 64-bit for p < 2^16
+                        unsigned long long q = (unsigned long long)min(prm, 65535);
+                        q = q * q;
+                        q = q * q;
+                        int bk = 63 - __clzll((long long)q);
+                        v = __int_as_float(min(bk, p.n_buckets - 1));
+                    }
+                }
+                LP[e] = v;
+            }
+            __syncthreads();
+            for (int e = tid; e < da * R; e += kGenericThreads) {
+                const int r = e % R, j = e / R;
+                float v = 0.0f;
+                if (t < m_len[r]) {
+                    const int id = m_id[r];
+                    if (p.embed == WM_EMBED_LINEAR) {
+                        v = __ldg(p.E + (size_t)id * da + j) + __ldg(p.bp + j);
+                        for (int q = 0; q < P; ++q) v = fmaf(__ldg(p.WpT + (size_t)q * da + j), LP[r * P + q], v);
+                    } else {
+                        for (int q = 0; q < P; ++q) {
+                            const int bk = __float_as_int(LP[r * P + q]);
+                            v += __ldg(p.Tbl + ((size_t)(id * P + q) * p.n_buckets + bk) * da + j);
+                        }
+                    }
+                    AS[e] += v;   // a4: running sum for phi
+                }
+                X[(size_t)(d + j) * R + r] = v;
+            }
+            __syncthreads();
+
+            // ---- a2/a3: one transition step, rows with t >= len frozen
+            if (p.kind != WM_KIND_GRU) {
+                linear_T<R, ACT_GELU>(p.W1t, p.b1, X, K1, p.hidden, Hb);
+                __syncthreads();
+                linear_T<R, ACT_NONE>(p.W2t, p.b2, Hb, p.hidden, d, V);
+                __syncthreads();
+                if (p.kind == WM_KIND_MLP_LN) {
+                    // v = z + V; two-pass LayerNorm over the d features of each row
+                    float s = 0.0f;
+                    for (int j = g_of; j < d; j += G) {
+                        const float v = X[(size_t)j * R + r_of] + V[(size_t)j * R + r_of];
+                        V[(size_t)j * R + r_of] = v;
+                        s += v;
+                    }
+                    RED[g_of * R + r_of] = s;
+                    __syncthreads();
+                    float mean = 0.0f;
+                    for (int g = 0; g < G; ++g) mean += RED[g * R + r_of];
+                    mean /= (float)d;
+                    __syncthreads();
+                    float q = 0.0f;
+                    for (int j = g_of; j < d; j += G) {
+                        const float c = V[(size_t)j * R + r_of] - mean;
+                        q = fmaf(c, c, q);
+                    }
+                    RED[g_of * R + r_of] = q;
+                    __syncthreads();
+                    float var = 0.0f;
+                    for (int g = 0; g < G; ++g) var += RED[g * R + r_of];
+                    var /= (float)d;
+                    const float rstd = 1.0f / sqrtf(var + p.ln_eps);
+                    if (t < m_len[r_of]) {
+                        for (int j = g_of; j < d; j += G) {
+                            const float c = (V[(size_t)j * R + r_of] - mean) * rstd;
+                            X[(size_t)j * R + r_of] = fmaf(__ldg(p.gamma + j), c, __ldg(p.beta + j));
+                        }
+                    }
+                } else {
+                    if (t < m_len[r_of]) {
+                        for (int j = g_of; j < d; j += G) X[(size_t)j * R + r_of] += V[(size_t)j * R + r_of];
+                    }
+                }
+            } else {
+                linear_T<R, ACT_SIGMOID>(p.Wgt, nullptr, X, K1, d, Hb);   // g
+                linear_T<R, ACT_SIGMOID>(p.Wrt, nullptr, X, K1, d, V);    // r
+                __syncthreads();
+                for (int e = tid; e < K1 * R; e += kGenericThreads)
+                    Y[e] = e < d * R ? V[e] * X[e] : X[e];                // [r*z ; a]
+                __syncthreads();
+                linear_T<R, ACT_TANH>(p.Wht, nullptr, Y, K1, d, V);       // candidate h
+                __syncthreads();
+                if (t < m_len[r_of]) {
+                    for (int j = g_of; j < d; j += G) {
+                        const size_t o = (size_t)j * R + r_of;
+                        const float g = Hb[o];
+                        X[o] = (1.0f - g) * X[o] + g * V[o];
+                    }
+                }
+            }
+            __syncthreads();
+        }
+
+        // ---- a4/a5: x = [z_T ; phi ; hw], scorer MLP
+        for (int e = tid; e < da * R; e += kGenericThreads) {
+            const int r = e % R;
+            const int len = m_len[r];
+            X[(size_t)d * R + e] = len > 0 ? AS[e] / (float)len : 0.0f;
+        }
+        for (int e = tid; e < H * R; e += kGenericThreads) {
+            const int r = e % R, j = e / R;
+            X[(size_t)K1 * R + e] = m_cand[r] >= 0 ? __ldg(a.hw_feats + (size_t)m_seg[r] * H + j) : 0.0f;
+        }
+        __syncthreads();
+        const float* in = X;
+        for (int l = 0; l < p.n_lin; ++l) {
+            float* out = (l & 1) ? ALT : Hb;
+            if (l + 1 < p.n_lin)
+                linear_T<R, ACT_GELU>(p.Wst[l], p.bs[l], in, p.sdim[l], p.sdim[l + 1], out);
+            else
+                linear_T<R, ACT_NONE>(p.Wst[l], p.bs[l], in, p.sdim[l], p.sdim[l + 1], out);
+            __syncthreads();
+            in = out;
+        }
+        // ---- a6: scatter to the original order
+        if (tid < R && m_cand[tid] >= 0) a.scores_out[m_cand[tid]] = in[tid];
+    }
+}
+
+static size_t generic_smem_bytes(const Model& m, int R, int* maxw_out, int* alt_rows_out) {
+    int maxw = m.d > m.hidden ? m.d : m.hidden;
+    int maxsw = 1;
+    for (int l = 1; l <= m.n_lin; ++l) maxsw = m.sdim[l] > maxsw ? m.sdim[l] : maxsw;
+    if (maxsw > maxw) maxw = maxsw;
+    int alt = m.d + m.d_a + (m.kind == WM_KIND_GRU ? m.d + m.d_a : 0);
+    if (maxsw > alt) alt = maxsw;
+    *maxw_out = maxw;
+    *alt_rows_out = alt;
+    size_t floats = (size_t)(m.d + m.d_a + m.H) * R + (size_t)maxw * R + (size_t)alt * R + (size_t)R * m.P +
+                    kGenericThreads;
+    return floats * 4 + (4 * R + 4) * sizeof(int);
+}
+
+template <int R>
+static int launch_R(wm_ctx* ctx, const GenericParams& p, size_t smem, int grid, cudaStream_t st) {
+    WM_CUDA_TRY(cudaFuncSetAttribute(wm_generic_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    wm_generic_kernel<R><<<grid, kGenericThreads, smem, st>>>(p);
+    WM_CUDA_TRY(cudaGetLastError());
+    ctx->launches.fetch_add(1);
+    return WM_OK;
+}
+
+static int pick_R(const wm_ctx* ctx, int64_t B, size_t* smem_out, int* maxw, int* alt) {
+    // Largest tile that fits shared memory; small batches take smaller tiles so the (latency-bound) work
+    // spreads over the SMs.
+    const int cands[4] = {32, 16, 8, 4};
+    int fallback = 0;
+    for (int i = 0; i < 4; ++i) {
+        const int R = cands[i];
+        if (generic_smem_bytes(ctx->m, R, maxw, alt) > (size_t)ctx->smem_optin) continue;
+        if (!fallback) fallback = R;
+        if ((B + R - 1) / R >= ctx->n_sms || R == 4) {
+            *smem_out = generic_smem_bytes(ctx->m, R, maxw, alt);
+            return R;
+        }
+    }
+    if (fallback) *smem_out = generic_smem_bytes(ctx->m, fallback, maxw, alt);
+    return fallback;
+}
+
+int generic_supported(const wm_ctx* ctx) {
+    size_t s;
+    int a, b;
+    return pick_R(ctx, 1 << 20, &s, &a, &b) != 0;
+}
+
+int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st) {
+    const Model& m = ctx->m;
+    GenericParams p;
+    p.kind = m.kind; p.embed = m.embed; p.d = m.d; p.da = m.d_a; p.hidden = m.hidden; p.n_types = m.n_types;
+    p.P = m.P; p.n_buckets = m.n_buckets; p.H = m.H; p.n_lin = m.n_lin;
+    for (int i = 0; i <= kMaxScorerLinears; ++i) p.sdim[i] = m.sdim[i];
+    p.ln_eps = m.ln_eps;
+    p.E = m.E; p.WpT = m.WpT; p.bp = m.bp; p.Tbl = m.Tbl;
+    p.W1t = m.W1t; p.b1 = m.b1; p.W2t = m.W2t; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.Wgt = m.Wgt; p.Wrt = m.Wrt; p.Wht = m.Wht;
+    for (int i = 0; i < kMaxScorerLinears; ++i) { p.Wst[i] = m.Wst[i]; p.bs[i] = m.bs[i]; }
+    p.a = a;
+    size_t smem = 0;
+    const int R = pick_R(ctx, a.B, &smem, &p.maxw, &p.alt_rows);
+    if (R == 0) {
+        set_error("model too wide for the fp32 kernel's shared-memory tile");
+        return WM_ERR_UNSUPPORTED;
+    }
+    p.n_tiles = (int)((a.B + R - 1) / R);
+    int grid = p.n_tiles < ctx->n_sms * 4 ? p.n_tiles : ctx->n_sms * 4;
+    if (grid < 1) return WM_OK;
+    switch (R) {
+        case 32: return launch_R<32>(ctx, p, smem, grid, st);
+        case 16: return launch_R<16>(ctx, p, smem, grid, st);
+        case 8: return launch_R<8>(ctx, p, smem, grid, st);
+        default: return launch_R<4>(ctx, p, smem, grid, st);
+    }
+}
+
+}  // namespace wm

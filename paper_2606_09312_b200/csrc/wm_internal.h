@@ -1,0 +1,128 @@
+// Internal declarations shared by the library's translation units (not part of the ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "wm.h"
+
+namespace wm {
+
+constexpr int kMaxScorerLinears = 7;
+
+// ---------------------------------------------------------------------------------------------------------
+// Model description + device weights in every layout a kernel wants.
+struct Model {
+    int kind = 0, dtype = 0, embed = 0;
+    int d = 0, d_a = 0, hidden = 0, n_types = 0, P = 0, n_buckets = 0, H = 0;
+    int n_lin = 0;                       // linears of G
+    int sdim[kMaxScorerLinears + 1] = {};  // sdim[0] = d+d_a+H, ..., sdim[n_lin] = 1
+    float ln_eps = 1e-5f;
+
+    // fp32 CUDA-core path: matrices stored TRANSPOSED ([in][out]) so that consecutive threads (one output unit
+    // each) read consecutive addresses; vectors as in the file.
+    float* E = nullptr;        // [n_types][d_a]
+    float* WpT = nullptr;      // [P][d_a]
+    float* bp = nullptr;       // [d_a]
+    float* Tbl = nullptr;      // [n_types*P*n_buckets][d_a]
+    float* W1t = nullptr;      // [d+d_a][hidden]
+    float* b1 = nullptr;
+    float* W2t = nullptr;      // [hidden][d]
+    float* b2 = nullptr;
+    float* gamma = nullptr;
+    float* beta = nullptr;
+    float* Wgt = nullptr;      // [d+d_a][d]
+    float* Wrt = nullptr;
+    float* Wht = nullptr;
+    float* Wst[kMaxScorerLinears] = {};   // [in_i][out_i]
+    float* bs[kMaxScorerLinears] = {};
+
+    // tcgen05 path (bf16 MLP_LN models): weight images pre-tiled into the shared-memory layout the MMA
+    // descriptors expect, see wm_tc.cu.  nullptr when the path does not apply.
+    void* tc_blob = nullptr;
+    size_t tc_blob_bytes = 0;
+    int tc_ok = 0;
+};
+
+// Per-stream slice of the workspace (perm, histogram/cursors, tile counter).
+struct Workspace {
+    cudaStream_t stream = nullptr;
+    int32_t* perm = nullptr;
+    int64_t perm_cap = 0;
+    int32_t* counters = nullptr;   // [kCounterInts] hist[WM_MAX_T+1], cursor[WM_MAX_T+1], tile counter, ...
+    // staging for wm_score_topk_host
+    void* stage = nullptr;
+    size_t stage_cap = 0;
+};
+
+constexpr int kHistOff = 0;
+constexpr int kCursorOff = WM_MAX_T + 1;
+constexpr int kTileCtrOff = 2 * (WM_MAX_T + 1);
+constexpr int kCounterInts = 2 * (WM_MAX_T + 1) + 8;
+
+}  // namespace wm
+
+struct wm_ctx {
+    wm::Model m;
+    int device = 0;
+    int n_sms = 148;
+    int smem_optin = 0;
+    int opt_path = 0;     // WM_OPT_PATH
+    int opt_sort = 1;     // WM_OPT_SORT
+    uint32_t* fault = nullptr;   // device fault word
+    std::mutex mu;
+    std::vector<wm::Workspace*> pool;
+    std::vector<void*> allocs;   // every device allocation owned by the ctx (weights)
+    std::atomic<int64_t> launches{0};
+};
+
+namespace wm {
+
+void set_error(const char* fmt, ...);
+#define WM_CUDA_TRY(expr)                                                                       \
+    do {                                                                                        \
+        cudaError_t e__ = (expr);                                                               \
+        if (e__ != cudaSuccess) {                                                               \
+            ::wm::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+            return WM_ERR_CUDA;                                                                 \
+        }                                                                                       \
+    } while (0)
+
+// Arguments of one wm_rollout_score call, after validation.
+struct CallArgs {
+    const float* init_states;
+    const int32_t* action_ids;
+    const int32_t* action_params;
+    const int32_t* lengths;
+    const float* hw_feats;
+    float* scores_out;
+    const int32_t* offsets;   // may be null (per-candidate mode)
+    const int32_t* perm;      // may be null (identity)
+    int64_t B;
+    int S, T_max;
+    uint32_t* fault;
+};
+
+// K1 (wm_bucket.cu): perm = candidates sorted by clamped length, descending.  2 launches + 1 memset.
+int launch_length_bucketing(wm_ctx* ctx, Workspace* ws, const int32_t* lengths, int64_t B, int T_max,
+                            cudaStream_t st);
+
+// K2-fp32 (wm_generic.cu): every model kind, fp32 CUDA cores.
+int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st);
+int generic_supported(const wm_ctx* ctx);
+
+// K2 tcgen05 (wm_tc.cu): bf16 MLP_LN models with d = 256.
+int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
+               const std::vector<std::string>& names);
+int tc_supported(const wm_ctx* ctx);
+int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
+
+// K3 (wm_topk.cu)
+int launch_topk(const float* scores, const int32_t* offsets, int S, int k, int32_t* idx_out, cudaStream_t st);
+
+}  // namespace wm

@@ -1,0 +1,98 @@
+"""CPU-only checks of the boundary: libwm.so loads, exports every symbol include/wm.h declares, and the argument /
+file-format errors that need no GPU behave as the header says.  No compute calls."""
+import os
+import re
+import struct
+
+import pytest
+
+import gen
+import paper_2606_09312_b200 as wm
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_2606_09312_b200 import build
+    build.build()
+    return wm.lib()
+
+
+def test_exports_every_declared_symbol(L):
+    hdr = open(os.path.join(ROOT, "include", "wm.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(wm_[a-z_]+)\s*\(", hdr))
+    assert declared == set(wm.ABI_SYMBOLS), declared ^ set(wm.ABI_SYMBOLS)
+    for s in declared:
+        assert hasattr(L, s), s
+
+
+def test_constants_match_header():
+    hdr = open(os.path.join(ROOT, "include", "wm.h")).read()
+    for name in ("WM_OK", "WM_ERR_ARG", "WM_ERR_IO", "WM_ERR_FORMAT", "WM_ERR_CUDA", "WM_ERR_UNSUPPORTED",
+                 "WM_MAX_T", "WM_MAX_K", "WM_OPT_PATH", "WM_OPT_SORT"):
+        m = re.search(rf"#define\s+{name}\s+(-?\d+)", hdr)
+        assert m and int(m.group(1)) == getattr(wm, name), name
+
+
+def test_topk_argument_errors(L):
+    assert L.wm_topk(None, None, -1, 3, None, None) == wm.WM_ERR_ARG
+    assert "S=-1" in wm.wm_last_error()
+    assert L.wm_topk(None, None, 4, 0, None, None) == wm.WM_ERR_ARG
+    assert L.wm_topk(None, None, 4, wm.WM_MAX_K + 1, None, None) == wm.WM_ERR_ARG
+    assert L.wm_topk(None, None, 4, 8, None, None) == wm.WM_ERR_ARG       # null pointers with S > 0
+    assert L.wm_topk(None, None, 0, 8, None, None) == wm.WM_OK            # S = 0 is a no-op
+
+
+def test_null_ctx_errors(L):
+    assert L.wm_rollout_score(None, None, None, None, None, None, None, None, 1, 1, 1, None) == wm.WM_ERR_ARG
+    assert L.wm_check(None, None) == wm.WM_ERR_ARG
+    assert L.wm_set_option(None, 1, 0) == wm.WM_ERR_ARG
+    L.wm_free(None)
+
+
+def test_load_weights_io_and_format_errors(tmp_path):
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "missing.wmw"))
+    assert e.value.code == wm.WM_ERR_IO
+    bad = tmp_path / "bad.wmw"
+    bad.write_bytes(b"NOPE" + b"\0" * 100)
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(bad))
+    assert e.value.code == wm.WM_ERR_FORMAT
+    short = tmp_path / "short.wmw"
+    short.write_bytes(b"WMW1" + struct.pack("<I", 1))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(short))
+    assert e.value.code == wm.WM_ERR_FORMAT
+    # a valid header whose tensors are cut short, and one with trailing bytes
+    cfg = gen.get_config(1)
+    good = tmp_path / "good.wmw"
+    gen.write_weight_file(str(good), cfg, gen.make_weights(cfg))
+    raw = good.read_bytes()
+    (tmp_path / "trunc.wmw").write_bytes(raw[:-8])
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "trunc.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT and "truncated" in str(e.value)
+    (tmp_path / "trail.wmw").write_bytes(raw + b"\0")
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "trail.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT and "trailing" in str(e.value)
+    # header field out of range (d = 0)
+    hdr = bytearray(raw)
+    struct.pack_into("<I", hdr, 4 + 4 * 4, 0)
+    (tmp_path / "d0.wmw").write_bytes(bytes(hdr))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "d0.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT
+
+
+def test_no_product_import_of_oracle():
+    """The product path must not route through the oracle (or any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_2606_09312_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh", ".cpp")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), f

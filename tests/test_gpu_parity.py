@@ -1,0 +1,225 @@
+"""GPU parity: the C-ABI path against the float64 oracle, element by element, on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; metric S15 of DESIGN.md §3 = |y - y_ref| / max(|y_ref|, RMS_subgraph(y_ref))):
+  fp32 config (cfg 1): max relative error <= 1e-4
+  bf16 configs (cfg 2-5): max relative error <= 2e-2 and mean top-k overlap >= 0.95
+Top-k indices are bit-exact given identical scores (tests/test_gpu_topk.py).
+"""
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from gen.configs import DTYPE_FP32
+from wm_harness import weight_file, gpu_scores, gpu_topk, oracle_scores
+
+pytestmark = pytest.mark.gpu
+
+TOL = {True: 1e-4, False: 2e-2}
+
+# sizes the oracle finishes in seconds, several tiles of every kernel (4..128 rows) plus a ragged tail
+SMALL = {1: dict(S=1, per_subgraph=64), 2: dict(S=3, per_subgraph=171), 3: dict(S=3, per_subgraph=139),
+         4: dict(S=2, per_subgraph=320), 5: dict(S=3, per_subgraph=150)}
+
+
+@pytest.fixture(scope="module")
+def wm():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2606_09312_b200 as wm
+    return wm
+
+
+def _ctx(wm, cfg, path=None):
+    ctx = wm.wm_load_weights(weight_file(cfg))
+    if path is not None:
+        wm.wm_set_option(ctx, wm.WM_OPT_PATH, path)
+    return ctx
+
+
+def _paths(wm, cfg):
+    ctx = wm.wm_load_weights(weight_file(cfg))
+    auto = wm.wm_get_info(ctx).path
+    wm.wm_free(ctx)
+    return sorted({wm.PATH_FP32, auto})
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5])
+def test_config_parity_small(wm, n):
+    cfg = gen.get_config(n).scaled(**SMALL[n])
+    w = gen.make_weights(cfg)
+    b = gen.make_inputs(cfg)
+    ref = oracle_scores(cfg, w, b)
+    for path in _paths(wm, cfg):
+        ctx = _ctx(wm, cfg, path)
+        y = gpu_scores(ctx, b)
+        wm.wm_free(ctx)
+        tol = TOL[cfg.dtype == DTYPE_FP32] if path != wm.PATH_FP32 else (1e-4 if n == 1 else 2e-3)
+        err = oracle.score_error(y, ref, b.subgraph_offsets)
+        assert np.isfinite(y).all()
+        assert err <= tol, (n, path, err)
+        idx = gpu_topk(y, b.subgraph_offsets, cfg.k)
+        ref_idx = oracle.topk_segments(ref, b.subgraph_offsets, cfg.k)
+        mean_ov, _ = oracle.topk_overlap(idx, ref_idx)
+        assert mean_ov >= 0.95, (n, path, mean_ov)
+        # top-k is bit-exact given identical scores
+        np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
+
+
+def _edge_batch(cfg, lengths=None, S=None, per=None):
+    c = cfg.scaled(S=S or cfg.S, per_subgraph=per or cfg.per_subgraph)
+    b = gen.make_inputs(c, sentinel_padding=False)
+    if lengths is not None:
+        b.lengths[:] = np.asarray(lengths, dtype=np.int32)
+    # re-apply the sentinel padding for the new lengths
+    T = b.T_max
+    pad = np.arange(T)[None, :] >= b.lengths[:, None]
+    sent = np.where((np.arange(T) % 2) == 0, -2**31, 2**31 - 1).astype(np.int32)
+    b.action_ids = np.where(pad, sent[None, :], b.action_ids).astype(np.int32)
+    b.action_params = np.where(pad[:, :, None], sent[None, :, None], b.action_params).astype(np.int32)
+    return c, b
+
+
+@pytest.mark.parametrize("n", [1, 2, 5])
+@pytest.mark.parametrize("case", ["B1", "B127", "B129", "B257", "len0", "lenmax", "one_long", "param_ends"])
+def test_edge_cases(wm, n, case):
+    base = gen.get_config(n)
+    T = base.T_max
+    if case.startswith("B"):
+        B = int(case[1:])
+        cfg, b = _edge_batch(base, S=1, per=B)
+    elif case == "len0":
+        cfg, b = _edge_batch(base, lengths=0, S=2, per=70)
+    elif case == "lenmax":
+        cfg, b = _edge_batch(base, lengths=T, S=2, per=70)
+    elif case == "one_long":
+        ln = np.full(140, min(2, T), dtype=np.int32)
+        ln[77] = T
+        cfg, b = _edge_batch(base, lengths=ln, S=2, per=70)
+    else:
+        cfg, b = _edge_batch(base, lengths=T, S=1, per=66)
+        b.action_params[0::2] = 1
+        b.action_params[1::2] = base.param_hi
+    w = gen.make_weights(cfg)
+    ref = oracle_scores(cfg, w, b)
+    for path in _paths(wm, cfg):
+        ctx = _ctx(wm, cfg, path)
+        y = gpu_scores(ctx, b)
+        wm.wm_free(ctx)
+        tol = 1e-4 if n == 1 else (2e-3 if path == wm.PATH_FP32 else 2e-2)
+        assert oracle.score_error(y, ref, b.subgraph_offsets) <= tol, (n, case, path)
+
+
+@pytest.mark.parametrize("n", [1, 2, 5])
+def test_per_candidate_mode_and_segments(wm, n):
+    """subgraph_offsets = NULL (per-candidate z0/hw); ragged, empty and many segments (S > #CTAs)."""
+    base = gen.get_config(n)
+    cfg = base.scaled(S=1, per_subgraph=150)
+    b = gen.make_inputs(cfg)
+    w = gen.make_weights(cfg)
+    rng = np.random.default_rng(5)
+    # per-candidate mode
+    b.init_states = rng.standard_normal((150, cfg.d)).astype(np.float32)
+    b.hw_feats = rng.standard_normal((150, cfg.H)).astype(np.float32)
+    ref = oracle_scores(cfg, w, b, per_candidate=True)
+    for path in _paths(wm, cfg):
+        ctx = _ctx(wm, cfg, path)
+        y = gpu_scores(ctx, b, per_candidate=True)
+        tol = 1e-4 if n == 1 else (2e-3 if path == wm.PATH_FP32 else 2e-2)
+        assert oracle.score_error(y, ref, None) <= tol
+        # ragged CSR with empty segments, S = 300 > 148 SMs
+        cuts = np.sort(rng.integers(0, 151, size=299))
+        off = np.concatenate([[0], cuts, [150]]).astype(np.int32)
+        b2 = gen.Batch(rng.standard_normal((300, cfg.d)).astype(np.float32),
+                       rng.standard_normal((300, cfg.H)).astype(np.float32),
+                       b.action_ids, b.action_params, b.lengths, off, b.T_max)
+        ref2 = oracle_scores(cfg, w, b2)
+        y2 = gpu_scores(ctx, b2)
+        wm.wm_free(ctx)
+        assert oracle.score_error(y2, ref2, off) <= tol
+
+
+def test_p2_padding_invariance_bitwise(wm):
+    """Changing ids/params at t >= len (incl. out-of-range values) leaves GPU scores bit-identical."""
+    for n in (1, 2):
+        cfg = gen.get_config(n).scaled(S=2, per_subgraph=100)
+        b = gen.make_inputs(cfg)
+        for path in _paths(wm, cfg):
+            ctx = _ctx(wm, cfg, path)
+            y1 = gpu_scores(ctx, b)
+            b2 = gen.make_inputs(cfg, sentinel_padding=False)   # padding = in-range random values instead
+            y2 = gpu_scores(ctx, b2)
+            wm.wm_free(ctx)
+            np.testing.assert_array_equal(y1.view(np.uint32), y2.view(np.uint32))
+
+
+def test_sort_option_is_bit_invariant(wm):
+    """Length bucketing only permutes rows between tiles: scores are bit-identical with it off."""
+    for n in (1, 2):
+        cfg = gen.get_config(n).scaled(S=2, per_subgraph=333)
+        b = gen.make_inputs(cfg)
+        for path in _paths(wm, cfg):
+            ctx = _ctx(wm, cfg, path)
+            y1 = gpu_scores(ctx, b)
+            wm.wm_set_option(ctx, wm.WM_OPT_SORT, 0)
+            y2 = gpu_scores(ctx, b)
+            wm.wm_free(ctx)
+            np.testing.assert_array_equal(y1.view(np.uint32), y2.view(np.uint32))
+
+
+def test_fault_word(wm):
+    import torch
+    from wm_harness import to_device
+    cfg = gen.get_config(1)
+    b = gen.make_inputs(cfg, sentinel_padding=False)
+    b.lengths[:] = 4
+    b.lengths[3] = 100            # > T_max
+    b.action_ids[5, 1] = 99       # type out of range at a valid position
+    b.action_params[7, 2, 0] = 0  # parameter < 1 at a valid position
+    ctx = _ctx(wm, cfg)
+    dv = to_device(b)
+    out = torch.empty(b.B, dtype=torch.float32, device="cuda:0")
+    wm.wm_rollout_score(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                        dv["hw_feats"], out, dv["subgraph_offsets"])
+    assert wm.wm_check(ctx) == (wm.WM_FAULT_LEN | wm.WM_FAULT_TYPE | wm.WM_FAULT_PARAM)
+    assert wm.wm_check(ctx) == 0
+    assert torch.isfinite(out).all()
+    wm.wm_free(ctx)
+
+
+def test_two_streams_share_one_ctx(wm):
+    import torch
+    cfg = gen.get_config(2).scaled(S=2, per_subgraph=300)
+    b = gen.make_inputs(cfg)
+    ctx = _ctx(wm, cfg)
+    ref = gpu_scores(ctx, b)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    from wm_harness import to_device
+    dv = to_device(b)
+    outs = [torch.empty(b.B, dtype=torch.float32, device="cuda:0") for _ in range(6)]
+    torch.cuda.synchronize()
+    for i, o in enumerate(outs):
+        st = s1 if i % 2 == 0 else s2
+        wm.wm_rollout_score(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                            dv["hw_feats"], o, dv["subgraph_offsets"], stream=st)
+    torch.cuda.synchronize()
+    for o in outs:
+        np.testing.assert_array_equal(o.cpu().numpy().view(np.uint32), ref.view(np.uint32))
+    wm.wm_free(ctx)
+
+
+def test_host_entry_matches_device_entry(wm):
+    import torch
+    cfg = gen.get_config(2).scaled(S=3, per_subgraph=200)
+    b = gen.make_inputs(cfg)
+    ctx = _ctx(wm, cfg)
+    y = gpu_scores(ctx, b)
+    idx = gpu_topk(y, b.subgraph_offsets, cfg.k)
+    h = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    sc = torch.empty(b.B, dtype=torch.float32).pin_memory()
+    ix = torch.empty((b.S, cfg.k), dtype=torch.int32).pin_memory()
+    wm.wm_score_topk_host(ctx, h(b.init_states), h(b.action_ids), h(b.action_params), h(b.lengths),
+                          h(b.hw_feats), h(b.subgraph_offsets), cfg.k, sc, ix)
+    np.testing.assert_array_equal(sc.numpy().view(np.uint32), y.view(np.uint32))
+    np.testing.assert_array_equal(ix.numpy(), idx)
+    wm.wm_free(ctx)
