@@ -68,6 +68,8 @@ extern "C" {
 /* wm_set_option keys */
 #define WM_OPT_PATH      1      /* 0 = auto (default), 1 = force the fp32 CUDA-core kernel, 2 = force tcgen05  */
 #define WM_OPT_SORT      2      /* 1 = bucket candidates by length before tiling (default), 0 = input order    */
+#define WM_OPT_TIMING    3      /* 1 = record CUDA events around the rollout+score kernel (K2) of every call,   */
+                                /*     read back with wm_last_kernel_ms; 0 = off (default)                      */
 
 typedef struct wm_ctx wm_ctx;   /* opaque: device weights (all layouts the kernels need) + workspace pool      */
 
@@ -147,6 +149,11 @@ int wm_score_topk_host(wm_ctx* ctx,
                        const int32_t* lengths, const float* hw_feats, const int32_t* subgraph_offsets,
                        int64_t B, int32_t S, int32_t T_max, int32_t k,
                        float* scores_out, int32_t* idx_out, void* cuda_stream);
+
+/* With WM_OPT_TIMING = 1: synchronise `cuda_stream` and return, in *ms_out, the device time of the rollout+score
+ * kernel (K2 alone: bucketing and top-k excluded) of the most recent wm_rollout_score call made on that stream.
+ * bench.py's roofline leg uses it.  Errors: WM_ERR_ARG (null, timing off, or no call yet), WM_ERR_CUDA. */
+int wm_last_kernel_ms(wm_ctx* ctx, void* cuda_stream, float* ms_out);
 
 /* Number of kernels the library launched on behalf of this ctx since it was created (bench.py's
  * gpu_launches); wm_topk's launches are counted in a process-wide counter returned when ctx == NULL. */

@@ -17,12 +17,12 @@ LIB_PATH = os.path.join(_HERE, "libwm.so")
 WM_OK, WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_CUDA, WM_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 WM_MAX_T, WM_MAX_K = 256, 1024
 WM_FAULT_LEN, WM_FAULT_TYPE, WM_FAULT_PARAM = 1, 2, 4
-WM_OPT_PATH, WM_OPT_SORT = 1, 2
+WM_OPT_PATH, WM_OPT_SORT, WM_OPT_TIMING = 1, 2, 3
 PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 
 # every symbol include/wm.h declares
 ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
-               "wm_check", "wm_score_topk_host", "wm_launch_count", "wm_last_error")
+               "wm_check", "wm_score_topk_host", "wm_last_kernel_ms", "wm_launch_count", "wm_last_error")
 
 
 class WmInfo(ctypes.Structure):
@@ -68,6 +68,8 @@ def lib() -> ctypes.CDLL:
     L.wm_check.restype = ctypes.c_int
     L.wm_score_topk_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp, vp, vp]
     L.wm_score_topk_host.restype = ctypes.c_int
+    L.wm_last_kernel_ms.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_float)]
+    L.wm_last_kernel_ms.restype = ctypes.c_int
     L.wm_launch_count.argtypes = [vp]
     L.wm_launch_count.restype = i64
     L.wm_last_error.argtypes = []
@@ -149,6 +151,12 @@ def wm_score_topk_host(ctx: int, init_states, action_ids, action_params, lengths
     _check(lib().wm_score_topk_host(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
                                     _ptr(hw_feats), _ptr(subgraph_offsets), B, S, T_max, int(k),
                                     _ptr(scores_out), _ptr(idx_out), _stream(stream)))
+
+
+def wm_last_kernel_ms(ctx: int, stream=None) -> float:
+    ms = ctypes.c_float()
+    _check(lib().wm_last_kernel_ms(ctx, _stream(stream), ctypes.byref(ms)))
+    return float(ms.value)
 
 
 def wm_launch_count(ctx: Optional[int]) -> int:

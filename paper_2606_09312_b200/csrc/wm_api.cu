@@ -17,8 +17,6 @@ void set_error(const char* fmt, ...) {
     va_end(ap);
 }
 
-int64_t topk_launches();
-
 namespace {
 
 struct Header {
@@ -256,6 +254,8 @@ void wm_free(wm_ctx* ctx) {
         if (w->perm) cudaFree(w->perm);
         if (w->counters) cudaFree(w->counters);
         if (w->stage) cudaFree(w->stage);
+        if (w->ev0) cudaEventDestroy(w->ev0);
+        if (w->ev1) cudaEventDestroy(w->ev1);
         delete w;
     }
     for (void* p : ctx->allocs) cudaFree(p);
@@ -305,6 +305,14 @@ int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value) {
         ctx->opt_sort = value;
         return WM_OK;
     }
+    if (key == WM_OPT_TIMING) {
+        if (value < 0 || value > 1) {
+            set_error("wm_set_option: WM_OPT_TIMING takes 0 or 1");
+            return WM_ERR_ARG;
+        }
+        ctx->opt_timing = value;
+        return WM_OK;
+    }
     set_error("wm_set_option: unknown key %d", key);
     return WM_ERR_ARG;
 }
@@ -344,8 +352,40 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
         if (rc != WM_OK) return rc;
         a.perm = ws->perm;
     }
-    if (pick_path(ctx) == 2) return launch_tc(ctx, ws, a, st);
-    return launch_generic(ctx, a, st);
+    if (ctx->opt_timing) {
+        if (!ws->ev0) {
+            WM_CUDA_TRY(cudaEventCreate(&ws->ev0));
+            WM_CUDA_TRY(cudaEventCreate(&ws->ev1));
+        }
+        WM_CUDA_TRY(cudaEventRecord(ws->ev0, st));
+    }
+    const int rc = pick_path(ctx) == 2 ? launch_tc(ctx, ws, a, st) : launch_generic(ctx, a, st);
+    if (ctx->opt_timing && rc == WM_OK) {
+        WM_CUDA_TRY(cudaEventRecord(ws->ev1, st));
+        ws->timed = true;
+    }
+    return rc;
+}
+
+int wm_last_kernel_ms(wm_ctx* ctx, void* cuda_stream, float* ms_out) {
+    if (!ctx || !ms_out) {
+        set_error("wm_last_kernel_ms: null argument");
+        return WM_ERR_ARG;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Workspace* ws = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        for (Workspace* w : ctx->pool)
+            if (w->stream == st) ws = w;
+    }
+    if (!ws || !ws->timed) {
+        set_error("wm_last_kernel_ms: no timed call on this stream (set WM_OPT_TIMING first)");
+        return WM_ERR_ARG;
+    }
+    WM_CUDA_TRY(cudaEventSynchronize(ws->ev1));
+    WM_CUDA_TRY(cudaEventElapsedTime(ms_out, ws->ev0, ws->ev1));
+    return WM_OK;
 }
 
 int wm_topk(const float* scores, const int32_t* subgraph_offsets, int32_t S, int32_t k, int32_t* idx_out,

@@ -58,6 +58,9 @@ struct Workspace {
     // staging for wm_score_topk_host
     void* stage = nullptr;
     size_t stage_cap = 0;
+    // WM_OPT_TIMING
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool timed = false;
 };
 
 constexpr int kHistOff = 0;
@@ -74,6 +77,7 @@ struct wm_ctx {
     int smem_optin = 0;
     int opt_path = 0;     // WM_OPT_PATH
     int opt_sort = 1;     // WM_OPT_SORT
+    int opt_timing = 0;   // WM_OPT_TIMING
     uint32_t* fault = nullptr;   // device fault word
     std::mutex mu;
     std::vector<wm::Workspace*> pool;
@@ -123,6 +127,7 @@ int tc_supported(const wm_ctx* ctx);
 int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 
 // K3 (wm_topk.cu)
+int64_t topk_launches();
 int launch_topk(const float* scores, const int32_t* offsets, int S, int k, int32_t* idx_out, cudaStream_t st);
 
 }  // namespace wm

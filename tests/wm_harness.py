@@ -25,9 +25,9 @@ def weight_file(cfg, weights=None) -> str:
     return path
 
 
-def to_device(batch, per_candidate=False):
+def to_device(batch, per_candidate=False, device="cuda:0"):
     import torch
-    dev = torch.device("cuda:0")
+    dev = torch.device(device)
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     d = dict(init_states=t(batch.init_states), hw_feats=t(batch.hw_feats), action_ids=t(batch.action_ids),
              action_params=t(batch.action_params), lengths=t(batch.lengths),
