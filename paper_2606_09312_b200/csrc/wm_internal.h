@@ -46,6 +46,7 @@ struct Model {
     // descriptors expect, see wm_tc.cu.  nullptr when the path does not apply.
     void* tc_blob = nullptr;
     size_t tc_blob_bytes = 0;
+    void* tc_E = nullptr;      // bf16 [n_types][d_a]
     int tc_ok = 0;
 };
 

@@ -1,11 +1,910 @@
-// K2 tcgen05 path — placeholder until the kernel lands (next commit).
+// K2 (tcgen05): fused persistent rollout + score kernel for the bf16 residual-MLP + LayerNorm models with
+// d = 256, d_a = 128 (BASELINE.json cfg 2 and cfg 4), sm_100a only.
+//
+// PAPER.md:162 Eq.8 / :166 — z_t = F(z_{t-1}, a_t) applied recurrently; :176 — masked steps leave z unchanged;
+// :186-188 Eq.12 — y = G([z_T ; phi ; h]).  Parametrisation: BASELINE.json cfg 2/4.
+//
+// One CTA owns a tile of 128 candidates (length-sorted by K1) for ALL of its steps:
+//   * the fp32 master latent of the tile lives in TMEM columns [0,256) and IS the accumulator of GEMM2: the
+//     residual add is the MMA's accumulate, the epilogue adds b2, applies LayerNorm and writes z' back;
+//   * a bf16 copy of [z ; a] lives in shared memory (K-major, 128B-swizzled 64-column K-blocks) as the A operand
+//     of GEMM1;
+//   * GEMM1 runs in 128-column chunks of the hidden layer into two alternating TMEM accumulators; the GELU
+//     epilogue writes the bf16 hidden chunk back INTO TMEM (over its own fp32 columns) and GEMM2 consumes it as a
+//     TMEM A operand (tcgen05.mma with A in tensor memory), so the hidden activations never touch shared memory;
+//   * weights stream from L2 through a 5-stage ring of 16 KB tiles filled by bulk async copies (TMA engine,
+//     mbarrier complete_tx); the weight image in global memory is pre-tiled, pre-swizzled and laid out in exactly
+//     the order the MMA warp consumes it, so the producer is a linear stream;
+//   * the scorer's two hidden layers run on the same machinery (layer-1 output kept in TMEM as layer-2's A
+//     operand), the last 512->1 layer is a dot product in the epilogue.
+// Warp roles (512 threads): warp 0 tile scheduler + weight producer, warp 1 MMA issuer (one thread), warp 2 TMEM
+// allocator, warps 4-11 epilogue (GELU / LayerNorm / scorer; one thread per row and column half), warps 12-15
+// action embedding (a_t for step t+1 while step t runs; phi and hw at the end of the tile).
+#include <cuda_bf16.h>
+
+#include <cstdio>
+#include <cstring>
+
 #include "wm_internal.h"
 
 namespace wm {
-int tc_prepare(wm_ctx*, const std::vector<std::vector<float>>&, const std::vector<std::string>&) { return WM_OK; }
-int tc_supported(const wm_ctx*) { return 0; }
-int launch_tc(wm_ctx*, Workspace*, const CallArgs&, cudaStream_t) {
-    set_error("tcgen05 path not built");
-    return WM_ERR_UNSUPPORTED;
+
+namespace tc {
+
+constexpr int TM = 128;            // candidates per tile (MMA M)
+constexpr int D = 256;             // latent width
+constexpr int DA = 128;            // action-embedding width
+constexpr int SW = 512;            // scorer hidden width (both hidden layers)
+constexpr int TILE_BYTES = 16384;  // one [128 x 64] bf16 K-block tile, SW128 K-major
+constexpr int NSTAGE = 5;
+constexpr int A1_KB = 7;           // z: 0-3, a/phi: 4-5, hw: 6
+constexpr int THREADS = 512;
+constexpr int EPI_WARP0 = 4, ACT_WARP0 = 12;
+constexpr int MAX_TYPES = 64, MAX_P = 8, MAX_H = 64, MAX_HID = 1024;
+constexpr int SC_TILES = 4 * 7 + 4 * 8;   // scorer stream: layer 1 (4 chunks x 7 tiles), layer 2 (4 x 8)
+
+// barrier indices
+enum {
+    B_FULL = 0,                 // [NSTAGE] producer -> MMA
+    B_EMPTY = B_FULL + NSTAGE,  // [NSTAGE] MMA commit -> producer
+    B_D1FULL = B_EMPTY + NSTAGE,   // [2] MMA commit -> epilogue: accumulator buffer b filled
+    B_HREADY = B_D1FULL + 2,       // [2] epilogue -> MMA: buffer b consumed (bf16 hidden written)
+    B_D2FULL = B_HREADY + 2,       // MMA commit -> epilogue: GEMM2 of the step done
+    B_ZREADY,                      // epilogue -> MMA: z (bf16 smem + fp32 TMEM) written
+    B_AFREE,                       // MMA commit -> action warps: a-part of A1 no longer read
+    B_AREADY,                      // action warps -> MMA: a-part written
+    B_SFULL,                       // [2] scheduler -> consumers
+    B_SEMPTY = B_SFULL + 2,        // [2] consumers -> scheduler
+    B_COUNT = B_SEMPTY + 2
+};
+
+struct Params {
+    // model
+    int hid, nc, n_types, P, H, hw_ksteps;
+    float ln_eps;
+    const uint8_t* blob;        // weight tiles in consumption order
+    const __nv_bfloat16* E;     // [n_types][128]
+    const float *WpT, *bp;      // [P][128], [128]
+    const float *b1, *b2, *gamma, *beta;
+    const float *bs0, *bs1, *w3, *bs2;
+    // call
+    CallArgs a;
+    int n_tiles;
+    int* tile_counter;
+};
+
+struct SmemLayout {
+    uint32_t a1, ring, e_tab, lp, ids, lens, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
+};
+
+__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid) {
+    SmemLayout L;
+    uint32_t o = 0;
+    L.a1 = o; o += A1_KB * TILE_BYTES;
+    L.ring = o; o += NSTAGE * TILE_BYTES;
+    L.e_tab = o; o += (uint32_t)n_types * DA * 2;
+    L.lp = o; o += TM * MAX_P * 4;
+    L.ids = o; o += TM * 4;
+    L.lens = o; o += TM * 4;
+    L.cnt = o; o += TM * (uint32_t)n_types;           // u8 counts, row-major [128][n_types]
+    o = (o + 15) & ~15u;
+    L.b1 = o; o += (uint32_t)hid * 4;
+    L.b2 = o; o += D * 4;
+    L.gamma = o; o += D * 4;
+    L.beta = o; o += D * 4;
+    L.red = o; o += 2 * TM * 8;
+    L.bars = o; o += B_COUNT * 8;
+    L.sched = o; o += 2 * 8;
+    L.tmem_slot = o; o += 16;
+    L.total = o;
+    return L;
 }
+
+// ------------------------------------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// Bounded wait: a protocol bug must trap (and fail the test), never hang the GPU box.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
+    const long long t0 = clock64();
+    while (!mbar_try_wait(bar, parity)) {
+        if (clock64() - t0 > 4000000000LL) {
+            printf("wm_tc: mbarrier wait timed out (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x,
+                   bar, parity);
+            __trap();
+        }
+    }
+}
+__device__ __forceinline__ void fence_barrier_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+__device__ __forceinline__ void tmem_alloc(uint32_t slot_smem, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(slot_smem), "r"(ncols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+
+// D[tmem] (+)= A[smem desc] * B[smem desc]
+__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem desc]
+__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+          "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+          "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
+        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
+        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// bf16x2 pack: lo -> bits [0,16), hi -> bits [16,32)
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+
+// GELU, tanh form (hardware tanh.approx): |gelu_tanh - gelu_erf| <= 5e-4 abs, below the bf16 rounding of the
+// hidden activations it feeds (DESIGN.md §3 S5).
+__device__ __forceinline__ float gelu_fast(float x) {
+    const float x2 = x * x;
+    const float inner = x * fmaf(0.0356774081f, x2, 0.7978845608f);
+    float t;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(inner));
+    const float hx = 0.5f * x;
+    return fmaf(hx, t, hx);
+}
+
+// UMMA shared-memory descriptor, K-major, 128B swizzle, 8-row groups 1024 B apart (SBO), version 1 (sm_100).
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
+    const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | (1u << 16);
+    const uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);
+    return ((uint64_t)hi << 32) | lo;
+}
+// kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N = 128.
+constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+
+}  // namespace tc
+
+namespace tc {
+
+__device__ __forceinline__ int find_seg(const int32_t* __restrict__ off, int S, int cand) {
+    int lo = 0, hi = S;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(off + mid) <= cand) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// Row metadata of tile row r: candidate index (-1 = dead row), clamped length, subgraph (z0 / hw row).
+__device__ __forceinline__ void row_meta(const CallArgs& a, int tile, int r, int& cand, int& len, int& seg,
+                                         bool report) {
+    const int64_t i = (int64_t)tile * TM + r;
+    cand = -1; len = 0; seg = 0;
+    if (i < a.B) {
+        cand = a.perm ? __ldg(a.perm + i) : (int)i;
+        len = __ldg(a.lengths + cand);
+        if (len < 0 || len > a.T_max) {
+            if (report) atomicOr(a.fault, WM_FAULT_LEN);
+            len = len < 0 ? 0 : a.T_max;
+        }
+        seg = a.offsets ? find_seg(a.offsets, a.S, cand) : cand;
+    }
+}
+
+// byte offset of the 16-byte chunk `chunk` (8 bf16 columns) of row `row` inside a SW128 K-major K-block tile
+__device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
+    return (uint32_t)row * 128u + (uint32_t)((chunk ^ (row & 7)) << 4);
+}
+
+__global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const SmemLayout L = smem_layout(p.n_types, p.hid);
+    const uint32_t s_base = smem_u32(smem);
+    const uint32_t s_a1 = s_base + L.a1, s_ring = s_base + L.ring, s_bars = s_base + L.bars;
+    auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
+    volatile int* s_sched = reinterpret_cast<volatile int*>(smem + L.sched);   // [2][2]: tile, nsteps
+    float* s_b1 = reinterpret_cast<float*>(smem + L.b1);
+    float* s_b2 = reinterpret_cast<float*>(smem + L.b2);
+    float* s_gamma = reinterpret_cast<float*>(smem + L.gamma);
+    float* s_beta = reinterpret_cast<float*>(smem + L.beta);
+    float2* s_red = reinterpret_cast<float2*>(smem + L.red);                  // [2][128]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int NC = p.nc;
+    const int ROLL_TILES = NC * 10;
+
+    // ---- one-time setup
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NSTAGE; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 1); }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(bar(B_D1FULL + i), 1);
+            mbar_init(bar(B_HREADY + i), 8);
+            mbar_init(bar(B_SFULL + i), 1);
+            mbar_init(bar(B_SEMPTY + i), 13);
+        }
+        mbar_init(bar(B_D2FULL), 1);
+        mbar_init(bar(B_ZREADY), 8);
+        mbar_init(bar(B_AFREE), 1);
+        mbar_init(bar(B_AREADY), 4);
+        fence_barrier_init();
+        fence_proxy_async();
+    }
+    if (warp == 2) tmem_alloc(s_base + L.tmem_slot, 512);
+    for (int i = threadIdx.x; i < p.hid; i += THREADS) s_b1[i] = __ldg(p.b1 + i);
+    for (int i = threadIdx.x; i < D; i += THREADS) {
+        s_b2[i] = __ldg(p.b2 + i);
+        s_gamma[i] = __ldg(p.gamma + i);
+        s_beta[i] = __ldg(p.beta + i);
+    }
+    {
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(p.E);
+        uint32_t* dst = reinterpret_cast<uint32_t*>(smem + L.e_tab);
+        for (int i = threadIdx.x; i < p.n_types * DA / 2; i += THREADS) dst[i] = __ldg(src + i);
+        // the hw K-block is only ever written in its first columns: clear it once so unread bytes are not NaNs
+        uint32_t* hwk = reinterpret_cast<uint32_t*>(smem + L.a1 + 6 * TILE_BYTES);
+        for (int i = threadIdx.x; i < TILE_BYTES / 4; i += THREADS) hwk[i] = 0u;
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem + L.tmem_slot);
+    const uint32_t T_Z = tmem_base;                 // fp32 latent / GEMM2 accumulator, 256 columns
+    const uint32_t T_D1 = tmem_base + 256;          // two 128-column GEMM1 accumulators
+
+    if (warp == 0) {
+        // =============================================================== scheduler + weight producer
+        uint32_t stage = 0, ph = 0;
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            int tile = 0;
+            if (lane == 0) tile = atomicAdd(p.tile_counter, 1);
+            tile = __shfl_sync(0xffffffffu, tile, 0);
+            int nsteps = 0;
+            if (tile < p.n_tiles) {
+                for (int r = lane; r < TM; r += 32) {
+                    int cand, len, seg;
+                    row_meta(p.a, tile, r, cand, len, seg, true);
+                    nsteps = max(nsteps, len);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) nsteps = max(nsteps, __shfl_xor_sync(0xffffffffu, nsteps, o));
+            } else {
+                tile = -1;
+            }
+            if (lane == 0) {
+                mbar_wait(bar(B_SEMPTY + slot), ((it >> 1) & 1) ^ 1);
+                s_sched[slot * 2 + 0] = tile;
+                s_sched[slot * 2 + 1] = nsteps;
+                mbar_arrive(bar(B_SFULL + slot));   // release semantics order the two stores before it
+            }
+            if (tile < 0) break;
+            if (lane == 0) {
+                const int roll_total = nsteps * ROLL_TILES, total = roll_total + SC_TILES;
+                for (int i = 0; i < total; ++i) {
+                    const int src_tile = i < roll_total ? i % ROLL_TILES : ROLL_TILES + (i - roll_total);
+                    mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
+                    mbar_arrive_expect_tx(bar(B_FULL + stage), TILE_BYTES);
+                    bulk_g2s(s_ring + stage * TILE_BYTES, p.blob + (size_t)src_tile * TILE_BYTES, TILE_BYTES,
+                             bar(B_FULL + stage));
+                    if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+                }
+            }
+            __syncwarp();
+        }
+    } else if (warp == 1) {
+        // =============================================================== MMA issuer (one thread)
+        if (lane == 0) {
+            uint32_t stage = 0, ph = 0;
+            uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
+            bool pend[2] = {false, false};
+            auto wait_h = [&](int b) {
+                if (pend[b]) {
+                    mbar_wait(bar(B_HREADY + b), n_h[b] & 1);
+                    ++n_h[b];
+                    pend[b] = false;
+                    tc_fence_after();
+                }
+            };
+            // one ring stage = one [128 x 64] B tile = `ksteps` MMAs of K = 16
+            auto stage_ss = [&](uint32_t d_tmem, uint32_t a_tile, int ksteps, bool first) {
+                mbar_wait(bar(B_FULL + stage), ph);
+                tc_fence_after();
+                const uint64_t ad = smem_desc(a_tile), bd = smem_desc(s_ring + stage * TILE_BYTES);
+                for (int j = 0; j < ksteps; ++j)
+                    mma_ss(d_tmem, ad + 2u * j, bd + 2u * j, IDESC, (first && j == 0) ? 0u : 1u);
+                mma_commit(bar(B_EMPTY + stage));
+                if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+            };
+            auto stage_ts = [&](uint32_t d_tmem, uint32_t a_tmem, bool first) {
+                mbar_wait(bar(B_FULL + stage), ph);
+                tc_fence_after();
+                const uint64_t bd = smem_desc(s_ring + stage * TILE_BYTES);
+                for (int j = 0; j < 4; ++j) mma_ts(d_tmem, a_tmem + 8u * j, bd + 2u * j, IDESC, (first && j == 0) ? 0u : 1u);
+                mma_commit(bar(B_EMPTY + stage));
+                if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+            };
+            // GEMM over the A1 K-blocks in the order a/phi (4,5), [hw (6)], z (0..3); waits for the operands of
+            // the first chunk of a step / of the scorer.
+            auto gemm_a1 = [&](int b, bool first_chunk, bool with_hw) {
+                wait_h(b);
+                const uint32_t d = T_D1 + 128u * b;
+                if (first_chunk) { mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
+                stage_ss(d, s_a1 + 4 * TILE_BYTES, 4, true);
+                stage_ss(d, s_a1 + 5 * TILE_BYTES, 4, false);
+                if (with_hw) stage_ss(d, s_a1 + 6 * TILE_BYTES, p.hw_ksteps, false);
+                if (first_chunk) { mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
+                for (int kb = 0; kb < 4; ++kb) stage_ss(d, s_a1 + kb * TILE_BYTES, 4, false);
+                mma_commit(bar(B_D1FULL + b));
+                pend[b] = true;
+            };
+            for (uint32_t it = 0;; ++it) {
+                const uint32_t slot = it & 1;
+                mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+                const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+                mbar_arrive(bar(B_SEMPTY + slot));
+                if (tile < 0) break;
+                for (int t = 0; t < nsteps; ++t) {
+                    for (int i = 0; i <= NC; ++i) {
+                        if (i < NC) {
+                            gemm_a1(i & 1, i == 0, false);                       // GEMM1 chunk i
+                            if (i == NC - 1) mma_commit(bar(B_AFREE));
+                        }
+                        if (i >= 1) {                                            // GEMM2 chunk i-1 (A from TMEM)
+                            const int c = i - 1, b = c & 1;
+                            wait_h(b);
+                            const uint32_t hbuf = T_D1 + 128u * b;
+                            for (int ks = 0; ks < 2; ++ks)
+                                for (int h = 0; h < 2; ++h) stage_ts(T_Z + 128u * h, hbuf + 64u * ks, false);
+                            if (c == NC - 1) mma_commit(bar(B_D2FULL));
+                        }
+                    }
+                }
+                // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
+                for (int c = 0; c < 4; ++c) {
+                    gemm_a1(c & 1, c == 0, true);
+                    if (c == 3) mma_commit(bar(B_AFREE));
+                }
+                wait_h(0);
+                wait_h(1);   // all of H1 (bf16, TMEM columns [0,256)) written
+                // ---- scorer layer 2: A = H1 from TMEM, K = 512
+                for (int c = 0; c < 4; ++c) {
+                    const int b = c & 1;
+                    wait_h(b);
+                    for (int kb = 0; kb < 8; ++kb) stage_ts(T_D1 + 128u * b, T_Z + 32u * kb, kb == 0);
+                    mma_commit(bar(B_D1FULL + b));
+                    pend[b] = true;
+                }
+            }
+        }
+        __syncwarp();
+    }
+    else if (warp >= EPI_WARP0 && warp < ACT_WARP0) {
+        // =============================================================== epilogue warps (GELU / LayerNorm / scorer)
+        const int q = warp & 3, hh = (warp - EPI_WARP0) >> 2;
+        const int row = 32 * q + lane;
+        const uint32_t lane_off = (uint32_t)(32 * q) << 16;
+        uint8_t* a1 = smem + L.a1;
+        uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
+        const float inv_d = 1.0f / (float)D;
+        // write 32 consecutive z columns of this row: fp32 -> TMEM, bf16 -> A1 (when `to_smem`)
+        auto put_z = [&](int col0, const uint32_t (&v)[32], bool to_smem) {
+            tmem_st32(T_Z + lane_off + (uint32_t)col0, v);
+            if (to_smem) {
+                uint8_t* kb = a1 + (col0 >> 6) * TILE_BYTES;
+                const int chunk0 = (col0 & 63) >> 3;
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
+                    uint4 o;
+                    o.x = pack_bf16(__uint_as_float(v[8 * ch + 0]), __uint_as_float(v[8 * ch + 1]));
+                    o.y = pack_bf16(__uint_as_float(v[8 * ch + 2]), __uint_as_float(v[8 * ch + 3]));
+                    o.z = pack_bf16(__uint_as_float(v[8 * ch + 4]), __uint_as_float(v[8 * ch + 5]));
+                    o.w = pack_bf16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
+                    *reinterpret_cast<uint4*>(kb + sw128_off(row, chunk0 + ch)) = o;
+                }
+            }
+        };
+        auto publish = [&](int barrier, bool smem_written) {
+            tmem_st_wait();
+            if (smem_written) fence_proxy_async();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(barrier));
+        };
+        // bias + GELU over this thread's 64 columns of accumulator buffer b, bf16 result to TMEM at dst_col
+        auto gelu_chunk = [&](int b, const float* bias, bool bias_in_smem, uint32_t dst_col) {
+            mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+            ++n_d1[b];
+            tc_fence_after();
+#pragma unroll
+            for (int p2 = 0; p2 < 2; ++p2) {
+                uint32_t v[32], o[16];
+                tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u * p2, v);
+                tmem_ld_wait();
+                const float* bp_ = bias + 32 * p2;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const float b0 = bias_in_smem ? bp_[2 * i] : __ldg(bp_ + 2 * i);
+                    const float b1v = bias_in_smem ? bp_[2 * i + 1] : __ldg(bp_ + 2 * i + 1);
+                    o[i] = pack_bf16(gelu_fast(__uint_as_float(v[2 * i]) + b0),
+                                     gelu_fast(__uint_as_float(v[2 * i + 1]) + b1v));
+                }
+                tmem_st16(dst_col + lane_off + 16u * p2, o);
+            }
+            publish(B_HREADY + b, false);
+        };
+
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand, len, seg;
+            row_meta(p.a, tile, row, cand, len, seg, false);
+
+            // ---- z_0 (the task's initial latent)
+#pragma unroll 1
+            for (int p4 = 0; p4 < 4; ++p4) {
+                const int col0 = 128 * hh + 32 * p4;
+                uint32_t v[32];
+                if (cand >= 0) {
+                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + col0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 f = __ldg(src + i);
+                        v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
+                        v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) v[i] = 0u;
+                }
+                put_z(col0, v, true);
+            }
+            publish(B_ZREADY, true);
+
+            for (int t = 0; t < nsteps; ++t) {
+                for (int c = 0; c < NC; ++c)
+                    gelu_chunk(c & 1, s_b1 + c * 128 + 64 * hh, true, T_D1 + 128u * (c & 1) + 64u * hh);
+                // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
+                mbar_wait(bar(B_D2FULL), n_d2 & 1);
+                ++n_d2;
+                tc_fence_after();
+                float s1 = 0.0f, s2 = 0.0f;
+#pragma unroll 1
+                for (int p4 = 0; p4 < 4; ++p4) {
+                    const int col0 = 128 * hh + 32 * p4;
+                    uint32_t v[32];
+                    tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        const float x = __uint_as_float(v[i]) + s_b2[col0 + i];
+                        s1 += x;
+                        s2 = fmaf(x, x, s2);
+                    }
+                }
+                s_red[hh * TM + row] = make_float2(s1, s2);
+                named_bar_sync(1 + q, 64);
+                const float2 other = s_red[(hh ^ 1) * TM + row];
+                const float mean = (s1 + other.x) * inv_d;
+                const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
+                const float rstd = rsqrtf(var + p.ln_eps);
+                const bool live = t < len;     // masked steps leave the state unchanged
+#pragma unroll 1
+                for (int p4 = 0; p4 < 4; ++p4) {
+                    const int col0 = 128 * hh + 32 * p4;
+                    uint32_t v[32];
+                    tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        const float x = __uint_as_float(v[i]) + s_b2[col0 + i];
+                        v[i] = __float_as_uint(fmaf((x - mean) * rstd, s_gamma[col0 + i], s_beta[col0 + i]));
+                    }
+                    // frozen rows: the bf16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
+                    // fp32 master is never read again
+                    put_z(col0, v, live);
+                }
+                publish(B_ZREADY, true);
+            }
+
+            // ---- scorer layer 1 -> H1 (bf16) in TMEM columns [0,256)
+            for (int c = 0; c < 4; ++c)
+                gelu_chunk(c & 1, p.bs0 + c * 128 + 64 * hh, false, T_Z + 64u * c + 32u * hh);
+            // ---- scorer layer 2 + output dot product
+            float part = 0.0f;
+            for (int c = 0; c < 4; ++c) {
+                const int b = c & 1;
+                mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+                ++n_d1[b];
+                tc_fence_after();
+#pragma unroll
+                for (int p2 = 0; p2 < 2; ++p2) {
+                    uint32_t v[32];
+                    tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u * p2, v);
+                    tmem_ld_wait();
+                    const int n0 = c * 128 + 64 * hh + 32 * p2;
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        part = fmaf(gelu_fast(__uint_as_float(v[i]) + __ldg(p.bs1 + n0 + i)), __ldg(p.w3 + n0 + i), part);
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_HREADY + b));
+            }
+            s_red[hh * TM + row] = make_float2(part, 0.0f);
+            named_bar_sync(1 + q, 64);
+            if (hh == 0 && cand >= 0) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
+            named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
+        }
+    } else if (warp >= ACT_WARP0) {
+        // =============================================================== action-embedding warps
+        const int aw = warp - ACT_WARP0;
+        const int row = 32 * aw + lane;       // row-mapped phases
+        const int col4 = 4 * lane;            // column-mapped phases: this lane's 4 embedding columns
+        uint8_t* a1 = smem + L.a1;
+        const uint8_t* s_E = smem + L.e_tab;
+        float* s_lp = reinterpret_cast<float*>(smem + L.lp);
+        int* s_ids = reinterpret_cast<int*>(smem + L.ids);
+        int* s_lens = reinterpret_cast<int*>(smem + L.lens);
+        uint8_t* s_cnt = smem + L.cnt;
+        const int P = p.P, NT = p.n_types;
+        float wp[MAX_P][4], bp4[4];
+#pragma unroll
+        for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) wp[j][e] = j < P ? __ldg(p.WpT + j * DA + col4 + e) : 0.0f;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) bp4[e] = __ldg(p.bp + col4 + e);
+        uint32_t n_w = 0;
+        // A1 destination of this lane's 4 columns (8 bytes) in row r: K-block 4 + lane/16
+        auto a_dst = [&](int r) -> uint2* {
+            return reinterpret_cast<uint2*>(a1 + (4 + (lane >> 4)) * TILE_BYTES + sw128_off(r, (lane & 15) >> 1) +
+                                            (lane & 1) * 8);
+        };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand, len, seg;
+            row_meta(p.a, tile, row, cand, len, seg, false);
+            for (int c = 0; c < NT; ++c) s_cnt[row * NT + c] = 0;
+            float slp[MAX_P];
+#pragma unroll
+            for (int j = 0; j < MAX_P; ++j) slp[j] = 0.0f;
+            uint2 pk[32];
+
+            for (int t = 0; t < nsteps; ++t) {
+                // phase 1 (one row per lane): read the step's action, log2 of its parameters, phi statistics
+                int id = -1;
+                float lp[MAX_P];
+#pragma unroll
+                for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                if (t < len) {
+                    id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
+                    if (id < 0 || id >= NT) {
+                        atomicOr(p.a.fault, WM_FAULT_TYPE);
+                        id = id < 0 ? 0 : NT - 1;
+                    }
+                    const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j) {
+                        if (j < P) {
+                            int prm = __ldg(pp + j);
+                            if (prm < 1) {
+                                atomicOr(p.a.fault, WM_FAULT_PARAM);
+                                prm = 1;
+                            }
+                            lp[j] = log2f((float)prm);
+                            slp[j] += lp[j];
+                        }
+                    }
+                    s_cnt[row * NT + id] += 1;
+                }
+                s_ids[row] = id;
+                *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
+                *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
+                __syncwarp();
+                // phase 2 (4 columns per lane, loop over the warp's 32 rows): a = E[id] + W_p log2(p) + b_p
+#pragma unroll
+                for (int rr = 0; rr < 32; ++rr) {
+                    const int r = 32 * aw + rr;
+                    const int idr = s_ids[r];
+                    float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+                    if (idr >= 0) {
+                        const uint2 e = *reinterpret_cast<const uint2*>(s_E + ((size_t)idr * DA + col4) * 2);
+                        a4[0] = __uint_as_float(e.x << 16) + bp4[0];
+                        a4[1] = __uint_as_float(e.x & 0xffff0000u) + bp4[1];
+                        a4[2] = __uint_as_float(e.y << 16) + bp4[2];
+                        a4[3] = __uint_as_float(e.y & 0xffff0000u) + bp4[3];
+                        const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
+                        const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
+                        const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+                            for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
+                    }
+                    pk[rr] = make_uint2(pack_bf16(a4[0], a4[1]), pack_bf16(a4[2], a4[3]));
+                }
+                __syncwarp();
+                // store once GEMM1 of the previous step no longer reads the a-part
+                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+                ++n_w;
+#pragma unroll
+                for (int rr = 0; rr < 32; ++rr) *a_dst(32 * aw + rr) = pk[rr];
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(B_AREADY));
+            }
+
+            // ---- phi = mean_t a_t = (sum_c count_c E[c] + W_p sum_t log2 p_t) / len + b_p   (0 when len = 0)
+            s_lens[row] = len;
+            *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(slp[0], slp[1], slp[2], slp[3]);
+            *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(slp[4], slp[5], slp[6], slp[7]);
+            __syncwarp();
+#pragma unroll
+            for (int rr = 0; rr < 32; ++rr) {
+                const int r = 32 * aw + rr;
+                const int lr_ = s_lens[r];
+                float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+                if (lr_ > 0) {
+                    for (int c = 0; c < NT; ++c) {
+                        const float cn = (float)s_cnt[r * NT + c];
+                        const uint2 e = *reinterpret_cast<const uint2*>(s_E + ((size_t)c * DA + col4) * 2);
+                        a4[0] = fmaf(cn, __uint_as_float(e.x << 16), a4[0]);
+                        a4[1] = fmaf(cn, __uint_as_float(e.x & 0xffff0000u), a4[1]);
+                        a4[2] = fmaf(cn, __uint_as_float(e.y << 16), a4[2]);
+                        a4[3] = fmaf(cn, __uint_as_float(e.y & 0xffff0000u), a4[3]);
+                    }
+                    const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
+                    const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
+                    const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+                        for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
+                    const float inv = 1.0f / (float)lr_;
+#pragma unroll
+                    for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(a4[e2], inv, bp4[e2]);
+                }
+                pk[rr] = make_uint2(pack_bf16(a4[0], a4[1]), pack_bf16(a4[2], a4[3]));
+            }
+            __syncwarp();
+            if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+            ++n_w;
+#pragma unroll
+            for (int rr = 0; rr < 32; ++rr) *a_dst(32 * aw + rr) = pk[rr];
+            // hardware features of this row -> K-block 6 (columns >= H stay zero)
+            for (int ch = 0; ch < p.H / 8; ++ch) {
+                uint4 o = make_uint4(0u, 0u, 0u, 0u);
+                if (cand >= 0) {
+                    const float4* src = reinterpret_cast<const float4*>(p.a.hw_feats + (size_t)seg * p.H + 8 * ch);
+                    const float4 f0 = __ldg(src), f1 = __ldg(src + 1);
+                    o.x = pack_bf16(f0.x, f0.y); o.y = pack_bf16(f0.z, f0.w);
+                    o.z = pack_bf16(f1.x, f1.y); o.w = pack_bf16(f1.z, f1.w);
+                }
+                *reinterpret_cast<uint4*>(a1 + 6 * TILE_BYTES + sw128_off(row, ch)) = o;
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_AREADY));
+        }
+    }
+
+    // ---- teardown
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc(tmem_base, 512);
+}
+
+}  // namespace tc
+
+// ------------------------------------------------------------------------------------------------ host side
+namespace {
+
+uint16_t f32_to_bf16(float f) {
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    u += 0x7FFFu + ((u >> 16) & 1u);   // round to nearest even (the stored values are already bf16-exact)
+    return (uint16_t)(u >> 16);
+}
+
+// Append the [128 x 64] tile W[n0 + n][k0 + k] (k < kvalid, else 0) in the SW128 K-major shared-memory image.
+void append_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid) {
+    const size_t base = blob.size();
+    blob.resize(base + tc::TILE_BYTES / 2, 0);
+    for (int n = 0; n < 128; ++n)
+        for (int k = 0; k < 64; ++k) {
+            const float v = k < kvalid ? W[(size_t)(n0 + n) * ld + k0 + k] : 0.0f;
+            const size_t off = (size_t)n * 128 + (size_t)((((k >> 3) ^ (n & 7)) << 4)) + (size_t)(k & 7) * 2;
+            blob[base + off / 2] = f32_to_bf16(v);
+        }
+}
+
+struct TcState {
+    tc::Params p;
+};
+
+}  // namespace
+
+static bool tc_model_ok(const Model& m) {
+    return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc::D &&
+           m.d_a == tc::DA && m.hidden >= 256 && m.hidden <= tc::MAX_HID && m.hidden % 128 == 0 && m.n_lin == 3 &&
+           m.sdim[1] == tc::SW && m.sdim[2] == tc::SW && m.H >= 8 && m.H <= tc::MAX_H && m.H % 8 == 0 &&
+           m.n_types <= tc::MAX_TYPES && m.P <= tc::MAX_P;
+}
+
+int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
+    Model& m = ctx->m;
+    m.tc_ok = 0;
+    if (!tc_model_ok(m)) return WM_OK;
+    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden);
+    if ((int)L.total > ctx->smem_optin) return WM_OK;
+    auto get = [&](const char* n) -> const std::vector<float>& {
+        for (size_t i = 0; i < names.size(); ++i)
+            if (names[i] == n) return hv[i];
+        static const std::vector<float> empty;
+        return empty;
+    };
+    const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1"), &E = get("E");
+    const int hid = m.hidden, NC = hid / 128, K1 = tc::D + tc::DA, K0 = K1 + m.H;
+    std::vector<uint16_t> blob;
+    blob.reserve((size_t)(NC * 10 + tc::SC_TILES) * tc::TILE_BYTES / 2);
+    auto g1 = [&](int c) {   // GEMM1 chunk c: K-blocks a (4,5) then z (0..3)
+        const int order[6] = {4, 5, 0, 1, 2, 3};
+        for (int i = 0; i < 6; ++i) append_tile(blob, W1, K1, c * 128, order[i] * 64, 64);
+    };
+    auto g2 = [&](int c) {   // GEMM2 chunk c: K halves of the hidden chunk x N halves of d
+        for (int ks = 0; ks < 2; ++ks)
+            for (int h = 0; h < 2; ++h) append_tile(blob, W2, hid, h * 128, c * 128 + ks * 64, 64);
+    };
+    for (int i = 0; i <= NC; ++i) {   // same interleave as the MMA warp: G1(i), then G2(i-1)
+        if (i < NC) g1(i);
+        if (i >= 1) g2(i - 1);
+    }
+    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw (1), z (4)
+        append_tile(blob, Ws0, K0, c * 128, tc::D, 64);
+        append_tile(blob, Ws0, K0, c * 128, tc::D + 64, 64);
+        append_tile(blob, Ws0, K0, c * 128, K1, m.H);
+        for (int kb = 0; kb < 4; ++kb) append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
+    }
+    for (int c = 0; c < 4; ++c)       // scorer layer 2
+        for (int kb = 0; kb < 8; ++kb) append_tile(blob, Ws1, tc::SW, c * 128, kb * 64, 64);
+
+    void* d_blob = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&d_blob, blob.size() * 2));
+    ctx->allocs.push_back(d_blob);
+    WM_CUDA_TRY(cudaMemcpy(d_blob, blob.data(), blob.size() * 2, cudaMemcpyHostToDevice));
+    std::vector<uint16_t> e16(E.size());
+    for (size_t i = 0; i < E.size(); ++i) e16[i] = f32_to_bf16(E[i]);
+    void* d_e = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&d_e, e16.size() * 2 + 16));
+    ctx->allocs.push_back(d_e);
+    WM_CUDA_TRY(cudaMemcpy(d_e, e16.data(), e16.size() * 2, cudaMemcpyHostToDevice));
+    m.tc_blob = d_blob;
+    m.tc_blob_bytes = blob.size() * 2;
+    m.tc_E = d_e;
+    WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    m.tc_ok = 1;
+    return WM_OK;
+}
+
+int tc_supported(const wm_ctx* ctx) { return ctx->m.tc_ok; }
+
+int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
+    const Model& m = ctx->m;
+    // per-call conditions the kernel relies on; otherwise the fp32 kernel takes the call
+    const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0);
+    if (!m.tc_ok || a.T_max > 255 || !aligned) {
+        if (ctx->opt_path == 2) {
+            set_error("tcgen05 path: needs T_max <= 255 and 16-byte aligned init_states / hw_feats");
+            return WM_ERR_UNSUPPORTED;
+        }
+        return launch_generic(ctx, a, st);
+    }
+    tc::Params p;
+    p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
+    p.hw_ksteps = (m.H + 15) / 16;
+    p.ln_eps = m.ln_eps;
+    p.blob = static_cast<const uint8_t*>(m.tc_blob);
+    p.E = static_cast<const __nv_bfloat16*>(m.tc_E);
+    p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
+    p.a = a;
+    p.n_tiles = (int)((a.B + tc::TM - 1) / tc::TM);
+    p.tile_counter = ws->counters + kTileCtrOff;
+    WM_CUDA_TRY(cudaMemsetAsync(p.tile_counter, 0, sizeof(int), st));
+    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden);
+    const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
+    tc::wm_tc_kernel<<<grid, tc::THREADS, L.total, st>>>(p);
+    WM_CUDA_TRY(cudaGetLastError());
+    ctx->launches.fetch_add(1);
+    return WM_OK;
+}
+
 }  // namespace wm
