@@ -18,6 +18,8 @@ SOURCES = ["wm_api.cu", "wm_bucket.cu", "wm_generic.cu", "wm_tc.cu", "wm_topk.cu
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+if os.environ.get("WM_TC_PROFILE"):   # dev instrumentation of wm_tc.cu (per-role wait-cycle counters)
+    FLAGS.append("-DWM_TC_PROFILE")
 
 
 def _stale() -> bool:

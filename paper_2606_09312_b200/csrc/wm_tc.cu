@@ -258,6 +258,20 @@ __device__ __forceinline__ float gelu_fast(float x) {
     return fmaf(hx, t, hx);
 }
 
+// Two GELUs at once on the packed fp32x2 pipe (FFMA2/FMUL2/FADD2 halve the epilogue's FP instruction count).
+__device__ __forceinline__ uint32_t gelu2_bf16(float2 acc, float2 bias) {
+    const float2 x = __fadd2_rn(acc, bias);
+    const float2 hx = __fmul2_rn(x, make_float2(0.5f, 0.5f));
+    const float2 x2 = __fmul2_rn(x, x);
+    const float2 pin = __ffma2_rn(x2, make_float2(0.0356774081f, 0.0356774081f), make_float2(0.7978845608f, 0.7978845608f));
+    const float2 inner = __fmul2_rn(x, pin);
+    float2 t;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t.x) : "f"(inner.x));
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t.y) : "f"(inner.y));
+    const float2 g = __ffma2_rn(hx, t, hx);
+    return pack_bf16(g.x, g.y);
+}
+
 // UMMA shared-memory descriptor, K-major, 128B swizzle, 8-row groups 1024 B apart (SBO), version 1 (sm_100).
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
     const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | (1u << 16);
@@ -589,13 +603,14 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 uint32_t v[32], o[16];
                 tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u * p2, v);
                 tmem_ld_wait();
-                const float* bp_ = bias + 32 * p2;
+                const float4* bp_ = reinterpret_cast<const float4*>(bias + 32 * p2);
 #pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    const float b0 = bias_in_smem ? bp_[2 * i] : __ldg(bp_ + 2 * i);
-                    const float b1v = bias_in_smem ? bp_[2 * i + 1] : __ldg(bp_ + 2 * i + 1);
-                    o[i] = pack_bf16(gelu_fast(__uint_as_float(v[2 * i]) + b0),
-                                     gelu_fast(__uint_as_float(v[2 * i + 1]) + b1v));
+                for (int i = 0; i < 8; ++i) {
+                    const float4 bv = bias_in_smem ? bp_[i] : __ldg(bp_ + i);
+                    o[2 * i] = gelu2_bf16(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                          make_float2(bv.x, bv.y));
+                    o[2 * i + 1] = gelu2_bf16(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                              make_float2(bv.z, bv.w));
                 }
                 tmem_st16(dst_col + lane_off + 16u * p2, o);
             }
@@ -640,20 +655,27 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 mbar_wait_t(bar(B_D2FULL), n_d2 & 1, eprof ? &ef[1] : nullptr);
                 ++n_d2;
                 tc_fence_after();
-                float s1 = 0.0f, s2 = 0.0f;
+                float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
 #pragma unroll 1
                 for (int p4 = 0; p4 < 4; ++p4) {
                     const int col0 = 128 * hh + 32 * p4;
                     uint32_t v[32];
                     tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
                     tmem_ld_wait();
+                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        const float x = __uint_as_float(v[i]) + s_b2[col0 + i];
-                        s1 += x;
-                        s2 = fmaf(x, x, s2);
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 bb = b2v[i];
+                        const float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                                     make_float2(bb.x, bb.y));
+                        const float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                                     make_float2(bb.z, bb.w));
+                        s1v = __fadd2_rn(s1v, __fadd2_rn(x0, x1));
+                        s2v = __ffma2_rn(x0, x0, s2v);
+                        s2v = __ffma2_rn(x1, x1, s2v);
                     }
                 }
+                const float s1 = s1v.x + s1v.y, s2 = s2v.x + s2v.y;
                 s_red[hh * TM + row] = make_float2(s1, s2);
                 named_bar_sync(1 + q, 64);
                 const float2 other = s_red[(hh ^ 1) * TM + row];
@@ -667,10 +689,21 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     uint32_t v[32];
                     tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
                     tmem_ld_wait();
+                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
+                    const float4* gv = reinterpret_cast<const float4*>(s_gamma + col0);
+                    const float4* bev = reinterpret_cast<const float4*>(s_beta + col0);
+                    const float2 rs2 = make_float2(rstd, rstd), mr2 = make_float2(-mean * rstd, -mean * rstd);
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) {
-                        const float x = __uint_as_float(v[i]) + s_b2[col0 + i];
-                        v[i] = __float_as_uint(fmaf((x - mean) * rstd, s_gamma[col0 + i], s_beta[col0 + i]));
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 bb = b2v[i], gg = gv[i], be = bev[i];
+                        float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                               make_float2(bb.x, bb.y));
+                        float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                               make_float2(bb.z, bb.w));
+                        x0 = __ffma2_rn(__ffma2_rn(x0, rs2, mr2), make_float2(gg.x, gg.y), make_float2(be.x, be.y));
+                        x1 = __ffma2_rn(__ffma2_rn(x1, rs2, mr2), make_float2(gg.z, gg.w), make_float2(be.z, be.w));
+                        v[4 * i] = __float_as_uint(x0.x); v[4 * i + 1] = __float_as_uint(x0.y);
+                        v[4 * i + 2] = __float_as_uint(x1.x); v[4 * i + 3] = __float_as_uint(x1.y);
                     }
                     // frozen rows: the bf16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
                     // fp32 master is never read again
