@@ -74,7 +74,7 @@ struct Params {
     CallArgs a;
     int n_tiles;
     int* tile_counter;
-    unsigned long long* prof;   // dev instrumentation (WM_TC_PROF=1): per-CTA wait-cycle counters, else nullptr
+    unsigned long long* prof;   // dev instrumentation trace buffer (WM_TC_PROFILE builds), else nullptr
 };
 
 struct SmemLayout {
@@ -141,18 +141,21 @@ __device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (!mbar_try_wait(bar, parity)) mbar_wait_slow(bar, parity);
 }
-// wait and add the cycles spent to *acc (dev instrumentation, compiled in with -DWM_TC_PROFILE)
-__device__ __forceinline__ void mbar_wait_t(uint32_t bar, uint32_t parity, unsigned long long* acc) {
+// Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of CTA 0 appends
+// (tag, clock) records to a trace buffer that launch_tc dumps.  Compiled out otherwise.
 #ifdef WM_TC_PROFILE
-    if (acc) {
-        const long long t0 = clock64();
-        mbar_wait(bar, parity);
-        *acc += (unsigned long long)(clock64() - t0);
-        return;
-    }
+#define WM_TRACE_DECL(role, cond)                                                                       \
+    uint2* tr_buf = p.prof ? reinterpret_cast<uint2*>(p.prof) + (role) * 8192 : nullptr;                 \
+    const bool tr_on = tr_buf != nullptr && blockIdx.x == 0 && lane == 0 && (cond);                     \
+    uint32_t tr_n = 0;
+#define WM_TRACE(tag)                                                                                   \
+    do {                                                                                                \
+        if (tr_on && tr_n < 8191) { tr_buf[1 + tr_n] = make_uint2((uint32_t)(tag), (uint32_t)clock64()); ++tr_n; tr_buf[0].x = tr_n; } \
+    } while (0)
+#else
+#define WM_TRACE_DECL(role, cond)
+#define WM_TRACE(tag) do { } while (0)
 #endif
-    mbar_wait(bar, parity);
-}
 __device__ __forceinline__ void fence_barrier_init() {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
@@ -412,53 +415,50 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         }
     } else if (warp == MMA_WARP) {
         // =============================================================== MMA issuer (converged warp, one elected lane)
+        // tcgen05.mma dispatch occupies the issuing warp for the MMA's duration, so every other instruction this
+        // warp executes is tensor-pipe idle time: waits are batched (one warp-wide try_wait covers the full
+        // barriers of up to two ring stages, one lane per barrier) and the issue loops stay rolled and small.
         {
             uint32_t stage = 0, ph = 0;
             uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
             bool pend[2] = {false, false};
-            unsigned long long pf[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // full, h, a, z, total
-            unsigned long long ps[4] = {0, 0, 0, 0};                // cycles inside SS / TS issue blocks, fence, gaps
-            long long t_last = clock64();
-#ifdef WM_TC_PROFILE
-            const bool prof = p.prof != nullptr;
-#else
-            constexpr bool prof = false;
-#endif
-            const long long t_begin = clock64();
+            WM_TRACE_DECL(0, true)
             auto wait_h = [&](int b) {
                 if (pend[b]) {
-                    mbar_wait_t(bar(B_HREADY + b), n_h[b] & 1, prof ? &pf[1] : nullptr);
+                    WM_TRACE(10 + b);
+                    mbar_wait(bar(B_HREADY + b), n_h[b] & 1);
                     ++n_h[b];
                     pend[b] = false;
                     tc_fence_after();
+                    WM_TRACE(12 + b);
                 }
             };
-            // one ring stage = one [128 x 64] B tile = `ksteps` MMAs of K = 16
-            auto stage_ss = [&](uint32_t d_tmem, uint32_t a_tile, int ksteps, bool first) {
-                if (prof) ps[3] += (unsigned long long)(clock64() - t_last);
-                mbar_wait_t(bar(B_FULL + stage), ph, prof ? &pf[0] : nullptr);
-                const long long tf0 = prof ? clock64() : 0;
+            // wait until the next n (<= 2) ring stages are full: lane i polls stage + i
+            auto wait_full = [&](int n) {
+                WM_TRACE(1);
+                if (lane < n) {
+                    uint32_t sidx = stage + lane, sp = ph;
+                    if (sidx >= NSTAGE) { sidx -= NSTAGE; sp ^= 1; }
+                    mbar_wait(bar(B_FULL + sidx), sp);
+                }
+                __syncwarp();
                 tc_fence_after();
-                if (prof) ps[2] += (unsigned long long)(clock64() - tf0);
+                WM_TRACE(2);
+            };
+            // one ring stage = one [128 x 64] B tile = `ksteps` MMAs of K = 16; the stage must already be full
+            auto issue_ss = [&](uint32_t d_tmem, uint32_t a_tile, int ksteps, bool first) {
                 const uint64_t ad = smem_desc(a_tile), bd = smem_desc(s_ring + stage * TILE_BYTES);
-                const long long ti0 = prof ? clock64() : 0;
                 if (elect_one()) {
                     for (int j = 0; j < ksteps; ++j)
                         mma_ss(d_tmem, ad + 2u * j, bd + 2u * j, IDESC, (first && j == 0) ? 0u : 1u);
                     mma_commit(bar(B_EMPTY + stage));
                 }
                 __syncwarp();
-                if (prof) { t_last = clock64(); ps[0] += (unsigned long long)(t_last - ti0); }
+                WM_TRACE(3);
                 if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
             };
-            auto stage_ts = [&](uint32_t d_tmem, uint32_t a_tmem, bool first) {
-                if (prof) ps[3] += (unsigned long long)(clock64() - t_last);
-                mbar_wait_t(bar(B_FULL + stage), ph, prof ? &pf[0] : nullptr);
-                const long long tf0 = prof ? clock64() : 0;
-                tc_fence_after();
-                if (prof) ps[2] += (unsigned long long)(clock64() - tf0);
+            auto issue_ts = [&](uint32_t d_tmem, uint32_t a_tmem, bool first) {
                 const uint64_t bd = smem_desc(s_ring + stage * TILE_BYTES);
-                const long long ti0 = prof ? clock64() : 0;
                 if (elect_one()) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
@@ -466,7 +466,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     mma_commit(bar(B_EMPTY + stage));
                 }
                 __syncwarp();
-                if (prof) { t_last = clock64(); ps[1] += (unsigned long long)(t_last - ti0); }
+                WM_TRACE(3);
                 if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
             };
             // GEMM over the A1 K-blocks in the order a/phi (4,5), [hw (6)], z (0..3); waits for the operands of
@@ -474,26 +474,32 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             auto gemm_a1 = [&](int b, bool first_chunk, bool with_hw) {
                 wait_h(b);
                 const uint32_t d = T_D1 + 128u * b;
-                if (first_chunk) { mbar_wait_t(bar(B_AREADY), n_a & 1, prof ? &pf[2] : nullptr); ++n_a; tc_fence_after(); }
-                stage_ss(d, s_a1 + 4 * TILE_BYTES, 4, true);
-                stage_ss(d, s_a1 + 5 * TILE_BYTES, 4, false);
-                if (with_hw) stage_ss(d, s_a1 + 6 * TILE_BYTES, p.hw_ksteps, false);
-                if (first_chunk) { mbar_wait_t(bar(B_ZREADY), n_z & 1, prof ? &pf[3] : nullptr); ++n_z; tc_fence_after(); }
+                if (first_chunk) { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); }
+                wait_full(2);
+                issue_ss(d, s_a1 + 4 * TILE_BYTES, 4, true);
+                issue_ss(d, s_a1 + 5 * TILE_BYTES, 4, false);
+                if (with_hw) {
+                    wait_full(1);
+                    issue_ss(d, s_a1 + 6 * TILE_BYTES, p.hw_ksteps, false);
+                }
+                if (first_chunk) { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); }
 #pragma unroll 1
-                for (int kb = 0; kb < 4; ++kb) stage_ss(d, s_a1 + kb * TILE_BYTES, 4, false);
+                for (int kb = 0; kb < 4; kb += 2) {
+                    wait_full(2);
+                    issue_ss(d, s_a1 + kb * TILE_BYTES, 4, false);
+                    issue_ss(d, s_a1 + (kb + 1) * TILE_BYTES, 4, false);
+                }
                 if (elect_one()) mma_commit(bar(B_D1FULL + b));
                 __syncwarp();
                 pend[b] = true;
             };
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it & 1;
-                mbar_wait_t(bar(B_SFULL + slot), (it >> 1) & 1, prof ? &pf[4] : nullptr);
+                mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
                 const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
                 if (tile < 0) break;
-                pf[5] += (unsigned long long)nsteps;
-                pf[6] += 1;
 #pragma unroll 1
                 for (int t = 0; t < nsteps; ++t) {
 #pragma unroll 1
@@ -510,8 +516,11 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                             wait_h(b);
                             const uint32_t hbuf = T_D1 + 128u * b;
 #pragma unroll 1
-                            for (int kh = 0; kh < 4; ++kh)
-                                stage_ts(T_Z + 128u * (kh & 1), hbuf + 64u * (kh >> 1), false);
+                            for (int ks = 0; ks < 2; ++ks) {
+                                wait_full(2);
+                                issue_ts(T_Z, hbuf + 64u * ks, false);
+                                issue_ts(T_Z + 128u, hbuf + 64u * ks, false);
+                            }
                             if (c == NC - 1) {
                                 if (elect_one()) mma_commit(bar(B_D2FULL));
                                 __syncwarp();
@@ -536,20 +545,15 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     const int b = c & 1;
                     wait_h(b);
 #pragma unroll 1
-                    for (int kb = 0; kb < 8; ++kb) stage_ts(T_D1 + 128u * b, T_Z + 32u * kb, kb == 0);
+                    for (int kb = 0; kb < 8; kb += 2) {
+                        wait_full(2);
+                        issue_ts(T_D1 + 128u * b, T_Z + 32u * kb, kb == 0);
+                        issue_ts(T_D1 + 128u * b, T_Z + 32u * (kb + 1), false);
+                    }
                     if (elect_one()) mma_commit(bar(B_D1FULL + b));
                     __syncwarp();
                     pend[b] = true;
                 }
-            }
-            if (prof && lane == 0) {
-                pf[7] = (unsigned long long)(clock64() - t_begin);
-                for (int i = 0; i < 8; ++i) p.prof[(size_t)blockIdx.x * 16 + i] = pf[i];
-                p.prof[(size_t)blockIdx.x * 16 + 13] = ps[0];
-                p.prof[(size_t)blockIdx.x * 16 + 14] = ps[1];
-                p.prof[(size_t)blockIdx.x * 16 + 15] = ps[2];
-                p.prof[(size_t)blockIdx.x * 16 + 9 + 0] += 0;
-                p.prof[(size_t)blockIdx.x * 16 + 3] = ps[3];   // (overwrites wait z slot: printed as gaps)
             }
         }
         __syncwarp();
@@ -562,13 +566,6 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         uint8_t* a1 = smem + L.a1;
         uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
         const float inv_d = 1.0f / (float)D;
-        unsigned long long ef[4] = {0, 0, 0, 0};   // wait d1, wait d2, total
-#ifdef WM_TC_PROFILE
-        const bool eprof = p.prof != nullptr && warp == EPI_WARP0 && lane == 0;
-#else
-        constexpr bool eprof = false;
-#endif
-        const long long e_begin = clock64();
         // write 32 consecutive z columns of this row: fp32 -> TMEM, bf16 -> A1 (when `to_smem`)
         auto put_z = [&](int col0, const uint32_t (&v)[32], bool to_smem) {
             tmem_st32(T_Z + lane_off + (uint32_t)col0, v);
@@ -595,7 +592,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         };
         // bias + GELU over this thread's 64 columns of accumulator buffer b, bf16 result to TMEM at dst_col
         auto gelu_chunk = [&](int b, const float* bias, bool bias_in_smem, uint32_t dst_col) {
-            mbar_wait_t(bar(B_D1FULL + b), n_d1[b] & 1, eprof ? &ef[0] : nullptr);
+            mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
             ++n_d1[b];
             tc_fence_after();
 #pragma unroll
@@ -652,7 +649,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 for (int c = 0; c < NC; ++c)
                     gelu_chunk(c & 1, s_b1 + c * 128 + 64 * hh, true, T_D1 + 128u * (c & 1) + 64u * hh);
                 // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
-                mbar_wait_t(bar(B_D2FULL), n_d2 & 1, eprof ? &ef[1] : nullptr);
+                mbar_wait(bar(B_D2FULL), n_d2 & 1);
                 ++n_d2;
                 tc_fence_after();
                 float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
@@ -741,10 +738,6 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             if (hh == 0 && cand >= 0) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
             named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
         }
-        if (eprof) {
-            ef[2] = (unsigned long long)(clock64() - e_begin);
-            for (int i = 0; i < 3; ++i) p.prof[(size_t)blockIdx.x * 16 + 8 + i] = ef[i];
-        }
     } else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
         // =============================================================== action-embedding warps
         const int aw = warp - ACT_WARP0;
@@ -765,13 +758,6 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) bp4[e] = __ldg(p.bp + col4 + e);
         uint32_t n_w = 0;
-        unsigned long long af[2] = {0, 0};
-#ifdef WM_TC_PROFILE
-        const bool aprof = p.prof != nullptr && warp == ACT_WARP0 && lane == 0;
-#else
-        constexpr bool aprof = false;
-#endif
-        const long long a_begin = clock64();
         // A1 destination of this lane's 4 columns (8 bytes) in row r: K-block 4 + lane/16
         auto a_dst = [&](int r) -> uint2* {
             return reinterpret_cast<uint2*>(a1 + (4 + (lane >> 4)) * TILE_BYTES + sw128_off(r, (lane & 15) >> 1) +
@@ -823,7 +809,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
                 __syncwarp();
                 // store only once GEMM1 of the previous step no longer reads the a-part of A1
-                if (n_w > 0) mbar_wait_t(bar(B_AFREE), (n_w - 1) & 1, aprof ? &af[0] : nullptr);
+                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
                 ++n_w;
                 // phase 2 (4 columns per lane, loop over the warp's 32 rows): a = E[id] + W_p log2(p) + b_p
 #pragma unroll 2
@@ -857,7 +843,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(slp[0], slp[1], slp[2], slp[3]);
             *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(slp[4], slp[5], slp[6], slp[7]);
             __syncwarp();
-            if (n_w > 0) mbar_wait_t(bar(B_AFREE), (n_w - 1) & 1, aprof ? &af[0] : nullptr);
+            if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
 #pragma unroll 1
             for (int rr = 0; rr < 32; ++rr) {
@@ -901,10 +887,6 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_AREADY));
-        }
-        if (aprof) {
-            p.prof[(size_t)blockIdx.x * 16 + 11] = af[0];
-            p.prof[(size_t)blockIdx.x * 16 + 12] = (unsigned long long)(clock64() - a_begin);
         }
     }
 
@@ -1035,8 +1017,8 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     static unsigned long long* d_prof = nullptr;
 #ifdef WM_TC_PROFILE
     if (getenv("WM_TC_PROF")) {
-        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, 148 * 16 * 8));
-        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, 148 * 16 * 8, st));
+        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, 3 * 8192 * 8));
+        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, 3 * 8192 * 8, st));
         p.prof = d_prof;
     }
 #endif
@@ -1045,18 +1027,20 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     tc::wm_tc_kernel<<<grid, tc::THREADS, L.total, st>>>(p);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
-    if (p.prof) {   // dev instrumentation: synchronous dump of the per-CTA wait-cycle counters
-        std::vector<unsigned long long> h(148 * 16);
+#ifdef WM_TC_PROFILE
+    if (p.prof) {   // dev instrumentation: dump CTA 0's per-role (tag, clock) traces to WM_TC_PROF's path
+        std::vector<uint2> h(3 * 8192);
         WM_CUDA_TRY(cudaStreamSynchronize(st));
         WM_CUDA_TRY(cudaMemcpy(h.data(), d_prof, h.size() * 8, cudaMemcpyDeviceToHost));
-        double s[16] = {};
-        for (int b = 0; b < grid; ++b)
-            for (int i = 0; i < 16; ++i) s[i] += (double)h[b * 16 + i] / grid;
-        fprintf(stderr,
-                "[wm_tc prof] per-CTA mean cycles: mma total %.0f | wait full %.0f h %.0f a %.0f z %.0f sched %.0f | "
-                "steps %.1f tiles %.2f || epi total %.0f wait d1 %.0f d2 %.0f || act total %.0f wait afree(step) %.0f || issue ss %.0f ts %.0f\n",
-                s[7], s[0], s[1], s[2], s[3], s[4], s[5], s[6], s[10], s[8], s[9], s[12], s[11], s[13], s[14]);
+        FILE* f = fopen(getenv("WM_TC_PROF"), "w");
+        if (f) {
+            for (int r = 0; r < 3; ++r)
+                for (uint32_t i = 0; i < h[r * 8192].x; ++i)
+                    fprintf(f, "%d %u %u\n", r, h[r * 8192 + 1 + i].x, h[r * 8192 + 1 + i].y);
+            fclose(f);
+        }
     }
+#endif
     return WM_OK;
 }
 
