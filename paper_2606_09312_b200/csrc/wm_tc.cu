@@ -12,7 +12,7 @@
 //   * GEMM1 runs in 128-column chunks of the hidden layer into two alternating TMEM accumulators; the GELU
 //     epilogue writes the bf16 hidden chunk back INTO TMEM (over its own fp32 columns) and GEMM2 consumes it as a
 //     TMEM A operand (tcgen05.mma with A in tensor memory), so the hidden activations never touch shared memory;
-//   * weights stream from L2 through a 5-stage ring of 16 KB tiles filled by bulk async copies (TMA engine,
+//   * weights stream from L2 through a 3-stage ring of 32 KB tile pairs filled by bulk async copies (TMA engine,
 //     mbarrier complete_tx); the weight image in global memory is pre-tiled, pre-swizzled and laid out in exactly
 //     the order the MMA warp consumes it, so the producer is a linear stream;
 //   * the scorer's two hidden layers run on the same machinery (layer-1 output kept in TMEM as layer-2's A
@@ -37,14 +37,16 @@ constexpr int D = 256;             // latent width
 constexpr int DA = 128;            // action-embedding width
 constexpr int SW = 512;            // scorer hidden width (both hidden layers)
 constexpr int TILE_BYTES = 16384;  // one [128 x 64] bf16 K-block tile, SW128 K-major
-constexpr int NSTAGE = 5;
-constexpr int A1_KB = 7;           // z: 0-3, a/phi: 4-5, hw: 6
+constexpr int STAGE_BYTES = 2 * TILE_BYTES;   // one ring stage = a PAIR of tiles (one barrier wait / commit per 8 MMAs)
+constexpr int NSTAGE = 3;
+constexpr int A1_KB = 6;           // z: 0-3, a/phi: 4-5
+constexpr int HWK_BYTES = 4096;    // hw operand: one [128 x 16] no-swizzle K-major tile per K = 16 step
 constexpr int THREADS = 512;
 // Warp roles.  The SM's warp arbiter favours higher warp ids, so the latency-critical single-warp roles (MMA
 // issuer, weight producer) sit at the top and the throughput roles (epilogue, action) below them.
 constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
 constexpr int MAX_TYPES = 64, MAX_P = 8, MAX_H = 64, MAX_HID = 1024;
-constexpr int SC_TILES = 4 * 7 + 4 * 8;   // scorer stream: layer 1 (4 chunks x 7 tiles), layer 2 (4 x 8)
+constexpr int SC_TILES = 4 * 8 + 4 * 8;   // scorer stream: layer 1 (4 chunks x (2 phi, hw + pad, 4 z)), layer 2 (4 x 8)
 
 // barrier indices
 enum {
@@ -78,14 +80,15 @@ struct Params {
 };
 
 struct SmemLayout {
-    uint32_t a1, ring, e_tab, lp, ids, lens, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
+    uint32_t a1, hwk, ring, e_tab, lp, ids, lens, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
 };
 
-__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid) {
+__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps) {
     SmemLayout L;
     uint32_t o = 0;
     L.a1 = o; o += A1_KB * TILE_BYTES;
-    L.ring = o; o += NSTAGE * TILE_BYTES;
+    L.ring = o; o += NSTAGE * STAGE_BYTES;
+    L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
     L.e_tab = o; o += (uint32_t)n_types * DA * 2;
     L.lp = o; o += TM * MAX_P * 4;
     L.ids = o; o += TM * 4;
@@ -281,6 +284,13 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
     const uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);
     return ((uint64_t)hi << 32) | lo;
 }
+// Same, no swizzle ("interleave"), for a [128 x 16] K-major tile stored as 16-byte rows of 8-row core matrices:
+// the two K halves of a core-matrix row group are 128 B apart (LBO), row groups 256 B apart (SBO).
+__device__ __forceinline__ uint64_t smem_desc_nosw(uint32_t saddr) {
+    const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | ((128u >> 4) << 16);
+    const uint32_t hi = (256u >> 4) | (1u << 14);
+    return ((uint64_t)hi << 32) | lo;
+}
 // kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N = 128.
 constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
 
@@ -320,7 +330,7 @@ __device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
 
 __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     extern __shared__ __align__(1024) uint8_t smem[];
-    const SmemLayout L = smem_layout(p.n_types, p.hid);
+    const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps);
     const uint32_t s_base = smem_u32(smem);
     const uint32_t s_a1 = s_base + L.a1, s_ring = s_base + L.ring, s_bars = s_base + L.bars;
     auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
@@ -363,8 +373,8 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         uint32_t* dst = reinterpret_cast<uint32_t*>(smem + L.e_tab);
         for (int i = threadIdx.x; i < p.n_types * DA / 2; i += THREADS) dst[i] = __ldg(src + i);
         // the hw K-block is only ever written in its first columns: clear it once so unread bytes are not NaNs
-        uint32_t* hwk = reinterpret_cast<uint32_t*>(smem + L.a1 + 6 * TILE_BYTES);
-        for (int i = threadIdx.x; i < TILE_BYTES / 4; i += THREADS) hwk[i] = 0u;
+        uint32_t* hwk = reinterpret_cast<uint32_t*>(smem + L.hwk);
+        for (int i = threadIdx.x; i < p.hw_ksteps * HWK_BYTES / 4; i += THREADS) hwk[i] = 0u;
     }
     tc_fence_before();
     __syncthreads();
@@ -401,12 +411,13 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             }
             if (tile < 0) break;
             if (lane == 0) {
+                // the stream is consumed in pairs of tiles that are adjacent in the image: one 32 KB copy per stage
                 const int roll_total = nsteps * ROLL_TILES, total = roll_total + SC_TILES;
-                for (int i = 0; i < total; ++i) {
+                for (int i = 0; i < total; i += 2) {
                     const int src_tile = i < roll_total ? i % ROLL_TILES : ROLL_TILES + (i - roll_total);
                     mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
-                    mbar_arrive_expect_tx(bar(B_FULL + stage), TILE_BYTES);
-                    bulk_g2s(s_ring + stage * TILE_BYTES, p.blob + (size_t)src_tile * TILE_BYTES, TILE_BYTES,
+                    mbar_arrive_expect_tx(bar(B_FULL + stage), STAGE_BYTES);
+                    bulk_g2s(s_ring + stage * STAGE_BYTES, p.blob + (size_t)src_tile * TILE_BYTES, STAGE_BYTES,
                              bar(B_FULL + stage));
                     if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
                 }
@@ -415,13 +426,14 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         }
     } else if (warp == MMA_WARP) {
         // =============================================================== MMA issuer (converged warp, one elected lane)
-        // tcgen05.mma dispatch occupies the issuing warp for the MMA's duration, so every other instruction this
-        // warp executes is tensor-pipe idle time: waits are batched (one warp-wide try_wait covers the full
-        // barriers of up to two ring stages, one lane per barrier) and the issue loops stay rolled and small.
+        // The MMAs themselves are asynchronous (4 issue in ~70 cycles and queue in the tensor pipe), so the pipe
+        // stays busy only while this warp's bookkeeping per 8 MMAs (512 pipe cycles) costs less than 512 cycles:
+        // one full-barrier wait and one commit per ring stage (a pair of tiles), rolled loops, nothing else.
         {
             uint32_t stage = 0, ph = 0;
             uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
             bool pend[2] = {false, false};
+            const uint32_t s_hwk = s_base + L.hwk;
             WM_TRACE_DECL(0, true)
             auto wait_h = [&](int b) {
                 if (pend[b]) {
@@ -433,64 +445,74 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     WM_TRACE(12 + b);
                 }
             };
-            // wait until the next n (<= 2) ring stages are full: lane i polls stage + i
-            auto wait_full = [&](int n) {
+            auto wait_full = [&]() {
                 WM_TRACE(1);
-                if (lane < n) {
-                    uint32_t sidx = stage + lane, sp = ph;
-                    if (sidx >= NSTAGE) { sidx -= NSTAGE; sp ^= 1; }
-                    mbar_wait(bar(B_FULL + sidx), sp);
-                }
-                __syncwarp();
+                mbar_wait(bar(B_FULL + stage), ph);
                 tc_fence_after();
                 WM_TRACE(2);
             };
-            // one ring stage = one [128 x 64] B tile = `ksteps` MMAs of K = 16; the stage must already be full
-            auto issue_ss = [&](uint32_t d_tmem, uint32_t a_tile, int ksteps, bool first) {
-                const uint64_t ad = smem_desc(a_tile), bd = smem_desc(s_ring + stage * TILE_BYTES);
-                if (elect_one()) {
-                    for (int j = 0; j < ksteps; ++j)
-                        mma_ss(d_tmem, ad + 2u * j, bd + 2u * j, IDESC, (first && j == 0) ? 0u : 1u);
-                    mma_commit(bar(B_EMPTY + stage));
-                }
+            auto release = [&]() {   // called by the elected lane after the stage's last MMA
+                mma_commit(bar(B_EMPTY + stage));
+            };
+            auto advance = [&]() {
                 __syncwarp();
                 WM_TRACE(3);
                 if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
             };
-            auto issue_ts = [&](uint32_t d_tmem, uint32_t a_tmem, bool first) {
-                const uint64_t bd = smem_desc(s_ring + stage * TILE_BYTES);
+            // stage = two [128 x 64] B tiles against the A1 K-blocks a_tile0, a_tile1 (8 MMAs of K = 16)
+            auto pair_ss = [&](uint32_t d_tmem, uint32_t a_tile0, uint32_t a_tile1, bool first) {
+                wait_full();
+                const uint64_t a0 = smem_desc(a_tile0), a1d = smem_desc(a_tile1);
+                const uint64_t b0 = smem_desc(s_ring + stage * STAGE_BYTES), b1 = b0 + (TILE_BYTES >> 4);
                 if (elect_one()) {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        mma_ts(d_tmem, a_tmem + 8u * j, bd + 2u * j, IDESC, (first && j == 0) ? 0u : 1u);
-                    mma_commit(bar(B_EMPTY + stage));
+                    for (int j = 0; j < 4; ++j) mma_ss(d_tmem, a0 + 2u * j, b0 + 2u * j, IDESC, (first && j == 0) ? 0u : 1u);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) mma_ss(d_tmem, a1d + 2u * j, b1 + 2u * j, IDESC, 1u);
+                    release();
                 }
-                __syncwarp();
-                WM_TRACE(3);
-                if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+                advance();
             };
-            // GEMM over the A1 K-blocks in the order a/phi (4,5), [hw (6)], z (0..3); waits for the operands of
-            // the first chunk of a step / of the scorer.
+            // stage = (hw tile, padding tile): hw_ksteps MMAs whose A operand is the no-swizzle [128 x 16] hw tile
+            auto pair_hw = [&](uint32_t d_tmem) {
+                wait_full();
+                const uint64_t b0 = smem_desc(s_ring + stage * STAGE_BYTES);
+                if (elect_one()) {
+                    for (int j = 0; j < p.hw_ksteps; ++j)
+                        mma_ss(d_tmem, smem_desc_nosw(s_hwk + j * HWK_BYTES), b0 + 2u * j, IDESC, 1u);
+                    release();
+                }
+                advance();
+            };
+            // stage = two B tiles against TMEM A operands a_tmem0, a_tmem1 into d0, d1
+            auto pair_ts = [&](uint32_t d0, uint32_t d1, uint32_t a_tmem0, uint32_t a_tmem1, bool first) {
+                wait_full();
+                const uint64_t b0 = smem_desc(s_ring + stage * STAGE_BYTES), b1 = b0 + (TILE_BYTES >> 4);
+                if (elect_one()) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) mma_ts(d0, a_tmem0 + 8u * j, b0 + 2u * j, IDESC, (first && j == 0) ? 0u : 1u);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) mma_ts(d1, a_tmem1 + 8u * j, b1 + 2u * j, IDESC, 1u);
+                    release();
+                }
+                advance();
+            };
+            auto commit = [&](int barrier) {
+                if (elect_one()) mma_commit(bar(barrier));
+                __syncwarp();
+            };
+            // GEMM over the A1 K-blocks in the order a/phi (4,5), [hw], z (0..3); waits for the operands of the
+            // first chunk of a step / of the scorer.
             auto gemm_a1 = [&](int b, bool first_chunk, bool with_hw) {
                 wait_h(b);
                 const uint32_t d = T_D1 + 128u * b;
                 if (first_chunk) { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); }
-                wait_full(2);
-                issue_ss(d, s_a1 + 4 * TILE_BYTES, 4, true);
-                issue_ss(d, s_a1 + 5 * TILE_BYTES, 4, false);
-                if (with_hw) {
-                    wait_full(1);
-                    issue_ss(d, s_a1 + 6 * TILE_BYTES, p.hw_ksteps, false);
-                }
+                pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
+                if (with_hw) pair_hw(d);
                 if (first_chunk) { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); }
-#pragma unroll 1
-                for (int kb = 0; kb < 4; kb += 2) {
-                    wait_full(2);
-                    issue_ss(d, s_a1 + kb * TILE_BYTES, 4, false);
-                    issue_ss(d, s_a1 + (kb + 1) * TILE_BYTES, 4, false);
-                }
-                if (elect_one()) mma_commit(bar(B_D1FULL + b));
-                __syncwarp();
+                pair_ss(d, s_a1, s_a1 + TILE_BYTES, false);
+                pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
+                commit(B_D1FULL + b);
                 pend[b] = true;
             };
             for (uint32_t it = 0;; ++it) {
@@ -506,25 +528,15 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     for (int i = 0; i <= NC; ++i) {
                         if (i < NC) {
                             gemm_a1(i & 1, i == 0, false);                       // GEMM1 chunk i
-                            if (i == NC - 1) {
-                                if (elect_one()) mma_commit(bar(B_AFREE));
-                                __syncwarp();
-                            }
+                            if (i == NC - 1) commit(B_AFREE);
                         }
                         if (i >= 1) {                                            // GEMM2 chunk i-1 (A from TMEM)
                             const int c = i - 1, b = c & 1;
                             wait_h(b);
                             const uint32_t hbuf = T_D1 + 128u * b;
-#pragma unroll 1
-                            for (int ks = 0; ks < 2; ++ks) {
-                                wait_full(2);
-                                issue_ts(T_Z, hbuf + 64u * ks, false);
-                                issue_ts(T_Z + 128u, hbuf + 64u * ks, false);
-                            }
-                            if (c == NC - 1) {
-                                if (elect_one()) mma_commit(bar(B_D2FULL));
-                                __syncwarp();
-                            }
+                            pair_ts(T_Z, T_Z + 128u, hbuf, hbuf, false);
+                            pair_ts(T_Z, T_Z + 128u, hbuf + 64u, hbuf + 64u, false);
+                            if (c == NC - 1) commit(B_D2FULL);
                         }
                     }
                 }
@@ -532,10 +544,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll 1
                 for (int c = 0; c < 4; ++c) {
                     gemm_a1(c & 1, c == 0, true);
-                    if (c == 3) {
-                        if (elect_one()) mma_commit(bar(B_AFREE));
-                        __syncwarp();
-                    }
+                    if (c == 3) commit(B_AFREE);
                 }
                 wait_h(0);
                 wait_h(1);   // all of H1 (bf16, TMEM columns [0,256)) written
@@ -545,13 +554,9 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     const int b = c & 1;
                     wait_h(b);
 #pragma unroll 1
-                    for (int kb = 0; kb < 8; kb += 2) {
-                        wait_full(2);
-                        issue_ts(T_D1 + 128u * b, T_Z + 32u * kb, kb == 0);
-                        issue_ts(T_D1 + 128u * b, T_Z + 32u * (kb + 1), false);
-                    }
-                    if (elect_one()) mma_commit(bar(B_D1FULL + b));
-                    __syncwarp();
+                    for (int kb = 0; kb < 8; kb += 2)
+                        pair_ts(T_D1 + 128u * b, T_D1 + 128u * b, T_Z + 32u * kb, T_Z + 32u * (kb + 1), kb == 0);
+                    commit(B_D1FULL + b);
                     pend[b] = true;
                 }
             }
@@ -812,7 +817,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
                 ++n_w;
                 // phase 2 (4 columns per lane, loop over the warp's 32 rows): a = E[id] + W_p log2(p) + b_p
-#pragma unroll 2
+#pragma unroll 4
                 for (int rr = 0; rr < 32; ++rr) {
                     const int r = 32 * aw + rr;
                     const int idr = s_ids[r];
@@ -873,7 +878,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 }
                 *a_dst(r) = make_uint2(pack_bf16(a4[0], a4[1]), pack_bf16(a4[2], a4[3]));
             }
-            // hardware features of this row -> K-block 6 (columns >= H stay zero)
+            // hardware features of this row -> the hw operand tile (columns >= H stay zero)
             for (int ch = 0; ch < p.H / 8; ++ch) {
                 uint4 o = make_uint4(0u, 0u, 0u, 0u);
                 if (cand >= 0) {
@@ -882,7 +887,9 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     o.x = pack_bf16(f0.x, f0.y); o.y = pack_bf16(f0.z, f0.w);
                     o.z = pack_bf16(f1.x, f1.y); o.w = pack_bf16(f1.z, f1.w);
                 }
-                *reinterpret_cast<uint4*>(a1 + 6 * TILE_BYTES + sw128_off(row, ch)) = o;
+                // K-step ch/2, K half ch&1 of the no-swizzle tile (see smem_desc_nosw)
+                *reinterpret_cast<uint4*>(smem + L.hwk + (ch >> 1) * HWK_BYTES + (row >> 3) * 256 + (ch & 1) * 128 +
+                                          (row & 7) * 16) = o;
             }
             fence_proxy_async();
             __syncwarp();
@@ -937,7 +944,7 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     Model& m = ctx->m;
     m.tc_ok = 0;
     if (!tc_model_ok(m)) return WM_OK;
-    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden);
+    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16);
     if ((int)L.total > ctx->smem_optin) return WM_OK;
     auto get = [&](const char* n) -> const std::vector<float>& {
         for (size_t i = 0; i < names.size(); ++i)
@@ -961,10 +968,11 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         if (i < NC) g1(i);
         if (i >= 1) g2(i - 1);
     }
-    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw (1), z (4)
+    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
         append_tile(blob, Ws0, K0, c * 128, tc::D, 64);
         append_tile(blob, Ws0, K0, c * 128, tc::D + 64, 64);
         append_tile(blob, Ws0, K0, c * 128, K1, m.H);
+        append_tile(blob, Ws0, K0, c * 128, K1, 0);
         for (int kb = 0; kb < 4; ++kb) append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
     }
     for (int c = 0; c < 4; ++c)       // scorer layer 2
@@ -1022,7 +1030,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
         p.prof = d_prof;
     }
 #endif
-    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden);
+    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
     const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
     tc::wm_tc_kernel<<<grid, tc::THREADS, L.total, st>>>(p);
     WM_CUDA_TRY(cudaGetLastError());
