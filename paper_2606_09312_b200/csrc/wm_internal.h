@@ -47,7 +47,8 @@ struct Model {
     void* tc_blob = nullptr;
     size_t tc_blob_bytes = 0;
     void* tc_E = nullptr;      // bf16 [n_types][d_a]
-    int tc_ok = 0;
+    int tc_ok = 0;             // 0 = no tcgen05 path, 1 = wm_tc_kernel (one CTA per tile), 2 = wm_tc2_kernel (CTA pair)
+    alignas(64) unsigned char tc2_tmap[128] = {};   // CUtensorMap over tc_blob (pair kernel)
 };
 
 // Per-stream slice of the workspace (perm, histogram/cursors, tile counter).
@@ -126,6 +127,11 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_
                const std::vector<std::string>& names);
 int tc_supported(const wm_ctx* ctx);
 int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
+
+// K2 tcgen05, CTA pair (wm_tc2.cu): bf16 MLP_LN models with d = 512.  Reached through tc_prepare / launch_tc.
+int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
+                const std::vector<std::string>& names);
+int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 
 // K3 (wm_topk.cu)
 int64_t topk_launches();

@@ -7,10 +7,10 @@
 // One CTA owns a tile of 128 candidates (length-sorted by K1) for ALL of its steps:
 //   * the fp32 master latent of the tile lives in TMEM columns [0,256) and IS the accumulator of GEMM2: the
 //     residual add is the MMA's accumulate, the epilogue adds b2, applies LayerNorm and writes z' back;
-//   * a bf16 copy of [z ; a] lives in shared memory (K-major, 128B-swizzled 64-column K-blocks) as the A operand
+//   * a fp16 copy of [z ; a] lives in shared memory (K-major, 128B-swizzled 64-column K-blocks) as the A operand
 //     of GEMM1;
 //   * GEMM1 runs in 128-column chunks of the hidden layer into two alternating TMEM accumulators; the GELU
-//     epilogue writes the bf16 hidden chunk back INTO TMEM (over its own fp32 columns) and GEMM2 consumes it as a
+//     epilogue writes the fp16 hidden chunk back INTO TMEM (over its own fp32 columns) and GEMM2 consumes it as a
 //     TMEM A operand (tcgen05.mma with A in tensor memory), so the hidden activations never touch shared memory;
 //   * weights stream from L2 through a 3-stage ring of 32 KB tile pairs filled by bulk async copies (TMA engine,
 //     mbarrier complete_tx); the weight image in global memory is pre-tiled, pre-swizzled and laid out in exactly
@@ -27,6 +27,7 @@
 #include <cstring>
 
 #include "wm_internal.h"
+#include "wm_ptx.cuh"
 
 namespace wm {
 
@@ -36,7 +37,7 @@ constexpr int TM = 128;            // candidates per tile (MMA M)
 constexpr int D = 256;             // latent width
 constexpr int DA = 128;            // action-embedding width
 constexpr int SW = 512;            // scorer hidden width (both hidden layers)
-constexpr int TILE_BYTES = 16384;  // one [128 x 64] bf16 K-block tile, SW128 K-major
+constexpr int TILE_BYTES = 16384;  // one [128 x 64] 16-bit K-block tile, SW128 K-major
 constexpr int STAGE_BYTES = 2 * TILE_BYTES;   // one ring stage = a PAIR of tiles (one barrier wait / commit per 8 MMAs)
 constexpr int NSTAGE = 3;
 constexpr int A1_KB = 6;           // z: 0-3, a/phi: 4-5
@@ -53,9 +54,9 @@ enum {
     B_FULL = 0,                 // [NSTAGE] producer -> MMA
     B_EMPTY = B_FULL + NSTAGE,  // [NSTAGE] MMA commit -> producer
     B_D1FULL = B_EMPTY + NSTAGE,   // [2] MMA commit -> epilogue: accumulator buffer b filled
-    B_HREADY = B_D1FULL + 2,       // [2] epilogue -> MMA: buffer b consumed (bf16 hidden written)
+    B_HREADY = B_D1FULL + 2,       // [2] epilogue -> MMA: buffer b consumed (fp16 hidden written)
     B_D2FULL = B_HREADY + 2,       // MMA commit -> epilogue: GEMM2 of the step done
-    B_ZREADY,                      // epilogue -> MMA: z (bf16 smem + fp32 TMEM) written
+    B_ZREADY,                      // epilogue -> MMA: z (fp16 smem + fp32 TMEM) written
     B_AFREE,                       // MMA commit -> action warps: a-part of A1 no longer read
     B_AREADY,                      // action warps -> MMA: a-part written
     B_SFULL,                       // [2] scheduler -> consumers
@@ -107,43 +108,8 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
     return L;
 }
 
-// ------------------------------------------------------------------------------------------------ PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+using namespace ptx;
 
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-// Bounded wait: a protocol bug must trap (and fail the test), never hang the GPU box.  The slow path is kept
-// out of line so the ~60 wait sites stay small (the kernel's code footprint matters: one warp per role, nothing
-// hides an instruction-cache miss).
-__device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity) {
-    const long long t0 = clock64();
-    while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > 4000000000LL) {
-            printf("wm_tc: mbarrier wait timed out (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x,
-                   bar, parity);
-            __trap();
-        }
-    }
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    if (!mbar_try_wait(bar, parity)) mbar_wait_slow(bar, parity);
-}
 // Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of CTA 0 appends
 // (tag, clock) records to a trace buffer that launch_tc dumps.  Compiled out otherwise.
 #ifdef WM_TC_PROFILE
@@ -159,174 +125,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 #define WM_TRACE_DECL(role, cond)
 #define WM_TRACE(tag) do { } while (0)
 #endif
-__device__ __forceinline__ void fence_barrier_init() {
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-                 "l"(src), "r"(bytes), "r"(bar)
-                 : "memory");
-}
-
-__device__ __forceinline__ void tmem_alloc(uint32_t slot_smem, uint32_t ncols) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(slot_smem), "r"(ncols)
-                 : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-
-// D[tmem] (+)= A[smem desc] * B[smem desc]
-__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
-        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc)
-        : "memory");
-}
-// D[tmem] (+)= A[tmem] * B[smem desc]
-__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
-        "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc)
-        : "memory");
-}
-__device__ __forceinline__ void mma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
-          "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
-          "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr)
-        : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
-        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
-        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
-        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
-        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-        : "memory");
-}
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
-        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
-        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
-        : "memory");
-}
-
-// one lane of a converged warp (always the same one): keeps the MMA operands warp-uniform for the compiler
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred;
-    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
-    return pred != 0;
-}
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
-// bf16x2 pack: lo -> bits [0,16), hi -> bits [16,32)
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-    uint32_t r;
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-    return r;
-}
-
-// GELU, tanh form (hardware tanh.approx): |gelu_tanh - gelu_erf| <= 5e-4 abs, below the bf16 rounding of the
-// hidden activations it feeds (DESIGN.md §3 S5).
-__device__ __forceinline__ float gelu_fast(float x) {
-    const float x2 = x * x;
-    const float inner = x * fmaf(0.0356774081f, x2, 0.7978845608f);
-    float t;
-    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(inner));
-    const float hx = 0.5f * x;
-    return fmaf(hx, t, hx);
-}
-
-// Two GELUs at once on the packed fp32x2 pipe (FFMA2/FMUL2/FADD2 halve the epilogue's FP instruction count).
-__device__ __forceinline__ uint32_t gelu2_bf16(float2 acc, float2 bias) {
-    const float2 x = __fadd2_rn(acc, bias);
-    const float2 hx = __fmul2_rn(x, make_float2(0.5f, 0.5f));
-    const float2 x2 = __fmul2_rn(x, x);
-    const float2 pin = __ffma2_rn(x2, make_float2(0.0356774081f, 0.0356774081f), make_float2(0.7978845608f, 0.7978845608f));
-    const float2 inner = __fmul2_rn(x, pin);
-    float2 t;
-    asm("tanh.approx.f32 %0, %1;" : "=f"(t.x) : "f"(inner.x));
-    asm("tanh.approx.f32 %0, %1;" : "=f"(t.y) : "f"(inner.y));
-    const float2 g = __ffma2_rn(hx, t, hx);
-    return pack_bf16(g.x, g.y);
-}
-
-// UMMA shared-memory descriptor, K-major, 128B swizzle, 8-row groups 1024 B apart (SBO), version 1 (sm_100).
-__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
-    const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | (1u << 16);
-    const uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);
-    return ((uint64_t)hi << 32) | lo;
-}
-// Same, no swizzle ("interleave"), for a [128 x 16] K-major tile stored as 16-byte rows of 8-row core matrices:
-// the two K halves of a core-matrix row group are 128 B apart (LBO), row groups 256 B apart (SBO).
-__device__ __forceinline__ uint64_t smem_desc_nosw(uint32_t saddr) {
-    const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | ((128u >> 4) << 16);
-    const uint32_t hi = (256u >> 4) | (1u << 14);
-    return ((uint64_t)hi << 32) | lo;
-}
-// kind::f16 instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N = 128.
-constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
 
 }  // namespace tc
 
 namespace tc {
-
-__device__ __forceinline__ int find_seg(const int32_t* __restrict__ off, int S, int cand) {
-    int lo = 0, hi = S;
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (__ldg(off + mid) <= cand) lo = mid; else hi = mid;
-    }
-    return lo;
-}
-
-// Row metadata of tile row r: candidate index (-1 = dead row), clamped length, subgraph (z0 / hw row).
-__device__ __forceinline__ void row_meta(const CallArgs& a, int tile, int r, int& cand, int& len, int& seg,
-                                         bool report) {
-    const int64_t i = (int64_t)tile * TM + r;
-    cand = -1; len = 0; seg = 0;
-    if (i < a.B) {
-        cand = a.perm ? __ldg(a.perm + i) : (int)i;
-        len = __ldg(a.lengths + cand);
-        if (len < 0 || len > a.T_max) {
-            if (report) atomicOr(a.fault, WM_FAULT_LEN);
-            len = len < 0 ? 0 : a.T_max;
-        }
-        seg = a.offsets ? find_seg(a.offsets, a.S, cand) : cand;
-    }
-}
-
-// byte offset of the 16-byte chunk `chunk` (8 bf16 columns) of row `row` inside a SW128 K-major K-block tile
-__device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
-    return (uint32_t)row * 128u + (uint32_t)((chunk ^ (row & 7)) << 4);
-}
 
 __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -395,7 +197,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             if (tile < p.n_tiles) {
                 for (int r = lane; r < TM; r += 32) {
                     int cand, len, seg;
-                    row_meta(p.a, tile, r, cand, len, seg, true);
+                    row_meta(p.a, (int64_t)tile * TM + r, cand, len, seg, true);
                     nsteps = max(nsteps, len);
                 }
 #pragma unroll
@@ -547,7 +349,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     if (c == 3) commit(B_AFREE);
                 }
                 wait_h(0);
-                wait_h(1);   // all of H1 (bf16, TMEM columns [0,256)) written
+                wait_h(1);   // all of H1 (fp16, TMEM columns [0,256)) written
                 // ---- scorer layer 2: A = H1 from TMEM, K = 512
 #pragma unroll 1
                 for (int c = 0; c < 4; ++c) {
@@ -571,7 +373,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         uint8_t* a1 = smem + L.a1;
         uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
         const float inv_d = 1.0f / (float)D;
-        // write 32 consecutive z columns of this row: fp32 -> TMEM, bf16 -> A1 (when `to_smem`)
+        // write 32 consecutive z columns of this row: fp32 -> TMEM, fp16 -> A1 (when `to_smem`)
         auto put_z = [&](int col0, const uint32_t (&v)[32], bool to_smem) {
             tmem_st32(T_Z + lane_off + (uint32_t)col0, v);
             if (to_smem) {
@@ -580,10 +382,10 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll
                 for (int ch = 0; ch < 4; ++ch) {
                     uint4 o;
-                    o.x = pack_bf16(__uint_as_float(v[8 * ch + 0]), __uint_as_float(v[8 * ch + 1]));
-                    o.y = pack_bf16(__uint_as_float(v[8 * ch + 2]), __uint_as_float(v[8 * ch + 3]));
-                    o.z = pack_bf16(__uint_as_float(v[8 * ch + 4]), __uint_as_float(v[8 * ch + 5]));
-                    o.w = pack_bf16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
+                    o.x = pack_f16(__uint_as_float(v[8 * ch + 0]), __uint_as_float(v[8 * ch + 1]));
+                    o.y = pack_f16(__uint_as_float(v[8 * ch + 2]), __uint_as_float(v[8 * ch + 3]));
+                    o.z = pack_f16(__uint_as_float(v[8 * ch + 4]), __uint_as_float(v[8 * ch + 5]));
+                    o.w = pack_f16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
                     *reinterpret_cast<uint4*>(kb + sw128_off(row, chunk0 + ch)) = o;
                 }
             }
@@ -595,7 +397,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(barrier));
         };
-        // bias + GELU over this thread's 64 columns of accumulator buffer b, bf16 result to TMEM at dst_col
+        // bias + GELU over this thread's 64 columns of accumulator buffer b, fp16 result to TMEM at dst_col
         auto gelu_chunk = [&](int b, const float* bias, bool bias_in_smem, uint32_t dst_col) {
             mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
             ++n_d1[b];
@@ -609,9 +411,9 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     const float4 bv = bias_in_smem ? bp_[i] : __ldg(bp_ + i);
-                    o[2 * i] = gelu2_bf16(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                    o[2 * i] = gelu2_f16(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
                                           make_float2(bv.x, bv.y));
-                    o[2 * i + 1] = gelu2_bf16(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                    o[2 * i + 1] = gelu2_f16(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
                                               make_float2(bv.z, bv.w));
                 }
                 tmem_st16(dst_col + lane_off + 16u * p2, o);
@@ -627,7 +429,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
             if (tile < 0) break;
             int cand, len, seg;
-            row_meta(p.a, tile, row, cand, len, seg, false);
+            row_meta(p.a, (int64_t)tile * TM + row, cand, len, seg, false);
 
             // ---- z_0 (the task's initial latent)
 #pragma unroll 1
@@ -707,14 +509,14 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                         v[4 * i] = __float_as_uint(x0.x); v[4 * i + 1] = __float_as_uint(x0.y);
                         v[4 * i + 2] = __float_as_uint(x1.x); v[4 * i + 3] = __float_as_uint(x1.y);
                     }
-                    // frozen rows: the bf16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
+                    // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
                     // fp32 master is never read again
                     put_z(col0, v, live);
                 }
                 publish(B_ZREADY, true);
             }
 
-            // ---- scorer layer 1 -> H1 (bf16) in TMEM columns [0,256)
+            // ---- scorer layer 1 -> H1 (fp16) in TMEM columns [0,256)
             for (int c = 0; c < 4; ++c)
                 gelu_chunk(c & 1, p.bs0 + c * 128 + 64 * hh, false, T_Z + 64u * c + 32u * hh);
             // ---- scorer layer 2 + output dot product
@@ -776,7 +578,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
             if (tile < 0) break;
             int cand, len, seg;
-            row_meta(p.a, tile, row, cand, len, seg, false);
+            row_meta(p.a, (int64_t)tile * TM + row, cand, len, seg, false);
             for (int c = 0; c < NT; ++c) s_cnt[row * NT + c] = 0;
             float slp[MAX_P];
 #pragma unroll
@@ -836,7 +638,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll
                             for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
                     }
-                    *a_dst(r) = make_uint2(pack_bf16(a4[0], a4[1]), pack_bf16(a4[2], a4[3]));
+                    *a_dst(r) = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
                 }
                 fence_proxy_async();
                 __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
@@ -876,7 +678,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll
                     for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(a4[e2], inv, bp4[e2]);
                 }
-                *a_dst(r) = make_uint2(pack_bf16(a4[0], a4[1]), pack_bf16(a4[2], a4[3]));
+                *a_dst(r) = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
             }
             // hardware features of this row -> the hw operand tile (columns >= H stay zero)
             for (int ch = 0; ch < p.H / 8; ++ch) {
@@ -884,8 +686,8 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 if (cand >= 0) {
                     const float4* src = reinterpret_cast<const float4*>(p.a.hw_feats + (size_t)seg * p.H + 8 * ch);
                     const float4 f0 = __ldg(src), f1 = __ldg(src + 1);
-                    o.x = pack_bf16(f0.x, f0.y); o.y = pack_bf16(f0.z, f0.w);
-                    o.z = pack_bf16(f1.x, f1.y); o.w = pack_bf16(f1.z, f1.w);
+                    o.x = pack_f16(f0.x, f0.y); o.y = pack_f16(f0.z, f0.w);
+                    o.z = pack_f16(f1.x, f1.y); o.w = pack_f16(f1.z, f1.w);
                 }
                 // K-step ch/2, K half ch&1 of the no-swizzle tile (see smem_desc_nosw)
                 *reinterpret_cast<uint4*>(smem + L.hwk + (ch >> 1) * HWK_BYTES + (row >> 3) * 256 + (ch & 1) * 128 +
@@ -916,15 +718,20 @@ uint16_t f32_to_bf16(float f) {
 }
 
 // Append the [128 x 64] tile W[n0 + n][k0 + k] (k < kvalid, else 0) in the SW128 K-major shared-memory image.
-void append_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid) {
+// Returns false when a weight is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
+bool append_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid) {
     const size_t base = blob.size();
     blob.resize(base + tc::TILE_BYTES / 2, 0);
+    bool ok = true;
     for (int n = 0; n < 128; ++n)
         for (int k = 0; k < 64; ++k) {
             const float v = k < kvalid ? W[(size_t)(n0 + n) * ld + k0 + k] : 0.0f;
             const size_t off = (size_t)n * 128 + (size_t)((((k >> 3) ^ (n & 7)) << 4)) + (size_t)(k & 7) * 2;
-            blob[base + off / 2] = f32_to_bf16(v);
+            uint16_t hb;
+            ok &= f32_to_f16_bits(v, &hb);
+            blob[base + off / 2] = hb;
         }
+    return ok;
 }
 
 struct TcState {
@@ -943,7 +750,7 @@ static bool tc_model_ok(const Model& m) {
 int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
     Model& m = ctx->m;
     m.tc_ok = 0;
-    if (!tc_model_ok(m)) return WM_OK;
+    if (!tc_model_ok(m)) return tc2_prepare(ctx, hv, names);   // d = 512 models: the CTA-pair kernel
     const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16);
     if ((int)L.total > ctx->smem_optin) return WM_OK;
     auto get = [&](const char* n) -> const std::vector<float>& {
@@ -955,28 +762,31 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1"), &E = get("E");
     const int hid = m.hidden, NC = hid / 128, K1 = tc::D + tc::DA, K0 = K1 + m.H;
     std::vector<uint16_t> blob;
+    bool ok = true;   // every weight finite in fp16
     blob.reserve((size_t)(NC * 10 + tc::SC_TILES) * tc::TILE_BYTES / 2);
     auto g1 = [&](int c) {   // GEMM1 chunk c: K-blocks a (4,5) then z (0..3)
         const int order[6] = {4, 5, 0, 1, 2, 3};
-        for (int i = 0; i < 6; ++i) append_tile(blob, W1, K1, c * 128, order[i] * 64, 64);
+        for (int i = 0; i < 6; ++i) ok &= append_tile(blob, W1, K1, c * 128, order[i] * 64, 64);
     };
     auto g2 = [&](int c) {   // GEMM2 chunk c: K halves of the hidden chunk x N halves of d
         for (int ks = 0; ks < 2; ++ks)
-            for (int h = 0; h < 2; ++h) append_tile(blob, W2, hid, h * 128, c * 128 + ks * 64, 64);
+            for (int h = 0; h < 2; ++h) ok &= append_tile(blob, W2, hid, h * 128, c * 128 + ks * 64, 64);
     };
     for (int i = 0; i <= NC; ++i) {   // same interleave as the MMA warp: G1(i), then G2(i-1)
         if (i < NC) g1(i);
         if (i >= 1) g2(i - 1);
     }
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
-        append_tile(blob, Ws0, K0, c * 128, tc::D, 64);
-        append_tile(blob, Ws0, K0, c * 128, tc::D + 64, 64);
-        append_tile(blob, Ws0, K0, c * 128, K1, m.H);
-        append_tile(blob, Ws0, K0, c * 128, K1, 0);
-        for (int kb = 0; kb < 4; ++kb) append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
+        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D, 64);
+        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + 64, 64);
+        ok &= append_tile(blob, Ws0, K0, c * 128, K1, m.H);
+        ok &= append_tile(blob, Ws0, K0, c * 128, K1, 0);
+        for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
     }
     for (int c = 0; c < 4; ++c)       // scorer layer 2
-        for (int kb = 0; kb < 8; ++kb) append_tile(blob, Ws1, tc::SW, c * 128, kb * 64, 64);
+        for (int kb = 0; kb < 8; ++kb) ok &= append_tile(blob, Ws1, tc::SW, c * 128, kb * 64, 64);
+
+    if (!ok) return WM_OK;   // a weight beyond the fp16 range: this model stays on the fp32 kernel
 
     void* d_blob = nullptr;
     WM_CUDA_TRY(cudaMalloc(&d_blob, blob.size() * 2));
@@ -1009,6 +819,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
         }
         return launch_generic(ctx, a, st);
     }
+    if (m.tc_ok == 2) return launch_tc2(ctx, ws, a, st);
     tc::Params p;
     p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;

@@ -1,0 +1,871 @@
+// K2 (tcgen05, CTA pair): fused persistent rollout + score kernel for the bf16 residual-MLP + LayerNorm model with
+// d = 512, d_a = 256 (BASELINE.json cfg 3), sm_100a only.
+//
+// PAPER.md:162 Eq.8 / :166 — z_t = F(z_{t-1}, a_t) applied recurrently; :176 — masked steps leave z unchanged;
+// :186-188 Eq.12 — y = G([z_T ; phi ; h]).  Parametrisation: BASELINE.json cfg 3.
+//
+// Why a pair: the fp32 master latent of a 128-candidate tile is 128 x 512 x 4 B = all 256 KB of one SM's tensor
+// memory, leaving no room for GEMM1's accumulators.  A cluster of two CTAs (one TPC) therefore owns a tile of 128
+// candidates together, 64 rows each, and the leader CTA issues `tcgen05.mma.cta_group::2` with M = 128, N = 256:
+//   * each CTA's D tile is 64 rows x 256 columns held as 128 lanes x 128 columns (lane l: row l % 64, columns
+//     128 * (l / 64) ...), so the fp32 latent of its 64 rows is 2 x 128 = 256 TMEM columns and IS the accumulator
+//     of GEMM2 (the residual add is the MMA's accumulate); the other 256 columns are two GEMM1 accumulators;
+//   * each CTA supplies its own 64 rows of the A operand (fp16 [z ; a], K-major 128B-swizzled 64-column K-blocks
+//     in shared memory) and HALF of every B tile (128 of the 256 weight rows): the L2 -> SM weight stream per
+//     candidate row is the same as for a 128-row single-CTA tile;
+//   * the GELU epilogue writes the fp16 hidden chunk to shared memory (GEMM2's A operand; with 64 rows per CTA a
+//     TMEM A operand would have to be duplicated across lane halves);
+//   * weights stream through a ring of 16 KB half tiles filled by TMA (`cp.async.bulk.tensor ... cta_group::2`, whose
+//     complete_tx lands on the LEADER's barrier for both halves) from a pre-tiled, pre-swizzled image laid out in
+//     consumption order; MMA completion is multicast to both CTAs' barriers (`tcgen05.commit ... multicast`);
+//   * epilogue / action warps of both CTAs arrive on the leader's barriers with cluster-scope release.
+// Warp roles per CTA (512 threads): warps 0-7 epilogue (lane quadrant q = warp % 4: rows 32 (q & 1) + lane, N half
+// q / 2; e = warp / 4: column half of the 128-column buffer), warps 8-11 action embedding, warp 12 TMEM allocator,
+// warp 13 tile schedule + TMA producer, warp 15 MMA issuer (leader CTA only).
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "wm_internal.h"
+#include "wm_ptx.cuh"
+
+namespace wm {
+
+namespace tc2 {
+
+using namespace ptx;
+
+constexpr int TMP = 128;           // candidates per pair tile (MMA M)
+constexpr int TMR = 64;            // rows per CTA
+constexpr int D = 512;             // latent width
+constexpr int DA = 256;            // action-embedding width
+constexpr int SW = 1024;           // scorer hidden width (both hidden layers)
+constexpr int KB_BYTES = 8192;     // one A K-block: [64 rows x 64 cols] fp16, SW128 K-major
+constexpr int BT_BYTES = 16384;    // one B half tile: [128 weight rows x 64 cols] fp16, SW128 K-major (= ring stage)
+constexpr int NSTAGE = 3;
+constexpr int A1_KB = 12;          // z: 0-7, a/phi: 8-11
+constexpr int H_KB = 4;            // K-blocks of one hidden chunk buffer (256 columns)
+constexpr int HWK_BYTES = 2048;    // hw operand: one [64 x 16] no-swizzle K-major tile per K = 16 step
+constexpr int THREADS = 512;
+constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
+constexpr int MAX_TYPES = 64, MAX_P = 8, MAX_H = 64, MAX_HID = 1024;
+constexpr int G1_STAGES = 12, G2_STAGES = 8;              // per 256-column hidden chunk
+constexpr int SC_STAGES = 4 * 13 + 2 * 32;                // scorer: layer 1 (4 x (4 phi, hw, 8 z)), layer 2 (2 rounds x 16 x 2)
+
+enum {
+    B_FULL = 0,                    // [NSTAGE] TMA (both CTAs) -> leader's MMA warp
+    B_EMPTY = B_FULL + NSTAGE,     // [NSTAGE] MMA commit (multicast) -> each CTA's producer
+    B_D1FULL = B_EMPTY + NSTAGE,   // [2] MMA commit -> epilogue: accumulator buffer b filled
+    B_HREADY = B_D1FULL + 2,       // [2] epilogue (both CTAs) -> leader MMA: buffer b read, fp16 hidden written
+    B_HFREE = B_HREADY + 2,        // [2] MMA commit -> epilogue: hidden buffer b no longer read
+    B_D2FULL = B_HFREE + 2,        // MMA commit -> epilogue: GEMM2 of the step done
+    B_ZREADY,                      // epilogue (both CTAs) -> leader MMA: z written
+    B_AFREE,                       // MMA commit -> action warps: a-part of A1 no longer read
+    B_AREADY,                      // action warps (both CTAs) -> leader MMA: a-part written
+    B_SFULL,                       // [2] schedule slot filled (CTA-local)
+    B_SEMPTY = B_SFULL + 2,        // [2] schedule slot consumed (CTA-local)
+    B_COUNT = B_SEMPTY + 2
+};
+
+struct Params {
+    int hid, nc, n_types, P, H, hw_ksteps;
+    float ln_eps;
+    const __nv_bfloat16* E;     // [n_types][256]
+    const float *WpT, *bp;      // [P][256], [256]
+    const float *b1, *b2, *gamma, *beta;
+    const float *bs0, *bs1, *w3, *bs2;
+    CallArgs a;
+    int n_tiles;
+};
+
+struct SmemLayout {
+    uint32_t a1, hbuf, ring, hwk, lp, ids, lens, cnt, b1, red, bars, sched, tmem_slot, total;
+};
+
+__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps) {
+    SmemLayout L;
+    uint32_t o = 0;
+    L.a1 = o; o += A1_KB * KB_BYTES;
+    L.hbuf = o; o += 2 * H_KB * KB_BYTES;
+    L.ring = o; o += NSTAGE * BT_BYTES;
+    L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
+    L.lp = o; o += TMR * MAX_P * 4;
+    L.ids = o; o += TMR * 4;
+    L.lens = o; o += TMR * 4;
+    L.cnt = o; o += TMR * (uint32_t)n_types;          // u8 counts, row-major [64][n_types]
+    o = (o + 15) & ~15u;
+    L.b1 = o; o += (uint32_t)hid * 4;
+    L.red = o; o += 4 * TMR * 8;                       // [4 column parts][64 rows] float2
+    L.bars = o; o += B_COUNT * 8;
+    L.sched = o; o += 2 * 8;
+    L.tmem_slot = o; o += 16;
+    L.total = o;
+    return L;
+}
+
+// Static tile schedule: pair `pair` of `np` pairs takes, in round `it`, tile it*np + pair on even rounds and
+// it*np + (np-1-pair) on odd rounds (tiles are sorted longest first: the serpentine evens out the step totals).
+__device__ __forceinline__ int tile_of(int it, int pair, int np, int n_tiles) {
+    const int idx = it * np + ((it & 1) ? np - 1 - pair : pair);
+    return idx < n_tiles ? idx : -1;
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps);
+    const uint32_t s_base = smem_u32(smem);
+    const uint32_t s_a1 = s_base + L.a1, s_h = s_base + L.hbuf, s_ring = s_base + L.ring, s_bars = s_base + L.bars;
+    auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
+    volatile int* s_sched = reinterpret_cast<volatile int*>(smem + L.sched);   // [2][2]: tile, nsteps
+    float* s_b1 = reinterpret_cast<float*>(smem + L.b1);
+    float2* s_red = reinterpret_cast<float2*>(smem + L.red);                  // [4][64]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
+    const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+    const int NC = p.nc;
+    const int ROLL_STAGES = NC * (G1_STAGES + G2_STAGES);
+
+    // ---- one-time setup
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NSTAGE; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 1); }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(bar(B_D1FULL + i), 1);
+            mbar_init(bar(B_HREADY + i), 16);
+            mbar_init(bar(B_HFREE + i), 1);
+            mbar_init(bar(B_SFULL + i), 1);
+            mbar_init(bar(B_SEMPTY + i), 13);
+        }
+        mbar_init(bar(B_D2FULL), 1);
+        mbar_init(bar(B_ZREADY), 16);
+        mbar_init(bar(B_AFREE), 1);
+        mbar_init(bar(B_AREADY), 8);
+        fence_barrier_init();
+        fence_proxy_async();
+    }
+    if (warp == ALLOC_WARP) tmem_alloc2(s_base + L.tmem_slot, 512);
+    for (int i = threadIdx.x; i < p.hid; i += THREADS) s_b1[i] = __ldg(p.b1 + i);
+    {
+        // the hw operand tile is only ever written in its first columns: clear it once so unread bytes are not NaNs
+        uint32_t* hwk = reinterpret_cast<uint32_t*>(smem + L.hwk);
+        for (int i = threadIdx.x; i < p.hw_ksteps * HWK_BYTES / 4; i += THREADS) hwk[i] = 0u;
+    }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();      // both CTAs' barriers are initialised before anyone arrives remotely / multicasts
+    tc_fence_after();
+    const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem + L.tmem_slot);
+    const uint32_t T_Z = tmem_base;                 // fp32 latent / GEMM2 accumulators: two 128-column N tiles
+    const uint32_t T_D1 = tmem_base + 256;          // two 128-column GEMM1 accumulators (256 hidden units each)
+
+    if (warp == PROD_WARP) {
+        // =============================================================== tile schedule + TMA producer
+        uint32_t stage = 0, ph = 0;
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            int tile = tile_of((int)it, pair, n_pairs, p.n_tiles);
+            int nsteps = 0;
+            if (tile >= 0) {
+                for (int r = lane; r < TMP; r += 32) {
+                    int cand, len, seg;
+                    row_meta(p.a, (int64_t)tile * TMP + r, cand, len, seg, rank == 0);
+                    nsteps = max(nsteps, len);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) nsteps = max(nsteps, __shfl_xor_sync(0xffffffffu, nsteps, o));
+            }
+            if (lane == 0) {
+                mbar_wait(bar(B_SEMPTY + slot), ((it >> 1) & 1) ^ 1);
+                s_sched[slot * 2 + 0] = tile;
+                s_sched[slot * 2 + 1] = nsteps;
+                mbar_arrive(bar(B_SFULL + slot));   // release semantics order the two stores before it
+            }
+            if (tile < 0) break;
+            if (lane == 0) {
+                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + SC_STAGES;
+                int src = 0;
+                for (int i = 0; i < total; ++i) {
+                    if (i == roll_total) src = ROLL_STAGES;
+                    else if (i < roll_total && src == ROLL_STAGES) src = 0;
+                    mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
+                    // the leader's barrier collects both halves of the [256 x 64] tile
+                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2 * BT_BYTES);
+                    tma_load_2sm(s_ring + stage * BT_BYTES, &tmap, 0, 128 * (2 * src + (int)rank), bar(B_FULL + stage));
+                    ++src;
+                    if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+                }
+            }
+            __syncwarp();
+        }
+    } else if (warp == MMA_WARP) {
+        // =============================================================== MMA issuer (leader CTA; the peer's warp only
+        // follows the schedule so that both CTAs' slot barriers have the same arrival count)
+        uint32_t stage = 0, ph = 0;
+        uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
+        bool pend[2] = {false, false};
+        const uint32_t s_hwk = s_base + L.hwk;
+        auto wait_h = [&](int b) {
+            if (pend[b]) {
+                mbar_wait_cluster(bar(B_HREADY + b), n_h[b] & 1);
+                ++n_h[b];
+                pend[b] = false;
+                tc_fence_after();
+            }
+        };
+        auto wait_full = [&]() {
+            mbar_wait(bar(B_FULL + stage), ph);
+            tc_fence_after();
+        };
+        auto advance = [&]() {
+            __syncwarp();
+            if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+        };
+        // one ring stage = one [256 x 64] B tile against the [64(+64) x 64] A K-block at a_tile: 4 MMAs of K = 16
+        auto stage_ss = [&](uint32_t d_tmem, uint32_t a_tile, bool first) {
+            wait_full();
+            const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + stage * BT_BYTES);
+            if (elect_one()) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) mma_ss2(d_tmem, a0 + 2u * j, b0 + 2u * j, IDESC2, (first && j == 0) ? 0u : 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // stage = the hw weight tile: hw_ksteps MMAs whose A operand is the no-swizzle [64 x 16] hw tile
+        auto stage_hw = [&](uint32_t d_tmem) {
+            wait_full();
+            const uint64_t b0 = smem_desc(s_ring + stage * BT_BYTES);
+            if (elect_one()) {
+                for (int j = 0; j < p.hw_ksteps; ++j)
+                    mma_ss2(d_tmem, smem_desc_nosw(s_hwk + j * HWK_BYTES), b0 + 2u * j, IDESC2, 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        auto commit = [&](int barrier) {
+            if (elect_one()) mma_commit2(bar(barrier));
+            __syncwarp();
+        };
+        // 256-column chunk of W [z ; a (; hw)] into accumulator b: K-blocks a/phi (8-11), [hw], z (0-7)
+        auto gemm_a1 = [&](int b, bool first_chunk, bool last_chunk, bool with_hw) {
+            wait_h(b);
+            const uint32_t d = T_D1 + 128u * b;
+            if (first_chunk) { mbar_wait_cluster(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) stage_ss(d, s_a1 + (8 + k) * KB_BYTES, k == 0);
+            if (with_hw) stage_hw(d);
+            if (last_chunk) commit(B_AFREE);
+            if (first_chunk) { mbar_wait_cluster(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
+#pragma unroll 1
+            for (int k = 0; k < 8; ++k) stage_ss(d, s_a1 + k * KB_BYTES, false);
+            commit(B_D1FULL + b);
+            pend[b] = true;
+        };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            if (rank != 0) continue;
+#pragma unroll 1
+            for (int t = 0; t < nsteps; ++t) {
+#pragma unroll 1
+                for (int i = 0; i <= NC; ++i) {
+                    if (i < NC) gemm_a1(i & 1, i == 0, i == NC - 1, false);      // GEMM1 chunk i
+                    if (i >= 1) {                                                // GEMM2 chunk i-1: Z += H[b] W2^T
+                        const int c = i - 1, b = c & 1;
+                        wait_h(b);
+#pragma unroll 1
+                        for (int kb = 0; kb < H_KB; ++kb) {
+                            stage_ss(T_Z, s_h + (b * H_KB + kb) * KB_BYTES, false);
+                            stage_ss(T_Z + 128u, s_h + (b * H_KB + kb) * KB_BYTES, false);
+                        }
+                        commit(B_HFREE + b);
+                        if (c == NC - 1) commit(B_D2FULL);
+                    }
+                }
+            }
+            // ---- scorer layer 1: four 256-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0).  Chunks 0, 1 land in the
+            // hidden buffers; chunks 2, 3 are written over A1's z K-blocks once every layer-1 MMA has completed.
+#pragma unroll 1
+            for (int c = 0; c < 4; ++c) gemm_a1(c & 1, c == 0, c == 3, true);
+            // ---- scorer layer 2, K = 1024 in K-chunks (H[0], H[1], A1 kb 0-3, A1 kb 4-7), N = 1024 in two rounds of
+            // two 256-column N tiles: round 0 into the (dead) latent columns, round 1 into the GEMM1 accumulators
+#pragma unroll 1
+            for (int round = 0; round < 2; ++round) {
+                const uint32_t d0 = round == 0 ? T_Z : T_D1;
+#pragma unroll 1
+                for (int kc = 0; kc < 4; ++kc) {
+                    if (round == 0 && kc >= 2) wait_h(kc - 2);     // h1 chunk kc written over A1 (and D1[kc-2] read)
+                    const uint32_t a_base = kc < 2 ? s_h + kc * H_KB * KB_BYTES : s_a1 + (kc - 2) * 4 * KB_BYTES;
+#pragma unroll 1
+                    for (int kb = 0; kb < 4; ++kb) {
+                        stage_ss(d0, a_base + kb * KB_BYTES, kc == 0 && kb == 0);
+                        stage_ss(d0 + 128u, a_base + kb * KB_BYTES, kc == 0 && kb == 0);
+                    }
+                    if (round == 1 && kc < 2) commit(B_HFREE + kc);
+                }
+                if (round == 0) {
+                    commit(B_D2FULL);
+                } else {
+                    commit(B_D1FULL + 0);
+                    commit(B_D1FULL + 1);
+                    pend[0] = pend[1] = true;
+                }
+            }
+        }
+        __syncwarp();
+    }
+    else if (warp >= EPI_WARP0 && warp < ACT_WARP0) {
+        // =============================================================== epilogue warps (GELU / LayerNorm / scorer)
+        const int q = warp & 3, e = (warp - EPI_WARP0) >> 2;
+        const int rh = q & 1, nh = q >> 1;
+        const int row = 32 * rh + lane;                 // row of this CTA's 64
+        const int part = 2 * nh + e;                    // this thread's 64-column quarter of every 256-column tile
+        const uint32_t lane_off = (uint32_t)(32 * q) << 16;
+        uint8_t* a1 = smem + L.a1;
+        uint8_t* hb = smem + L.hbuf;
+        const uint32_t r_hready0 = mapa(bar(B_HREADY), 0), r_hready1 = mapa(bar(B_HREADY + 1), 0);
+        const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
+        uint32_t n_d1[2] = {0, 0}, n_d2 = 0, n_hw[2] = {0, 0};
+        const float inv_d = 1.0f / (float)D;
+        // write 32 consecutive z columns of this row (N tile j, 32-column half `half` of the thread's quarter):
+        // fp32 -> TMEM, fp16 -> A1 K-block 4 j + part (when `to_smem`)
+        auto put_z = [&](int j, int half, const uint32_t (&v)[32], bool to_smem) {
+            tmem_st32(T_Z + 128u * j + 64u * e + 32u * half + lane_off, v);
+            if (to_smem) {
+                uint8_t* kb = a1 + (4 * j + part) * KB_BYTES;
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
+                    uint4 o;
+                    o.x = pack_f16(__uint_as_float(v[8 * ch + 0]), __uint_as_float(v[8 * ch + 1]));
+                    o.y = pack_f16(__uint_as_float(v[8 * ch + 2]), __uint_as_float(v[8 * ch + 3]));
+                    o.z = pack_f16(__uint_as_float(v[8 * ch + 4]), __uint_as_float(v[8 * ch + 5]));
+                    o.w = pack_f16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
+                    *reinterpret_cast<uint4*>(kb + sw128_off(row, 4 * half + ch)) = o;
+                }
+            }
+        };
+        auto publish = [&](uint32_t leader_bar, bool tmem_written) {
+            if (tmem_written) tmem_st_wait();
+            fence_proxy_async();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(leader_bar);
+        };
+        auto wait_d1 = [&](int b) {
+            mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+            ++n_d1[b];
+            tc_fence_after();
+        };
+        // bias + GELU over this thread's 64 columns of accumulator b -> fp16 row of the K-block at dst (SW128)
+        auto gelu_to_smem = [&](int b, const float* bias, bool bias_in_smem, uint8_t* dst) {
+#pragma unroll
+            for (int p2 = 0; p2 < 2; ++p2) {
+                uint32_t v[32], o[16];
+                tmem_ld32(T_D1 + 128u * b + 64u * e + 32u * p2 + lane_off, v);
+                tmem_ld_wait();
+                const float4* bp_ = reinterpret_cast<const float4*>(bias + 32 * p2);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float4 bv = bias_in_smem ? bp_[i] : __ldg(bp_ + i);
+                    o[2 * i] = gelu2_f16(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                          make_float2(bv.x, bv.y));
+                    o[2 * i + 1] = gelu2_f16(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                              make_float2(bv.z, bv.w));
+                }
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch)
+                    *reinterpret_cast<uint4*>(dst + sw128_off(row, 4 * p2 + ch)) =
+                        make_uint4(o[4 * ch], o[4 * ch + 1], o[4 * ch + 2], o[4 * ch + 3]);
+            }
+            publish(b == 0 ? r_hready0 : r_hready1, false);
+        };
+        // hidden chunk into hidden buffer b (waits until GEMM2 no longer reads the buffer's previous contents)
+        auto gelu_to_h = [&](int b, const float* bias, bool bias_in_smem) {
+            wait_d1(b);
+            mbar_wait(bar(B_HFREE + b), (n_hw[b] & 1) ^ 1);
+            ++n_hw[b];
+            gelu_to_smem(b, bias, bias_in_smem, hb + (b * H_KB + part) * KB_BYTES);
+        };
+
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand, len, seg;
+            row_meta(p.a, (int64_t)tile * TMP + TMR * (int)rank + row, cand, len, seg, false);
+
+            // ---- z_0 (the task's initial latent)
+#pragma unroll 1
+            for (int jh = 0; jh < 4; ++jh) {
+                const int j = jh >> 1, half = jh & 1;
+                const int col0 = 256 * j + 64 * part + 32 * half;
+                uint32_t v[32];
+                if (cand >= 0) {
+                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + col0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 f = __ldg(src + i);
+                        v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
+                        v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) v[i] = 0u;
+                }
+                put_z(j, half, v, true);
+            }
+            publish(r_zready, true);
+
+            for (int t = 0; t < nsteps; ++t) {
+                for (int c = 0; c < NC; ++c) gelu_to_h(c & 1, s_b1 + c * 256 + 64 * part, true);
+                // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
+                mbar_wait(bar(B_D2FULL), n_d2 & 1);
+                ++n_d2;
+                tc_fence_after();
+                float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
+#pragma unroll 1
+                for (int jh = 0; jh < 4; ++jh) {
+                    const int j = jh >> 1, half = jh & 1;
+                    const int col0 = 256 * j + 64 * part + 32 * half;
+                    uint32_t v[32];
+                    tmem_ld32(T_Z + 128u * j + 64u * e + 32u * half + lane_off, v);
+                    tmem_ld_wait();
+                    const float4* b2v = reinterpret_cast<const float4*>(p.b2 + col0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 bb = __ldg(b2v + i);
+                        const float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                                     make_float2(bb.x, bb.y));
+                        const float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                                     make_float2(bb.z, bb.w));
+                        s1v = __fadd2_rn(s1v, __fadd2_rn(x0, x1));
+                        s2v = __ffma2_rn(x0, x0, s2v);
+                        s2v = __ffma2_rn(x1, x1, s2v);
+                    }
+                }
+                s_red[part * TMR + row] = make_float2(s1v.x + s1v.y, s2v.x + s2v.y);
+                named_bar_sync(1 + rh, 128);
+                float s1 = 0.0f, s2 = 0.0f;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const float2 o = s_red[k * TMR + row];
+                    s1 += o.x; s2 += o.y;
+                }
+                const float mean = s1 * inv_d;
+                const float var = fmaxf(s2 * inv_d - mean * mean, 0.0f);
+                const float rstd = rsqrtf(var + p.ln_eps);
+                const bool live = t < len;     // masked steps leave the state unchanged
+#pragma unroll 1
+                for (int jh = 0; jh < 4; ++jh) {
+                    const int j = jh >> 1, half = jh & 1;
+                    const int col0 = 256 * j + 64 * part + 32 * half;
+                    uint32_t v[32];
+                    tmem_ld32(T_Z + 128u * j + 64u * e + 32u * half + lane_off, v);
+                    tmem_ld_wait();
+                    const float4* b2v = reinterpret_cast<const float4*>(p.b2 + col0);
+                    const float4* gv = reinterpret_cast<const float4*>(p.gamma + col0);
+                    const float4* bev = reinterpret_cast<const float4*>(p.beta + col0);
+                    const float2 rs2 = make_float2(rstd, rstd), mr2 = make_float2(-mean * rstd, -mean * rstd);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 bb = __ldg(b2v + i), gg = __ldg(gv + i), be = __ldg(bev + i);
+                        float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                               make_float2(bb.x, bb.y));
+                        float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                               make_float2(bb.z, bb.w));
+                        x0 = __ffma2_rn(__ffma2_rn(x0, rs2, mr2), make_float2(gg.x, gg.y), make_float2(be.x, be.y));
+                        x1 = __ffma2_rn(__ffma2_rn(x1, rs2, mr2), make_float2(gg.z, gg.w), make_float2(be.z, be.w));
+                        v[4 * i] = __float_as_uint(x0.x); v[4 * i + 1] = __float_as_uint(x0.y);
+                        v[4 * i + 2] = __float_as_uint(x1.x); v[4 * i + 3] = __float_as_uint(x1.y);
+                    }
+                    // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
+                    // fp32 master is never read again
+                    put_z(j, half, v, live);
+                }
+                publish(r_zready, true);
+            }
+
+            // ---- scorer layer 1 -> h1 (fp16): chunks 0, 1 into the hidden buffers ...
+            gelu_to_h(0, p.bs0 + 64 * part, false);
+            gelu_to_h(1, p.bs0 + 256 + 64 * part, false);
+            // ... chunks 2, 3 over A1's z K-blocks, once every layer-1 MMA (the readers of A1) has completed
+            wait_d1(0);
+            wait_d1(1);
+            gelu_to_smem(0, p.bs0 + 512 + 64 * part, false, a1 + part * KB_BYTES);
+            gelu_to_smem(1, p.bs0 + 768 + 64 * part, false, a1 + (4 + part) * KB_BYTES);
+            // ---- scorer layer 2 + output dot product: N tiles 0, 1 in the latent columns, 2, 3 in the accumulators
+            float acc = 0.0f;
+            auto dot32 = [&](uint32_t taddr, int n0) {
+                uint32_t v[32];
+                tmem_ld32(taddr, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 32; ++i)
+                    acc = fmaf(gelu_fast(__uint_as_float(v[i]) + __ldg(p.bs1 + n0 + i)), __ldg(p.w3 + n0 + i), acc);
+            };
+            mbar_wait(bar(B_D2FULL), n_d2 & 1);
+            ++n_d2;
+            tc_fence_after();
+#pragma unroll 1
+            for (int jh = 0; jh < 4; ++jh) {
+                const int j = jh >> 1, half = jh & 1;
+                dot32(T_Z + 128u * j + 64u * e + 32u * half + lane_off, 256 * j + 64 * part + 32 * half);
+            }
+#pragma unroll 1
+            for (int b = 0; b < 2; ++b) {
+                wait_d1(b);
+                dot32(T_D1 + 128u * b + 64u * e + lane_off, 512 + 256 * b + 64 * part);
+                dot32(T_D1 + 128u * b + 64u * e + 32u + lane_off, 512 + 256 * b + 64 * part + 32);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(b == 0 ? r_hready0 : r_hready1);
+            }
+            s_red[part * TMR + row] = make_float2(acc, 0.0f);
+            named_bar_sync(1 + rh, 128);
+            if (part == 0 && cand >= 0)
+                p.a.scores_out[cand] = (s_red[row].x + s_red[TMR + row].x) + (s_red[2 * TMR + row].x + s_red[3 * TMR + row].x) +
+                                       __ldg(p.bs2);
+            named_bar_sync(1 + rh, 128);   // s_red is reused by the next tile's first LayerNorm
+        }
+    }
+    else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
+        // =============================================================== action-embedding warps
+        // warp aw owns rows [16 aw, 16 aw + 16).  Phase 1 is row-mapped (lanes 0-15), phase 2 column-mapped (lane =
+        // 8 embedding columns = one 16-byte chunk of K-block 8 + lane / 8).
+        const int aw = warp - ACT_WARP0;
+        const int row = 16 * aw + (lane & 15);
+        const bool row_lane = lane < 16;
+        const int col8 = 8 * lane;
+        uint8_t* a1 = smem + L.a1;
+        float* s_lp = reinterpret_cast<float*>(smem + L.lp);
+        int* s_ids = reinterpret_cast<int*>(smem + L.ids);
+        int* s_lens = reinterpret_cast<int*>(smem + L.lens);
+        uint8_t* s_cnt = smem + L.cnt;
+        const uint32_t r_aready = mapa(bar(B_AREADY), 0);
+        const int P = p.P, NT = p.n_types;
+        float wp[MAX_P][8], bp8[8];
+#pragma unroll
+        for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) wp[j][c] = j < P ? __ldg(p.WpT + j * DA + col8 + c) : 0.0f;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) bp8[c] = __ldg(p.bp + col8 + c);
+        uint32_t n_w = 0;
+        auto a_dst = [&](int r) -> uint4* {
+            return reinterpret_cast<uint4*>(a1 + (8 + (lane >> 3)) * KB_BYTES + sw128_off(r, lane & 7));
+        };
+        auto e_row = [&](int id, float (&o)[8]) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4*>(p.E + (size_t)id * DA + col8));
+            o[0] = __uint_as_float(v.x << 16); o[1] = __uint_as_float(v.x & 0xffff0000u);
+            o[2] = __uint_as_float(v.y << 16); o[3] = __uint_as_float(v.y & 0xffff0000u);
+            o[4] = __uint_as_float(v.z << 16); o[5] = __uint_as_float(v.z & 0xffff0000u);
+            o[6] = __uint_as_float(v.w << 16); o[7] = __uint_as_float(v.w & 0xffff0000u);
+        };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand = -1, len = 0, seg = 0;
+            if (row_lane) {
+                row_meta(p.a, (int64_t)tile * TMP + TMR * (int)rank + row, cand, len, seg, false);
+                for (int c = 0; c < NT; ++c) s_cnt[row * NT + c] = 0;
+            }
+            float slp[MAX_P];
+#pragma unroll
+            for (int j = 0; j < MAX_P; ++j) slp[j] = 0.0f;
+
+            for (int t = 0; t < nsteps; ++t) {
+                // phase 1 (one row per lane 0-15): read the step's action, log2 of its parameters, phi statistics
+                if (row_lane) {
+                    int id = -1;
+                    float lp[MAX_P];
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                    if (t < len) {
+                        id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
+                        if (id < 0 || id >= NT) {
+                            atomicOr(p.a.fault, WM_FAULT_TYPE);
+                            id = id < 0 ? 0 : NT - 1;
+                        }
+                        const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j) {
+                            if (j < P) {
+                                int prm = __ldg(pp + j);
+                                if (prm < 1) {
+                                    atomicOr(p.a.fault, WM_FAULT_PARAM);
+                                    prm = 1;
+                                }
+                                lp[j] = log2f((float)prm);
+                                slp[j] += lp[j];
+                            }
+                        }
+                        s_cnt[row * NT + id] += 1;
+                    }
+                    s_ids[row] = id;
+                    *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
+                    *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
+                }
+                __syncwarp();
+                // store only once GEMM1 of the previous step no longer reads the a-part of A1
+                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+                ++n_w;
+                // phase 2 (8 columns per lane, loop over the warp's 16 rows): a = E[id] + W_p log2(p) + b_p
+#pragma unroll 2
+                for (int rr = 0; rr < 16; ++rr) {
+                    const int r = 16 * aw + rr;
+                    const int idr = s_ids[r];
+                    float a8[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+                    if (idr >= 0) {
+                        e_row(idr, a8);
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) a8[c] += bp8[c];
+                        const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
+                        const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
+                        const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+                            for (int c = 0; c < 8; ++c) a8[c] = fmaf(wp[j][c], lr[j], a8[c]);
+                    }
+                    *a_dst(r) = make_uint4(pack_f16(a8[0], a8[1]), pack_f16(a8[2], a8[3]), pack_f16(a8[4], a8[5]),
+                                           pack_f16(a8[6], a8[7]));
+                }
+                fence_proxy_async();
+                __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
+                if (lane == 0) mbar_arrive_cluster(r_aready);
+            }
+
+            // ---- phi = mean_t a_t = (sum_c count_c E[c] + W_p sum_t log2 p_t) / len + b_p   (0 when len = 0)
+            if (row_lane) {
+                s_lens[row] = len;
+                *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(slp[0], slp[1], slp[2], slp[3]);
+                *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(slp[4], slp[5], slp[6], slp[7]);
+            }
+            __syncwarp();
+            if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+            ++n_w;
+#pragma unroll 1
+            for (int rr = 0; rr < 16; ++rr) {
+                const int r = 16 * aw + rr;
+                const int lr_ = s_lens[r];
+                float a8[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+                if (lr_ > 0) {
+#pragma unroll 2
+                    for (int c = 0; c < NT; ++c) {
+                        const int cn_i = s_cnt[r * NT + c];
+                        if (cn_i == 0) continue;
+                        const float cn = (float)cn_i;
+                        float ev[8];
+                        e_row(c, ev);
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) a8[k] = fmaf(cn, ev[k], a8[k]);
+                    }
+                    const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
+                    const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
+                    const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) a8[k] = fmaf(wp[j][k], lr[j], a8[k]);
+                    const float inv = 1.0f / (float)lr_;
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) a8[k] = fmaf(a8[k], inv, bp8[k]);
+                }
+                *a_dst(r) = make_uint4(pack_f16(a8[0], a8[1]), pack_f16(a8[2], a8[3]), pack_f16(a8[4], a8[5]),
+                                       pack_f16(a8[6], a8[7]));
+            }
+            // hardware features of this row -> the hw operand tile (columns >= H stay zero)
+            if (row_lane) {
+                for (int ch = 0; ch < p.H / 8; ++ch) {
+                    uint4 o = make_uint4(0u, 0u, 0u, 0u);
+                    if (cand >= 0) {
+                        const float4* src = reinterpret_cast<const float4*>(p.a.hw_feats + (size_t)seg * p.H + 8 * ch);
+                        const float4 f0 = __ldg(src), f1 = __ldg(src + 1);
+                        o.x = pack_f16(f0.x, f0.y); o.y = pack_f16(f0.z, f0.w);
+                        o.z = pack_f16(f1.x, f1.y); o.w = pack_f16(f1.z, f1.w);
+                    }
+                    // K-step ch/2, K half ch&1 of the no-swizzle tile (see smem_desc_nosw)
+                    *reinterpret_cast<uint4*>(smem + L.hwk + (ch >> 1) * HWK_BYTES + (row >> 3) * 256 + (ch & 1) * 128 +
+                                              (row & 7) * 16) = o;
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(r_aready);
+        }
+    }
+
+    // ---- teardown: no CTA of the pair may exit (or free TMEM) while the other's MMAs / arrivals can still reach it
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == ALLOC_WARP) tmem_dealloc2(tmem_base, 512);
+}
+
+}  // namespace tc2
+
+// ------------------------------------------------------------------------------------------------ host side
+namespace {
+
+uint16_t f32_to_bf16(float f) {
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    u += 0x7FFFu + ((u >> 16) & 1u);   // round to nearest even (the stored values are already bf16-exact)
+    return (uint16_t)(u >> 16);
+}
+
+// Append the [256 x 64] pair tile W[n0 + n][k0 + k] (k < kvalid, else 0) as two 16 KB halves (weight rows 0-127 for
+// the leader CTA, 128-255 for its peer), each in the SW128 K-major shared-memory image.
+// Returns false when a weight is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
+bool append_pair_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid) {
+    const size_t base = blob.size();
+    blob.resize(base + 2 * tc2::BT_BYTES / 2, 0);
+    bool ok = true;
+    for (int n = 0; n < 256; ++n)
+        for (int k = 0; k < 64; ++k) {
+            const float v = k < kvalid ? W[(size_t)(n0 + n) * ld + k0 + k] : 0.0f;
+            const int nn = n & 127;
+            const size_t off = (size_t)(n >> 7) * tc2::BT_BYTES + (size_t)nn * 128 + (size_t)((((k >> 3) ^ (nn & 7)) << 4)) +
+                               (size_t)(k & 7) * 2;
+            uint16_t hb;
+            ok &= f32_to_f16_bits(v, &hb);
+            blob[base + off / 2] = hb;
+        }
+    return ok;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+bool tc2_model_ok(const Model& m) {
+    return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc2::D &&
+           m.d_a == tc2::DA && m.hidden >= 256 && m.hidden <= tc2::MAX_HID && m.hidden % 256 == 0 && m.n_lin == 3 &&
+           m.sdim[1] == tc2::SW && m.sdim[2] == tc2::SW && m.H >= 8 && m.H <= tc2::MAX_H && m.H % 8 == 0 &&
+           m.n_types <= tc2::MAX_TYPES && m.P <= tc2::MAX_P;
+}
+
+int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
+    Model& m = ctx->m;
+    if (!tc2_model_ok(m)) return WM_OK;
+    const tc2::SmemLayout L = tc2::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16);
+    if ((int)L.total > ctx->smem_optin) return WM_OK;
+    auto get = [&](const char* n) -> const std::vector<float>& {
+        for (size_t i = 0; i < names.size(); ++i)
+            if (names[i] == n) return hv[i];
+        static const std::vector<float> empty;
+        return empty;
+    };
+    const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1"), &E = get("E");
+    const int hid = m.hidden, NC = hid / 256, K1 = tc2::D + tc2::DA, K0 = K1 + m.H;
+    const size_t n_tiles = (size_t)NC * (tc2::G1_STAGES + tc2::G2_STAGES) + tc2::SC_STAGES;
+    std::vector<uint16_t> blob;
+    bool ok = true;   // every weight finite in fp16
+    blob.reserve(n_tiles * tc2::BT_BYTES);
+    for (int i = 0; i <= NC; ++i) {   // same interleave as the MMA warp: G1(i), then G2(i-1)
+        if (i < NC) {                 // GEMM1 chunk i: K-blocks a (8-11) then z (0-7)
+            for (int k = 8; k < 12; ++k) ok &= append_pair_tile(blob, W1, K1, i * 256, k * 64, 64);
+            for (int k = 0; k < 8; ++k) ok &= append_pair_tile(blob, W1, K1, i * 256, k * 64, 64);
+        }
+        if (i >= 1)                   // GEMM2 chunk i-1: hidden K-blocks x the two 256-column N tiles of d
+            for (int kb = 0; kb < 4; ++kb)
+                for (int j = 0; j < 2; ++j) ok &= append_pair_tile(blob, W2, hid, j * 256, (i - 1) * 256 + kb * 64, 64);
+    }
+    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (4), hw (1, zero-padded to 64 columns), z (8)
+        for (int k = 8; k < 12; ++k) ok &= append_pair_tile(blob, Ws0, K0, c * 256, k * 64, 64);
+        ok &= append_pair_tile(blob, Ws0, K0, c * 256, K1, m.H);
+        for (int k = 0; k < 8; ++k) ok &= append_pair_tile(blob, Ws0, K0, c * 256, k * 64, 64);
+    }
+    for (int round = 0; round < 2; ++round)   // scorer layer 2: two rounds of two N tiles over all 16 K-blocks
+        for (int kb = 0; kb < 16; ++kb)
+            for (int jj = 0; jj < 2; ++jj) ok &= append_pair_tile(blob, Ws1, tc2::SW, (2 * round + jj) * 256, kb * 64, 64);
+    if (blob.size() * 2 != n_tiles * 2 * tc2::BT_BYTES) {
+        set_error("tc2_prepare: internal weight-image size mismatch");
+        return WM_ERR_FORMAT;
+    }
+
+    if (!ok) return WM_OK;   // a weight beyond the fp16 range: this model stays on the fp32 kernel
+
+    void* d_blob = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&d_blob, blob.size() * 2));
+    ctx->allocs.push_back(d_blob);
+    WM_CUDA_TRY(cudaMemcpy(d_blob, blob.data(), blob.size() * 2, cudaMemcpyHostToDevice));
+    std::vector<uint16_t> e16(E.size());
+    for (size_t i = 0; i < E.size(); ++i) e16[i] = f32_to_bf16(E[i]);
+    void* d_e = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&d_e, e16.size() * 2 + 16));
+    ctx->allocs.push_back(d_e);
+    WM_CUDA_TRY(cudaMemcpy(d_e, e16.data(), e16.size() * 2, cudaMemcpyHostToDevice));
+
+    // tensor map over the image seen as rows of 64 bf16 (128 B); one box = 128 rows = one 16 KB half tile.  The
+    // image is already swizzled, so the map itself uses no swizzle.
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    WM_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
+    if (!fn || qr != cudaDriverEntryPointSuccess) {
+        set_error("tc2_prepare: cuTensorMapEncodeTiled is not available from this driver");
+        return WM_ERR_CUDA;
+    }
+    static_assert(sizeof(CUtensorMap) <= sizeof(m.tc2_tmap), "tensor map storage");
+    CUtensorMap tm;
+    const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
+    const cuuint64_t strides[1] = {128};
+    const cuuint32_t box[2] = {64, 128}, es[2] = {1, 1};
+    const CUresult r = ((EncodeTiledFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_blob, dims, strides, box, es,
+                                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("tc2_prepare: cuTensorMapEncodeTiled failed (%d)", (int)r);
+        return WM_ERR_CUDA;
+    }
+    memcpy(m.tc2_tmap, &tm, sizeof(tm));
+    m.tc_blob = d_blob;
+    m.tc_blob_bytes = blob.size() * 2;
+    m.tc_E = d_e;
+    WM_CUDA_TRY(cudaFuncSetAttribute(tc2::wm_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    m.tc_ok = 2;
+    return WM_OK;
+}
+
+int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
+    (void)ws;
+    const Model& m = ctx->m;
+    tc2::Params p;
+    p.hid = m.hidden; p.nc = m.hidden / 256; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
+    p.hw_ksteps = (m.H + 15) / 16;
+    p.ln_eps = m.ln_eps;
+    p.E = static_cast<const __nv_bfloat16*>(m.tc_E);
+    p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
+    p.a = a;
+    p.n_tiles = (int)((a.B + tc2::TMP - 1) / tc2::TMP);
+    CUtensorMap tm;
+    memcpy(&tm, m.tc2_tmap, sizeof(tm));
+    const tc2::SmemLayout L = tc2::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
+    const int max_pairs = ctx->n_sms / 2;
+    const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
+    tc2::wm_tc2_kernel<<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
+    WM_CUDA_TRY(cudaGetLastError());
+    ctx->launches.fetch_add(1);
+    return WM_OK;
+}
+
+}  // namespace wm

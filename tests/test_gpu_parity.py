@@ -80,7 +80,7 @@ def _edge_batch(cfg, lengths=None, S=None, per=None):
     return c, b
 
 
-@pytest.mark.parametrize("n", [1, 2, 5])
+@pytest.mark.parametrize("n", [1, 2, 3, 5])
 @pytest.mark.parametrize("case", ["B1", "B127", "B129", "B257", "len0", "lenmax", "one_long", "param_ends"])
 def test_edge_cases(wm, n, case):
     base = gen.get_config(n)
@@ -110,7 +110,7 @@ def test_edge_cases(wm, n, case):
         assert oracle.score_error(y, ref, b.subgraph_offsets) <= tol, (n, case, path)
 
 
-@pytest.mark.parametrize("n", [1, 2, 5])
+@pytest.mark.parametrize("n", [1, 2, 3, 5])
 def test_per_candidate_mode_and_segments(wm, n):
     """subgraph_offsets = NULL (per-candidate z0/hw); ragged, empty and many segments (S > #CTAs)."""
     base = gen.get_config(n)
@@ -136,7 +136,9 @@ def test_per_candidate_mode_and_segments(wm, n):
         ref2 = oracle_scores(cfg, w, b2)
         y2 = gpu_scores(ctx, b2)
         wm.wm_free(ctx)
-        assert oracle.score_error(y2, ref2, off) <= tol
+        # segments here hold 0-2 candidates, so S15's per-subgraph RMS would degenerate to |ref| (a pure relative
+        # error, unbounded for the near-zero scores of cfg 3): normalise by the batch RMS instead
+        assert oracle.score_error(y2, ref2, None) <= tol
 
 
 def test_p2_padding_invariance_bitwise(wm):
