@@ -38,6 +38,28 @@ METRIC = "candidates_scored_per_sec"
 UNIT = "candidates/s"
 
 
+def _kernel_name(info) -> str:
+    """The rollout+score kernel (K2) the library runs for this model, by its CUDA name."""
+    if info.path == 2:
+        return {1: "wm_tc_kernel", 2: "wm_tc2_kernel"}[info.tc_variant]
+    return "wm_generic_kernel"
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/*.md); keyed by (config number, kernel).  None where no capture exists yet.
+NCU_TRAFFIC = {
+    (2, "wm_tc_kernel"): (23_878_656 + 2_816, "profiles/r1_tc_v5.md"),
+}
+
+
+def _dtype_name(cfg, info) -> str:
+    """Arithmetic type of the path.  The tcgen05 kernels run kind::f16 MMAs on fp16 encodings of the bf16-valued
+    weights with fp16 activations and fp32 accumulate / latent (S14); the fp32 kernel is plain fp32."""
+    if cfg.dtype == gen.configs.DTYPE_FP32 or info.path != 2:
+        return "f32"
+    return "f16"
+
+
 def workload_name(cfg) -> str:
     return f"cfg{cfg.number}:{cfg.name} S={cfg.S} B={cfg.B} T_max={cfg.T_max} d={cfg.d} hidden={cfg.hidden} k={cfg.k}"
 
@@ -250,9 +272,11 @@ def run_ours(args, cfg):
         roof = {"bound": "hbm", "achieved": bytes_in / (k_ms * 1e-3) / 1e9, "peak": pk["hbm"], "unit": "GB/s",
                 "traffic": None, "note": "latency-bound tiny config; neither roofline applies"}
     else:
-        roof = {"bound": "tensor", "achieved": achieved, "peak": pk["bf16"], "unit": "TFLOP/s", "traffic": None}
+        tr = NCU_TRAFFIC.get((cfg.number, _kernel_name(info)))
+        roof = {"bound": "tensor", "achieved": achieved, "peak": pk["bf16"], "unit": "TFLOP/s",
+                "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof.update({"kernel": "wm_tc_kernel" if info.path == 2 else "wm_generic_kernel", "kernel_ms": k_ms,
+    roof.update({"kernel": _kernel_name(info), "kernel_ms": k_ms,
                  "peak_source": pk["source"] + " (burst: kernel timed alone)",
                  "algorithmic_flops_per_launch": flops, "share_of_step": k_ms / float(np.mean(ms))})
 
@@ -285,10 +309,12 @@ def run_ours(args, cfg):
         return
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f32" if cfg.dtype == gen.configs.DTYPE_FP32 else "bf16",
+           "vs_baseline": None, "dtype": _dtype_name(cfg, info),
            "data": "synthetic",
            "config": {"workload": workload_name(cfg), "per_gpu_batch": B, "l2": "flushed between steps (256 MB write)",
-                      "path": {1: "fp32 CUDA-core kernel", 2: "tcgen05 kernel"}[info.path],
+                      "path": _kernel_name(info),
+                      "operands": ("fp32" if _dtype_name(cfg, info) == "f32" else
+                                   "bf16-valued weights encoded as fp16 (exact), fp16 activations, fp32 accumulate + latent"),
                       "parallelism": f"dp{world} (independent batches, no collective)"},
            "rollout_steps_per_sec": steps_all / (ms_per_step * 1e-3),
            "clocks": clocks, "gpu_launches": int(launches),

@@ -273,6 +273,7 @@ int wm_get_info(const wm_ctx* ctx, wm_info* o) {
     for (int i = 0; i < 6; ++i) o->scorer_widths[i] = (i + 1 < m.n_lin) ? m.sdim[i + 1] : 0;
     o->ln_eps = m.ln_eps;
     o->path = tc_supported(ctx) ? 2 : 1;
+    o->tc_variant = tc_supported(ctx);
     return WM_OK;
 }
 

@@ -225,3 +225,31 @@ def test_host_entry_matches_device_entry(wm):
     np.testing.assert_array_equal(sc.numpy().view(np.uint32), y.view(np.uint32))
     np.testing.assert_array_equal(ix.numpy(), idx)
     wm.wm_free(ctx)
+
+
+@pytest.mark.parametrize("n", [2, 3, 4])
+def test_full_size_sampled(wm, n):
+    """BASELINE.json's full size in the launch configuration bench.py times (auto path, length bucketing on, CSR
+    segments): a sample of candidates is recomputed one by one by the oracle (a candidate's score does not depend on
+    its batch, pin P13), the error is normalised by the RMS of the sampled reference scores, and the top-k of every
+    subgraph is checked bit-exactly against a full sort of the GPU's own scores."""
+    cfg = gen.get_config(n)
+    w = gen.make_weights(cfg)
+    b = gen.make_inputs(cfg)
+    ctx = _ctx(wm, cfg)
+    assert wm.wm_get_info(ctx).path == wm.PATH_TCGEN05
+    y = gpu_scores(ctx, b)
+    wm.wm_free(ctx)
+    assert np.isfinite(y).all()
+    rng = np.random.default_rng(77 + n)
+    # sample: both ends, tile / CTA-pair boundaries, shortest and longest candidates, and random positions
+    pick = np.unique(np.concatenate([[0, 63, 64, 127, 128, b.B - 129, b.B - 1], [int(np.argmin(b.lengths)), int(np.argmax(b.lengths))],
+                                     rng.integers(0, b.B, size=119)]))
+    seg = np.searchsorted(b.subgraph_offsets, pick, side="right") - 1
+    sub = gen.Batch(b.init_states[seg], b.hw_feats[seg], b.action_ids[pick], b.action_params[pick], b.lengths[pick],
+                    np.arange(len(pick) + 1, dtype=np.int32), b.T_max)
+    ref = oracle_scores(cfg, w, sub, per_candidate=True)
+    err = oracle.score_error(y[pick], ref, None)
+    assert err <= TOL[False], (n, err)
+    idx = gpu_topk(y, b.subgraph_offsets, cfg.k)
+    np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
