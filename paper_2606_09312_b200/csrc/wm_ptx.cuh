@@ -112,6 +112,15 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         : "r"(taddr)
         : "memory");
 }
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -168,6 +177,14 @@ __device__ __forceinline__ float gelu_fast(float x) {
     const float hx = 0.5f * x;
     return fmaf(hx, t, hx);
 }
+
+// tanh / logistic sigmoid on the hardware tanh.approx (relative error 2^-11): sigma(x) = 0.5 tanh(0.5 x) + 0.5
+__device__ __forceinline__ float tanh_fast(float x) {
+    float t;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(x));
+    return t;
+}
+__device__ __forceinline__ float sigmoid_fast(float x) { return fmaf(0.5f, tanh_fast(0.5f * x), 0.5f); }
 
 // Two GELUs at once on the packed fp32x2 pipe (FFMA2/FMUL2/FADD2 halve the epilogue's FP instruction count).
 __device__ __forceinline__ uint32_t gelu2_f16(float2 acc, float2 bias) {
@@ -305,7 +322,8 @@ __device__ __forceinline__ void tma_load_2sm(uint32_t dst, const void* tmap, int
         : "memory");
 }
 // kind::f16 instruction descriptor of the pair MMA: D fp32, A/B fp16, both K-major, M = 128, N = 256
-constexpr uint32_t IDESC2 = (1u << 4) | ((256u >> 3) << 17) | ((128u >> 4) << 24);
+constexpr uint32_t idesc_pair(uint32_t n) { return (1u << 4) | ((n >> 3) << 17) | ((128u >> 4) << 24); }
+constexpr uint32_t IDESC2 = idesc_pair(256);
 
 }  // namespace ptx
 }  // namespace wm

@@ -750,7 +750,10 @@ static bool tc_model_ok(const Model& m) {
 int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
     Model& m = ctx->m;
     m.tc_ok = 0;
-    if (!tc_model_ok(m)) return tc2_prepare(ctx, hv, names);   // d = 512 models: the CTA-pair kernel
+    if (!tc_model_ok(m)) {   // d = 512 MLP+LN models and the GRU model: the CTA-pair kernels
+        const int rc = tc2_prepare(ctx, hv, names);
+        return rc != WM_OK || m.tc_ok ? rc : tcg_prepare(ctx, hv, names);
+    }
     const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16);
     if ((int)L.total > ctx->smem_optin) return WM_OK;
     auto get = [&](const char* n) -> const std::vector<float>& {
@@ -820,6 +823,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
         return launch_generic(ctx, a, st);
     }
     if (m.tc_ok == 2) return launch_tc2(ctx, ws, a, st);
+    if (m.tc_ok == 3) return launch_tcg(ctx, ws, a, st);
     tc::Params p;
     p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;

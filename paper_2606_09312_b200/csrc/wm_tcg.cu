@@ -1,0 +1,789 @@
+// K2 (tcgen05, CTA pair, gated): fused persistent rollout + score kernel for the bf16 GRU-style transition with
+// d = 384, d_a = 128 and the bucketed action-parameter table (BASELINE.json cfg 5), sm_100a only.
+//
+// PAPER.md:162 Eq.8 / :166 — z_t = F(z_{t-1}, a_t) applied recurrently; :176 — masked steps leave z unchanged;
+// :186-188 Eq.12 — y = G([z_T ; phi ; h]).  Parametrisation (BASELINE.json cfg 5, DESIGN.md §3 S10):
+//   g = sigma(W_g [z;a]),  r = sigma(W_r [z;a]),  z' = (1 - g) z + g tanh(W_h [r*z ; a]),  a = sum_j Tbl[slot_j row].
+//
+// A cluster of two CTAs owns a tile of 128 candidates, 64 rows each; the leader issues tcgen05.mma.cta_group::2 with
+// M = 128, N = 192 (d = 2 N tiles).  Per CTA, a D tile is 64 rows x 192 columns held as 128 lanes x 96 columns (lane
+// l: row l % 64, columns 96 (l / 64) ...).  Tensor memory (512 columns): the fp32 master latent (2 x 96) and three
+// 96-column accumulators X0..X2.  Per step the MMA warp issues six N tiles of K = 512 in the order
+//     R_0 -> X2, R_1 -> X1, G_0 -> X0, H_0 -> X2, H_1 -> X1, G_1 -> X0
+// (H_j needs all of r*z, i.e. both R epilogues; G_1 reuses G_0's accumulator once blend_0 has read it), while the
+// epilogue warps turn R_j into the fp16 operand r*z (shared memory) and (G_j, H_j) into z' (fp32 -> TMEM, fp16 ->
+// the OTHER of two z operand buffers: G_1 still reads the old z while z'_0 is written).  Everything else — weight
+// ring fed by TMA into both CTAs with completion on the leader's barrier, multicast commits, cluster-scope arrivals,
+// static serpentine tile schedule, scorer on the same machinery — is as in wm_tc2.cu.
+// Warp roles per CTA (512 threads): warps 0-7 epilogue (q = warp % 4: rows 32 (q & 1) + lane, N half q / 2; e = warp / 4:
+// 48-column half of the 96-column buffer), warps 8-11 action embedding (bucket-table gather), warp 12 TMEM allocator,
+// warp 13 tile schedule + TMA producer, warp 15 MMA issuer (leader CTA only).
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "wm_internal.h"
+#include "wm_ptx.cuh"
+
+namespace wm {
+
+namespace tcg {
+
+using namespace ptx;
+
+constexpr int TMP = 128;           // candidates per pair tile (MMA M)
+constexpr int TMR = 64;            // rows per CTA
+constexpr int D = 384;             // latent width
+constexpr int DA = 128;            // action-embedding width
+constexpr int SW = 768;            // scorer hidden width (both hidden layers)
+constexpr int NT = 192;            // MMA N (columns per tile)
+constexpr int XC = NT / 2;         // TMEM columns per tile and CTA
+constexpr int KB_BYTES = 8192;     // one A K-block: [64 rows x 64 cols] fp16, SW128 K-major
+constexpr int BT_BYTES = 12288;    // one B half tile: [96 weight rows x 64 cols] fp16, SW128 K-major (= ring stage)
+constexpr int NSTAGE = 4;
+constexpr int Z_KB = 6, A_KB = 2;  // K-blocks of the z part / the a (phi) part of an operand
+constexpr int ZB_BYTES = Z_KB * KB_BYTES;
+constexpr int HWK_BYTES = 2048;    // hw operand: one [64 x 16] no-swizzle K-major tile per K = 16 step
+constexpr int THREADS = 512;
+constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
+constexpr int MAX_P = 8, MAX_H = 64, MAX_BUCKETS = 64;
+constexpr int TILE_STAGES = A_KB + Z_KB;                  // ring stages of one N tile of the rollout
+constexpr int ROLL_STAGES = 6 * TILE_STAGES;              // per step
+constexpr int SC_STAGES = 4 * (A_KB + 1 + Z_KB) + 2 * 24; // scorer: layer 1 (4 x (2 phi, hw, 6 z)), layer 2 (2 rounds x 12 x 2)
+constexpr uint32_t IDESC_G = idesc_pair(NT);
+constexpr int NXB = 5;             // accumulators: X0, X1, X2 and, in the scorer, the two (dead) latent tiles
+
+enum {
+    B_FULL = 0,                    // [NSTAGE] TMA (both CTAs) -> leader's MMA warp
+    B_EMPTY = B_FULL + NSTAGE,     // [NSTAGE] MMA commit (multicast) -> each CTA's producer
+    B_XFULL = B_EMPTY + NSTAGE,    // [NXB] MMA commit -> epilogue: accumulator b filled
+    B_XFREE = B_XFULL + NXB,       // [NXB] epilogue (both CTAs) -> leader MMA: accumulator b read, its output written
+    B_ZREADY = B_XFREE + NXB,      // epilogue (both CTAs) -> leader MMA: z' (both tiles) written
+    B_AFREE,                       // MMA commit -> action warps: a-part no longer read
+    B_AREADY,                      // action warps (both CTAs) -> leader MMA: a-part written
+    B_SFULL,                       // [2] schedule slot filled (CTA-local)
+    B_SEMPTY = B_SFULL + 2,        // [2] schedule slot consumed (CTA-local)
+    B_COUNT = B_SEMPTY + 2
+};
+
+struct Params {
+    int n_types, P, n_buckets, H, hw_ksteps;
+    const __nv_bfloat16* Tbl;   // [n_types * P * n_buckets][128]
+    const float *bs0, *bs1, *w3, *bs2;
+    CallArgs a;
+    int n_tiles;
+};
+
+struct SmemLayout {
+    uint32_t zbuf, abuf, rz, ring, hwk, idx, lens, red, bars, sched, tmem_slot, total;
+};
+
+__host__ __device__ inline SmemLayout smem_layout(int hw_ksteps) {
+    SmemLayout L;
+    uint32_t o = 0;
+    L.zbuf = o; o += 2 * ZB_BYTES;                     // two fp16 z operand buffers (6 K-blocks each)
+    L.abuf = o; o += A_KB * KB_BYTES;                  // fp16 a_t / phi
+    L.rz = o; o += ZB_BYTES;                           // fp16 r*z
+    L.ring = o; o += NSTAGE * BT_BYTES;
+    L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
+    L.idx = o; o += TMR * MAX_P * 4;                   // table row of every parameter slot of the step
+    L.lens = o; o += TMR * 4;
+    L.red = o; o += 4 * TMR * 4;                       // [4 column parts][64 rows] float
+    L.bars = o; o += B_COUNT * 8;
+    L.sched = o; o += 2 * 8;
+    L.tmem_slot = o; o += 16;
+    L.total = o;
+    return L;
+}
+
+__device__ __forceinline__ int tile_of(int it, int pair, int np, int n_tiles) {
+    const int idx = it * np + ((it & 1) ? np - 1 - pair : pair);
+    return idx < n_tiles ? idx : -1;
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const SmemLayout L = smem_layout(p.hw_ksteps);
+    const uint32_t s_base = smem_u32(smem);
+    const uint32_t s_z = s_base + L.zbuf, s_a = s_base + L.abuf, s_rz = s_base + L.rz, s_ring = s_base + L.ring;
+    const uint32_t s_bars = s_base + L.bars;
+    auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
+    volatile int* s_sched = reinterpret_cast<volatile int*>(smem + L.sched);   // [2][2]: tile, nsteps
+    float* s_red = reinterpret_cast<float*>(smem + L.red);                     // [4][64]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
+    const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+
+    // ---- one-time setup
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NSTAGE; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 1); }
+        for (int i = 0; i < NXB; ++i) { mbar_init(bar(B_XFULL + i), 1); mbar_init(bar(B_XFREE + i), 16); }
+        for (int i = 0; i < 2; ++i) { mbar_init(bar(B_SFULL + i), 1); mbar_init(bar(B_SEMPTY + i), 13); }
+        mbar_init(bar(B_ZREADY), 16);
+        mbar_init(bar(B_AFREE), 1);
+        mbar_init(bar(B_AREADY), 8);
+        fence_barrier_init();
+        fence_proxy_async();
+    }
+    if (warp == ALLOC_WARP) tmem_alloc2(s_base + L.tmem_slot, 512);
+    {
+        // the hw operand tile is only ever written in its first columns: clear it once so unread bytes are not NaNs
+        uint32_t* hwk = reinterpret_cast<uint32_t*>(smem + L.hwk);
+        for (int i = threadIdx.x; i < p.hw_ksteps * HWK_BYTES / 4; i += THREADS) hwk[i] = 0u;
+    }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();      // both CTAs' barriers are initialised before anyone arrives remotely / multicasts
+    tc_fence_after();
+    const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem + L.tmem_slot);
+    const uint32_t T_Z = tmem_base;                 // fp32 latent: two 96-column tiles
+    const uint32_t T_X = tmem_base + 2 * XC;        // accumulators X0, X1, X2
+    // TMEM column base of accumulator b (3, 4 = the latent tiles, free once the rollout of a tile is over)
+    auto xcol = [&](int b) -> uint32_t { return b < 3 ? T_X + (uint32_t)(XC * b) : T_Z + (uint32_t)(XC * (b - 3)); };
+
+    if (warp == PROD_WARP) {
+        // =============================================================== tile schedule + TMA producer
+        uint32_t stage = 0, ph = 0;
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            const int tile = tile_of((int)it, pair, n_pairs, p.n_tiles);
+            int nsteps = 0;
+            if (tile >= 0) {
+                for (int r = lane; r < TMP; r += 32) {
+                    int cand, len, seg;
+                    row_meta(p.a, (int64_t)tile * TMP + r, cand, len, seg, rank == 0);
+                    nsteps = max(nsteps, len);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) nsteps = max(nsteps, __shfl_xor_sync(0xffffffffu, nsteps, o));
+            }
+            if (lane == 0) {
+                mbar_wait(bar(B_SEMPTY + slot), ((it >> 1) & 1) ^ 1);
+                s_sched[slot * 2 + 0] = tile;
+                s_sched[slot * 2 + 1] = nsteps;
+                mbar_arrive(bar(B_SFULL + slot));   // release semantics order the two stores before it
+            }
+            if (tile < 0) break;
+            if (lane == 0) {
+                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + SC_STAGES;
+                int src = 0;
+                for (int i = 0; i < total; ++i) {
+                    if (i == roll_total) src = ROLL_STAGES;
+                    else if (i < roll_total && src == ROLL_STAGES) src = 0;
+                    mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
+                    // the leader's barrier collects both halves of the [192 x 64] tile
+                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2 * BT_BYTES);
+                    tma_load_2sm(s_ring + stage * BT_BYTES, &tmap, 0, XC * (2 * src + (int)rank), bar(B_FULL + stage));
+                    ++src;
+                    if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+                }
+            }
+            __syncwarp();
+        }
+    } else if (warp == MMA_WARP) {
+        // =============================================================== MMA issuer (leader CTA; the peer's warp only
+        // follows the schedule so that both CTAs' slot barriers have the same arrival count)
+        uint32_t stage = 0, ph = 0;
+        uint32_t n_z = 0, n_a = 0;
+        uint32_t pend = 0, xpar = 0;     // per accumulator: a commit is outstanding / parity of its XFREE barrier
+        const uint32_t s_hwk = s_base + L.hwk;
+        auto wait_x = [&](int b) {       // accumulator b read by the epilogue (and that epilogue's output written)
+            if ((pend >> b) & 1u) {
+                mbar_wait_cluster(bar(B_XFREE + b), (xpar >> b) & 1u);
+                xpar ^= 1u << b;
+                pend &= ~(1u << b);
+                tc_fence_after();
+            }
+        };
+        auto wait_full = [&]() {
+            mbar_wait(bar(B_FULL + stage), ph);
+            tc_fence_after();
+        };
+        auto advance = [&]() {
+            __syncwarp();
+            if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+        };
+        // one ring stage = one [192 x 64] B tile against the [64(+64) x 64] A K-block at a_tile: 4 MMAs of K = 16
+        auto stage_ss = [&](uint32_t d_tmem, uint32_t a_tile, bool first) {
+            wait_full();
+            const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + stage * BT_BYTES);
+            if (elect_one()) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) mma_ss2(d_tmem, a0 + 2u * j, b0 + 2u * j, IDESC_G, (first && j == 0) ? 0u : 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        auto stage_hw = [&](uint32_t d_tmem) {
+            wait_full();
+            const uint64_t b0 = smem_desc(s_ring + stage * BT_BYTES);
+            if (elect_one()) {
+                for (int j = 0; j < p.hw_ksteps; ++j)
+                    mma_ss2(d_tmem, smem_desc_nosw(s_hwk + j * HWK_BYTES), b0 + 2u * j, IDESC_G, 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        auto commit = [&](int barrier) {
+            if (elect_one()) mma_commit2(bar(barrier));
+            __syncwarp();
+        };
+        auto a_part = [&](int b) {       // K-blocks a (or phi): always the first K-blocks of a tile
+            stage_ss(xcol(b), s_a, true);
+            stage_ss(xcol(b), s_a + KB_BYTES, false);
+        };
+        auto z_part = [&](int b, uint32_t zbase) {
+#pragma unroll 1
+            for (int k = 0; k < Z_KB; ++k) stage_ss(xcol(b), zbase + k * KB_BYTES, false);
+            commit(B_XFULL + b);
+            pend |= 1u << b;
+        };
+        auto wait_a = [&]() { mbar_wait_cluster(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); };
+        auto wait_z = [&]() { mbar_wait_cluster(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            if (rank != 0) continue;
+#pragma unroll 1
+            for (int t = 0; t < nsteps; ++t) {
+                const uint32_t zc = s_z + (uint32_t)(t & 1) * ZB_BYTES;     // fp16 z_t
+                wait_x(2); wait_a(); a_part(2); wait_z(); z_part(2, zc);    // R_0 -> X2
+                wait_x(1); a_part(1); z_part(1, zc);                        // R_1 -> X1
+                wait_x(0); a_part(0); z_part(0, zc);                        // G_0 -> X0
+                wait_x(2); wait_x(1);                                       // r*z complete, X2 / X1 read
+                a_part(2); z_part(2, s_rz);                                 // H_0 -> X2
+                a_part(1); z_part(1, s_rz);                                 // H_1 -> X1
+                wait_x(0);                                                  // blend_0 has read G_0
+                a_part(0); commit(B_AFREE); z_part(0, zc);                  // G_1 -> X0 (still the OLD z)
+            }
+            // ---- scorer layer 1: four 192-column tiles of gelu(Ws0 [z_T; phi; hw] + bs0) into X2, X1, X0 and latent
+            // tile 0; their fp16 outputs h1 go to the spare z buffer (tiles 0, 1) and the r*z buffer (tiles 2, 3)
+            const uint32_t zc = s_z + (uint32_t)(nsteps & 1) * ZB_BYTES;    // z_T
+            const uint32_t h1a = s_z + (uint32_t)((nsteps & 1) ^ 1) * ZB_BYTES, h1b = s_rz;
+            const int l1buf[4] = {2, 1, 0, 3};
+#pragma unroll
+            for (int n = 0; n < 4; ++n) {
+                const int b = l1buf[n];
+                wait_x(b);
+                if (n == 0) wait_a();
+                a_part(b);
+                stage_hw(xcol(b));
+                if (n == 3) commit(B_AFREE);
+                if (n == 0) wait_z();
+                z_part(b, zc);
+            }
+            // ---- scorer layer 2, K = 768 as the four h1 tiles (3 K-blocks each), N = 768 in two rounds of two
+            // 192-column tiles: round 0 into latent tile 1 and X2, round 1 into X1 and X0
+#pragma unroll
+            for (int round = 0; round < 2; ++round) {
+                const int b0 = round == 0 ? 4 : 1, b1 = round == 0 ? 2 : 0;
+                if (round == 0) wait_x(4);
+#pragma unroll 1
+                for (int kc = 0; kc < 4; ++kc) {
+                    if (round == 0) wait_x(kc == 0 ? 2 : kc == 1 ? 1 : kc == 2 ? 0 : 3);   // h1 tile kc written
+                    const uint32_t a_base = (kc < 2 ? h1a : h1b) + (uint32_t)((kc & 1) * 3) * KB_BYTES;
+#pragma unroll 1
+                    for (int kb = 0; kb < 3; ++kb) {
+                        stage_ss(xcol(b0), a_base + kb * KB_BYTES, kc == 0 && kb == 0);
+                        stage_ss(xcol(b1), a_base + kb * KB_BYTES, kc == 0 && kb == 0);
+                    }
+                }
+                commit(B_XFULL + b0);
+                commit(B_XFULL + b1);
+                pend |= (1u << b0) | (1u << b1);
+            }
+        }
+        __syncwarp();
+    }
+    else if (warp >= EPI_WARP0 && warp < ACT_WARP0) {
+        // =============================================================== epilogue warps (gates / blend / scorer)
+        const int q = warp & 3, e = (warp - EPI_WARP0) >> 2;
+        const int rh = q & 1, nh = q >> 1;
+        const int row = 32 * rh + lane;                 // row of this CTA's 64
+        const int part = 2 * nh + e;                    // this thread's 48-column quarter of every 192-column tile
+        const int cb = 48 * part;                       // first column of the quarter inside a tile
+        const uint32_t lane_off = (uint32_t)(32 * q) << 16;
+        const uint32_t tcol = 48u * e + lane_off;       // TMEM offset of the quarter inside a 96-column buffer
+        uint8_t* zb = smem + L.zbuf;
+        uint8_t* rzb = smem + L.rz;
+        const uint32_t r_xfree0 = mapa(bar(B_XFREE), 0);      // leader's XFREE[b] = r_xfree0 + 8 b
+        auto r_xfree = [&](int b) -> uint32_t { return r_xfree0 + 8u * (uint32_t)b; };
+        const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
+        uint32_t fpar = 0;                              // parity of every XFULL barrier
+        auto wait_full = [&](int b) {
+            mbar_wait(bar(B_XFULL + b), (fpar >> b) & 1u);
+            fpar ^= 1u << b;
+            tc_fence_after();
+        };
+        // 16 fp16 values of this row at column m0 (multiple of 16) of a 384-wide operand buffer (6 K-blocks)
+        auto put16 = [&](uint8_t* buf, int m0, const uint32_t (&o)[8]) {
+            uint8_t* kb = buf + (m0 >> 6) * KB_BYTES;
+            const int ch = (m0 & 63) >> 3;
+            *reinterpret_cast<uint4*>(kb + sw128_off(row, ch)) = make_uint4(o[0], o[1], o[2], o[3]);
+            *reinterpret_cast<uint4*>(kb + sw128_off(row, ch + 1)) = make_uint4(o[4], o[5], o[6], o[7]);
+        };
+        // arrive on up to two leader barriers after this warp's TMEM / shared-memory writes are visible
+        auto publish = [&](uint32_t bar_a, uint32_t bar_b, bool tmem_written) {
+            if (tmem_written) tmem_st_wait();
+            fence_proxy_async();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive_cluster(bar_a);
+                if (bar_b) mbar_arrive_cluster(bar_b);
+            }
+        };
+
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand, len, seg;
+            row_meta(p.a, (int64_t)tile * TMP + TMR * (int)rank + row, cand, len, seg, false);
+
+            // ---- z_0 (the task's initial latent) -> fp32 TMEM + fp16 buffer 0
+#pragma unroll 1
+            for (int js = 0; js < 6; ++js) {
+                const int j = js / 3, s = js % 3;
+                const int m0 = NT * j + cb + 16 * s;
+                uint32_t v[16], o[8];
+                if (cand >= 0) {
+                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + m0);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const float4 f = __ldg(src + i);
+                        v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
+                        v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) v[i] = 0u;
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i) o[i] = pack_f16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+                tmem_st16(T_Z + (uint32_t)(XC * j) + tcol + 16u * s, v);
+                put16(zb, m0, o);
+            }
+            publish(r_zready, 0u, true);
+
+            for (int t = 0; t < nsteps; ++t) {
+                uint8_t* znext = zb + ((t & 1) ^ 1) * ZB_BYTES;
+                const bool live = t < len;     // masked steps leave the state unchanged
+                // ---- r = sigma(R_j), fp16 r*z -> the r*z operand buffer (R_0 in X2, R_1 in X1)
+#pragma unroll 1
+                for (int j = 0; j < 2; ++j) {
+                    const int xb = j == 0 ? 2 : 1;
+                    wait_full(xb);
+#pragma unroll 1
+                    for (int s = 0; s < 3; ++s) {
+                        uint32_t x[16], z[16], o[8];
+                        tmem_ld16(xcol(xb) + tcol + 16u * s, x);
+                        tmem_ld16(T_Z + (uint32_t)(XC * j) + tcol + 16u * s, z);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+                            o[i] = pack_f16(sigmoid_fast(__uint_as_float(x[2 * i])) * __uint_as_float(z[2 * i]),
+                                            sigmoid_fast(__uint_as_float(x[2 * i + 1])) * __uint_as_float(z[2 * i + 1]));
+                        put16(rzb, NT * j + cb + 16 * s, o);
+                    }
+                    publish(r_xfree(xb), 0u, false);
+                }
+                // ---- z'_j = z + g (tanh(H_j) - z) = (1 - g) z + g h,  g = sigma(G_j)  (G_j in X0; H_0 in X2, H_1 in X1)
+#pragma unroll 1
+                for (int j = 0; j < 2; ++j) {
+                    const int xh = j == 0 ? 2 : 1;
+                    wait_full(0);
+                    wait_full(xh);
+#pragma unroll 1
+                    for (int s = 0; s < 3; ++s) {
+                        uint32_t g[16], h[16], z[16], o[8];
+                        tmem_ld16(xcol(0) + tcol + 16u * s, g);
+                        tmem_ld16(xcol(xh) + tcol + 16u * s, h);
+                        tmem_ld16(T_Z + (uint32_t)(XC * j) + tcol + 16u * s, z);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) {
+                            const float zf = __uint_as_float(z[i]);
+                            const float gf = sigmoid_fast(__uint_as_float(g[i]));
+                            const float hf = tanh_fast(__uint_as_float(h[i]));
+                            z[i] = __float_as_uint(live ? fmaf(gf, hf - zf, zf) : zf);
+                        }
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) o[i] = pack_f16(__uint_as_float(z[2 * i]), __uint_as_float(z[2 * i + 1]));
+                        tmem_st16(T_Z + (uint32_t)(XC * j) + tcol + 16u * s, z);
+                        put16(znext, NT * j + cb + 16 * s, o);
+                    }
+                    publish(r_xfree(0), r_xfree(xh), true);
+                }
+                // both tiles of z' are written (the arrivals above already ordered the writes)
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(r_zready);
+            }
+
+            // ---- scorer layer 1 -> h1 (fp16): tiles 0, 1 into the spare z buffer, tiles 2, 3 into the r*z buffer
+            uint8_t* h1a = zb + ((nsteps & 1) ^ 1) * ZB_BYTES;
+#pragma unroll 1
+            for (int n = 0; n < 4; ++n) {
+                const int xb = n == 0 ? 2 : n == 1 ? 1 : n == 2 ? 0 : 3;
+                wait_full(xb);
+#pragma unroll 1
+                for (int s = 0; s < 3; ++s) {
+                    uint32_t x[16], o[8];
+                    tmem_ld16(xcol(xb) + tcol + 16u * s, x);
+                    tmem_ld_wait();
+                    const int m0 = NT * n + cb + 16 * s;
+                    const float4* bp_ = reinterpret_cast<const float4*>(p.bs0 + m0);
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const float4 bv = __ldg(bp_ + i);
+                        o[2 * i] = gelu2_f16(make_float2(__uint_as_float(x[4 * i]), __uint_as_float(x[4 * i + 1])),
+                                             make_float2(bv.x, bv.y));
+                        o[2 * i + 1] = gelu2_f16(make_float2(__uint_as_float(x[4 * i + 2]), __uint_as_float(x[4 * i + 3])),
+                                                 make_float2(bv.z, bv.w));
+                    }
+                    put16(n < 2 ? h1a : rzb, (n & 1) * NT + cb + 16 * s, o);
+                }
+                publish(r_xfree(xb), 0u, false);
+            }
+            // ---- scorer layer 2 + output dot product: N tiles 0..3 arrive in latent tile 1, X2, X1, X0
+            float acc = 0.0f;
+#pragma unroll 1
+            for (int n = 0; n < 4; ++n) {
+                const int xb = n == 0 ? 4 : n == 1 ? 2 : n == 2 ? 1 : 0;
+                wait_full(xb);
+#pragma unroll 1
+                for (int s = 0; s < 3; ++s) {
+                    uint32_t x[16];
+                    tmem_ld16(xcol(xb) + tcol + 16u * s, x);
+                    tmem_ld_wait();
+                    const int n0 = NT * n + cb + 16 * s;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+                        acc = fmaf(gelu_fast(__uint_as_float(x[i]) + __ldg(p.bs1 + n0 + i)), __ldg(p.w3 + n0 + i), acc);
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(r_xfree(xb));
+            }
+            s_red[part * TMR + row] = acc;
+            named_bar_sync(1 + rh, 128);
+            if (part == 0 && cand >= 0)
+                p.a.scores_out[cand] = (s_red[row] + s_red[TMR + row]) + (s_red[2 * TMR + row] + s_red[3 * TMR + row]) +
+                                       __ldg(p.bs2);
+            named_bar_sync(1 + rh, 128);   // s_red is reused by the next tile
+        }
+    }
+    else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
+        // =============================================================== action-embedding warps
+        // warp aw owns rows [16 aw, 16 aw + 16).  Phase 1 is row-mapped (lanes 0-15: table row of every parameter
+        // slot), phase 2 column-mapped (lane = 4 embedding columns: gather P table rows per candidate row and add).
+        const int aw = warp - ACT_WARP0;
+        const int row = 16 * aw + (lane & 15);
+        const bool row_lane = lane < 16;
+        const int col4 = 4 * lane;
+        uint8_t* ab = smem + L.abuf;
+        int* s_idx = reinterpret_cast<int*>(smem + L.idx);
+        int* s_lens = reinterpret_cast<int*>(smem + L.lens);
+        const uint32_t r_aready = mapa(bar(B_AREADY), 0);
+        const int P = p.P, NB = p.n_buckets;
+        uint32_t n_w = 0;
+        auto a_dst = [&](int r) -> uint2* {
+            return reinterpret_cast<uint2*>(ab + (lane >> 4) * KB_BYTES + sw128_off(r, (lane & 15) >> 1) + (lane & 1) * 8);
+        };
+        // a (4 columns of this lane) of row r of the step whose slot rows are in s_idx; false when the row is masked
+        auto embed_row = [&](int r, float (&a4)[4]) -> bool {
+            const int4 i0 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P);
+            const int4 i1 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P + 4);
+            a4[0] = a4[1] = a4[2] = a4[3] = 0.0f;
+            if (i0.x < 0) return false;
+            const int ix[8] = {i0.x, i0.y, i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
+#pragma unroll
+            for (int j = 0; j < MAX_P; ++j) {
+                if (j < P) {
+                    const uint2 v = __ldg(reinterpret_cast<const uint2*>(p.Tbl + (size_t)ix[j] * DA + col4));
+                    a4[0] += __uint_as_float(v.x << 16);
+                    a4[1] += __uint_as_float(v.x & 0xffff0000u);
+                    a4[2] += __uint_as_float(v.y << 16);
+                    a4[3] += __uint_as_float(v.y & 0xffff0000u);
+                }
+            }
+            return true;
+        };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand = -1, len = 0, seg = 0;
+            if (row_lane) row_meta(p.a, (int64_t)tile * TMP + TMR * (int)rank + row, cand, len, seg, false);
+            float phi[16][4];
+#pragma unroll
+            for (int rr = 0; rr < 16; ++rr) phi[rr][0] = phi[rr][1] = phi[rr][2] = phi[rr][3] = 0.0f;
+
+            for (int t = 0; t < nsteps; ++t) {
+                // phase 1: table row of every parameter slot: (id P + j) n_b + bucket(p_j)
+                if (row_lane) {
+                    int ix[MAX_P];
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j) ix[j] = 0;
+                    if (t < len) {
+                        int id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
+                        if (id < 0 || id >= p.n_types) {
+                            atomicOr(p.a.fault, WM_FAULT_TYPE);
+                            id = id < 0 ? 0 : p.n_types - 1;
+                        }
+                        const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j) {
+                            if (j < P) {
+                                int prm = __ldg(pp + j);
+                                if (prm < 1) {
+                                    atomicOr(p.a.fault, WM_FAULT_PARAM);
+                                    prm = 1;
+                                }
+                                // bucket(p) = min(n_b - 1, floor(4 log2 p)) = bit_length(p^4) - 1, exact in 64-bit
+                                // integers for p < 2^16 (beyond that the bucket is saturated for n_b <= 64)
+                                unsigned long long q4 = (unsigned long long)min(prm, 65535);
+                                q4 = q4 * q4;
+                                q4 = q4 * q4;
+                                const int bk = min(63 - __clzll((long long)q4), NB - 1);
+                                ix[j] = (id * P + j) * NB + bk;
+                            }
+                        }
+                    } else {
+                        ix[0] = -1;
+                    }
+                    *reinterpret_cast<int4*>(s_idx + row * MAX_P) = make_int4(ix[0], ix[1], ix[2], ix[3]);
+                    *reinterpret_cast<int4*>(s_idx + row * MAX_P + 4) = make_int4(ix[4], ix[5], ix[6], ix[7]);
+                }
+                __syncwarp();
+                // phase 2: the first 8 rows are gathered into registers before the a-part is free, the rest after
+                uint2 pk[8];
+#pragma unroll
+                for (int rr = 0; rr < 8; ++rr) {
+                    float a4[4];
+                    if (embed_row(16 * aw + rr, a4)) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) phi[rr][c] += a4[c];
+                    }
+                    pk[rr] = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+                }
+                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+                ++n_w;
+#pragma unroll
+                for (int rr = 0; rr < 8; ++rr) *a_dst(16 * aw + rr) = pk[rr];
+#pragma unroll
+                for (int rr = 8; rr < 16; ++rr) {
+                    float a4[4];
+                    if (embed_row(16 * aw + rr, a4)) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) phi[rr][c] += a4[c];
+                    }
+                    *a_dst(16 * aw + rr) = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+                }
+                fence_proxy_async();
+                __syncwarp();   // also: phase 2 reads of s_idx are done before the next phase 1 overwrites
+                if (lane == 0) mbar_arrive_cluster(r_aready);
+            }
+
+            // ---- phi = mean_t a_t (0 when len = 0)
+            if (row_lane) s_lens[row] = len;
+            __syncwarp();
+            if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+            ++n_w;
+#pragma unroll
+            for (int rr = 0; rr < 16; ++rr) {
+                const int lr_ = s_lens[16 * aw + rr];
+                const float inv = lr_ > 0 ? 1.0f / (float)lr_ : 0.0f;
+                *a_dst(16 * aw + rr) = make_uint2(pack_f16(phi[rr][0] * inv, phi[rr][1] * inv),
+                                                  pack_f16(phi[rr][2] * inv, phi[rr][3] * inv));
+            }
+            // hardware features of this row -> the hw operand tile (columns >= H stay zero)
+            if (row_lane) {
+                for (int ch = 0; ch < p.H / 8; ++ch) {
+                    uint4 o = make_uint4(0u, 0u, 0u, 0u);
+                    if (cand >= 0) {
+                        const float4* src = reinterpret_cast<const float4*>(p.a.hw_feats + (size_t)seg * p.H + 8 * ch);
+                        const float4 f0 = __ldg(src), f1 = __ldg(src + 1);
+                        o.x = pack_f16(f0.x, f0.y); o.y = pack_f16(f0.z, f0.w);
+                        o.z = pack_f16(f1.x, f1.y); o.w = pack_f16(f1.z, f1.w);
+                    }
+                    // K-step ch/2, K half ch&1 of the no-swizzle tile (see smem_desc_nosw)
+                    *reinterpret_cast<uint4*>(smem + L.hwk + (ch >> 1) * HWK_BYTES + (row >> 3) * 256 + (ch & 1) * 128 +
+                                              (row & 7) * 16) = o;
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(r_aready);
+        }
+    }
+
+    // ---- teardown: no CTA of the pair may exit (or free TMEM) while the other's MMAs / arrivals can still reach it
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == ALLOC_WARP) tmem_dealloc2(tmem_base, 512);
+}
+
+}  // namespace tcg
+
+// ------------------------------------------------------------------------------------------------ host side
+namespace {
+
+uint16_t f32_to_bf16(float f) {
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    u += 0x7FFFu + ((u >> 16) & 1u);   // round to nearest even (the stored values are already bf16-exact)
+    return (uint16_t)(u >> 16);
+}
+
+// Append the [192 x 64] pair tile W[n0 + n][k0 + k] (k < kvalid, else 0) as two 12 KB halves (weight rows 0-95 for the
+// leader CTA, 96-191 for its peer), each in the SW128 K-major shared-memory image, fp16.  Returns false when a weight
+// is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
+bool append_pair_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid) {
+    const size_t base = blob.size();
+    blob.resize(base + 2 * tcg::BT_BYTES / 2, 0);
+    bool ok = true;
+    for (int n = 0; n < tcg::NT; ++n)
+        for (int k = 0; k < 64; ++k) {
+            const float v = k < kvalid ? W[(size_t)(n0 + n) * ld + k0 + k] : 0.0f;
+            const int nn = n % tcg::XC;
+            const size_t off = (size_t)(n / tcg::XC) * tcg::BT_BYTES + (size_t)nn * 128 +
+                               (size_t)((((k >> 3) ^ (nn & 7)) << 4)) + (size_t)(k & 7) * 2;
+            uint16_t hb;
+            ok &= f32_to_f16_bits(v, &hb);
+            blob[base + off / 2] = hb;
+        }
+    return ok;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+bool tcg_model_ok(const Model& m) {
+    return m.kind == WM_KIND_GRU && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_BUCKET && m.d == tcg::D &&
+           m.d_a == tcg::DA && m.n_lin == 3 && m.sdim[1] == tcg::SW && m.sdim[2] == tcg::SW && m.H >= 8 &&
+           m.H <= tcg::MAX_H && m.H % 8 == 0 && m.P >= 1 && m.P <= tcg::MAX_P && m.n_buckets >= 1 &&
+           m.n_buckets <= tcg::MAX_BUCKETS;
+}
+
+int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
+    Model& m = ctx->m;
+    if (!tcg_model_ok(m)) return WM_OK;
+    const tcg::SmemLayout L = tcg::smem_layout((m.H + 15) / 16);
+    if ((int)L.total > ctx->smem_optin) return WM_OK;
+    auto get = [&](const char* n) -> const std::vector<float>& {
+        for (size_t i = 0; i < names.size(); ++i)
+            if (names[i] == n) return hv[i];
+        static const std::vector<float> empty;
+        return empty;
+    };
+    const std::vector<float>&Wg = get("W_g"), &Wr = get("W_r"), &Wh = get("W_h"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1");
+    const std::vector<float>& Tbl = get("Tbl");
+    const int K1 = tcg::D + tcg::DA, K0 = K1 + m.H;
+    const size_t n_tiles = (size_t)tcg::ROLL_STAGES + tcg::SC_STAGES;
+    std::vector<uint16_t> blob;
+    bool ok = true;   // every weight finite in fp16
+    blob.reserve(n_tiles * tcg::BT_BYTES);
+    auto roll_tile = [&](const std::vector<float>& W, int j) {   // K-blocks a (6, 7) then z / r*z (0-5)
+        for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
+        for (int k = 0; k < tcg::Z_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
+    };
+    // the MMA warp's order: R_0, R_1, G_0, H_0, H_1, G_1
+    roll_tile(Wr, 0); roll_tile(Wr, 1); roll_tile(Wg, 0); roll_tile(Wh, 0); roll_tile(Wh, 1); roll_tile(Wg, 1);
+    for (int n = 0; n < 4; ++n) {     // scorer layer 1: phi (2), hw (1, zero-padded to 64 columns), z (6)
+        for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, k * 64, 64);
+        ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, K1, m.H);
+        for (int k = 0; k < tcg::Z_KB; ++k) ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, k * 64, 64);
+    }
+    for (int round = 0; round < 2; ++round)   // scorer layer 2: two rounds of two N tiles over all 12 K-blocks
+        for (int kb = 0; kb < 12; ++kb)
+            for (int jj = 0; jj < 2; ++jj) ok &= append_pair_tile(blob, Ws1, tcg::SW, (2 * round + jj) * tcg::NT, kb * 64, 64);
+    if (blob.size() * 2 != n_tiles * 2 * tcg::BT_BYTES) {
+        set_error("tcg_prepare: internal weight-image size mismatch");
+        return WM_ERR_FORMAT;
+    }
+    if (!ok) return WM_OK;   // a weight beyond the fp16 range: this model stays on the fp32 kernel
+
+    void* d_blob = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&d_blob, blob.size() * 2));
+    ctx->allocs.push_back(d_blob);
+    WM_CUDA_TRY(cudaMemcpy(d_blob, blob.data(), blob.size() * 2, cudaMemcpyHostToDevice));
+    std::vector<uint16_t> t16(Tbl.size());
+    for (size_t i = 0; i < Tbl.size(); ++i) t16[i] = f32_to_bf16(Tbl[i]);
+    void* d_t = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&d_t, t16.size() * 2 + 16));
+    ctx->allocs.push_back(d_t);
+    WM_CUDA_TRY(cudaMemcpy(d_t, t16.data(), t16.size() * 2, cudaMemcpyHostToDevice));
+
+    // tensor map over the image seen as rows of 64 fp16 (128 B); one box = 96 rows = one 12 KB half tile.  The
+    // image is already swizzled, so the map itself uses no swizzle.
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    WM_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
+    if (!fn || qr != cudaDriverEntryPointSuccess) {
+        set_error("tcg_prepare: cuTensorMapEncodeTiled is not available from this driver");
+        return WM_ERR_CUDA;
+    }
+    static_assert(sizeof(CUtensorMap) <= sizeof(m.tc2_tmap), "tensor map storage");
+    CUtensorMap tm;
+    const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
+    const cuuint64_t strides[1] = {128};
+    const cuuint32_t box[2] = {64, (cuuint32_t)tcg::XC}, es[2] = {1, 1};
+    const CUresult r = ((EncodeTiledFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, d_blob, dims, strides, box, es,
+                                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("tcg_prepare: cuTensorMapEncodeTiled failed (%d)", (int)r);
+        return WM_ERR_CUDA;
+    }
+    memcpy(m.tc2_tmap, &tm, sizeof(tm));
+    m.tc_blob = d_blob;
+    m.tc_blob_bytes = blob.size() * 2;
+    m.tc_E = d_t;
+    WM_CUDA_TRY(cudaFuncSetAttribute(tcg::wm_tcg_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    m.tc_ok = 3;
+    return WM_OK;
+}
+
+int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
+    (void)ws;
+    const Model& m = ctx->m;
+    tcg::Params p;
+    p.n_types = m.n_types; p.P = m.P; p.n_buckets = m.n_buckets; p.H = m.H;
+    p.hw_ksteps = (m.H + 15) / 16;
+    p.Tbl = static_cast<const __nv_bfloat16*>(m.tc_E);
+    p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
+    p.a = a;
+    p.n_tiles = (int)((a.B + tcg::TMP - 1) / tcg::TMP);
+    CUtensorMap tm;
+    memcpy(&tm, m.tc2_tmap, sizeof(tm));
+    const tcg::SmemLayout L = tcg::smem_layout(p.hw_ksteps);
+    const int max_pairs = ctx->n_sms / 2;
+    const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
+    tcg::wm_tcg_kernel<<<2 * pairs, tcg::THREADS, L.total, st>>>(p, tm);
+    WM_CUDA_TRY(cudaGetLastError());
+    ctx->launches.fetch_add(1);
+    return WM_OK;
+}
+
+}  // namespace wm

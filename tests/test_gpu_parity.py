@@ -227,7 +227,7 @@ def test_host_entry_matches_device_entry(wm):
     wm.wm_free(ctx)
 
 
-@pytest.mark.parametrize("n", [2, 3, 4])
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
 def test_full_size_sampled(wm, n):
     """BASELINE.json's full size in the launch configuration bench.py times (auto path, length bucketing on, CSR
     segments): a sample of candidates is recomputed one by one by the oracle (a candidate's score does not depend on
