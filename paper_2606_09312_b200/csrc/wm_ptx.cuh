@@ -42,6 +42,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+// non-blocking probe (try_wait may suspend the thread for a system-dependent time when the phase is not complete)
+__device__ __forceinline__ bool mbar_test_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
 // Bounded wait: a protocol bug must trap (and fail the test), never hang the GPU box.  The slow path is kept
 // out of line so the ~60 wait sites stay small (the kernel's code footprint matters: one warp per role, nothing
 // hides an instruction-cache miss).
@@ -57,6 +67,17 @@ static __device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (!mbar_try_wait(bar, parity)) mbar_wait_slow(bar, parity);
+}
+// the same for a CONVERGED warp whose lanes all wait on the same barrier: the vote makes the branch warp-uniform (no
+// reconvergence bookkeeping around the slow path)
+// No function call on any path (a call would force the caller's loop state out of the uniform registers): the slow
+// path spins in line and traps after ~2 s.
+__device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity) {
+    if (!__all_sync(0xffffffffu, mbar_try_wait(bar, parity))) {
+        const long long t0 = clock64();
+        while (!mbar_try_wait(bar, parity))
+            if (clock64() - t0 > 4000000000LL) __trap();
+    }
 }
 __device__ __forceinline__ void fence_barrier_init() {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -290,6 +311,13 @@ static __device__ __noinline__ void mbar_wait_cluster_slow(uint32_t bar, uint32_
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
     if (!mbar_try_wait_cluster(bar, parity)) mbar_wait_cluster_slow(bar, parity);
 }
+__device__ __forceinline__ void mbar_wait_cluster_warp(uint32_t bar, uint32_t parity) {
+    if (!__all_sync(0xffffffffu, mbar_try_wait_cluster(bar, parity))) {
+        const long long t0 = clock64();
+        while (!mbar_try_wait_cluster(bar, parity))
+            if (clock64() - t0 > 4000000000LL) __trap();
+    }
+}
 // One warp of EACH CTA of the pair (same warp id) allocates / frees; both get the same column base.
 __device__ __forceinline__ void tmem_alloc2(uint32_t slot_smem, uint32_t ncols) {
     asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(slot_smem), "r"(ncols)
@@ -321,6 +349,12 @@ __device__ __forceinline__ void tma_load_2sm(uint32_t dst, const void* tmap, int
         "l"(tmap), "r"(bar & 0xFEFFFFFFu), "r"(x), "r"(y)
         : "memory");
 }
+// low word of the SW128 K-major descriptor of a tile at shared address saddr (the high word is DESC_HI for every
+// tile); a tile `bytes` further on has low word + (bytes >> 4), the next K = 16 step inside a tile + 2
+constexpr uint32_t DESC_HI = (1024u >> 4) | (1u << 14) | (2u << 29);
+__device__ __forceinline__ uint32_t smem_desc_lo(uint32_t saddr) { return ((saddr >> 4) & 0x3FFFu) | (1u << 16); }
+__device__ __forceinline__ uint64_t desc_of(uint32_t lo) { return ((uint64_t)DESC_HI << 32) | lo; }
+
 // kind::f16 instruction descriptor of the pair MMA: D fp32, A/B fp16, both K-major, M = 128, N = 256
 constexpr uint32_t idesc_pair(uint32_t n) { return (1u << 4) | ((n >> 3) << 17) | ((128u >> 4) << 24); }
 constexpr uint32_t IDESC2 = idesc_pair(256);

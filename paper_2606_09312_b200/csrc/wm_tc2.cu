@@ -20,8 +20,8 @@
 //     consumption order; MMA completion is multicast to both CTAs' barriers (`tcgen05.commit ... multicast`);
 //   * epilogue / action warps of both CTAs arrive on the leader's barriers with cluster-scope release.
 // Warp roles per CTA (512 threads): warps 0-7 epilogue (lane quadrant q = warp % 4: rows 32 (q & 1) + lane, N half
-// q / 2; e = warp / 4: column half of the 128-column buffer), warps 8-11 action embedding, warp 12 TMEM allocator,
-// warp 13 tile schedule + TMA producer, warp 15 MMA issuer (leader CTA only).
+// q / 2; e = warp / 4: column half of the 128-column buffer), warps 8-10 and 12 action embedding, warp 11 TMEM
+// allocator, warp 13 tile schedule + TMA producer, warp 15 MMA issuer (leader CTA only).
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -50,7 +50,11 @@ constexpr int A1_KB = 12;          // z: 0-7, a/phi: 8-11
 constexpr int H_KB = 4;            // K-blocks of one hidden chunk buffer (256 columns)
 constexpr int HWK_BYTES = 2048;    // hw operand: one [64 x 16] no-swizzle K-major tile per K = 16 step
 constexpr int THREADS = 512;
-constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
+// The MMA issuer is one serial instruction stream (~70 instructions per ring stage) racing the stage's 256 tensor
+// cycles, so its scheduler (SMSP 3 = warps 3, 7, 11, 15) carries as little else as possible: the fourth action warp is
+// warp 12, and warp 11 is the TMEM allocator, idle after setup.
+constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 11, PROD_WARP = 13, MMA_WARP = 15;
+__device__ __forceinline__ int action_index(int warp) { return warp == 12 ? 3 : (warp >= 8 && warp <= 10) ? warp - 8 : -1; }
 constexpr int MAX_TYPES = 64, MAX_P = 8, MAX_H = 64, MAX_HID = 1024;
 constexpr int G1_STAGES = 12, G2_STAGES = 8;              // per 256-column hidden chunk
 constexpr int SC_STAGES = 4 * 13 + 2 * 32;                // scorer: layer 1 (4 x (4 phi, hw, 8 z)), layer 2 (2 rounds x 16 x 2)
@@ -79,7 +83,25 @@ struct Params {
     const float *bs0, *bs1, *w3, *bs2;
     CallArgs a;
     int n_tiles;
+    unsigned long long* prof;   // dev instrumentation trace buffer (WM_TC_PROFILE builds), else nullptr
 };
+
+// Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of the leader CTA of pair 0
+// appends (tag, clock) records to a trace buffer that launch_tc2 dumps.  Compiled out otherwise.
+#ifdef WM_TC_PROFILE
+constexpr int TRACE_CAP = 16384;
+#define WM_TRACE_DECL(role)                                                                            \
+    uint2* tr_buf = p.prof ? reinterpret_cast<uint2*>(p.prof) + (role) * TRACE_CAP : nullptr;           \
+    const bool tr_on = tr_buf != nullptr && blockIdx.x == 0 && lane == 0;                              \
+    uint32_t tr_n = 0;
+#define WM_TRACE(tag)                                                                                  \
+    do {                                                                                               \
+        if (tr_on && tr_n < TRACE_CAP - 1) { tr_buf[1 + tr_n] = make_uint2((uint32_t)(tag), (uint32_t)clock64()); ++tr_n; tr_buf[0].x = tr_n; } \
+    } while (0)
+#else
+#define WM_TRACE_DECL(role)
+#define WM_TRACE(tag) do { } while (0)
+#endif
 
 struct SmemLayout {
     uint32_t a1, hbuf, ring, hwk, lp, ids, lens, cnt, b1, red, bars, sched, tmem_slot, total;
@@ -166,6 +188,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     if (warp == PROD_WARP) {
         // =============================================================== tile schedule + TMA producer
         uint32_t stage = 0, ph = 0;
+        WM_TRACE_DECL(1)
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
             int tile = tile_of((int)it, pair, n_pairs, p.n_tiles);
@@ -192,7 +215,9 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int i = 0; i < total; ++i) {
                     if (i == roll_total) src = ROLL_STAGES;
                     else if (i < roll_total && src == ROLL_STAGES) src = 0;
+                    WM_TRACE(30);
                     mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
+                    WM_TRACE(31);
                     // the leader's barrier collects both halves of the [256 x 64] tile
                     if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2 * BT_BYTES);
                     tma_load_2sm(s_ring + stage * BT_BYTES, &tmap, 0, 128 * (2 * src + (int)rank), bar(B_FULL + stage));
@@ -205,44 +230,65 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     } else if (warp == MMA_WARP) {
         // =============================================================== MMA issuer (leader CTA; the peer's warp only
         // follows the schedule so that both CTAs' slot barriers have the same arrival count)
+        // Everything this warp computes with is made PROVABLY warp-uniform (a warp reduction's result lives in a uniform
+        // register): ptxas then keeps descriptors, ring state and loop counters in the uniform datapath instead of
+        // moving them there (R2UR) for every MMA — the issuing warp is one instruction stream, its latency per stage
+        // competes with the stage's 256 tensor cycles.
+        const uint32_t T_Z = __reduce_max_sync(0xffffffffu, tmem_base);
+        const uint32_t T_D1 = T_Z + 256;
         uint32_t stage = 0, ph = 0;
         uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
         bool pend[2] = {false, false};
         const uint32_t s_hwk = s_base + L.hwk;
+        WM_TRACE_DECL(0)
         auto wait_h = [&](int b) {
             if (pend[b]) {
-                mbar_wait_cluster(bar(B_HREADY + b), n_h[b] & 1);
+                WM_TRACE(10 + b);
+                mbar_wait_cluster_warp(bar(B_HREADY + b), n_h[b] & 1);
+                WM_TRACE(12 + b);
                 ++n_h[b];
                 pend[b] = false;
                 tc_fence_after();
             }
         };
-        auto wait_full = [&]() {
-            mbar_wait(bar(B_FULL + stage), ph);
+        // Ring consumer state.  `ready` = the current stage's full barrier is already known complete: it was probed
+        // (non-blocking test_wait) before the previous stage's MMAs were issued, so the probe's latency overlaps that
+        // issue instead of preceding this one.  b_lo = descriptor low word of the current ring slot.
+        const uint32_t ring_lo0 = smem_desc_lo(s_ring);
+        uint32_t b_lo = ring_lo0;
+        bool ready = false;
+        auto acquire_stage = [&]() {       // returns with the current stage's data landed; probes the next stage
+            WM_TRACE(1);
+            if (!ready) mbar_wait_warp(bar(B_FULL + stage), ph);
+            WM_TRACE(2);
             tc_fence_after();
+            const uint32_t nst = stage + 1 == NSTAGE ? 0u : stage + 1;
+            ready = __all_sync(0xffffffffu, mbar_test_wait(bar(B_FULL + nst), nst == 0 ? ph ^ 1u : ph));
         };
         auto advance = [&]() {
             __syncwarp();
-            if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+            b_lo += BT_BYTES >> 4;
+            if (++stage == NSTAGE) { stage = 0; ph ^= 1; b_lo = ring_lo0; }
         };
         // one ring stage = one [256 x 64] B tile against the [64(+64) x 64] A K-block at a_tile: 4 MMAs of K = 16
         auto stage_ss = [&](uint32_t d_tmem, uint32_t a_tile, bool first) {
-            wait_full();
-            const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + stage * BT_BYTES);
+            const uint32_t a_lo = smem_desc_lo(a_tile);
+            acquire_stage();
             if (elect_one()) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) mma_ss2(d_tmem, a0 + 2u * j, b0 + 2u * j, IDESC2, (first && j == 0) ? 0u : 1u);
+                for (int j = 0; j < 4; ++j)
+                    mma_ss2(d_tmem, desc_of(a_lo + 2u * j), desc_of(b_lo + 2u * j), IDESC2, (first && j == 0) ? 0u : 1u);
                 mma_commit2(bar(B_EMPTY + stage));
             }
+            WM_TRACE(3);
             advance();
         };
         // stage = the hw weight tile: hw_ksteps MMAs whose A operand is the no-swizzle [64 x 16] hw tile
         auto stage_hw = [&](uint32_t d_tmem) {
-            wait_full();
-            const uint64_t b0 = smem_desc(s_ring + stage * BT_BYTES);
+            acquire_stage();
             if (elect_one()) {
                 for (int j = 0; j < p.hw_ksteps; ++j)
-                    mma_ss2(d_tmem, smem_desc_nosw(s_hwk + j * HWK_BYTES), b0 + 2u * j, IDESC2, 1u);
+                    mma_ss2(d_tmem, smem_desc_nosw(s_hwk + j * HWK_BYTES), desc_of(b_lo + 2u * j), IDESC2, 1u);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
@@ -255,12 +301,12 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         auto gemm_a1 = [&](int b, bool first_chunk, bool last_chunk, bool with_hw) {
             wait_h(b);
             const uint32_t d = T_D1 + 128u * b;
-            if (first_chunk) { mbar_wait_cluster(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
+            if (first_chunk) { WM_TRACE(20); mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); }
 #pragma unroll 1
             for (int k = 0; k < 4; ++k) stage_ss(d, s_a1 + (8 + k) * KB_BYTES, k == 0);
             if (with_hw) stage_hw(d);
             if (last_chunk) commit(B_AFREE);
-            if (first_chunk) { mbar_wait_cluster(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
+            if (first_chunk) { WM_TRACE(22); mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); }
 #pragma unroll 1
             for (int k = 0; k < 8; ++k) stage_ss(d, s_a1 + k * KB_BYTES, false);
             commit(B_D1FULL + b);
@@ -268,8 +314,9 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         };
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
-            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
-            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            mbar_wait_warp(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = __reduce_max_sync(0xffffffffu, (int)s_sched[slot * 2 + 0]);
+            const int nsteps = __reduce_max_sync(0xffffffffu, (int)s_sched[slot * 2 + 1]);
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
             if (tile < 0) break;
@@ -336,6 +383,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
         uint32_t n_d1[2] = {0, 0}, n_d2 = 0, n_hw[2] = {0, 0};
         const float inv_d = 1.0f / (float)D;
+        WM_TRACE_DECL(2)
         // write 32 consecutive z columns of this row (N tile j, 32-column half `half` of the thread's quarter):
         // fp32 -> TMEM, fp16 -> A1 K-block 4 j + part (when `to_smem`)
         auto put_z = [&](int j, int half, const uint32_t (&v)[32], bool to_smem) {
@@ -390,10 +438,14 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         };
         // hidden chunk into hidden buffer b (waits until GEMM2 no longer reads the buffer's previous contents)
         auto gelu_to_h = [&](int b, const float* bias, bool bias_in_smem) {
+            WM_TRACE(40);
             wait_d1(b);
+            WM_TRACE(41);
             mbar_wait(bar(B_HFREE + b), (n_hw[b] & 1) ^ 1);
             ++n_hw[b];
+            WM_TRACE(42);
             gelu_to_smem(b, bias, bias_in_smem, hb + (b * H_KB + part) * KB_BYTES);
+            WM_TRACE(43);
         };
 
         for (uint32_t it = 0;; ++it) {
@@ -431,7 +483,9 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             for (int t = 0; t < nsteps; ++t) {
                 for (int c = 0; c < NC; ++c) gelu_to_h(c & 1, s_b1 + c * 256 + 64 * part, true);
                 // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
+                WM_TRACE(50);
                 mbar_wait(bar(B_D2FULL), n_d2 & 1);
+                WM_TRACE(51);
                 ++n_d2;
                 tc_fence_after();
                 float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
@@ -495,6 +549,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     put_z(j, half, v, live);
                 }
                 publish(r_zready, true);
+                WM_TRACE(52);
             }
 
             // ---- scorer layer 1 -> h1 (fp16): chunks 0, 1 into the hidden buffers ...
@@ -540,11 +595,11 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             named_bar_sync(1 + rh, 128);   // s_red is reused by the next tile's first LayerNorm
         }
     }
-    else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
+    else if (action_index(warp) >= 0) {
         // =============================================================== action-embedding warps
         // warp aw owns rows [16 aw, 16 aw + 16).  Phase 1 is row-mapped (lanes 0-15), phase 2 column-mapped (lane =
         // 8 embedding columns = one 16-byte chunk of K-block 8 + lane / 8).
-        const int aw = warp - ACT_WARP0;
+        const int aw = action_index(warp);
         const int row = 16 * aw + (lane & 15);
         const bool row_lane = lane < 16;
         const int col8 = 8 * lane;
@@ -857,6 +912,16 @@ int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
     p.a = a;
     p.n_tiles = (int)((a.B + tc2::TMP - 1) / tc2::TMP);
+    p.prof = nullptr;
+#ifdef WM_TC_PROFILE
+    static unsigned long long* d_prof = nullptr;
+    const size_t prof_bytes = (size_t)3 * tc2::TRACE_CAP * 8;
+    if (getenv("WM_TC_PROF")) {
+        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, prof_bytes));
+        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, prof_bytes, st));
+        p.prof = d_prof;
+    }
+#endif
     CUtensorMap tm;
     memcpy(&tm, m.tc2_tmap, sizeof(tm));
     const tc2::SmemLayout L = tc2::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
@@ -865,6 +930,20 @@ int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     tc2::wm_tc2_kernel<<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
+#ifdef WM_TC_PROFILE
+    if (p.prof) {   // dev instrumentation: dump pair 0's per-role (tag, clock) traces to WM_TC_PROF's path
+        std::vector<uint2> h((size_t)3 * tc2::TRACE_CAP);
+        WM_CUDA_TRY(cudaStreamSynchronize(st));
+        WM_CUDA_TRY(cudaMemcpy(h.data(), p.prof, h.size() * 8, cudaMemcpyDeviceToHost));
+        FILE* f = fopen(getenv("WM_TC_PROF"), "w");
+        if (f) {
+            for (int r = 0; r < 3; ++r)
+                for (uint32_t i = 0; i < h[(size_t)r * tc2::TRACE_CAP].x; ++i)
+                    fprintf(f, "%d %u %u\n", r, h[(size_t)r * tc2::TRACE_CAP + 1 + i].x, h[(size_t)r * tc2::TRACE_CAP + 1 + i].y);
+            fclose(f);
+        }
+    }
+#endif
     return WM_OK;
 }
 
