@@ -165,6 +165,12 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16
         : "memory");
 }
 
+// Register reallocation between warpgroups (4 consecutive warps; every warp of the group executes the SAME instruction):
+// the kernel is compiled for 128 registers per thread, service warps give registers back, register-hungry roles take
+// them.  N is a multiple of 8.
+template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
 // one lane of a converged warp (always the same one): keeps the MMA operands warp-uniform for the compiler
 __device__ __forceinline__ bool elect_one() {
     uint32_t pred;

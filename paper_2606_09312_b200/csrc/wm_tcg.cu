@@ -75,7 +75,25 @@ struct Params {
     const float *bs0, *bs1, *w3, *bs2;
     CallArgs a;
     int n_tiles;
+    unsigned long long* prof;   // dev instrumentation trace buffer (WM_TC_PROFILE builds), else nullptr
 };
+
+// Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of the leader CTA of pair 0
+// appends (tag, clock) records to a trace buffer that launch_tcg dumps.  Compiled out otherwise.
+#ifdef WM_TC_PROFILE
+constexpr int TRACE_CAP = 16384;
+#define WM_TRACE_DECL(role)                                                                            \
+    uint2* tr_buf = p.prof ? reinterpret_cast<uint2*>(p.prof) + (role) * TRACE_CAP : nullptr;           \
+    const bool tr_on = tr_buf != nullptr && blockIdx.x == 0 && lane == 0;                              \
+    uint32_t tr_n = 0;
+#define WM_TRACE(tag)                                                                                  \
+    do {                                                                                               \
+        if (tr_on && tr_n < TRACE_CAP - 1) { tr_buf[1 + tr_n] = make_uint2((uint32_t)(tag), (uint32_t)clock64()); ++tr_n; tr_buf[0].x = tr_n; } \
+    } while (0)
+#else
+#define WM_TRACE_DECL(role)
+#define WM_TRACE(tag) do { } while (0)
+#endif
 
 struct SmemLayout {
     uint32_t zbuf, abuf, rz, ring, hwk, idx, lens, red, bars, sched, tmem_slot, total;
@@ -193,20 +211,26 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint32_t n_z = 0, n_a = 0;
         uint32_t pend = 0, xpar = 0;     // per accumulator: a commit is outstanding / parity of its XFREE barrier
         const uint32_t s_hwk = s_base + L.hwk;
+        WM_TRACE_DECL(0)
         auto wait_x = [&](int b) {       // accumulator b read by the epilogue (and that epilogue's output written)
             if ((pend >> b) & 1u) {
+                WM_TRACE(10 + b);
                 mbar_wait_cluster(bar(B_XFREE + b), (xpar >> b) & 1u);
+                WM_TRACE(15);
                 xpar ^= 1u << b;
                 pend &= ~(1u << b);
                 tc_fence_after();
             }
         };
         auto wait_full = [&]() {
+            WM_TRACE(1);
             mbar_wait(bar(B_FULL + stage), ph);
+            WM_TRACE(2);
             tc_fence_after();
         };
         auto advance = [&]() {
             __syncwarp();
+            WM_TRACE(3);
             if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
         };
         // one ring stage = one [192 x 64] B tile against the [64(+64) x 64] A K-block at a_tile: 4 MMAs of K = 16
@@ -234,18 +258,24 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (elect_one()) mma_commit2(bar(barrier));
             __syncwarp();
         };
-        auto a_part = [&](int b) {       // K-blocks a (or phi): always the first K-blocks of a tile
-            stage_ss(xcol(b), s_a, true);
+        // A tile = its a (or phi) K-blocks and its z (or r*z, h1) K-blocks, in either order; `first` marks the segment
+        // that starts the accumulation
+        auto seg_a = [&](int b, bool first) {
+            stage_ss(xcol(b), s_a, first);
             stage_ss(xcol(b), s_a + KB_BYTES, false);
         };
-        auto z_part = [&](int b, uint32_t zbase) {
+        auto seg_z = [&](int b, uint32_t zbase, bool first) {
 #pragma unroll 1
-            for (int k = 0; k < Z_KB; ++k) stage_ss(xcol(b), zbase + k * KB_BYTES, false);
+            for (int k = 0; k < Z_KB; ++k) stage_ss(xcol(b), zbase + k * KB_BYTES, first && k == 0);
+        };
+        auto finish = [&](int b) {
             commit(B_XFULL + b);
             pend |= 1u << b;
         };
-        auto wait_a = [&]() { mbar_wait_cluster(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); };
-        auto wait_z = [&]() { mbar_wait_cluster(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); };
+        auto a_part = [&](int b) { seg_a(b, true); };
+        auto z_part = [&](int b, uint32_t zbase) { seg_z(b, zbase, false); finish(b); };
+        auto wait_a = [&]() { WM_TRACE(20); mbar_wait_cluster(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); };
+        auto wait_z = [&]() { WM_TRACE(22); mbar_wait_cluster(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); };
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
             mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
@@ -257,9 +287,11 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll 1
             for (int t = 0; t < nsteps; ++t) {
                 const uint32_t zc = s_z + (uint32_t)(t & 1) * ZB_BYTES;     // fp16 z_t
-                wait_x(2); wait_a(); a_part(2); wait_z(); z_part(2, zc);    // R_0 -> X2
-                wait_x(1); a_part(1); z_part(1, zc);                        // R_1 -> X1
-                wait_x(0); a_part(0); z_part(0, zc);                        // G_0 -> X0
+                // the first three tiles take their z K-blocks first and their a K-blocks last: a_{t+1} is written only
+                // after G_1 of step t has released the a-buffer, and its gather latency hides under these z stages
+                wait_x(2); wait_z(); seg_z(2, zc, true); wait_a(); seg_a(2, false); finish(2);   // R_0 -> X2
+                wait_x(1); seg_z(1, zc, true); seg_a(1, false); finish(1);                       // R_1 -> X1
+                wait_x(0); seg_z(0, zc, true); seg_a(0, false); finish(0);                       // G_0 -> X0
                 wait_x(2); wait_x(1);                                       // r*z complete, X2 / X1 read
                 a_part(2); z_part(2, s_rz);                                 // H_0 -> X2
                 a_part(1); z_part(1, s_rz);                                 // H_1 -> X1
@@ -572,10 +604,14 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     *reinterpret_cast<int4*>(s_idx + row * MAX_P + 4) = make_int4(ix[4], ix[5], ix[6], ix[7]);
                 }
                 __syncwarp();
-                // phase 2: the first 8 rows are gathered into registers before the a-part is free, the rest after
-                uint2 pk[8];
+                // phase 2: the first PRE rows are gathered and summed in registers BEFORE the a-part is free (the table rows
+                // come from L2; that latency sits between the a-buffer's release and the next step's first MMAs), the
+                // rest after.  PRE = 12 / 16 and a setmaxnreg hand-over of registers to these warps were measured:
+                // both spill under the kernel's 128-register cap and are slower (715 vs 794 TFLOP/s).
+                constexpr int PRE = 8;
+                uint2 pk[PRE];
 #pragma unroll
-                for (int rr = 0; rr < 8; ++rr) {
+                for (int rr = 0; rr < PRE; ++rr) {
                     float a4[4];
                     if (embed_row(16 * aw + rr, a4)) {
 #pragma unroll
@@ -586,9 +622,9 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
                 ++n_w;
 #pragma unroll
-                for (int rr = 0; rr < 8; ++rr) *a_dst(16 * aw + rr) = pk[rr];
+                for (int rr = 0; rr < PRE; ++rr) *a_dst(16 * aw + rr) = pk[rr];
 #pragma unroll
-                for (int rr = 8; rr < 16; ++rr) {
+                for (int rr = PRE; rr < 16; ++rr) {
                     float a4[4];
                     if (embed_row(16 * aw + rr, a4)) {
 #pragma unroll
@@ -704,12 +740,16 @@ int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
     blob.reserve(n_tiles * tcg::BT_BYTES);
-    auto roll_tile = [&](const std::vector<float>& W, int j) {   // K-blocks a (6, 7) then z / r*z (0-5)
-        for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
+    auto roll_tile = [&](const std::vector<float>& W, int j, bool a_first) {   // K-blocks a (6, 7) and z / r*z (0-5)
+        if (a_first)
+            for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
         for (int k = 0; k < tcg::Z_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
+        if (!a_first)
+            for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
     };
-    // the MMA warp's order: R_0, R_1, G_0, H_0, H_1, G_1
-    roll_tile(Wr, 0); roll_tile(Wr, 1); roll_tile(Wg, 0); roll_tile(Wh, 0); roll_tile(Wh, 1); roll_tile(Wg, 1);
+    // the MMA warp's order: R_0, R_1, G_0 (z K-blocks first), H_0, H_1, G_1 (a K-blocks first)
+    roll_tile(Wr, 0, false); roll_tile(Wr, 1, false); roll_tile(Wg, 0, false);
+    roll_tile(Wh, 0, true); roll_tile(Wh, 1, true); roll_tile(Wg, 1, true);
     for (int n = 0; n < 4; ++n) {     // scorer layer 1: phi (2), hw (1, zero-padded to 64 columns), z (6)
         for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, k * 64, 64);
         ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, K1, m.H);
@@ -775,6 +815,16 @@ int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
     p.a = a;
     p.n_tiles = (int)((a.B + tcg::TMP - 1) / tcg::TMP);
+    p.prof = nullptr;
+#ifdef WM_TC_PROFILE
+    static unsigned long long* d_prof = nullptr;
+    const size_t prof_bytes = (size_t)tcg::TRACE_CAP * 8;
+    if (getenv("WM_TC_PROF")) {
+        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, prof_bytes));
+        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, prof_bytes, st));
+        p.prof = d_prof;
+    }
+#endif
     CUtensorMap tm;
     memcpy(&tm, m.tc2_tmap, sizeof(tm));
     const tcg::SmemLayout L = tcg::smem_layout(p.hw_ksteps);
@@ -783,6 +833,18 @@ int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     tcg::wm_tcg_kernel<<<2 * pairs, tcg::THREADS, L.total, st>>>(p, tm);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
+#ifdef WM_TC_PROFILE
+    if (p.prof) {   // dev instrumentation: dump the leader MMA warp's (tag, clock) trace to WM_TC_PROF's path
+        std::vector<uint2> h((size_t)tcg::TRACE_CAP);
+        WM_CUDA_TRY(cudaStreamSynchronize(st));
+        WM_CUDA_TRY(cudaMemcpy(h.data(), p.prof, h.size() * 8, cudaMemcpyDeviceToHost));
+        FILE* f = fopen(getenv("WM_TC_PROF"), "w");
+        if (f) {
+            for (uint32_t i = 0; i < h[0].x; ++i) fprintf(f, "0 %u %u\n", h[1 + i].x, h[1 + i].y);
+            fclose(f);
+        }
+    }
+#endif
     return WM_OK;
 }
 
