@@ -232,12 +232,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         // stays busy only while this warp's bookkeeping per 8 MMAs (512 pipe cycles) costs less than 512 cycles:
         // one full-barrier wait and one commit per ring stage (a pair of tiles), rolled loops, nothing else.
         {
-            // The warp's state is made PROVABLY warp-uniform (a warp reduction's result lives in a uniform register) and
-            // no wait contains a call, so ptxas keeps ring state and descriptors in the uniform datapath.
-            const uint32_t T_Z = __reduce_max_sync(0xffffffffu, tmem_base);
-            const uint32_t T_D1 = T_Z + 256;
             uint32_t stage = 0, ph = 0;
-            bool ready = false;      // the current stage's full barrier was already seen complete (probed a stage ahead)
             uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
             bool pend[2] = {false, false};
             const uint32_t s_hwk = s_base + L.hwk;
@@ -245,7 +240,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             auto wait_h = [&](int b) {
                 if (pend[b]) {
                     WM_TRACE(10 + b);
-                    mbar_wait_warp(bar(B_HREADY + b), n_h[b] & 1);
+                    mbar_wait(bar(B_HREADY + b), n_h[b] & 1);
                     ++n_h[b];
                     pend[b] = false;
                     tc_fence_after();
@@ -254,11 +249,8 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             };
             auto wait_full = [&]() {
                 WM_TRACE(1);
-                if (!ready) mbar_wait_warp(bar(B_FULL + stage), ph);
+                mbar_wait(bar(B_FULL + stage), ph);
                 tc_fence_after();
-                // probe the next stage now (non-blocking): the probe's latency overlaps the MMA issue below
-                const uint32_t nst = stage + 1 == NSTAGE ? 0u : stage + 1;
-                ready = __all_sync(0xffffffffu, mbar_test_wait(bar(B_FULL + nst), nst == 0 ? ph ^ 1u : ph));
                 WM_TRACE(2);
             };
             auto release = [&]() {   // called by the elected lane after the stage's last MMA
@@ -316,10 +308,10 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             auto gemm_a1 = [&](int b, bool first_chunk, bool with_hw) {
                 wait_h(b);
                 const uint32_t d = T_D1 + 128u * b;
-                if (first_chunk) { WM_TRACE(20); mbar_wait_warp(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); }
+                if (first_chunk) { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); }
                 pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
                 if (with_hw) pair_hw(d);
-                if (first_chunk) { WM_TRACE(22); mbar_wait_warp(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); }
+                if (first_chunk) { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); }
                 pair_ss(d, s_a1, s_a1 + TILE_BYTES, false);
                 pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
                 commit(B_D1FULL + b);
@@ -327,9 +319,8 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             };
             for (uint32_t it = 0;; ++it) {
                 const uint32_t slot = it & 1;
-                mbar_wait_warp(bar(B_SFULL + slot), (it >> 1) & 1);
-                const int tile = __reduce_max_sync(0xffffffffu, (int)s_sched[slot * 2 + 0]);
-                const int nsteps = __reduce_max_sync(0xffffffffu, (int)s_sched[slot * 2 + 1]);
+                mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+                const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
                 if (tile < 0) break;
