@@ -243,6 +243,8 @@ __device__ __forceinline__ uint64_t smem_desc_nosw(uint32_t saddr) {
 // kind::f16 instruction descriptor: D fp32 (bit 4), A/B fp16 (format fields [7,10) and [10,13) = 0; 1 would be bf16),
 // both K-major, M = 128, N = 128.
 constexpr uint32_t IDESC = (1u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+// the same with N = 256 (one MMA = 128 tensor cycles: half the issue work per FLOP of N = 128)
+constexpr uint32_t IDESC_N256 = (1u << 4) | ((256u >> 3) << 17) | ((128u >> 4) << 24);
 
 // ------------------------------------------------------------------------------------------------ tile helpers
 __device__ __forceinline__ int find_seg(const int32_t* __restrict__ off, int S, int cand) {

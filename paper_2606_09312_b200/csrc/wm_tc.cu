@@ -299,6 +299,20 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 }
                 advance();
             };
+            // stage = ONE [256 x 64] B tile (the two adjacent [128 x 64] tiles of a stage are exactly that: row n at
+            // n * 128 B, same swizzle) against the TMEM A operand a_tmem into the 256-column accumulator d: 4 MMAs with
+            // N = 256 instead of 8 with N = 128.  The issuing warp, not the tensor pipe, bounds this kernel, and an
+            // N = 256 MMA carries twice the work per issued instruction.
+            auto stage_ts256 = [&](uint32_t d, uint32_t a_tmem) {
+                wait_full();
+                const uint64_t b0 = smem_desc(s_ring + stage * STAGE_BYTES);
+                if (elect_one()) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) mma_ts(d, a_tmem + 8u * j, b0 + 2u * j, IDESC_N256, 1u);
+                    release();
+                }
+                advance();
+            };
             auto commit = [&](int barrier) {
                 if (elect_one()) mma_commit(bar(barrier));
                 __syncwarp();
@@ -336,8 +350,8 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                             const int c = i - 1, b = c & 1;
                             wait_h(b);
                             const uint32_t hbuf = T_D1 + 128u * b;
-                            pair_ts(T_Z, T_Z + 128u, hbuf, hbuf, false);
-                            pair_ts(T_Z, T_Z + 128u, hbuf + 64u, hbuf + 64u, false);
+                            stage_ts256(T_Z, hbuf);            // K-block 0 of the chunk x all 256 latent columns
+                            stage_ts256(T_Z, hbuf + 64u);      // K-block 1
                             if (c == NC - 1) commit(B_D2FULL);
                         }
                     }
