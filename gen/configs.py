@@ -8,7 +8,7 @@ from __future__ import annotations
 from dataclasses import dataclass, field, replace
 from typing import Tuple
 
-KIND_MLP, KIND_MLP_LN, KIND_GRU = 0, 1, 2
+KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH = 0, 1, 2, 3
 DTYPE_FP32, DTYPE_BF16 = 0, 1
 EMBED_LINEAR, EMBED_BUCKET = 0, 1
 
@@ -16,7 +16,7 @@ EMBED_LINEAR, EMBED_BUCKET = 0, 1
 @dataclass(frozen=True)
 class WMConfig:
     name: str
-    number: int                 # 1..5 (BASELINE.json configs[number-1])
+    number: int                 # 1..5 (BASELINE.json configs[number-1]); 6, 7 = NEXT row f1
     kind: int                   # KIND_*
     dtype: int                  # DTYPE_*
     embed: int                  # EMBED_*
@@ -64,6 +64,8 @@ class WMConfig:
         """Literal transition FLOP per rollout step."""
         if self.kind == KIND_GRU:
             return 2 * 3 * self.d * (self.d + self.d_a)
+        if self.kind == KIND_TRANSH:   # W_w a, W_d a, then the residual MLP (the projection / norms are O(d))
+            return 2 * (2 * self.d * self.d_a + self.hidden * (self.d + self.d_a) + self.d * self.hidden)
         return 2 * (self.hidden * (self.d + self.d_a) + self.d * self.hidden)
 
     def flops_scorer(self) -> int:
@@ -89,6 +91,14 @@ CONFIGS = {
     5: WMConfig("cfg5_gated", 5, KIND_GRU, DTYPE_BF16, EMBED_BUCKET, S=128, per_subgraph=16384, T_max=64,
                 len_dist="uniform", len_lo=16, len_hi=64, n_types=32, P=8, param_dist="loguniform",
                 param_hi=1024, n_buckets=40, d=384, d_a=128, hidden=0, H=32, scorer_widths=(768, 768), k=64),
+    # NEXT row f1: the paper's TransH-style transition, not a BASELINE.json config.
+    # 6 = cfg 1's shapes (fp32, the parity case), 7 = cfg 2's shapes and batch (the measurement case).
+    6: WMConfig("f1_transh_tiny_fp32", 6, KIND_TRANSH, DTYPE_FP32, EMBED_LINEAR, S=1, per_subgraph=64, T_max=8,
+                len_dist="uniform", len_lo=0, len_hi=8, n_types=16, P=4, param_dist="uniform", param_hi=64,
+                n_buckets=0, d=64, d_a=32, hidden=128, H=8, scorer_widths=(128,), k=8),
+    7: WMConfig("f1_transh_evolution_round", 7, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, S=16, per_subgraph=2048,
+                T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
+                param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(512, 512), k=64),
 }
 
 

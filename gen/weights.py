@@ -14,7 +14,7 @@ from typing import Dict, List
 
 import numpy as np
 
-from .configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, DTYPE_BF16, EMBED_LINEAR, EMBED_BUCKET)
+from .configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, EMBED_BUCKET)
 
 MAGIC = b"WMW1"
 VERSION = 1
@@ -40,6 +40,8 @@ def tensor_order(cfg: WMConfig) -> List[str]:
         names += ["W1", "b1", "W2", "b2"]
         if cfg.kind == KIND_MLP_LN:
             names += ["gamma", "beta"]
+    elif cfg.kind == KIND_TRANSH:      # hyperplane normal, translation, then the residual MLP
+        names += ["W_w", "W_d", "W1", "b1", "W2", "b2"]
     else:
         names += ["W_g", "W_r", "W_h"]
     for i in range(len(cfg.scorer_widths) + 1):
@@ -56,7 +58,10 @@ def tensor_shapes(cfg: WMConfig) -> Dict[str, tuple]:
         sh["b_p"] = (da,)
     else:
         sh["Tbl"] = (cfg.n_types * cfg.P * cfg.n_buckets, da)
-    if cfg.kind in (KIND_MLP, KIND_MLP_LN):
+    if cfg.kind == KIND_TRANSH:
+        sh["W_w"] = (d, da)
+        sh["W_d"] = (d, da)
+    if cfg.kind in (KIND_MLP, KIND_MLP_LN, KIND_TRANSH):
         sh["W1"] = (hid, d + da)
         sh["b1"] = (hid,)
         sh["W2"] = (d, hid)

@@ -30,7 +30,7 @@ from typing import Dict, Optional, Tuple
 import numpy as np
 from scipy.special import erf as _erf
 
-KIND_MLP, KIND_MLP_LN, KIND_GRU = 0, 1, 2
+KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH = 0, 1, 2, 3
 EMBED_LINEAR, EMBED_BUCKET = 0, 1
 F64 = np.float64
 
@@ -109,6 +109,28 @@ def step_gru(z, a, W_g, W_r, W_h) -> np.ndarray:
     return (1.0 - g) * z + g * h
 
 
+TRANSH_EPS = 1e-12   # added under both square roots of step_transh (DESIGN.md §3 S24)
+
+
+def step_transh(z, a, W_w, W_d, W1, b1, W2, b2, eps: float = TRANSH_EPS) -> np.ndarray:
+    """The paper's TransH-based predictor (ref [41]; NEXT row f1, reading S24), in its three stated stages:
+      1. "the current state is first transformed in an action-conditioned geometric space": the action defines a
+         hyperplane with unit normal w = W_w a / sqrt(|W_w a|^2 + eps); the state is projected onto it,
+         z_perp = z - (w.z) w, and translated inside it by d = W_d a (TransH: h_perp + d_r);
+      2. "then combined with the action embedding through a residual multilayer transformation":
+         v = x + W2 gelu(W1 [x ; a] + b1) + b2 with x = z_perp + d;
+      3. "and finally normalized": z' = v / sqrt(|v|^2 + eps)  (the losses live in the normalized
+         state-representation space)."""
+    W_w, W_d = np.asarray(W_w, F64), np.asarray(W_d, F64)
+    u = a @ W_w.T
+    w = u / np.sqrt(np.sum(u * u, axis=-1, keepdims=True) + eps)
+    z_perp = z - np.sum(w * z, axis=-1, keepdims=True) * w
+    x = z_perp + a @ W_d.T
+    h = gelu(np.concatenate([x, a], axis=-1) @ np.asarray(W1, F64).T + np.asarray(b1, F64))
+    v = x + h @ np.asarray(W2, F64).T + np.asarray(b2, F64)
+    return v / np.sqrt(np.sum(v * v, axis=-1, keepdims=True) + eps)
+
+
 def scorer(x: np.ndarray, w: Dict[str, np.ndarray], n_layers: int) -> np.ndarray:
     """G as an MLP: hidden linears followed by GELU, last linear plain (S8). Returns [...]."""
     for i in range(n_layers):
@@ -128,6 +150,8 @@ def _n_scorer_layers(w) -> int:
 def _kind(w) -> int:
     if "W_g" in w:
         return KIND_GRU
+    if "W_w" in w:
+        return KIND_TRANSH
     return KIND_MLP_LN if "gamma" in w else KIND_MLP
 
 
@@ -141,6 +165,8 @@ def _step(w, z, a, eps):
     k = _kind(w)
     if k == KIND_GRU:
         return step_gru(z, a, w["W_g"], w["W_r"], w["W_h"])
+    if k == KIND_TRANSH:
+        return step_transh(z, a, w["W_w"], w["W_d"], w["W1"], w["b1"], w["W2"], w["b2"])
     if k == KIND_MLP_LN:
         return step_mlp(z, a, w["W1"], w["b1"], w["W2"], w["b2"], w["gamma"], w["beta"], eps)
     return step_mlp(z, a, w["W1"], w["b1"], w["W2"], w["b2"])
@@ -244,6 +270,18 @@ def rollout_score_scalar(w, init_states, action_ids, action_params, lengths, hw_
                 r = [sig(u) for u in mv(W["W_r"], x)]
                 hcand = [math.tanh(u) for u in mv(W["W_h"], [ri * zi for ri, zi in zip(r, z)] + a)]
                 z = [(1.0 - gi) * zi + gi * hi for gi, zi, hi in zip(g, z, hcand)]
+            elif kind == KIND_TRANSH:
+                # PAPER.md:164 in its three stages (see step_transh): project onto the action's hyperplane and
+                # translate, residual MLP with the action embedding, L2-normalise
+                uw = mv(W["W_w"], a)
+                nw = math.sqrt(sum(x * x for x in uw) + TRANSH_EPS)
+                wn = [x / nw for x in uw]
+                dot = sum(wi * zi for wi, zi in zip(wn, z))
+                xs = [zi - dot * wi + di for zi, wi, di in zip(z, wn, mv(W["W_d"], a))]
+                hdn = [gelu1(ui + bi) for ui, bi in zip(mv(W["W1"], xs + a), W["b1"])]
+                v = [xi + wi + bi for xi, wi, bi in zip(xs, mv(W["W2"], hdn), W["b2"])]
+                nv = math.sqrt(sum(x * x for x in v) + TRANSH_EPS)
+                z = [x / nv for x in v]
             else:
                 u = [ui + bi for ui, bi in zip(mv(W["W1"], z + a), W["b1"])]
                 hdn = [gelu1(ui) for ui in u]
@@ -353,6 +391,9 @@ def read_weight_file(path: str):
         take("W1", hidden, d + d_a); take("b1", hidden); take("W2", d, hidden); take("b2", d)
         if kind == KIND_MLP_LN:
             take("gamma", d); take("beta", d)
+    elif kind == KIND_TRANSH:
+        take("W_w", d, d_a); take("W_d", d, d_a)
+        take("W1", hidden, d + d_a); take("b1", hidden); take("W2", d, hidden); take("b2", d)
     else:
         take("W_g", d, d + d_a); take("W_r", d, d + d_a); take("W_h", d, d + d_a)
     dims = [d + d_a + H] + widths + [1]

@@ -31,6 +31,20 @@ def main():
     h = [math.tanh(rz[0] + rz[1] + 0.5), math.tanh(rz[0] - rz[1] + 1.0)]
     zn = [(1 - gate[i]) * z[i] + gate[i] * h[i] for i in range(2)]
     print("p6 g", gate, "r", r, "h", h, "z'", zn)
+    # P14 (TransH step, PAPER.md:164 / DESIGN.md S24): z=[3,4], a=[2], W_w=[[1],[0]], W_d=[[.5],[-1]], eps=1e-12
+    eps = 1e-12
+    uw = [2.0, 0.0]
+    nw = math.sqrt(uw[0] ** 2 + uw[1] ** 2 + eps)
+    w = [uw[0] / nw, uw[1] / nw]
+    dot = w[0] * 3.0 + w[1] * 4.0
+    x = [3.0 - dot * w[0] + 1.0, 4.0 - dot * w[1] - 2.0]          # z_perp + W_d a  (= [1, 2] up to eps)
+    # W1=[[1,0,-1.25],[2,1,-.5]], b1=[0,0] => u = [x0 - 2.5, 2 x0 + x1 - 1] (= [-1.5, 3] up to eps)
+    u = [x[0] - 2.5, 2 * x[0] + x[1] - 1.0]
+    phi = lambda t: 0.5 * (1.0 + math.erf(t / math.sqrt(2.0)))
+    g = [u[0] * phi(u[0]), u[1] * phi(u[1])]
+    v = [x[0] + g[0] + g[1] + 0.25, x[1] + 2 * g[1] - 0.5]        # W2=[[1,1],[0,2]], b2=[.25,-.5]
+    nv = math.sqrt(v[0] ** 2 + v[1] ** 2 + eps)
+    print("p14 x", x, "v", v, "z'", [v[0] / nv, v[1] / nv])
 
 
 if __name__ == "__main__":

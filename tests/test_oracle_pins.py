@@ -12,7 +12,8 @@ import torch
 
 import gen
 import oracle
-from gen.configs import WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, DTYPE_FP32, EMBED_LINEAR, EMBED_BUCKET
+from gen.configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH, DTYPE_FP32, EMBED_LINEAR,
+                         EMBED_BUCKET)
 
 
 def tiny_cfg(kind=KIND_MLP_LN, embed=EMBED_LINEAR, S=3, n=7, T=5, d=6, da=4, hid=8, H=3, widths=(5, 4),
@@ -29,7 +30,7 @@ def run_vec(cfg, w, b, **kw):
 
 
 ALL_KINDS = [(KIND_MLP, EMBED_LINEAR), (KIND_MLP_LN, EMBED_LINEAR), (KIND_GRU, EMBED_BUCKET),
-             (KIND_GRU, EMBED_LINEAR), (KIND_MLP_LN, EMBED_BUCKET)]
+             (KIND_GRU, EMBED_LINEAR), (KIND_MLP_LN, EMBED_BUCKET), (KIND_TRANSH, EMBED_LINEAR)]
 
 
 # ---- P4 / P5 / P6 / P11: hand-expanded fixtures ---------------------------------------------------
@@ -59,6 +60,61 @@ def test_p6_gru_step_hand_expanded(golden):
     z = np.array([[1.0, -2.0]]); a = np.array([[0.5]])
     W_g = [[1, 0, 2], [0, 1, -2]]; W_r = [[0, 1, 0], [1, 0, 0]]; W_h = [[1, 1, 1], [1, -1, 2]]
     np.testing.assert_allclose(oracle.step_gru(z, a, W_g, W_r, W_h)[0], g["z_next"], rtol=0, atol=1e-14)
+
+
+def test_p14_transh_step_hand_expanded(golden):
+    g = golden("p14_transh_step.txt")
+    z = np.array([[3.0, 4.0]]); a = np.array([[2.0]])
+    Ww = [[1.0], [0.0]]; Wd = [[0.5], [-1.0]]
+    W1 = [[1, 0, -1.25], [2, 1, -0.5]]; b1 = [0.0, 0.0]; W2 = [[1, 1], [0, 2]]; b2 = [0.25, -0.5]
+    out = oracle.step_transh(z, a, Ww, Wd, W1, b1, W2, b2)[0]
+    np.testing.assert_allclose(out, g["z_next"], rtol=0, atol=1e-14)
+    # the fixture discriminates: no projection, no translation, a transposed W2 or no normalisation must each fail
+    assert np.abs(oracle.step_transh(z, a, [[0.0], [1.0]], Wd, W1, b1, W2, b2)[0] - g["z_next"]).max() > 1e-2
+    assert np.abs(oracle.step_transh(z, a, Ww, [[0.0], [0.0]], W1, b1, W2, b2)[0] - g["z_next"]).max() > 1e-2
+    assert np.abs(oracle.step_transh(z, a, Ww, Wd, W1, b1, np.array(W2).T, b2)[0] - g["z_next"]).max() > 1e-2
+    assert abs(np.linalg.norm(g["v"]) - 1.0) > 1.0
+
+
+def test_p15_transh_closed_forms():
+    rng = np.random.default_rng(15)
+    d, da, hid, n = 7, 3, 5, 6
+    z = rng.standard_normal((n, d)); a = rng.standard_normal((n, da))
+    Ww = rng.standard_normal((d, da)); Wd = rng.standard_normal((d, da))
+    W1 = rng.standard_normal((hid, d + da)); b1 = rng.standard_normal(hid)
+    W2 = rng.standard_normal((d, hid)); b2 = rng.standard_normal(d)
+    Z0 = np.zeros_like
+    # (a) the result is always a unit vector ("finally normalized")
+    np.testing.assert_allclose(np.linalg.norm(oracle.step_transh(z, a, Ww, Wd, W1, b1, W2, b2), axis=1), 1.0, atol=1e-12)
+    # (b) no translation, no MLP: z' is the normalised projection onto the hyperplane, orthogonal to its normal
+    zp = oracle.step_transh(z, a, Ww, Z0(Wd), W1, b1, Z0(W2), Z0(b2))
+    np.testing.assert_allclose(np.sum(zp * (a @ Ww.T), axis=1), 0.0, atol=1e-12)
+    # ... and equals (I - w w^T) z / |.| computed with a projection matrix (library linear algebra)
+    for i in range(n):
+        w = Ww @ a[i]; w = w / np.linalg.norm(w)
+        ref = (np.eye(d) - np.outer(w, w)) @ z[i]
+        np.testing.assert_allclose(zp[i], ref / np.linalg.norm(ref), atol=1e-11)
+    # (c) the projection is idempotent: the same action again leaves the (unit, in-plane) state unchanged
+    np.testing.assert_allclose(oracle.step_transh(zp, a, Ww, Z0(Wd), W1, b1, Z0(W2), Z0(b2)), zp, atol=1e-11)
+    # (d) TransH proper: without the MLP, v = z_perp + d_r (Wang et al.: h_perp + d_r), up to the final normalisation
+    v = oracle.step_transh(z, a, Ww, Wd, W1, b1, Z0(W2), Z0(b2))
+    for i in range(n):
+        w = Ww @ a[i]; w = w / np.linalg.norm(w)
+        ref = z[i] - (w @ z[i]) * w + Wd @ a[i]
+        np.testing.assert_allclose(v[i], ref / np.linalg.norm(ref), atol=1e-11)
+    # (e) a state already orthogonal to the normal is only normalised
+    zo = z - np.sum(z * (a @ Ww.T), axis=1, keepdims=True) * (a @ Ww.T) / np.sum((a @ Ww.T) ** 2, axis=1, keepdims=True)
+    np.testing.assert_allclose(oracle.step_transh(zo, a, Ww, Z0(Wd), W1, b1, Z0(W2), Z0(b2)),
+                               zo / np.linalg.norm(zo, axis=1, keepdims=True), atol=1e-11)
+    # (f) library cross-check of the full step with torch float64 (gelu, normalize)
+    zt, at = torch.from_numpy(z), torch.from_numpy(a)
+    u = at @ torch.from_numpy(Ww).T
+    wt = torch.nn.functional.normalize(u, dim=1, eps=0.0)
+    xt = zt - (wt * zt).sum(1, keepdim=True) * wt + at @ torch.from_numpy(Wd).T
+    ht = torch.nn.functional.gelu(torch.cat([xt, at], 1) @ torch.from_numpy(W1).T + torch.from_numpy(b1))
+    vt = xt + ht @ torch.from_numpy(W2).T + torch.from_numpy(b2)
+    np.testing.assert_allclose(oracle.step_transh(z, a, Ww, Wd, W1, b1, W2, b2),
+                               torch.nn.functional.normalize(vt, dim=1, eps=0.0).numpy(), atol=1e-11)
 
 
 def test_p11_bucket_function(golden):
@@ -296,7 +352,7 @@ def test_p12_prefix_reuse_equals_scratch():
 # ---- generator / file format ----------------------------------------------------------------------------------
 
 def test_weight_file_roundtrip(tmp_path):
-    for n in (1, 2, 5):
+    for n in (1, 2, 5, 6):
         cfg = gen.get_config(n)
         if n != 1:
             cfg = WMConfig(**{**cfg.__dict__, "d": 16, "d_a": 8, "hidden": 0 if n == 5 else 24,
