@@ -365,7 +365,7 @@ def test_weight_file_roundtrip(tmp_path):
         assert list(w2.keys()) == gen.tensor_order(cfg)
         for kname in w:
             np.testing.assert_array_equal(w[kname], w2[kname])
-        if n != 1:   # bf16 configs: stored values are bf16-representable
+        if cfg.dtype != DTYPE_FP32:   # bf16 configs: stored values are bf16-representable
             for v in w.values():
                 assert (v.view(np.uint32) & 0xFFFF == 0).all()
 
