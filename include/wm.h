@@ -60,6 +60,8 @@ extern "C" {
 #define WM_KIND_MLP     0
 #define WM_KIND_MLP_LN  1
 #define WM_KIND_GRU     2
+#define WM_KIND_TRANSH  3      /* the paper's TransH-style transition (S24): project z onto the */
+                               /* action's hyperplane, translate, residual MLP with the action embedding, L2-normalise  */
 #define WM_DTYPE_FP32   0
 #define WM_DTYPE_BF16   1
 #define WM_EMBED_LINEAR 0

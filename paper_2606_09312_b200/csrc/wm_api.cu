@@ -116,8 +116,8 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         set_error("wm_load_weights: bad magic or version");
         return WM_ERR_FORMAT;
     }
-    const bool mlp = h.kind == WM_KIND_MLP || h.kind == WM_KIND_MLP_LN;
-    if (h.kind > 2 || h.dtype > 1 || h.embed > 1 || h.d == 0 || h.d_a == 0 || h.n_types == 0 || h.P == 0 ||
+    const bool mlp = h.kind == WM_KIND_MLP || h.kind == WM_KIND_MLP_LN || h.kind == WM_KIND_TRANSH;
+    if (h.kind > 3 || h.dtype > 1 || h.embed > 1 || h.d == 0 || h.d_a == 0 || h.n_types == 0 || h.P == 0 ||
         h.d > 65536 || h.d_a > 65536 || h.hidden > 65536 || h.P > 64 || h.H > 65536 || h.n_types > (1u << 20) ||
         h.n_lin < 1 || h.n_lin > 7 || (mlp && h.hidden == 0) || (h.embed == WM_EMBED_BUCKET && h.n_buckets == 0) ||
         h.n_buckets > 4096 || !(h.ln_eps >= 0.0f)) {
@@ -147,6 +147,7 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
     } else {
         add("Tbl", h.n_types * h.P * h.n_buckets, da);
     }
+    if (h.kind == WM_KIND_TRANSH) { add("W_w", d, da); add("W_d", d, da); }
     if (mlp) {
         add("W1", hid, d + da); add("b1", hid, 1); add("W2", d, hid); add("b2", d, 1);
         if (h.kind == WM_KIND_MLP_LN) { add("gamma", d, 1); add("beta", d, 1); }
@@ -209,6 +210,7 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
     up("E", &m.E, false); up("W_p", &m.WpT, true); up("b_p", &m.bp, false); up("Tbl", &m.Tbl, false);
     up("W1", &m.W1t, true); up("b1", &m.b1, false); up("W2", &m.W2t, true); up("b2", &m.b2, false);
     up("gamma", &m.gamma, false); up("beta", &m.beta, false);
+    up("W_w", &m.Wwt, true); up("W_d", &m.Wdt, true);
     up("W_g", &m.Wgt, true); up("W_r", &m.Wrt, true); up("W_h", &m.Wht, true);
     for (int i = 0; i < m.n_lin; ++i) {
         char nm[16];

@@ -22,6 +22,7 @@ struct GenericParams {
     float ln_eps;
     const float *E, *WpT, *bp, *Tbl;
     const float *W1t, *b1, *W2t, *b2, *gamma, *beta;
+    const float *Wwt, *Wdt;      // TransH
     const float *Wgt, *Wrt, *Wht;
     const float* Wst[kMaxScorerLinears];
     const float* bs[kMaxScorerLinears];
@@ -117,7 +118,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
     float* ALT = Hb + (size_t)p.maxw * R;              // [alt_rows][R]: V | AS | Y   (scorer: ping-pong buffer)
     float* V = ALT;                                    // [d][R]
     float* AS = V + (size_t)d * R;                     // [da][R]
-    float* Y = AS + (size_t)da * R;                    // [(d+da)][R], GRU only
+    float* Y = AS + (size_t)da * R;                    // [(d+da)][R], GRU and TransH only
     float* LP = ALT + (size_t)p.alt_rows * R;          // [R][P] log2(param) or bucket index (as int bits)
     float* RED = LP + (size_t)R * P;                   // [G][R] reduction scratch, G = threads / R
     int* meta = reinterpret_cast<int*>(RED + kGenericThreads);   // cand[R], len[R], seg[R], id[R], tile_len
@@ -221,7 +222,57 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
             __syncthreads();
 
             // ---- a2/a3: one transition step, rows with t >= len frozen
-            if (p.kind != WM_KIND_GRU) {
+            if (p.kind == WM_KIND_TRANSH) {
+                // PAPER.md:164 (S24): u = W_w a, w = u / sqrt(|u|^2 + eps); x = z - (w.z) w + W_d a;
+                // v = x + W2 gelu(W1 [x;a] + b1) + b2; z' = v / sqrt(|v|^2 + eps).  (w.z) w = (u.z) u / (|u|^2 + eps).
+                constexpr float kEps = 1e-12f;
+                const float* A_ = X + (size_t)d * R;
+                linear_T<R, ACT_NONE>(p.Wwt, nullptr, A_, da, d, V);     // u
+                linear_T<R, ACT_NONE>(p.Wdt, nullptr, A_, da, d, Y);     // translation W_d a
+                __syncthreads();
+                float s1 = 0.0f, s2 = 0.0f;
+                for (int j = g_of; j < d; j += G) {
+                    const float u = V[(size_t)j * R + r_of];
+                    s1 = fmaf(u, u, s1);
+                    s2 = fmaf(u, X[(size_t)j * R + r_of], s2);
+                }
+                RED[g_of * R + r_of] = s1;
+                __syncthreads();
+                float nw2 = 0.0f;
+                for (int g = 0; g < G; ++g) nw2 += RED[g * R + r_of];
+                __syncthreads();
+                RED[g_of * R + r_of] = s2;
+                __syncthreads();
+                float dot = 0.0f;
+                for (int g = 0; g < G; ++g) dot += RED[g * R + r_of];
+                __syncthreads();
+                const float c = dot / (nw2 + kEps);
+                for (int j = g_of; j < d; j += G) {
+                    const size_t o = (size_t)j * R + r_of;
+                    Y[o] = X[o] - c * V[o] + Y[o];                        // x = z_perp + W_d a
+                }
+                for (int e = tid; e < da * R; e += kGenericThreads) Y[(size_t)d * R + e] = X[(size_t)d * R + e];
+                __syncthreads();
+                linear_T<R, ACT_GELU>(p.W1t, p.b1, Y, K1, p.hidden, Hb);
+                __syncthreads();
+                linear_T<R, ACT_NONE>(p.W2t, p.b2, Hb, p.hidden, d, V);
+                __syncthreads();
+                float q = 0.0f;
+                for (int j = g_of; j < d; j += G) {
+                    const size_t o = (size_t)j * R + r_of;
+                    const float v = Y[o] + V[o];
+                    V[o] = v;
+                    q = fmaf(v, v, q);
+                }
+                RED[g_of * R + r_of] = q;
+                __syncthreads();
+                float n2 = 0.0f;
+                for (int g = 0; g < G; ++g) n2 += RED[g * R + r_of];
+                const float rn = 1.0f / sqrtf(n2 + kEps);
+                if (t < m_len[r_of]) {
+                    for (int j = g_of; j < d; j += G) X[(size_t)j * R + r_of] = V[(size_t)j * R + r_of] * rn;
+                }
+            } else if (p.kind != WM_KIND_GRU) {
                 linear_T<R, ACT_GELU>(p.W1t, p.b1, X, K1, p.hidden, Hb);
                 __syncthreads();
                 linear_T<R, ACT_NONE>(p.W2t, p.b2, Hb, p.hidden, d, V);
@@ -313,7 +364,7 @@ static size_t generic_smem_bytes(const Model& m, int R, int* maxw_out, int* alt_
     int maxsw = 1;
     for (int l = 1; l <= m.n_lin; ++l) maxsw = m.sdim[l] > maxsw ? m.sdim[l] : maxsw;
     if (maxsw > maxw) maxw = maxsw;
-    int alt = m.d + m.d_a + (m.kind == WM_KIND_GRU ? m.d + m.d_a : 0);
+    int alt = m.d + m.d_a + (m.kind == WM_KIND_GRU || m.kind == WM_KIND_TRANSH ? m.d + m.d_a : 0);
     if (maxsw > alt) alt = maxsw;
     *maxw_out = maxw;
     *alt_rows_out = alt;
@@ -364,6 +415,7 @@ int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st) {
     p.ln_eps = m.ln_eps;
     p.E = m.E; p.WpT = m.WpT; p.bp = m.bp; p.Tbl = m.Tbl;
     p.W1t = m.W1t; p.b1 = m.b1; p.W2t = m.W2t; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.Wwt = m.Wwt; p.Wdt = m.Wdt;
     p.Wgt = m.Wgt; p.Wrt = m.Wrt; p.Wht = m.Wht;
     for (int i = 0; i < kMaxScorerLinears; ++i) { p.Wst[i] = m.Wst[i]; p.bs[i] = m.bs[i]; }
     p.a = a;

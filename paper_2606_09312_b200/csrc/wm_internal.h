@@ -36,6 +36,8 @@ struct Model {
     float* b2 = nullptr;
     float* gamma = nullptr;
     float* beta = nullptr;
+    float* Wwt = nullptr;      // [d_a][d]  TransH: hyperplane normal W_w, translation W_d (transposed)
+    float* Wdt = nullptr;
     float* Wgt = nullptr;      // [d+d_a][d]
     float* Wrt = nullptr;
     float* Wht = nullptr;
