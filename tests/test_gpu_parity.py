@@ -255,3 +255,33 @@ def test_full_size_sampled(wm, n):
     assert err <= TOL[False], (n, err)
     idx = gpu_topk(y, b.subgraph_offsets, cfg.k)
     np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6])
+def test_outputs_do_not_overrun(wm, n):
+    """compute-sanitizer is closed on this pool: canaries instead.  The score and index buffers are sub-ranges of
+    larger allocations filled with sentinels; everything outside [0, B) / [0, S*k) must come back untouched, and a
+    ragged last tile (B not a multiple of any tile size) must not write past B."""
+    import torch
+    from wm_harness import to_device
+    cfg = gen.get_config(n).scaled(S=3, per_subgraph=43)      # B = 129: one full 128-row tile + 1 row
+    b = gen.make_inputs(cfg)
+    dv = to_device(b)
+    pad = 4096
+    for path in _paths(wm, cfg):
+        ctx = _ctx(wm, cfg, path)
+        big = torch.full((pad + b.B + pad,), -12345.0, dtype=torch.float32, device="cuda:0")
+        out = big[pad:pad + b.B]
+        wm.wm_rollout_score(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                            dv["hw_feats"], out, dv["subgraph_offsets"])
+        assert wm.wm_check(ctx) == 0
+        S, k = len(b.subgraph_offsets) - 1, cfg.k
+        bigi = torch.full((pad + S * k + pad,), -77, dtype=torch.int32, device="cuda:0")
+        idx = bigi[pad:pad + S * k].view(S, k)
+        wm.wm_topk(out, dv["subgraph_offsets"], k, idx)
+        torch.cuda.synchronize()
+        wm.wm_free(ctx)
+        h, hi = big.cpu().numpy(), bigi.cpu().numpy()
+        assert (h[:pad] == -12345.0).all() and (h[pad + b.B:] == -12345.0).all(), (n, path)
+        assert np.isfinite(h[pad:pad + b.B]).all()
+        assert (hi[:pad] == -77).all() and (hi[pad + S * k:] == -77).all(), (n, path)
