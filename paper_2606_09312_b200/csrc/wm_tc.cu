@@ -319,15 +319,31 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             };
             // GEMM over the A1 K-blocks in the order a/phi (4,5), [hw], z (0..3); waits for the operands of the
             // first chunk of a step / of the scorer.
-            auto gemm_a1 = [&](int b, bool first_chunk, bool with_hw) {
+            // `z_first` (chunk 0 of a rollout step): the z K-blocks are issued before the a K-blocks — a_{t+1} is written
+            // only after the last chunk of step t has released the a-buffer, and the trace showed the issuer waiting
+            // ~4.4 K cycles per step for it; z' (LayerNorm) is ready earlier.  The a-buffer is released right after the
+            // last chunk's a K-blocks, not after the whole chunk.
+            auto gemm_a1 = [&](int b, bool first_chunk, bool last_chunk, bool with_hw, bool z_first) {
                 wait_h(b);
                 const uint32_t d = T_D1 + 128u * b;
-                if (first_chunk) { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); }
-                pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
-                if (with_hw) pair_hw(d);
-                if (first_chunk) { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); }
-                pair_ss(d, s_a1, s_a1 + TILE_BYTES, false);
-                pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
+                auto wait_a = [&]() { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); };
+                auto wait_z = [&]() { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); };
+                if (z_first) {
+                    wait_z();
+                    pair_ss(d, s_a1, s_a1 + TILE_BYTES, true);
+                    pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
+                    wait_a();
+                    pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, false);
+                    if (last_chunk) commit(B_AFREE);
+                } else {
+                    if (first_chunk) wait_a();
+                    pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
+                    if (with_hw) pair_hw(d);
+                    if (last_chunk) commit(B_AFREE);
+                    if (first_chunk) wait_z();
+                    pair_ss(d, s_a1, s_a1 + TILE_BYTES, false);
+                    pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
+                }
                 commit(B_D1FULL + b);
                 pend[b] = true;
             };
@@ -343,8 +359,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll 1
                     for (int i = 0; i <= NC; ++i) {
                         if (i < NC) {
-                            gemm_a1(i & 1, i == 0, false);                       // GEMM1 chunk i
-                            if (i == NC - 1) commit(B_AFREE);
+                            gemm_a1(i & 1, i == 0, i == NC - 1, false, false);      // GEMM1 chunk i
                         }
                         if (i >= 1) {                                            // GEMM2 chunk i-1 (A from TMEM)
                             const int c = i - 1, b = c & 1;
@@ -359,8 +374,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
 #pragma unroll 1
                 for (int c = 0; c < 4; ++c) {
-                    gemm_a1(c & 1, c == 0, true);
-                    if (c == 3) commit(B_AFREE);
+                    gemm_a1(c & 1, c == 0, c == 3, true, false);
                 }
                 wait_h(0);
                 wait_h(1);   // all of H1 (fp16, TMEM columns [0,256)) written
@@ -629,13 +643,12 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
                 *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
                 __syncwarp();
-                // store only once GEMM1 of the previous step no longer reads the a-part of A1
-                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
-                ++n_w;
-                // phase 2 (4 columns per lane, loop over the warp's 32 rows): a = E[id] + W_p log2(p) + b_p
-#pragma unroll 4
-                for (int rr = 0; rr < 32; ++rr) {
-                    const int r = 32 * aw + rr;
+                // phase 2 (4 columns per lane, loop over the warp's 32 rows): a = E[id] + W_p log2(p) + b_p.  The first
+                // PRE rows are computed into registers BEFORE the wait below (the issuer needs a_{t+1} soon after it has
+                // released the a-buffer), the rest after it.
+                constexpr int PRE = 16;
+                uint2 pk[PRE];
+                auto a_row = [&](int r) -> uint2 {
                     const int idr = s_ids[r];
                     float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
                     if (idr >= 0) {
@@ -652,7 +665,19 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll
                             for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
                     }
-                    *a_dst(r) = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+                    return make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+                };
+#pragma unroll
+                for (int rr = 0; rr < PRE; ++rr) pk[rr] = a_row(32 * aw + rr);
+                // store only once GEMM1 of the previous step no longer reads the a-part of A1
+                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+                ++n_w;
+#pragma unroll
+                for (int rr = 0; rr < PRE; ++rr) *a_dst(32 * aw + rr) = pk[rr];
+#pragma unroll 4
+                for (int rr = PRE; rr < 32; ++rr) {
+                    const int r = 32 * aw + rr;
+                    *a_dst(r) = a_row(r);
                 }
                 fence_proxy_async();
                 __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
@@ -781,8 +806,10 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
     blob.reserve((size_t)(NC * 10 + tc::SC_TILES) * tc::TILE_BYTES / 2);
-    auto g1 = [&](int c) {   // GEMM1 chunk c: K-blocks a (4,5) then z (0..3)
-        const int order[6] = {4, 5, 0, 1, 2, 3};
+    auto g1 = [&](int c) {   // GEMM1 chunk c: K-blocks a (4,5) then z (0..3); chunk 0: z first (see gemm_a1)
+        const int a_first[6] = {4, 5, 0, 1, 2, 3}, z_first[6] = {0, 1, 2, 3, 4, 5};
+        const int* order = a_first;   // (z_first for chunk 0 measured slower once a_{t+1} arrives early)
+        (void)z_first; (void)c;
         for (int i = 0; i < 6; ++i) ok &= append_tile(blob, W1, K1, c * 128, order[i] * 64, 64);
     };
     auto g2 = [&](int c) {   // GEMM2 chunk c: K halves of the hidden chunk x N halves of d
