@@ -356,19 +356,37 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 if (tile < 0) break;
 #pragma unroll 1
                 for (int t = 0; t < nsteps; ++t) {
+                    // Step boundary: the a K-blocks of chunk 0 AND chunk 1 depend only on a_{t+1} and both GEMM1
+                    // accumulators are free, so both a-parts are issued before the wait for z' (pipe drain + LayerNorm
+                    // is the serial section of a step); then the z K-blocks of chunks 0 and 1.
+                    {
+                        wait_h(0);
+                        wait_h(1);
+                        WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21);
+                        pair_ss(T_D1, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
+                        pair_ss(T_D1 + 128u, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
+                        if (NC == 2) commit(B_AFREE);
+                        WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23);
+                        for (int b = 0; b < 2; ++b) {
+                            pair_ss(T_D1 + 128u * b, s_a1, s_a1 + TILE_BYTES, false);
+                            pair_ss(T_D1 + 128u * b, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
+                            commit(B_D1FULL + b);
+                            pend[b] = true;
+                        }
+                    }
+                    auto gemm2 = [&](int c) {                                    // GEMM2 chunk c (A from TMEM)
+                        const int b = c & 1;
+                        wait_h(b);
+                        const uint32_t hbuf = T_D1 + 128u * b;
+                        stage_ts256(T_Z, hbuf);            // K-block 0 of the chunk x all 256 latent columns
+                        stage_ts256(T_Z, hbuf + 64u);      // K-block 1
+                        if (c == NC - 1) commit(B_D2FULL);
+                    };
+                    gemm2(0);
 #pragma unroll 1
-                    for (int i = 0; i <= NC; ++i) {
-                        if (i < NC) {
-                            gemm_a1(i & 1, i == 0, i == NC - 1, false, false);      // GEMM1 chunk i
-                        }
-                        if (i >= 1) {                                            // GEMM2 chunk i-1 (A from TMEM)
-                            const int c = i - 1, b = c & 1;
-                            wait_h(b);
-                            const uint32_t hbuf = T_D1 + 128u * b;
-                            stage_ts256(T_Z, hbuf);            // K-block 0 of the chunk x all 256 latent columns
-                            stage_ts256(T_Z, hbuf + 64u);      // K-block 1
-                            if (c == NC - 1) commit(B_D2FULL);
-                        }
+                    for (int i = 2; i <= NC; ++i) {
+                        if (i < NC) gemm_a1(i & 1, false, i == NC - 1, false, false);   // GEMM1 chunk i
+                        gemm2(i - 1);
                     }
                 }
                 // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
@@ -816,9 +834,15 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         for (int ks = 0; ks < 2; ++ks)
             for (int h = 0; h < 2; ++h) ok &= append_tile(blob, W2, hid, h * 128, c * 128 + ks * 64, 64);
     };
-    for (int i = 0; i <= NC; ++i) {   // same interleave as the MMA warp: G1(i), then G2(i-1)
+    // same order as the MMA warp: a K-blocks of chunks 0 and 1, z K-blocks of chunks 0 and 1, G2(0), then G1(i), G2(i-1)
+    auto g1_part = [&](int c, int k0, int k1) {
+        for (int k = k0; k < k1; ++k) ok &= append_tile(blob, W1, K1, c * 128, k * 64, 64);
+    };
+    g1_part(0, 4, 6); g1_part(1, 4, 6); g1_part(0, 0, 4); g1_part(1, 0, 4);
+    g2(0);
+    for (int i = 2; i <= NC; ++i) {
         if (i < NC) g1(i);
-        if (i >= 1) g2(i - 1);
+        g2(i - 1);
     }
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
         ok &= append_tile(blob, Ws0, K0, c * 128, tc::D, 64);
