@@ -327,20 +327,41 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (rank != 0) continue;
 #pragma unroll 1
             for (int t = 0; t < nsteps; ++t) {
+                // Step boundary: the a K-blocks of chunk 0 AND chunk 1 depend only on a_{t+1} and both GEMM1 accumulators
+                // are free, so both a-parts are issued before the wait for z' (pipe drain + LayerNorm is the serial
+                // section of a step); then the z K-blocks of chunks 0 and 1.  (NC >= 2.)
+                wait_h(0);
+                wait_h(1);
+                WM_TRACE(20); mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after();
 #pragma unroll 1
-                for (int i = 0; i <= NC; ++i) {
-                    if (i < NC) gemm_a1(i & 1, i == 0, i == NC - 1, false);      // GEMM1 chunk i
-                    if (i >= 1) {                                                // GEMM2 chunk i-1: Z += H[b] W2^T
-                        const int c = i - 1, b = c & 1;
-                        wait_h(b);
+                for (int b = 0; b < 2; ++b)
 #pragma unroll 1
-                        for (int kb = 0; kb < H_KB; ++kb) {
-                            stage_ss(T_Z, s_h + (b * H_KB + kb) * KB_BYTES, false);
-                            stage_ss(T_Z + 128u, s_h + (b * H_KB + kb) * KB_BYTES, false);
-                        }
-                        commit(B_HFREE + b);
-                        if (c == NC - 1) commit(B_D2FULL);
+                    for (int k = 0; k < 4; ++k) stage_ss(T_D1 + 128u * b, s_a1 + (8 + k) * KB_BYTES, k == 0);
+                if (NC == 2) commit(B_AFREE);
+                WM_TRACE(22); mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after();
+#pragma unroll 1
+                for (int b = 0; b < 2; ++b) {
+#pragma unroll 1
+                    for (int k = 0; k < 8; ++k) stage_ss(T_D1 + 128u * b, s_a1 + k * KB_BYTES, false);
+                    commit(B_D1FULL + b);
+                    pend[b] = true;
+                }
+                auto gemm2 = [&](int c) {                                        // GEMM2 chunk c: Z += H[b] W2^T
+                    const int b = c & 1;
+                    wait_h(b);
+#pragma unroll 1
+                    for (int kb = 0; kb < H_KB; ++kb) {
+                        stage_ss(T_Z, s_h + (b * H_KB + kb) * KB_BYTES, false);
+                        stage_ss(T_Z + 128u, s_h + (b * H_KB + kb) * KB_BYTES, false);
                     }
+                    commit(B_HFREE + b);
+                    if (c == NC - 1) commit(B_D2FULL);
+                };
+                gemm2(0);
+#pragma unroll 1
+                for (int i = 2; i <= NC; ++i) {
+                    if (i < NC) gemm_a1(i & 1, false, i == NC - 1, false);       // GEMM1 chunk i
+                    gemm2(i - 1);
                 }
             }
             // ---- scorer layer 1: four 256-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0).  Chunks 0, 1 land in the
@@ -817,7 +838,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 bool tc2_model_ok(const Model& m) {
     return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc2::D &&
-           m.d_a == tc2::DA && m.hidden >= 256 && m.hidden <= tc2::MAX_HID && m.hidden % 256 == 0 && m.n_lin == 3 &&
+           m.d_a == tc2::DA && m.hidden >= 512 && m.hidden <= tc2::MAX_HID && m.hidden % 256 == 0 && m.n_lin == 3 &&
            m.sdim[1] == tc2::SW && m.sdim[2] == tc2::SW && m.H >= 8 && m.H <= tc2::MAX_H && m.H % 8 == 0 &&
            m.n_types <= tc2::MAX_TYPES && m.P <= tc2::MAX_P;
 }
@@ -839,14 +860,20 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
     blob.reserve(n_tiles * tc2::BT_BYTES);
-    for (int i = 0; i <= NC; ++i) {   // same interleave as the MMA warp: G1(i), then G2(i-1)
-        if (i < NC) {                 // GEMM1 chunk i: K-blocks a (8-11) then z (0-7)
-            for (int k = 8; k < 12; ++k) ok &= append_pair_tile(blob, W1, K1, i * 256, k * 64, 64);
-            for (int k = 0; k < 8; ++k) ok &= append_pair_tile(blob, W1, K1, i * 256, k * 64, 64);
-        }
-        if (i >= 1)                   // GEMM2 chunk i-1: hidden K-blocks x the two 256-column N tiles of d
-            for (int kb = 0; kb < 4; ++kb)
-                for (int j = 0; j < 2; ++j) ok &= append_pair_tile(blob, W2, hid, j * 256, (i - 1) * 256 + kb * 64, 64);
+    // the MMA warp's order: a K-blocks (8-11) of chunks 0 and 1, z K-blocks (0-7) of chunks 0 and 1, G2(0), then G1(i)
+    // (a then z), G2(i-1)
+    auto g1_part = [&](int c, int k0, int k1) {
+        for (int k = k0; k < k1; ++k) ok &= append_pair_tile(blob, W1, K1, c * 256, k * 64, 64);
+    };
+    auto g2 = [&](int c) {            // GEMM2 chunk c: hidden K-blocks x the two 256-column N tiles of d
+        for (int kb = 0; kb < 4; ++kb)
+            for (int j = 0; j < 2; ++j) ok &= append_pair_tile(blob, W2, hid, j * 256, c * 256 + kb * 64, 64);
+    };
+    g1_part(0, 8, 12); g1_part(1, 8, 12); g1_part(0, 0, 8); g1_part(1, 0, 8);
+    g2(0);
+    for (int i = 2; i <= NC; ++i) {
+        if (i < NC) { g1_part(i, 8, 12); g1_part(i, 0, 8); }
+        g2(i - 1);
     }
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (4), hw (1, zero-padded to 64 columns), z (8)
         for (int k = 8; k < 12; ++k) ok &= append_pair_tile(blob, Ws0, K0, c * 256, k * 64, 64);
