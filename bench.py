@@ -41,7 +41,7 @@ UNIT = "candidates/s"
 def _kernel_name(info) -> str:
     """The rollout+score kernel (K2) the library runs for this model, by its CUDA name."""
     if info.path == 2:
-        return {1: "wm_tc_kernel", 2: "wm_tc2_kernel", 3: "wm_tcg_kernel"}[info.tc_variant]
+        return {1: "wm_tc_kernel", 2: "wm_tc2_kernel", 3: "wm_tcg_kernel", 4: "wm_tct_kernel"}[info.tc_variant]
     return "wm_generic_kernel"
 
 

@@ -84,7 +84,8 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
     int32_t path;               /* kernel the auto policy picks for this model: 1 = fp32 CUDA-core, 2 = tcgen05 */
     int32_t tc_variant;         /* tcgen05 kernel built for this model: 0 = none, 1 = wm_tc_kernel (one CTA per  */
                                 /* 128-candidate tile, d = 256), 2 = wm_tc2_kernel (CTA pair per tile, d = 512),  */
-                                /* 3 = wm_tcg_kernel (CTA pair per tile, GRU transition, d = 384)              */
+                                /* 3 = wm_tcg_kernel (CTA pair per tile, GRU transition, d = 384),             */
+                                /* 4 = wm_tct_kernel (TransH transition, d = 256)                              */
 } wm_info;
 
 /* Read a WMW1 weight file (format below), convert to the kernels' layouts and copy to `device`.

@@ -1,25 +1,19 @@
-// K2 (tcgen05): fused persistent rollout + score kernel for the bf16 residual-MLP + LayerNorm models with
-// d = 256, d_a = 128 (BASELINE.json cfg 2 and cfg 4), sm_100a only.
+// K2 (tcgen05, TransH): fused persistent rollout + score kernel for the paper's TransH-style transition (NEXT row f1)
+// with d = 256, d_a = 128, bf16-valued weights (gen config 7), sm_100a only.  Derived from wm_tc.cu (same tile, TMEM
+// and ring machinery, same scorer); what differs is the step:
 //
-// PAPER.md:162 Eq.8 / :166 — z_t = F(z_{t-1}, a_t) applied recurrently; :176 — masked steps leave z unchanged;
-// :186-188 Eq.12 — y = G([z_T ; phi ; h]).  Parametrisation: BASELINE.json cfg 2/4.
-//
-// One CTA owns a tile of 128 candidates (length-sorted by K1) for ALL of its steps:
-//   * the fp32 master latent of the tile lives in TMEM columns [0,256) and IS the accumulator of GEMM2: the
-//     residual add is the MMA's accumulate, the epilogue adds b2, applies LayerNorm and writes z' back;
-//   * a fp16 copy of [z ; a] lives in shared memory (K-major, 128B-swizzled 64-column K-blocks) as the A operand
-//     of GEMM1;
-//   * GEMM1 runs in 128-column chunks of the hidden layer into two alternating TMEM accumulators; the GELU
-//     epilogue writes the fp16 hidden chunk back INTO TMEM (over its own fp32 columns) and GEMM2 consumes it as a
-//     TMEM A operand (tcgen05.mma with A in tensor memory), so the hidden activations never touch shared memory;
-//   * weights stream from L2 through a 3-stage ring of 32 KB tile pairs filled by bulk async copies (TMA engine,
-//     mbarrier complete_tx); the weight image in global memory is pre-tiled, pre-swizzled and laid out in exactly
-//     the order the MMA warp consumes it, so the producer is a linear stream;
-//   * the scorer's two hidden layers run on the same machinery (layer-1 output kept in TMEM as layer-2's A
-//     operand), the last 512->1 layer is a dot product in the epilogue.
-// Warp roles (512 threads): warps 0-7 epilogue (GELU / LayerNorm / scorer; one thread per row and column half),
-// warps 8-11 action embedding (a_t for step t+1 while step t runs; phi and hw at the end of the tile), warp 12 TMEM
-// allocator, warp 13 tile scheduler + weight producer, warp 15 MMA issuer (one elected lane).
+// PAPER.md:164 (DESIGN.md §3 S24):  u = W_w a,  w = u / sqrt(|u|^2 + eps),  z_perp = z - (w.z) w,  x = z_perp + W_d a,
+//   v = x + W2 gelu(W1 [x ; a] + b1) + b2,  z' = v / sqrt(|v|^2 + eps).
+//   * GEMM0: u_{t} = a_t W_w^T is an N = 256 MMA pair of stages into the two GEMM1 accumulators (free at the step
+//     boundary), issued as soon as a_t is there — before the previous step's normalisation has finished;
+//   * ONE fused epilogue per step boundary normalises v (step t) and projects the result onto the hyperplane of
+//     a_{t+1}: pass 1 reads v and u once for |v|^2, |u|^2 and u.v (so w.z' = (u.v) rn / sqrt(|u|^2+eps)), pass 2
+//     writes z_perp = v rn - c u (fp32 -> TMEM, fp16 -> the A operand); rows whose last step this was get their
+//     terminal z' (fp16, the scorer's input) instead and are frozen;
+//   * the translation W_d a is accumulated straight ONTO the latent accumulator by an N = 256 MMA pair of stages
+//     (x = z_perp + W_d a is never formed by a thread), and GEMM1 consumes z_perp with W1's a-columns pre-folded on the
+//     host, W1a' = W1a + W1z W_d, because W1 [x ; a] = W1z z_perp + (W1z W_d + W1a) a;
+//   * GEMM2 accumulates W2 h onto the same accumulator: it then holds v - b2.
 #include <cuda_bf16.h>
 
 #include <cstdio>
@@ -31,7 +25,7 @@
 
 namespace wm {
 
-namespace tc {
+namespace tct {
 
 constexpr int TM = 128;            // candidates per tile (MMA M)
 constexpr int D = 256;             // latent width
@@ -56,6 +50,7 @@ enum {
     B_D1FULL = B_EMPTY + NSTAGE,   // [2] MMA commit -> epilogue: accumulator buffer b filled
     B_HREADY = B_D1FULL + 2,       // [2] epilogue -> MMA: buffer b consumed (fp16 hidden written)
     B_D2FULL = B_HREADY + 2,       // MMA commit -> epilogue: GEMM2 of the step done
+    B_UFULL,                       // MMA commit -> epilogue: u = W_w a (GEMM0) in the two GEMM1 accumulators
     B_ZREADY,                      // epilogue -> MMA: z (fp16 smem + fp32 TMEM) written
     B_AFREE,                       // MMA commit -> action warps: a-part of A1 no longer read
     B_AREADY,                      // action warps -> MMA: a-part written
@@ -100,7 +95,7 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
     L.b2 = o; o += D * 4;
     L.gamma = o; o += D * 4;
     L.beta = o; o += D * 4;
-    L.red = o; o += 2 * TM * 8;
+    L.red = o; o += 2 * TM * 16;                       // [2 column halves][128 rows] float4: |v|^2, |u|^2, u.v
     L.bars = o; o += B_COUNT * 8;
     L.sched = o; o += 2 * 8;
     L.tmem_slot = o; o += 16;
@@ -126,11 +121,11 @@ using namespace ptx;
 #define WM_TRACE(tag) do { } while (0)
 #endif
 
-}  // namespace tc
+}  // namespace tct
 
-namespace tc {
+namespace tct {
 
-__global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
+__global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps);
     const uint32_t s_base = smem_u32(smem);
@@ -139,13 +134,11 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     volatile int* s_sched = reinterpret_cast<volatile int*>(smem + L.sched);   // [2][2]: tile, nsteps
     float* s_b1 = reinterpret_cast<float*>(smem + L.b1);
     float* s_b2 = reinterpret_cast<float*>(smem + L.b2);
-    float* s_gamma = reinterpret_cast<float*>(smem + L.gamma);
-    float* s_beta = reinterpret_cast<float*>(smem + L.beta);
-    float2* s_red = reinterpret_cast<float2*>(smem + L.red);                  // [2][128]
+    float4* s_red = reinterpret_cast<float4*>(smem + L.red);                  // [2][128]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int NC = p.nc;
-    const int ROLL_TILES = NC * 10;
+    const int ROLL_TILES = NC * 10 + 8;      // per step: W_d (4 tiles), the GEMM1 / GEMM2 interleave, W_w (4 tiles)
 
     // ---- one-time setup
     if (threadIdx.x == 0) {
@@ -157,6 +150,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             mbar_init(bar(B_SEMPTY + i), 13);
         }
         mbar_init(bar(B_D2FULL), 1);
+        mbar_init(bar(B_UFULL), 1);
         mbar_init(bar(B_ZREADY), 8);
         mbar_init(bar(B_AFREE), 1);
         mbar_init(bar(B_AREADY), 4);
@@ -167,8 +161,6 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     for (int i = threadIdx.x; i < p.hid; i += THREADS) s_b1[i] = __ldg(p.b1 + i);
     for (int i = threadIdx.x; i < D; i += THREADS) {
         s_b2[i] = __ldg(p.b2 + i);
-        s_gamma[i] = __ldg(p.gamma + i);
-        s_beta[i] = __ldg(p.beta + i);
     }
     {
         const uint32_t* src = reinterpret_cast<const uint32_t*>(p.E);
@@ -214,9 +206,12 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             if (tile < 0) break;
             if (lane == 0) {
                 // the stream is consumed in pairs of tiles that are adjacent in the image: one 32 KB copy per stage
-                const int roll_total = nsteps * ROLL_TILES, total = roll_total + SC_TILES;
+                // stream of a tile: [W_w for step 0 (= the last 4 tiles of the step image)] nsteps x [step image] [scorer]
+                const int pre = nsteps > 0 ? 4 : 0;
+                const int roll_total = nsteps * ROLL_TILES, total = pre + roll_total + SC_TILES;
                 for (int i = 0; i < total; i += 2) {
-                    const int src_tile = i < roll_total ? i % ROLL_TILES : ROLL_TILES + (i - roll_total);
+                    const int j = i - pre;
+                    const int src_tile = j < 0 ? ROLL_TILES - 4 + i : j < roll_total ? j % ROLL_TILES : ROLL_TILES + (j - roll_total);
                     mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
                     mbar_arrive_expect_tx(bar(B_FULL + stage), STAGE_BYTES);
                     bulk_g2s(s_ring + stage * STAGE_BYTES, p.blob + (size_t)src_tile * TILE_BYTES, STAGE_BYTES,
@@ -354,39 +349,58 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
                 if (tile < 0) break;
+                // one ring stage = ONE [256 x 64] B tile against the A1 K-block a_tile (shared memory): 4 MMAs with N = 256
+                auto stage_ss256 = [&](uint32_t d, uint32_t a_tile, bool first) {
+                    wait_full();
+                    const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + stage * STAGE_BYTES);
+                    if (elect_one()) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) mma_ss(d, a0 + 2u * j, b0 + 2u * j, IDESC_N256, (first && j == 0) ? 0u : 1u);
+                        release();
+                    }
+                    advance();
+                };
+                // GEMM0: u = a W_w^T (K = 128) into the two GEMM1 accumulators taken as one 256-column tile
+                auto gemm0 = [&]() {
+                    wait_h(0);
+                    wait_h(1);
+                    WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21);
+                    stage_ss256(T_D1, s_a1 + 4 * TILE_BYTES, true);
+                    stage_ss256(T_D1, s_a1 + 5 * TILE_BYTES, false);
+                    commit(B_UFULL);
+                    pend[0] = pend[1] = true;      // the fused epilogue arrives on both HREADY barriers once u is read
+                };
+                auto gemm2 = [&](int c) {                                        // GEMM2 chunk c (A from TMEM)
+                    const int b = c & 1;
+                    wait_h(b);
+                    const uint32_t hbuf = T_D1 + 128u * b;
+                    stage_ts256(T_Z, hbuf);            // K-block 0 of the chunk x all 256 latent columns
+                    stage_ts256(T_Z, hbuf + 64u);      // K-block 1
+                    if (c == NC - 1) commit(B_D2FULL);
+                };
+                if (nsteps > 0) gemm0();                                         // u_0
 #pragma unroll 1
                 for (int t = 0; t < nsteps; ++t) {
-                    // Step boundary: the a K-blocks of chunk 0 AND chunk 1 depend only on a_{t+1} and both GEMM1
-                    // accumulators are free, so both a-parts are issued before the wait for z' (pipe drain + LayerNorm
-                    // is the serial section of a step); then the z K-blocks of chunks 0 and 1.
-                    {
-                        wait_h(0);
-                        wait_h(1);
-                        WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21);
-                        pair_ss(T_D1, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
-                        pair_ss(T_D1 + 128u, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
-                        if (NC == 2) commit(B_AFREE);
-                        WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23);
-                        for (int b = 0; b < 2; ++b) {
-                            pair_ss(T_D1 + 128u * b, s_a1, s_a1 + TILE_BYTES, false);
-                            pair_ss(T_D1 + 128u * b, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
-                            commit(B_D1FULL + b);
-                            pend[b] = true;
-                        }
-                    }
-                    auto gemm2 = [&](int c) {                                    // GEMM2 chunk c (A from TMEM)
-                        const int b = c & 1;
-                        wait_h(b);
-                        const uint32_t hbuf = T_D1 + 128u * b;
-                        stage_ts256(T_Z, hbuf);            // K-block 0 of the chunk x all 256 latent columns
-                        stage_ts256(T_Z, hbuf + 64u);      // K-block 1
-                        if (c == NC - 1) commit(B_D2FULL);
-                    };
-                    gemm2(0);
+                    // z_perp (fp32 accumulator + fp16 operand) written by the fused epilogue
+                    WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23);
+                    tc_fence_after();
+                    // translation: W_d a accumulated straight onto the latent accumulator (x = z_perp + W_d a)
+                    stage_ss256(T_Z, s_a1 + 4 * TILE_BYTES, false);
+                    stage_ss256(T_Z, s_a1 + 5 * TILE_BYTES, false);
+                    // residual MLP: GEMM1 chunks (a K-blocks with the folded W1a', z K-blocks on z_perp) / GEMM2
 #pragma unroll 1
-                    for (int i = 2; i <= NC; ++i) {
-                        if (i < NC) gemm_a1(i & 1, false, i == NC - 1, false, false);   // GEMM1 chunk i
-                        gemm2(i - 1);
+                    for (int i = 0; i <= NC; ++i) {
+                        if (i < NC) gemm_a1(i & 1, false, i == NC - 1, false, false);
+                        if (i >= 1) gemm2(i - 1);
+                    }
+                    if (t + 1 < nsteps) {
+                        gemm0();                                                 // u_{t+1}
+                    } else {                                                     // the step image ends with W_w: skip it
+                        for (int k = 0; k < 2; ++k) {
+                            wait_full();
+                            if (elect_one()) release();
+                            advance();
+                        }
                     }
                 }
                 // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
@@ -417,7 +431,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         const int row = 32 * q + lane;
         const uint32_t lane_off = (uint32_t)(32 * q) << 16;
         uint8_t* a1 = smem + L.a1;
-        uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
+        uint32_t n_d1[2] = {0, 0}, n_d2 = 0, n_u = 0;   // phase counters live across tiles
         const float inv_d = 1.0f / (float)D;
         // write 32 consecutive z columns of this row: fp32 -> TMEM, fp16 -> A1 (when `to_smem`)
         auto put_z = [&](int col0, const uint32_t (&v)[32], bool to_smem) {
@@ -477,89 +491,119 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             int cand, len, seg;
             row_meta(p.a, (int64_t)tile * TM + row, cand, len, seg, false);
 
-            // ---- z_0 (the task's initial latent)
-#pragma unroll 1
-            for (int p4 = 0; p4 < 4; ++p4) {
-                const int col0 = 128 * hh + 32 * p4;
-                uint32_t v[32];
-                if (cand >= 0) {
-                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + col0);
+            constexpr float kEps = 1e-12f;     // under both square roots (DESIGN.md §3 S24)
+            // load 32 columns of this row's source vector: z_0 from global (step -1) or v = accumulator + b2
+            auto load_src = [&](bool from_z0, int col0, uint32_t (&v)[32]) {
+                if (from_z0) {
+                    if (cand >= 0) {
+                        const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + col0);
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const float4 f = __ldg(src + i);
-                        v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
-                        v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
+                        for (int i = 0; i < 8; ++i) {
+                            const float4 f = __ldg(src + i);
+                            v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
+                            v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = 0u;
                     }
                 } else {
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) v[i] = 0u;
-                }
-                put_z(col0, v, true);
-            }
-            publish(B_ZREADY, true);
-
-            for (int t = 0; t < nsteps; ++t) {
-                for (int c = 0; c < NC; ++c)
-                    gelu_chunk(c & 1, s_b1 + c * 128 + 64 * hh, true, T_D1 + 128u * (c & 1) + 64u * hh);
-                // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
-                mbar_wait(bar(B_D2FULL), n_d2 & 1);
-                ++n_d2;
-                tc_fence_after();
-                float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
-#pragma unroll 1
-                for (int p4 = 0; p4 < 4; ++p4) {
-                    const int col0 = 128 * hh + 32 * p4;
-                    uint32_t v[32];
                     tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
                     tmem_ld_wait();
                     const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const float4 bb = b2v[i];
-                        const float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
-                                                     make_float2(bb.x, bb.y));
-                        const float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
-                                                     make_float2(bb.z, bb.w));
-                        s1v = __fadd2_rn(s1v, __fadd2_rn(x0, x1));
-                        s2v = __ffma2_rn(x0, x0, s2v);
-                        s2v = __ffma2_rn(x1, x1, s2v);
+                        v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) + bb.x);
+                        v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) + bb.y);
+                        v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) + bb.z);
+                        v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) + bb.w);
                     }
                 }
-                const float s1 = s1v.x + s1v.y, s2 = s2v.x + s2v.y;
-                s_red[hh * TM + row] = make_float2(s1, s2);
-                named_bar_sync(1 + q, 64);
-                const float2 other = s_red[(hh ^ 1) * TM + row];
-                const float mean = (s1 + other.x) * inv_d;
-                const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
-                const float rstd = rsqrtf(var + p.ln_eps);
-                const bool live = t < len;     // masked steps leave the state unchanged
+            };
+            // The fused epilogue of a step boundary: "finally normalized" for the step that has just
+            // finished (t >= 0; t = -1: z_0 is taken as it is), then "transformed in an action-conditioned geometric
+            // space" for the next one — z_perp = z' - (w.z') w with w = u / sqrt(|u|^2 + eps), u = W_w a_{t+1} from
+            // GEMM0 — when there is a next step.  Rows whose last step was t keep z' as their terminal latent.
+            auto boundary = [&](int t) {
+                const bool from_z0 = t < 0;
+                const bool has_next = t + 1 < nsteps;
+                if (!from_z0) {
+                    mbar_wait(bar(B_D2FULL), n_d2 & 1);
+                    ++n_d2;
+                }
+                if (has_next) {
+                    mbar_wait(bar(B_UFULL), n_u & 1);
+                    ++n_u;
+                }
+                tc_fence_after();
+                float n2 = 0.0f, s1 = 0.0f, s2 = 0.0f;       // |v|^2, |u|^2, u.v over this thread's 128 columns
 #pragma unroll 1
                 for (int p4 = 0; p4 < 4; ++p4) {
                     const int col0 = 128 * hh + 32 * p4;
                     uint32_t v[32];
-                    tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
-                    tmem_ld_wait();
-                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
-                    const float4* gv = reinterpret_cast<const float4*>(s_gamma + col0);
-                    const float4* bev = reinterpret_cast<const float4*>(s_beta + col0);
-                    const float2 rs2 = make_float2(rstd, rstd), mr2 = make_float2(-mean * rstd, -mean * rstd);
+                    load_src(from_z0, col0, v);
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const float4 bb = b2v[i], gg = gv[i], be = bev[i];
-                        float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
-                                               make_float2(bb.x, bb.y));
-                        float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
-                                               make_float2(bb.z, bb.w));
-                        x0 = __ffma2_rn(__ffma2_rn(x0, rs2, mr2), make_float2(gg.x, gg.y), make_float2(be.x, be.y));
-                        x1 = __ffma2_rn(__ffma2_rn(x1, rs2, mr2), make_float2(gg.z, gg.w), make_float2(be.z, be.w));
-                        v[4 * i] = __float_as_uint(x0.x); v[4 * i + 1] = __float_as_uint(x0.y);
-                        v[4 * i + 2] = __float_as_uint(x1.x); v[4 * i + 3] = __float_as_uint(x1.y);
+                    for (int i = 0; i < 32; ++i) n2 = fmaf(__uint_as_float(v[i]), __uint_as_float(v[i]), n2);
+                    if (has_next) {
+                        uint32_t u[32];
+                        tmem_ld32(T_D1 + lane_off + (uint32_t)col0, u);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) {
+                            s1 = fmaf(__uint_as_float(u[i]), __uint_as_float(u[i]), s1);
+                            s2 = fmaf(__uint_as_float(u[i]), __uint_as_float(v[i]), s2);
+                        }
                     }
-                    // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
-                    // fp32 master is never read again
-                    put_z(col0, v, live);
                 }
-                publish(B_ZREADY, true);
+                s_red[hh * TM + row] = make_float4(n2, s1, s2, 0.0f);
+                named_bar_sync(1 + q, 64);
+                const float4 other = s_red[(hh ^ 1) * TM + row];
+                n2 += other.x; s1 += other.y; s2 += other.z;
+                const float rn = from_z0 ? 1.0f : rsqrtf(n2 + kEps);
+                const float c = s2 * rn / (s1 + kEps);            // (w.z') w = (u.z') u / (|u|^2 + eps),  z' = v rn
+                const bool live_now = from_z0 ? true : t < len;   // the row took part in step t
+                const bool next_live = t + 1 < len;
+#pragma unroll 1
+                for (int p4 = 0; p4 < 4; ++p4) {
+                    const int col0 = 128 * hh + 32 * p4;
+                    uint32_t v[32];
+                    load_src(from_z0, col0, v);
+                    if (has_next) {
+                        uint32_t u[32];
+                        tmem_ld32(T_D1 + lane_off + (uint32_t)col0, u);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) {
+                            const float zn = __uint_as_float(v[i]) * rn;
+                            v[i] = __float_as_uint(next_live ? fmaf(-c, __uint_as_float(u[i]), zn) : zn);
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = __float_as_uint(__uint_as_float(v[i]) * rn);
+                    }
+                    // frozen rows (their last step was before t): the fp16 copy keeps the terminal latent
+                    put_z(col0, v, live_now);
+                }
+                named_bar_sync(1 + q, 64);       // both halves have read s_red before the next boundary rewrites it
+                tmem_st_wait();
+                fence_proxy_async();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if (has_next) {              // u has been read: the two GEMM1 accumulators are free again
+                        mbar_arrive(bar(B_HREADY + 0));
+                        mbar_arrive(bar(B_HREADY + 1));
+                    }
+                    mbar_arrive(bar(B_ZREADY));
+                }
+            };
+
+            boundary(-1);      // z_0 (the task's initial latent), projected for the first action
+            for (int t = 0; t < nsteps; ++t) {
+                for (int c = 0; c < NC; ++c)
+                    gelu_chunk(c & 1, s_b1 + c * 128 + 64 * hh, true, T_D1 + 128u * (c & 1) + 64u * hh);
+                boundary(t);
             }
 
             // ---- scorer layer 1 -> H1 (fp16) in TMEM columns [0,256)
@@ -586,7 +630,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(B_HREADY + b));
             }
-            s_red[hh * TM + row] = make_float2(part, 0.0f);
+            s_red[hh * TM + row] = make_float4(part, 0.0f, 0.0f, 0.0f);
             named_bar_sync(1 + q, 64);
             if (hh == 0 && cand >= 0) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
             named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
@@ -762,7 +806,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     if (warp == ALLOC_WARP) tmem_dealloc(tmem_base, 512);
 }
 
-}  // namespace tc
+}  // namespace tct
 
 // ------------------------------------------------------------------------------------------------ host side
 namespace {
@@ -778,7 +822,7 @@ uint16_t f32_to_bf16(float f) {
 // Returns false when a weight is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
 bool append_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid) {
     const size_t base = blob.size();
-    blob.resize(base + tc::TILE_BYTES / 2, 0);
+    blob.resize(base + tct::TILE_BYTES / 2, 0);
     bool ok = true;
     for (int n = 0; n < 128; ++n)
         for (int k = 0; k < 64; ++k) {
@@ -792,28 +836,22 @@ bool append_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int l
 }
 
 struct TcState {
-    tc::Params p;
+    tct::Params p;
 };
 
 }  // namespace
 
-static bool tc_model_ok(const Model& m) {
-    return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc::D &&
-           m.d_a == tc::DA && m.hidden >= 256 && m.hidden <= tc::MAX_HID && m.hidden % 128 == 0 && m.n_lin == 3 &&
-           m.sdim[1] == tc::SW && m.sdim[2] == tc::SW && m.H >= 8 && m.H <= tc::MAX_H && m.H % 8 == 0 &&
-           m.n_types <= tc::MAX_TYPES && m.P <= tc::MAX_P;
+static bool tct_model_ok(const Model& m) {
+    return m.kind == WM_KIND_TRANSH && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tct::D &&
+           m.d_a == tct::DA && m.hidden >= 256 && m.hidden <= tct::MAX_HID && m.hidden % 128 == 0 && m.n_lin == 3 &&
+           m.sdim[1] == tct::SW && m.sdim[2] == tct::SW && m.H >= 8 && m.H <= tct::MAX_H && m.H % 8 == 0 &&
+           m.n_types <= tct::MAX_TYPES && m.P <= tct::MAX_P;
 }
 
-int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
+int tct_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
     Model& m = ctx->m;
-    m.tc_ok = 0;
-    if (!tc_model_ok(m)) {   // d = 512 MLP+LN models and the GRU model: the CTA-pair kernels
-        const int rc = tc2_prepare(ctx, hv, names);
-        if (rc != WM_OK || m.tc_ok) return rc;
-        const int rc2 = tcg_prepare(ctx, hv, names);
-        return rc2 != WM_OK || m.tc_ok ? rc2 : tct_prepare(ctx, hv, names);   // TransH models (NEXT row f1)
-    }
-    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16);
+    if (!tct_model_ok(m)) return WM_OK;
+    const tct::SmemLayout L = tct::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16);
     if ((int)L.total > ctx->smem_optin) return WM_OK;
     auto get = [&](const char* n) -> const std::vector<float>& {
         for (size_t i = 0; i < names.size(); ++i)
@@ -822,39 +860,49 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         return empty;
     };
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1"), &E = get("E");
-    const int hid = m.hidden, NC = hid / 128, K1 = tc::D + tc::DA, K0 = K1 + m.H;
+    const std::vector<float>&Ww = get("W_w"), &Wd = get("W_d");
+    const int hid = m.hidden, NC = hid / 128, K1 = tct::D + tct::DA, K0 = K1 + m.H;
+    // W1 [x ; a] with x = z_perp + W_d a  =  W1z z_perp + (W1a + W1z W_d) a: fold the translation into W1's a-columns
+    // (fp64 accumulate; the folded columns are rounded to fp16 like every other operand)
+    std::vector<float> W1f(W1);
+    for (int n = 0; n < hid; ++n)
+        for (int j = 0; j < tct::DA; ++j) {
+            double acc = W1[(size_t)n * K1 + tct::D + j];
+            for (int k = 0; k < tct::D; ++k) acc += (double)W1[(size_t)n * K1 + k] * (double)Wd[(size_t)k * tct::DA + j];
+            W1f[(size_t)n * K1 + tct::D + j] = (float)acc;
+        }
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
-    blob.reserve((size_t)(NC * 10 + tc::SC_TILES) * tc::TILE_BYTES / 2);
-    auto g1 = [&](int c) {   // GEMM1 chunk c: K-blocks a (4,5) then z (0..3); chunk 0: z first (see gemm_a1)
-        const int a_first[6] = {4, 5, 0, 1, 2, 3}, z_first[6] = {0, 1, 2, 3, 4, 5};
-        const int* order = a_first;   // (z_first for chunk 0 measured slower once a_{t+1} arrives early)
-        (void)z_first; (void)c;
-        for (int i = 0; i < 6; ++i) ok &= append_tile(blob, W1, K1, c * 128, order[i] * 64, 64);
+    blob.reserve((size_t)(NC * 10 + 8 + tct::SC_TILES) * tct::TILE_BYTES / 2);
+    // a [256 x 128] matrix applied to a (K = 128): two stages, each ONE [256 x 64] tile = two adjacent [128 x 64] tiles
+    auto a_gemm = [&](const std::vector<float>& W) {
+        for (int kb = 0; kb < 2; ++kb)
+            for (int h = 0; h < 2; ++h) ok &= append_tile(blob, W, tct::DA, h * 128, kb * 64, 64);
+    };
+    auto g1 = [&](int c) {   // GEMM1 chunk c: K-blocks a (4,5; folded W1a') then z (0..3)
+        const int order[6] = {4, 5, 0, 1, 2, 3};
+        for (int i = 0; i < 6; ++i) ok &= append_tile(blob, W1f, K1, c * 128, order[i] * 64, 64);
     };
     auto g2 = [&](int c) {   // GEMM2 chunk c: K halves of the hidden chunk x N halves of d
         for (int ks = 0; ks < 2; ++ks)
             for (int h = 0; h < 2; ++h) ok &= append_tile(blob, W2, hid, h * 128, c * 128 + ks * 64, 64);
     };
-    // same order as the MMA warp: a K-blocks of chunks 0 and 1, z K-blocks of chunks 0 and 1, G2(0), then G1(i), G2(i-1)
-    auto g1_part = [&](int c, int k0, int k1) {
-        for (int k = k0; k < k1; ++k) ok &= append_tile(blob, W1, K1, c * 128, k * 64, 64);
-    };
-    g1_part(0, 4, 6); g1_part(1, 4, 6); g1_part(0, 0, 4); g1_part(1, 0, 4);
-    g2(0);
-    for (int i = 2; i <= NC; ++i) {
+    // the step image, in the MMA warp's order: W_d (translation), G1(i) / G2(i-1) interleaved, W_w (u of the next step)
+    a_gemm(Wd);
+    for (int i = 0; i <= NC; ++i) {
         if (i < NC) g1(i);
-        g2(i - 1);
+        if (i >= 1) g2(i - 1);
     }
+    a_gemm(Ww);
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
-        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D, 64);
-        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + 64, 64);
+        ok &= append_tile(blob, Ws0, K0, c * 128, tct::D, 64);
+        ok &= append_tile(blob, Ws0, K0, c * 128, tct::D + 64, 64);
         ok &= append_tile(blob, Ws0, K0, c * 128, K1, m.H);
         ok &= append_tile(blob, Ws0, K0, c * 128, K1, 0);
         for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
     }
     for (int c = 0; c < 4; ++c)       // scorer layer 2
-        for (int kb = 0; kb < 8; ++kb) ok &= append_tile(blob, Ws1, tc::SW, c * 128, kb * 64, 64);
+        for (int kb = 0; kb < 8; ++kb) ok &= append_tile(blob, Ws1, tct::SW, c * 128, kb * 64, 64);
 
     if (!ok) return WM_OK;   // a weight beyond the fp16 range: this model stays on the fp32 kernel
 
@@ -871,67 +919,31 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     m.tc_blob = d_blob;
     m.tc_blob_bytes = blob.size() * 2;
     m.tc_E = d_e;
-    WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
-    m.tc_ok = 1;
+    WM_CUDA_TRY(cudaFuncSetAttribute(tct::wm_tct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    m.tc_ok = 4;
     return WM_OK;
 }
 
-int tc_supported(const wm_ctx* ctx) { return ctx->m.tc_ok; }
-
-int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
+int launch_tct(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const Model& m = ctx->m;
-    // per-call conditions the kernel relies on; otherwise the fp32 kernel takes the call
-    const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0);
-    if (!m.tc_ok || a.T_max > 255 || !aligned) {
-        if (ctx->opt_path == 2) {
-            set_error("tcgen05 path: needs T_max <= 255 and 16-byte aligned init_states / hw_feats");
-            return WM_ERR_UNSUPPORTED;
-        }
-        return launch_generic(ctx, a, st);
-    }
-    if (m.tc_ok == 2) return launch_tc2(ctx, ws, a, st);
-    if (m.tc_ok == 3) return launch_tcg(ctx, ws, a, st);
-    if (m.tc_ok == 4) return launch_tct(ctx, ws, a, st);
-    tc::Params p;
+    tct::Params p;
     p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;
     p.ln_eps = m.ln_eps;
     p.blob = static_cast<const uint8_t*>(m.tc_blob);
     p.E = static_cast<const __nv_bfloat16*>(m.tc_E);
-    p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = nullptr; p.beta = nullptr;
     p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
     p.a = a;
-    p.n_tiles = (int)((a.B + tc::TM - 1) / tc::TM);
+    p.n_tiles = (int)((a.B + tct::TM - 1) / tct::TM);
     p.tile_counter = ws->counters + kTileCtrOff;
     WM_CUDA_TRY(cudaMemsetAsync(p.tile_counter, 0, sizeof(int), st));
     p.prof = nullptr;
-    static unsigned long long* d_prof = nullptr;
-#ifdef WM_TC_PROFILE
-    if (getenv("WM_TC_PROF")) {
-        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, 3 * 8192 * 8));
-        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, 3 * 8192 * 8, st));
-        p.prof = d_prof;
-    }
-#endif
-    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
+    const tct::SmemLayout L = tct::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
     const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
-    tc::wm_tc_kernel<<<grid, tc::THREADS, L.total, st>>>(p);
+    tct::wm_tct_kernel<<<grid, tct::THREADS, L.total, st>>>(p);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
-#ifdef WM_TC_PROFILE
-    if (p.prof) {   // dev instrumentation: dump CTA 0's per-role (tag, clock) traces to WM_TC_PROF's path
-        std::vector<uint2> h(3 * 8192);
-        WM_CUDA_TRY(cudaStreamSynchronize(st));
-        WM_CUDA_TRY(cudaMemcpy(h.data(), d_prof, h.size() * 8, cudaMemcpyDeviceToHost));
-        FILE* f = fopen(getenv("WM_TC_PROF"), "w");
-        if (f) {
-            for (int r = 0; r < 3; ++r)
-                for (uint32_t i = 0; i < h[r * 8192].x; ++i)
-                    fprintf(f, "%d %u %u\n", r, h[r * 8192 + 1 + i].x, h[r * 8192 + 1 + i].y);
-            fclose(f);
-        }
-    }
-#endif
     return WM_OK;
 }
 

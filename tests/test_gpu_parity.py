@@ -82,7 +82,7 @@ def _edge_batch(cfg, lengths=None, S=None, per=None):
     return c, b
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7])
 @pytest.mark.parametrize("case", ["B1", "B127", "B129", "B257", "len0", "lenmax", "one_long", "param_ends"])
 def test_edge_cases(wm, n, case):
     base = gen.get_config(n)
@@ -229,7 +229,7 @@ def test_host_entry_matches_device_entry(wm):
     wm.wm_free(ctx)
 
 
-@pytest.mark.parametrize("n", [2, 3, 4, 5])
+@pytest.mark.parametrize("n", [2, 3, 4, 5, 7])
 def test_full_size_sampled(wm, n):
     """BASELINE.json's full size in the launch configuration bench.py times (auto path, length bucketing on, CSR
     segments): a sample of candidates is recomputed one by one by the oracle (a candidate's score does not depend on
@@ -257,7 +257,7 @@ def test_full_size_sampled(wm, n):
     np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7])
 def test_outputs_do_not_overrun(wm, n):
     """compute-sanitizer is closed on this pool: canaries instead.  The score and index buffers are sub-ranges of
     larger allocations filled with sentinels; everything outside [0, B) / [0, S*k) must come back untouched, and a
@@ -285,3 +285,19 @@ def test_outputs_do_not_overrun(wm, n):
         assert (h[:pad] == -12345.0).all() and (h[pad + b.B:] == -12345.0).all(), (n, path)
         assert np.isfinite(h[pad:pad + b.B]).all()
         assert (hi[:pad] == -77).all() and (hi[pad + S * k:] == -77).all(), (n, path)
+
+
+@pytest.mark.parametrize("n", [2, 3, 5, 7])
+def test_repeatable_bitwise_with_several_tiles_per_cta(wm, n):
+    """A batch large enough that every persistent CTA (or CTA pair) walks several tiles, scored three times: the
+    scores must be bit-identical.  Barrier phase counters that do not survive a tile boundary, or a wait that passes
+    on a stale phase, show up as run-to-run differences long before they exceed the parity tolerance."""
+    cfg = gen.get_config(n).scaled(S=10, per_subgraph=2048 if n != 5 else 2047)
+    b = gen.make_inputs(cfg)
+    ctx = _ctx(wm, cfg)
+    assert wm.wm_get_info(ctx).path == wm.PATH_TCGEN05
+    y0 = gpu_scores(ctx, b)
+    for _ in range(2):
+        np.testing.assert_array_equal(gpu_scores(ctx, b).view(np.uint32), y0.view(np.uint32))
+    wm.wm_free(ctx)
+    assert np.isfinite(y0).all()
