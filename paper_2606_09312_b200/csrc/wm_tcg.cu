@@ -433,12 +433,12 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     }
                     publish(r_xfree(xb), 0u, false);
                 }
-                // ---- z'_j = z + g (tanh(H_j) - z) = (1 - g) z + g h,  g = sigma(G_j)  (G_j in X0; H_0 in X2, H_1 in X1)
-#pragma unroll 1
-                for (int j = 0; j < 2; ++j) {
-                    const int xh = j == 0 ? 2 : 1;
-                    wait_full(0);
-                    wait_full(xh);
+                // ---- z'_j = z + g (tanh(H_j) - z) = (1 - g) z + g h,  g = sigma(G_j)  (G_j in X0; H_0 in X2, H_1 in X1).
+                // The blend is bound by the special-function unit (sigma and tanh: 2 of 16 per clock and SM for each of
+                // 12,288 elements of a tile) and blend_1 is the serial section of a step (G_1 is the last tile), so
+                // tanh(H_1) - z is applied IN PLACE to X1 as soon as H_1 completes, while G_1 is still running:
+                // blend_1 then needs one special function and one FMA per element.
+                auto blend = [&](int j, int xh, bool h_is_delta) {
 #pragma unroll 1
                     for (int s = 0; s < 3; ++s) {
                         uint32_t g[16], h[16], z[16], o[8];
@@ -450,8 +450,8 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                         for (int i = 0; i < 16; ++i) {
                             const float zf = __uint_as_float(z[i]);
                             const float gf = sigmoid_fast(__uint_as_float(g[i]));
-                            const float hf = tanh_fast(__uint_as_float(h[i]));
-                            z[i] = __float_as_uint(live ? fmaf(gf, hf - zf, zf) : zf);
+                            const float df = h_is_delta ? __uint_as_float(h[i]) : tanh_fast(__uint_as_float(h[i])) - zf;
+                            z[i] = __float_as_uint(live ? fmaf(gf, df, zf) : zf);
                         }
 #pragma unroll
                         for (int i = 0; i < 8; ++i) o[i] = pack_f16(__uint_as_float(z[2 * i]), __uint_as_float(z[2 * i + 1]));
@@ -459,7 +459,25 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                         put16(znext, NT * j + cb + 16 * s, o);
                     }
                     publish(r_xfree(0), r_xfree(xh), true);
+                };
+                wait_full(0);      // G_0
+                wait_full(2);      // H_0
+                blend(0, 2, false);
+                wait_full(1);      // H_1: X1 <- tanh(H_1) - z (tile 1), off the critical path
+#pragma unroll 1
+                for (int s = 0; s < 3; ++s) {
+                    uint32_t h[16], z[16];
+                    tmem_ld16(xcol(1) + tcol + 16u * s, h);
+                    tmem_ld16(T_Z + (uint32_t)XC + tcol + 16u * s, z);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+                        h[i] = __float_as_uint(tanh_fast(__uint_as_float(h[i])) - __uint_as_float(z[i]));
+                    tmem_st16(xcol(1) + tcol + 16u * s, h);
                 }
+                tmem_st_wait();
+                wait_full(0);      // G_1
+                blend(1, 1, true);
                 // both tiles of z' are written (the arrivals above already ordered the writes)
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(r_zready);
