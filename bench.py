@@ -51,6 +51,7 @@ NCU_TRAFFIC = {
     (2, "wm_tc_kernel"): (23_903_744 + 3_584, "profiles/r1_tc_v6.md"),
     (3, "wm_tc2_kernel"): (56_579_840 + 713_472, "profiles/r1_tc2_v2.md"),
     (5, "wm_tcg_kernel"): (3_450_484_000 + 61_085_952, "profiles/r1_tcg_v1.md"),
+    (7, "wm_tct_kernel"): (24_100_608 + 2_048, "profiles/r1_tct_v1.md"),
 }
 
 
