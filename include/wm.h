@@ -149,7 +149,11 @@ int wm_check(wm_ctx* ctx, void* cuda_stream);
 /* End-to-end convenience entry: same computation as wm_rollout_score followed by wm_topk, with HOST buffers.
  * Copies the inputs host->device into ctx-owned staging, runs both steps on `cuda_stream`, copies scores
  * ([B] fp32, may be NULL to skip) and idx ([S,k] int32) back, and synchronises the stream before returning.
- * subgraph_offsets must be non-NULL (top-k needs segments).  Used by bench.py's e2e leg. */
+ * subgraph_offsets must be non-NULL (top-k needs segments) and, like every input here, a HOST array (it is read on
+ * the host to plan the copies).  From 65,536 candidates on, the call is pipelined internally over chunks of whole
+ * subgraphs (copies on a ctx-owned stream overlap the kernels of the previous chunk; everything is ordered after the
+ * work already queued on `cuda_stream` and complete when the call returns); results are bit-identical to the
+ * unpipelined sequence.  Concurrent calls on one ctx are serialised.  Used by bench.py's e2e leg. */
 int wm_score_topk_host(wm_ctx* ctx,
                        const float* init_states, const int32_t* action_ids, const int32_t* action_params,
                        const int32_t* lengths, const float* hw_feats, const int32_t* subgraph_offsets,

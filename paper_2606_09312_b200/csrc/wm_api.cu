@@ -261,6 +261,15 @@ void wm_free(wm_ctx* ctx) {
         delete w;
     }
     for (void* p : ctx->allocs) cudaFree(p);
+    if (ctx->hs_copy) cudaStreamDestroy(ctx->hs_copy);
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->hs_k[i]) cudaStreamDestroy(ctx->hs_k[i]);
+        if (ctx->hev_done[i]) cudaEventDestroy(ctx->hev_done[i]);
+    }
+    if (ctx->hev_start) cudaEventDestroy(ctx->hev_start);
+    for (int i = 0; i < 8; ++i)
+        if (ctx->hev_copy[i]) cudaEventDestroy(ctx->hev_copy[i]);
+    if (ctx->h_off) cudaFreeHost(ctx->h_off);
     delete ctx;
 }
 
@@ -419,6 +428,18 @@ int wm_check(wm_ctx* ctx, void* cuda_stream) {
     return (int)(word & 0x7fffffffu);
 }
 
+// wm_score_topk_host splits a call into chunks of whole subgraphs of at least this many candidates (WM_HOST_CHUNK_MIN
+// in the environment overrides it: the tests use a small value to exercise the chunked path on small batches)
+static int64_t host_chunk_min() {
+    static const int64_t v = [] {
+        const char* e = getenv("WM_HOST_CHUNK_MIN");
+        const long long x = e ? atoll(e) : 0;
+        return (int64_t)(x > 0 ? x : 16384);
+    }();
+    return v;
+}
+#define kHostChunkMin host_chunk_min()
+
 int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* action_ids,
                        const int32_t* action_params, const int32_t* lengths, const float* hw_feats,
                        const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
@@ -446,7 +467,23 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
     const size_t b_ids = up16((size_t)B * T_max * 4), b_par = up16((size_t)B * T_max * m.P * 4);
     const size_t b_len = up16((size_t)B * 4), b_off = up16((size_t)(S + 1) * 4);
     const size_t b_sc = up16((size_t)B * 4), b_idx = up16((size_t)S * k * 4);
-    const size_t need = b_z0 + b_hw + b_ids + b_par + b_len + b_off + b_sc + b_idx;
+    // Chunk plan: up to 4 chunks of whole subgraphs with about equal candidate counts.  The copy of chunk i+1 then
+    // overlaps the kernels of chunk i (PCIe and the rollout kernel are about equally long on the bf16 configs), and
+    // consecutive chunks' kernels run on alternating streams so that a chunk too small to fill the GPU does not idle it.
+    // (at least kHostChunkMin candidates per chunk: below that the extra launches cost more than the overlap gains)
+    // (measured: cfg 3, 65,536 candidates, +33 %; cfg 2, 32,768 candidates / 1 ms per call, -10 % with 2 or 4 chunks)
+    int nch = B >= 4 * kHostChunkMin ? 4 : 1;
+    nch = nch > S ? S : nch;
+    int cs[5] = {0, 0, 0, 0, 0};
+    if (nch > 1) {
+        int c = 1;
+        for (int s = 1; s < S && c < nch; ++s)
+            if ((int64_t)subgraph_offsets[s] * nch >= (int64_t)B * c) cs[c++] = s;
+        nch = c;
+        cs[nch] = S;
+    }
+    const size_t b_reb = up16((size_t)(S + 5) * 4);
+    const size_t need = b_z0 + b_hw + b_ids + b_par + b_len + b_off + b_sc + b_idx + b_reb;
     if (ws->stage_cap < need) {
         if (ws->stage) {
             WM_CUDA_TRY(cudaStreamSynchronize(st));
@@ -465,8 +502,75 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
     int32_t* dlen = (int32_t*)p; p += b_len;
     int32_t* doff = (int32_t*)p; p += b_off;
     float* dsc = (float*)p; p += b_sc;
-    int32_t* didx = (int32_t*)p;
+    int32_t* didx = (int32_t*)p; p += b_idx;
+    int32_t* dreb = (int32_t*)p;
     const auto H2D = cudaMemcpyHostToDevice;
+    if (nch > 1) {
+        std::lock_guard<std::mutex> host_lock(ctx->host_mu);
+        if (!ctx->hs_copy) {
+            WM_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->hs_copy, cudaStreamNonBlocking));
+            for (int i = 0; i < 2; ++i) {
+                WM_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->hs_k[i], cudaStreamNonBlocking));
+                WM_CUDA_TRY(cudaEventCreateWithFlags(&ctx->hev_done[i], cudaEventDisableTiming));
+            }
+            WM_CUDA_TRY(cudaEventCreateWithFlags(&ctx->hev_start, cudaEventDisableTiming));
+            for (int i = 0; i < 8; ++i) WM_CUDA_TRY(cudaEventCreateWithFlags(&ctx->hev_copy[i], cudaEventDisableTiming));
+        }
+        if (ctx->h_off_cap < (size_t)(S + 5)) {
+            if (ctx->h_off) WM_CUDA_TRY(cudaFreeHost(ctx->h_off));
+            ctx->h_off = nullptr;
+            WM_CUDA_TRY(cudaMallocHost(&ctx->h_off, (size_t)(S + 5 + 1024) * 4));
+            ctx->h_off_cap = (size_t)(S + 5 + 1024);
+        }
+        // per-chunk offsets rebased to the chunk's first candidate (the rollout kernel indexes candidates from 0)
+        int reb_at[4];
+        {
+            int o = 0;
+            for (int c = 0; c < nch; ++c) {
+                reb_at[c] = o;
+                for (int s = cs[c]; s <= cs[c + 1]; ++s) ctx->h_off[o++] = subgraph_offsets[s] - subgraph_offsets[cs[c]];
+            }
+        }
+        cudaStream_t cp = ctx->hs_copy;
+        WM_CUDA_TRY(cudaEventRecord(ctx->hev_start, st));     // everything below is ordered after prior work on `st`
+        WM_CUDA_TRY(cudaStreamWaitEvent(cp, ctx->hev_start, 0));
+        for (int i = 0; i < 2; ++i) WM_CUDA_TRY(cudaStreamWaitEvent(ctx->hs_k[i], ctx->hev_start, 0));
+        WM_CUDA_TRY(cudaMemcpyAsync(dz0, init_states, (size_t)S * m.d * 4, H2D, cp));
+        if (m.H) WM_CUDA_TRY(cudaMemcpyAsync(dhw, hw_feats, (size_t)S * m.H * 4, H2D, cp));
+        WM_CUDA_TRY(cudaMemcpyAsync(doff, subgraph_offsets, (size_t)(S + 1) * 4, H2D, cp));
+        WM_CUDA_TRY(cudaMemcpyAsync(dreb, ctx->h_off, (size_t)(S + nch) * 4, H2D, cp));
+        for (int c = 0; c < nch; ++c) {
+            const int s0 = cs[c], Sc = cs[c + 1] - cs[c];
+            const int64_t c0 = subgraph_offsets[s0], Bc = (int64_t)subgraph_offsets[cs[c + 1]] - c0;
+            if (Bc > 0) {
+                WM_CUDA_TRY(cudaMemcpyAsync(dlen + c0, lengths + c0, (size_t)Bc * 4, H2D, cp));
+                if (T_max > 0) {
+                    WM_CUDA_TRY(cudaMemcpyAsync(dids + c0 * T_max, action_ids + c0 * T_max, (size_t)Bc * T_max * 4, H2D, cp));
+                    WM_CUDA_TRY(cudaMemcpyAsync(dpar + c0 * T_max * m.P, action_params + c0 * T_max * m.P,
+                                                (size_t)Bc * T_max * m.P * 4, H2D, cp));
+                }
+            }
+            WM_CUDA_TRY(cudaEventRecord(ctx->hev_copy[c], cp));
+            cudaStream_t ks = ctx->hs_k[c & 1];
+            WM_CUDA_TRY(cudaStreamWaitEvent(ks, ctx->hev_copy[c], 0));
+            if (Bc > 0) {
+                const int rc = wm_rollout_score(ctx, dz0 + (size_t)s0 * m.d, dids + c0 * T_max, dpar + c0 * T_max * m.P,
+                                                dlen + c0, dhw + (size_t)s0 * m.H, dsc + c0, dreb + reb_at[c], Bc, Sc, T_max, ks);
+                if (rc != WM_OK) return rc;
+            }
+            // global offsets + the global score array: the indices come out global
+            const int rc2 = wm_topk(dsc, doff + s0, Sc, k, didx + (size_t)s0 * k, ks);
+            if (rc2 != WM_OK) return rc2;
+        }
+        for (int i = 0; i < 2; ++i) {
+            WM_CUDA_TRY(cudaEventRecord(ctx->hev_done[i], ctx->hs_k[i]));
+            WM_CUDA_TRY(cudaStreamWaitEvent(st, ctx->hev_done[i], 0));
+        }
+        if (scores_out && B) WM_CUDA_TRY(cudaMemcpyAsync(scores_out, dsc, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+        WM_CUDA_TRY(cudaMemcpyAsync(idx_out, didx, (size_t)S * k * 4, cudaMemcpyDeviceToHost, st));
+        WM_CUDA_TRY(cudaStreamSynchronize(st));
+        return WM_OK;
+    }
     WM_CUDA_TRY(cudaMemcpyAsync(dz0, init_states, (size_t)S * m.d * 4, H2D, st));
     if (m.H) WM_CUDA_TRY(cudaMemcpyAsync(dhw, hw_feats, (size_t)S * m.H * 4, H2D, st));
     if (B && T_max) {

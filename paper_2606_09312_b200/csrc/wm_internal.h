@@ -87,6 +87,13 @@ struct wm_ctx {
     std::vector<wm::Workspace*> pool;
     std::vector<void*> allocs;   // every device allocation owned by the ctx (weights)
     std::atomic<int64_t> launches{0};
+    // wm_score_topk_host pipelines a call by chunks of whole subgraphs: a copy stream, two compute streams, events and
+    // a pinned staging buffer for the per-chunk (rebased) offsets; created on first use
+    std::mutex host_mu;
+    cudaStream_t hs_copy = nullptr, hs_k[2] = {nullptr, nullptr};
+    cudaEvent_t hev_start = nullptr, hev_done[2] = {nullptr, nullptr}, hev_copy[8] = {};
+    int32_t* h_off = nullptr;
+    size_t h_off_cap = 0;
 };
 
 namespace wm {

@@ -4,6 +4,9 @@ import sys
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+# the library pipelines wm_score_topk_host by chunks of at least this many candidates (default 16384): a small value
+# makes the chunked path run on the small batches of the tests; it must be set before libwm.so is first used
+os.environ.setdefault("WM_HOST_CHUNK_MIN", "1024")
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 

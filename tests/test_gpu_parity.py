@@ -212,9 +212,12 @@ def test_two_streams_share_one_ctx(wm):
     wm.wm_free(ctx)
 
 
-def test_host_entry_matches_device_entry(wm):
+@pytest.mark.parametrize("S,per", [(3, 200), (4, 1100), (7, 900)])
+def test_host_entry_matches_device_entry(wm, S, per):
+    """wm_score_topk_host (host buffers; pipelined by chunks of whole subgraphs, here forced small through
+    WM_HOST_CHUNK_MIN in conftest.py) returns bit-identical scores and indices to the device-pointer entry points."""
     import torch
-    cfg = gen.get_config(2).scaled(S=3, per_subgraph=200)
+    cfg = gen.get_config(2).scaled(S=S, per_subgraph=per)
     b = gen.make_inputs(cfg)
     ctx = _ctx(wm, cfg)
     y = gpu_scores(ctx, b)
