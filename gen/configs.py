@@ -11,12 +11,13 @@ from typing import Tuple
 KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH = 0, 1, 2, 3
 DTYPE_FP32, DTYPE_BF16 = 0, 1
 EMBED_LINEAR, EMBED_BUCKET = 0, 1
+PHI_MEAN, PHI_STRUCT = 0, 1     # action features of the ranker: mean action embedding | structured statistics (f2)
 
 
 @dataclass(frozen=True)
 class WMConfig:
     name: str
-    number: int                 # 1..5 (BASELINE.json configs[number-1]); 6, 7 = NEXT row f1
+    number: int                 # 1..5 (BASELINE.json configs[number-1]); 6, 7 = NEXT row f1; 8, 9 = NEXT row f2
     kind: int                   # KIND_*
     dtype: int                  # DTYPE_*
     embed: int                  # EMBED_*
@@ -42,6 +43,7 @@ class WMConfig:
     prefix_children: int = 0    # cfg 4: children per parent (0 = no shared-prefix structure)
     prefix_cut_lo: int = 0
     prefix_cut_hi: int = 0
+    phi_kind: int = PHI_MEAN    # PHI_STRUCT: the paper's structured action features (S25)
 
     @property
     def B(self) -> int:
@@ -52,8 +54,14 @@ class WMConfig:
         return 1000 + self.number
 
     @property
+    def phi_dim(self) -> int:
+        """Width of phi: d_a for the mean action embedding; per-type counts, length and per-slot sum / mean / max of
+        log2 params for the structured form."""
+        return self.d_a if self.phi_kind == PHI_MEAN else self.n_types + 1 + 3 * self.P
+
+    @property
     def scorer_in(self) -> int:
-        return self.d + self.d_a + self.H
+        return self.d + self.phi_dim + self.H
 
     def scaled(self, S: int | None = None, per_subgraph: int | None = None) -> "WMConfig":
         """Same model, smaller batch (parity-test and cpu-baseline samples)."""
@@ -99,6 +107,15 @@ CONFIGS = {
     7: WMConfig("f1_transh_evolution_round", 7, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, S=16, per_subgraph=2048,
                 T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
                 param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(512, 512), k=64),
+    # NEXT row f2: the paper's structured action features phi in place of the mean
+    # action embedding.  8 = cfg 1's shapes (fp32, the parity case), 9 = cfg 2's shapes and batch (the measurement case).
+    8: WMConfig("f2_structphi_tiny_fp32", 8, KIND_MLP, DTYPE_FP32, EMBED_LINEAR, S=1, per_subgraph=64, T_max=8,
+                len_dist="uniform", len_lo=0, len_hi=8, n_types=16, P=4, param_dist="uniform", param_hi=64,
+                n_buckets=0, d=64, d_a=32, hidden=128, H=8, scorer_widths=(128,), k=8, phi_kind=PHI_STRUCT),
+    9: WMConfig("f2_structphi_evolution_round", 9, KIND_MLP_LN, DTYPE_BF16, EMBED_LINEAR, S=16, per_subgraph=2048,
+                T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
+                param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(512, 512), k=64,
+                phi_kind=PHI_STRUCT),
 }
 
 

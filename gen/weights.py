@@ -6,6 +6,10 @@ Draw order (one Generator(PCG64(weight_seed))):
 Matrices ~ N(0, 1/fan_in) (variance), tables ~ N(0,1), biases ~ N(0, 1/fan_in) of their layer,
 gamma = 1 + 0.1 N(0,1), beta = 0.1 N(0,1).  bf16 configs: every tensor is rounded to the nearest-even
 bf16 value and stored as fp32 (S14), so every consumer sees identical weights.
+Structured-phi configs (f2): the phi columns of Ws0 are scaled, before the bf16 rounding, by the inverse of the
+feature's range (counts and length 1/T_max, sums 1/(10 T_max), means and maxima 1/10; log2 of a parameter <= 1024 is
+<= 10), as a trained ranker's first layer would be for raw count features, so that the latent still matters to the
+score.  Version-2 header: the version-1 fields followed by uint32 phi_kind.
 """
 from __future__ import annotations
 
@@ -14,7 +18,8 @@ from typing import Dict, List
 
 import numpy as np
 
-from .configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, EMBED_BUCKET)
+from .configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, EMBED_BUCKET,
+                      PHI_STRUCT)
 
 MAGIC = b"WMW1"
 VERSION = 1
@@ -96,11 +101,23 @@ def make_weights(cfg: WMConfig) -> Dict[str, np.ndarray]:
         else:  # bias of the layer drawn just before it
             fan_in = shapes[_matrix_of(name)][1]
             t = rng.standard_normal(shp) / np.sqrt(fan_in)
+        if name == "Ws0" and cfg.phi_kind == PHI_STRUCT:
+            t = t * phi_column_scale(cfg)[None, :]
         t = t.astype(np.float32)
         if cfg.dtype == DTYPE_BF16:
             t = round_to_bf16(t)
         w[name] = t
     return w
+
+
+def phi_column_scale(cfg: WMConfig) -> np.ndarray:
+    """Per-input-column factor of Ws0 for structured-phi configs (1 for the z and hw columns)."""
+    sc = np.ones(cfg.scorer_in)
+    o, nt, P, T = cfg.d, cfg.n_types, cfg.P, float(cfg.T_max)
+    sc[o:o + nt + 1] = 1.0 / T                              # per-type counts, length
+    sc[o + nt + 1:o + nt + 1 + P] = 1.0 / (10.0 * T)        # sums of log2 params
+    sc[o + nt + 1 + P:o + nt + 1 + 3 * P] = 0.1             # means, maxima
+    return sc
 
 
 def _matrix_of(bias: str) -> str:
@@ -109,10 +126,12 @@ def _matrix_of(bias: str) -> str:
 
 def header_bytes(cfg: WMConfig) -> bytes:
     widths = list(cfg.scorer_widths) + [0] * (MAX_SCORER_HIDDEN - len(cfg.scorer_widths))
-    return MAGIC + struct.pack(
+    version = VERSION if cfg.phi_kind == 0 else 2      # version 2 = version 1 + a trailing uint32 phi_kind
+    hdr = MAGIC + struct.pack(
         "<12I%dIf" % MAX_SCORER_HIDDEN,
-        VERSION, cfg.kind, cfg.dtype, cfg.embed, cfg.d, cfg.d_a, cfg.hidden, cfg.n_types, cfg.P,
+        version, cfg.kind, cfg.dtype, cfg.embed, cfg.d, cfg.d_a, cfg.hidden, cfg.n_types, cfg.P,
         cfg.n_buckets, cfg.H, len(cfg.scorer_widths) + 1, *widths, cfg.ln_eps)
+    return hdr if version == 1 else hdr + struct.pack("<I", cfg.phi_kind)
 
 
 def write_weight_file(path: str, cfg: WMConfig, weights: Dict[str, np.ndarray]) -> None:

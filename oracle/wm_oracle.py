@@ -6,6 +6,7 @@ What it computes is the plain definition (no approximation in the method, so no 
     z_t = F(z_{t-1}, a_t),  t = 1..len                     PAPER.md:68-71 Eq.1, :162 Eq.8, :166 (recurrent rollout)
     steps with t > len leave z unchanged                   PAPER.md:176 Eq.11 (rollout mask m_t)
     phi = mean_t a_t (0 if len = 0)                        PAPER.md:186 (action features; BASELINE.json cfg 1 form)
+      or, phi_kind = PHI_STRUCT, the paper's structured statistics (phi_struct below; S25)
     y   = G([z_T ; phi ; h])                               PAPER.md:122 Eq.3, :188 Eq.12
     top-k per subgraph by (score desc, index asc)
 
@@ -18,7 +19,8 @@ mask) and `rollout_score_scalar` (pure per-candidate python loops, math.erf) —
 
 Pins (tests/test_oracle_pins.py): P1..P13 of SURVEY.md §8(c) — hand-expanded 2x3 MLP step and GRU step
 (values in tests/golden/), closed forms, torch float64 library cross-checks, scalar-vs-vector brute
-force, top-k vs full sort.  The paper prints no worked numeric example of this path, so the composition
+force, top-k vs full sort; P14/P15 the TransH step, P16/P17 the structured phi (hand-worked sequence in
+tests/golden/p16_phi_struct.txt, closed forms, a scorer that reads single features).  The paper prints no worked numeric example of this path, so the composition
 at full size rests on those pins: beyond them, parity unpinned.
 """
 from __future__ import annotations
@@ -32,6 +34,7 @@ from scipy.special import erf as _erf
 
 KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH = 0, 1, 2, 3
 EMBED_LINEAR, EMBED_BUCKET = 0, 1
+PHI_MEAN, PHI_STRUCT = 0, 1
 F64 = np.float64
 
 
@@ -131,6 +134,30 @@ def step_transh(z, a, W_w, W_d, W1, b1, W2, b2, eps: float = TRANSH_EPS) -> np.n
     return v / np.sqrt(np.sum(v * v, axis=-1, keepdims=True) + eps)
 
 
+def phi_struct(ids, params, n_types: int) -> np.ndarray:
+    """Structured action features of ONE action sequence, given by its valid steps only (ids [len], params [len,P]).
+
+    PAPER.md:186: phi(a_1:T) is "a structured action feature vector derived from the scheduling actions, including
+    statistics such as action counts, sequence length, and action-specific numeric attributes" — the paper lists the
+    ingredients, not a layout; reading S25 fixes it as, in this order,
+        c_k   = #{t : id_t = k},             k = 0..n_types-1     (action counts)
+        len                                                       (sequence length)
+        s_j   = sum_t log2 p_tj,             j = 0..P-1           (numeric attributes: total per parameter slot)
+        m_j   = s_j / len                                         (mean; 0 for an empty sequence)
+        x_j   = max_t log2 p_tj                                   (largest; 0 for an empty sequence)
+    Returns float64 [n_types + 1 + 3P]."""
+    ids = np.asarray(ids).astype(np.int64).reshape(-1)
+    par = np.asarray(params)
+    n, P = ids.shape[0], par.shape[-1]
+    counts = np.array([np.count_nonzero(ids == k) for k in range(n_types)], dtype=F64)
+    if n == 0:
+        s = m = x = np.zeros(P, dtype=F64)
+    else:
+        lp = np.log2(par.reshape(n, P).astype(F64))
+        s, m, x = lp.sum(axis=0), lp.sum(axis=0) / n, lp.max(axis=0)
+    return np.concatenate([counts, [float(n)], s, m, x])
+
+
 def scorer(x: np.ndarray, w: Dict[str, np.ndarray], n_layers: int) -> np.ndarray:
     """G as an MLP: hidden linears followed by GELU, last linear plain (S8). Returns [...]."""
     for i in range(n_layers):
@@ -176,8 +203,9 @@ def _step(w, z, a, eps):
 
 def rollout_score_vec(w: Dict[str, np.ndarray], init_states, action_ids, action_params, lengths, hw_feats,
                       subgraph_offsets: Optional[np.ndarray], n_buckets: int = 0, ln_eps: float = 1e-5,
-                      return_latent: bool = False):
-    """Scores [B] float64.  subgraph_offsets None => per-candidate init_states [B,d] / hw_feats [B,H] (S1/S2)."""
+                      return_latent: bool = False, phi_kind: int = PHI_MEAN):
+    """Scores [B] float64.  subgraph_offsets None => per-candidate init_states [B,d] / hw_feats [B,H] (S1/S2).
+    phi_kind = PHI_STRUCT replaces the mean action embedding by phi_struct of the candidate's valid steps."""
     ids = np.asarray(action_ids)
     par = np.asarray(action_params)
     lens = np.asarray(lengths).astype(np.int64)
@@ -213,6 +241,9 @@ def rollout_score_vec(w: Dict[str, np.ndarray], init_states, action_ids, action_
             asum[idx] += a
             z[idx] = _step(w, z[idx], a, ln_eps)       # masked rows keep z unchanged
         phi = np.where(ln[:, None] > 0, asum / np.maximum(ln, 1)[:, None], 0.0)
+        if phi_kind == PHI_STRUCT:
+            n_types = w["E"].shape[0] if "E" in w else w["Tbl"].shape[0] // (P * n_buckets)
+            phi = np.stack([phi_struct(ids[lo + i, :ln[i]], par[lo + i, :ln[i], :], n_types) for i in range(n)])
         scores[lo:hi] = scorer(np.concatenate([z, phi, h], axis=-1), w, nl)
         if return_latent:
             lat[lo:hi] = z
@@ -220,7 +251,7 @@ def rollout_score_vec(w: Dict[str, np.ndarray], init_states, action_ids, action_
 
 
 def rollout_score_scalar(w, init_states, action_ids, action_params, lengths, hw_feats, subgraph_offsets,
-                         n_buckets: int = 0, ln_eps: float = 1e-5) -> np.ndarray:
+                         n_buckets: int = 0, ln_eps: float = 1e-5, phi_kind: int = PHI_MEAN) -> np.ndarray:
     """Pure-python per-candidate loops (tiny inputs only); independent of the vector code above."""
     W = {k: np.asarray(v, F64).tolist() for k, v in w.items()}
     ids = np.asarray(action_ids).tolist()
@@ -294,6 +325,18 @@ def rollout_score_scalar(w, init_states, action_ids, action_params, lengths, hw_
                 else:
                     z = v
         phi = [x / lens[b] for x in asum] if lens[b] > 0 else [0.0] * da
+        if phi_kind == PHI_STRUCT:   # S25, by counting loops (independent of phi_struct above)
+            n_types = len(W["E"]) if "E" in W else len(W["Tbl"]) // (P * n_buckets)
+            cnt = [0.0] * n_types
+            tot = [0.0] * P
+            big = [0.0] * P
+            for t in range(lens[b]):
+                cnt[ids[b][t]] += 1.0
+                for j in range(P):
+                    l2 = math.log2(par[b][t][j])
+                    tot[j] += l2
+                    big[j] = l2 if t == 0 else max(big[j], l2)
+            phi = cnt + [float(lens[b])] + tot + [v / lens[b] if lens[b] > 0 else 0.0 for v in tot] + big
         x = z + phi + list(hw[s])
         nl = _n_scorer_layers(w)
         for i in range(nl):
@@ -375,6 +418,11 @@ def read_weight_file(path: str):
                n_types=n_types, P=P, n_buckets=n_buckets, H=H, n_scorer_layers=n_lin,
                scorer_widths=widths, ln_eps=eps)
     pos = 4 + struct.calcsize("<12I6If")
+    hdr["phi_kind"] = PHI_MEAN
+    if version == 2:      # version 2 = version 1 + uint32 phi_kind
+        hdr["phi_kind"] = struct.unpack_from("<I", raw, pos)[0]
+        pos += 4
+    phi_dim = d_a if hdr["phi_kind"] == PHI_MEAN else n_types + 1 + 3 * P
     w = {}
 
     def take(name, *shape):
@@ -396,7 +444,7 @@ def read_weight_file(path: str):
         take("W1", hidden, d + d_a); take("b1", hidden); take("W2", d, hidden); take("b2", d)
     else:
         take("W_g", d, d + d_a); take("W_r", d, d + d_a); take("W_h", d, d + d_a)
-    dims = [d + d_a + H] + widths + [1]
+    dims = [d + phi_dim + H] + widths + [1]
     for i in range(n_lin):
         take(f"Ws{i}", dims[i + 1], dims[i]); take(f"bs{i}", dims[i + 1])
     if pos != len(raw):

@@ -13,20 +13,22 @@ import torch
 import gen
 import oracle
 from gen.configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH, DTYPE_FP32, EMBED_LINEAR,
-                         EMBED_BUCKET)
+                         EMBED_BUCKET, PHI_MEAN, PHI_STRUCT)
 
 
 def tiny_cfg(kind=KIND_MLP_LN, embed=EMBED_LINEAR, S=3, n=7, T=5, d=6, da=4, hid=8, H=3, widths=(5, 4),
-             number=9, len_lo=0):
+             number=9, len_lo=0, phi_kind=PHI_MEAN):
     return WMConfig("tiny", number, kind, DTYPE_FP32, embed, S=S, per_subgraph=n, T_max=T,
                     len_dist="uniform", len_lo=len_lo, len_hi=T, n_types=5, P=3,
                     param_dist="loguniform", param_hi=1024, n_buckets=40 if embed == EMBED_BUCKET else 0,
-                    d=d, d_a=da, hidden=0 if kind == KIND_GRU else hid, H=H, scorer_widths=widths, k=3)
+                    d=d, d_a=da, hidden=0 if kind == KIND_GRU else hid, H=H, scorer_widths=widths, k=3,
+                    phi_kind=phi_kind)
 
 
 def run_vec(cfg, w, b, **kw):
     return oracle.rollout_score_vec(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.hw_feats,
-                                    b.subgraph_offsets, n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps, **kw)
+                                    b.subgraph_offsets, n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps,
+                                    phi_kind=cfg.phi_kind, **kw)
 
 
 ALL_KINDS = [(KIND_MLP, EMBED_LINEAR), (KIND_MLP_LN, EMBED_LINEAR), (KIND_GRU, EMBED_BUCKET),
@@ -115,6 +117,79 @@ def test_p15_transh_closed_forms():
     vt = xt + ht @ torch.from_numpy(W2).T + torch.from_numpy(b2)
     np.testing.assert_allclose(oracle.step_transh(z, a, Ww, Wd, W1, b1, W2, b2),
                                torch.nn.functional.normalize(vt, dim=1, eps=0.0).numpy(), atol=1e-11)
+
+
+# ---- P16 / P17: structured action features (NEXT row f2, S25) -----------------------
+
+def test_p16_phi_struct_hand_worked(golden):
+    g = golden("p16_phi_struct.txt")
+    ids = [2, 0, 2]; par = [[1, 8], [4, 2], [16, 8]]
+    np.testing.assert_allclose(oracle.phi_struct(ids, par, 4), g["phi"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(oracle.phi_struct(ids[:1], par[:1], 4), g["phi_prefix1"], rtol=0, atol=0)
+    np.testing.assert_allclose(oracle.phi_struct([], np.zeros((0, 2), dtype=np.int32), 4), g["phi_empty"], rtol=0, atol=0)
+    # the fixture discriminates: swapping the parameter slots or the type ids must change the vector
+    assert np.abs(oracle.phi_struct(ids, [q[::-1] for q in par], 4) - np.array(g["phi"])).max() >= 1.0
+    assert np.abs(oracle.phi_struct([0, 2, 0], par, 4) - np.array(g["phi"])).max() >= 1.0
+
+
+def test_p17_phi_struct_closed_forms_and_placement():
+    rng = np.random.default_rng(17)
+    nt, P, n = 7, 3, 11
+    ids = rng.integers(0, nt, n); par = rng.integers(1, 1025, (n, P))
+    f = oracle.phi_struct(ids, par, nt)
+    c, ln, s, m, x = f[:nt], f[nt], f[nt + 1:nt + 1 + P], f[nt + 1 + P:nt + 1 + 2 * P], f[nt + 1 + 2 * P:]
+    assert f.shape == (nt + 1 + 3 * P,) and ln == n and c.sum() == n
+    np.testing.assert_array_equal(c, np.bincount(ids, minlength=nt))
+    # sum of log2 = log2 of the product (exact integers in python), mean = sum / len, max = log2 of the largest
+    for j in range(P):
+        prod = 1
+        for v in par[:, j]:
+            prod *= int(v)
+        assert abs(s[j] - math.log2(prod)) < 1e-11
+        assert abs(m[j] - math.log2(prod) / n) < 1e-12
+        assert x[j] == math.log2(int(par[:, j].max()))
+    # order of the steps does not matter; concatenation adds counts, lengths and sums and takes the larger maximum
+    perm = rng.permutation(n)
+    np.testing.assert_allclose(oracle.phi_struct(ids[perm], par[perm], nt), f, rtol=0, atol=1e-12)
+    fa, fb = oracle.phi_struct(ids[:4], par[:4], nt), oracle.phi_struct(ids[4:], par[4:], nt)
+    np.testing.assert_allclose(fa[:nt + 1 + P] + fb[:nt + 1 + P], f[:nt + 1 + P], rtol=0, atol=1e-12)
+    np.testing.assert_array_equal(np.maximum(fa[nt + 1 + 2 * P:], fb[nt + 1 + 2 * P:]), x)
+    # constant parameters 2^q: sum = q len, mean = max = q; all-ones parameters: every numeric attribute 0
+    fq = oracle.phi_struct(ids, np.full((n, P), 32), nt)
+    np.testing.assert_array_equal(fq[nt + 1:], [5.0 * n] * P + [5.0] * P + [5.0] * P)
+    assert not oracle.phi_struct(ids, np.ones((n, P), dtype=int), nt)[nt + 1:].any()
+    # placement in the ranker input [z_T ; phi ; h] (Eq.12): a one-linear scorer whose weight row is a unit vector
+    # returns exactly that feature of each candidate
+    cfg = tiny_cfg(KIND_MLP, EMBED_LINEAR, widths=(), phi_kind=PHI_STRUCT)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    F = cfg.phi_dim
+    assert w["Ws0"].shape == (1, cfg.d + F + cfg.H)
+    for col in (0, 2, cfg.n_types, cfg.n_types + 1, F - 1):
+        w1 = dict(w); w1["Ws0"] = np.zeros_like(w["Ws0"]); w1["Ws0"][0, cfg.d + col] = 1.0
+        w1["bs0"] = np.zeros_like(w["bs0"])
+        want = [oracle.phi_struct(b.action_ids[i, :b.lengths[i]], b.action_params[i, :b.lengths[i]], cfg.n_types)[col]
+                for i in range(b.B)]
+        np.testing.assert_allclose(run_vec(cfg, w1, b), want, rtol=0, atol=1e-13)
+    w1 = dict(w); w1["Ws0"] = np.zeros_like(w["Ws0"]); w1["Ws0"][0, cfg.d + F] = 1.0; w1["bs0"] = np.zeros_like(w["bs0"])
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    np.testing.assert_allclose(run_vec(cfg, w1, b), b.hw_feats[seg, 0].astype(np.float64), rtol=0, atol=0)
+
+
+@pytest.mark.parametrize("kind,embed", [(KIND_MLP, EMBED_LINEAR), (KIND_GRU, EMBED_BUCKET)])
+def test_p9_scalar_vs_vector_struct_phi(kind, embed):
+    cfg = tiny_cfg(kind, embed, phi_kind=PHI_STRUCT)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    ys = oracle.rollout_score_scalar(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.hw_feats,
+                                     b.subgraph_offsets, n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps,
+                                     phi_kind=PHI_STRUCT)
+    np.testing.assert_allclose(run_vec(cfg, w, b), ys, rtol=0, atol=1e-12)
+    # zero-length candidates see phi = 0: their score is G([z_0 ; 0 ; h])
+    z = np.where(b.lengths == 0)[0]
+    assert z.size > 0
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    x0 = np.concatenate([b.init_states[seg[z]], np.zeros((z.size, cfg.phi_dim)), b.hw_feats[seg[z]]], axis=1)
+    np.testing.assert_allclose(run_vec(cfg, w, b)[z], oracle.scorer(x0, w, len(cfg.scorer_widths) + 1), rtol=0,
+                               atol=1e-12)
 
 
 def test_p11_bucket_function(golden):
@@ -352,9 +427,9 @@ def test_p12_prefix_reuse_equals_scratch():
 # ---- generator / file format ----------------------------------------------------------------------------------
 
 def test_weight_file_roundtrip(tmp_path):
-    for n in (1, 2, 5, 6):
+    for n in (1, 2, 5, 6, 8, 9):
         cfg = gen.get_config(n)
-        if n != 1:
+        if n not in (1, 8):
             cfg = WMConfig(**{**cfg.__dict__, "d": 16, "d_a": 8, "hidden": 0 if n == 5 else 24,
                               "scorer_widths": (12, 10)})
         w = gen.make_weights(cfg)
@@ -362,6 +437,8 @@ def test_weight_file_roundtrip(tmp_path):
         gen.write_weight_file(p, cfg, w)
         hdr, w2 = oracle.read_weight_file(p)
         assert hdr["d"] == cfg.d and hdr["kind"] == cfg.kind and hdr["P"] == cfg.P
+        assert hdr["phi_kind"] == cfg.phi_kind and hdr["version"] == (1 if cfg.phi_kind == PHI_MEAN else 2)
+        assert w2["Ws0"].shape[1] == cfg.d + cfg.phi_dim + cfg.H
         assert list(w2.keys()) == gen.tensor_order(cfg)
         for kname in w:
             np.testing.assert_array_equal(w[kname], w2[kname])

@@ -65,4 +65,4 @@ def oracle_scores(cfg, weights, batch, per_candidate=False):
     return oracle.rollout_score_vec(weights, batch.init_states, batch.action_ids, batch.action_params,
                                     batch.lengths, batch.hw_feats,
                                     None if per_candidate else batch.subgraph_offsets,
-                                    n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps)
+                                    n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps, phi_kind=cfg.phi_kind)
