@@ -7,6 +7,8 @@
  *                                              recurrently                               PAPER.md:68-71 Eq.1, :162 Eq.8, :166
  *   steps t > len leave z unchanged            rollout mask m_t                          PAPER.md:176 Eq.11
  *   phi = mean_t a_t (0 when len = 0)          action features
+ *         or (WM_PHI_STRUCT) the paper's structured statistics: per-type action counts, sequence length and, per
+ *         parameter slot, the sum / mean / max over the steps of log2 p   (S25)
  *   y   = G([z_T ; phi ; h])                   ranking score                             PAPER.md:122 Eq.3, :188 Eq.12
  *   top-k per subgraph, (score desc, idx asc)  candidates prioritised for measurement
  *
@@ -66,6 +68,11 @@ extern "C" {
 #define WM_DTYPE_BF16   1
 #define WM_EMBED_LINEAR 0
 #define WM_EMBED_BUCKET 1
+#define WM_PHI_MEAN     0      /* phi = mean over the valid steps of the action embedding (BASELINE.json cfg 1)       */
+#define WM_PHI_STRUCT   1      /* phi = [c_0..c_{n_types-1} | len | s_0..s_{P-1} | m_0..m_{P-1} | x_0..x_{P-1}]:      */
+                               /* c_k = number of steps of type k, s_j / m_j / x_j = sum / mean / max over the valid   */
+                               /* steps of log2 p_tj, all 0 for an empty sequence (S25).       */
+                               /* n_types + 1 + 3P values; this build needs n_types + 1 + 3P <= d_a                    */
 
 /* wm_set_option keys */
 #define WM_OPT_PATH      1      /* 0 = auto (default), 1 = force the fp32 CUDA-core kernel, 2 = force tcgen05  */
@@ -86,19 +93,21 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
                                 /* 128-candidate tile, d = 256), 2 = wm_tc2_kernel (CTA pair per tile, d = 512),  */
                                 /* 3 = wm_tcg_kernel (CTA pair per tile, GRU transition, d = 384),             */
                                 /* 4 = wm_tct_kernel (TransH transition, d = 256)                              */
+    int32_t phi_kind;           /* WM_PHI_*: which action features G reads                                     */
 } wm_info;
 
 /* Read a WMW1 weight file (format below), convert to the kernels' layouts and copy to `device`.
  *   path     host path, NUL-terminated.
  *   device   CUDA device ordinal.
  *   ctx_out  receives the context (caller frees with wm_free).
- * File format (little-endian): "WMW1", then uint32 version(=1), kind, dtype, embed, d, d_a, hidden, n_types, P,
- * n_buckets, H, n_scorer_layers, uint32 scorer_widths[6], float ln_eps (80 bytes in all), then fp32 tensors,
- * row-major, in this order:
+ * File format (little-endian): "WMW1", then uint32 version, kind, dtype, embed, d, d_a, hidden, n_types, P,
+ * n_buckets, H, n_scorer_layers, uint32 scorer_widths[6], float ln_eps (80 bytes in all); version 2 files carry one
+ * more uint32, phi_kind (version 1 means WM_PHI_MEAN); then fp32 tensors, row-major, in this order:
  *   EMBED_LINEAR: E[n_types,d_a], W_p[d_a,P], b_p[d_a]        EMBED_BUCKET: Tbl[n_types*P*n_buckets, d_a]
  *   MLP / MLP_LN: W1[hidden,d+d_a], b1[hidden], W2[d,hidden], b2[d] (, gamma[d], beta[d])
  *   GRU:          W_g[d,d+d_a], W_r[d,d+d_a], W_h[d,d+d_a]
- *   G:            for each linear i: Ws_i[out_i,in_i], bs_i[out_i];  in_0 = d+d_a+H, out_last = 1
+ *   TRANSH:       W_w[d,d_a], W_d[d,d_a], then W1, b1, W2, b2 as for MLP
+ *   G:            for each linear i: Ws_i[out_i,in_i], bs_i[out_i];  in_0 = d+dim(phi)+H, out_last = 1
  * With dtype = bf16 every stored value is already bf16-representable (BASELINE.json cfg 2-5: "bf16 weights with
  * fp32 accumulate"); the tcgen05 path then runs bf16 x bf16 -> fp32 MMAs with an fp32 latent.
  * Errors: WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_UNSUPPORTED, WM_ERR_CUDA.  Synchronous. */

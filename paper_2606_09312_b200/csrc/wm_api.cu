@@ -111,9 +111,15 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         set_error("wm_load_weights: file shorter than the header");
         return WM_ERR_FORMAT;
     }
-    if (memcmp(magic, "WMW1", 4) != 0 || h.version != 1) {
+    if (memcmp(magic, "WMW1", 4) != 0 || (h.version != 1 && h.version != 2)) {
         fclose(f);
         set_error("wm_load_weights: bad magic or version");
+        return WM_ERR_FORMAT;
+    }
+    uint32_t phi_kind = WM_PHI_MEAN;   // version 2 = the version-1 header followed by uint32 phi_kind
+    if (h.version == 2 && (fread(&phi_kind, 4, 1, f) != 1 || phi_kind > WM_PHI_STRUCT)) {
+        fclose(f);
+        set_error("wm_load_weights: bad phi_kind");
         return WM_ERR_FORMAT;
     }
     const bool mlp = h.kind == WM_KIND_MLP || h.kind == WM_KIND_MLP_LN || h.kind == WM_KIND_TRANSH;
@@ -142,6 +148,13 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         ts.push_back(t);
     };
     const int d = h.d, da = h.d_a, hid = h.hidden;
+    // width of phi: the mean action embedding, or counts | len | per-slot sum, mean, max of log2 params (S25)
+    const int phi_dim = phi_kind == WM_PHI_MEAN ? da : (int)(h.n_types + 1 + 3 * h.P);
+    if (phi_dim > da) {   // the kernels keep phi in the rows / K-blocks of the action embedding
+        fclose(f);
+        set_error("wm_load_weights: structured phi needs n_types + 1 + 3 P <= d_a in this build");
+        return WM_ERR_UNSUPPORTED;
+    }
     if (h.embed == WM_EMBED_LINEAR) {
         add("E", h.n_types, da); add("W_p", da, h.P); add("b_p", da, 1);
     } else {
@@ -155,7 +168,7 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         add("W_g", d, d + da); add("W_r", d, d + da); add("W_h", d, d + da);
     }
     int sdim[kMaxScorerLinears + 1] = {};
-    sdim[0] = d + da + h.H;
+    sdim[0] = d + phi_dim + h.H;
     for (uint32_t i = 0; i + 1 < h.n_lin; ++i) sdim[i + 1] = h.widths[i];
     sdim[h.n_lin] = 1;
     for (uint32_t i = 0; i < h.n_lin; ++i) {
@@ -195,6 +208,8 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
     m.n_types = h.n_types; m.P = h.P; m.n_buckets = h.n_buckets; m.H = h.H; m.n_lin = h.n_lin;
     for (int i = 0; i <= kMaxScorerLinears; ++i) m.sdim[i] = sdim[i];
     m.ln_eps = h.ln_eps;
+    m.phi_kind = (int)phi_kind;
+    m.phi_dim = phi_dim;
 
     int rc = WM_OK;
     auto find = [&](const std::string& n) -> const HostTensor* {
@@ -285,6 +300,7 @@ int wm_get_info(const wm_ctx* ctx, wm_info* o) {
     o->ln_eps = m.ln_eps;
     o->path = tc_supported(ctx) ? 2 : 1;
     o->tc_variant = tc_supported(ctx);
+    o->phi_kind = m.phi_kind;
     return WM_OK;
 }
 

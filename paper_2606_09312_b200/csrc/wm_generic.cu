@@ -16,6 +16,7 @@ namespace wm {
 
 struct GenericParams {
     int kind, embed, d, da, hidden, n_types, P, n_buckets, H, n_lin;
+    int phi_kind, phi_dim;   // WM_PHI_*; rows of phi in the scorer input (<= da)
     int sdim[kMaxScorerLinears + 1];
     int maxw;        // rows of buffer Hb
     int alt_rows;    // rows of the region that holds V, AS, Y (and the scorer's second ping-pong buffer)
@@ -117,7 +118,9 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
     float* Hb = X + (size_t)(K1 + H) * R;              // [maxw][R]
     float* ALT = Hb + (size_t)p.maxw * R;              // [alt_rows][R]: V | AS | Y   (scorer: ping-pong buffer)
     float* V = ALT;                                    // [d][R]
-    float* AS = V + (size_t)d * R;                     // [da][R]
+    float* AS = V + (size_t)d * R;                     // [da][R] running sum of a (WM_PHI_MEAN), or the running
+                                                       // statistics of WM_PHI_STRUCT: counts [n_types], then per
+                                                       // parameter slot sum [P] and max [P] of log2 p
     float* Y = AS + (size_t)da * R;                    // [(d+da)][R], GRU and TransH only
     float* LP = ALT + (size_t)p.alt_rows * R;          // [R][P] log2(param) or bucket index (as int bits)
     float* RED = LP + (size_t)R * P;                   // [G][R] reduction scratch, G = threads / R
@@ -177,6 +180,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     }
                 }
                 m_id[tid] = id;
+                if (p.phi_kind == WM_PHI_STRUCT && t < m_len[tid]) AS[(size_t)id * R + tid] += 1.0f;
             }
             for (int e = tid; e < R * P; e += kGenericThreads) {
                 const int r = e / P, j = e % P;
@@ -186,6 +190,13 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     if (prm < 1) {
                         atomicOr(a.fault, WM_FAULT_PARAM);
                         prm = 1;
+                    }
+                    if (p.phi_kind == WM_PHI_STRUCT) {   // (r, j) belongs to this thread alone
+                        const float l2 = log2f((float)prm);
+                        float* sum = AS + (size_t)(p.n_types + j) * R + r;
+                        float* mx = AS + (size_t)(p.n_types + P + j) * R + r;
+                        *sum += l2;
+                        *mx = fmaxf(*mx, l2);
                     }
                     if (p.embed == WM_EMBED_LINEAR) {
                         v = log2f((float)prm);
@@ -215,7 +226,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                             v += __ldg(p.Tbl + ((size_t)(id * P + q) * p.n_buckets + bk) * da + j);
                         }
                     }
-                    AS[e] += v;   // a4: running sum for phi
+                    if (p.phi_kind == WM_PHI_MEAN) AS[e] += v;   // a4: running sum for phi
                 }
                 X[(size_t)(d + j) * R + r] = v;
             }
@@ -334,14 +345,29 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
         }
 
         // ---- a4/a5: x = [z_T ; phi ; hw], scorer MLP
-        for (int e = tid; e < da * R; e += kGenericThreads) {
-            const int r = e % R;
+        const int F = p.phi_dim, NT = p.n_types;
+        for (int e = tid; e < F * R; e += kGenericThreads) {
+            const int r = e % R, j = e / R;
             const int len = m_len[r];
-            X[(size_t)d * R + e] = len > 0 ? AS[e] / (float)len : 0.0f;
+            float v;
+            if (p.phi_kind == WM_PHI_MEAN) {
+                v = len > 0 ? AS[e] / (float)len : 0.0f;
+            } else if (j < NT) {                       // counts (S25)
+                v = AS[e];
+            } else if (j == NT) {                      // length
+                v = (float)len;
+            } else if (j < NT + 1 + P) {               // sums of log2 p
+                v = AS[(size_t)(j - 1) * R + r];
+            } else if (j < NT + 1 + 2 * P) {           // means
+                v = len > 0 ? AS[(size_t)(j - 1 - P) * R + r] / (float)len : 0.0f;
+            } else {                                   // maxima (log2 p >= 0, so the running max starts at 0)
+                v = AS[(size_t)(j - 1 - P) * R + r];
+            }
+            X[(size_t)d * R + e] = v;
         }
         for (int e = tid; e < H * R; e += kGenericThreads) {
             const int r = e % R, j = e / R;
-            X[(size_t)K1 * R + e] = m_cand[r] >= 0 ? __ldg(a.hw_feats + (size_t)m_seg[r] * H + j) : 0.0f;
+            X[(size_t)(d + F) * R + e] = m_cand[r] >= 0 ? __ldg(a.hw_feats + (size_t)m_seg[r] * H + j) : 0.0f;
         }
         __syncthreads();
         const float* in = X;
@@ -411,6 +437,7 @@ int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st) {
     GenericParams p;
     p.kind = m.kind; p.embed = m.embed; p.d = m.d; p.da = m.d_a; p.hidden = m.hidden; p.n_types = m.n_types;
     p.P = m.P; p.n_buckets = m.n_buckets; p.H = m.H; p.n_lin = m.n_lin;
+    p.phi_kind = m.phi_kind; p.phi_dim = m.phi_dim;
     for (int i = 0; i <= kMaxScorerLinears; ++i) p.sdim[i] = m.sdim[i];
     p.ln_eps = m.ln_eps;
     p.E = m.E; p.WpT = m.WpT; p.bp = m.bp; p.Tbl = m.Tbl;

@@ -21,8 +21,10 @@ struct Model {
     int kind = 0, dtype = 0, embed = 0;
     int d = 0, d_a = 0, hidden = 0, n_types = 0, P = 0, n_buckets = 0, H = 0;
     int n_lin = 0;                       // linears of G
-    int sdim[kMaxScorerLinears + 1] = {};  // sdim[0] = d+d_a+H, ..., sdim[n_lin] = 1
+    int sdim[kMaxScorerLinears + 1] = {};  // sdim[0] = d+phi_dim+H, ..., sdim[n_lin] = 1
     float ln_eps = 1e-5f;
+    int phi_kind = 0;                    // WM_PHI_*
+    int phi_dim = 0;                     // d_a (mean embedding) or n_types + 1 + 3P (structured), <= d_a
 
     // fp32 CUDA-core path: matrices stored TRANSPOSED ([in][out]) so that consecutive threads (one output unit
     // each) read consecutive addresses; vectors as in the file.

@@ -81,10 +81,11 @@ struct Params {
 };
 
 struct SmemLayout {
-    uint32_t a1, hwk, ring, e_tab, lp, ids, lens, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
+    uint32_t a1, hwk, ring, e_tab, lp, mx, ids, lens, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
 };
 
-__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps) {
+// phi_struct: the structured action features (WM_PHI_STRUCT) also keep a per-row, per-slot running maximum
+__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps, int phi_struct) {
     SmemLayout L;
     uint32_t o = 0;
     L.a1 = o; o += A1_KB * TILE_BYTES;
@@ -92,6 +93,7 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
     L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
     L.e_tab = o; o += (uint32_t)n_types * DA * 2;
     L.lp = o; o += TM * MAX_P * 4;
+    L.mx = o; o += phi_struct ? TM * MAX_P * 4 : 0;
     L.ids = o; o += TM * 4;
     L.lens = o; o += TM * 4;
     L.cnt = o; o += TM * (uint32_t)n_types;           // u8 counts, row-major [128][n_types]
@@ -130,9 +132,12 @@ using namespace ptx;
 
 namespace tc {
 
+// PHI = WM_PHI_MEAN: phi = mean action embedding; WM_PHI_STRUCT: the paper's structured statistics (S25),
+// which only changes what the action warps write into the phi K-blocks at the end of a tile.
+template <int PHI>
 __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     extern __shared__ __align__(1024) uint8_t smem[];
-    const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps);
+    const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps, PHI);
     const uint32_t s_base = smem_u32(smem);
     const uint32_t s_a1 = s_base + L.a1, s_ring = s_base + L.ring, s_bars = s_base + L.bars;
     auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
@@ -600,7 +605,6 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
         const uint8_t* s_E = smem + L.e_tab;
         float* s_lp = reinterpret_cast<float*>(smem + L.lp);
         int* s_ids = reinterpret_cast<int*>(smem + L.ids);
-        int* s_lens = reinterpret_cast<int*>(smem + L.lens);
         uint8_t* s_cnt = smem + L.cnt;
         const int P = p.P, NT = p.n_types;
         float wp[MAX_P][4], bp4[4];
@@ -626,9 +630,12 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             int cand, len, seg;
             row_meta(p.a, (int64_t)tile * TM + row, cand, len, seg, false);
             for (int c = 0; c < NT; ++c) s_cnt[row * NT + c] = 0;
-            float slp[MAX_P];
+            float slp[MAX_P];   // per parameter slot: running sum of log2 p
 #pragma unroll
             for (int j = 0; j < MAX_P; ++j) slp[j] = 0.0f;
+            // structured phi: the per-slot running maximum lives in shared memory (the registers of this role are full)
+            float4* s_mx4 = reinterpret_cast<float4*>(smem + L.mx) + row * (MAX_P / 4);
+            if (PHI == WM_PHI_STRUCT) s_mx4[0] = s_mx4[1] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
 
             for (int t = 0; t < nsteps; ++t) {
                 // phase 1 (one row per lane): read the step's action, log2 of its parameters, phi statistics
@@ -656,6 +663,12 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                         }
                     }
                     s_cnt[row * NT + id] += 1;
+                    if (PHI == WM_PHI_STRUCT) {
+                        float4 m0 = s_mx4[0], m1 = s_mx4[1];
+                        m0.x = fmaxf(m0.x, lp[0]); m0.y = fmaxf(m0.y, lp[1]); m0.z = fmaxf(m0.z, lp[2]); m0.w = fmaxf(m0.w, lp[3]);
+                        m1.x = fmaxf(m1.x, lp[4]); m1.y = fmaxf(m1.y, lp[5]); m1.z = fmaxf(m1.z, lp[6]); m1.w = fmaxf(m1.w, lp[7]);
+                        s_mx4[0] = m0; s_mx4[1] = m1;
+                    }
                 }
                 s_ids[row] = id;
                 *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
@@ -702,40 +715,43 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 if (lane == 0) mbar_arrive(bar(B_AREADY));
             }
 
-            // ---- phi = mean_t a_t = (sum_c count_c E[c] + W_p sum_t log2 p_t) / len + b_p   (0 when len = 0)
-            s_lens[row] = len;
-            *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(slp[0], slp[1], slp[2], slp[3]);
-            *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(slp[4], slp[5], slp[6], slp[7]);
-            __syncwarp();
+            // ---- the phi K-blocks of the scorer's A operand, one ROW per lane (uniform control flow; everything a lane
+            // needs is its own row's): clear the row's two K-blocks, then one 16-bit store per feature.
+            //   WM_PHI_MEAN    phi = mean_t a_t = (sum_c count_c E[c] + W_p sum_t log2 p_t) / len + b_p is LINEAR in
+            //                  psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) | 1 (len > 0)], so the host folds
+            //                  E, W_p and b_p into scorer layer 1's phi weights (tc_prepare) and the kernel only writes psi
+            //   WM_PHI_STRUCT  phi = [count_c (NT) | len | sum_j (P) | mean_j (P) | max_j (P)]   (S25)
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
-#pragma unroll 1
-            for (int rr = 0; rr < 32; ++rr) {
-                const int r = 32 * aw + rr;
-                const int lr_ = s_lens[r];
-                float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-                if (lr_ > 0) {
-#pragma unroll 4
-                    for (int c = 0; c < NT; ++c) {
-                        const float cn = (float)s_cnt[r * NT + c];
-                        const uint2 e = *reinterpret_cast<const uint2*>(s_E + ((size_t)c * DA + col4) * 2);
-                        a4[0] = fmaf(cn, __uint_as_float(e.x << 16), a4[0]);
-                        a4[1] = fmaf(cn, __uint_as_float(e.x & 0xffff0000u), a4[1]);
-                        a4[2] = fmaf(cn, __uint_as_float(e.y << 16), a4[2]);
-                        a4[3] = fmaf(cn, __uint_as_float(e.y & 0xffff0000u), a4[3]);
-                    }
-                    const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
-                    const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
-                    const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+            {
+                auto put = [&](int c, float v) {
+                    *reinterpret_cast<uint16_t*>(a1 + (4 + (c >> 6)) * TILE_BYTES + sw128_off(row, (c & 63) >> 3) +
+                                                 (c & 7) * 2) = (uint16_t)pack_f16(v, 0.0f);
+                };
+#pragma unroll
+                for (int ch = 0; ch < 16; ++ch)
+                    *reinterpret_cast<uint4*>(a1 + (4 + (ch >> 3)) * TILE_BYTES + sw128_off(row, ch & 7)) =
+                        make_uint4(0u, 0u, 0u, 0u);
+                const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
+                if (PHI == WM_PHI_STRUCT) {
+                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c]);
+                    put(NT, (float)len);
+                    const float4 m0 = s_mx4[0], m1 = s_mx4[1];
+                    const float mxr[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
 #pragma unroll
                     for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) {
+                            put(NT + 1 + j, slp[j]);
+                            put(NT + 1 + P + j, slp[j] * inv);
+                            put(NT + 1 + 2 * P + j, mxr[j]);
+                        }
+                } else {
+                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c] * inv);
 #pragma unroll
-                        for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
-                    const float inv = 1.0f / (float)lr_;
-#pragma unroll
-                    for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(a4[e2], inv, bp4[e2]);
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) put(NT + j, slp[j] * inv);
+                    put(NT + P, len > 0 ? 1.0f : 0.0f);
                 }
-                *a_dst(r) = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
             }
             // hardware features of this row -> the hw operand tile (columns >= H stay zero)
             for (int ch = 0; ch < p.H / 8; ++ch) {
@@ -813,7 +829,7 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         const int rc2 = tcg_prepare(ctx, hv, names);
         return rc2 != WM_OK || m.tc_ok ? rc2 : tct_prepare(ctx, hv, names);   // TransH models (NEXT row f1)
     }
-    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16);
+    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT);
     if ((int)L.total > ctx->smem_optin) return WM_OK;
     auto get = [&](const char* n) -> const std::vector<float>& {
         for (size_t i = 0; i < names.size(); ++i)
@@ -822,7 +838,8 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         return empty;
     };
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1"), &E = get("E");
-    const int hid = m.hidden, NC = hid / 128, K1 = tc::D + tc::DA, K0 = K1 + m.H;
+    const int hid = m.hidden, NC = hid / 128, K1 = tc::D + tc::DA;
+    const int F = m.phi_dim, K0 = tc::D + F + m.H;   // scorer input [z ; phi (F <= 128 columns) ; hw]
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
     blob.reserve((size_t)(NC * 10 + tc::SC_TILES) * tc::TILE_BYTES / 2);
@@ -846,11 +863,37 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         if (i < NC) g1(i);
         g2(i - 1);
     }
+    // phi weights of scorer layer 1 as the kernel's phi K-blocks see them, [SW][128].  WM_PHI_STRUCT: the F columns of
+    // Ws0 as they are.  WM_PHI_MEAN: the mean action embedding is linear in psi = [count_c / len | sum log2 p_j / len | 1]
+    // (see the action warps), so its weights are Ws0_phi E^T, Ws0_phi W_p and Ws0_phi b_p, summed in double here.
+    std::vector<float> Wphi((size_t)tc::SW * 128, 0.0f);
+    if (m.phi_kind == WM_PHI_STRUCT) {
+        for (int n = 0; n < tc::SW; ++n)
+            for (int c = 0; c < F; ++c) Wphi[(size_t)n * 128 + c] = Ws0[(size_t)n * K0 + tc::D + c];
+    } else {
+        const std::vector<float>&Wp = get("W_p"), &bpv = get("b_p");
+        for (int n = 0; n < tc::SW; ++n) {
+            const float* wr = &Ws0[(size_t)n * K0 + tc::D];
+            for (int c = 0; c < m.n_types; ++c) {
+                double acc = 0.0;
+                for (int k = 0; k < tc::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tc::DA + k];
+                Wphi[(size_t)n * 128 + c] = (float)acc;
+            }
+            for (int j = 0; j < m.P; ++j) {
+                double acc = 0.0;
+                for (int k = 0; k < tc::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * m.P + j];
+                Wphi[(size_t)n * 128 + m.n_types + j] = (float)acc;
+            }
+            double acc = 0.0;
+            for (int k = 0; k < tc::DA; ++k) acc += (double)wr[k] * bpv[k];
+            Wphi[(size_t)n * 128 + m.n_types + m.P] = (float)acc;
+        }
+    }
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
-        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D, 64);
-        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + 64, 64);
-        ok &= append_tile(blob, Ws0, K0, c * 128, K1, m.H);
-        ok &= append_tile(blob, Ws0, K0, c * 128, K1, 0);
+        ok &= append_tile(blob, Wphi, 128, c * 128, 0, 64);
+        ok &= append_tile(blob, Wphi, 128, c * 128, 64, 64);
+        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + F, m.H);
+        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + F, 0);
         for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
     }
     for (int c = 0; c < 4; ++c)       // scorer layer 2
@@ -871,7 +914,12 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     m.tc_blob = d_blob;
     m.tc_blob_bytes = blob.size() * 2;
     m.tc_E = d_e;
-    WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    if (m.phi_kind == WM_PHI_STRUCT)
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_STRUCT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)L.total));
+    else
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_MEAN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)L.total));
     m.tc_ok = 1;
     return WM_OK;
 }
@@ -913,9 +961,12 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
         p.prof = d_prof;
     }
 #endif
-    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
+    const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
     const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
-    tc::wm_tc_kernel<<<grid, tc::THREADS, L.total, st>>>(p);
+    if (m.phi_kind == WM_PHI_STRUCT)
+        tc::wm_tc_kernel<WM_PHI_STRUCT><<<grid, tc::THREADS, L.total, st>>>(p);
+    else
+        tc::wm_tc_kernel<WM_PHI_MEAN><<<grid, tc::THREADS, L.total, st>>>(p);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
 #ifdef WM_TC_PROFILE

@@ -837,7 +837,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 }  // namespace
 
 bool tc2_model_ok(const Model& m) {
-    return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc2::D &&
+    return m.kind == WM_KIND_MLP_LN && m.phi_kind == WM_PHI_MEAN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc2::D &&
            m.d_a == tc2::DA && m.hidden >= 512 && m.hidden <= tc2::MAX_HID && m.hidden % 256 == 0 && m.n_lin == 3 &&
            m.sdim[1] == tc2::SW && m.sdim[2] == tc2::SW && m.H >= 8 && m.H <= tc2::MAX_H && m.H % 8 == 0 &&
            m.n_types <= tc2::MAX_TYPES && m.P <= tc2::MAX_P;

@@ -734,7 +734,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 }  // namespace
 
 bool tcg_model_ok(const Model& m) {
-    return m.kind == WM_KIND_GRU && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_BUCKET && m.d == tcg::D &&
+    return m.kind == WM_KIND_GRU && m.phi_kind == WM_PHI_MEAN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_BUCKET && m.d == tcg::D &&
            m.d_a == tcg::DA && m.n_lin == 3 && m.sdim[1] == tcg::SW && m.sdim[2] == tcg::SW && m.H >= 8 &&
            m.H <= tcg::MAX_H && m.H % 8 == 0 && m.P >= 1 && m.P <= tcg::MAX_P && m.n_buckets >= 1 &&
            m.n_buckets <= tcg::MAX_BUCKETS;

@@ -842,7 +842,7 @@ struct TcState {
 }  // namespace
 
 static bool tct_model_ok(const Model& m) {
-    return m.kind == WM_KIND_TRANSH && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tct::D &&
+    return m.kind == WM_KIND_TRANSH && m.phi_kind == WM_PHI_MEAN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tct::D &&
            m.d_a == tct::DA && m.hidden >= 256 && m.hidden <= tct::MAX_HID && m.hidden % 128 == 0 && m.n_lin == 3 &&
            m.sdim[1] == tct::SW && m.sdim[2] == tct::SW && m.H >= 8 && m.H <= tct::MAX_H && m.H % 8 == 0 &&
            m.n_types <= tct::MAX_TYPES && m.P <= tct::MAX_P;

@@ -21,7 +21,9 @@ TOL = {True: 1e-4, False: 2e-2}
 SMALL = {1: dict(S=1, per_subgraph=64), 2: dict(S=3, per_subgraph=171), 3: dict(S=3, per_subgraph=139),
          4: dict(S=2, per_subgraph=320), 5: dict(S=3, per_subgraph=150),
          # NEXT row f1 (TransH transition): 6 = the fp32 parity case, 7 = cfg 2's shapes (bf16-valued weights)
-         6: dict(S=1, per_subgraph=64), 7: dict(S=3, per_subgraph=171)}
+         6: dict(S=1, per_subgraph=64), 7: dict(S=3, per_subgraph=171),
+         # NEXT row f2 (structured phi): 8 = the fp32 parity case, 9 = cfg 2's shapes
+         8: dict(S=1, per_subgraph=64), 9: dict(S=3, per_subgraph=171)}
 
 
 @pytest.fixture(scope="module")
@@ -46,7 +48,7 @@ def _paths(wm, cfg):
     return sorted({wm.PATH_FP32, auto})
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9])
 def test_config_parity_small(wm, n):
     cfg = gen.get_config(n).scaled(**SMALL[n])
     w = gen.make_weights(cfg)
@@ -82,7 +84,7 @@ def _edge_batch(cfg, lengths=None, S=None, per=None):
     return c, b
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9])
 @pytest.mark.parametrize("case", ["B1", "B127", "B129", "B257", "len0", "lenmax", "one_long", "param_ends"])
 def test_edge_cases(wm, n, case):
     base = gen.get_config(n)
@@ -108,11 +110,11 @@ def test_edge_cases(wm, n, case):
         ctx = _ctx(wm, cfg, path)
         y = gpu_scores(ctx, b)
         wm.wm_free(ctx)
-        tol = 1e-4 if n in (1, 6) else (2e-3 if path == wm.PATH_FP32 else 2e-2)
+        tol = 1e-4 if cfg.dtype == DTYPE_FP32 else (2e-3 if path == wm.PATH_FP32 else 2e-2)
         assert oracle.score_error(y, ref, b.subgraph_offsets) <= tol, (n, case, path)
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 9])
 def test_per_candidate_mode_and_segments(wm, n):
     """subgraph_offsets = NULL (per-candidate z0/hw); ragged, empty and many segments (S > #CTAs)."""
     base = gen.get_config(n)
@@ -232,7 +234,7 @@ def test_host_entry_matches_device_entry(wm, S, per):
     wm.wm_free(ctx)
 
 
-@pytest.mark.parametrize("n", [2, 3, 4, 5, 7])
+@pytest.mark.parametrize("n", [2, 3, 4, 5, 7, 9])
 def test_full_size_sampled(wm, n):
     """BASELINE.json's full size in the launch configuration bench.py times (auto path, length bucketing on, CSR
     segments): a sample of candidates is recomputed one by one by the oracle (a candidate's score does not depend on
@@ -260,7 +262,7 @@ def test_full_size_sampled(wm, n):
     np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9])
 def test_outputs_do_not_overrun(wm, n):
     """compute-sanitizer is closed on this pool: canaries instead.  The score and index buffers are sub-ranges of
     larger allocations filled with sentinels; everything outside [0, B) / [0, S*k) must come back untouched, and a
@@ -290,7 +292,7 @@ def test_outputs_do_not_overrun(wm, n):
         assert (hi[:pad] == -77).all() and (hi[pad + S * k:] == -77).all(), (n, path)
 
 
-@pytest.mark.parametrize("n", [2, 3, 5, 7])
+@pytest.mark.parametrize("n", [2, 3, 5, 7, 9])
 def test_repeatable_bitwise_with_several_tiles_per_cta(wm, n):
     """A batch large enough that every persistent CTA (or CTA pair) walks several tiles, scored three times: the
     scores must be bit-identical.  Barrier phase counters that do not survive a tile boundary, or a wait that passes
@@ -304,3 +306,32 @@ def test_repeatable_bitwise_with_several_tiles_per_cta(wm, n):
         np.testing.assert_array_equal(gpu_scores(ctx, b).view(np.uint32), y0.view(np.uint32))
     wm.wm_free(ctx)
     assert np.isfinite(y0).all()
+
+
+@pytest.mark.parametrize("n", [8, 9])
+def test_struct_phi_feature_readout(wm, n):
+    """NEXT row f2: with a first scorer layer that copies single inputs (unit-vector rows, zero bias) followed by
+    identity-like layers, the fp32 kernel's score IS one entry of [z_T ; phi ; h].  Config 8 (one linear): every
+    structured feature of every candidate against oracle.phi_struct, to fp32 rounding of log2."""
+    from dataclasses import replace
+    base = gen.get_config(n)
+    cfg = replace(base.scaled(S=2, per_subgraph=75), scorer_widths=())
+    w = gen.make_weights(cfg)
+    b = gen.make_inputs(cfg)
+    F = cfg.phi_dim
+    want = np.stack([oracle.phi_struct(b.action_ids[i, :b.lengths[i]], b.action_params[i, :b.lengths[i]], cfg.n_types)
+                     for i in range(b.B)])
+    for col in list(range(F)) + [F]:      # F = first hardware feature: hw sits right after phi
+        w1 = dict(w)
+        w1["Ws0"] = np.zeros_like(w["Ws0"]); w1["Ws0"][0, cfg.d + col] = 1.0
+        w1["bs0"] = np.zeros_like(w["bs0"])
+        ctx = wm.wm_load_weights(weight_file(cfg, w1))
+        wm.wm_set_option(ctx, wm.WM_OPT_PATH, wm.PATH_FP32)
+        assert wm.wm_get_info(ctx).phi_kind == 1
+        y = gpu_scores(ctx, b)
+        wm.wm_free(ctx)
+        if col < F:
+            np.testing.assert_allclose(y, want[:, col], rtol=2e-6, atol=1e-6, err_msg=f"feature {col}")
+        else:
+            seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+            np.testing.assert_array_equal(y, b.hw_feats[seg, 0])

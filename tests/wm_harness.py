@@ -12,6 +12,7 @@ import numpy as np
 import gen
 
 _TMP = None
+_SEQ = 0
 
 
 def weight_file(cfg, weights=None) -> str:
@@ -19,9 +20,15 @@ def weight_file(cfg, weights=None) -> str:
     global _TMP
     if _TMP is None:
         _TMP = tempfile.mkdtemp(prefix="wmw_")
-    path = os.path.join(_TMP, f"{cfg.name}_{cfg.d}_{cfg.d_a}_{cfg.hidden}_{id(weights) if weights is not None else 0}.wmw")
+    if weights is not None:      # caller-supplied weights: always a fresh file (object ids are reused after a free)
+        global _SEQ
+        _SEQ += 1
+        path = os.path.join(_TMP, f"{cfg.name}_custom{_SEQ}.wmw")
+        gen.write_weight_file(path, cfg, weights)
+        return path
+    path = os.path.join(_TMP, f"{cfg.name}_{cfg.d}_{cfg.d_a}_{cfg.hidden}_{len(cfg.scorer_widths)}.wmw")
     if not os.path.exists(path):
-        gen.write_weight_file(path, cfg, gen.make_weights(cfg) if weights is None else weights)
+        gen.write_weight_file(path, cfg, gen.make_weights(cfg))
     return path
 
 
