@@ -631,7 +631,6 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint8_t* a1 = smem + L.a1;
         float* s_lp = reinterpret_cast<float*>(smem + L.lp);
         int* s_ids = reinterpret_cast<int*>(smem + L.ids);
-        int* s_lens = reinterpret_cast<int*>(smem + L.lens);
         uint8_t* s_cnt = smem + L.cnt;
         const uint32_t r_aready = mapa(bar(B_AREADY), 0);
         const int P = p.P, NT = p.n_types;
@@ -731,44 +730,31 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 if (lane == 0) mbar_arrive_cluster(r_aready);
             }
 
-            // ---- phi = mean_t a_t = (sum_c count_c E[c] + W_p sum_t log2 p_t) / len + b_p   (0 when len = 0)
-            if (row_lane) {
-                s_lens[row] = len;
-                *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(slp[0], slp[1], slp[2], slp[3]);
-                *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(slp[4], slp[5], slp[6], slp[7]);
-            }
-            __syncwarp();
+            // ---- the phi K-blocks (8-11) of the scorer's A operand.  phi = mean_t a_t = (sum_c count_c E[c] +
+            // W_p sum_t log2 p_t) / len + b_p is LINEAR in psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) |
+            // 1 (len > 0)]: the host folds E, W_p and b_p into scorer layer 1's phi weights (tc2_prepare) and the kernel
+            // only writes psi, one row per lane: lanes l and l + 16 clear the row's four K-blocks (two each), then the row's
+            // lane stores one 16-bit value per feature (n_types + P + 1 <= 128: all in the K-blocks it cleared itself).
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
-#pragma unroll 1
-            for (int rr = 0; rr < 16; ++rr) {
-                const int r = 16 * aw + rr;
-                const int lr_ = s_lens[r];
-                float a8[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
-                if (lr_ > 0) {
-#pragma unroll 2
-                    for (int c = 0; c < NT; ++c) {
-                        const int cn_i = s_cnt[r * NT + c];
-                        if (cn_i == 0) continue;
-                        const float cn = (float)cn_i;
-                        float ev[8];
-                        e_row(c, ev);
+            {
+                const int hk = 8 + 2 * (lane >> 4);
 #pragma unroll
-                        for (int k = 0; k < 8; ++k) a8[k] = fmaf(cn, ev[k], a8[k]);
-                    }
-                    const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
-                    const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
-                    const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+                for (int ch = 0; ch < 16; ++ch)
+                    *reinterpret_cast<uint4*>(a1 + (hk + (ch >> 3)) * KB_BYTES + sw128_off(row, ch & 7)) =
+                        make_uint4(0u, 0u, 0u, 0u);
+                if (row_lane) {
+                    auto put = [&](int c, float v) {
+                        *reinterpret_cast<uint16_t*>(a1 + (8 + (c >> 6)) * KB_BYTES + sw128_off(row, (c & 63) >> 3) +
+                                                     (c & 7) * 2) = (uint16_t)pack_f16(v, 0.0f);
+                    };
+                    const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
+                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c] * inv);
 #pragma unroll
                     for (int j = 0; j < MAX_P; ++j)
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) a8[k] = fmaf(wp[j][k], lr[j], a8[k]);
-                    const float inv = 1.0f / (float)lr_;
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) a8[k] = fmaf(a8[k], inv, bp8[k]);
+                        if (j < P) put(NT + j, slp[j] * inv);
+                    put(NT + P, len > 0 ? 1.0f : 0.0f);
                 }
-                *a_dst(r) = make_uint4(pack_f16(a8[0], a8[1]), pack_f16(a8[2], a8[3]), pack_f16(a8[4], a8[5]),
-                                       pack_f16(a8[6], a8[7]));
             }
             // hardware features of this row -> the hw operand tile (columns >= H stay zero)
             if (row_lane) {
@@ -875,8 +861,30 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         if (i < NC) { g1_part(i, 8, 12); g1_part(i, 0, 8); }
         g2(i - 1);
     }
+    // phi weights of scorer layer 1 folded onto psi = [count_c / len | sum log2 p_j / len | 1] (see the action warps):
+    // Ws0_phi E^T, Ws0_phi W_p, Ws0_phi b_p, summed in double; [SW][256], columns past n_types + P + 1 zero
+    std::vector<float> Wphi((size_t)tc2::SW * 256, 0.0f);
+    {
+        const std::vector<float>&Wp = get("W_p"), &bpv = get("b_p");
+        for (int n = 0; n < tc2::SW; ++n) {
+            const float* wr = &Ws0[(size_t)n * K0 + tc2::D];
+            for (int c = 0; c < m.n_types; ++c) {
+                double acc = 0.0;
+                for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tc2::DA + k];
+                Wphi[(size_t)n * 256 + c] = (float)acc;
+            }
+            for (int j = 0; j < m.P; ++j) {
+                double acc = 0.0;
+                for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * m.P + j];
+                Wphi[(size_t)n * 256 + m.n_types + j] = (float)acc;
+            }
+            double acc = 0.0;
+            for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * bpv[k];
+            Wphi[(size_t)n * 256 + m.n_types + m.P] = (float)acc;
+        }
+    }
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (4), hw (1, zero-padded to 64 columns), z (8)
-        for (int k = 8; k < 12; ++k) ok &= append_pair_tile(blob, Ws0, K0, c * 256, k * 64, 64);
+        for (int k = 0; k < 4; ++k) ok &= append_pair_tile(blob, Wphi, 256, c * 256, k * 64, 64);
         ok &= append_pair_tile(blob, Ws0, K0, c * 256, K1, m.H);
         for (int k = 0; k < 8; ++k) ok &= append_pair_tile(blob, Ws0, K0, c * 256, k * 64, 64);
     }

@@ -644,7 +644,6 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
         const uint8_t* s_E = smem + L.e_tab;
         float* s_lp = reinterpret_cast<float*>(smem + L.lp);
         int* s_ids = reinterpret_cast<int*>(smem + L.ids);
-        int* s_lens = reinterpret_cast<int*>(smem + L.lens);
         uint8_t* s_cnt = smem + L.cnt;
         const int P = p.P, NT = p.n_types;
         float wp[MAX_P][4], bp4[4];
@@ -746,40 +745,27 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                 if (lane == 0) mbar_arrive(bar(B_AREADY));
             }
 
-            // ---- phi = mean_t a_t = (sum_c count_c E[c] + W_p sum_t log2 p_t) / len + b_p   (0 when len = 0)
-            s_lens[row] = len;
-            *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(slp[0], slp[1], slp[2], slp[3]);
-            *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(slp[4], slp[5], slp[6], slp[7]);
-            __syncwarp();
+            // ---- the phi K-blocks of the scorer's A operand, one ROW per lane.  phi = mean_t a_t = (sum_c count_c E[c] +
+            // W_p sum_t log2 p_t) / len + b_p is LINEAR in psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) |
+            // 1 (len > 0)]: the host folds E, W_p and b_p into scorer layer 1's phi weights (tct_prepare) and the kernel
+            // only writes psi (clear the row's two K-blocks, then one 16-bit store per feature).
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
-#pragma unroll 1
-            for (int rr = 0; rr < 32; ++rr) {
-                const int r = 32 * aw + rr;
-                const int lr_ = s_lens[r];
-                float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-                if (lr_ > 0) {
-#pragma unroll 4
-                    for (int c = 0; c < NT; ++c) {
-                        const float cn = (float)s_cnt[r * NT + c];
-                        const uint2 e = *reinterpret_cast<const uint2*>(s_E + ((size_t)c * DA + col4) * 2);
-                        a4[0] = fmaf(cn, __uint_as_float(e.x << 16), a4[0]);
-                        a4[1] = fmaf(cn, __uint_as_float(e.x & 0xffff0000u), a4[1]);
-                        a4[2] = fmaf(cn, __uint_as_float(e.y << 16), a4[2]);
-                        a4[3] = fmaf(cn, __uint_as_float(e.y & 0xffff0000u), a4[3]);
-                    }
-                    const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
-                    const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
-                    const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+            {
+                auto put = [&](int c, float v) {
+                    *reinterpret_cast<uint16_t*>(a1 + (4 + (c >> 6)) * TILE_BYTES + sw128_off(row, (c & 63) >> 3) +
+                                                 (c & 7) * 2) = (uint16_t)pack_f16(v, 0.0f);
+                };
 #pragma unroll
-                    for (int j = 0; j < MAX_P; ++j)
+                for (int ch = 0; ch < 16; ++ch)
+                    *reinterpret_cast<uint4*>(a1 + (4 + (ch >> 3)) * TILE_BYTES + sw128_off(row, ch & 7)) =
+                        make_uint4(0u, 0u, 0u, 0u);
+                const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
+                for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c] * inv);
 #pragma unroll
-                        for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
-                    const float inv = 1.0f / (float)lr_;
-#pragma unroll
-                    for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(a4[e2], inv, bp4[e2]);
-                }
-                *a_dst(r) = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+                for (int j = 0; j < MAX_P; ++j)
+                    if (j < P) put(NT + j, slp[j] * inv);
+                put(NT + P, len > 0 ? 1.0f : 0.0f);
             }
             // hardware features of this row -> the hw operand tile (columns >= H stay zero)
             for (int ch = 0; ch < p.H / 8; ++ch) {
@@ -894,9 +880,31 @@ int tct_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         if (i >= 1) g2(i - 1);
     }
     a_gemm(Ww);
+    // phi weights of scorer layer 1 folded onto psi = [count_c / len | sum log2 p_j / len | 1] (see the action warps):
+    // Ws0_phi E^T, Ws0_phi W_p, Ws0_phi b_p, summed in double
+    std::vector<float> Wphi((size_t)tct::SW * 128, 0.0f);
+    {
+        const std::vector<float>&Wp = get("W_p"), &bpv = get("b_p");
+        for (int n = 0; n < tct::SW; ++n) {
+            const float* wr = &Ws0[(size_t)n * K0 + tct::D];
+            for (int c = 0; c < m.n_types; ++c) {
+                double acc = 0.0;
+                for (int k = 0; k < tct::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tct::DA + k];
+                Wphi[(size_t)n * 128 + c] = (float)acc;
+            }
+            for (int j = 0; j < m.P; ++j) {
+                double acc = 0.0;
+                for (int k = 0; k < tct::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * m.P + j];
+                Wphi[(size_t)n * 128 + m.n_types + j] = (float)acc;
+            }
+            double acc = 0.0;
+            for (int k = 0; k < tct::DA; ++k) acc += (double)wr[k] * bpv[k];
+            Wphi[(size_t)n * 128 + m.n_types + m.P] = (float)acc;
+        }
+    }
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
-        ok &= append_tile(blob, Ws0, K0, c * 128, tct::D, 64);
-        ok &= append_tile(blob, Ws0, K0, c * 128, tct::D + 64, 64);
+        ok &= append_tile(blob, Wphi, 128, c * 128, 0, 64);
+        ok &= append_tile(blob, Wphi, 128, c * 128, 64, 64);
         ok &= append_tile(blob, Ws0, K0, c * 128, K1, m.H);
         ok &= append_tile(blob, Ws0, K0, c * 128, K1, 0);
         for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
