@@ -86,6 +86,28 @@ def test_load_weights_io_and_format_errors(tmp_path):
     with pytest.raises(wm.WmError) as e:
         wm.wm_load_weights(str(tmp_path / "d0.wmw"))
     assert e.value.code == wm.WM_ERR_FORMAT
+    # version 2 (structured phi, NEXT row f2): unknown phi_kind, and more features than d_a has room for
+    cfg8 = gen.get_config(8)
+    v2 = tmp_path / "v2.wmw"
+    gen.write_weight_file(str(v2), cfg8, gen.make_weights(cfg8))
+    raw2 = bytearray(v2.read_bytes())
+    assert struct.unpack_from("<I", raw2, 4)[0] == 2 and struct.unpack_from("<I", raw2, 80)[0] == 1
+    struct.pack_into("<I", raw2, 80, 7)
+    (tmp_path / "phi7.wmw").write_bytes(bytes(raw2))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "phi7.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT and "phi_kind" in str(e.value)
+    from dataclasses import replace
+    wide = replace(cfg8, n_types=40)            # 40 + 1 + 12 = 53 features > d_a = 32
+    gen.write_weight_file(str(tmp_path / "wide.wmw"), wide, gen.make_weights(wide))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "wide.wmw"))
+    assert e.value.code == wm.WM_ERR_UNSUPPORTED and "d_a" in str(e.value)
+    struct.pack_into("<I", raw2, 4, 3)          # version 3 does not exist
+    (tmp_path / "v3.wmw").write_bytes(bytes(raw2))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "v3.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT
 
 
 def test_no_product_import_of_oracle():
