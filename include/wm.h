@@ -141,6 +141,35 @@ int wm_rollout_score(wm_ctx* ctx,
                      const int32_t* lengths, const float* hw_feats, float* scores_out,
                      const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream);
 
+/* Prefix-latent reuse (SURVEY.md §8(b) extension and NEXT row f3; the online loop of PAPER.md:215 scores, round after
+ * round, candidates that share long action prefixes with survivors of earlier rounds).  Two calls:
+ *
+ * wm_rollout_latents rolls every candidate like wm_rollout_score but stores the latent after every step instead of
+ * ranking:  latents_out[b][t][:] = z_{t+1} of candidate b for 0 <= t < lengths[b]  ([B, T_max, d] fp32, device; entries
+ * with t >= lengths[b] are not written).  init_states / subgraph_offsets as in wm_rollout_score.
+ *
+ * wm_rollout_score_from scores candidates whose first start[b] steps were rolled before:
+ *   bank              [n_bank, d] fp32: latents (rows of a latents_out array, or any other store)
+ *   bank_index        [B] int32: the row of `bank` that holds candidate b's latent after its first start[b] steps
+ *                     (the task's initial latent when start[b] = 0); 0 <= bank_index[b] < n_bank is the CALLER's
+ *                     contract (not checked on the device)
+ *   start             [B] int32, clamped to [0, lengths[b]]: steps [0, start) are not rolled, they only feed phi
+ *   action_ids, action_params, lengths, hw_feats, scores_out, subgraph_offsets (non-NULL), B, S, T_max: as in
+ *                     wm_rollout_score, the action arrays holding each candidate's WHOLE sequence
+ * The score equals wm_rollout_score's for the same candidate (to the rounding of the stored fp32 latent: the
+ * tcgen05 kernels keep the latent in fp32 between steps, so a bank written by wm_rollout_latents reproduces them).
+ * Candidates are bucketed by their remaining steps lengths[b] - start[b].
+ * Errors: as wm_rollout_score; WM_ERR_ARG also for a null bank / bank_index / start / latents_out or n_bank < 1. */
+int wm_rollout_latents(wm_ctx* ctx,
+                       const float* init_states, const int32_t* action_ids, const int32_t* action_params,
+                       const int32_t* lengths, const int32_t* subgraph_offsets, float* latents_out,
+                       int64_t B, int32_t S, int32_t T_max, void* cuda_stream);
+int wm_rollout_score_from(wm_ctx* ctx,
+                          const float* bank, const int32_t* bank_index, const int32_t* start,
+                          const int32_t* action_ids, const int32_t* action_params, const int32_t* lengths,
+                          const float* hw_feats, float* scores_out, const int32_t* subgraph_offsets,
+                          int64_t B, int32_t S, int32_t T_max, int64_t n_bank, void* cuda_stream);
+
 /* Per subgraph segment [offsets[s], offsets[s+1]) select the k largest scores, ordered by
  * (score descending, index ascending).  -0.0 == +0.0; NaN ranks below every number (ties by index).
  *   scores            [offsets[S]] fp32

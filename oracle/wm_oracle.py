@@ -250,6 +250,61 @@ def rollout_score_vec(w: Dict[str, np.ndarray], init_states, action_ids, action_
     return (scores, lat) if return_latent else scores
 
 
+def rollout_latents(w, init_states, action_ids, action_params, lengths, subgraph_offsets: Optional[np.ndarray],
+                    n_buckets: int = 0, ln_eps: float = 1e-5) -> np.ndarray:
+    """Latent after every step (prefix-latent reuse, NEXT row f3; Eq.1/8 applied recurrently):
+    out[b][t] = z_{t+1} of candidate b for t < len[b], NaN elsewhere.  float64 [B, T_max, d]; one candidate at a
+    time, one step at a time."""
+    ids = np.asarray(action_ids); par = np.asarray(action_params)
+    lens = np.asarray(lengths).astype(np.int64)
+    z0 = np.asarray(init_states, F64)
+    B, T = ids.shape
+    P = par.shape[2]
+    out = np.full((B, T, z0.shape[1]), np.nan, dtype=F64)
+    seg = np.arange(B)
+    if subgraph_offsets is not None:
+        off = np.asarray(subgraph_offsets).astype(np.int64)
+        seg = np.searchsorted(off, np.arange(B), side="right") - 1
+    for b in range(B):
+        z = z0[seg[b]][None, :].copy()
+        for t in range(int(lens[b])):
+            a = _embed(w, ids[b:b + 1, t], par[b:b + 1, t, :], P, n_buckets)
+            z = _step(w, z, a, ln_eps)
+            out[b, t] = z[0]
+    return out
+
+
+def rollout_score_from(w, bank, bank_index, start, action_ids, action_params, lengths, hw_feats, subgraph_offsets,
+                       n_buckets: int = 0, ln_eps: float = 1e-5, phi_kind: int = PHI_MEAN) -> np.ndarray:
+    """Scores of candidates whose first start[b] steps were rolled before: z starts at bank[bank_index[b]], steps
+    start[b] .. len[b]-1 are applied, phi is taken over the WHOLE sequence, y = G([z_T ; phi ; h_s]).  Plain
+    definition, one candidate at a time (the online loop re-scores mutated survivors)."""
+    ids = np.asarray(action_ids); par = np.asarray(action_params)
+    lens = np.asarray(lengths).astype(np.int64)
+    bank = np.asarray(bank, F64); hw = np.asarray(hw_feats, F64)
+    off = np.asarray(subgraph_offsets).astype(np.int64)
+    B = ids.shape[0]
+    P = par.shape[2]
+    nl = _n_scorer_layers(w)
+    n_types = w["E"].shape[0] if "E" in w else w["Tbl"].shape[0] // (P * n_buckets)
+    seg = np.searchsorted(off, np.arange(B), side="right") - 1
+    out = np.zeros(B, dtype=F64)
+    for b in range(B):
+        n = int(lens[b])
+        st = min(max(int(start[b]), 0), n)
+        z = bank[int(bank_index[b])][None, :].copy()
+        for t in range(st, n):
+            z = _step(w, z, _embed(w, ids[b:b + 1, t], par[b:b + 1, t, :], P, n_buckets), ln_eps)
+        if phi_kind == PHI_STRUCT:
+            phi = phi_struct(ids[b, :n], par[b, :n, :], n_types)
+        elif n > 0:
+            phi = _embed(w, ids[b, :n], par[b, :n, :], P, n_buckets).sum(axis=0) / n
+        else:
+            phi = np.zeros((w["Tbl"] if "Tbl" in w else w["E"]).shape[1], dtype=F64)
+        out[b] = scorer(np.concatenate([z[0], phi, hw[seg[b]]])[None, :], w, nl)[0]
+    return out
+
+
 def rollout_score_scalar(w, init_states, action_ids, action_params, lengths, hw_feats, subgraph_offsets,
                          n_buckets: int = 0, ln_eps: float = 1e-5, phi_kind: int = PHI_MEAN) -> np.ndarray:
     """Pure-python per-candidate loops (tiny inputs only); independent of the vector code above."""

@@ -22,6 +22,7 @@ PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 
 # every symbol include/wm.h declares
 ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
+               "wm_rollout_latents", "wm_rollout_score_from",
                "wm_check", "wm_score_topk_host", "wm_last_kernel_ms", "wm_launch_count", "wm_last_error")
 
 
@@ -63,6 +64,10 @@ def lib() -> ctypes.CDLL:
     L.wm_set_option.restype = ctypes.c_int
     L.wm_rollout_score.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, vp]
     L.wm_rollout_score.restype = ctypes.c_int
+    L.wm_rollout_latents.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, vp]
+    L.wm_rollout_score_from.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i64, vp]
+    L.wm_rollout_latents.restype = ctypes.c_int
+    L.wm_rollout_score_from.restype = ctypes.c_int
     L.wm_topk.argtypes = [vp, vp, i32, i32, vp, vp]
     L.wm_topk.restype = ctypes.c_int
     L.wm_check.argtypes = [vp, vp]
@@ -131,6 +136,28 @@ def wm_rollout_score(ctx: int, init_states, action_ids, action_params, lengths, 
     _check(lib().wm_rollout_score(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
                                   _ptr(hw_feats), _ptr(scores_out), _ptr(subgraph_offsets), B, S, T_max,
                                   _stream(stream)))
+
+
+def wm_rollout_latents(ctx: int, init_states, action_ids, action_params, lengths, latents_out,
+                       subgraph_offsets=None, stream=None) -> None:
+    """latents_out [B, T_max, d] fp32 (device): z after step t+1 at [b][t] for t < lengths[b].  include/wm.h."""
+    B = int(lengths.numel())
+    T_max = int(action_ids.shape[1]) if action_ids is not None and action_ids.dim() == 2 else 0
+    S = int(subgraph_offsets.numel()) - 1 if subgraph_offsets is not None else 0
+    _check(lib().wm_rollout_latents(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
+                                    _ptr(subgraph_offsets), _ptr(latents_out), B, S, T_max, _stream(stream)))
+
+
+def wm_rollout_score_from(ctx: int, bank, bank_index, start, action_ids, action_params, lengths, hw_feats, scores_out,
+                          subgraph_offsets, stream=None) -> None:
+    """Score candidates whose first start[b] steps were rolled before (latent in bank[bank_index[b]]).  include/wm.h."""
+    B = int(lengths.numel())
+    T_max = int(action_ids.shape[1]) if action_ids is not None and action_ids.dim() == 2 else 0
+    S = int(subgraph_offsets.numel()) - 1
+    n_bank = int(bank.numel() // bank.shape[-1])
+    _check(lib().wm_rollout_score_from(ctx, _ptr(bank), _ptr(bank_index), _ptr(start), _ptr(action_ids),
+                                       _ptr(action_params), _ptr(lengths), _ptr(hw_feats), _ptr(scores_out),
+                                       _ptr(subgraph_offsets), B, S, T_max, n_bank, _stream(stream)))
 
 
 def wm_topk(scores, subgraph_offsets, k: int, idx_out, stream=None) -> None:

@@ -345,38 +345,20 @@ int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value) {
     return WM_ERR_ARG;
 }
 
-int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* action_ids, const int32_t* action_params,
-                     const int32_t* lengths, const float* hw_feats, float* scores_out,
-                     const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream) {
-    if (!ctx) {
-        set_error("wm_rollout_score: null ctx");
-        return WM_ERR_ARG;
-    }
-    if (B < 0 || B > 0x7fffffffLL || S < 0 || T_max < 0 || T_max > WM_MAX_T) {
-        set_error("wm_rollout_score: size out of range (B=%lld S=%d T_max=%d)", (long long)B, S, T_max);
-        return WM_ERR_ARG;
-    }
-    if (B == 0) return WM_OK;
-    if (!init_states || !lengths || !scores_out || (ctx->m.H > 0 && !hw_feats) ||
-        (T_max > 0 && (!action_ids || !action_params)) || (subgraph_offsets && S < 1)) {
-        set_error("wm_rollout_score: null pointer (or S < 1 with offsets) for a non-empty batch");
-        return WM_ERR_ARG;
-    }
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+// Common tail of the three rollout entries: workspace, bucketing by rollout steps, timing events, dispatch.
+static int run_rollout(wm_ctx* ctx, CallArgs a, cudaStream_t st, const char* who) {
     WM_CUDA_TRY(cudaSetDevice(ctx->device));
     Workspace* ws = acquire_ws(ctx, st);
     if (!ws) {
-        set_error("wm_rollout_score: cannot allocate workspace");
+        set_error("%s: cannot allocate workspace", who);
         return WM_ERR_CUDA;
     }
-    CallArgs a;
-    a.init_states = init_states; a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
-    a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets; a.perm = nullptr;
-    a.B = B; a.S = S; a.T_max = T_max; a.fault = ctx->fault;
+    a.perm = nullptr;
+    a.fault = ctx->fault;
     if (ctx->opt_sort) {
-        int rc = ensure_perm(ws, B, st);
+        int rc = ensure_perm(ws, a.B, st);
         if (rc != WM_OK) return rc;
-        rc = launch_length_bucketing(ctx, ws, lengths, B, T_max, st);
+        rc = launch_length_bucketing(ctx, ws, a.lengths, a.start, a.B, a.T_max, st);
         if (rc != WM_OK) return rc;
         a.perm = ws->perm;
     }
@@ -393,6 +375,78 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
         ws->timed = true;
     }
     return rc;
+}
+
+static bool sizes_ok(const char* who, int64_t B, int32_t S, int32_t T_max) {
+    if (B < 0 || B > 0x7fffffffLL || S < 0 || T_max < 0 || T_max > WM_MAX_T) {
+        set_error("%s: size out of range (B=%lld S=%d T_max=%d)", who, (long long)B, S, T_max);
+        return false;
+    }
+    return true;
+}
+
+int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* action_ids, const int32_t* action_params,
+                     const int32_t* lengths, const float* hw_feats, float* scores_out,
+                     const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream) {
+    if (!ctx) {
+        set_error("wm_rollout_score: null ctx");
+        return WM_ERR_ARG;
+    }
+    if (!sizes_ok("wm_rollout_score", B, S, T_max)) return WM_ERR_ARG;
+    if (B == 0) return WM_OK;
+    if (!init_states || !lengths || !scores_out || (ctx->m.H > 0 && !hw_feats) ||
+        (T_max > 0 && (!action_ids || !action_params)) || (subgraph_offsets && S < 1)) {
+        set_error("wm_rollout_score: null pointer (or S < 1 with offsets) for a non-empty batch");
+        return WM_ERR_ARG;
+    }
+    CallArgs a = {};
+    a.init_states = init_states; a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
+    a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets;
+    a.B = B; a.S = S; a.T_max = T_max;
+    return run_rollout(ctx, a, static_cast<cudaStream_t>(cuda_stream), "wm_rollout_score");
+}
+
+int wm_rollout_latents(wm_ctx* ctx, const float* init_states, const int32_t* action_ids, const int32_t* action_params,
+                       const int32_t* lengths, const int32_t* subgraph_offsets, float* latents_out, int64_t B,
+                       int32_t S, int32_t T_max, void* cuda_stream) {
+    if (!ctx) {
+        set_error("wm_rollout_latents: null ctx");
+        return WM_ERR_ARG;
+    }
+    if (!sizes_ok("wm_rollout_latents", B, S, T_max)) return WM_ERR_ARG;
+    if (B == 0 || T_max == 0) return WM_OK;
+    if (!init_states || !lengths || !latents_out || !action_ids || !action_params || (subgraph_offsets && S < 1)) {
+        set_error("wm_rollout_latents: null pointer (or S < 1 with offsets) for a non-empty batch");
+        return WM_ERR_ARG;
+    }
+    CallArgs a = {};
+    a.init_states = init_states; a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
+    a.offsets = subgraph_offsets; a.latents_out = latents_out;
+    a.B = B; a.S = S; a.T_max = T_max;
+    return run_rollout(ctx, a, static_cast<cudaStream_t>(cuda_stream), "wm_rollout_latents");
+}
+
+int wm_rollout_score_from(wm_ctx* ctx, const float* bank, const int32_t* bank_index, const int32_t* start,
+                          const int32_t* action_ids, const int32_t* action_params, const int32_t* lengths,
+                          const float* hw_feats, float* scores_out, const int32_t* subgraph_offsets, int64_t B,
+                          int32_t S, int32_t T_max, int64_t n_bank, void* cuda_stream) {
+    if (!ctx) {
+        set_error("wm_rollout_score_from: null ctx");
+        return WM_ERR_ARG;
+    }
+    if (!sizes_ok("wm_rollout_score_from", B, S, T_max)) return WM_ERR_ARG;
+    if (B == 0) return WM_OK;
+    if (!bank || !bank_index || !start || n_bank < 1 || !lengths || !scores_out || (ctx->m.H > 0 && !hw_feats) ||
+        (T_max > 0 && (!action_ids || !action_params)) || !subgraph_offsets || S < 1) {
+        set_error("wm_rollout_score_from: null pointer, n_bank < 1 or S < 1 for a non-empty batch");
+        return WM_ERR_ARG;
+    }
+    CallArgs a = {};
+    a.init_states = bank; a.init_index = bank_index; a.start = start;
+    a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
+    a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets;
+    a.B = B; a.S = S; a.T_max = T_max;
+    return run_rollout(ctx, a, static_cast<cudaStream_t>(cuda_stream), "wm_rollout_score_from");
 }
 
 int wm_last_kernel_ms(wm_ctx* ctx, void* cuda_stream, float* ms_out) {

@@ -16,8 +16,15 @@ constexpr int kBucketThreads = 512;
 constexpr int kBucketItems = 8;   // candidates per thread
 
 __device__ __forceinline__ int clamp_len(int len, int T_max) { return len < 0 ? 0 : (len > T_max ? T_max : len); }
+// sort key: the number of rollout steps, i.e. the clamped length minus the clamped start (prefix-latent reuse)
+__device__ __forceinline__ int steps_of(const int32_t* __restrict__ lengths, const int32_t* __restrict__ start, int64_t i,
+                                        int T_max) {
+    const int len = clamp_len(__ldg(lengths + i), T_max);
+    return start ? len - clamp_start(__ldg(start + i), len) : len;
+}
 
-__global__ void __launch_bounds__(kBucketThreads) wm_len_hist_kernel(const int32_t* __restrict__ lengths, int64_t B,
+__global__ void __launch_bounds__(kBucketThreads) wm_len_hist_kernel(const int32_t* __restrict__ lengths,
+                                                                     const int32_t* __restrict__ start, int64_t B,
                                                                      int T_max, int32_t* __restrict__ hist) {
     __shared__ int sh[WM_MAX_T + 1];
     for (int i = threadIdx.x; i <= T_max; i += blockDim.x) sh[i] = 0;
@@ -26,7 +33,7 @@ __global__ void __launch_bounds__(kBucketThreads) wm_len_hist_kernel(const int32
 #pragma unroll
     for (int it = 0; it < kBucketItems; ++it) {
         const int64_t i = base + (int64_t)it * kBucketThreads + threadIdx.x;
-        if (i < B) atomicAdd(&sh[clamp_len(__ldg(lengths + i), T_max)], 1);
+        if (i < B) atomicAdd(&sh[steps_of(lengths, start, i, T_max)], 1);
     }
     __syncthreads();
     for (int i = threadIdx.x; i <= T_max; i += blockDim.x)
@@ -34,6 +41,7 @@ __global__ void __launch_bounds__(kBucketThreads) wm_len_hist_kernel(const int32
 }
 
 __global__ void __launch_bounds__(kBucketThreads) wm_len_scatter_kernel(const int32_t* __restrict__ lengths,
+                                                                        const int32_t* __restrict__ start,
                                                                         int64_t B, int T_max,
                                                                         const int32_t* __restrict__ hist,
                                                                         int32_t* __restrict__ cursor,
@@ -49,7 +57,7 @@ __global__ void __launch_bounds__(kBucketThreads) wm_len_scatter_kernel(const in
         const int64_t i = base + (int64_t)it * kBucketThreads + threadIdx.x;
         my_len[it] = -1;
         if (i < B) {
-            my_len[it] = clamp_len(__ldg(lengths + i), T_max);
+            my_len[it] = steps_of(lengths, start, i, T_max);
             atomicAdd(&s_cnt[my_len[it]], 1);
         }
     }
@@ -96,15 +104,15 @@ __global__ void __launch_bounds__(kBucketThreads) wm_len_scatter_kernel(const in
     }
 }
 
-int launch_length_bucketing(wm_ctx* ctx, Workspace* ws, const int32_t* lengths, int64_t B, int T_max,
-                            cudaStream_t st) {
+int launch_length_bucketing(wm_ctx* ctx, Workspace* ws, const int32_t* lengths, const int32_t* start, int64_t B,
+                            int T_max, cudaStream_t st) {
     if (B <= 0) return WM_OK;
     WM_CUDA_TRY(cudaMemsetAsync(ws->counters, 0, sizeof(int32_t) * kCounterInts, st));
     const int64_t per_cta = (int64_t)kBucketThreads * kBucketItems;
     const int grid = (int)((B + per_cta - 1) / per_cta);
-    wm_len_hist_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, B, T_max, ws->counters + kHistOff);
+    wm_len_hist_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, start, B, T_max, ws->counters + kHistOff);
     WM_CUDA_TRY(cudaGetLastError());
-    wm_len_scatter_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, B, T_max, ws->counters + kHistOff,
+    wm_len_scatter_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, start, B, T_max, ws->counters + kHistOff,
                                                            ws->counters + kCursorOff, ws->perm);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(2);

@@ -124,12 +124,14 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
     float* Y = AS + (size_t)da * R;                    // [(d+da)][R], GRU and TransH only
     float* LP = ALT + (size_t)p.alt_rows * R;          // [R][P] log2(param) or bucket index (as int bits)
     float* RED = LP + (size_t)R * P;                   // [G][R] reduction scratch, G = threads / R
-    int* meta = reinterpret_cast<int*>(RED + kGenericThreads);   // cand[R], len[R], seg[R], id[R], tile_len
+    int* meta = reinterpret_cast<int*>(RED + kGenericThreads);   // cand[R], len[R], seg[R], id[R], start[R], tile_len, tile_pre
     int* m_cand = meta;
     int* m_len = meta + R;
     int* m_seg = meta + 2 * R;
     int* m_id = meta + 3 * R;
-    int* m_tile_len = meta + 4 * R;
+    int* m_start = meta + 4 * R;       // prefix-latent reuse: steps [0, start) only feed phi
+    int* m_tile_len = meta + 5 * R;    // rollout steps of the tile = max (len - start)
+    int* m_tile_pre = meta + 5 * R + 1;   // max start of the tile
 
     const int tid = threadIdx.x;
     const int r_of = tid % R;
@@ -139,11 +141,11 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
 
     for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
         __syncthreads();
-        if (tid == 0) *m_tile_len = 0;
+        if (tid == 0) *m_tile_len = *m_tile_pre = 0;
         __syncthreads();
         if (tid < R) {
             const int64_t i = (int64_t)tile * R + tid;
-            int cand = -1, len = 0, seg = 0;
+            int cand = -1, len = 0, seg = 0, st = 0;
             if (i < a.B) {
                 cand = a.perm ? __ldg(a.perm + i) : (int)i;
                 len = __ldg(a.lengths + cand);
@@ -152,41 +154,57 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     len = len < 0 ? 0 : a.T_max;
                 }
                 seg = a.offsets ? find_segment(a.offsets, a.S, cand) : cand;
+                if (a.start) st = clamp_start(__ldg(a.start + cand), len);
             }
             m_cand[tid] = cand;
             m_len[tid] = len;
             m_seg[tid] = seg;
-            atomicMax(m_tile_len, len);
+            m_start[tid] = st;
+            atomicMax(m_tile_len, len - st);
+            atomicMax(m_tile_pre, st);
         }
         __syncthreads();
-        const int tile_len = *m_tile_len;
-        // z_0 and the running action sum
+        const int tile_len = *m_tile_len, tile_pre = *m_tile_pre;
+        // z_0 (the subgraph's, the candidate's, or the row init_index names) and the running action sum
         for (int e = tid; e < d * R; e += kGenericThreads) {
             const int r = e % R, j = e / R;   // lanes over rows: conflict-free store; global read strided but tiny
-            X[(size_t)j * R + r] = m_cand[r] >= 0 ? __ldg(a.init_states + (size_t)m_seg[r] * d + j) : 0.0f;
+            float v = 0.0f;
+            if (m_cand[r] >= 0) {
+                const size_t zrow = a.init_index ? (size_t)__ldg(a.init_index + m_cand[r]) : (size_t)m_seg[r];
+                v = __ldg(a.init_states + zrow * d + j);
+            }
+            X[(size_t)j * R + r] = v;
         }
         for (int e = tid; e < da * R; e += kGenericThreads) AS[e] = 0.0f;
         __syncthreads();
 
-        for (int t = 0; t < tile_len; ++t) {
-            // ---- a1: action embedding of step t (rows with t >= len get a = 0 and touch no input)
+        // Iterations tq < 0 walk the prefix positions [0, start) of every row: embedding and phi statistics only, no
+        // transition (prefix-latent reuse: the latent at `start` was supplied).  Iterations tq >= 0 are rollout steps:
+        // row r is at position start[r] + tq.
+        for (int tq = -tile_pre; tq < tile_len; ++tq) {
+            const bool prefix = tq < 0;
+            const int t = tq;   // (name kept for the masks below: live rows have pos < len)
+            auto pos_of = [&](int r) { return prefix ? tq + tile_pre : m_start[r] + tq; };
+            auto live_of = [&](int r) { return prefix ? tq + tile_pre < m_start[r] : m_start[r] + tq < m_len[r]; };
+            (void)t;
+            // ---- a1: action embedding at this position (rows that are not live get a = 0 and touch no input)
             if (tid < R) {
                 int id = 0;
-                if (t < m_len[tid]) {
-                    id = __ldg(a.action_ids + (size_t)m_cand[tid] * a.T_max + t);
+                if (live_of(tid)) {
+                    id = __ldg(a.action_ids + (size_t)m_cand[tid] * a.T_max + pos_of(tid));
                     if (id < 0 || id >= p.n_types) {
                         atomicOr(a.fault, WM_FAULT_TYPE);
                         id = id < 0 ? 0 : p.n_types - 1;
                     }
                 }
                 m_id[tid] = id;
-                if (p.phi_kind == WM_PHI_STRUCT && t < m_len[tid]) AS[(size_t)id * R + tid] += 1.0f;
+                if (p.phi_kind == WM_PHI_STRUCT && live_of(tid)) AS[(size_t)id * R + tid] += 1.0f;
             }
             for (int e = tid; e < R * P; e += kGenericThreads) {
                 const int r = e / P, j = e % P;
                 float v = 0.0f;
-                if (t < m_len[r]) {
-                    int prm = __ldg(a.action_params + ((size_t)m_cand[r] * a.T_max + t) * P + j);
+                if (live_of(r)) {
+                    int prm = __ldg(a.action_params + ((size_t)m_cand[r] * a.T_max + pos_of(r)) * P + j);
                     if (prm < 1) {
                         atomicOr(a.fault, WM_FAULT_PARAM);
                         prm = 1;
@@ -215,7 +233,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
             for (int e = tid; e < da * R; e += kGenericThreads) {
                 const int r = e % R, j = e / R;
                 float v = 0.0f;
-                if (t < m_len[r]) {
+                if (live_of(r)) {
                     const int id = m_id[r];
                     if (p.embed == WM_EMBED_LINEAR) {
                         v = __ldg(p.E + (size_t)id * da + j) + __ldg(p.bp + j);
@@ -231,8 +249,10 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                 X[(size_t)(d + j) * R + r] = v;
             }
             __syncthreads();
+            if (prefix) continue;
+            const bool live_row = live_of(r_of);
 
-            // ---- a2/a3: one transition step, rows with t >= len frozen
+            // ---- a2/a3: one transition step, rows that are not live frozen
             if (p.kind == WM_KIND_TRANSH) {
                 // PAPER.md:164 (S24): u = W_w a, w = u / sqrt(|u|^2 + eps); x = z - (w.z) w + W_d a;
                 // v = x + W2 gelu(W1 [x;a] + b1) + b2; z' = v / sqrt(|v|^2 + eps).  (w.z) w = (u.z) u / (|u|^2 + eps).
@@ -280,7 +300,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                 float n2 = 0.0f;
                 for (int g = 0; g < G; ++g) n2 += RED[g * R + r_of];
                 const float rn = 1.0f / sqrtf(n2 + kEps);
-                if (t < m_len[r_of]) {
+                if (live_row) {
                     for (int j = g_of; j < d; j += G) X[(size_t)j * R + r_of] = V[(size_t)j * R + r_of] * rn;
                 }
             } else if (p.kind != WM_KIND_GRU) {
@@ -313,14 +333,14 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     for (int g = 0; g < G; ++g) var += RED[g * R + r_of];
                     var /= (float)d;
                     const float rstd = 1.0f / sqrtf(var + p.ln_eps);
-                    if (t < m_len[r_of]) {
+                    if (live_row) {
                         for (int j = g_of; j < d; j += G) {
                             const float c = (V[(size_t)j * R + r_of] - mean) * rstd;
                             X[(size_t)j * R + r_of] = fmaf(__ldg(p.gamma + j), c, __ldg(p.beta + j));
                         }
                     }
                 } else {
-                    if (t < m_len[r_of]) {
+                    if (live_row) {
                         for (int j = g_of; j < d; j += G) X[(size_t)j * R + r_of] += V[(size_t)j * R + r_of];
                     }
                 }
@@ -333,7 +353,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                 __syncthreads();
                 linear_T<R, ACT_TANH>(p.Wht, nullptr, Y, K1, d, V);       // candidate h
                 __syncthreads();
-                if (t < m_len[r_of]) {
+                if (live_row) {
                     for (int j = g_of; j < d; j += G) {
                         const size_t o = (size_t)j * R + r_of;
                         const float g = Hb[o];
@@ -342,7 +362,15 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                 }
             }
             __syncthreads();
+            if (a.latents_out) {   // z after this step, rows that took it: latents_out[cand][pos][:]
+                for (int e = tid; e < d * R; e += kGenericThreads) {
+                    const int r = e / d, j = e % d;    // lanes over features: coalesced global store
+                    if (live_of(r))
+                        a.latents_out[((size_t)m_cand[r] * a.T_max + pos_of(r)) * d + j] = X[(size_t)j * R + r];
+                }
+            }
         }
+        if (!a.scores_out) continue;   // wm_rollout_latents: no ranking
 
         // ---- a4/a5: x = [z_T ; phi ; hw], scorer MLP
         const int F = p.phi_dim, NT = p.n_types;
@@ -396,7 +424,7 @@ static size_t generic_smem_bytes(const Model& m, int R, int* maxw_out, int* alt_
     *alt_rows_out = alt;
     size_t floats = (size_t)(m.d + m.d_a + m.H) * R + (size_t)maxw * R + (size_t)alt * R + (size_t)R * m.P +
                     kGenericThreads;
-    return floats * 4 + (4 * R + 4) * sizeof(int);
+    return floats * 4 + (5 * R + 4) * sizeof(int);
 }
 
 template <int R>

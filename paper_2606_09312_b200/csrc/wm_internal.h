@@ -123,11 +123,18 @@ struct CallArgs {
     int64_t B;
     int S, T_max;
     uint32_t* fault;
+    // prefix-latent reuse (NEXT row f3; wm_rollout_latents / wm_rollout_score_from), all null for wm_rollout_score:
+    const int32_t* start;       // [B] steps [0, start) only feed phi, the rollout runs over [start, len)
+    const int32_t* init_index;  // [B] row of init_states that holds candidate b's initial latent
+    float* latents_out;         // [B, T_max, d] z after step t+1 at [b][t] for start <= t < len; scores_out may be null
 };
 
+// rollout steps of a candidate: its clamped length minus its clamped start (the single place that defines it)
+__host__ __device__ inline int clamp_start(int start, int len) { return start < 0 ? 0 : (start > len ? len : start); }
+
 // K1 (wm_bucket.cu): perm = candidates sorted by clamped length, descending.  2 launches + 1 memset.
-int launch_length_bucketing(wm_ctx* ctx, Workspace* ws, const int32_t* lengths, int64_t B, int T_max,
-                            cudaStream_t st);
+int launch_length_bucketing(wm_ctx* ctx, Workspace* ws, const int32_t* lengths, const int32_t* start, int64_t B,
+                            int T_max, cudaStream_t st);
 
 // K2-fp32 (wm_generic.cu): every model kind, fp32 CUDA cores.
 int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st);

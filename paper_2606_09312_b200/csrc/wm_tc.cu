@@ -930,9 +930,11 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const Model& m = ctx->m;
     // per-call conditions the kernel relies on; otherwise the fp32 kernel takes the call
     const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0);
-    if (!m.tc_ok || a.T_max > 255 || !aligned) {
+    const bool prefix_call = a.start || a.init_index || a.latents_out;   // wm_rollout_latents / wm_rollout_score_from
+    if (prefix_call && ctx->opt_path != 2) return launch_generic(ctx, a, st);
+    if (!m.tc_ok || a.T_max > 255 || !aligned || prefix_call) {
         if (ctx->opt_path == 2) {
-            set_error("tcgen05 path: needs T_max <= 255 and 16-byte aligned init_states / hw_feats");
+            set_error("tcgen05 path: needs T_max <= 255, 16-byte aligned init_states / hw_feats, and wm_rollout_score");
             return WM_ERR_UNSUPPORTED;
         }
         return launch_generic(ctx, a, st);

@@ -11,7 +11,7 @@ import pytest
 import gen
 import oracle
 from gen.configs import DTYPE_FP32
-from wm_harness import weight_file, gpu_scores, gpu_topk, oracle_scores
+from wm_harness import weight_file, gpu_scores, gpu_topk, oracle_scores, to_device
 
 pytestmark = pytest.mark.gpu
 
@@ -335,3 +335,88 @@ def test_struct_phi_feature_readout(wm, n):
         else:
             seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
             np.testing.assert_array_equal(y, b.hw_feats[seg, 0])
+
+
+PREFIX_TC_VARIANTS = ()      # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
+
+
+def _prefix_case(n, S, per):
+    cfg = gen.get_config(n).scaled(S=S, per_subgraph=per)
+    return cfg, gen.make_weights(cfg), gen.make_inputs(cfg)
+
+
+def _prefix_unsupported(wm, ctx, path, call):
+    """True (after checking the error code) when `path` is a forced tcgen05 kernel without prefix-reuse support."""
+    if path != wm.PATH_TCGEN05 or wm.wm_get_info(ctx).tc_variant in PREFIX_TC_VARIANTS:
+        return False
+    with pytest.raises(wm.WmError) as e:
+        call()
+    assert e.value.code == wm.WM_ERR_UNSUPPORTED
+    wm.wm_free(ctx)
+    return True
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 9])
+def test_rollout_latents_match_oracle(wm, n):
+    """NEXT row f3: wm_rollout_latents against oracle.rollout_latents, every stored latent; entries past a candidate's
+    length keep the caller's bytes."""
+    import torch
+    cfg, w, b = _prefix_case(n, 2, 90 if n not in (1, 6) else 40)
+    ref = oracle.rollout_latents(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.subgraph_offsets,
+                                 n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps)
+    valid = np.arange(cfg.T_max)[None, :] < b.lengths[:, None]
+    dv = to_device(b)
+    for path in _paths(wm, cfg):
+        ctx = _ctx(wm, cfg, path)
+        out = torch.full((b.B, cfg.T_max, cfg.d), -777.0, dtype=torch.float32, device="cuda:0")
+        call = lambda: wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"],
+                                             dv["lengths"], out, dv["subgraph_offsets"])
+        if _prefix_unsupported(wm, ctx, path, call):
+            continue
+        call()
+        assert wm.wm_check(ctx) == 0
+        wm.wm_free(ctx)
+        lat = out.cpu().numpy()
+        assert (lat[~valid] == -777.0).all()
+        scale = np.sqrt(np.mean(ref[valid] ** 2))
+        err = np.abs(lat[valid] - ref[valid]).max() / scale
+        tol = 1e-4 if cfg.dtype == DTYPE_FP32 else (2e-3 if path == wm.PATH_FP32 else 2e-2)
+        assert err <= tol, (n, path, err)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 9])
+def test_score_from_bank_matches_literal(wm, n):
+    """NEXT row f3: candidates scored from latents banked by wm_rollout_latents at random cuts (0 and len included) get
+    the literal call's scores: against the oracle within the config's tolerance, and against the same path's own
+    literal scores to fp32 rounding (the bank holds the fp32 latent the literal rollout carries)."""
+    import torch
+    cfg, w, b = _prefix_case(n, 3, {1: 40, 6: 40, 4: 192}.get(n, 150))
+    ref = oracle_scores(cfg, w, b)
+    rng = np.random.default_rng(300 + n)
+    start = rng.integers(-1, cfg.T_max + 2, b.B).astype(np.int32)
+    start[:4] = [0, 0, cfg.T_max, cfg.T_max]
+    st = np.clip(start, 0, b.lengths)
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    index = np.where(st == 0, seg, cfg.S + np.arange(b.B) * cfg.T_max + st - 1).astype(np.int32)
+    dv = to_device(b)
+    d_start = torch.from_numpy(start).cuda(); d_index = torch.from_numpy(index).cuda()
+    for path in _paths(wm, cfg):
+        ctx = _ctx(wm, cfg, path)
+        lit = gpu_scores(ctx, b)
+        bank = torch.zeros((cfg.S + b.B * cfg.T_max, cfg.d), dtype=torch.float32, device="cuda:0")
+        bank[:cfg.S] = dv["init_states"]
+        call = lambda: wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"],
+                                             dv["lengths"], bank[cfg.S:].view(b.B, cfg.T_max, cfg.d),
+                                             dv["subgraph_offsets"])
+        if _prefix_unsupported(wm, ctx, path, call):
+            continue
+        call()
+        out = torch.full((b.B,), float("nan"), dtype=torch.float32, device="cuda:0")
+        wm.wm_rollout_score_from(ctx, bank, d_index, d_start, dv["action_ids"], dv["action_params"], dv["lengths"],
+                                 dv["hw_feats"], out, dv["subgraph_offsets"])
+        assert wm.wm_check(ctx) == 0
+        wm.wm_free(ctx)
+        y = out.cpu().numpy()
+        tol = 1e-4 if cfg.dtype == DTYPE_FP32 else (2e-3 if path == wm.PATH_FP32 else 2e-2)
+        assert oracle.score_error(y, ref, b.subgraph_offsets) <= tol, (n, path)
+        assert oracle.score_error(y, lit, b.subgraph_offsets) <= 2e-5, (n, path)

@@ -424,6 +424,65 @@ def test_p12_prefix_reuse_equals_scratch():
     assert np.isfinite(y).all()
 
 
+@pytest.mark.parametrize("kind,embed,phi", [(KIND_MLP_LN, EMBED_LINEAR, PHI_MEAN), (KIND_GRU, EMBED_BUCKET, PHI_MEAN),
+                                            (KIND_TRANSH, EMBED_LINEAR, PHI_MEAN), (KIND_MLP, EMBED_LINEAR, PHI_STRUCT)])
+def test_p18_latents_and_score_from(kind, embed, phi):
+    """NEXT row f3 (prefix-latent reuse).  rollout_latents / rollout_score_from are pinned to the already pinned literal
+    path: (a) the latent after step t+1 is the terminal latent of the sequence cut to t+1 steps; (b) scoring from a
+    banked latent at ANY cut (0 and len included) equals scoring from scratch; (c) start = len is the closed form
+    G([bank row ; phi ; h]); (d) phi covers the whole sequence, not the suffix."""
+    cfg = tiny_cfg(kind, embed, phi_kind=phi)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    kw = dict(n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps)
+    lat = oracle.rollout_latents(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.subgraph_offsets, **kw)
+    assert lat.shape == (b.B, cfg.T_max, cfg.d)
+    valid = np.arange(cfg.T_max)[None, :] < b.lengths[:, None]
+    assert np.isnan(lat[~valid]).all() and np.isfinite(lat[valid]).all()
+    for t in range(cfg.T_max):                     # (a)
+        cut = np.minimum(b.lengths, t + 1)
+        _, zt = oracle.rollout_score_vec(w, b.init_states, b.action_ids, b.action_params, cut, b.hw_feats,
+                                         b.subgraph_offsets, return_latent=True, phi_kind=phi, **kw)
+        rows = b.lengths > t
+        np.testing.assert_allclose(lat[rows, t], zt[rows], rtol=0, atol=1e-12)
+    y = run_vec(cfg, w, b)
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    # bank = [z_0 of every subgraph ; every stored latent], bank_index by (candidate, cut)
+    bank = np.concatenate([b.init_states.astype(np.float64), np.nan_to_num(lat).reshape(-1, cfg.d)])
+    rng = np.random.default_rng(18)
+    for starts in (np.zeros(b.B, dtype=np.int64), b.lengths.astype(np.int64),
+                   rng.integers(0, cfg.T_max + 1, b.B), np.full(b.B, 99), np.full(b.B, -3)):
+        st = np.clip(starts, 0, b.lengths)
+        index = np.where(st == 0, seg, cfg.S + np.arange(b.B) * cfg.T_max + st - 1)
+        yf = oracle.rollout_score_from(w, bank, index, starts, b.action_ids, b.action_params, b.lengths, b.hw_feats,
+                                       b.subgraph_offsets, phi_kind=phi, **kw)
+        np.testing.assert_allclose(yf, y, rtol=0, atol=1e-11)          # (b)
+    # (c) nothing left to roll: the score is the ranker on the banked latent
+    rb = rng.standard_normal((b.B, cfg.d))
+    yc = oracle.rollout_score_from(w, rb, np.arange(b.B), b.lengths, b.action_ids, b.action_params, b.lengths,
+                                   b.hw_feats, b.subgraph_offsets, phi_kind=phi, **kw)
+    nl = len(cfg.scorer_widths) + 1
+    if phi == PHI_STRUCT:
+        ph = np.stack([oracle.phi_struct(b.action_ids[i, :b.lengths[i]], b.action_params[i, :b.lengths[i]], cfg.n_types)
+                       for i in range(b.B)])
+    else:
+        ph = np.zeros((b.B, cfg.d_a))               # mean action embedding, from the (pinned) embedding functions
+        for i in range(b.B):
+            n = int(b.lengths[i])
+            if n:
+                emb = (oracle.embed_bucket(b.action_ids[i, :n], b.action_params[i, :n], w["Tbl"], cfg.P, cfg.n_buckets)
+                       if embed == EMBED_BUCKET else
+                       oracle.embed_linear(b.action_ids[i, :n], b.action_params[i, :n], w["E"], w["W_p"], w["b_p"]))
+                ph[i] = emb.mean(axis=0)
+    np.testing.assert_allclose(yc, oracle.scorer(np.concatenate([rb, ph, b.hw_feats[seg]], axis=1), w, nl),
+                               rtol=0, atol=1e-12)
+    # (d) scoring the suffix alone (phi over the suffix only) is a different number for cut > 0
+    i = int(np.argmax(b.lengths))
+    c = int(b.lengths[i]) // 2
+    sub = oracle.rollout_score_vec(w, lat[i:i + 1, c - 1], b.action_ids[i:i + 1, c:], b.action_params[i:i + 1, c:],
+                                   b.lengths[i:i + 1] - c, b.hw_feats[seg[i]][None], None, phi_kind=phi, **kw)
+    assert abs(sub[0] - y[i]) > 1e-6
+
+
 # ---- generator / file format ----------------------------------------------------------------------------------
 
 def test_weight_file_roundtrip(tmp_path):
