@@ -290,6 +290,54 @@ def run_ours(args, cfg):
                  "peak_source": pk["source"] + " (burst: kernel timed alone)",
                  "algorithmic_flops_per_launch": flops, "share_of_step": k_ms / float(np.mean(ms))})
 
+    # ---- prefix-latent reuse leg (NEXT row f3; configs with a shared-prefix structure, i.e. cfg 4): the representative of
+    # every family (the child with the longest copied prefix) is rolled once over that prefix with the latent stored
+    # after every step, then every child is scored from its cut.  Same scores, a third of the rollout steps.
+    prefix = None
+    if batch.cut is not None and args.prefix_reuse:
+        C = cfg.prefix_children
+        cut = batch.cut.reshape(-1, C)
+        rep = (np.arange(cut.shape[0]) * C + cut.argmax(axis=1)).astype(np.int64)       # one representative per family
+        rep_len = torch.from_numpy(cut.max(axis=1).astype(np.int32)).to(dev)
+        rep_ids = dv["action_ids"][torch.from_numpy(rep).to(dev)].contiguous()
+        rep_par = dv["action_params"][torch.from_numpy(rep).to(dev)].contiguous()
+        fam_off = torch.from_numpy((np.asarray(batch.subgraph_offsets, dtype=np.int64) // C).astype(np.int32)).to(dev)
+        T = batch.T_max
+        bank = torch.empty((rep.size, T, cfg.d), dtype=torch.float32, device=dev)
+        start = torch.from_numpy(batch.cut.astype(np.int32)).to(dev)
+        index = torch.from_numpy(((np.arange(B) // C) * T + batch.cut - 1).astype(np.int32)).to(dev)
+        scores2 = torch.empty_like(scores)
+        idx2 = torch.empty_like(idx)
+
+        def prefix_step():
+            wm.wm_rollout_latents(ctx, dv["init_states"], rep_ids, rep_par, rep_len, bank, fam_off)
+            wm.wm_rollout_score_from(ctx, bank.view(-1, cfg.d), index, start, dv["action_ids"], dv["action_params"],
+                                     dv["lengths"], dv["hw_feats"], scores2, dv["subgraph_offsets"])
+            wm.wm_topk(scores2, dv["subgraph_offsets"], k, idx2)
+
+        for _ in range(3):
+            flush.zero_()
+            prefix_step()
+        assert wm.wm_check(ctx) == 0
+        pms = []
+        for _ in range(args.steps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            prefix_step()
+            e1.record()
+            torch.cuda.synchronize()
+            pms.append(e0.elapsed_time(e1))
+        p_ms = float(np.mean(pms))
+        executed = int(cut.max(axis=1).sum() + (batch.lengths - batch.cut).sum())
+        prefix = {"value": B / (p_ms * 1e-3), "unit": UNIT, "ms_per_step": p_ms,
+                  "executed_rollout_steps": executed, "literal_rollout_steps": int(batch.lengths.sum()),
+                  "bank_bytes": int(bank.numel() * 4),
+                  "max_abs_score_diff_vs_literal": float((scores2 - scores).abs().max().item()),
+                  "topk_identical_to_literal": bool(torch.equal(idx2, idx)),
+                  "calls": "wm_rollout_latents (family representatives) + wm_rollout_score_from (children) + wm_topk"}
+        del bank
+
     # ---- e2e leg: host (pinned) buffers through wm_score_topk_host
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
     hb = dict(z0=pin(batch.init_states), ids=pin(batch.action_ids), par=pin(batch.action_params),
@@ -331,6 +379,8 @@ def run_ours(args, cfg):
            "e2e": {"value": cands_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "ms_per_step": e2e_s * 1e3},
            "roofline": roof}
+    if prefix is not None:
+        out["prefix_reuse"] = prefix
     if world == 1:
         out["cpu_baseline"] = cpu_baseline(cfg, 4 if cfg.number != 1 else cfg.S)
     print(json.dumps(out))
@@ -343,6 +393,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--prefix-reuse", action="store_true",
+                    help="config 4: also time the prefix-latent-reuse calls (extra 'prefix_reuse' object in the JSON line)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]; 6, 7 = NEXT row f1 (TransH transition); 8, 9 = NEXT row f2 (structured phi)")
     args = ap.parse_args()

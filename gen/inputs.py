@@ -27,6 +27,9 @@ class Batch:
     lengths: np.ndarray            # [B] int32
     subgraph_offsets: np.ndarray   # [S+1] int32
     T_max: int
+    # shared-prefix structure (cfg 4 only, else None): candidate b copies positions [0, cut[b]) from parent parent_of[b]
+    parent_of: np.ndarray = None   # [B] int64
+    cut: np.ndarray = None         # [B] int64
 
     @property
     def B(self) -> int:
@@ -62,6 +65,7 @@ def make_inputs(cfg: WMConfig, sentinel_padding: bool = True) -> Batch:
     z0 = rng.standard_normal((S, cfg.d)).astype(np.float32)
     hw = rng.standard_normal((S, cfg.H)).astype(np.float32)
     lengths = _draw_lengths(rng, cfg, B)
+    parent_of = cut = None
     if cfg.prefix_children == 0:
         ids = rng.integers(0, cfg.n_types, size=(B, T)).astype(np.int32)
         params = _draw_params(rng, cfg, (B, T, P))
@@ -85,4 +89,4 @@ def make_inputs(cfg: WMConfig, sentinel_padding: bool = True) -> Batch:
         params = np.where(pad[:, :, None], sent[None, :, None], params)
     offsets = (np.arange(S + 1, dtype=np.int64) * n).astype(np.int32)
     return Batch(z0, hw, np.ascontiguousarray(ids, dtype=np.int32),
-                 np.ascontiguousarray(params, dtype=np.int32), lengths, offsets, T)
+                 np.ascontiguousarray(params, dtype=np.int32), lengths, offsets, T, parent_of, cut)

@@ -270,6 +270,11 @@ __device__ __forceinline__ void row_meta(const CallArgs& a, int64_t i, int& cand
     }
 }
 
+// Prefix-latent reuse (wm_rollout_score_from): first position the rollout applies for this candidate; 0 otherwise.
+__device__ __forceinline__ int row_start(const CallArgs& a, int cand, int len) {
+    return (a.start && cand >= 0) ? clamp_start(__ldg(a.start + cand), len) : 0;
+}
+
 // byte offset of the 16-byte chunk `chunk` (8 bf16 columns) of row `row` inside a SW128 K-major K-block tile
 __device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
     return (uint32_t)row * 128u + (uint32_t)((chunk ^ (row & 7)) << 4);

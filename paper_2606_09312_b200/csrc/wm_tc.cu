@@ -134,7 +134,9 @@ namespace tc {
 
 // PHI = WM_PHI_MEAN: phi = mean action embedding; WM_PHI_STRUCT: the paper's structured statistics (S25),
 // which only changes what the action warps write into the phi K-blocks at the end of a tile.
-template <int PHI>
+// EXT = true: the prefix-latent-reuse calls (wm_rollout_latents / wm_rollout_score_from: per-candidate start position and
+// initial-latent row, latent stored after every step); false compiles all of that out of the literal path.
+template <int PHI, bool EXT>
 __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps, PHI);
@@ -203,7 +205,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 for (int r = lane; r < TM; r += 32) {
                     int cand, len, seg;
                     row_meta(p.a, (int64_t)tile * TM + r, cand, len, seg, true);
-                    nsteps = max(nsteps, len);
+                    nsteps = max(nsteps, EXT ? len - row_start(p.a, cand, len) : len);
                 }
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) nsteps = max(nsteps, __shfl_xor_sync(0xffffffffu, nsteps, o));
@@ -481,14 +483,17 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             if (tile < 0) break;
             int cand, len, seg;
             row_meta(p.a, (int64_t)tile * TM + row, cand, len, seg, false);
+            // prefix-latent reuse: the rollout covers positions [st, len) and starts from the row init_index names
+            const int st = EXT ? row_start(p.a, cand, len) : 0, rem = len - st;
+            const size_t zrow = (EXT && p.a.init_index && cand >= 0) ? (size_t)__ldg(p.a.init_index + cand) : (size_t)seg;
 
-            // ---- z_0 (the task's initial latent)
+            // ---- z_0 (the task's initial latent; or the banked latent after the first st steps)
 #pragma unroll 1
             for (int p4 = 0; p4 < 4; ++p4) {
                 const int col0 = 128 * hh + 32 * p4;
                 uint32_t v[32];
                 if (cand >= 0) {
-                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + col0);
+                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + zrow * D + col0);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const float4 f = __ldg(src + i);
@@ -537,7 +542,10 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 const float mean = (s1 + other.x) * inv_d;
                 const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
                 const float rstd = rsqrtf(var + p.ln_eps);
-                const bool live = t < len;     // masked steps leave the state unchanged
+                const bool live = t < rem;     // masked steps leave the state unchanged
+                float4* lat = (EXT && p.a.latents_out && live)     // wm_rollout_latents: z after this step, this row's half
+                                  ? reinterpret_cast<float4*>(p.a.latents_out + ((size_t)cand * p.a.T_max + st + t) * D)
+                                  : nullptr;
 #pragma unroll 1
                 for (int p4 = 0; p4 < 4; ++p4) {
                     const int col0 = 128 * hh + 32 * p4;
@@ -563,6 +571,12 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
                     // fp32 master is never read again
                     put_z(col0, v, live);
+                    if (lat) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+                            lat[(col0 >> 2) + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                                                               __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+                    }
                 }
                 publish(B_ZREADY, true);
             }
@@ -593,7 +607,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             }
             s_red[hh * TM + row] = make_float2(part, 0.0f);
             named_bar_sync(1 + q, 64);
-            if (hh == 0 && cand >= 0) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
+            if (hh == 0 && cand >= 0 && (!EXT || p.a.scores_out)) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
             named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
         }
     } else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
@@ -636,6 +650,47 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             // structured phi: the per-slot running maximum lives in shared memory (the registers of this role are full)
             float4* s_mx4 = reinterpret_cast<float4*>(smem + L.mx) + row * (MAX_P / 4);
             if (PHI == WM_PHI_STRUCT) s_mx4[0] = s_mx4[1] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            // the action at position `pos` of this row: type id (clamped), log2 of its parameters, phi statistics
+            auto take = [&](int pos, float (&lp)[MAX_P]) -> int {
+                int id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos);
+                if (id < 0 || id >= NT) {
+                    atomicOr(p.a.fault, WM_FAULT_TYPE);
+                    id = id < 0 ? 0 : NT - 1;
+                }
+                const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P;
+#pragma unroll
+                for (int j = 0; j < MAX_P; ++j) {
+                    if (j < P) {
+                        int prm = __ldg(pp + j);
+                        if (prm < 1) {
+                            atomicOr(p.a.fault, WM_FAULT_PARAM);
+                            prm = 1;
+                        }
+                        lp[j] = log2f((float)prm);
+                        slp[j] += lp[j];
+                    }
+                }
+                s_cnt[row * NT + id] += 1;
+                if (PHI == WM_PHI_STRUCT) {
+                    float4 m0 = s_mx4[0], m1 = s_mx4[1];
+                    m0.x = fmaxf(m0.x, lp[0]); m0.y = fmaxf(m0.y, lp[1]); m0.z = fmaxf(m0.z, lp[2]); m0.w = fmaxf(m0.w, lp[3]);
+                    m1.x = fmaxf(m1.x, lp[4]); m1.y = fmaxf(m1.y, lp[5]); m1.z = fmaxf(m1.z, lp[6]); m1.w = fmaxf(m1.w, lp[7]);
+                    s_mx4[0] = m0; s_mx4[1] = m1;
+                }
+                return id;
+            };
+            // prefix-latent reuse: positions [0, st) were rolled before (their latent is z_0 of this call); they only
+            // feed phi
+            const int st = EXT ? row_start(p.a, cand, len) : 0;
+            if (EXT && p.a.start) {
+#pragma unroll 2
+                for (int pos = 0; pos < st; ++pos) {
+                    float lp[MAX_P];
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                    take(pos, lp);
+                }
+            }
 
             for (int t = 0; t < nsteps; ++t) {
                 // phase 1 (one row per lane): read the step's action, log2 of its parameters, phi statistics
@@ -643,33 +698,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 float lp[MAX_P];
 #pragma unroll
                 for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
-                if (t < len) {
-                    id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
-                    if (id < 0 || id >= NT) {
-                        atomicOr(p.a.fault, WM_FAULT_TYPE);
-                        id = id < 0 ? 0 : NT - 1;
-                    }
-                    const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
-#pragma unroll
-                    for (int j = 0; j < MAX_P; ++j) {
-                        if (j < P) {
-                            int prm = __ldg(pp + j);
-                            if (prm < 1) {
-                                atomicOr(p.a.fault, WM_FAULT_PARAM);
-                                prm = 1;
-                            }
-                            lp[j] = log2f((float)prm);
-                            slp[j] += lp[j];
-                        }
-                    }
-                    s_cnt[row * NT + id] += 1;
-                    if (PHI == WM_PHI_STRUCT) {
-                        float4 m0 = s_mx4[0], m1 = s_mx4[1];
-                        m0.x = fmaxf(m0.x, lp[0]); m0.y = fmaxf(m0.y, lp[1]); m0.z = fmaxf(m0.z, lp[2]); m0.w = fmaxf(m0.w, lp[3]);
-                        m1.x = fmaxf(m1.x, lp[4]); m1.y = fmaxf(m1.y, lp[5]); m1.z = fmaxf(m1.z, lp[6]); m1.w = fmaxf(m1.w, lp[7]);
-                        s_mx4[0] = m0; s_mx4[1] = m1;
-                    }
-                }
+                if (st + t < len) id = take(st + t, lp);
                 s_ids[row] = id;
                 *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
                 *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
@@ -756,7 +785,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             // hardware features of this row -> the hw operand tile (columns >= H stay zero)
             for (int ch = 0; ch < p.H / 8; ++ch) {
                 uint4 o = make_uint4(0u, 0u, 0u, 0u);
-                if (cand >= 0) {
+                if (cand >= 0 && (!EXT || p.a.hw_feats)) {   // (wm_rollout_latents passes no hardware features: nothing is ranked)
                     const float4* src = reinterpret_cast<const float4*>(p.a.hw_feats + (size_t)seg * p.H + 8 * ch);
                     const float4 f0 = __ldg(src), f1 = __ldg(src + 1);
                     o.x = pack_f16(f0.x, f0.y); o.y = pack_f16(f0.z, f0.w);
@@ -914,12 +943,17 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     m.tc_blob = d_blob;
     m.tc_blob_bytes = blob.size() * 2;
     m.tc_E = d_e;
-    if (m.phi_kind == WM_PHI_STRUCT)
-        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_STRUCT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)L.total));
-    else
-        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_MEAN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)L.total));
+    if (m.phi_kind == WM_PHI_STRUCT) {
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_STRUCT, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_STRUCT, true>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    } else {
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_MEAN, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc::wm_tc_kernel<WM_PHI_MEAN, true>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    }
     m.tc_ok = 1;
     return WM_OK;
 }
@@ -931,10 +965,12 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     // per-call conditions the kernel relies on; otherwise the fp32 kernel takes the call
     const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0);
     const bool prefix_call = a.start || a.init_index || a.latents_out;   // wm_rollout_latents / wm_rollout_score_from
-    if (prefix_call && ctx->opt_path != 2) return launch_generic(ctx, a, st);
-    if (!m.tc_ok || a.T_max > 255 || !aligned || prefix_call) {
+    // the prefix-reuse calls are built into wm_tc_kernel only; the other models take the fp32 kernel for them
+    if (prefix_call && m.tc_ok != 1 && ctx->opt_path != 2) return launch_generic(ctx, a, st);
+    if (!m.tc_ok || a.T_max > 255 || !aligned || (prefix_call && m.tc_ok != 1)) {
         if (ctx->opt_path == 2) {
-            set_error("tcgen05 path: needs T_max <= 255, 16-byte aligned init_states / hw_feats, and wm_rollout_score");
+            set_error("tcgen05 path: needs T_max <= 255, 16-byte aligned init_states / hw_feats (and, for "
+                      "wm_rollout_latents / wm_rollout_score_from, a d = 256 MLP+LayerNorm model)");
             return WM_ERR_UNSUPPORTED;
         }
         return launch_generic(ctx, a, st);
@@ -965,10 +1001,13 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
 #endif
     const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
     const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
-    if (m.phi_kind == WM_PHI_STRUCT)
-        tc::wm_tc_kernel<WM_PHI_STRUCT><<<grid, tc::THREADS, L.total, st>>>(p);
-    else
-        tc::wm_tc_kernel<WM_PHI_MEAN><<<grid, tc::THREADS, L.total, st>>>(p);
+    if (m.phi_kind == WM_PHI_STRUCT) {
+        if (prefix_call) tc::wm_tc_kernel<WM_PHI_STRUCT, true><<<grid, tc::THREADS, L.total, st>>>(p);
+        else tc::wm_tc_kernel<WM_PHI_STRUCT, false><<<grid, tc::THREADS, L.total, st>>>(p);
+    } else {
+        if (prefix_call) tc::wm_tc_kernel<WM_PHI_MEAN, true><<<grid, tc::THREADS, L.total, st>>>(p);
+        else tc::wm_tc_kernel<WM_PHI_MEAN, false><<<grid, tc::THREADS, L.total, st>>>(p);
+    }
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
 #ifdef WM_TC_PROFILE

@@ -337,7 +337,7 @@ def test_struct_phi_feature_readout(wm, n):
             np.testing.assert_array_equal(y, b.hw_feats[seg, 0])
 
 
-PREFIX_TC_VARIANTS = ()      # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
+PREFIX_TC_VARIANTS = (1,)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
 
 
 def _prefix_case(n, S, per):
@@ -420,3 +420,37 @@ def test_score_from_bank_matches_literal(wm, n):
         tol = 1e-4 if cfg.dtype == DTYPE_FP32 else (2e-3 if path == wm.PATH_FP32 else 2e-2)
         assert oracle.score_error(y, ref, b.subgraph_offsets) <= tol, (n, path)
         assert oracle.score_error(y, lit, b.subgraph_offsets) <= 2e-5, (n, path)
+
+
+def test_cfg4_prefix_reuse_full_family_structure(wm):
+    """cfg 4's shared-prefix structure used the way a search loop would (bench.py --prefix-reuse): one representative per
+    family rolled over the copied prefix with every latent banked, every child scored from its cut.  Scores must equal the
+    literal call's (fp32 rounding of nothing: the bank holds the very latent the literal rollout carries) and the top-k
+    must be identical."""
+    import torch
+    cfg = gen.get_config(4).scaled(S=3, per_subgraph=1024)
+    b = gen.make_inputs(cfg)
+    C, T = cfg.prefix_children, cfg.T_max
+    ctx = _ctx(wm, cfg)
+    assert wm.wm_get_info(ctx).tc_variant == 1
+    lit = gpu_scores(ctx, b)
+    dv = to_device(b)
+    cut = b.cut.reshape(-1, C)
+    rep = torch.from_numpy(np.arange(cut.shape[0]) * C + cut.argmax(axis=1)).cuda()
+    rep_len = torch.from_numpy(cut.max(axis=1).astype(np.int32)).cuda()
+    fam_off = torch.from_numpy((b.subgraph_offsets.astype(np.int64) // C).astype(np.int32)).cuda()
+    bank = torch.full((cut.shape[0], T, cfg.d), float("nan"), dtype=torch.float32, device="cuda:0")
+    wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"][rep].contiguous(),
+                          dv["action_params"][rep].contiguous(), rep_len, bank, fam_off)
+    start = torch.from_numpy(b.cut.astype(np.int32)).cuda()
+    index = torch.from_numpy(((np.arange(b.B) // C) * T + b.cut - 1).astype(np.int32)).cuda()
+    out = torch.full((b.B,), float("nan"), dtype=torch.float32, device="cuda:0")
+    wm.wm_rollout_score_from(ctx, bank.view(-1, cfg.d), index, start, dv["action_ids"], dv["action_params"],
+                             dv["lengths"], dv["hw_feats"], out, dv["subgraph_offsets"])
+    assert wm.wm_check(ctx) == 0
+    wm.wm_free(ctx)
+    y = out.cpu().numpy()
+    np.testing.assert_array_equal(y.view(np.uint32), lit.view(np.uint32))
+    ref = oracle_scores(cfg, gen.make_weights(cfg), b)
+    assert oracle.score_error(y, ref, b.subgraph_offsets) <= TOL[False]
+    np.testing.assert_array_equal(gpu_topk(y, b.subgraph_offsets, cfg.k), gpu_topk(lit, b.subgraph_offsets, cfg.k))
