@@ -650,18 +650,16 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             // structured phi: the per-slot running maximum lives in shared memory (the registers of this role are full)
             float4* s_mx4 = reinterpret_cast<float4*>(smem + L.mx) + row * (MAX_P / 4);
             if (PHI == WM_PHI_STRUCT) s_mx4[0] = s_mx4[1] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-            // the action at position `pos` of this row: type id (clamped), log2 of its parameters, phi statistics
-            auto take = [&](int pos, float (&lp)[MAX_P]) -> int {
-                int id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos);
+            // one action of this row: type id (clamped), log2 of its parameters, phi statistics
+            auto account = [&](int id, const int (&raw)[MAX_P], float (&lp)[MAX_P]) -> int {
                 if (id < 0 || id >= NT) {
                     atomicOr(p.a.fault, WM_FAULT_TYPE);
                     id = id < 0 ? 0 : NT - 1;
                 }
-                const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P;
 #pragma unroll
                 for (int j = 0; j < MAX_P; ++j) {
                     if (j < P) {
-                        int prm = __ldg(pp + j);
+                        int prm = raw[j];
                         if (prm < 1) {
                             atomicOr(p.a.fault, WM_FAULT_PARAM);
                             prm = 1;
@@ -679,18 +677,43 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 }
                 return id;
             };
-            // prefix-latent reuse: positions [0, st) were rolled before (their latent is z_0 of this call); they only
-            // feed phi
-            const int st = EXT ? row_start(p.a, cand, len) : 0;
-            if (EXT && p.a.start) {
-#pragma unroll 2
-                for (int pos = 0; pos < st; ++pos) {
-                    float lp[MAX_P];
+            auto take = [&](int pos, float (&lp)[MAX_P]) -> int {   // the action at position `pos`
+                const int id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos);
+                const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P;
+                int raw[MAX_P];
 #pragma unroll
-                    for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
-                    take(pos, lp);
+                for (int j = 0; j < MAX_P; ++j) raw[j] = j < P ? __ldg(pp + j) : 1;
+                return account(id, raw, lp);
+            };
+            // prefix-latent reuse: positions [0, st) were rolled before (their latent is z_0 of this call); they only
+            // feed phi.  They are scanned four at a time (all loads issued before the first is used) BEFORE the first rollout
+            // step, in position order, so the running sums see the positions in the literal call's order and the scores
+            // of the two calls are bit-identical (interleaving the scan with the steps was no faster and was not).
+            const int st = EXT ? row_start(p.a, cand, len) : 0;
+            int scanned = 0;
+            auto scan4 = [&]() {
+                int rid[4], raw[4][MAX_P];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int pos = scanned + u < st ? scanned + u : 0;      // (in-bounds dummy for finished lanes)
+                    rid[u] = cand >= 0 ? __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos) : 0;
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+                        raw[u][j] = (cand >= 0 && j < P)
+                                        ? __ldg(p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P + j) : 1;
                 }
-            }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (scanned + u < st) {
+                        float lp[MAX_P];
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                        account(rid[u], raw[u], lp);
+                    }
+                scanned += 4;
+            };
+            if (EXT && p.a.start)
+                while (__any_sync(0xffffffffu, scanned < st)) scan4();
 
             for (int t = 0; t < nsteps; ++t) {
                 // phase 1 (one row per lane): read the step's action, log2 of its parameters, phi statistics
