@@ -47,6 +47,10 @@ def test_topk_argument_errors(L):
 
 def test_null_ctx_errors(L):
     assert L.wm_rollout_score(None, None, None, None, None, None, None, None, 1, 1, 1, None) == wm.WM_ERR_ARG
+    assert L.wm_rollout_latents(None, None, None, None, None, None, None, 1, 1, 1, None) == wm.WM_ERR_ARG
+    assert "null ctx" in wm.wm_last_error()
+    assert L.wm_rollout_score_from(None, None, None, None, None, None, None, None, None, None, 1, 1, 1, 1,
+                                   None) == wm.WM_ERR_ARG
     assert L.wm_check(None, None) == wm.WM_ERR_ARG
     assert L.wm_set_option(None, 1, 0) == wm.WM_ERR_ARG
     L.wm_free(None)

@@ -454,3 +454,68 @@ def test_cfg4_prefix_reuse_full_family_structure(wm):
     ref = oracle_scores(cfg, gen.make_weights(cfg), b)
     assert oracle.score_error(y, ref, b.subgraph_offsets) <= TOL[False]
     np.testing.assert_array_equal(gpu_topk(y, b.subgraph_offsets, cfg.k), gpu_topk(lit, b.subgraph_offsets, cfg.k))
+
+
+@pytest.mark.parametrize("n", [1, 2])
+def test_prefix_calls_argument_and_edge_cases(wm, n):
+    """Null / size errors of the two prefix-reuse entries, B = 0 and T_max = 0 no-ops, per-candidate init (offsets NULL)
+    for wm_rollout_latents, a batch whose every candidate has start = len (no step is rolled), and B = 1."""
+    import torch
+    L = wm.lib()
+    cfg, w, b = _prefix_case(n, 2, 33)
+    dv = to_device(b)
+    ctx = _ctx(wm, cfg)
+    lat = torch.full((b.B, cfg.T_max, cfg.d), -5.0, dtype=torch.float32, device="cuda:0")
+    p = lambda t: t.data_ptr()
+    args = (p(dv["init_states"]), p(dv["action_ids"]), p(dv["action_params"]), p(dv["lengths"]), p(dv["subgraph_offsets"]))
+    assert L.wm_rollout_latents(ctx, *args, None, b.B, b.S, cfg.T_max, None) == wm.WM_ERR_ARG          # null output
+    assert L.wm_rollout_latents(ctx, *args, p(lat), -1, b.S, cfg.T_max, None) == wm.WM_ERR_ARG         # B < 0
+    assert L.wm_rollout_latents(ctx, *args, p(lat), b.B, b.S, wm.WM_MAX_T + 1, None) == wm.WM_ERR_ARG
+    assert L.wm_rollout_latents(ctx, *args, p(lat), 0, b.S, cfg.T_max, None) == wm.WM_OK               # B = 0
+    assert L.wm_rollout_latents(ctx, *args, p(lat), b.B, b.S, 0, None) == wm.WM_OK                     # T_max = 0
+    torch.cuda.synchronize()
+    assert (lat == -5.0).all()
+    sc = torch.zeros(b.B, dtype=torch.float32, device="cuda:0")
+    z = torch.zeros(b.B, dtype=torch.int32, device="cuda:0")
+    fa = (p(dv["action_ids"]), p(dv["action_params"]), p(dv["lengths"]), p(dv["hw_feats"]), p(sc))
+    bank = dv["init_states"]
+    assert L.wm_rollout_score_from(ctx, None, p(z), p(z), *fa, p(dv["subgraph_offsets"]), b.B, b.S, cfg.T_max, b.S,
+                                   None) == wm.WM_ERR_ARG                                               # null bank
+    assert L.wm_rollout_score_from(ctx, p(bank), p(z), p(z), *fa, None, b.B, b.S, cfg.T_max, b.S,
+                                   None) == wm.WM_ERR_ARG                                               # null offsets
+    assert L.wm_rollout_score_from(ctx, p(bank), p(z), p(z), *fa, p(dv["subgraph_offsets"]), b.B, b.S, cfg.T_max, 0,
+                                   None) == wm.WM_ERR_ARG                                               # n_bank < 1
+    # start = 0 from the subgraph rows themselves == the literal call
+    seg = torch.from_numpy(np.repeat(np.arange(cfg.S), cfg.per_subgraph).astype(np.int32)).cuda()
+    wm.wm_rollout_score_from(ctx, bank, seg, z, dv["action_ids"], dv["action_params"], dv["lengths"], dv["hw_feats"],
+                             sc, dv["subgraph_offsets"])
+    lit = gpu_scores(ctx, b)
+    np.testing.assert_array_equal(sc.cpu().numpy().view(np.uint32), lit.view(np.uint32))
+    # per-candidate initial latents for wm_rollout_latents (offsets NULL), checked on the first and last candidate
+    rng = np.random.default_rng(9)
+    z0 = rng.standard_normal((b.B, cfg.d)).astype(np.float32)
+    wm.wm_rollout_latents(ctx, torch.from_numpy(z0).cuda(), dv["action_ids"], dv["action_params"], dv["lengths"], lat, None)
+    ref = oracle.rollout_latents(w, z0, b.action_ids, b.action_params, b.lengths, None, n_buckets=cfg.n_buckets,
+                                 ln_eps=cfg.ln_eps)
+    valid = np.arange(cfg.T_max)[None, :] < b.lengths[:, None]
+    got = lat.cpu().numpy()
+    tol = 1e-4 if cfg.dtype == DTYPE_FP32 else 2e-2
+    assert np.abs(got[valid] - ref[valid]).max() / np.sqrt(np.mean(ref[valid] ** 2)) <= tol
+    # nothing left to roll: every candidate starts at its length, the score is the ranker on the banked row
+    bank2 = torch.from_numpy(rng.standard_normal((b.B, cfg.d)).astype(np.float32)).cuda()
+    own = torch.arange(b.B, dtype=torch.int32, device="cuda:0")
+    wm.wm_rollout_score_from(ctx, bank2, own, dv["lengths"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                             dv["hw_feats"], sc, dv["subgraph_offsets"])
+    want = oracle.rollout_score_from(w, bank2.cpu().numpy(), np.arange(b.B), b.lengths, b.action_ids, b.action_params,
+                                     b.lengths, b.hw_feats, b.subgraph_offsets, n_buckets=cfg.n_buckets,
+                                     ln_eps=cfg.ln_eps)
+    assert oracle.score_error(sc.cpu().numpy(), want, b.subgraph_offsets) <= tol
+    # B = 1
+    one = torch.zeros(1, dtype=torch.float32, device="cuda:0")
+    off1 = torch.tensor([0, 1], dtype=torch.int32, device="cuda:0")
+    wm.wm_rollout_score_from(ctx, bank, seg[:1].contiguous(), z[:1].contiguous(), dv["action_ids"][:1].contiguous(),
+                             dv["action_params"][:1].contiguous(), dv["lengths"][:1].contiguous(),
+                             dv["hw_feats"][:1].contiguous(), one, off1)
+    assert wm.wm_check(ctx) == 0
+    assert abs(float(one.item()) - float(lit[0])) <= 2e-5 * max(1.0, abs(float(lit[0])))
+    wm.wm_free(ctx)
