@@ -109,7 +109,8 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
  *   TRANSH:       W_w[d,d_a], W_d[d,d_a], then W1, b1, W2, b2 as for MLP
  *   G:            for each linear i: Ws_i[out_i,in_i], bs_i[out_i];  in_0 = d+dim(phi)+H, out_last = 1
  * With dtype = bf16 every stored value is already bf16-representable (BASELINE.json cfg 2-5: "bf16 weights with
- * fp32 accumulate"); the tcgen05 path then runs bf16 x bf16 -> fp32 MMAs with an fp32 latent.
+ * fp32 accumulate"); the tcgen05 kernels encode them exactly as fp16 operands (activations rounded to fp16), accumulate
+ * in fp32 and keep the latent in fp32 (S14).
  * Errors: WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_UNSUPPORTED, WM_ERR_CUDA.  Synchronous. */
 int wm_load_weights(const char* path, int device, wm_ctx** ctx_out);
 

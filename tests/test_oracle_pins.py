@@ -1,4 +1,4 @@
-"""Pins for the float64 oracle.  CPU only.
+"""Pins for the float64 oracle (P14-P18 for the NEXT rows f1-f3).  CPU only.
 
 Each pin checks the oracle against something other than itself: hand-expanded fixtures under
 tests/golden/, closed forms, torch float64 library routines, brute force (scalar loops) and the
