@@ -104,7 +104,7 @@ constexpr int TRACE_CAP = 16384;
 #endif
 
 struct SmemLayout {
-    uint32_t a1, hbuf, ring, hwk, lp, ids, lens, cnt, b1, red, bars, sched, tmem_slot, total;
+    uint32_t a1, hbuf, ring, hwk, lp, ids, cnt, b1, red, bars, sched, tmem_slot, total;
 };
 
 __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps) {
@@ -116,7 +116,6 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
     L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
     L.lp = o; o += TMR * MAX_P * 4;
     L.ids = o; o += TMR * 4;
-    L.lens = o; o += TMR * 4;
     L.cnt = o; o += TMR * (uint32_t)n_types;          // u8 counts, row-major [64][n_types]
     o = (o + 15) & ~15u;
     L.b1 = o; o += 3 * D * 4;                          // b2, gamma, beta (LayerNorm: on the critical path; b1 is __ldg)

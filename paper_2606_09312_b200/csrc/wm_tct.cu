@@ -76,7 +76,7 @@ struct Params {
 };
 
 struct SmemLayout {
-    uint32_t a1, hwk, ring, e_tab, lp, ids, lens, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
+    uint32_t a1, hwk, ring, e_tab, lp, ids, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
 };
 
 __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps) {
@@ -88,7 +88,6 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
     L.e_tab = o; o += (uint32_t)n_types * DA * 2;
     L.lp = o; o += TM * MAX_P * 4;
     L.ids = o; o += TM * 4;
-    L.lens = o; o += TM * 4;
     L.cnt = o; o += TM * (uint32_t)n_types;           // u8 counts, row-major [128][n_types]
     o = (o + 15) & ~15u;
     L.b1 = o; o += (uint32_t)hid * 4;
@@ -313,32 +312,18 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                 __syncwarp();
             };
             // GEMM over the A1 K-blocks in the order a/phi (4,5), [hw], z (0..3); waits for the operands of the
-            // first chunk of a step / of the scorer.
-            // `z_first` (chunk 0 of a rollout step): the z K-blocks are issued before the a K-blocks — a_{t+1} is written
-            // only after the last chunk of step t has released the a-buffer, and the trace showed the issuer waiting
-            // ~4.4 K cycles per step for it; z' (LayerNorm) is ready earlier.  The a-buffer is released right after the
-            // last chunk's a K-blocks, not after the whole chunk.
-            auto gemm_a1 = [&](int b, bool first_chunk, bool last_chunk, bool with_hw, bool z_first) {
+            // first chunk of the scorer.  The a-buffer is released right after the last chunk's a K-blocks, not after
+            // the whole chunk (the action warps write a_{t+1} / phi into it as soon as it is free).
+            auto gemm_a1 = [&](int b, bool first_chunk, bool last_chunk, bool with_hw) {
                 wait_h(b);
                 const uint32_t d = T_D1 + 128u * b;
-                auto wait_a = [&]() { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); };
-                auto wait_z = [&]() { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); };
-                if (z_first) {
-                    wait_z();
-                    pair_ss(d, s_a1, s_a1 + TILE_BYTES, true);
-                    pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
-                    wait_a();
-                    pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, false);
-                    if (last_chunk) commit(B_AFREE);
-                } else {
-                    if (first_chunk) wait_a();
-                    pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
-                    if (with_hw) pair_hw(d);
-                    if (last_chunk) commit(B_AFREE);
-                    if (first_chunk) wait_z();
-                    pair_ss(d, s_a1, s_a1 + TILE_BYTES, false);
-                    pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
-                }
+                if (first_chunk) { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); ++n_a; WM_TRACE(21); }
+                pair_ss(d, s_a1 + 4 * TILE_BYTES, s_a1 + 5 * TILE_BYTES, true);
+                if (with_hw) pair_hw(d);
+                if (last_chunk) commit(B_AFREE);
+                if (first_chunk) { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); ++n_z; WM_TRACE(23); }
+                pair_ss(d, s_a1, s_a1 + TILE_BYTES, false);
+                pair_ss(d, s_a1 + 2 * TILE_BYTES, s_a1 + 3 * TILE_BYTES, false);
                 commit(B_D1FULL + b);
                 pend[b] = true;
             };
@@ -390,7 +375,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                     // residual MLP: GEMM1 chunks (a K-blocks with the folded W1a', z K-blocks on z_perp) / GEMM2
 #pragma unroll 1
                     for (int i = 0; i <= NC; ++i) {
-                        if (i < NC) gemm_a1(i & 1, false, i == NC - 1, false, false);
+                        if (i < NC) gemm_a1(i & 1, false, i == NC - 1, false);
                         if (i >= 1) gemm2(i - 1);
                     }
                     if (t + 1 < nsteps) {
@@ -406,7 +391,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                 // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
 #pragma unroll 1
                 for (int c = 0; c < 4; ++c) {
-                    gemm_a1(c & 1, c == 0, c == 3, true, false);
+                    gemm_a1(c & 1, c == 0, c == 3, true);
                 }
                 wait_h(0);
                 wait_h(1);   // all of H1 (fp16, TMEM columns [0,256)) written
