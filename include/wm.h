@@ -57,6 +57,7 @@ extern "C" {
 #define WM_FAULT_LEN    1u      /* a length was outside [0, T_max] (clamped)                                  */
 #define WM_FAULT_TYPE   2u      /* an action type id at a valid position was outside [0, n_types) (clamped)   */
 #define WM_FAULT_PARAM  4u      /* an action parameter at a valid position was < 1 (treated as 1)             */
+#define WM_FAULT_INDEX  8u      /* wm_rollout_score_from: a bank_index was outside [0, n_bank) (clamped)      */
 
 /* values of wm_info.kind / dtype / embed (the weight-file header fields) */
 #define WM_KIND_MLP     0
@@ -152,8 +153,8 @@ int wm_rollout_score(wm_ctx* ctx,
  * wm_rollout_score_from scores candidates whose first start[b] steps were rolled before:
  *   bank              [n_bank, d] fp32: latents (rows of a latents_out array, or any other store)
  *   bank_index        [B] int32: the row of `bank` that holds candidate b's latent after its first start[b] steps
- *                     (the task's initial latent when start[b] = 0); 0 <= bank_index[b] < n_bank is the CALLER's
- *                     contract (not checked on the device)
+ *                     (the task's initial latent when start[b] = 0); a value outside [0, n_bank) is clamped and
+ *                     raises WM_FAULT_INDEX in the fault word wm_check() reads
  *   start             [B] int32, clamped to [0, lengths[b]]: steps [0, start) are not rolled, they only feed phi
  *   action_ids, action_params, lengths, hw_feats, scores_out, subgraph_offsets (non-NULL), B, S, T_max: as in
  *                     wm_rollout_score, the action arrays holding each candidate's WHOLE sequence

@@ -442,7 +442,7 @@ int wm_rollout_score_from(wm_ctx* ctx, const float* bank, const int32_t* bank_in
         return WM_ERR_ARG;
     }
     CallArgs a = {};
-    a.init_states = bank; a.init_index = bank_index; a.start = start;
+    a.init_states = bank; a.init_index = bank_index; a.n_init = n_bank; a.start = start;
     a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
     a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets;
     a.B = B; a.S = S; a.T_max = T_max;

@@ -170,7 +170,15 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
             const int r = e % R, j = e / R;   // lanes over rows: conflict-free store; global read strided but tiny
             float v = 0.0f;
             if (m_cand[r] >= 0) {
-                const size_t zrow = a.init_index ? (size_t)__ldg(a.init_index + m_cand[r]) : (size_t)m_seg[r];
+                size_t zrow = (size_t)m_seg[r];
+                if (a.init_index) {   // banked latent (wm_rollout_score_from); clamped, WM_FAULT_INDEX when outside
+                    long long bi = __ldg(a.init_index + m_cand[r]);
+                    if (bi < 0 || bi >= a.n_init) {
+                        if (j == 0) atomicOr(a.fault, WM_FAULT_INDEX);
+                        bi = bi < 0 ? 0 : a.n_init - 1;
+                    }
+                    zrow = (size_t)bi;
+                }
                 v = __ldg(a.init_states + zrow * d + j);
             }
             X[(size_t)j * R + r] = v;

@@ -126,6 +126,7 @@ struct CallArgs {
     // prefix-latent reuse (NEXT row f3; wm_rollout_latents / wm_rollout_score_from), all null for wm_rollout_score:
     const int32_t* start;       // [B] steps [0, start) only feed phi, the rollout runs over [start, len)
     const int32_t* init_index;  // [B] row of init_states that holds candidate b's initial latent
+    int64_t n_init;             // rows of init_states when init_index is used (indices are clamped to it)
     float* latents_out;         // [B, T_max, d] z after step t+1 at [b][t] for start <= t < len; scores_out may be null
 };
 

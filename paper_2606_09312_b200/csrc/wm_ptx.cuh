@@ -275,6 +275,18 @@ __device__ __forceinline__ int row_start(const CallArgs& a, int cand, int len) {
     return (a.start && cand >= 0) ? clamp_start(__ldg(a.start + cand), len) : 0;
 }
 
+// Row of init_states that holds candidate `cand`'s initial latent: its subgraph's (seg), or the banked row
+// init_index names (clamped into [0, n_init), WM_FAULT_INDEX raised when it was outside).
+__device__ __forceinline__ size_t row_init(const CallArgs& a, int cand, int seg) {
+    if (!a.init_index || cand < 0) return (size_t)seg;
+    long long i = __ldg(a.init_index + cand);
+    if (i < 0 || i >= a.n_init) {
+        atomicOr(a.fault, WM_FAULT_INDEX);
+        i = i < 0 ? 0 : a.n_init - 1;
+    }
+    return (size_t)i;
+}
+
 // byte offset of the 16-byte chunk `chunk` (8 bf16 columns) of row `row` inside a SW128 K-major K-block tile
 __device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
     return (uint32_t)row * 128u + (uint32_t)((chunk ^ (row & 7)) << 4);

@@ -470,7 +470,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             row_meta(p.a, (int64_t)tile * TM + row, cand, len, seg, false);
             // prefix-latent reuse: the rollout covers positions [st, len) and starts from the row init_index names
             const int st = EXT ? row_start(p.a, cand, len) : 0, rem = len - st;
-            const size_t zrow = (EXT && p.a.init_index && cand >= 0) ? (size_t)__ldg(p.a.init_index + cand) : (size_t)seg;
+            const size_t zrow = EXT ? row_init(p.a, cand, seg) : (size_t)seg;
 
             // ---- z_0 (the task's initial latent; or the banked latent after the first st steps)
 #pragma unroll 1

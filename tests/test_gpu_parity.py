@@ -510,6 +510,15 @@ def test_prefix_calls_argument_and_edge_cases(wm, n):
                                      b.lengths, b.hw_feats, b.subgraph_offsets, n_buckets=cfg.n_buckets,
                                      ln_eps=cfg.ln_eps)
     assert oracle.score_error(sc.cpu().numpy(), want, b.subgraph_offsets) <= tol
+    # a bank_index outside [0, n_bank) is clamped and reported (both ends), the other candidates are unaffected
+    bad = own.clone(); bad[3] = -5; bad[7] = b.B + 1000
+    sc_bad = torch.zeros_like(sc)
+    wm.wm_rollout_score_from(ctx, bank2, bad, dv["lengths"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                             dv["hw_feats"], sc_bad, dv["subgraph_offsets"])
+    assert wm.wm_check(ctx) == wm.WM_FAULT_INDEX
+    keep = np.ones(b.B, dtype=bool); keep[[3, 7]] = False
+    np.testing.assert_array_equal(sc_bad.cpu().numpy()[keep].view(np.uint32), sc.cpu().numpy()[keep].view(np.uint32))
+    assert wm.wm_check(ctx) == 0
     # B = 1
     one = torch.zeros(1, dtype=torch.float32, device="cuda:0")
     off1 = torch.tensor([0, 1], dtype=torch.int32, device="cuda:0")
