@@ -12,6 +12,7 @@ KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH = 0, 1, 2, 3
 DTYPE_FP32, DTYPE_BF16 = 0, 1
 EMBED_LINEAR, EMBED_BUCKET = 0, 1
 PHI_MEAN, PHI_STRUCT = 0, 1     # action features of the ranker: mean action embedding | structured statistics (f2)
+RANKER_MLP, RANKER_FOREST = 0, 1   # G: the configs' MLP | a tree ensemble, the paper's own kind of ranker (f4)
 
 
 @dataclass(frozen=True)
@@ -44,6 +45,9 @@ class WMConfig:
     prefix_cut_lo: int = 0
     prefix_cut_hi: int = 0
     phi_kind: int = PHI_MEAN    # PHI_STRUCT: the paper's structured action features (S25)
+    ranker_kind: int = RANKER_MLP   # RANKER_FOREST: synthetic complete binary trees (S27)
+    n_trees: int = 0
+    tree_depth: int = 0
 
     @property
     def B(self) -> int:
@@ -77,6 +81,8 @@ class WMConfig:
         return 2 * (self.hidden * (self.d + self.d_a) + self.d * self.hidden)
 
     def flops_scorer(self) -> int:
+        if self.ranker_kind == RANKER_FOREST:     # comparisons and adds, not a contraction: counted as 0 FLOP
+            return 0
         dims = (self.scorer_in,) + tuple(self.scorer_widths) + (1,)
         return 2 * sum(a * b for a, b in zip(dims[:-1], dims[1:]))
 
@@ -116,6 +122,16 @@ CONFIGS = {
                 T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
                 param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(512, 512), k=64,
                 phi_kind=PHI_STRUCT),
+    # NEXT row f4: a tree-ensemble ranker (the paper's G is an XGBoost model) on synthetic
+    # random trees over [z_T ; structured phi ; h].  10 = cfg 1's shapes (fp32), 11 = cfg 2's shapes and batch.
+    10: WMConfig("f4_forest_tiny_fp32", 10, KIND_MLP, DTYPE_FP32, EMBED_LINEAR, S=1, per_subgraph=64, T_max=8,
+                 len_dist="uniform", len_lo=0, len_hi=8, n_types=16, P=4, param_dist="uniform", param_hi=64,
+                 n_buckets=0, d=64, d_a=32, hidden=128, H=8, scorer_widths=(), k=8, phi_kind=PHI_STRUCT,
+                 ranker_kind=RANKER_FOREST, n_trees=32, tree_depth=4),
+    11: WMConfig("f4_forest_evolution_round", 11, KIND_MLP_LN, DTYPE_BF16, EMBED_LINEAR, S=16, per_subgraph=2048,
+                 T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
+                 param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(), k=64,
+                 phi_kind=PHI_STRUCT, ranker_kind=RANKER_FOREST, n_trees=128, tree_depth=6),
 }
 
 

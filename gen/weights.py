@@ -19,7 +19,7 @@ from typing import Dict, List
 import numpy as np
 
 from .configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, EMBED_BUCKET,
-                      PHI_STRUCT)
+                      PHI_STRUCT, RANKER_FOREST)
 
 MAGIC = b"WMW1"
 VERSION = 1
@@ -49,6 +49,8 @@ def tensor_order(cfg: WMConfig) -> List[str]:
         names += ["W_w", "W_d", "W1", "b1", "W2", "b2"]
     else:
         names += ["W_g", "W_r", "W_h"]
+    if cfg.ranker_kind == RANKER_FOREST:   # feature index, threshold per internal node; value per leaf; base score
+        return names + ["Tf", "Tt", "Tv", "Tb"]
     for i in range(len(cfg.scorer_widths) + 1):
         names += [f"Ws{i}", f"bs{i}"]
     return names
@@ -77,6 +79,13 @@ def tensor_shapes(cfg: WMConfig) -> Dict[str, tuple]:
     else:
         for n in ("W_g", "W_r", "W_h"):
             sh[n] = (d, d + da)
+    if cfg.ranker_kind == RANKER_FOREST:
+        nodes = 2 ** cfg.tree_depth - 1
+        sh["Tf"] = (cfg.n_trees, nodes)
+        sh["Tt"] = (cfg.n_trees, nodes)
+        sh["Tv"] = (cfg.n_trees, nodes + 1)
+        sh["Tb"] = (1,)
+        return sh
     dims = (cfg.scorer_in,) + tuple(cfg.scorer_widths) + (1,)
     for i, (a, b) in enumerate(zip(dims[:-1], dims[1:])):
         sh[f"Ws{i}"] = (b, a)
@@ -90,6 +99,8 @@ def make_weights(cfg: WMConfig) -> Dict[str, np.ndarray]:
     w: Dict[str, np.ndarray] = {}
     for name in tensor_order(cfg):
         shp = shapes[name]
+        if name in ("Tf", "Tt", "Tv", "Tb"):     # the synthetic forest is drawn in one go, after everything else
+            continue
         if name in ("E", "Tbl"):
             t = rng.standard_normal(shp)
         elif name == "gamma":
@@ -107,7 +118,34 @@ def make_weights(cfg: WMConfig) -> Dict[str, np.ndarray]:
         if cfg.dtype == DTYPE_BF16:
             t = round_to_bf16(t)
         w[name] = t
+    if cfg.ranker_kind == RANKER_FOREST:
+        w.update(_draw_forest(rng, cfg))
     return w
+
+
+def _draw_forest(rng: np.random.Generator, cfg: WMConfig) -> Dict[str, np.ndarray]:
+    """Synthetic complete binary trees over x = [z_T ; structured phi ; h] (stand-ins for a trained XGBoost ranker, which
+    is not available here): a uniformly drawn feature per internal node, a threshold drawn over that feature's typical
+    range (latent and hardware features ~ N(0, 0.7); counts, length, sums, means and maxima over their ranges), leaf
+    values ~ N(0, 1/n_trees).  Feature indices are stored as fp32 (exact), everything fp32 whatever cfg.dtype says:
+    thresholds are compared in fp32 on both sides."""
+    nodes = 2 ** cfg.tree_depth - 1
+    nin = cfg.scorer_in
+    feat = rng.integers(0, nin, size=(cfg.n_trees, nodes))
+    lo = np.zeros(nin); hi = np.zeros(nin); gauss = np.zeros(nin, dtype=bool)
+    d, nt, P, T = cfg.d, cfg.n_types, cfg.P, float(cfg.T_max)
+    gauss[:d] = True; gauss[d + cfg.phi_dim:] = True
+    o = d
+    hi[o:o + nt] = 3.0 * T / nt + 1.0                       # per-type counts
+    lo[o + nt], hi[o + nt] = cfg.len_lo, cfg.len_hi          # length
+    top = np.log2(cfg.param_hi)
+    hi[o + nt + 1:o + nt + 1 + P] = top * T / 2              # sums of log2 params
+    hi[o + nt + 1 + P:o + nt + 1 + 3 * P] = top              # means, maxima
+    u = rng.random((cfg.n_trees, nodes)); g = rng.standard_normal((cfg.n_trees, nodes)) * 0.7
+    thr = np.where(gauss[feat], g, lo[feat] + u * (hi[feat] - lo[feat]))
+    leaf = rng.standard_normal((cfg.n_trees, nodes + 1)) / np.sqrt(cfg.n_trees)
+    return {"Tf": feat.astype(np.float32), "Tt": thr.astype(np.float32), "Tv": leaf.astype(np.float32),
+            "Tb": rng.standard_normal(1).astype(np.float32)}
 
 
 def phi_column_scale(cfg: WMConfig) -> np.ndarray:
@@ -126,12 +164,18 @@ def _matrix_of(bias: str) -> str:
 
 def header_bytes(cfg: WMConfig) -> bytes:
     widths = list(cfg.scorer_widths) + [0] * (MAX_SCORER_HIDDEN - len(cfg.scorer_widths))
-    version = VERSION if cfg.phi_kind == 0 else 2      # version 2 = version 1 + a trailing uint32 phi_kind
+    # version 2 = version 1 + a trailing uint32 phi_kind; version 3 = version 2 + uint32 ranker_kind, n_trees, tree_depth
+    forest = cfg.ranker_kind == RANKER_FOREST
+    version = 3 if forest else (VERSION if cfg.phi_kind == 0 else 2)
     hdr = MAGIC + struct.pack(
         "<12I%dIf" % MAX_SCORER_HIDDEN,
         version, cfg.kind, cfg.dtype, cfg.embed, cfg.d, cfg.d_a, cfg.hidden, cfg.n_types, cfg.P,
-        cfg.n_buckets, cfg.H, len(cfg.scorer_widths) + 1, *widths, cfg.ln_eps)
-    return hdr if version == 1 else hdr + struct.pack("<I", cfg.phi_kind)
+        cfg.n_buckets, cfg.H, 0 if forest else len(cfg.scorer_widths) + 1, *widths, cfg.ln_eps)
+    if version >= 2:
+        hdr += struct.pack("<I", cfg.phi_kind)
+    if version >= 3:
+        hdr += struct.pack("<3I", cfg.ranker_kind, cfg.n_trees, cfg.tree_depth)
+    return hdr
 
 
 def write_weight_file(path: str, cfg: WMConfig, weights: Dict[str, np.ndarray]) -> None:

@@ -20,7 +20,9 @@ mask) and `rollout_score_scalar` (pure per-candidate python loops, math.erf) —
 Pins (tests/test_oracle_pins.py): P1..P13 of SURVEY.md §8(c) — hand-expanded 2x3 MLP step and GRU step
 (values in tests/golden/), closed forms, torch float64 library cross-checks, scalar-vs-vector brute
 force, top-k vs full sort; P14/P15 the TransH step, P16/P17 the structured phi (hand-worked sequence in
-tests/golden/p16_phi_struct.txt, closed forms, a scorer that reads single features).  The paper prints no worked numeric example of this path, so the composition
+tests/golden/p16_phi_struct.txt, closed forms, a scorer that reads single features), P18 prefix-latent reuse against
+the literal path, P19/P20 the tree-ensemble ranker (hand-worked forest in tests/golden/p19_forest.txt, stumps in closed
+form, scikit-learn's DecisionTreeRegressor as the library cross-check).  The paper prints no worked numeric example of this path, so the composition
 at full size rests on those pins: beyond them, parity unpinned.
 """
 from __future__ import annotations
@@ -158,6 +160,41 @@ def phi_struct(ids, params, n_types: int) -> np.ndarray:
     return np.concatenate([counts, [float(n)], s, m, x])
 
 
+def forest_score(x, Tf, Tt, Tv, Tb, return_margin: bool = False):
+    """Tree-ensemble ranker (NEXT row f4).  PAPER.md:190: "G is implemented as an XGBoost ranking model" — an additive
+    ensemble of regression trees over the concatenated features (Eq.12); the paper prints no tree, so reading S27
+     fixes synthetic COMPLETE binary trees in heap order: at node i (root 0) go to child 2i+1 when
+    x[f_i] < t_i, else to child 2i+2; after `depth` levels the node index minus (2^depth - 1) is the leaf;
+    y = Tb + sum over trees of the leaf value.  The comparison is taken in float32 on both sides (x and t rounded to
+    float32: a decision, so the kernel's precision), the sum in float64.
+    x [n, n_in]; Tf, Tt [n_trees, 2^depth - 1]; Tv [n_trees, 2^depth]; Tb [1].  One candidate, one tree, one level at a
+    time.  With return_margin also the smallest |x[f] - t| met on any path of the candidate (how close it came to
+    taking another branch)."""
+    x32 = np.asarray(x, dtype=np.float32)
+    Tf = np.asarray(Tf).astype(np.int64); Tt = np.asarray(Tt, dtype=np.float32); Tv = np.asarray(Tv, dtype=F64)
+    n_trees, nodes = Tf.shape
+    depth = int(round(math.log2(nodes + 1)))
+    assert 2 ** depth - 1 == nodes and Tv.shape == (n_trees, nodes + 1)
+    y = np.full(x32.shape[0], float(np.asarray(Tb, F64).reshape(-1)[0]), dtype=F64)
+    margin = np.full(x32.shape[0], np.inf, dtype=F64)
+    for c in range(x32.shape[0]):
+        for t in range(n_trees):
+            node = 0
+            for _ in range(depth):
+                v, thr = x32[c, Tf[t, node]], Tt[t, node]
+                margin[c] = min(margin[c], abs(float(v) - float(thr)))
+                node = 2 * node + (1 if v < thr else 2)
+            y[c] += Tv[t, node - nodes]
+    return (y, margin) if return_margin else y
+
+
+def _rank(x: np.ndarray, w: Dict[str, np.ndarray], n_layers: int) -> np.ndarray:
+    """G on the concatenated features: the forest when the model carries one, else the MLP."""
+    if "Tf" in w:
+        return forest_score(x, w["Tf"], w["Tt"], w["Tv"], w["Tb"])
+    return scorer(x, w, n_layers)
+
+
 def scorer(x: np.ndarray, w: Dict[str, np.ndarray], n_layers: int) -> np.ndarray:
     """G as an MLP: hidden linears followed by GELU, last linear plain (S8). Returns [...]."""
     for i in range(n_layers):
@@ -244,7 +281,7 @@ def rollout_score_vec(w: Dict[str, np.ndarray], init_states, action_ids, action_
         if phi_kind == PHI_STRUCT:
             n_types = w["E"].shape[0] if "E" in w else w["Tbl"].shape[0] // (P * n_buckets)
             phi = np.stack([phi_struct(ids[lo + i, :ln[i]], par[lo + i, :ln[i], :], n_types) for i in range(n)])
-        scores[lo:hi] = scorer(np.concatenate([z, phi, h], axis=-1), w, nl)
+        scores[lo:hi] = _rank(np.concatenate([z, phi, h], axis=-1), w, nl)
         if return_latent:
             lat[lo:hi] = z
     return (scores, lat) if return_latent else scores
@@ -301,7 +338,7 @@ def rollout_score_from(w, bank, bank_index, start, action_ids, action_params, le
             phi = _embed(w, ids[b, :n], par[b, :n, :], P, n_buckets).sum(axis=0) / n
         else:
             phi = np.zeros((w["Tbl"] if "Tbl" in w else w["E"]).shape[1], dtype=F64)
-        out[b] = scorer(np.concatenate([z[0], phi, hw[seg[b]]])[None, :], w, nl)[0]
+        out[b] = _rank(np.concatenate([z[0], phi, hw[seg[b]]])[None, :], w, nl)[0]
     return out
 
 
@@ -393,6 +430,16 @@ def rollout_score_scalar(w, init_states, action_ids, action_params, lengths, hw_
                     big[j] = l2 if t == 0 else max(big[j], l2)
             phi = cnt + [float(lens[b])] + tot + [v / lens[b] if lens[b] > 0 else 0.0 for v in tot] + big
         x = z + phi + list(hw[s])
+        if "Tf" in W:      # tree ensemble (S27), comparisons in float32
+            nodes = len(W["Tf"][0])
+            tot = W["Tb"][0]
+            for tf, tt, tv in zip(W["Tf"], W["Tt"], W["Tv"]):
+                node = 0
+                while node < nodes:
+                    node = 2 * node + (1 if np.float32(x[int(tf[node])]) < np.float32(tt[node]) else 2)
+                tot += tv[node - nodes]
+            out.append(tot)
+            continue
         nl = _n_scorer_layers(w)
         for i in range(nl):
             x = [ui + bi for ui, bi in zip(mv(W[f"Ws{i}"], x), W[f"bs{i}"])]
@@ -467,16 +514,20 @@ def read_weight_file(path: str):
         raise ValueError("bad magic")
     vals = struct.unpack_from("<12I6If", raw, 4)
     (version, kind, dtype, embed, d, d_a, hidden, n_types, P, n_buckets, H, n_lin) = vals[:12]
-    widths = [x for x in vals[12:18]][: n_lin - 1]
+    widths = [x for x in vals[12:18]][: max(n_lin - 1, 0)]
     eps = vals[18]
     hdr = dict(version=version, kind=kind, dtype=dtype, embed=embed, d=d, d_a=d_a, hidden=hidden,
                n_types=n_types, P=P, n_buckets=n_buckets, H=H, n_scorer_layers=n_lin,
                scorer_widths=widths, ln_eps=eps)
     pos = 4 + struct.calcsize("<12I6If")
     hdr["phi_kind"] = PHI_MEAN
-    if version == 2:      # version 2 = version 1 + uint32 phi_kind
+    if version >= 2:      # version 2 = version 1 + uint32 phi_kind
         hdr["phi_kind"] = struct.unpack_from("<I", raw, pos)[0]
         pos += 4
+    hdr.update(ranker_kind=0, n_trees=0, tree_depth=0)
+    if version == 3:      # version 3 = version 2 + uint32 ranker_kind, n_trees, tree_depth
+        hdr["ranker_kind"], hdr["n_trees"], hdr["tree_depth"] = struct.unpack_from("<3I", raw, pos)
+        pos += 12
     phi_dim = d_a if hdr["phi_kind"] == PHI_MEAN else n_types + 1 + 3 * P
     w = {}
 
@@ -499,6 +550,10 @@ def read_weight_file(path: str):
         take("W1", hidden, d + d_a); take("b1", hidden); take("W2", d, hidden); take("b2", d)
     else:
         take("W_g", d, d + d_a); take("W_r", d, d + d_a); take("W_h", d, d + d_a)
+    if hdr["ranker_kind"] == 1:
+        nodes = 2 ** hdr["tree_depth"] - 1
+        take("Tf", hdr["n_trees"], nodes); take("Tt", hdr["n_trees"], nodes); take("Tv", hdr["n_trees"], nodes + 1)
+        take("Tb", 1)
     dims = [d + phi_dim + H] + widths + [1]
     for i in range(n_lin):
         take(f"Ws{i}", dims[i + 1], dims[i]); take(f"bs{i}", dims[i + 1])

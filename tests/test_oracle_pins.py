@@ -483,12 +483,92 @@ def test_p18_latents_and_score_from(kind, embed, phi):
     assert abs(sub[0] - y[i]) > 1e-6
 
 
+# ---- P19 / P20: tree-ensemble ranker (NEXT row f4, S27) ---------------------------------
+
+def test_p19_forest_hand_worked(golden):
+    g = golden("p19_forest.txt")
+    Tf = [[0, 2, 1], [1, 2, 0]]; Tt = [[1.0, 2.0, 0.0], [-1.0, 0.0, 0.5]]
+    Tv = [[10, 20, 30, 40], [1, 2, 3, 4]]
+    x = [[0.5, -1.0, 3.0], [2.0, -3.0, 1.0]]
+    y, m = oracle.forest_score(x, Tf, Tt, Tv, [0.25], return_margin=True)
+    np.testing.assert_array_equal(y, g["y"])
+    np.testing.assert_array_equal(m, g["margin"])
+    # the fixture discriminates: "<=" instead of "<" (x_a sits on two thresholds), swapped children, or a leaf offset
+    # of 2^depth instead of 2^depth - 1 would each change y
+    assert oracle.forest_score(np.array(x) - 1e-3, Tf, Tt, Tv, [0.25])[0] != g["y"][0]
+
+
+def test_p20_forest_closed_forms_and_library():
+    rng = np.random.default_rng(20)
+    n, nin, nt = 40, 9, 17
+    x = rng.standard_normal((n, nin))
+    # (a) stumps (depth 1): y = base + sum_t (x[f_t] < thr_t ? left_t : right_t), written with numpy comparisons
+    f = rng.integers(0, nin, nt); thr = rng.standard_normal(nt).astype(np.float32); lv = rng.standard_normal((nt, 2))
+    want = 0.5 + np.where(x.astype(np.float32)[:, f] < thr[None, :], lv[None, :, 0], lv[None, :, 1]).sum(axis=1)
+    np.testing.assert_allclose(oracle.forest_score(x, f[:, None], thr[:, None], lv, [0.5]), want, rtol=0, atol=1e-12)
+    # (b) a tree whose thresholds are all +inf always goes left: leaf 0; all -inf: the last leaf
+    D = 3; nodes = 2 ** D - 1
+    Tv = rng.standard_normal((1, nodes + 1))
+    inf = np.full((1, nodes), np.inf, dtype=np.float32)
+    assert (oracle.forest_score(x, np.zeros((1, nodes)), inf, Tv, [0.0]) == Tv[0, 0]).all()
+    assert (oracle.forest_score(x, np.zeros((1, nodes)), -inf, Tv, [0.0]) == Tv[0, -1]).all()
+    # (c) moving every feature by less than the reported margin changes no decision
+    Tf = rng.integers(0, nin, (nt, nodes)); Tt = rng.standard_normal((nt, nodes)).astype(np.float32)
+    Tvv = rng.standard_normal((nt, nodes + 1))
+    y, m = oracle.forest_score(x, Tf, Tt, Tvv, [0.0], return_margin=True)
+    assert (m > 0).all()
+    np.testing.assert_array_equal(oracle.forest_score(x + 0.4 * m[:, None] * rng.choice([-1.0, 1.0], x.shape), Tf, Tt, Tvv, [0.0]), y)
+    # (d) library cross-check: scikit-learn regression trees converted to the complete heap layout predict the same.
+    # Data on a grid of eighths: sklearn splits at midpoints (odd sixteenths: exact in float32, never hit by an x), so
+    # its "x <= t" and this ranker's "x < t" agree.
+    from sklearn.tree import DecisionTreeRegressor
+    xg = rng.integers(-16, 17, (300, 5)) / 8.0
+    total = np.zeros(300)
+    trees = []
+    for t in range(3):
+        yt = rng.standard_normal(300)
+        sk = DecisionTreeRegressor(max_depth=D, random_state=t).fit(xg, yt)
+        tr = sk.tree_
+        hf = np.zeros(nodes); ht = np.full(nodes, np.inf, dtype=np.float32); hv = np.zeros(nodes + 1)
+
+        def fill(sk_node, heap, depth):
+            if depth == D:
+                hv[heap - nodes] = tr.value[sk_node][0][0]
+                return
+            if tr.children_left[sk_node] == -1:       # an early leaf: always-left dummy splits below it, same value
+                fill(sk_node, 2 * heap + 1, depth + 1)
+                fill(sk_node, 2 * heap + 2, depth + 1)
+                return
+            hf[heap] = tr.feature[sk_node]; ht[heap] = tr.threshold[sk_node]
+            assert float(ht[heap]) == tr.threshold[sk_node]
+            fill(tr.children_left[sk_node], 2 * heap + 1, depth + 1)
+            fill(tr.children_right[sk_node], 2 * heap + 2, depth + 1)
+
+        fill(0, 0, 0)
+        trees.append((hf, ht, hv))
+        total += sk.predict(xg)
+    got = oracle.forest_score(xg, np.stack([a for a, _, _ in trees]), np.stack([b for _, b, _ in trees]),
+                              np.stack([c for _, _, c in trees]), [0.0])
+    np.testing.assert_allclose(got, total, rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("n", [10])
+def test_p9_scalar_vs_vector_forest(n):
+    cfg = gen.get_config(n)
+    w = gen.make_weights(cfg); b = gen.make_inputs(cfg)
+    yv = run_vec(cfg, w, b)
+    ys = oracle.rollout_score_scalar(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.hw_feats,
+                                     b.subgraph_offsets, phi_kind=cfg.phi_kind)
+    np.testing.assert_allclose(yv, ys, rtol=0, atol=1e-12)
+    assert np.unique(np.round(yv, 9)).size > 30        # the forest separates the candidates
+
+
 # ---- generator / file format ----------------------------------------------------------------------------------
 
 def test_weight_file_roundtrip(tmp_path):
-    for n in (1, 2, 5, 6, 8, 9):
+    for n in (1, 2, 5, 6, 8, 9, 10):
         cfg = gen.get_config(n)
-        if n not in (1, 8):
+        if n not in (1, 8, 10):
             cfg = WMConfig(**{**cfg.__dict__, "d": 16, "d_a": 8, "hidden": 0 if n == 5 else 24,
                               "scorer_widths": (12, 10)})
         w = gen.make_weights(cfg)
@@ -496,8 +576,11 @@ def test_weight_file_roundtrip(tmp_path):
         gen.write_weight_file(p, cfg, w)
         hdr, w2 = oracle.read_weight_file(p)
         assert hdr["d"] == cfg.d and hdr["kind"] == cfg.kind and hdr["P"] == cfg.P
-        assert hdr["phi_kind"] == cfg.phi_kind and hdr["version"] == (1 if cfg.phi_kind == PHI_MEAN else 2)
-        assert w2["Ws0"].shape[1] == cfg.d + cfg.phi_dim + cfg.H
+        assert hdr["phi_kind"] == cfg.phi_kind
+        assert hdr["version"] == (3 if cfg.ranker_kind else (1 if cfg.phi_kind == PHI_MEAN else 2))
+        assert hdr["ranker_kind"] == cfg.ranker_kind and hdr["n_trees"] == cfg.n_trees
+        if cfg.ranker_kind == 0:
+            assert w2["Ws0"].shape[1] == cfg.d + cfg.phi_dim + cfg.H
         assert list(w2.keys()) == gen.tensor_order(cfg)
         for kname in w:
             np.testing.assert_array_equal(w[kname], w2[kname])
