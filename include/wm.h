@@ -76,6 +76,12 @@ extern "C" {
                                /* n_types + 1 + 3P values; this build needs n_types + 1 + 3P <= d_a                    */
 
 /* wm_set_option keys */
+#define WM_RANKER_MLP    0     /* G = the configs' MLP                                                              */
+#define WM_RANKER_FOREST 1     /* G = an ensemble of complete binary regression trees over [z_T ; phi ; h] (*/
+                               /* the paper's G is an XGBoost model; S27): heap order, at node i go to child    */
+                               /* 2i+1 when x[f_i] < t_i (fp32 comparison), else 2i+2; score = base + sum of leaf values. */
+                               /* Needs WM_PHI_STRUCT and P <= 8 in this build                                           */
+
 #define WM_OPT_PATH      1      /* 0 = auto (default), 1 = force the fp32 CUDA-core kernel, 2 = force tcgen05  */
 #define WM_OPT_SORT      2      /* 1 = bucket candidates by length before tiling (default), 0 = input order    */
 #define WM_OPT_TIMING    3      /* 1 = record CUDA events around the rollout+score kernel (K2) of every call,   */
@@ -95,6 +101,8 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
                                 /* 3 = wm_tcg_kernel (CTA pair per tile, GRU transition, d = 384),             */
                                 /* 4 = wm_tct_kernel (TransH transition, d = 256)                              */
     int32_t phi_kind;           /* WM_PHI_*: which action features G reads                                     */
+    int32_t ranker_kind;        /* WM_RANKER_*                                                                 */
+    int32_t n_trees, tree_depth;   /* WM_RANKER_FOREST only                                                    */
 } wm_info;
 
 /* Read a WMW1 weight file (format below), convert to the kernels' layouts and copy to `device`.
@@ -103,12 +111,15 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
  *   ctx_out  receives the context (caller frees with wm_free).
  * File format (little-endian): "WMW1", then uint32 version, kind, dtype, embed, d, d_a, hidden, n_types, P,
  * n_buckets, H, n_scorer_layers, uint32 scorer_widths[6], float ln_eps (80 bytes in all); version 2 files carry one
- * more uint32, phi_kind (version 1 means WM_PHI_MEAN); then fp32 tensors, row-major, in this order:
+ * more uint32, phi_kind (version 1 means WM_PHI_MEAN); version 3 files three more, ranker_kind, n_trees, tree_depth (and
+ * n_scorer_layers = 0 for a forest); then fp32 tensors, row-major, in this order:
  *   EMBED_LINEAR: E[n_types,d_a], W_p[d_a,P], b_p[d_a]        EMBED_BUCKET: Tbl[n_types*P*n_buckets, d_a]
  *   MLP / MLP_LN: W1[hidden,d+d_a], b1[hidden], W2[d,hidden], b2[d] (, gamma[d], beta[d])
  *   GRU:          W_g[d,d+d_a], W_r[d,d+d_a], W_h[d,d+d_a]
  *   TRANSH:       W_w[d,d_a], W_d[d,d_a], then W1, b1, W2, b2 as for MLP
  *   G:            for each linear i: Ws_i[out_i,in_i], bs_i[out_i];  in_0 = d+dim(phi)+H, out_last = 1
+ *   G (forest):   Tf[n_trees, 2^depth-1] feature indices (stored as fp32), Tt[n_trees, 2^depth-1] thresholds,
+ *                 Tv[n_trees, 2^depth] leaf values, Tb[1] base score
  * With dtype = bf16 every stored value is already bf16-representable (BASELINE.json cfg 2-5: "bf16 weights with
  * fp32 accumulate"); the tcgen05 kernels encode them exactly as fp16 operands (activations rounded to fp16), accumulate
  * in fp32 and keep the latent in fp32 (S14).

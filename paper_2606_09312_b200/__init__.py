@@ -32,7 +32,8 @@ class WmInfo(ctypes.Structure):
                 ("n_types", ctypes.c_int32), ("P", ctypes.c_int32), ("n_buckets", ctypes.c_int32),
                 ("H", ctypes.c_int32), ("n_scorer_layers", ctypes.c_int32),
                 ("scorer_widths", ctypes.c_int32 * 6), ("ln_eps", ctypes.c_float), ("path", ctypes.c_int32),
-                ("tc_variant", ctypes.c_int32), ("phi_kind", ctypes.c_int32)]
+                ("tc_variant", ctypes.c_int32), ("phi_kind", ctypes.c_int32),
+                ("ranker_kind", ctypes.c_int32), ("n_trees", ctypes.c_int32), ("tree_depth", ctypes.c_int32)]
 
 
 class WmError(RuntimeError):

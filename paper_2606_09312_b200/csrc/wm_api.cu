@@ -111,21 +111,35 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         set_error("wm_load_weights: file shorter than the header");
         return WM_ERR_FORMAT;
     }
-    if (memcmp(magic, "WMW1", 4) != 0 || (h.version != 1 && h.version != 2)) {
+    if (memcmp(magic, "WMW1", 4) != 0 || h.version < 1 || h.version > 3) {
         fclose(f);
         set_error("wm_load_weights: bad magic or version");
         return WM_ERR_FORMAT;
     }
     uint32_t phi_kind = WM_PHI_MEAN;   // version 2 = the version-1 header followed by uint32 phi_kind
-    if (h.version == 2 && (fread(&phi_kind, 4, 1, f) != 1 || phi_kind > WM_PHI_STRUCT)) {
+    if (h.version >= 2 && (fread(&phi_kind, 4, 1, f) != 1 || phi_kind > WM_PHI_STRUCT)) {
         fclose(f);
         set_error("wm_load_weights: bad phi_kind");
         return WM_ERR_FORMAT;
     }
+    uint32_t forest[3] = {WM_RANKER_MLP, 0, 0};   // version 3 = version 2 + uint32 ranker_kind, n_trees, tree_depth
+    if (h.version == 3 && (fread(forest, 4, 3, f) != 3 || forest[0] > WM_RANKER_FOREST ||
+                           (forest[0] == WM_RANKER_FOREST &&
+                            (forest[1] < 1 || forest[1] > 65536 || forest[2] < 1 || forest[2] > 12 || h.n_lin != 0)))) {
+        fclose(f);
+        set_error("wm_load_weights: bad ranker fields (kind, n_trees 1..65536, tree_depth 1..12, n_scorer_layers 0)");
+        return WM_ERR_FORMAT;
+    }
+    const bool is_forest = forest[0] == WM_RANKER_FOREST;
+    if (is_forest && (phi_kind != WM_PHI_STRUCT || h.P > 8)) {
+        fclose(f);
+        set_error("wm_load_weights: the forest ranker needs the structured phi and P <= 8 in this build");
+        return WM_ERR_UNSUPPORTED;
+    }
     const bool mlp = h.kind == WM_KIND_MLP || h.kind == WM_KIND_MLP_LN || h.kind == WM_KIND_TRANSH;
     if (h.kind > 3 || h.dtype > 1 || h.embed > 1 || h.d == 0 || h.d_a == 0 || h.n_types == 0 || h.P == 0 ||
         h.d > 65536 || h.d_a > 65536 || h.hidden > 65536 || h.P > 64 || h.H > 65536 || h.n_types > (1u << 20) ||
-        h.n_lin < 1 || h.n_lin > 7 || (mlp && h.hidden == 0) || (h.embed == WM_EMBED_BUCKET && h.n_buckets == 0) ||
+        h.n_lin > 7 || (mlp && h.hidden == 0) || (h.embed == WM_EMBED_BUCKET && h.n_buckets == 0) ||
         h.n_buckets > 4096 || !(h.ln_eps >= 0.0f)) {
         fclose(f);
         set_error("wm_load_weights: header field out of range");
@@ -170,11 +184,19 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
     int sdim[kMaxScorerLinears + 1] = {};
     sdim[0] = d + phi_dim + h.H;
     for (uint32_t i = 0; i + 1 < h.n_lin; ++i) sdim[i + 1] = h.widths[i];
-    sdim[h.n_lin] = 1;
+    if (h.n_lin >= 1) sdim[h.n_lin] = 1;   // (a forest model has no linears: sdim[0] stays the feature count)
     for (uint32_t i = 0; i < h.n_lin; ++i) {
         char nm[16];
         snprintf(nm, sizeof(nm), "Ws%u", i); add(nm, sdim[i + 1], sdim[i]);
         snprintf(nm, sizeof(nm), "bs%u", i); add(nm, sdim[i + 1], 1);
+    }
+    if (is_forest) {
+        const int nodes = (1 << forest[2]) - 1;
+        add("Tf", forest[1], nodes); add("Tt", forest[1], nodes); add("Tv", forest[1], nodes + 1); add("Tb", 1, 1);
+    } else if (h.n_lin < 1) {
+        fclose(f);
+        set_error("wm_load_weights: header field out of range");
+        return WM_ERR_FORMAT;
     }
     for (HostTensor& t : ts) {
         t.v.resize((size_t)t.rows * t.cols);
@@ -210,6 +232,7 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
     m.ln_eps = h.ln_eps;
     m.phi_kind = (int)phi_kind;
     m.phi_dim = phi_dim;
+    m.ranker_kind = (int)forest[0]; m.n_trees = (int)forest[1]; m.tree_depth = (int)forest[2];
 
     int rc = WM_OK;
     auto find = [&](const std::string& n) -> const HostTensor* {
@@ -231,6 +254,34 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         char nm[16];
         snprintf(nm, sizeof(nm), "Ws%d", i); up(nm, &m.Wst[i], true);
         snprintf(nm, sizeof(nm), "bs%d", i); up(nm, &m.bs[i], false);
+    }
+    if (rc == WM_OK && is_forest) {
+        // forest tensors: feature indices as int32 (validated against the feature count), thresholds, leaves, base
+        const HostTensor* tf = find("Tf");
+        std::vector<int32_t> fi(tf->v.size());
+        for (size_t i = 0; i < fi.size(); ++i) {
+            const float v = tf->v[i];
+            if (!(v >= 0.0f) || v >= (float)sdim[0] || v != (float)(int)v) {
+                set_error("wm_load_weights: forest feature index out of range");
+                rc = WM_ERR_FORMAT;
+                break;
+            }
+            fi[i] = (int32_t)v;
+        }
+        void* p = nullptr;
+        if (rc == WM_OK) {
+            if (cudaMalloc(&p, fi.size() * 4 + 16) != cudaSuccess ||
+                cudaMemcpy(p, fi.data(), fi.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+                set_error("wm_load_weights: cannot upload the forest");
+                rc = WM_ERR_CUDA;
+            } else {
+                ctx->allocs.push_back(p);
+                m.Tf = static_cast<int32_t*>(p);
+            }
+        }
+        up("Tt", &m.Tt, false); up("Tv", &m.Tv, false);
+        m.Tb = find("Tb")->v[0];
+        if (rc == WM_OK) rc = upload(ctx, std::vector<float>(1024, 0.0f), &m.zeros);
     }
     if (rc == WM_OK) {
         void* p = nullptr;
@@ -271,6 +322,7 @@ void wm_free(wm_ctx* ctx) {
         if (w->perm) cudaFree(w->perm);
         if (w->counters) cudaFree(w->counters);
         if (w->stage) cudaFree(w->stage);
+        if (w->zt) cudaFree(w->zt);
         if (w->ev0) cudaEventDestroy(w->ev0);
         if (w->ev1) cudaEventDestroy(w->ev1);
         delete w;
@@ -301,6 +353,7 @@ int wm_get_info(const wm_ctx* ctx, wm_info* o) {
     o->path = tc_supported(ctx) ? 2 : 1;
     o->tc_variant = tc_supported(ctx);
     o->phi_kind = m.phi_kind;
+    o->ranker_kind = m.ranker_kind; o->n_trees = m.n_trees; o->tree_depth = m.tree_depth;
     return WM_OK;
 }
 
@@ -403,7 +456,33 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
     a.init_states = init_states; a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
     a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets;
     a.B = B; a.S = S; a.T_max = T_max;
-    return run_rollout(ctx, a, static_cast<cudaStream_t>(cuda_stream), "wm_rollout_score");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (ctx->m.ranker_kind == WM_RANKER_FOREST) {
+        // tree-ensemble ranker: K2 rolls the candidates and hands the terminal latents [B, d] to K4, which builds
+        // [z_T ; structured phi ; h] per candidate and walks the trees
+        WM_CUDA_TRY(cudaSetDevice(ctx->device));
+        Workspace* ws = acquire_ws(ctx, st);
+        if (!ws) {
+            set_error("wm_rollout_score: cannot allocate workspace");
+            return WM_ERR_CUDA;
+        }
+        const size_t need = (size_t)B * ctx->m.d;
+        if (ws->zt_cap < need) {
+            if (ws->zt) {
+                WM_CUDA_TRY(cudaStreamSynchronize(st));
+                WM_CUDA_TRY(cudaFree(ws->zt));
+                ws->zt = nullptr;
+                ws->zt_cap = 0;
+            }
+            WM_CUDA_TRY(cudaMalloc(&ws->zt, (need + need / 4 + 1024) * sizeof(float)));
+            ws->zt_cap = need + need / 4 + 1024;
+        }
+        CallArgs r = a;
+        r.scores_out = nullptr; r.latents_out = ws->zt; r.latents_terminal = true;
+        const int rc = run_rollout(ctx, r, st, "wm_rollout_score");
+        return rc != WM_OK ? rc : launch_forest(ctx, ws->zt, a, scores_out, st);
+    }
+    return run_rollout(ctx, a, st, "wm_rollout_score");
 }
 
 int wm_rollout_latents(wm_ctx* ctx, const float* init_states, const int32_t* action_ids, const int32_t* action_params,
@@ -436,6 +515,10 @@ int wm_rollout_score_from(wm_ctx* ctx, const float* bank, const int32_t* bank_in
     }
     if (!sizes_ok("wm_rollout_score_from", B, S, T_max)) return WM_ERR_ARG;
     if (B == 0) return WM_OK;
+    if (ctx->m.ranker_kind == WM_RANKER_FOREST) {
+        set_error("wm_rollout_score_from: not built for the forest ranker");
+        return WM_ERR_UNSUPPORTED;
+    }
     if (!bank || !bank_index || !start || n_bank < 1 || !lengths || !scores_out || (ctx->m.H > 0 && !hw_feats) ||
         (T_max > 0 && (!action_ids || !action_params)) || !subgraph_offsets || S < 1) {
         set_error("wm_rollout_score_from: null pointer, n_bank < 1 or S < 1 for a non-empty batch");

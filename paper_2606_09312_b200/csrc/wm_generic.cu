@@ -373,8 +373,11 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
             if (a.latents_out) {   // z after this step, rows that took it: latents_out[cand][pos][:]
                 for (int e = tid; e < d * R; e += kGenericThreads) {
                     const int r = e / d, j = e % d;    // lanes over features: coalesced global store
-                    if (live_of(r))
+                    if (!live_of(r)) continue;
+                    if (!a.latents_terminal)
                         a.latents_out[((size_t)m_cand[r] * a.T_max + pos_of(r)) * d + j] = X[(size_t)j * R + r];
+                    else if (pos_of(r) == m_len[r] - 1)     // [B, d]: the terminal latent only
+                        a.latents_out[(size_t)m_cand[r] * d + j] = X[(size_t)j * R + r];
                 }
             }
         }

@@ -23,6 +23,12 @@ struct Model {
     int n_lin = 0;                       // linears of G
     int sdim[kMaxScorerLinears + 1] = {};  // sdim[0] = d+phi_dim+H, ..., sdim[n_lin] = 1
     float ln_eps = 1e-5f;
+    int ranker_kind = 0, n_trees = 0, tree_depth = 0;   // WM_RANKER_*; forest geometry
+    int32_t* Tf = nullptr;               // forest: [n_trees][2^depth - 1] feature index
+    float* Tt = nullptr;                 //         [n_trees][2^depth - 1] threshold
+    float* Tv = nullptr;                 //         [n_trees][2^depth] leaf value
+    float Tb = 0.0f;                     //         base score
+    float* zeros = nullptr;              // 1024 zero floats (dummy scorer vectors of the tcgen05 kernel for forest models)
     int phi_kind = 0;                    // WM_PHI_*
     int phi_dim = 0;                     // d_a (mean embedding) or n_types + 1 + 3P (structured), <= d_a
 
@@ -64,6 +70,9 @@ struct Workspace {
     // staging for wm_score_topk_host
     void* stage = nullptr;
     size_t stage_cap = 0;
+    // terminal latents [B, d] handed from K2 to the forest kernel (WM_RANKER_FOREST)
+    float* zt = nullptr;
+    size_t zt_cap = 0;
     // WM_OPT_TIMING
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool timed = false;
@@ -128,6 +137,7 @@ struct CallArgs {
     const int32_t* init_index;  // [B] row of init_states that holds candidate b's initial latent
     int64_t n_init;             // rows of init_states when init_index is used (indices are clamped to it)
     float* latents_out;         // [B, T_max, d] z after step t+1 at [b][t] for start <= t < len; scores_out may be null
+    bool latents_terminal;      // latents_out is [B, d]: only the latent after the LAST step (t = len - 1) is stored
 };
 
 // rollout steps of a candidate: its clamped length minus its clamped start (the single place that defines it)
@@ -161,6 +171,9 @@ int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 int tct_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
                 const std::vector<std::string>& names);
 int launch_tct(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
+
+// K4 (wm_forest.cu): tree-ensemble ranker over [z_T ; structured phi ; h] (NEXT row f4)
+int launch_forest(wm_ctx* ctx, const float* zT, const CallArgs& a, float* scores_out, cudaStream_t st);
 
 // K3 (wm_topk.cu)
 int64_t topk_launches();

@@ -528,9 +528,13 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
                 const float rstd = rsqrtf(var + p.ln_eps);
                 const bool live = t < rem;     // masked steps leave the state unchanged
-                float4* lat = (EXT && p.a.latents_out && live)     // wm_rollout_latents: z after this step, this row's half
-                                  ? reinterpret_cast<float4*>(p.a.latents_out + ((size_t)cand * p.a.T_max + st + t) * D)
-                                  : nullptr;
+                float4* lat = nullptr;     // wm_rollout_latents: z after this step (or only the terminal one: [B, d])
+                if (EXT && p.a.latents_out && live) {
+                    if (!p.a.latents_terminal)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + ((size_t)cand * p.a.T_max + st + t) * D);
+                    else if (st + t == len - 1)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + (size_t)cand * D);
+                }
 #pragma unroll 1
                 for (int p4 = 0; p4 < 4; ++p4) {
                     const int col0 = 128 * hh + 32 * p4;
@@ -852,8 +856,8 @@ struct TcState {
 
 static bool tc_model_ok(const Model& m) {
     return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc::D &&
-           m.d_a == tc::DA && m.hidden >= 256 && m.hidden <= tc::MAX_HID && m.hidden % 128 == 0 && m.n_lin == 3 &&
-           m.sdim[1] == tc::SW && m.sdim[2] == tc::SW && m.H >= 8 && m.H <= tc::MAX_H && m.H % 8 == 0 &&
+           m.d_a == tc::DA && m.hidden >= 256 && m.hidden <= tc::MAX_HID && m.hidden % 128 == 0 &&
+           ((m.n_lin == 3 && m.sdim[1] == tc::SW && m.sdim[2] == tc::SW) || m.ranker_kind == WM_RANKER_FOREST) && m.H >= 8 && m.H <= tc::MAX_H && m.H % 8 == 0 &&
            m.n_types <= tc::MAX_TYPES && m.P <= tc::MAX_P;
 }
 
@@ -897,8 +901,12 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     // phi weights of scorer layer 1 as the kernel's phi K-blocks see them, [SW][128].  WM_PHI_STRUCT: the F columns of
     // Ws0 as they are.  WM_PHI_MEAN: the mean action embedding is linear in psi = [count_c / len | sum log2 p_j / len | 1]
     // (see the action warps), so its weights are Ws0_phi E^T, Ws0_phi W_p and Ws0_phi b_p, summed in double here.
+    // Forest models (WM_RANKER_FOREST) run this kernel for the rollout only (terminal latents -> wm_forest_kernel): their
+    // scorer image is all zero and its result is never stored.
+    const bool forest = m.ranker_kind == WM_RANKER_FOREST;
     std::vector<float> Wphi((size_t)tc::SW * 128, 0.0f);
-    if (m.phi_kind == WM_PHI_STRUCT) {
+    if (forest) {
+    } else if (m.phi_kind == WM_PHI_STRUCT) {
         for (int n = 0; n < tc::SW; ++n)
             for (int c = 0; c < F; ++c) Wphi[(size_t)n * 128 + c] = Ws0[(size_t)n * K0 + tc::D + c];
     } else {
@@ -923,12 +931,12 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
         ok &= append_tile(blob, Wphi, 128, c * 128, 0, 64);
         ok &= append_tile(blob, Wphi, 128, c * 128, 64, 64);
-        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + F, m.H);
+        ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + F, forest ? 0 : m.H);
         ok &= append_tile(blob, Ws0, K0, c * 128, tc::D + F, 0);
-        for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
+        for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, forest ? 0 : 64);
     }
     for (int c = 0; c < 4; ++c)       // scorer layer 2
-        for (int kb = 0; kb < 8; ++kb) ok &= append_tile(blob, Ws1, tc::SW, c * 128, kb * 64, 64);
+        for (int kb = 0; kb < 8; ++kb) ok &= append_tile(blob, Ws1, tc::SW, c * 128, kb * 64, forest ? 0 : 64);
 
     if (!ok) return WM_OK;   // a weight beyond the fp16 range: this model stays on the fp32 kernel
 
@@ -988,6 +996,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.E = static_cast<const __nv_bfloat16*>(m.tc_E);
     p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
     p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
+    if (m.ranker_kind == WM_RANKER_FOREST) p.bs0 = p.bs1 = p.w3 = p.bs2 = m.zeros;   // (unused scorer, zero image)
     p.a = a;
     p.n_tiles = (int)((a.B + tc::TM - 1) / tc::TM);
     p.tile_counter = ws->counters + kTileCtrOff;

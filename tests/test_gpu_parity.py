@@ -528,3 +528,55 @@ def test_prefix_calls_argument_and_edge_cases(wm, n):
     assert wm.wm_check(ctx) == 0
     assert abs(float(one.item()) - float(lit[0])) <= 2e-5 * max(1.0, abs(float(lit[0])))
     wm.wm_free(ctx)
+
+
+@pytest.mark.parametrize("n", [10, 11])
+def test_forest_ranker_margin_aware(wm, n):
+    """NEXT row f4: the tree-ensemble ranker.  A branch decision is an integer taken from floating point, so parity is
+    split the way the decision forces: (i) the forest kernel alone — the GPU's own terminal latents pushed through the
+    oracle's forest must give the GPU's scores for every candidate whose path stays clear of a threshold by more than
+    fp32 rounding; (ii) end to end — every candidate whose oracle path margin exceeds the measured error of ITS terminal
+    latent cannot have flipped and must carry the oracle's score; the others are counted, not compared."""
+    import torch
+    cfg = gen.get_config(n).scaled(S=2, per_subgraph=200 if n == 11 else 64)
+    w = gen.make_weights(cfg)
+    b = gen.make_inputs(cfg)
+    kw = dict(n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps)
+    _, z_ref = oracle.rollout_score_vec(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.hw_feats,
+                                        b.subgraph_offsets, return_latent=True, phi_kind=cfg.phi_kind, **kw)
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    phi = np.stack([oracle.phi_struct(b.action_ids[i, :b.lengths[i]], b.action_params[i, :b.lengths[i]], cfg.n_types)
+                    for i in range(b.B)])
+    forest = (w["Tf"], w["Tt"], w["Tv"], w["Tb"])
+    y_ref, m_ref = oracle.forest_score(np.concatenate([z_ref, phi, b.hw_feats[seg]], axis=1), *forest, return_margin=True)
+    np.testing.assert_allclose(y_ref, oracle_scores(cfg, w, b), rtol=0, atol=1e-12)
+    dv = to_device(b)
+    for path in _paths(wm, cfg):
+        ctx = _ctx(wm, cfg, path)
+        info = wm.wm_get_info(ctx)
+        assert info.ranker_kind == 1 and info.n_trees == cfg.n_trees and info.tree_depth == cfg.tree_depth
+        y = gpu_scores(ctx, b)
+        np.testing.assert_array_equal(gpu_scores(ctx, b).view(np.uint32), y.view(np.uint32))     # deterministic
+        lat = torch.zeros((b.B, cfg.T_max, cfg.d), dtype=torch.float32, device="cuda:0")
+        wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"], lat,
+                              dv["subgraph_offsets"])
+        wm.wm_free(ctx)
+        lat = lat.cpu().numpy()
+        z_gpu = np.where((b.lengths > 0)[:, None], lat[np.arange(b.B), np.maximum(b.lengths - 1, 0)],
+                         b.init_states[seg]).astype(np.float64)
+        # (i) the forest kernel on the GPU's own latents
+        y_k4, m_k4 = oracle.forest_score(np.concatenate([z_gpu, phi, b.hw_feats[seg]], axis=1), *forest,
+                                         return_margin=True)
+        clear = m_k4 > 1e-4            # phi sums are fp32 on the GPU: up to ~3e-5 away from the float64 sums
+        assert clear.mean() > 0.9
+        np.testing.assert_allclose(y[clear], y_k4[clear], rtol=0, atol=2e-5)
+        # (ii) end to end against the oracle, where no decision can have flipped
+        dz = np.abs(z_gpu - z_ref).max(axis=1)
+        safe = m_ref > dz * 1.01 + 1e-4
+        tol_z = 1e-4 if cfg.dtype == DTYPE_FP32 else 2e-2
+        assert dz.max() <= tol_z * max(1.0, np.abs(z_ref).max())
+        assert safe.mean() > (0.9 if path == wm.PATH_FP32 or cfg.dtype == DTYPE_FP32 else 0.3), safe.mean()
+        np.testing.assert_allclose(y[safe], y_ref[safe], rtol=0, atol=2e-5)
+        # ranking quality on the whole batch: the top-k of the two score vectors still overlap
+        ov, _ = oracle.topk_overlap(gpu_topk(y, b.subgraph_offsets, cfg.k), oracle.topk_segments(y_ref, b.subgraph_offsets, cfg.k))
+        assert ov >= (0.95 if cfg.dtype == DTYPE_FP32 else 0.8), ov
