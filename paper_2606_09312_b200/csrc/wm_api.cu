@@ -257,29 +257,30 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
     }
     if (rc == WM_OK && is_forest) {
         // forest tensors: feature indices as int32 (validated against the feature count), thresholds, leaves, base
-        const HostTensor* tf = find("Tf");
-        std::vector<int32_t> fi(tf->v.size());
-        for (size_t i = 0; i < fi.size(); ++i) {
+        const HostTensor *tf = find("Tf"), *tt = find("Tt");
+        std::vector<int2> nodes(tf->v.size());
+        for (size_t i = 0; i < nodes.size(); ++i) {
             const float v = tf->v[i];
             if (!(v >= 0.0f) || v >= (float)sdim[0] || v != (float)(int)v) {
                 set_error("wm_load_weights: forest feature index out of range");
                 rc = WM_ERR_FORMAT;
                 break;
             }
-            fi[i] = (int32_t)v;
+            nodes[i].x = (int)v;
+            memcpy(&nodes[i].y, &tt->v[i], 4);
         }
         void* p = nullptr;
         if (rc == WM_OK) {
-            if (cudaMalloc(&p, fi.size() * 4 + 16) != cudaSuccess ||
-                cudaMemcpy(p, fi.data(), fi.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+            if (cudaMalloc(&p, nodes.size() * sizeof(int2) + 16) != cudaSuccess ||
+                cudaMemcpy(p, nodes.data(), nodes.size() * sizeof(int2), cudaMemcpyHostToDevice) != cudaSuccess) {
                 set_error("wm_load_weights: cannot upload the forest");
                 rc = WM_ERR_CUDA;
             } else {
                 ctx->allocs.push_back(p);
-                m.Tf = static_cast<int32_t*>(p);
+                m.Tnode = static_cast<int2*>(p);
             }
         }
-        up("Tt", &m.Tt, false); up("Tv", &m.Tv, false);
+        up("Tv", &m.Tv, false);
         m.Tb = find("Tb")->v[0];
         if (rc == WM_OK) rc = upload(ctx, std::vector<float>(1024, 0.0f), &m.zeros);
     }

@@ -26,8 +26,8 @@ struct ForestParams {
     float* scores;
     int64_t B;
     int S, T_max, d, n_types, P, H, n_in, n_trees, nodes, depth;
-    const int32_t* Tf;
-    const float *Tt, *Tv;
+    const int2* Tnode;          // {feature index, threshold bits} per internal node
+    const float* Tv;
     float Tb;
 };
 
@@ -93,13 +93,22 @@ __global__ void __launch_bounds__(kForestWarps * 32) wm_forest_kernel(const Fore
         }
         __syncwarp();
         // the trees
+        // the trees: a walk is `depth` dependent (node load, feature read) pairs, so a lane walks four trees at once
         float acc = 0.0f;
-        for (int t = lane; t < p.n_trees; t += 32) {
-            const int32_t* tf = p.Tf + (size_t)t * p.nodes;
-            const float* tt = p.Tt + (size_t)t * p.nodes;
-            int node = 0;
-            for (int l = 0; l < p.depth; ++l) node = 2 * node + (x[__ldg(tf + node)] < __ldg(tt + node) ? 1 : 2);
-            acc += __ldg(p.Tv + (size_t)t * (p.nodes + 1) + (node - p.nodes));
+        for (int t0 = lane; t0 < p.n_trees; t0 += 128) {
+            int node[4] = {0, 0, 0, 0};
+            for (int l = 0; l < p.depth; ++l) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int t = t0 + 32 * u < p.n_trees ? t0 + 32 * u : t0;      // (in-bounds dummy past the last tree)
+                    const int2 nd = __ldg(p.Tnode + (size_t)t * p.nodes + node[u]);
+                    node[u] = 2 * node[u] + (x[nd.x] < __int_as_float(nd.y) ? 1 : 2);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (t0 + 32 * u < p.n_trees)
+                    acc += __ldg(p.Tv + (size_t)(t0 + 32 * u) * (p.nodes + 1) + (node[u] - p.nodes));
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -117,7 +126,7 @@ int launch_forest(wm_ctx* ctx, const float* zT, const CallArgs& a, float* scores
     p.offsets = a.offsets; p.hw = a.hw_feats; p.scores = scores_out;
     p.B = a.B; p.S = a.S; p.T_max = a.T_max; p.d = m.d; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.n_in = m.sdim[0]; p.n_trees = m.n_trees; p.depth = m.tree_depth; p.nodes = (1 << m.tree_depth) - 1;
-    p.Tf = m.Tf; p.Tt = m.Tt; p.Tv = m.Tv; p.Tb = m.Tb;
+    p.Tnode = m.Tnode; p.Tv = m.Tv; p.Tb = m.Tb;
     const size_t smem = (size_t)kForestWarps * p.n_in * sizeof(float);
     if (smem > (size_t)ctx->smem_optin) {
         set_error("forest ranker: feature vector too wide for shared memory");

@@ -24,8 +24,8 @@ struct Model {
     int sdim[kMaxScorerLinears + 1] = {};  // sdim[0] = d+phi_dim+H, ..., sdim[n_lin] = 1
     float ln_eps = 1e-5f;
     int ranker_kind = 0, n_trees = 0, tree_depth = 0;   // WM_RANKER_*; forest geometry
-    int32_t* Tf = nullptr;               // forest: [n_trees][2^depth - 1] feature index
-    float* Tt = nullptr;                 //         [n_trees][2^depth - 1] threshold
+    int2* Tnode = nullptr;               // forest: [n_trees][2^depth - 1] {feature index, threshold bits}: one 8-byte
+                                         //         load per level of a walk
     float* Tv = nullptr;                 //         [n_trees][2^depth] leaf value
     float Tb = 0.0f;                     //         base score
     float* zeros = nullptr;              // 1024 zero floats (dummy scorer vectors of the tcgen05 kernel for forest models)

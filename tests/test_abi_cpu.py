@@ -107,11 +107,35 @@ def test_load_weights_io_and_format_errors(tmp_path):
     with pytest.raises(wm.WmError) as e:
         wm.wm_load_weights(str(tmp_path / "wide.wmw"))
     assert e.value.code == wm.WM_ERR_UNSUPPORTED and "d_a" in str(e.value)
-    struct.pack_into("<I", raw2, 4, 3)          # version 3 does not exist
-    (tmp_path / "v3.wmw").write_bytes(bytes(raw2))
+    struct.pack_into("<I", raw2, 4, 4)          # version 4 does not exist
+    (tmp_path / "v4.wmw").write_bytes(bytes(raw2))
     with pytest.raises(wm.WmError) as e:
-        wm.wm_load_weights(str(tmp_path / "v3.wmw"))
+        wm.wm_load_weights(str(tmp_path / "v4.wmw"))
     assert e.value.code == wm.WM_ERR_FORMAT
+    # version 3 (forest ranker, NEXT row f4): bad tree depth, a feature index past the feature vector, forest + mean phi
+    cfg10 = gen.get_config(10)
+    w10 = gen.make_weights(cfg10)
+    v3 = tmp_path / "v3.wmw"
+    gen.write_weight_file(str(v3), cfg10, w10)
+    raw3 = bytearray(v3.read_bytes())
+    assert struct.unpack_from("<I", raw3, 4)[0] == 3 and struct.unpack_from("<3I", raw3, 84) == (1, 32, 4)
+    struct.pack_into("<I", raw3, 92, 13)
+    (tmp_path / "deep.wmw").write_bytes(bytes(raw3))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "deep.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT and "ranker" in str(e.value)
+    wbad = dict(w10); wbad["Tf"] = w10["Tf"].copy(); wbad["Tf"][3, 2] = cfg10.scorer_in
+    gen.write_weight_file(str(tmp_path / "feat.wmw"), cfg10, wbad)
+    try:
+        wm.wm_load_weights(str(tmp_path / "feat.wmw"))
+        raise AssertionError("a feature index past the feature vector was accepted")
+    except wm.WmError as e2:      # FORMAT when the check is reached; CUDA when no device is there to load onto
+        assert e2.code in (wm.WM_ERR_FORMAT, wm.WM_ERR_CUDA)
+    mean_forest = replace(cfg10, phi_kind=0)
+    gen.write_weight_file(str(tmp_path / "meanforest.wmw"), mean_forest, gen.make_weights(mean_forest))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "meanforest.wmw"))
+    assert e.value.code == wm.WM_ERR_UNSUPPORTED
 
 
 def test_no_product_import_of_oracle():
