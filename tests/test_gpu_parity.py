@@ -262,7 +262,7 @@ def test_full_size_sampled(wm, n):
     np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9, 10, 11])
 def test_outputs_do_not_overrun(wm, n):
     """compute-sanitizer is closed on this pool: canaries instead.  The score and index buffers are sub-ranges of
     larger allocations filled with sentinels; everything outside [0, B) / [0, S*k) must come back untouched, and a
@@ -292,7 +292,7 @@ def test_outputs_do_not_overrun(wm, n):
         assert (hi[:pad] == -77).all() and (hi[pad + S * k:] == -77).all(), (n, path)
 
 
-@pytest.mark.parametrize("n", [2, 3, 5, 7, 9])
+@pytest.mark.parametrize("n", [2, 3, 5, 7, 9, 11])
 def test_repeatable_bitwise_with_several_tiles_per_cta(wm, n):
     """A batch large enough that every persistent CTA (or CTA pair) walks several tiles, scored three times: the
     scores must be bit-identical.  Barrier phase counters that do not survive a tile boundary, or a wait that passes
