@@ -188,6 +188,9 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem + L.tmem_slot);
+    // EXT calls that store latents and rank nothing (wm_rollout_latents; the rollout half of a forest-ranker model) skip
+    // the scorer in every role: no scorer tiles streamed, no scorer MMAs, no phi / hw operand, no score
+    const bool rank = !EXT || p.a.scores_out != nullptr;
     const uint32_t T_Z = tmem_base;                 // fp32 latent / GEMM2 accumulator, 256 columns
     const uint32_t T_D1 = tmem_base + 256;          // two 128-column GEMM1 accumulators
 
@@ -220,7 +223,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             if (tile < 0) break;
             if (lane == 0) {
                 // the stream is consumed in pairs of tiles that are adjacent in the image: one 32 KB copy per stage
-                const int roll_total = nsteps * ROLL_TILES, total = roll_total + SC_TILES;
+                const int roll_total = nsteps * ROLL_TILES, total = roll_total + (rank ? SC_TILES : 0);
                 for (int i = 0; i < total; i += 2) {
                     const int src_tile = i < roll_total ? i % ROLL_TILES : ROLL_TILES + (i - roll_total);
                     mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
@@ -380,6 +383,11 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                         if (i < NC) gemm_a1(i & 1, false, i == NC - 1, false);   // GEMM1 chunk i
                         gemm2(i - 1);
                     }
+                }
+                if (!rank) {   // nothing to rank: only take the terminal latent's ZREADY so the phase count stays in step
+                    mbar_wait(bar(B_ZREADY), n_z & 1);
+                    ++n_z;
+                    continue;
                 }
                 // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
 #pragma unroll 1
@@ -570,6 +578,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                 publish(B_ZREADY, true);
             }
 
+            if (!rank) continue;
             // ---- scorer layer 1 -> H1 (fp16) in TMEM columns [0,256)
             for (int c = 0; c < 4; ++c)
                 gelu_chunk(c & 1, p.bs0 + c * 128 + 64 * hh, false, T_Z + 64u * c + 32u * hh);
@@ -762,6 +771,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             //                  psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) | 1 (len > 0)], so the host folds
             //                  E, W_p and b_p into scorer layer 1's phi weights (tc_prepare) and the kernel only writes psi
             //   WM_PHI_STRUCT  phi = [count_c (NT) | len | sum_j (P) | mean_j (P) | max_j (P)]   (S25)
+            if (!rank) continue;
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
             {
