@@ -148,6 +148,8 @@ int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value);
  *                     NULL selects per-candidate mode and S is ignored
  *   B, S, T_max       sizes; B = 0 is a no-op.  P, d, H come from the weight file.
  *   cuda_stream       stream to enqueue on
+ * WM_RANKER_FOREST models: the rollout stores the terminal latents in a ctx-owned [B, d] buffer and a second kernel
+ * ranks [z_T ; phi ; h] with the tree ensemble (two launches instead of one; same arguments, same output).
  * Errors: WM_ERR_ARG (null pointer with B > 0, B < 0, S < 0, T_max < 0 or > WM_MAX_T), WM_ERR_CUDA. */
 int wm_rollout_score(wm_ctx* ctx,
                      const float* init_states, const int32_t* action_ids, const int32_t* action_params,
@@ -172,7 +174,10 @@ int wm_rollout_score(wm_ctx* ctx,
  * The score equals wm_rollout_score's for the same candidate (to the rounding of the stored fp32 latent: the
  * tcgen05 kernels keep the latent in fp32 between steps, so a bank written by wm_rollout_latents reproduces them).
  * Candidates are bucketed by their remaining steps lengths[b] - start[b].
- * Errors: as wm_rollout_score; WM_ERR_ARG also for a null bank / bank_index / start / latents_out or n_bank < 1. */
+ * Errors: as wm_rollout_score; WM_ERR_ARG also for a null bank / bank_index / start / latents_out or n_bank < 1;
+ * WM_ERR_UNSUPPORTED for wm_rollout_score_from on a WM_RANKER_FOREST model, and when the tcgen05 path is forced
+ * (WM_OPT_PATH = 2) on a model whose tcgen05 kernel does not take these calls (only the d = 256 MLP+LayerNorm kernel does;
+ * under the automatic policy the other models run them on the fp32 kernel). */
 int wm_rollout_latents(wm_ctx* ctx,
                        const float* init_states, const int32_t* action_ids, const int32_t* action_params,
                        const int32_t* lengths, const int32_t* subgraph_offsets, float* latents_out,
