@@ -214,12 +214,12 @@ def test_two_streams_share_one_ctx(wm):
     wm.wm_free(ctx)
 
 
-@pytest.mark.parametrize("S,per", [(3, 200), (4, 1100), (7, 900)])
-def test_host_entry_matches_device_entry(wm, S, per):
+@pytest.mark.parametrize("n,S,per", [(2, 3, 200), (2, 4, 1100), (2, 7, 900), (11, 6, 900), (5, 5, 700)])
+def test_host_entry_matches_device_entry(wm, n, S, per):
     """wm_score_topk_host (host buffers; pipelined by chunks of whole subgraphs, here forced small through
     WM_HOST_CHUNK_MIN in conftest.py) returns bit-identical scores and indices to the device-pointer entry points."""
     import torch
-    cfg = gen.get_config(2).scaled(S=S, per_subgraph=per)
+    cfg = gen.get_config(n).scaled(S=S, per_subgraph=per)      # 11: forest ranker (two kernels per chunk); 5: pair kernel
     b = gen.make_inputs(cfg)
     ctx = _ctx(wm, cfg)
     y = gpu_scores(ctx, b)
