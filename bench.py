@@ -396,7 +396,7 @@ def main():
     ap.add_argument("--prefix-reuse", action="store_true",
                     help="config 4: also time the prefix-latent-reuse calls (extra 'prefix_reuse' object in the JSON line)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]; 6, 7 = NEXT row f1 (TransH transition); 8, 9 = NEXT row f2 (structured phi); 10, 11 = NEXT row f4 (forest ranker)")
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]; 6, 7 = NEXT row f1 (TransH transition); 8, 9 = NEXT row f2 (structured phi); 10, 11 = NEXT row f4 (forest ranker); 12 = TransH + structured phi + forest")
     args = ap.parse_args()
     cfg = gen.get_config(args.config)
     if args.impl == "reference":

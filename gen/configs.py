@@ -132,6 +132,12 @@ CONFIGS = {
                  T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
                  param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(), k=64,
                  phi_kind=PHI_STRUCT, ranker_kind=RANKER_FOREST, n_trees=128, tree_depth=6),
+    # The paper's own choice for every component at once (not a BASELINE.json config): TransH-style transition (f1),
+    # structured phi (f2), tree-ensemble ranker (f4), on cfg 2's shapes and batch.
+    12: WMConfig("paper_stack_evolution_round", 12, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, S=16, per_subgraph=2048,
+                 T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
+                 param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(), k=64,
+                 phi_kind=PHI_STRUCT, ranker_kind=RANKER_FOREST, n_trees=128, tree_depth=6),
 }
 
 

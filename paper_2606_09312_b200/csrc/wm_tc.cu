@@ -985,9 +985,11 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     // per-call conditions the kernel relies on; otherwise the fp32 kernel takes the call
     const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0);
     const bool prefix_call = a.start || a.init_index || a.latents_out;   // wm_rollout_latents / wm_rollout_score_from
-    // the prefix-reuse calls are built into wm_tc_kernel only; the other models take the fp32 kernel for them
-    if (prefix_call && m.tc_ok != 1 && ctx->opt_path != 2) return launch_generic(ctx, a, st);
-    if (!m.tc_ok || a.T_max > 255 || !aligned || (prefix_call && m.tc_ok != 1)) {
+    // the prefix-reuse calls are built into wm_tc_kernel only (the other models take the fp32 kernel for them); the
+    // TransH kernel has the latents-out piece (wm_rollout_latents; the rollout half of a forest-ranker model)
+    const bool ext_ok = m.tc_ok == 1 || (m.tc_ok == 4 && a.latents_out && !a.scores_out && !a.start && !a.init_index);
+    if (prefix_call && !ext_ok && ctx->opt_path != 2) return launch_generic(ctx, a, st);
+    if (!m.tc_ok || a.T_max > 255 || !aligned || (prefix_call && !ext_ok)) {
         if (ctx->opt_path == 2) {
             set_error("tcgen05 path: needs T_max <= 255, 16-byte aligned init_states / hw_feats (and, for "
                       "wm_rollout_latents / wm_rollout_score_from, a d = 256 MLP+LayerNorm model)");

@@ -124,6 +124,9 @@ using namespace ptx;
 
 namespace tct {
 
+// LAT = true: the rollout half of a forest-ranker model (NEXT row f4): every row's terminal latent is stored to
+// latents_out [B, d] and nothing is ranked — no scorer tiles streamed, no scorer MMAs, no phi / hw operand, no score.
+template <bool LAT>
 __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps);
@@ -207,7 +210,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                 // the stream is consumed in pairs of tiles that are adjacent in the image: one 32 KB copy per stage
                 // stream of a tile: [W_w for step 0 (= the last 4 tiles of the step image)] nsteps x [step image] [scorer]
                 const int pre = nsteps > 0 ? 4 : 0;
-                const int roll_total = nsteps * ROLL_TILES, total = pre + roll_total + SC_TILES;
+                const int roll_total = nsteps * ROLL_TILES, total = pre + roll_total + (LAT ? 0 : SC_TILES);
                 for (int i = 0; i < total; i += 2) {
                     const int j = i - pre;
                     const int src_tile = j < 0 ? ROLL_TILES - 4 + i : j < roll_total ? j % ROLL_TILES : ROLL_TILES + (j - roll_total);
@@ -388,6 +391,11 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                         }
                     }
                 }
+                if (LAT) {     // nothing to rank: only take the terminal latent's ZREADY so the phase count stays in step
+                    mbar_wait(bar(B_ZREADY), n_z & 1);
+                    ++n_z;
+                    continue;
+                }
                 // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
 #pragma unroll 1
                 for (int c = 0; c < 4; ++c) {
@@ -554,6 +562,16 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                     const int col0 = 128 * hh + 32 * p4;
                     uint32_t v[32];
                     load_src(from_z0, col0, v);
+                    // latents out (LAT): z' = v rn of the step this row has just taken, BEFORE it is projected for the
+                    // next action — every step (wm_rollout_latents) or the row's last one only (forest ranker)
+                    if (LAT && cand >= 0 && !from_z0 && (p.a.latents_terminal ? t == len - 1 : t < len)) {
+                        float4* lat = reinterpret_cast<float4*>(
+                            p.a.latents_out + (p.a.latents_terminal ? (size_t)cand : (size_t)cand * p.a.T_max + t) * D + col0);
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+                            lat[i] = make_float4(__uint_as_float(v[4 * i]) * rn, __uint_as_float(v[4 * i + 1]) * rn,
+                                                 __uint_as_float(v[4 * i + 2]) * rn, __uint_as_float(v[4 * i + 3]) * rn);
+                    }
                     if (has_next) {
                         uint32_t u[32];
                         tmem_ld32(T_D1 + lane_off + (uint32_t)col0, u);
@@ -591,6 +609,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
                 boundary(t);
             }
 
+            if (LAT) continue;
             // ---- scorer layer 1 -> H1 (fp16) in TMEM columns [0,256)
             for (int c = 0; c < 4; ++c)
                 gelu_chunk(c & 1, p.bs0 + c * 128 + 64 * hh, false, T_Z + 64u * c + 32u * hh);
@@ -734,6 +753,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
             // W_p sum_t log2 p_t) / len + b_p is LINEAR in psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) |
             // 1 (len > 0)]: the host folds E, W_p and b_p into scorer layer 1's phi weights (tct_prepare) and the kernel
             // only writes psi (clear the row's two K-blocks, then one 16-bit store per feature).
+            if (LAT) continue;
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
             {
@@ -813,9 +833,12 @@ struct TcState {
 }  // namespace
 
 static bool tct_model_ok(const Model& m) {
-    return m.kind == WM_KIND_TRANSH && m.phi_kind == WM_PHI_MEAN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tct::D &&
-           m.d_a == tct::DA && m.hidden >= 256 && m.hidden <= tct::MAX_HID && m.hidden % 128 == 0 && m.n_lin == 3 &&
-           m.sdim[1] == tct::SW && m.sdim[2] == tct::SW && m.H >= 8 && m.H <= tct::MAX_H && m.H % 8 == 0 &&
+    // MLP-ranked models with the mean-embedding phi; forest-ranked models (any phi: the kernel only rolls them)
+    const bool ranker_ok = m.ranker_kind == WM_RANKER_FOREST ||
+                           (m.phi_kind == WM_PHI_MEAN && m.n_lin == 3 && m.sdim[1] == tct::SW && m.sdim[2] == tct::SW);
+    return m.kind == WM_KIND_TRANSH && ranker_ok && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR &&
+           m.d == tct::D && m.d_a == tct::DA && m.hidden >= 256 && m.hidden <= tct::MAX_HID && m.hidden % 128 == 0 &&
+           m.H >= 8 && m.H <= tct::MAX_H && m.H % 8 == 0 &&
            m.n_types <= tct::MAX_TYPES && m.P <= tct::MAX_P;
 }
 
@@ -867,8 +890,9 @@ int tct_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     a_gemm(Ww);
     // phi weights of scorer layer 1 folded onto psi = [count_c / len | sum log2 p_j / len | 1] (see the action warps):
     // Ws0_phi E^T, Ws0_phi W_p, Ws0_phi b_p, summed in double
+    const bool forest = m.ranker_kind == WM_RANKER_FOREST;   // scorer image all zero and never streamed (LAT instance)
     std::vector<float> Wphi((size_t)tct::SW * 128, 0.0f);
-    {
+    if (!forest) {
         const std::vector<float>&Wp = get("W_p"), &bpv = get("b_p");
         for (int n = 0; n < tct::SW; ++n) {
             const float* wr = &Ws0[(size_t)n * K0 + tct::D];
@@ -890,12 +914,12 @@ int tct_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2), hw + an all-zero padding tile, z (4)
         ok &= append_tile(blob, Wphi, 128, c * 128, 0, 64);
         ok &= append_tile(blob, Wphi, 128, c * 128, 64, 64);
-        ok &= append_tile(blob, Ws0, K0, c * 128, K1, m.H);
+        ok &= append_tile(blob, Ws0, K0, c * 128, K1, forest ? 0 : m.H);
         ok &= append_tile(blob, Ws0, K0, c * 128, K1, 0);
-        for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, 64);
+        for (int kb = 0; kb < 4; ++kb) ok &= append_tile(blob, Ws0, K0, c * 128, kb * 64, forest ? 0 : 64);
     }
     for (int c = 0; c < 4; ++c)       // scorer layer 2
-        for (int kb = 0; kb < 8; ++kb) ok &= append_tile(blob, Ws1, tct::SW, c * 128, kb * 64, 64);
+        for (int kb = 0; kb < 8; ++kb) ok &= append_tile(blob, Ws1, tct::SW, c * 128, kb * 64, forest ? 0 : 64);
 
     if (!ok) return WM_OK;   // a weight beyond the fp16 range: this model stays on the fp32 kernel
 
@@ -912,7 +936,8 @@ int tct_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     m.tc_blob = d_blob;
     m.tc_blob_bytes = blob.size() * 2;
     m.tc_E = d_e;
-    WM_CUDA_TRY(cudaFuncSetAttribute(tct::wm_tct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    WM_CUDA_TRY(cudaFuncSetAttribute(tct::wm_tct_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    WM_CUDA_TRY(cudaFuncSetAttribute(tct::wm_tct_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
     m.tc_ok = 4;
     return WM_OK;
 }
@@ -934,7 +959,8 @@ int launch_tct(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.prof = nullptr;
     const tct::SmemLayout L = tct::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
     const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
-    tct::wm_tct_kernel<<<grid, tct::THREADS, L.total, st>>>(p);
+    if (a.latents_out) tct::wm_tct_kernel<true><<<grid, tct::THREADS, L.total, st>>>(p);    // terminal latents only
+    else tct::wm_tct_kernel<false><<<grid, tct::THREADS, L.total, st>>>(p);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
     return WM_OK;

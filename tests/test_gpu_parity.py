@@ -262,7 +262,7 @@ def test_full_size_sampled(wm, n):
     np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9, 10, 11])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9, 10, 11, 12])
 def test_outputs_do_not_overrun(wm, n):
     """compute-sanitizer is closed on this pool: canaries instead.  The score and index buffers are sub-ranges of
     larger allocations filled with sentinels; everything outside [0, B) / [0, S*k) must come back untouched, and a
@@ -292,7 +292,7 @@ def test_outputs_do_not_overrun(wm, n):
         assert (hi[:pad] == -77).all() and (hi[pad + S * k:] == -77).all(), (n, path)
 
 
-@pytest.mark.parametrize("n", [2, 3, 5, 7, 9, 11])
+@pytest.mark.parametrize("n", [2, 3, 5, 7, 9, 11, 12])
 def test_repeatable_bitwise_with_several_tiles_per_cta(wm, n):
     """A batch large enough that every persistent CTA (or CTA pair) walks several tiles, scored three times: the
     scores must be bit-identical.  Barrier phase counters that do not survive a tile boundary, or a wait that passes
@@ -337,7 +337,7 @@ def test_struct_phi_feature_readout(wm, n):
             np.testing.assert_array_equal(y, b.hw_feats[seg, 0])
 
 
-PREFIX_TC_VARIANTS = (1,)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
+PREFIX_TC_VARIANTS = (1,)       # (the TransH kernel, variant 4, takes wm_rollout_latents only)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
 
 
 def _prefix_case(n, S, per):
@@ -345,9 +345,9 @@ def _prefix_case(n, S, per):
     return cfg, gen.make_weights(cfg), gen.make_inputs(cfg)
 
 
-def _prefix_unsupported(wm, ctx, path, call):
+def _prefix_unsupported(wm, ctx, path, call, variants=None):
     """True (after checking the error code) when `path` is a forced tcgen05 kernel without prefix-reuse support."""
-    if path != wm.PATH_TCGEN05 or wm.wm_get_info(ctx).tc_variant in PREFIX_TC_VARIANTS:
+    if path != wm.PATH_TCGEN05 or wm.wm_get_info(ctx).tc_variant in (variants or PREFIX_TC_VARIANTS):
         return False
     with pytest.raises(wm.WmError) as e:
         call()
@@ -356,7 +356,7 @@ def _prefix_unsupported(wm, ctx, path, call):
     return True
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 9])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 9])
 def test_rollout_latents_match_oracle(wm, n):
     """NEXT row f3: wm_rollout_latents against oracle.rollout_latents, every stored latent; entries past a candidate's
     length keep the caller's bytes."""
@@ -371,7 +371,7 @@ def test_rollout_latents_match_oracle(wm, n):
         out = torch.full((b.B, cfg.T_max, cfg.d), -777.0, dtype=torch.float32, device="cuda:0")
         call = lambda: wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"],
                                              dv["lengths"], out, dv["subgraph_offsets"])
-        if _prefix_unsupported(wm, ctx, path, call):
+        if _prefix_unsupported(wm, ctx, path, call, variants=(1, 4)):
             continue
         call()
         assert wm.wm_check(ctx) == 0
@@ -530,7 +530,7 @@ def test_prefix_calls_argument_and_edge_cases(wm, n):
     wm.wm_free(ctx)
 
 
-@pytest.mark.parametrize("n", [10, 11])
+@pytest.mark.parametrize("n", [10, 11, 12])
 def test_forest_ranker_margin_aware(wm, n):
     """NEXT row f4: the tree-ensemble ranker.  A branch decision is an integer taken from floating point, so parity is
     split the way the decision forces: (i) the forest kernel alone — the GPU's own terminal latents pushed through the
@@ -538,7 +538,7 @@ def test_forest_ranker_margin_aware(wm, n):
     fp32 rounding; (ii) end to end — every candidate whose oracle path margin exceeds the measured error of ITS terminal
     latent cannot have flipped and must carry the oracle's score; the others are counted, not compared."""
     import torch
-    cfg = gen.get_config(n).scaled(S=2, per_subgraph=200 if n == 11 else 64)
+    cfg = gen.get_config(n).scaled(S=2, per_subgraph=64 if n == 10 else 200)
     w = gen.make_weights(cfg)
     b = gen.make_inputs(cfg)
     kw = dict(n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps)
