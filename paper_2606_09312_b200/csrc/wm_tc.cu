@@ -101,7 +101,7 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
     L.b2 = o; o += D * 4;
     L.gamma = o; o += D * 4;
     L.beta = o; o += D * 4;
-    L.red = o; o += 2 * TM * 8;
+    L.red = o; o += 4 * TM * 8;                        // [2 (LayerNorm parity)][2 column halves][128 rows] float2
     L.bars = o; o += B_COUNT * 8;
     L.sched = o; o += 2 * 8;
     L.tmem_slot = o; o += 16;
@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
     float* s_b2 = reinterpret_cast<float*>(smem + L.b2);
     float* s_gamma = reinterpret_cast<float*>(smem + L.gamma);
     float* s_beta = reinterpret_cast<float*>(smem + L.beta);
-    float2* s_red = reinterpret_cast<float2*>(smem + L.red);                  // [2][128]
+    float2* s_red = reinterpret_cast<float2*>(smem + L.red);                  // [2][2][128]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int NC = p.nc;
@@ -529,9 +529,12 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
                     }
                 }
                 const float s1 = s1v.x + s1v.y, s2 = s2v.x + s2v.y;
-                s_red[hh * TM + row] = make_float2(s1, s2);
+                // exchanged through the slot of this LayerNorm's parity: the partner reads the previous LayerNorm's value
+                // from the other slot, so no second barrier is needed before the next one writes
+                float2* red = s_red + (n_d2 & 1u) * 2 * TM;
+                red[hh * TM + row] = make_float2(s1, s2);
                 named_bar_sync(1 + q, 64);
-                const float2 other = s_red[(hh ^ 1) * TM + row];
+                const float2 other = red[(hh ^ 1) * TM + row];
                 const float mean = (s1 + other.x) * inv_d;
                 const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
                 const float rstd = rsqrtf(var + p.ln_eps);
