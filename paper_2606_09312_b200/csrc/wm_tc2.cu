@@ -541,6 +541,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     const float2 o = s_red[k * TMR + row];
                     s1 += o.x; s2 += o.y;
                 }
+                named_bar_sync(1 + rh, 128);   // all four parts have read s_red before the next LayerNorm rewrites it
                 const float mean = s1 * inv_d;
                 const float var = fmaxf(s2 * inv_d - mean * mean, 0.0f);
                 const float rstd = rsqrtf(var + p.ln_eps);
