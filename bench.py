@@ -48,7 +48,7 @@ def _kernel_name(info) -> str:
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*.md); keyed by (config number, kernel).  None where no capture exists yet.
 NCU_TRAFFIC = {
-    (2, "wm_tc_kernel"): (23_906_560 + 2_816, "profiles/r1_tc_v7.md"),
+    (2, "wm_tc_kernel"): (23_906_304 + 2_048, "profiles/r1_tc_v8.md"),
     (3, "wm_tc2_kernel"): (56_585_216 + 761_856, "profiles/r1_tc2_v4.md"),
     (5, "wm_tcg_kernel"): (3_450_484_000 + 61_085_952, "profiles/r1_tcg_v1.md"),
     (7, "wm_tct_kernel"): (24_100_608 + 2_048, "profiles/r1_tct_v1.md"),
