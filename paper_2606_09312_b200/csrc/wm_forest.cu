@@ -69,25 +69,28 @@ __global__ void __launch_bounds__(kForestWarps * 32) wm_forest_kernel(const Fore
             for (int j = 0; j < kMaxP; ++j)
                 if (j < P) {
                     const int prm = __ldg(pp + j);
-                    const float l2 = log2f((float)(prm < 1 ? 1 : prm));
+                    // MUFU.LG2 (2 ulp): the features feed comparisons whose margins the parity test accounts for
+                    const float l2 = __log2f((float)(prm < 1 ? 1 : prm));
                     sum[j] += l2;
                     mx[j] = fmaxf(mx[j], l2);
                 }
         }
 #pragma unroll
         for (int j = 0; j < kMaxP; ++j)
+            if (j < P) {      // (warp-uniform)
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                sum[j] += __shfl_xor_sync(0xffffffffu, sum[j], o);
-                mx[j] = fmaxf(mx[j], __shfl_xor_sync(0xffffffffu, mx[j], o));
+                for (int o = 16; o > 0; o >>= 1) sum[j] += __shfl_xor_sync(0xffffffffu, sum[j], o);
+                // log2 p >= 0: the float order is the order of the bit patterns, one redux instruction
+                mx[j] = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(mx[j])));
             }
         if (lane == 0) {
+            const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
             phi[NT] = (float)len;
 #pragma unroll
             for (int j = 0; j < kMaxP; ++j)
                 if (j < P) {
                     phi[NT + 1 + j] = sum[j];
-                    phi[NT + 1 + P + j] = len > 0 ? sum[j] / (float)len : 0.0f;
+                    phi[NT + 1 + P + j] = sum[j] * inv;
                     phi[NT + 1 + 2 * P + j] = mx[j];
                 }
         }
