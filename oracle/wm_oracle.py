@@ -83,11 +83,14 @@ def embed_bucket(ids: np.ndarray, params: np.ndarray, Tbl, P: int, n_buckets: in
 
 
 def _bucket_vec(p: np.ndarray, n_buckets: int) -> np.ndarray:
-    """Vectorised bucket_index: p^4 < 2^63 for p <= 32767, bit_length via exact integer compares."""
-    p4 = p.astype(np.int64) ** 4
-    bl = np.zeros(p4.shape, dtype=np.int64)
-    for b in range(1, 63):
-        bl += (p4 >= (np.int64(1) << np.int64(b))).astype(np.int64)
+    """Vectorised bucket_index, exact for every int32 p >= 1: bit_length(p^4) - 1 = #{b >= 1 : p^4 >= 2^b}, and
+    p^4 >= 2^b  <=>  p^2 >= ceil(sqrt(2^b)) (p^2 < 2^62 is exact in int64; the thresholds come from math.isqrt)."""
+    p2 = p.astype(np.int64) ** 2
+    bl = np.zeros(p2.shape, dtype=np.int64)
+    for b in range(1, 124):
+        r = math.isqrt(1 << b)
+        thr = r if r * r == (1 << b) else r + 1
+        bl += (p2 >= np.int64(thr)).astype(np.int64)
     return np.minimum(n_buckets - 1, bl)
 
 

@@ -206,6 +206,20 @@ def test_p11_bucket_function(golden):
     ps = np.arange(1, 1025).reshape(-1, 1)
     vec = oracle.wm_oracle._bucket_vec(ps, 40)[:, 0]
     assert all(int(vec[i]) == oracle.bucket_index(i + 1, 40) for i in range(1024))
+    # the whole int32 range and more buckets than 64 (a loader-accepted n_buckets goes up to 4096): the quarter-octave
+    # boundaries are the integers ceil(2^(b/4)); one below, at and one above each of them, plus random parameters
+    edges = []
+    for b in range(0, 124):
+        r = math.isqrt(math.isqrt(1 << b))           # floor(2^(b/4))
+        edges += [v for v in (r - 1, r, r + 1, r + 2) if 1 <= v <= 2**31 - 1]
+    rng = np.random.default_rng(11)
+    big = np.concatenate([np.array(edges, dtype=np.int64), rng.integers(1, 2**31, size=4000), [2**16 - 1, 2**16, 2**31 - 1]])
+    vec = oracle.wm_oracle._bucket_vec(big.reshape(-1, 1), 4096)[:, 0]
+    for v, got in zip(big, vec):
+        want = (int(v) ** 4).bit_length() - 1
+        assert int(got) == want == oracle.bucket_index(int(v), 4096), v
+        assert 2 ** want <= int(v) ** 4 < 2 ** (want + 1)           # i.e. want = floor(4 log2 v), no floating point
+    assert oracle.bucket_index(2**16, 4096) == 64 and oracle.bucket_index(2**31 - 1, 4096) == 123
 
 
 # ---- P1 / P2 / P3 / P13: invariants -----------------------------------------------------------------
@@ -561,6 +575,73 @@ def test_p9_scalar_vs_vector_forest(n):
                                      b.subgraph_offsets, phi_kind=cfg.phi_kind)
     np.testing.assert_allclose(yv, ys, rtol=0, atol=1e-12)
     assert np.unique(np.round(yv, 9)).size > 30        # the forest separates the candidates
+
+
+# ---- P21: the parity metrics themselves (S15) — every GPU parity assertion passes through these two ------------------
+
+def test_p21_score_error_hand_values():
+    """score_error = max_b |y - yref| / max(|yref|, RMS_s(yref)), RMS over the candidate's own subgraph (S15)."""
+    # two subgraphs; RMS_0 = sqrt((9 + 16) / 2) = sqrt(12.5) = 3.5355..., RMS_1 = sqrt((0.01 + 0.01 + 100) / 3) = 5.7741...
+    ref = np.array([3.0, -4.0, 0.1, -0.1, 10.0])
+    off = [0, 2, 5]
+    # candidate 0: |ref| = 3 < RMS_0  -> floor used:   0.5 / sqrt(12.5)
+    # candidate 1: |ref| = 4 > RMS_0  -> |ref| used:   1.0 / 4 = 0.25
+    # candidate 2: tiny score, floor:                  1.0 / sqrt(100.02 / 3)
+    # candidate 4: |ref| = 10 > RMS_1:                 0.5 / 10
+    y = ref + np.array([0.5, -1.0, 1.0, 0.0, -0.5])
+    want = [0.5 / math.sqrt(12.5), 0.25, 1.0 / math.sqrt(100.02 / 3.0), 0.0, 0.05]
+    assert oracle.score_error(y, ref, off) == pytest.approx(max(want), rel=1e-14)
+    assert max(want) == pytest.approx(0.25, rel=1e-14)
+    # one error at a time isolates every branch (a wrong floor, denominator or segment shows in exactly one of them)
+    for i, wv in enumerate(want):
+        yi = ref.copy(); yi[i] = y[i]
+        assert oracle.score_error(yi, ref, off) == pytest.approx(wv, rel=1e-14), i
+    # the floor is the candidate's OWN subgraph: moving the boundary changes candidate 2's denominator
+    y2 = ref.copy(); y2[2] += 1.0
+    assert oracle.score_error(y2, ref, [0, 3, 5]) == pytest.approx(1.0 / math.sqrt((9 + 16 + 0.01) / 3.0), rel=1e-14)
+    # None offsets: one floor over the whole batch, RMS = sqrt((9 + 16 + 0.01 + 0.01 + 100) / 5)
+    assert oracle.score_error(y2, ref, None) == pytest.approx(1.0 / math.sqrt(125.02 / 5.0), rel=1e-14)
+    # the sign of the difference does not matter; the metric is not symmetric in (y, ref)
+    assert oracle.score_error(2 * ref - y, ref, off) == pytest.approx(oracle.score_error(y, ref, off), rel=1e-14)
+    assert oracle.score_error(ref, y, off) != pytest.approx(oracle.score_error(y, ref, off), rel=1e-6)
+    # zero reference everywhere: the guard makes it an absolute error; identical vectors: 0; empty: 0
+    assert oracle.score_error([0.0, 0.25], [0.0, 0.0], [0, 2]) == 0.25
+    assert oracle.score_error(ref, ref, off) == 0.0
+    assert oracle.score_error([], [], [0]) == 0.0
+    # empty segments are skipped; a one-candidate segment is a pure relative error (RMS = |ref|)
+    assert oracle.score_error([2.2, 5.0], [2.0, 4.0], [0, 0, 1, 1, 2]) == pytest.approx(0.25, rel=1e-14)
+    # scale invariance: a relative metric
+    assert oracle.score_error(7.0 * y, 7.0 * ref, off) == pytest.approx(oracle.score_error(y, ref, off), rel=1e-13)
+    # NaN / inf in y must not pass as "small"
+    bad = ref.copy(); bad[1] = np.nan
+    assert not (oracle.score_error(bad, ref, off) <= 1e9)
+    bad[1] = np.inf
+    assert oracle.score_error(bad, ref, off) == np.inf
+
+
+def test_p21_topk_overlap_hand_values():
+    """topk_overlap = (mean, min) over segments of |A and B| / |valid entries of B| (S15), -1 = padding."""
+    a = np.array([[0, 1, 2, 3], [10, 11, -1, -1], [20, 21, 22, 23], [-1, -1, -1, -1]])
+    b = np.array([[3, 2, 9, 8], [11, 10, -1, -1], [24, 25, 26, 27], [-1, -1, -1, -1]])
+    # segment 0: {2,3} of 4 -> 0.5; segment 1: order does not matter, 2 of 2 valid -> 1.0; segment 2: 0 of 4 -> 0;
+    # segment 3: no valid reference entry -> skipped (not counted as 1.0 or 0.0)
+    mean, mn = oracle.topk_overlap(a, b)
+    assert mean == pytest.approx((0.5 + 1.0 + 0.0) / 3.0, rel=1e-15) and mn == 0.0
+    assert oracle.topk_overlap(b, b) == (1.0, 1.0)
+    # the denominator is the REFERENCE's valid count: a shorter GPU row cannot score 1.0, a padded reference row can
+    assert oracle.topk_overlap([[5, -1, -1]], [[5, 6, 7]]) == (pytest.approx(1.0 / 3.0), pytest.approx(1.0 / 3.0))
+    assert oracle.topk_overlap([[5, 6, 7]], [[5, -1, -1]]) == (1.0, 1.0)
+    # -1 padding never matches -1 padding
+    assert oracle.topk_overlap([[-1, -1]], [[4, -1]]) == (0.0, 0.0)
+    # nothing to compare at all
+    assert oracle.topk_overlap(np.zeros((0, 4), int), np.zeros((0, 4), int)) == (1.0, 1.0)
+    # against a brute-force count on random index sets
+    rng = np.random.default_rng(3)
+    A = np.stack([rng.permutation(50)[:8] for _ in range(6)])
+    B = np.stack([rng.permutation(50)[:8] for _ in range(6)])
+    per = [sum(int(x in set(B[s])) for x in A[s]) / 8.0 for s in range(6)]
+    mean, mn = oracle.topk_overlap(A, B)
+    assert mean == pytest.approx(np.mean(per), rel=1e-15) and mn == pytest.approx(min(per), rel=1e-15)
 
 
 # ---- generator / file format ----------------------------------------------------------------------------------
