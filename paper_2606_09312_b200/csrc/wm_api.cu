@@ -3,6 +3,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <new>
 
 #include "wm_internal.h"
 
@@ -28,7 +29,7 @@ static_assert(sizeof(Header) == 76, "WMW1 header is 4 + 76 bytes");
 
 struct HostTensor {
     std::string name;
-    int rows = 0, cols = 0;   // vectors: rows = n, cols = 1
+    uint64_t rows = 0, cols = 0;   // vectors: rows = n, cols = 1 (64-bit: header fields multiply past 2^32)
     std::vector<float> v;
 };
 
@@ -43,8 +44,8 @@ int upload(wm_ctx* ctx, const std::vector<float>& h, float** out) {
 
 std::vector<float> transposed(const HostTensor& t) {
     std::vector<float> o(t.v.size());
-    for (int r = 0; r < t.rows; ++r)
-        for (int c = 0; c < t.cols; ++c) o[(size_t)c * t.rows + r] = t.v[(size_t)r * t.cols + c];
+    for (uint64_t r = 0; r < t.rows; ++r)
+        for (uint64_t c = 0; c < t.cols; ++c) o[(size_t)(c * t.rows + r)] = t.v[(size_t)(r * t.cols + c)];
     return o;
 }
 
@@ -93,7 +94,7 @@ extern "C" {
 
 const char* wm_last_error(void) { return g_err; }
 
-int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
+static int load_weights_impl(const char* path, int device, wm_ctx** ctx_out) {
     if (!path || !ctx_out) {
         set_error("wm_load_weights: null argument");
         return WM_ERR_ARG;
@@ -154,11 +155,13 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
 
     // tensor list in file order
     std::vector<HostTensor> ts;
-    auto add = [&](const char* name, int rows, int cols) {
+    uint64_t payload_floats = 0;   // sum of all tensor sizes, in 64-bit: checked against the file size before any allocation
+    auto add = [&](const char* name, uint64_t rows, uint64_t cols) {
         HostTensor t;
         t.name = name;
         t.rows = rows;
         t.cols = cols;
+        payload_floats += rows * cols;   // every factor <= 2^20 and at most three of them: no 64-bit overflow
         ts.push_back(t);
     };
     const int d = h.d, da = h.d_a, hid = h.hidden;
@@ -172,7 +175,7 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
     if (h.embed == WM_EMBED_LINEAR) {
         add("E", h.n_types, da); add("W_p", da, h.P); add("b_p", da, 1);
     } else {
-        add("Tbl", h.n_types * h.P * h.n_buckets, da);
+        add("Tbl", (uint64_t)h.n_types * h.P * h.n_buckets, da);
     }
     if (h.kind == WM_KIND_TRANSH) { add("W_w", d, da); add("W_d", d, da); }
     if (mlp) {
@@ -198,8 +201,30 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         set_error("wm_load_weights: header field out of range");
         return WM_ERR_FORMAT;
     }
+    {   // the file must hold exactly the tensors the header announces: nothing is allocated for a header that lies
+        const long pos = ftell(f);
+        if (pos < 0 || fseek(f, 0, SEEK_END) != 0) {
+            fclose(f);
+            set_error("wm_load_weights: cannot seek in '%s'", path);
+            return WM_ERR_IO;
+        }
+        const long end = ftell(f);
+        if (end < 0 || fseek(f, pos, SEEK_SET) != 0) {
+            fclose(f);
+            set_error("wm_load_weights: cannot seek in '%s'", path);
+            return WM_ERR_IO;
+        }
+        const uint64_t have = (uint64_t)(end - pos);
+        if (have != payload_floats * 4) {
+            fclose(f);
+            set_error(have < payload_floats * 4 ? "wm_load_weights: file truncated (%llu tensor bytes, header needs %llu)"
+                                                : "wm_load_weights: trailing bytes after the last tensor (%llu tensor bytes, header needs %llu)",
+                      (unsigned long long)have, (unsigned long long)(payload_floats * 4));
+            return WM_ERR_FORMAT;
+        }
+    }
     for (HostTensor& t : ts) {
-        t.v.resize((size_t)t.rows * t.cols);
+        t.v.resize((size_t)(t.rows * t.cols));
         if (fread(t.v.data(), sizeof(float), t.v.size(), f) != t.v.size()) {
             fclose(f);
             set_error("wm_load_weights: file truncated in tensor %s", t.name.c_str());
@@ -341,6 +366,22 @@ void wm_free(wm_ctx* ctx) {
     delete ctx;
 }
 
+int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
+    // "No exceptions, no aborts" (include/wm.h): an allocation failure on the host is an error code, not a terminate
+    try {
+        nvtx::Range r("wm_load_weights");
+        return load_weights_impl(path, device, ctx_out);
+    } catch (const std::bad_alloc&) {
+        if (ctx_out) *ctx_out = nullptr;
+        set_error("wm_load_weights: out of host memory");
+        return WM_ERR_IO;
+    } catch (...) {
+        if (ctx_out) *ctx_out = nullptr;
+        set_error("wm_load_weights: unexpected host exception");
+        return WM_ERR_IO;
+    }
+}
+
 int wm_get_info(const wm_ctx* ctx, wm_info* o) {
     if (!ctx || !o) {
         set_error("wm_get_info: null argument");
@@ -399,14 +440,11 @@ int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value) {
     return WM_ERR_ARG;
 }
 
-// Common tail of the three rollout entries: workspace, bucketing by rollout steps, timing events, dispatch.
-static int run_rollout(wm_ctx* ctx, CallArgs a, cudaStream_t st, const char* who) {
-    WM_CUDA_TRY(cudaSetDevice(ctx->device));
-    Workspace* ws = acquire_ws(ctx, st);
-    if (!ws) {
-        set_error("%s: cannot allocate workspace", who);
-        return WM_ERR_CUDA;
-    }
+// Common tail of the three rollout entries: bucketing by rollout steps, timing events, dispatch.  The caller holds
+// ws->mu: one call's enqueue sequence (memset, histogram, scatter, K2 [, K4]) shares the slice's perm / counters / zt, so
+// two host threads that use the same stream must not interleave theirs (in stream order the sequences then run one
+// after the other and the second reuses the buffers only after the first has finished with them).
+static int run_rollout_locked(wm_ctx* ctx, Workspace* ws, CallArgs a, cudaStream_t st) {
     a.perm = nullptr;
     a.fault = ctx->fault;
     if (ctx->opt_sort) {
@@ -429,6 +467,18 @@ static int run_rollout(wm_ctx* ctx, CallArgs a, cudaStream_t st, const char* who
         ws->timed = true;
     }
     return rc;
+}
+
+static int run_rollout(wm_ctx* ctx, const CallArgs& a, cudaStream_t st, const char* who) {
+    WM_CUDA_TRY(cudaSetDevice(ctx->device));
+    Workspace* ws = acquire_ws(ctx, st);
+    if (!ws) {
+        set_error("%s: cannot allocate workspace", who);
+        return WM_ERR_CUDA;
+    }
+    std::lock_guard<std::mutex> lk(ws->mu);
+    nvtx::Range r(who);
+    return run_rollout_locked(ctx, ws, a, st);
 }
 
 static bool sizes_ok(const char* who, int64_t B, int32_t S, int32_t T_max) {
@@ -467,6 +517,8 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
             set_error("wm_rollout_score: cannot allocate workspace");
             return WM_ERR_CUDA;
         }
+        std::lock_guard<std::mutex> lk(ws->mu);
+        nvtx::Range nr("wm_rollout_score");
         const size_t need = (size_t)B * ctx->m.d;
         if (ws->zt_cap < need) {
             if (ws->zt) {
@@ -480,7 +532,7 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
         }
         CallArgs r = a;
         r.scores_out = nullptr; r.latents_out = ws->zt; r.latents_terminal = true;
-        const int rc = run_rollout(ctx, r, st, "wm_rollout_score");
+        const int rc = run_rollout_locked(ctx, ws, r, st);
         return rc != WM_OK ? rc : launch_forest(ctx, ws->zt, a, scores_out, st);
     }
     return run_rollout(ctx, a, st, "wm_rollout_score");
@@ -565,6 +617,7 @@ int wm_topk(const float* scores, const int32_t* subgraph_offsets, int32_t S, int
         set_error("wm_topk: null pointer");
         return WM_ERR_ARG;
     }
+    nvtx::Range r("wm_topk");
     return launch_topk(scores, subgraph_offsets, S, k, idx_out, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -610,6 +663,10 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     WM_CUDA_TRY(cudaSetDevice(ctx->device));
+    // host-entry calls on one ctx are serialised (include/wm.h): the staging buffer, the helper streams and their events
+    // are shared by every call
+    std::lock_guard<std::mutex> host_lock(ctx->host_mu);
+    nvtx::Range nr("wm_score_topk_host");
     Workspace* ws = acquire_ws(ctx, st);
     if (!ws) {
         set_error("wm_score_topk_host: cannot allocate workspace");
@@ -660,7 +717,6 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
     int32_t* dreb = (int32_t*)p;
     const auto H2D = cudaMemcpyHostToDevice;
     if (nch > 1) {
-        std::lock_guard<std::mutex> host_lock(ctx->host_mu);
         if (!ctx->hs_copy) {
             WM_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->hs_copy, cudaStreamNonBlocking));
             for (int i = 0; i < 2; ++i) {
@@ -693,7 +749,8 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
         if (m.H) WM_CUDA_TRY(cudaMemcpyAsync(dhw, hw_feats, (size_t)S * m.H * 4, H2D, cp));
         WM_CUDA_TRY(cudaMemcpyAsync(doff, subgraph_offsets, (size_t)(S + 1) * 4, H2D, cp));
         WM_CUDA_TRY(cudaMemcpyAsync(dreb, ctx->h_off, (size_t)(S + nch) * 4, H2D, cp));
-        for (int c = 0; c < nch; ++c) {
+        // one chunk: its copies on the copy stream, its kernels on one of the two compute streams
+        auto chunk = [&](int c) -> int {
             const int s0 = cs[c], Sc = cs[c + 1] - cs[c];
             const int64_t c0 = subgraph_offsets[s0], Bc = (int64_t)subgraph_offsets[cs[c + 1]] - c0;
             if (Bc > 0) {
@@ -713,12 +770,19 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
                 if (rc != WM_OK) return rc;
             }
             // global offsets + the global score array: the indices come out global
-            const int rc2 = wm_topk(dsc, doff + s0, Sc, k, didx + (size_t)s0 * k, ks);
-            if (rc2 != WM_OK) return rc2;
-        }
+            return wm_topk(dsc, doff + s0, Sc, k, didx + (size_t)s0 * k, ks);
+        };
+        int crc = WM_OK;
+        for (int c = 0; c < nch && crc == WM_OK; ++c) crc = chunk(c);
+        // join the helper streams back into `st` on every path: after an error the caller's stream must still be ordered
+        // after whatever was already enqueued on them (they read the staging buffer a later call may free or refill)
         for (int i = 0; i < 2; ++i) {
-            WM_CUDA_TRY(cudaEventRecord(ctx->hev_done[i], ctx->hs_k[i]));
-            WM_CUDA_TRY(cudaStreamWaitEvent(st, ctx->hev_done[i], 0));
+            if (cudaEventRecord(ctx->hev_done[i], ctx->hs_k[i]) == cudaSuccess) cudaStreamWaitEvent(st, ctx->hev_done[i], 0);
+        }
+        if (cudaEventRecord(ctx->hev_copy[7], cp) == cudaSuccess) cudaStreamWaitEvent(st, ctx->hev_copy[7], 0);
+        if (crc != WM_OK) {
+            cudaStreamSynchronize(st);
+            return crc;
         }
         if (scores_out && B) WM_CUDA_TRY(cudaMemcpyAsync(scores_out, dsc, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
         WM_CUDA_TRY(cudaMemcpyAsync(idx_out, didx, (size_t)S * k * 4, cudaMemcpyDeviceToHost, st));

@@ -227,12 +227,8 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     if (p.embed == WM_EMBED_LINEAR) {
                         v = log2f((float)prm);
                     } else {
-                        // bucket(p) = min(n_b-1, floor(4 log2 p)) = bit_length(p^4)-1, exact in 64-bit for p < 2^16
-                        unsigned long long q = (unsigned long long)min(prm, 65535);
-                        q = q * q;
-                        q = q * q;
-                        int bk = 63 - __clzll((long long)q);
-                        v = __int_as_float(min(bk, p.n_buckets - 1));
+                        // bucket(p) = min(n_b-1, floor(4 log2 p)), exact for every int32 p (n_buckets goes up to 4096)
+                        v = __int_as_float(min(quarter_octave_bucket(prm), p.n_buckets - 1));
                     }
                 }
                 LP[e] = v;

@@ -2,6 +2,7 @@
 #pragma once
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <stdint.h>
 
 #include <atomic>
@@ -61,8 +62,19 @@ struct Model {
     alignas(64) unsigned char tc2_tmap[128] = {};   // CUtensorMap over tc_blob (pair kernel)
 };
 
+// NVTX range around an ABI call (header-only NVTX 3: a no-op unless a profiler injects itself)
+namespace nvtx {
+struct Range {
+    explicit Range(const char* name) { nvtxRangePushA(name); }
+    ~Range() { nvtxRangePop(); }
+    Range(const Range&) = delete;
+    Range& operator=(const Range&) = delete;
+};
+}  // namespace nvtx
+
 // Per-stream slice of the workspace (perm, histogram/cursors, tile counter).
 struct Workspace {
+    std::mutex mu;                 // held while one call enqueues its kernels on this slice (wm_api.cu run_rollout)
     cudaStream_t stream = nullptr;
     int32_t* perm = nullptr;
     int64_t perm_cap = 0;
@@ -139,6 +151,26 @@ struct CallArgs {
     float* latents_out;         // [B, T_max, d] z after step t+1 at [b][t] for start <= t < len; scores_out may be null
     bool latents_terminal;      // latents_out is [B, d]: only the latent after the LAST step (t = len - 1) is stored
 };
+
+// Quarter-octave bucket floor(4 log2 p) of a parameter p >= 1, exact for every int32 p (S10): with
+// e = floor(log2 p) and q = p << (31 - e) in [2^31, 2^32), q^2 is exact in 64 bits and p^4 >= 2^(4e + j)  <=>
+// (q^2)^2 >= 2^(124 + j)  <=>  hi64((q^2)^2) >= 2^(60 + j).  The caller clamps to n_buckets - 1.
+__host__ __device__ inline int quarter_octave_bucket(int p) {
+    const unsigned up = (unsigned)p;
+#ifdef __CUDA_ARCH__
+    const int e = 31 - __clz((int)up);
+    const unsigned long long q = (unsigned long long)(up << (31 - e));
+    const unsigned long long q2 = q * q;
+    const unsigned long long hi = __umul64hi(q2, q2);
+#else
+    int e = 31;
+    while (!((up >> e) & 1u)) --e;
+    const unsigned long long q = (unsigned long long)(up << (31 - e));
+    const unsigned long long q2 = q * q;
+    const unsigned long long hi = (unsigned long long)(((unsigned __int128)q2 * q2) >> 64);
+#endif
+    return 4 * e + (hi >= (1ull << 61)) + (hi >= (1ull << 62)) + (hi >= (1ull << 63));
+}
 
 // rollout steps of a candidate: its clamped length minus its clamped start (the single place that defines it)
 __host__ __device__ inline int clamp_start(int start, int len) { return start < 0 ? 0 : (start > len ? len : start); }

@@ -986,7 +986,9 @@ int tc_supported(const wm_ctx* ctx) { return ctx->m.tc_ok; }
 int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const Model& m = ctx->m;
     // per-call conditions the kernel relies on; otherwise the fp32 kernel takes the call
-    const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0);
+    // (the EXT kernels store latents as float4: a latents_out view that is only 4-byte aligned goes to the fp32 kernel)
+    const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0) &&
+                         ((uintptr_t)a.latents_out % 16 == 0);
     const bool prefix_call = a.start || a.init_index || a.latents_out;   // wm_rollout_latents / wm_rollout_score_from
     // the prefix-reuse calls are built into wm_tc_kernel only (the other models take the fp32 kernel for them); the
     // TransH kernel has the latents-out piece (wm_rollout_latents; the rollout half of a forest-ranker model)

@@ -138,6 +138,34 @@ def test_load_weights_io_and_format_errors(tmp_path):
     assert e.value.code == wm.WM_ERR_UNSUPPORTED
 
 
+def test_load_weights_huge_header_is_a_format_error(tmp_path):
+    """A header whose tensor sizes multiply past 2^32 (or ask for tens of GB) must be answered with WM_ERR_FORMAT before
+    anything is allocated: sizes are summed in 64-bit and compared with the file size (include/wm.h: no exceptions, no aborts)."""
+    cfg = gen.get_config(5).scaled(S=1, per_subgraph=8)
+    from dataclasses import replace
+    small = replace(cfg, d=16, d_a=8, scorer_widths=(8,), n_types=4, P=2, n_buckets=4, H=8)
+    f = tmp_path / "b.wmw"
+    gen.write_weight_file(str(f), small, gen.make_weights(small))
+    raw = bytearray(f.read_bytes())
+    # header layout: magic, version, kind, dtype, embed, d, d_a, hidden, n_types, P, n_buckets, H, n_lin, widths[6], eps
+    fld = lambda i: 4 + 4 * i
+    big = bytearray(raw)
+    struct.pack_into("<I", big, fld(7), 1 << 20)      # n_types = 2^20
+    struct.pack_into("<I", big, fld(8), 64)           # P = 64
+    struct.pack_into("<I", big, fld(9), 4096)         # n_buckets = 4096: rows = 2^38 (wraps to 0 in 32 bits)
+    (tmp_path / "wrap.wmw").write_bytes(bytes(big))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "wrap.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT and "truncated" in str(e.value)
+    big = bytearray(raw)
+    struct.pack_into("<I", big, fld(4), 65536)        # d = 65536
+    struct.pack_into("<I", big, fld(5), 65536)        # d_a = 65536: W_g alone would be 34 GB
+    (tmp_path / "wide.wmw").write_bytes(bytes(big))
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_load_weights(str(tmp_path / "wide.wmw"))
+    assert e.value.code == wm.WM_ERR_FORMAT and "truncated" in str(e.value)
+
+
 def test_no_product_import_of_oracle():
     """The product path must not route through the oracle (or any CPU fallback)."""
     pkg = os.path.join(ROOT, "paper_2606_09312_b200")

@@ -243,6 +243,81 @@ def test_two_streams_share_one_ctx(wm):
     wm.wm_free(ctx)
 
 
+def test_two_host_threads_share_one_stream(wm):
+    """Two host threads calling on the SAME ctx and stream (ctypes drops the GIL): the per-slice lock keeps each call's
+    enqueue sequence (memset, histogram, scatter, K2) together, so every result is bit-identical to a lone call."""
+    import threading
+    import torch
+    for n in (2, 11):                      # 11: forest ranker (K2 -> terminal latents -> K4 share the slice's buffer)
+        cfg = gen.get_config(n).scaled(S=2, per_subgraph=700)
+        b = gen.make_inputs(cfg)
+        ctx = _ctx(wm, cfg)
+        ref = gpu_scores(ctx, b)
+        dv = to_device(b)
+        outs = [torch.empty(b.B, dtype=torch.float32, device="cuda:0") for _ in range(16)]
+        torch.cuda.synchronize()
+        errs = []
+
+        def work(lo):
+            try:
+                for o in outs[lo::2]:
+                    wm.wm_rollout_score(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                                        dv["hw_feats"], o, dv["subgraph_offsets"])
+            except Exception as e:     # noqa: BLE001
+                errs.append(e)
+
+        th = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+        [t.start() for t in th]
+        [t.join() for t in th]
+        torch.cuda.synchronize()
+        assert not errs, errs
+        assert wm.wm_check(ctx) == 0
+        for o in outs:
+            np.testing.assert_array_equal(o.cpu().numpy().view(np.uint32), ref.view(np.uint32))
+        wm.wm_free(ctx)
+
+
+def test_latents_out_offset_by_one_float(wm):
+    """include/wm.h allows any fp32-aligned latents_out: a view that starts one float into an allocation (4-byte, not
+    16-byte aligned) must work (the tcgen05 kernel stores float4, so such a call is routed to the fp32 kernel)."""
+    import torch
+    cfg, w, b = _prefix_case(2, 2, 90)
+    ref = oracle.rollout_latents(w, b.init_states, b.action_ids, b.action_params, b.lengths, b.subgraph_offsets,
+                                 n_buckets=cfg.n_buckets, ln_eps=cfg.ln_eps)
+    valid = np.arange(cfg.T_max)[None, :] < b.lengths[:, None]
+    dv = to_device(b)
+    ctx = _ctx(wm, cfg)
+    n = b.B * cfg.T_max * cfg.d
+    big = torch.full((n + 8,), -777.0, dtype=torch.float32, device="cuda:0")
+    out = big[1:1 + n].view(b.B, cfg.T_max, cfg.d)
+    assert out.data_ptr() % 16 == 4
+    wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"], out,
+                          dv["subgraph_offsets"])
+    assert wm.wm_check(ctx) == 0
+    wm.wm_free(ctx)
+    lat = out.cpu().numpy()
+    assert (lat[~valid] == -777.0).all() and float(big[0]) == -777.0 and (big[1 + n:] == -777.0).all()
+    assert np.abs(lat[valid] - ref[valid]).max() / np.sqrt(np.mean(ref[valid] ** 2)) <= 2e-2
+
+
+def test_bucket_embedding_beyond_64_buckets(wm):
+    """EMBED_BUCKET with more than 64 buckets and parameters up to 2^31 - 1: bucket = floor(4 log2 p) exactly (DESIGN.md
+    S10), on the fp32 kernel (the GRU tcgen05 kernel takes models with at most 64 buckets)."""
+    cfg = replace(gen.get_config(5).scaled(S=2, per_subgraph=40), d=64, d_a=32, n_types=4, P=2, n_buckets=128, H=8,
+                  scorer_widths=(32,), T_max=6, len_lo=1, len_hi=6, k=4)
+    w = gen.make_weights(cfg)
+    b = gen.make_inputs(cfg)
+    vals = np.array([1, 2, 3, 65535, 65536, 65537, 2**20, 2**31 - 1, 19, 304, 77936, 77935], dtype=np.int32)
+    rng = np.random.default_rng(4)
+    b.action_params[:] = vals[rng.integers(0, len(vals), size=b.action_params.shape)]
+    ref = oracle_scores(cfg, w, b)
+    ctx = wm.wm_load_weights(weight_file(cfg, w))
+    assert wm.wm_get_info(ctx).path == wm.PATH_FP32
+    y = gpu_scores(ctx, b)
+    wm.wm_free(ctx)
+    assert oracle.score_error(y, ref, None) <= 2e-3
+
+
 @pytest.mark.parametrize("n,S,per", [(2, 3, 200), (2, 4, 1100), (2, 7, 900), (11, 6, 900), (5, 5, 700)])
 def test_host_entry_matches_device_entry(wm, n, S, per):
     """wm_score_topk_host (host buffers; pipelined by chunks of whole subgraphs, here forced small through
