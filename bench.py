@@ -2,25 +2,38 @@
 """bench.py — candidates scored/sec of the batched evaluator (BASELINE.json `metric`) on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+                    [--scaling weak|strong] [--no-per-config] [--no-sustained] [--prefix-reuse]
 
 A "step" is one pass of the whole hot path (length bucketing, rollout + score, top-k: DESIGN.md §1 rows a0-a7)
 over one seeded synthetic batch of the workload config (default: BASELINE.json configs[1] = cfg 2, the
-"evolution-round batch": 16 subgraphs x 2048 candidates, lengths U{8..32}).  With N > 1 (torchrun, one rank per
-GPU) every rank scores its own full batch (different input seed, same weights): candidates are independent and
-top-k is per subgraph, so there is no data-path collective ("scaling": "weak").
+"evolution-round batch": 16 subgraphs x 2048 candidates, lengths U{8..32}).
 
-`value`   : candidates/s, inputs resident in HBM, CUDA-event time per step, max over ranks, L2 flushed between steps.
-`e2e`     : the same metric through the C-ABI entry that takes HOST (pinned) buffers: H2D of the step's inputs and
-            D2H of scores + top-k indices inside the timed region.
-`roofline`: rollout+score kernel (K2) alone: literal FLOPs of the batch / its CUDA-event time (WM_OPT_TIMING).
+`value`      : candidates/s, inputs resident in HBM, CUDA-event time per step, max over ranks, L2 flushed between steps.
+`e2e`        : the same metric through the C-ABI entry that takes HOST (pinned) buffers: H2D of the step's inputs and
+               D2H of scores + top-k indices inside the timed region.
+`roofline`   : rollout+score kernel (K2) alone: literal FLOPs of the batch / its CUDA-event time (WM_OPT_TIMING).
+`sustained`  : (N = 1) the headline config's wm_rollout_score launched back to back for >= 2 s with no flush in between —
+               the online loop of PAPER.md:215 calls the evaluator round after round — with the clocks seen, against the
+               measured SUSTAINED bf16 peak.
+`per_config` : (N = 1, default config only) the other BASELINE.json configs (1, 3, 4, 5) through the same legs: ms per
+               step, K2 ms, TFLOP/s, fraction of the burst and of the sustained peak, clocks; cfg 1 also as a ratio to an
+               empty-kernel launch.
 `cpu_baseline`: the float64 numpy oracle, as it stands, on a bounded sample of the same workload on the host cores.
 --impl reference times that oracle (the only "reference" there is: the paper ships no code).
+
+N > 1: one rank per GPU (torchrun; `python bench.py --gpus N` without torchrun re-executes itself under it).  Candidates
+are independent and top-k is per subgraph, so there is no data-path collective.  --scaling weak (default): every rank
+scores its own full batch (different input seed, same weights).  --scaling strong: ONE batch is
+partitioned by whole-subgraph ranges, each rank scores and ranks its subgraphs, the [S_local, k] index blocks are
+all-gathered.
 """
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
+import re
 import subprocess
 import sys
 import threading
@@ -36,23 +49,29 @@ import gen
 
 METRIC = "candidates_scored_per_sec"
 UNIT = "candidates/s"
+KERNELS = {1: "wm_tc_kernel", 2: "wm_tc2_kernel", 3: "wm_tcg_kernel", 4: "wm_tct_kernel", 5: "wm_tcp_kernel"}
 
 
 def _kernel_name(info) -> str:
     """The rollout+score kernel (K2) the library runs for this model, by its CUDA name."""
-    if info.path == 2:
-        return {1: "wm_tc_kernel", 2: "wm_tc2_kernel", 3: "wm_tcg_kernel", 4: "wm_tct_kernel"}[info.tc_variant]
-    return "wm_generic_kernel"
+    return KERNELS.get(info.tc_variant, "wm_tc_kernel") if info.path == 2 else "wm_generic_kernel"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/*.md); keyed by (config number, kernel).  None where no capture exists yet.
-NCU_TRAFFIC = {
-    (2, "wm_tc_kernel"): (23_906_304 + 2_048, "profiles/r1_tc_v8.md"),
-    (3, "wm_tc2_kernel"): (56_585_216 + 761_856, "profiles/r1_tc2_v4.md"),
-    (5, "wm_tcg_kernel"): (3_450_484_000 + 61_085_952, "profiles/r1_tcg_v1.md"),
-    (7, "wm_tct_kernel"): (24_100_608 + 2_048, "profiles/r1_tct_v1.md"),
-}
+def ncu_traffic(config: int, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `config`, from the NEWEST committed
+    `ncu --set full` summary under profiles/ that carries a line
+        <!-- traffic: config=<n> kernel=<name> dram_bytes_per_launch=<bytes> -->
+    (files sort by round and version: r2_* after r1_*).  (bytes, file) or (None, None) when no capture names the pair."""
+    best = (None, None)
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*.md"))):
+        try:
+            text = open(path).read()
+        except OSError:
+            continue
+        for m in re.finditer(r"<!--\s*traffic:\s*config=(\d+)\s+kernel=(\w+)\s+dram_bytes_per_launch=(\d+)\s*-->", text):
+            if int(m.group(1)) == config and m.group(2) == kernel:
+                best = (int(m.group(3)), os.path.relpath(path, ROOT))
+    return best
 
 
 def _dtype_name(cfg, info) -> str:
@@ -78,53 +97,98 @@ def peaks():
         j = json.load(open(p))
         return dict(bf16=j["bf16_tflops"], bf16_sustained=j.get("bf16_tflops_sustained", j["bf16_tflops"]),
                     hbm=j["hbm_gbs"], sm_max_mhz=float(j.get("sm_max_mhz", 1965.0)), source="measured")
-    return dict(bf16=1590.0, bf16_sustained=1400.0, hbm=6650.0, source="fallback")
+    return dict(bf16=1590.0, bf16_sustained=1400.0, hbm=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
 class ClockSampler:
-    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    """SM clock, power and throttle reasons DURING a timed region (B200_PROFILING.md's clocks line).  Polls NVML from a
+    thread every ~2 ms (the timed region of the default run is ~20 ms: nvidia-smi's 100 ms loop saw two samples of it);
+    falls back to the `nvidia-smi -lms` loop when pynvml cannot be initialised."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
-        self.index = index
-        self.rows = []
-        self.proc = None
+    def __init__(self, index: int, period_s: float = 0.002):
+        self.index, self.period = index, period_s
+        self.sm, self.power, self.reasons, self.mx = [], [], set(), None
+        self.proc = self.thread = None
+        self.stop_flag = False
+        self.nvml = None
 
     def start(self):
         try:
+            import pynvml
+            pynvml.nvmlInit()
+            # NVML enumerates all GPUs of the host; CUDA_VISIBLE_DEVICES may renumber them
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            phys = self.index
+            if vis and all(t.strip().isdigit() for t in vis.split(",")):
+                phys = int(vis.split(",")[self.index])
+            h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.mx = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            self.nvml = (pynvml, h)
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return self
+        except Exception:     # noqa: BLE001 - any NVML problem: use the CLI loop instead
+            self.nvml = None
+        try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE,
+                                          "-i", str(self.index), "-lms", "20"], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
-            threading.Thread(target=self._read, daemon=True).start()
+            self.thread = threading.Thread(target=self._read_cli, daemon=True)
+            self.thread.start()
         except OSError:
             self.proc = None
+        return self
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
-
-    def stop(self):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+    def _poll(self):
+        pynvml, h = self.nvml
+        bits = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+        get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+            getattr(pynvml, "nvmlDeviceGetCurrentClocksThrottleReasons")
+        while not self.stop_flag:
             try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
+                self.sm.append(float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                self.power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                r = int(get_reasons(h))
+                for name, bit in bits.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:     # noqa: BLE001
+                pass
+            time.sleep(self.period)
+
+    def _read_cli(self):
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.proc.stdout:
+            r = [x.strip() for x in line.split(",")]
+            try:
+                self.sm.append(float(r[0]))
+                self.mx = float(r[1])
+                self.power.append(float(r[2]))
             except (ValueError, IndexError):
                 continue
             for n, v in zip(names, r[3:7]):
                 if v.lower().startswith("active"):
-                    reasons.add(n)
+                    self.reasons.add(n)
+
+    def stop(self):
+        if self.nvml is None and self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["clock sampling unavailable"], "samples": 0}
+        if self.proc is not None:
+            time.sleep(0.05)
+            self.proc.terminate()
+        self.stop_flag = True
+        if self.thread is not None:
+            self.thread.join(1.0)
+        sm = sorted(self.sm)
         # "under load" = the upper half of the samples (the sampler also sees the idle gaps between steps)
-        sm.sort()
         load = sm[len(sm) // 2:] if sm else []
-        return {"sm_mhz": float(np.median(load)) if load else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+        return {"sm_mhz": float(np.median(load)) if load else None, "sm_min_mhz": sm[0] if sm else None,
+                "sm_max_mhz": self.mx, "power_w_max": max(self.power) if self.power else None,
+                "reasons": sorted(self.reasons), "samples": len(sm),
+                "source": "nvml poll 2 ms" if self.nvml else "nvidia-smi -lms 20"}
 
 
 def cpu_baseline(cfg, n_subgraphs: int):
@@ -187,15 +251,218 @@ def reduce_sum(value: float, dist_mod=None, device=None) -> float:
 
 
 def rank_config(cfg, rank: int):
-    """Rank r's batch: same model and shapes, its own input seed (weak scaling; no exchange between ranks)."""
+    """Rank r's batch under WEAK scaling: same model and shapes, its own input seed (no exchange between ranks)."""
     from dataclasses import replace
     return cfg if rank == 0 else replace(cfg, number=cfg.number + 1000 * rank)
+
+
+def subgraph_range(S: int, world: int, rank: int):
+    """STRONG scaling: rank r owns the whole subgraphs [s0, s1) of the one batch — contiguous,
+    near-equal counts, every subgraph owned exactly once."""
+    return (S * rank) // world, (S * (rank + 1)) // world
+
+
+def slice_batch(batch, s0: int, s1: int):
+    """The sub-batch of subgraphs [s0, s1): candidates and offsets rebased to the slice (views, no arithmetic)."""
+    off = np.asarray(batch.subgraph_offsets, dtype=np.int64)
+    c0, c1 = int(off[s0]), int(off[s1])
+    return gen.Batch(batch.init_states[s0:s1], batch.hw_feats[s0:s1], batch.action_ids[c0:c1], batch.action_params[c0:c1],
+                     batch.lengths[c0:c1], (off[s0:s1 + 1] - c0).astype(np.int32), batch.T_max,
+                     None if batch.parent_of is None else batch.parent_of[c0:c1],
+                     None if batch.cut is None else batch.cut[c0:c1]), c0
+
+
+def gather_topk(idx_local, c0: int, S: int, k: int, world: int, dist_mod, device):
+    """All-gather of the per-rank [S_local, k] index blocks into the batch's [S, k] (global candidate indices: the
+    slice's base is added to every valid entry).  The only exchange of the strong-scaling mode, after the timed kernels."""
+    import torch
+    glob_idx = torch.where(idx_local >= 0, idx_local + int(c0), idx_local)
+    if dist_mod is None or not dist_mod.is_initialized():
+        return glob_idx
+    rows = max(subgraph_range(S, world, r)[1] - subgraph_range(S, world, r)[0] for r in range(world))
+    pad = torch.full((rows, k), -1, dtype=torch.int32, device=device)
+    pad[:glob_idx.shape[0]] = glob_idx
+    parts = [torch.empty_like(pad) for _ in range(world)]
+    dist_mod.all_gather(parts, pad)
+    out = [parts[r][:subgraph_range(S, world, r)[1] - subgraph_range(S, world, r)[0]] for r in range(world)]
+    return torch.cat(out, dim=0)
+
+
+class Leg:
+    """One config on one device: weights, resident inputs, and the timed legs."""
+
+    def __init__(self, wm, cfg, batch, dev, flush):
+        import torch
+        from wm_harness import weight_file, to_device
+        self.wm, self.cfg, self.batch, self.dev, self.flush = wm, cfg, batch, dev, flush
+        self.ctx = wm.wm_load_weights(weight_file(cfg), dev.index or 0)
+        self.info = wm.wm_get_info(self.ctx)
+        self.dv = to_device(batch, device=dev)
+        self.B, self.S, self.k = batch.B, batch.S, cfg.k
+        self.scores = torch.empty(self.B, dtype=torch.float32, device=dev)
+        self.idx = torch.empty((self.S, self.k), dtype=torch.int32, device=dev)
+
+    def score(self):
+        dv = self.dv
+        self.wm.wm_rollout_score(self.ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                                 dv["hw_feats"], self.scores, dv["subgraph_offsets"])
+
+    def step(self):
+        self.score()
+        self.wm.wm_topk(self.scores, self.dv["subgraph_offsets"], self.k, self.idx)
+
+    def warm(self, n):
+        for _ in range(max(n, 3)):
+            self.flush.zero_()
+            self.step()
+        assert self.wm.wm_check(self.ctx) == 0
+
+    def launches(self):
+        return self.wm.wm_launch_count(self.ctx) + self.wm.wm_launch_count(None)
+
+    def timed_steps(self, steps, barrier):
+        """K steps, each bracketed by CUDA events on the launching stream, L2 flushed (untimed) in between; clocks
+        sampled during the region.  -> (list of ms, clocks, launches)"""
+        import torch
+        sampler = ClockSampler(self.dev.index or 0)
+        barrier()
+        n0 = self.launches()
+        sampler.start()
+        evs = []
+        for _ in range(steps):
+            self.flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            self.step()
+            e1.record()
+            evs.append((e0, e1))
+        barrier()
+        clocks = sampler.stop()
+        return [a.elapsed_time(b) for a, b in evs], clocks, self.launches() - n0
+
+    def kernel_ms(self, steps):
+        """K2 alone (WM_OPT_TIMING: events recorded by the library around the rollout+score launch)."""
+        wm = self.wm
+        wm.wm_set_option(self.ctx, wm.WM_OPT_TIMING, 1)
+        kms = []
+        for _ in range(steps):
+            self.flush.zero_()
+            self.score()
+            kms.append(wm.wm_last_kernel_ms(self.ctx))
+        wm.wm_set_option(self.ctx, wm.WM_OPT_TIMING, 0)
+        return float(np.mean(kms))
+
+    def roofline(self, k_ms, step_ms):
+        cfg, info, pk = self.cfg, self.info, peaks()
+        flops = literal_flops(cfg, self.batch.lengths)
+        achieved = flops / (k_ms * 1e-3) / 1e12
+        b = self.batch
+        bytes_in = sum(int(np.asarray(a).nbytes) for a in (b.action_ids, b.action_params, b.lengths)) + 4 * self.B
+        if cfg.dtype == gen.configs.DTYPE_FP32:
+            # cfg 1: 12 MFLOP / 10 KB, launch-latency-bound; report the achieved HBM GB/s as north_star asks
+            roof = {"bound": "hbm", "achieved": bytes_in / (k_ms * 1e-3) / 1e9, "peak": pk["hbm"], "unit": "GB/s",
+                    "traffic": None, "note": "latency-bound tiny config; neither roofline applies"}
+        elif info.path == 2:
+            tr, src = ncu_traffic(cfg.number, _kernel_name(info))
+            roof = {"bound": "tensor", "achieved": achieved, "peak": pk["bf16"], "unit": "TFLOP/s",
+                    "traffic": tr, "traffic_source": src, "frac_of_sustained_peak": achieved / pk["bf16_sustained"],
+                    "peak_sustained": pk["bf16_sustained"]}
+        else:
+            # the fp32 CUDA-core kernel is bound by plain FFMA issue: 148 SMs x 128 lanes x 2 FLOP x SM clock
+            # (DESIGN.md §5, K2-fp32), not by the tensor pipe
+            alu_peak = 148 * 128 * 2 * (pk.get("sm_max_mhz", 1965.0) * 1e6) / 1e12
+            roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "traffic": None,
+                    "traffic_source": None, "note": "fp32 FFMA peak derived from unit counts and the SM clock"}
+        roof["frac"] = roof["achieved"] / roof["peak"]
+        roof.update({"kernel": _kernel_name(info), "kernel_ms": k_ms,
+                     "peak_source": pk["source"] + " (burst: kernel timed alone)",
+                     "algorithmic_flops_per_launch": flops, "share_of_step": k_ms / step_ms})
+        return roof
+
+    def sustained(self, seconds=2.0):
+        """wm_rollout_score back to back for >= `seconds` with no flush and no host sync in between (the regime of an
+        online search loop): ms per call (bucketing + K2), literal TFLOP/s, clocks and throttle reasons seen."""
+        import torch
+        self.score()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); self.score(); e1.record(); torch.cuda.synchronize()
+        one = max(e0.elapsed_time(e1), 1e-3)
+        n = int(min(max(seconds * 1e3 / one, 10), 200000))
+        sampler = ClockSampler(self.dev.index or 0, period_s=0.01).start()
+        e0.record()
+        for _ in range(n):
+            self.score()
+        e1.record()
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        ms = e0.elapsed_time(e1) / n
+        pk = peaks()
+        tf = literal_flops(self.cfg, self.batch.lengths) / (ms * 1e-3) / 1e12
+        return {"calls": n, "seconds": ms * n * 1e-3, "ms_per_call": ms, "tflops": tf,
+                "frac_of_sustained_peak": tf / pk["bf16_sustained"], "frac_of_burst_peak": tf / pk["bf16"],
+                "peak_sustained": pk["bf16_sustained"], "clocks": clocks,
+                "what": "wm_rollout_score (bucketing + K2) back to back, inputs L2-warm, literal FLOPs / call time"}
+
+    def close(self):
+        self.wm.wm_free(self.ctx)
+        self.ctx = None
+
+
+def per_config_leg(wm, n, dev, flush, steps):
+    """One of the other BASELINE.json configs through the device-resident legs (default run, N = 1)."""
+    import torch
+    cfg = gen.get_config(n)
+    t0 = time.perf_counter()
+    batch = gen.make_inputs(cfg)
+    gen_s = time.perf_counter() - t0
+    leg = Leg(wm, cfg, batch, dev, flush)
+    leg.warm(3)
+    ms, clocks, launches = leg.timed_steps(steps, torch.cuda.synchronize)
+    step_ms = float(np.mean(ms))
+    k_ms = leg.kernel_ms(steps)
+    roof = leg.roofline(k_ms, step_ms)
+    out = {"workload": workload_name(cfg), "kernel": roof["kernel"], "steps": steps, "ms_per_step": step_ms,
+           "value": leg.B / (step_ms * 1e-3), "unit": UNIT,
+           "rollout_steps_per_sec": float(batch.lengths.sum()) / (step_ms * 1e-3), "kernel_ms": k_ms,
+           "gpu_launches": int(launches), "clocks": clocks, "input_generation_s": gen_s}
+    if roof["bound"] == "tensor":
+        out.update({"tflops": roof["achieved"], "frac_of_burst_peak": roof["frac"],
+                    "frac_of_sustained_peak": roof["frac_of_sustained_peak"], "traffic": roof["traffic"],
+                    "traffic_source": roof.get("traffic_source")})
+    else:
+        # cfg 1: launch-latency-bound.  Yardstick: one empty kernel launch, timed the same way (events around
+        # back-to-back launches on the stream); the step is bucketing (2 launches + memset) + K2 + top-k.
+        for _ in range(20):
+            wm.wm_launch_empty()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 200
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            wm.wm_launch_empty()
+        e1.record()
+        torch.cuda.synchronize()
+        empty_ms = e0.elapsed_time(e1) / reps
+        one = []
+        for _ in range(50):      # a lone launch between two events (launch + drain, not back-to-back throughput)
+            a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); wm.wm_launch_empty(); b_.record(); torch.cuda.synchronize()
+            one.append(a.elapsed_time(b_))
+        lone_ms = float(np.median(one))
+        out.update({"achieved_gbs": roof["achieved"], "empty_kernel_launch_ms": lone_ms,
+                    "empty_kernel_back_to_back_ms": empty_ms,
+                    "step_over_empty_launch": step_ms / lone_ms, "k2_over_empty_launch": k_ms / lone_ms,
+                    "note": "launch-latency-bound: 12 MFLOP, 10 KB of input"})
+    leg.close()
+    del leg, batch
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_ours(args, cfg):
     import torch
     import paper_2606_09312_b200 as wm
-    from wm_harness import weight_file, to_device
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -207,93 +474,52 @@ def run_ours(args, cfg):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = torch.device("cuda", local_rank)
+    strong = args.scaling == "strong" and world > 1
 
-    ctx = wm.wm_load_weights(weight_file(cfg), local_rank)
-    info = wm.wm_get_info(ctx)
-    rcfg = rank_config(cfg, rank)
-    batch = gen.make_inputs(rcfg)
-    dv = to_device(batch, device=dev)
-    B, S, k = batch.B, batch.S, cfg.k
-    scores = torch.empty(B, dtype=torch.float32, device=dev)
-    idx = torch.empty((S, k), dtype=torch.int32, device=dev)
+    c0 = 0
+    if strong:      # one batch, this rank's whole subgraphs
+        full = gen.make_inputs(cfg)
+        s0, s1 = subgraph_range(full.S, world, rank)
+        batch, c0 = slice_batch(full, s0, s1)
+    else:
+        batch = gen.make_inputs(rank_config(cfg, rank))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
-
-    def step():
-        wm.wm_rollout_score(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
-                            dv["hw_feats"], scores, dv["subgraph_offsets"])
-        wm.wm_topk(scores, dv["subgraph_offsets"], k, idx)
+    leg = Leg(wm, cfg, batch, dev, flush)
+    info = leg.info
+    B, S, k = leg.B, leg.S, leg.k
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        flush.zero_()
-        step()
-    assert wm.wm_check(ctx) == 0
-    launches0 = wm.wm_launch_count(ctx) + wm.wm_launch_count(None)
+    leg.warm(args.warmup)
 
-    # ---- device-resident timing: K steps, each bracketed by events, L2 flushed (untimed) in between
-    sampler = ClockSampler(local_rank)
-    barrier()
-    sampler.start()
-    evs = []
-    for _ in range(args.steps):
-        flush.zero_()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        step()
-        e1.record()
-        evs.append((e0, e1))
-    barrier()
-    clocks = sampler.stop()
-    launches = wm.wm_launch_count(ctx) + wm.wm_launch_count(None) - launches0
-    ms = [a.elapsed_time(b) for a, b in evs]
+    # ---- device-resident timing
+    ms, clocks, launches = leg.timed_steps(args.steps, barrier)
     total_ms = reduce_max(float(np.sum(ms)), dist, dev)
     ms_per_step = total_ms / args.steps
     cands_all = reduce_sum(float(B), dist, dev)
     steps_all = reduce_sum(float(batch.lengths.sum()), dist, dev)
     value = cands_all / (ms_per_step * 1e-3)
+    gathered_rows = None
+    if strong:      # the result exchange of the strong mode: [S_local, k] -> [S, k] on every rank
+        gathered_rows = int(gather_topk(leg.idx, c0, cfg.S, k, world, dist, dev).shape[0])
 
-    # ---- roofline leg: K2 alone, literal FLOPs / CUDA-event time on its stream
-    wm.wm_set_option(ctx, wm.WM_OPT_TIMING, 1)
-    kms = []
-    for _ in range(args.steps):
-        flush.zero_()
-        wm.wm_rollout_score(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
-                            dv["hw_feats"], scores, dv["subgraph_offsets"])
-        kms.append(wm.wm_last_kernel_ms(ctx))
-    wm.wm_set_option(ctx, wm.WM_OPT_TIMING, 0)
-    k_ms = float(np.mean(kms))
-    flops = literal_flops(cfg, batch.lengths)
-    pk = peaks()
-    achieved = flops / (k_ms * 1e-3) / 1e12
-    bytes_in = sum(int(np.asarray(a).nbytes) for a in (batch.action_ids, batch.action_params, batch.lengths)) + 4 * B
-    if cfg.dtype == gen.configs.DTYPE_FP32:
-        # cfg 1: 12 MFLOP / 10 KB, launch-latency-bound; report the achieved HBM GB/s as north_star asks
-        roof = {"bound": "hbm", "achieved": bytes_in / (k_ms * 1e-3) / 1e9, "peak": pk["hbm"], "unit": "GB/s",
-                "traffic": None, "note": "latency-bound tiny config; neither roofline applies"}
-    else:
-        tr = NCU_TRAFFIC.get((cfg.number, _kernel_name(info)))
-        if info.path == 2:
-            roof = {"bound": "tensor", "achieved": achieved, "peak": pk["bf16"], "unit": "TFLOP/s",
-                    "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None}
-        else:
-            # the fp32 CUDA-core kernel is bound by plain FFMA issue: 148 SMs x 128 lanes x 2 FLOP x SM clock
-            # (K2-fp32), not by the tensor pipe
-            alu_peak = 148 * 128 * 2 * (pk.get("sm_max_mhz", 1965.0) * 1e6) / 1e12
-            roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "traffic": None,
-                    "traffic_source": None, "note": "fp32 FFMA peak derived from unit counts and the SM clock"}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof.update({"kernel": _kernel_name(info), "kernel_ms": k_ms,
-                 "peak_source": pk["source"] + " (burst: kernel timed alone)",
-                 "algorithmic_flops_per_launch": flops, "share_of_step": k_ms / float(np.mean(ms))})
+    # ---- roofline leg: K2 alone
+    k_ms = leg.kernel_ms(args.steps)
+    roof = leg.roofline(k_ms, float(np.mean(ms)))
+
+    # ---- sustained leg (N = 1): back-to-back launches for >= 2 s
+    sustained = None
+    if world == 1 and not args.no_sustained and roof["bound"] == "tensor":
+        sustained = leg.sustained(2.0)
 
     # ---- prefix-latent reuse leg (NEXT row f3; configs with a shared-prefix structure, i.e. cfg 4): the representative of
     # every family (the child with the longest copied prefix) is rolled once over that prefix with the latent stored
     # after every step, then every child is scored from its cut.  Same scores, a third of the rollout steps.
     prefix = None
+    ctx, dv, scores, idx = leg.ctx, leg.dv, leg.scores, leg.idx
     if batch.cut is not None and args.prefix_reuse:
         C = cfg.prefix_children
         cut = batch.cut.reshape(-1, C)
@@ -359,33 +585,57 @@ def run_ours(args, cfg):
     h2d = sum(int(t.numel() * t.element_size()) for t in hb.values())
     d2h = int(h_scores.numel() * 4 + h_idx.numel() * 4)
     np.testing.assert_array_equal(h_idx.numpy(), idx.cpu().numpy())   # same answer through both entries
+    del hb, h_scores, h_idx
 
-    wm.wm_free(ctx)
+    leg.close()
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
+    scaling = "strong" if strong else "weak"
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-           "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+           "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": scaling,
            "vs_baseline": None, "dtype": _dtype_name(cfg, info),
            "data": "synthetic",
            "config": {"workload": workload_name(cfg), "per_gpu_batch": B, "l2": "flushed between steps (256 MB write)",
                       "path": _kernel_name(info),
                       "operands": ("fp32" if _dtype_name(cfg, info) == "f32" else
-                                   "bf16-valued weights encoded as fp16 (exact), fp16 activations, fp32 accumulate + latent"),
-                      "parallelism": f"dp{world} (independent batches, no collective)"},
+                                   "bf16-valued weights encoded as fp16 (exact for 2^-14 <= |w| <= 65504), fp16 "
+                                   "activations, fp32 accumulate + latent"),
+                      "parallelism": (f"dp{world}: one batch split by whole-subgraph ranges, [S_local,k] all-gather "
+                                      f"after the timed kernels ({gathered_rows} rows gathered)" if strong else
+                                      f"dp{world} (independent batches, no collective)")},
            "rollout_steps_per_sec": steps_all / (ms_per_step * 1e-3),
            "clocks": clocks, "gpu_launches": int(launches),
            "e2e": {"value": cands_all / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                    "ms_per_step": e2e_s * 1e3},
            "roofline": roof}
+    if sustained is not None:
+        out["sustained"] = sustained
     if prefix is not None:
         out["prefix_reuse"] = prefix
     if world == 1:
+        if args.config == 2 and not args.no_per_config:
+            del batch
+            torch.cuda.empty_cache()
+            out["per_config"] = {}
+            for n, st in ((1, 20), (3, 10), (4, 5), (5, 5)):
+                out["per_config"][f"cfg{n}"] = per_config_leg(wm, n, dev, flush, st)
         out["cpu_baseline"] = cpu_baseline(cfg, 4 if cfg.number != 1 else cfg.S)
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def relaunch_under_torchrun(args) -> None:
+    """`python bench.py --gpus N` outside torchrun: start the N ranks ourselves (same launch line the driver uses)."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
 
 
 def main():
@@ -396,9 +646,15 @@ def main():
     ap.add_argument("--prefix-reuse", action="store_true",
                     help="config 4: also time the prefix-latent-reuse calls (extra 'prefix_reuse' object in the JSON line)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = a full batch per rank; strong = one batch split by whole-subgraph ranges (SURVEY.md §8(e))")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (cfg 1, 3, 4, 5) of the default run")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the 2 s back-to-back leg")
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]; 6, 7 = NEXT row f1 (TransH transition); 8, 9 = NEXT row f2 (structured phi); 10, 11 = NEXT row f4 (forest ranker); 12 = TransH + structured phi + forest")
     args = ap.parse_args()
     cfg = gen.get_config(args.config)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        relaunch_under_torchrun(args)
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

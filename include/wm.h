@@ -225,6 +225,11 @@ int wm_last_kernel_ms(wm_ctx* ctx, void* cuda_stream, float* ms_out);
  * gpu_launches); wm_topk's launches are counted in a process-wide counter returned when ctx == NULL. */
 int64_t wm_launch_count(const wm_ctx* ctx);
 
+/* Launch one empty kernel (1 block, 32 threads, no work) on `cuda_stream`: the launch-latency yardstick of bench.py's
+ * cfg 1 line (cfg 1 is 12 MFLOP and 10 KB, bound by launch latency; its time is reported as a ratio
+ * to this).  Needs no context.  Errors: WM_ERR_CUDA. */
+int wm_launch_empty(void* cuda_stream);
+
 /* Message for the last nonzero status returned on this thread ("" if none). */
 const char* wm_last_error(void);
 

@@ -23,7 +23,7 @@ PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 # every symbol include/wm.h declares
 ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
                "wm_rollout_latents", "wm_rollout_score_from",
-               "wm_check", "wm_score_topk_host", "wm_last_kernel_ms", "wm_launch_count", "wm_last_error")
+               "wm_check", "wm_score_topk_host", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error")
 
 
 class WmInfo(ctypes.Structure):
@@ -79,6 +79,8 @@ def lib() -> ctypes.CDLL:
     L.wm_last_kernel_ms.restype = ctypes.c_int
     L.wm_launch_count.argtypes = [vp]
     L.wm_launch_count.restype = i64
+    L.wm_launch_empty.argtypes = [vp]
+    L.wm_launch_empty.restype = ctypes.c_int
     L.wm_last_error.argtypes = []
     L.wm_last_error.restype = ctypes.c_char_p
     _lib = L
@@ -190,3 +192,8 @@ def wm_last_kernel_ms(ctx: int, stream=None) -> float:
 
 def wm_launch_count(ctx: Optional[int]) -> int:
     return int(lib().wm_launch_count(ctx))
+
+
+def wm_launch_empty(stream=None) -> None:
+    """One empty kernel on the stream (bench.py's launch-latency yardstick).  include/wm.h."""
+    _check(lib().wm_launch_empty(_stream(stream)))

@@ -89,6 +89,8 @@ int pick_path(const wm_ctx* ctx) {
 
 using namespace wm;
 
+__global__ void wm_empty_kernel() {}
+
 #pragma GCC visibility push(default)
 extern "C" {
 
@@ -804,6 +806,12 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
     if (scores_out && B) WM_CUDA_TRY(cudaMemcpyAsync(scores_out, dsc, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
     WM_CUDA_TRY(cudaMemcpyAsync(idx_out, didx, (size_t)S * k * 4, cudaMemcpyDeviceToHost, st));
     WM_CUDA_TRY(cudaStreamSynchronize(st));
+    return WM_OK;
+}
+
+int wm_launch_empty(void* cuda_stream) {
+    wm_empty_kernel<<<1, 32, 0, static_cast<cudaStream_t>(cuda_stream)>>>();
+    WM_CUDA_TRY(cudaGetLastError());
     return WM_OK;
 }
 
