@@ -1,0 +1,1045 @@
+// K2 (tcgen05, CTA pair, M = 256): fused persistent rollout + score kernel for the bf16 residual-MLP + LayerNorm
+// models with d = 256, d_a = 128 (BASELINE.json cfg 2 and cfg 4) — the pair form of wm_tc_kernel, sm_100a only.
+//
+// PAPER.md:162 Eq.8 / :166 — z_t = F(z_{t-1}, a_t) applied recurrently; :176 — masked steps leave z unchanged;
+// :186-188 Eq.12 — y = G([z_T ; phi ; h]).  Parametrisation: BASELINE.json cfg 2/4.
+//
+// Why a pair: wm_tc_kernel is bound by its single MMA-issuing warp (one ring stage of bookkeeping per 512
+// tensor cycles) and, next, by the L2 -> SM weight stream.  A cluster of two CTAs (one TPC) owns a tile of 256
+// length-sorted candidates, 128 rows per CTA, and the leader CTA issues `tcgen05.mma.cta_group::2` with M = 256:
+//   * per CTA nothing changes in TMEM (fp32 latent = GEMM2 accumulator in columns [0,256), two 128-column GEMM1
+//     accumulators whose fp16 GELU output is written back over them and read by GEMM2 as a TMEM A operand) nor in the A
+//     operand ([z ; a] fp16, six 16 KB K-blocks in shared memory): each CTA supplies ITS 128 rows;
+//   * each CTA supplies HALF of every B (weight) tile, so the L2 -> SM weight stream per SM halves, and one issued MMA
+//     drives both SMs' tensor pipes: the issuer executes half the instructions, waits and commits per FLOP;
+//   * a ring stage is two 16 KB TMA boxes per CTA = 1024 tensor cycles of work for the pair (8 or 16 MMAs per wait / commit);
+//     the weight image is laid out in consumption order, one box per CTA side by side, and read through a tensor map
+//     (`cp.async.bulk.tensor ... cta_group::2`: both halves' complete_tx land on the leader's barrier);
+//   * MMA completion is multicast to both CTAs' barriers; epilogue / action warps of both CTAs arrive on the leader's
+//     barriers (cluster-scope release).
+// Warp roles per CTA (512 threads) as in wm_tc_kernel: warps 0-7 epilogue (one thread per row and column half), warps
+// 8-11 action embedding, warp 12 TMEM allocator, warp 13 tile schedule + TMA producer, warp 15 MMA issuer (leader only).
+#include <cuda.h>
+#include <cuda_bf16.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "wm_internal.h"
+#include "wm_ptx.cuh"
+
+namespace wm {
+
+namespace tcp {
+
+using namespace ptx;
+
+constexpr int TMP = 256;           // candidates per pair tile (MMA M)
+constexpr int TM = 128;            // rows per CTA
+constexpr int D = 256;             // latent width
+constexpr int DA = 128;            // action-embedding width
+constexpr int SW = 512;            // scorer hidden width (both hidden layers)
+constexpr int KB_BYTES = 16384;    // one A K-block: [128 rows x 64 cols] fp16, SW128 K-major
+constexpr int BOX_BYTES = 16384;   // one TMA box: 128 image rows of 128 B = this CTA's half of two N = 128 K-blocks (2 x 64
+                                   // weight rows) or of one N = 256 K-block (128 weight rows); 512 tensor cycles of MMAs
+constexpr int HALF_BYTES = 8192;   // one N = 128 K-block half: [64 weight rows x 64 cols]
+constexpr int STAGE_BYTES = 2 * BOX_BYTES;
+constexpr int NSTAGE = 3;
+constexpr int A1_KB = 6;           // z: 0-3, a/phi: 4-5
+constexpr int HWK_BYTES = 4096;    // hw operand: one [128 x 16] no-swizzle K-major tile per K = 16 step
+constexpr int THREADS = 512;
+constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
+constexpr int MAX_TYPES = 64, MAX_P = 8, MAX_H = 64, MAX_HID = 1024;
+constexpr int SC_BOXES = 4 * 4 + 4 * 4;   // scorer stream per CTA: layer 1 (4 chunks x (phi, hw, z, z)), layer 2 (4 x 4)
+
+enum {
+    B_FULL = 0,                    // [NSTAGE] TMA (both CTAs) -> leader's MMA warp
+    B_EMPTY = B_FULL + NSTAGE,     // [NSTAGE] MMA commit (multicast) -> each CTA's producer
+    B_D1FULL = B_EMPTY + NSTAGE,   // [2] MMA commit -> epilogue: accumulator buffer b filled
+    B_HREADY = B_D1FULL + 2,       // [2] epilogue (both CTAs) -> leader MMA: buffer b read, fp16 hidden written to TMEM
+    B_D2FULL = B_HREADY + 2,       // MMA commit -> epilogue: GEMM2 of the step done
+    B_ZREADY,                      // epilogue (both CTAs) -> leader MMA: z written
+    B_AFREE,                       // MMA commit -> action warps: a-part of A1 no longer read
+    B_AREADY,                      // action warps (both CTAs) -> leader MMA: a-part written
+    B_SFULL,                       // [2] schedule slot filled (CTA-local)
+    B_SEMPTY = B_SFULL + 2,        // [2] schedule slot consumed (CTA-local)
+    B_COUNT = B_SEMPTY + 2
+};
+
+struct Params {
+    int hid, nc, n_types, P, H, hw_ksteps;
+    float ln_eps;
+    const __nv_bfloat16* E;     // [n_types][128]
+    const float *WpT, *bp;      // [P][128], [128]
+    const float *b1, *b2, *gamma, *beta;
+    const float *bs0, *bs1, *w3, *bs2;
+    CallArgs a;
+    int n_tiles;
+};
+
+struct SmemLayout {
+    uint32_t a1, hwk, ring, e_tab, lp, mx, ids, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
+};
+
+__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps, int phi_struct) {
+    SmemLayout L;
+    uint32_t o = 0;
+    L.a1 = o; o += A1_KB * KB_BYTES;
+    L.ring = o; o += NSTAGE * STAGE_BYTES;
+    L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
+    L.e_tab = o; o += (uint32_t)n_types * DA * 2;
+    L.lp = o; o += TM * MAX_P * 4;
+    L.mx = o; o += phi_struct ? TM * MAX_P * 4 : 0;
+    L.ids = o; o += TM * 4;
+    L.cnt = o; o += TM * (uint32_t)n_types;           // u8 counts, row-major [128][n_types]
+    o = (o + 15) & ~15u;
+    L.b1 = o; o += (uint32_t)hid * 4;
+    L.b2 = o; o += D * 4;
+    L.gamma = o; o += D * 4;
+    L.beta = o; o += D * 4;
+    L.red = o; o += 4 * TM * 8;                        // [2 (LayerNorm parity)][2 column halves][128 rows] float2
+    L.bars = o; o += B_COUNT * 8;
+    L.sched = o; o += 2 * 8;
+    L.tmem_slot = o; o += 16;
+    L.total = o;
+    return L;
+}
+
+// Static tile schedule (as wm_tc2_kernel): pair `pair` of `np` takes tile it*np + pair on even rounds and
+// it*np + (np-1-pair) on odd rounds; tiles are sorted longest first, the serpentine evens out the step totals.
+__device__ __forceinline__ int tile_of(int it, int pair, int np, int n_tiles) {
+    const int idx = it * np + ((it & 1) ? np - 1 - pair : pair);
+    return idx < n_tiles ? idx : -1;
+}
+
+// Ring-stage program of one rollout step, per CTA, in boxes: stage 0 = a K-blocks of chunks 0 and 1, stages 1, 2 = z
+// K-blocks of chunk 0 / chunk 1, stage 3 = GEMM2 chunk 0, then per further chunk i: a K-blocks (ONE box), z K-blocks, GEMM2
+// chunk i-1; last stage = GEMM2 chunk NC-1.  3 NC - 1 stages, 5 NC boxes.
+__host__ __device__ inline int step_stages(int nc) { return 3 * nc - 1; }
+__host__ __device__ inline int stage_boxes(int j, int nc) { return (j >= 4 && j < 3 * nc - 2 && (j - 4) % 3 == 0) ? 1 : 2; }
+
+constexpr uint32_t idesc_m256(uint32_t n) { return (1u << 4) | ((n >> 3) << 17) | ((256u >> 4) << 24); }
+constexpr uint32_t ID_N128 = idesc_m256(128), ID_N256 = idesc_m256(256);
+
+// pair MMA with the A operand in tensor memory (each CTA's own 128 lanes)
+__device__ __forceinline__ void mma_ts2(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc)
+        : "memory");
+}
+
+// PHI / EXT as in wm_tc_kernel: PHI = WM_PHI_MEAN | WM_PHI_STRUCT (what the action warps write into the phi K-blocks);
+// EXT = the prefix-latent-reuse calls (per-candidate start and initial-latent row, latents stored), compiled out of
+// the literal path.
+template <int PHI, bool EXT>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps, PHI);
+    const uint32_t s_base = smem_u32(smem);
+    const uint32_t s_a1 = s_base + L.a1, s_ring = s_base + L.ring, s_bars = s_base + L.bars;
+    auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
+    volatile int* s_sched = reinterpret_cast<volatile int*>(smem + L.sched);   // [2][2]: tile, nsteps
+    float* s_b1 = reinterpret_cast<float*>(smem + L.b1);
+    float* s_b2 = reinterpret_cast<float*>(smem + L.b2);
+    float* s_gamma = reinterpret_cast<float*>(smem + L.gamma);
+    float* s_beta = reinterpret_cast<float*>(smem + L.beta);
+    float2* s_red = reinterpret_cast<float2*>(smem + L.red);                  // [2][2][128]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
+    const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+    const int NC = p.nc;
+    const int ROLL_BOXES = 5 * NC, ROLL_STAGES = step_stages(NC);
+
+    // ---- one-time setup
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NSTAGE; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 1); }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(bar(B_D1FULL + i), 1);
+            mbar_init(bar(B_HREADY + i), 16);
+            mbar_init(bar(B_SFULL + i), 1);
+            mbar_init(bar(B_SEMPTY + i), 13);
+        }
+        mbar_init(bar(B_D2FULL), 1);
+        mbar_init(bar(B_ZREADY), 16);
+        mbar_init(bar(B_AFREE), 1);
+        mbar_init(bar(B_AREADY), 8);
+        fence_barrier_init();
+        fence_proxy_async();
+    }
+    if (warp == ALLOC_WARP) tmem_alloc2(s_base + L.tmem_slot, 512);
+    for (int i = threadIdx.x; i < p.hid; i += THREADS) s_b1[i] = __ldg(p.b1 + i);
+    for (int i = threadIdx.x; i < D; i += THREADS) {
+        s_b2[i] = __ldg(p.b2 + i);
+        s_gamma[i] = __ldg(p.gamma + i);
+        s_beta[i] = __ldg(p.beta + i);
+    }
+    {
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(p.E);
+        uint32_t* dst = reinterpret_cast<uint32_t*>(smem + L.e_tab);
+        for (int i = threadIdx.x; i < p.n_types * DA / 2; i += THREADS) dst[i] = __ldg(src + i);
+        // the hw K-block is only ever written in its first columns: clear it once so unread bytes are not NaNs
+        uint32_t* hwk = reinterpret_cast<uint32_t*>(smem + L.hwk);
+        for (int i = threadIdx.x; i < p.hw_ksteps * HWK_BYTES / 4; i += THREADS) hwk[i] = 0u;
+    }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();      // both CTAs' barriers are initialised before anyone arrives remotely / multicasts
+    tc_fence_after();
+    const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem + L.tmem_slot);
+    // EXT calls that store latents and rank nothing skip the scorer in every role
+    const bool rank_it = !EXT || p.a.scores_out != nullptr;
+    const uint32_t T_Z = tmem_base;                 // fp32 latent / GEMM2 accumulator, 256 columns
+    const uint32_t T_D1 = tmem_base + 256;          // two 128-column GEMM1 accumulators
+
+    if (warp == PROD_WARP) {
+        // =============================================================== tile schedule + TMA producer
+        uint32_t stage = 0, ph = 0;
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            int tile = tile_of((int)it, pair, n_pairs, p.n_tiles);
+            int nsteps = 0;
+            if (tile >= 0) {
+                for (int r = lane; r < TMP; r += 32) {
+                    int cand, len, seg;
+                    row_meta(p.a, (int64_t)tile * TMP + r, cand, len, seg, rank == 0);
+                    nsteps = max(nsteps, EXT ? len - row_start(p.a, cand, len) : len);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) nsteps = max(nsteps, __shfl_xor_sync(0xffffffffu, nsteps, o));
+            }
+            if (lane == 0) {
+                mbar_wait(bar(B_SEMPTY + slot), ((it >> 1) & 1) ^ 1);
+                s_sched[slot * 2 + 0] = tile;
+                s_sched[slot * 2 + 1] = nsteps;
+                mbar_arrive(bar(B_SFULL + slot));   // release semantics order the two stores before it
+            }
+            if (tile < 0) break;
+            if (lane == 0) {
+                // image row of box `b` of this CTA: boxes of the two CTAs alternate, 128 rows each
+                auto issue = [&](int nbox, int box0) {
+                    mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
+                    // the leader's barrier collects both CTAs' boxes of the stage
+                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2u * (uint32_t)nbox * BOX_BYTES);
+                    for (int b = 0; b < nbox; ++b)
+                        tma_load_2sm(s_ring + stage * STAGE_BYTES + b * BOX_BYTES, &tmap, 0,
+                                     128 * (2 * (box0 + b) + (int)rank), bar(B_FULL + stage));
+                    if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
+                };
+                for (int t = 0; t < nsteps; ++t) {
+                    int box = 0;
+                    for (int j = 0; j < ROLL_STAGES; ++j) {
+                        const int nb = stage_boxes(j, NC);
+                        issue(nb, box);
+                        box += nb;
+                    }
+                }
+                if (rank_it)
+                    for (int j = 0; j < SC_BOXES / 2; ++j) issue(2, ROLL_BOXES + 2 * j);
+            }
+            __syncwarp();
+        }
+    } else if (warp == MMA_WARP) {
+        // =============================================================== MMA issuer (leader CTA; the peer's warp only
+        // follows the schedule so that both CTAs' slot barriers have the same arrival count)
+        const uint32_t TZ = __reduce_max_sync(0xffffffffu, tmem_base);   // provably warp-uniform (uniform registers)
+        const uint32_t TD1 = TZ + 256;
+        uint32_t stage = 0, ph = 0;
+        uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
+        bool pend[2] = {false, false};
+        const uint32_t s_hwk = s_base + L.hwk;
+        auto wait_h = [&](int b) {
+            if (pend[b]) {
+                mbar_wait_cluster_warp(bar(B_HREADY + b), n_h[b] & 1);
+                ++n_h[b];
+                pend[b] = false;
+                tc_fence_after();
+            }
+        };
+        const uint32_t ring_lo0 = smem_desc_lo(s_ring);
+        uint32_t b_lo = ring_lo0;
+        bool ready = false;
+        auto acquire_stage = [&]() {       // returns with the current stage's data landed; probes the next stage
+            if (!ready) mbar_wait_warp(bar(B_FULL + stage), ph);
+            tc_fence_after();
+            const uint32_t nst = stage + 1 == NSTAGE ? 0u : stage + 1;
+            ready = __all_sync(0xffffffffu, mbar_test_wait(bar(B_FULL + nst), nst == 0 ? ph ^ 1u : ph));
+        };
+        auto advance = [&]() {
+            __syncwarp();
+            b_lo += STAGE_BYTES >> 4;
+            if (++stage == NSTAGE) { stage = 0; ph ^= 1; b_lo = ring_lo0; }
+        };
+        // one box against two A K-blocks (N = 128: the box holds this CTA's 64-row halves of two K-blocks): 8 MMAs
+        auto box_ss = [&](uint32_t d, uint32_t a_lo0, uint32_t a_lo1, uint32_t blo, bool first) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) mma_ss2(d, desc_of(a_lo0 + 2u * j), desc_of(blo + 2u * j), ID_N128, (first && j == 0) ? 0u : 1u);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) mma_ss2(d, desc_of(a_lo1 + 2u * j), desc_of(blo + (HALF_BYTES >> 4) + 2u * j), ID_N128, 1u);
+        };
+        const uint32_t a_lo = smem_desc_lo(s_a1);
+        constexpr uint32_t KBL = KB_BYTES >> 4, BXL = BOX_BYTES >> 4;
+        auto commit = [&](int barrier) {
+            if (elect_one()) mma_commit2(bar(barrier));
+            __syncwarp();
+        };
+        // stage: a K-blocks (4, 5) of chunk buffers 0 AND 1
+        auto stage_a01 = [&]() {
+            acquire_stage();
+            if (elect_one()) {
+                box_ss(TD1, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo, true);
+                box_ss(TD1 + 128u, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo + BXL, true);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // stage of ONE box: a / phi K-blocks (4, 5) into buffer b
+        auto stage_a = [&](int b) {
+            acquire_stage();
+            if (elect_one()) {
+                box_ss(TD1 + 128u * b, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo, true);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // stage: z K-blocks 0-3 into buffer b
+        auto stage_z = [&](int b) {
+            acquire_stage();
+            if (elect_one()) {
+                box_ss(TD1 + 128u * b, a_lo, a_lo + KBL, b_lo, false);
+                box_ss(TD1 + 128u * b, a_lo + 2 * KBL, a_lo + 3 * KBL, b_lo + BXL, false);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // stage: GEMM2 of hidden chunk buffer b (fp16 in TMEM: K-block 0 at +0, K-block 1 at +64 columns) x all 256
+        // latent columns: each box is this CTA's 128 weight rows of one [256 x 64] B tile, 4 MMAs with N = 256
+        auto stage_g2 = [&](int b) {
+            acquire_stage();
+            if (elect_one()) {
+                const uint32_t hbuf = TD1 + 128u * b;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) mma_ts2(TZ, hbuf + 8u * j, desc_of(b_lo + 2u * j), ID_N256, 1u);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) mma_ts2(TZ, hbuf + 64u + 8u * j, desc_of(b_lo + BXL + 2u * j), ID_N256, 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // scorer layer 1 stage: phi K-blocks (box 0) + the hw tile (first half of box 1; its second half is padding)
+        auto stage_phihw = [&](int b) {
+            acquire_stage();
+            if (elect_one()) {
+                box_ss(TD1 + 128u * b, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo, true);
+                for (int j = 0; j < p.hw_ksteps; ++j)
+                    mma_ss2(TD1 + 128u * b, smem_desc_nosw(s_hwk + j * HWK_BYTES), desc_of(b_lo + BXL + 2u * j), ID_N128, 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // scorer layer 2 stage: H1 K-blocks kb .. kb+3 (fp16 in TMEM columns [32 kb, ...)) into buffer b
+        auto stage_l2 = [&](int b, int kb) {
+            acquire_stage();
+            if (elect_one()) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        mma_ts2(TD1 + 128u * b, TZ + 32u * (kb + q) + 8u * j,
+                                desc_of(b_lo + (uint32_t)q * (HALF_BYTES >> 4) + 2u * j), ID_N128, (kb == 0 && q == 0 && j == 0) ? 0u : 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait_warp(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = __reduce_max_sync(0xffffffffu, (int)s_sched[slot * 2 + 0]);
+            const int nsteps = __reduce_max_sync(0xffffffffu, (int)s_sched[slot * 2 + 1]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            if (rank != 0) continue;
+#pragma unroll 1
+            for (int t = 0; t < nsteps; ++t) {
+                // Step boundary: the a K-blocks of chunks 0 and 1 depend only on a_{t+1} and both GEMM1 accumulators are
+                // free, so they are issued before the wait for z' (pipe drain + LayerNorm is the serial section of a step)
+                wait_h(0);
+                wait_h(1);
+                mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after();
+                stage_a01();
+                if (NC == 2) commit(B_AFREE);
+                mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after();
+                stage_z(0); commit(B_D1FULL + 0); pend[0] = true;
+                stage_z(1); commit(B_D1FULL + 1); pend[1] = true;
+                wait_h(0);
+                stage_g2(0);
+                if (NC == 1) commit(B_D2FULL);
+#pragma unroll 1
+                for (int i = 2; i <= NC; ++i) {
+                    if (i < NC) {                       // GEMM1 chunk i into buffer i & 1 (its GEMM2 reader has been issued)
+                        const int b = i & 1;
+                        wait_h(b);
+                        stage_a(b);
+                        if (i == NC - 1) commit(B_AFREE);
+                        stage_z(b);
+                        commit(B_D1FULL + b);
+                        pend[b] = true;
+                    }
+                    wait_h((i - 1) & 1);
+                    stage_g2((i - 1) & 1);              // GEMM2 chunk i - 1
+                    if (i == NC) commit(B_D2FULL);
+                }
+            }
+            if (!rank_it) {   // nothing to rank: only take the terminal latent's ZREADY so the phase count stays in step
+                mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1);
+                ++n_z;
+                continue;
+            }
+            // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
+#pragma unroll 1
+            for (int c = 0; c < 4; ++c) {
+                const int b = c & 1;
+                wait_h(b);
+                if (c == 0) { mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
+                stage_phihw(b);
+                if (c == 3) commit(B_AFREE);
+                if (c == 0) { mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
+                stage_z(b);
+                commit(B_D1FULL + b);
+                pend[b] = true;
+            }
+            wait_h(0);
+            wait_h(1);   // all of H1 (fp16, TMEM columns [0,256)) written
+            // ---- scorer layer 2: A = H1 from TMEM, K = 512
+#pragma unroll 1
+            for (int c = 0; c < 4; ++c) {
+                const int b = c & 1;
+                wait_h(b);
+                stage_l2(b, 0);
+                stage_l2(b, 4);
+                commit(B_D1FULL + b);
+                pend[b] = true;
+            }
+        }
+        __syncwarp();
+    }
+    else if (warp >= EPI_WARP0 && warp < ACT_WARP0) {
+        // =============================================================== epilogue warps (GELU / LayerNorm / scorer)
+        const int q = warp & 3, hh = (warp - EPI_WARP0) >> 2;
+        const int row = 32 * q + lane;
+        const uint32_t lane_off = (uint32_t)(32 * q) << 16;
+        uint8_t* a1 = smem + L.a1;
+        const uint32_t r_hready0 = mapa(bar(B_HREADY), 0), r_hready1 = mapa(bar(B_HREADY + 1), 0);
+        const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
+        uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
+        const float inv_d = 1.0f / (float)D;
+        // write 32 consecutive z columns of this row: fp32 -> TMEM, fp16 -> A1 (when `to_smem`)
+        auto put_z = [&](int col0, const uint32_t (&v)[32], bool to_smem) {
+            tmem_st32(T_Z + lane_off + (uint32_t)col0, v);
+            if (to_smem) {
+                uint8_t* kb = a1 + (col0 >> 6) * KB_BYTES;
+                const int chunk0 = (col0 & 63) >> 3;
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch) {
+                    uint4 o;
+                    o.x = pack_f16(__uint_as_float(v[8 * ch + 0]), __uint_as_float(v[8 * ch + 1]));
+                    o.y = pack_f16(__uint_as_float(v[8 * ch + 2]), __uint_as_float(v[8 * ch + 3]));
+                    o.z = pack_f16(__uint_as_float(v[8 * ch + 4]), __uint_as_float(v[8 * ch + 5]));
+                    o.w = pack_f16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
+                    *reinterpret_cast<uint4*>(kb + sw128_off(row, chunk0 + ch)) = o;
+                }
+            }
+        };
+        auto publish = [&](uint32_t leader_bar, bool smem_written) {
+            tmem_st_wait();
+            if (smem_written) fence_proxy_async();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(leader_bar);
+        };
+        // bias + GELU over this thread's 64 columns of accumulator buffer b, fp16 result to TMEM at dst_col
+        auto gelu_chunk = [&](int b, const float* bias, bool bias_in_smem, uint32_t dst_col) {
+            mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+            ++n_d1[b];
+            tc_fence_after();
+#pragma unroll
+            for (int p2 = 0; p2 < 2; ++p2) {
+                uint32_t v[32], o[16];
+                tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u * p2, v);
+                tmem_ld_wait();
+                const float4* bp_ = reinterpret_cast<const float4*>(bias + 32 * p2);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float4 bv = bias_in_smem ? bp_[i] : __ldg(bp_ + i);
+                    o[2 * i] = gelu2_f16(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                          make_float2(bv.x, bv.y));
+                    o[2 * i + 1] = gelu2_f16(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                              make_float2(bv.z, bv.w));
+                }
+                tmem_st16(dst_col + lane_off + 16u * p2, o);
+            }
+            publish(b == 0 ? r_hready0 : r_hready1, false);
+        };
+
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand, len, seg;
+            row_meta(p.a, (int64_t)tile * TMP + TM * (int)rank + row, cand, len, seg, false);
+            // prefix-latent reuse: the rollout covers positions [st, len) and starts from the row init_index names
+            const int st = EXT ? row_start(p.a, cand, len) : 0, rem = len - st;
+            const size_t zrow = EXT ? row_init(p.a, cand, seg) : (size_t)seg;
+
+            // ---- z_0 (the task's initial latent; or the banked latent after the first st steps)
+#pragma unroll 1
+            for (int p4 = 0; p4 < 4; ++p4) {
+                const int col0 = 128 * hh + 32 * p4;
+                uint32_t v[32];
+                if (cand >= 0) {
+                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + zrow * D + col0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 f = __ldg(src + i);
+                        v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
+                        v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) v[i] = 0u;
+                }
+                put_z(col0, v, true);
+            }
+            publish(r_zready, true);
+
+            for (int t = 0; t < nsteps; ++t) {
+                for (int c = 0; c < NC; ++c)
+                    gelu_chunk(c & 1, s_b1 + c * 128 + 64 * hh, true, T_D1 + 128u * (c & 1) + 64u * hh);
+                // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
+                mbar_wait(bar(B_D2FULL), n_d2 & 1);
+                ++n_d2;
+                tc_fence_after();
+                float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
+#pragma unroll 1
+                for (int p4 = 0; p4 < 4; ++p4) {
+                    const int col0 = 128 * hh + 32 * p4;
+                    uint32_t v[32];
+                    tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
+                    tmem_ld_wait();
+                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 bb = b2v[i];
+                        const float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                                     make_float2(bb.x, bb.y));
+                        const float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                                     make_float2(bb.z, bb.w));
+                        s1v = __fadd2_rn(s1v, __fadd2_rn(x0, x1));
+                        s2v = __ffma2_rn(x0, x0, s2v);
+                        s2v = __ffma2_rn(x1, x1, s2v);
+                    }
+                }
+                const float s1 = s1v.x + s1v.y, s2 = s2v.x + s2v.y;
+                // exchanged through the slot of this LayerNorm's parity: the partner reads the previous LayerNorm's value
+                // from the other slot, so no second barrier is needed before the next one writes
+                float2* red = s_red + (n_d2 & 1u) * 2 * TM;
+                red[hh * TM + row] = make_float2(s1, s2);
+                named_bar_sync(1 + q, 64);
+                const float2 other = red[(hh ^ 1) * TM + row];
+                const float mean = (s1 + other.x) * inv_d;
+                const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
+                const float rstd = rsqrtf(var + p.ln_eps);
+                const bool live = t < rem;     // masked steps leave the state unchanged
+                float4* lat = nullptr;     // wm_rollout_latents: z after this step (or only the terminal one: [B, d])
+                if (EXT && p.a.latents_out && live) {
+                    if (!p.a.latents_terminal)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + ((size_t)cand * p.a.T_max + st + t) * D);
+                    else if (st + t == len - 1)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + (size_t)cand * D);
+                }
+#pragma unroll 1
+                for (int p4 = 0; p4 < 4; ++p4) {
+                    const int col0 = 128 * hh + 32 * p4;
+                    uint32_t v[32];
+                    tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
+                    tmem_ld_wait();
+                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
+                    const float4* gv = reinterpret_cast<const float4*>(s_gamma + col0);
+                    const float4* bev = reinterpret_cast<const float4*>(s_beta + col0);
+                    const float2 rs2 = make_float2(rstd, rstd), mr2 = make_float2(-mean * rstd, -mean * rstd);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 bb = b2v[i], gg = gv[i], be = bev[i];
+                        float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
+                                               make_float2(bb.x, bb.y));
+                        float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
+                                               make_float2(bb.z, bb.w));
+                        x0 = __ffma2_rn(__ffma2_rn(x0, rs2, mr2), make_float2(gg.x, gg.y), make_float2(be.x, be.y));
+                        x1 = __ffma2_rn(__ffma2_rn(x1, rs2, mr2), make_float2(gg.z, gg.w), make_float2(be.z, be.w));
+                        v[4 * i] = __float_as_uint(x0.x); v[4 * i + 1] = __float_as_uint(x0.y);
+                        v[4 * i + 2] = __float_as_uint(x1.x); v[4 * i + 3] = __float_as_uint(x1.y);
+                    }
+                    // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
+                    // fp32 master is never read again
+                    put_z(col0, v, live);
+                    if (lat) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+                            lat[(col0 >> 2) + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                                                               __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+                    }
+                }
+                publish(r_zready, true);
+            }
+
+            if (!rank_it) continue;
+            // ---- scorer layer 1 -> H1 (fp16) in TMEM columns [0,256)
+            for (int c = 0; c < 4; ++c)
+                gelu_chunk(c & 1, p.bs0 + c * 128 + 64 * hh, false, T_Z + 64u * c + 32u * hh);
+            // ---- scorer layer 2 + output dot product
+            float part = 0.0f;
+            for (int c = 0; c < 4; ++c) {
+                const int b = c & 1;
+                mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+                ++n_d1[b];
+                tc_fence_after();
+#pragma unroll
+                for (int p2 = 0; p2 < 2; ++p2) {
+                    uint32_t v[32];
+                    tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u * p2, v);
+                    tmem_ld_wait();
+                    const int n0 = c * 128 + 64 * hh + 32 * p2;
+#pragma unroll
+                    for (int i = 0; i < 32; ++i)
+                        part = fmaf(gelu_fast(__uint_as_float(v[i]) + __ldg(p.bs1 + n0 + i)), __ldg(p.w3 + n0 + i), part);
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(b == 0 ? r_hready0 : r_hready1);
+            }
+            s_red[hh * TM + row] = make_float2(part, 0.0f);
+            named_bar_sync(1 + q, 64);
+            if (hh == 0 && cand >= 0 && (!EXT || p.a.scores_out)) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
+            named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
+        }
+    } else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
+        // =============================================================== action-embedding warps
+        const int aw = warp - ACT_WARP0;
+        const int row = 32 * aw + lane;       // row-mapped phases
+        const int col4 = 4 * lane;            // column-mapped phases: this lane's 4 embedding columns
+        uint8_t* a1 = smem + L.a1;
+        const uint8_t* s_E = smem + L.e_tab;
+        float* s_lp = reinterpret_cast<float*>(smem + L.lp);
+        int* s_ids = reinterpret_cast<int*>(smem + L.ids);
+        uint8_t* s_cnt = smem + L.cnt;
+        const uint32_t r_aready = mapa(bar(B_AREADY), 0);
+        const int P = p.P, NT = p.n_types;
+        float wp[MAX_P][4], bp4[4];
+#pragma unroll
+        for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) wp[j][e] = j < P ? __ldg(p.WpT + j * DA + col4 + e) : 0.0f;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) bp4[e] = __ldg(p.bp + col4 + e);
+        uint32_t n_w = 0;
+        // A1 destination of this lane's 4 columns (8 bytes) in row r: K-block 4 + lane/16
+        auto a_dst = [&](int r) -> uint2* {
+            return reinterpret_cast<uint2*>(a1 + (4 + (lane >> 4)) * KB_BYTES + sw128_off(r, (lane & 15) >> 1) +
+                                            (lane & 1) * 8);
+        };
+        for (uint32_t it = 0;; ++it) {
+            const uint32_t slot = it & 1;
+            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
+            if (tile < 0) break;
+            int cand, len, seg;
+            row_meta(p.a, (int64_t)tile * TMP + TM * (int)rank + row, cand, len, seg, false);
+            for (int c = 0; c < NT; ++c) s_cnt[row * NT + c] = 0;
+            float slp[MAX_P];   // per parameter slot: running sum of log2 p
+#pragma unroll
+            for (int j = 0; j < MAX_P; ++j) slp[j] = 0.0f;
+            // structured phi: the per-slot running maximum lives in shared memory (the registers of this role are full)
+            float4* s_mx4 = reinterpret_cast<float4*>(smem + L.mx) + row * (MAX_P / 4);
+            if (PHI == WM_PHI_STRUCT) s_mx4[0] = s_mx4[1] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            // one action of this row: type id (clamped), log2 of its parameters, phi statistics
+            auto account = [&](int id, const int (&raw)[MAX_P], float (&lp)[MAX_P]) -> int {
+                if (id < 0 || id >= NT) {
+                    atomicOr(p.a.fault, WM_FAULT_TYPE);
+                    id = id < 0 ? 0 : NT - 1;
+                }
+#pragma unroll
+                for (int j = 0; j < MAX_P; ++j) {
+                    if (j < P) {
+                        int prm = raw[j];
+                        if (prm < 1) {
+                            atomicOr(p.a.fault, WM_FAULT_PARAM);
+                            prm = 1;
+                        }
+                        lp[j] = log2f((float)prm);
+                        slp[j] += lp[j];
+                    }
+                }
+                s_cnt[row * NT + id] += 1;
+                if (PHI == WM_PHI_STRUCT) {
+                    float4 m0 = s_mx4[0], m1 = s_mx4[1];
+                    m0.x = fmaxf(m0.x, lp[0]); m0.y = fmaxf(m0.y, lp[1]); m0.z = fmaxf(m0.z, lp[2]); m0.w = fmaxf(m0.w, lp[3]);
+                    m1.x = fmaxf(m1.x, lp[4]); m1.y = fmaxf(m1.y, lp[5]); m1.z = fmaxf(m1.z, lp[6]); m1.w = fmaxf(m1.w, lp[7]);
+                    s_mx4[0] = m0; s_mx4[1] = m1;
+                }
+                return id;
+            };
+            auto take = [&](int pos, float (&lp)[MAX_P]) -> int {   // the action at position `pos`
+                const int id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos);
+                const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P;
+                int raw[MAX_P];
+#pragma unroll
+                for (int j = 0; j < MAX_P; ++j) raw[j] = j < P ? __ldg(pp + j) : 1;
+                return account(id, raw, lp);
+            };
+            // prefix-latent reuse: positions [0, st) only feed phi; scanned four at a time BEFORE the first rollout step, in
+            // position order, so the running sums see the positions in the literal call's order (bit-identical scores)
+            const int st = EXT ? row_start(p.a, cand, len) : 0;
+            int scanned = 0;
+            auto scan4 = [&]() {
+                int rid[4], raw[4][MAX_P];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int pos = scanned + u < st ? scanned + u : 0;      // (in-bounds dummy for finished lanes)
+                    rid[u] = cand >= 0 ? __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos) : 0;
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+                        raw[u][j] = (cand >= 0 && j < P)
+                                        ? __ldg(p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P + j) : 1;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (scanned + u < st) {
+                        float lp[MAX_P];
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                        account(rid[u], raw[u], lp);
+                    }
+                scanned += 4;
+            };
+            if (EXT && p.a.start)
+                while (__any_sync(0xffffffffu, scanned < st)) scan4();
+
+            for (int t = 0; t < nsteps; ++t) {
+                // phase 1 (one row per lane): read the step's action, log2 of its parameters, phi statistics
+                int id = -1;
+                float lp[MAX_P];
+#pragma unroll
+                for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                if (st + t < len) id = take(st + t, lp);
+                s_ids[row] = id;
+                *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
+                *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
+                __syncwarp();
+                // phase 2 (4 columns per lane, loop over the warp's 32 rows): a = E[id] + W_p log2(p) + b_p.  The first
+                // PRE rows are computed into registers BEFORE the wait below, the rest after it.
+                constexpr int PRE = 16;
+                uint2 pk[PRE];
+                auto a_row = [&](int r) -> uint2 {
+                    const int idr = s_ids[r];
+                    float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+                    if (idr >= 0) {
+                        const uint2 e = *reinterpret_cast<const uint2*>(s_E + ((size_t)idr * DA + col4) * 2);
+                        a4[0] = __uint_as_float(e.x << 16) + bp4[0];
+                        a4[1] = __uint_as_float(e.x & 0xffff0000u) + bp4[1];
+                        a4[2] = __uint_as_float(e.y << 16) + bp4[2];
+                        a4[3] = __uint_as_float(e.y & 0xffff0000u) + bp4[3];
+                        const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
+                        const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
+                        const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j)
+#pragma unroll
+                            for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
+                    }
+                    return make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+                };
+#pragma unroll
+                for (int rr = 0; rr < PRE; ++rr) pk[rr] = a_row(32 * aw + rr);
+                // store only once GEMM1 of the previous step no longer reads the a-part of A1
+                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+                ++n_w;
+#pragma unroll
+                for (int rr = 0; rr < PRE; ++rr) *a_dst(32 * aw + rr) = pk[rr];
+#pragma unroll 4
+                for (int rr = PRE; rr < 32; ++rr) {
+                    const int r = 32 * aw + rr;
+                    *a_dst(r) = a_row(r);
+                }
+                fence_proxy_async();
+                __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
+                if (lane == 0) mbar_arrive_cluster(r_aready);
+            }
+
+            // ---- the phi K-blocks of the scorer's A operand, one ROW per lane (see wm_tc_kernel): psi for WM_PHI_MEAN
+            // (the host folds E, W_p, b_p into scorer layer 1), the statistics themselves for WM_PHI_STRUCT
+            if (!rank_it) continue;
+            if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+            ++n_w;
+            {
+                auto put = [&](int c, float v) {
+                    *reinterpret_cast<uint16_t*>(a1 + (4 + (c >> 6)) * KB_BYTES + sw128_off(row, (c & 63) >> 3) +
+                                                 (c & 7) * 2) = (uint16_t)pack_f16(v, 0.0f);
+                };
+#pragma unroll
+                for (int ch = 0; ch < 16; ++ch)
+                    *reinterpret_cast<uint4*>(a1 + (4 + (ch >> 3)) * KB_BYTES + sw128_off(row, ch & 7)) =
+                        make_uint4(0u, 0u, 0u, 0u);
+                const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
+                if (PHI == WM_PHI_STRUCT) {
+                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c]);
+                    put(NT, (float)len);
+                    const float4 m0 = s_mx4[0], m1 = s_mx4[1];
+                    const float mxr[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) {
+                            put(NT + 1 + j, slp[j]);
+                            put(NT + 1 + P + j, slp[j] * inv);
+                            put(NT + 1 + 2 * P + j, mxr[j]);
+                        }
+                } else {
+                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c] * inv);
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) put(NT + j, slp[j] * inv);
+                    put(NT + P, len > 0 ? 1.0f : 0.0f);
+                }
+            }
+            // hardware features of this row -> the hw operand tile (columns >= H stay zero)
+            for (int ch = 0; ch < p.H / 8; ++ch) {
+                uint4 o = make_uint4(0u, 0u, 0u, 0u);
+                if (cand >= 0 && (!EXT || p.a.hw_feats)) {
+                    const float4* src = reinterpret_cast<const float4*>(p.a.hw_feats + (size_t)seg * p.H + 8 * ch);
+                    const float4 f0 = __ldg(src), f1 = __ldg(src + 1);
+                    o.x = pack_f16(f0.x, f0.y); o.y = pack_f16(f0.z, f0.w);
+                    o.z = pack_f16(f1.x, f1.y); o.w = pack_f16(f1.z, f1.w);
+                }
+                // K-step ch/2, K half ch&1 of the no-swizzle tile (see smem_desc_nosw)
+                *reinterpret_cast<uint4*>(smem + L.hwk + (ch >> 1) * HWK_BYTES + (row >> 3) * 256 + (ch & 1) * 128 +
+                                          (row & 7) * 16) = o;
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(r_aready);
+        }
+    }
+
+    // ---- teardown: no CTA of the pair may exit (or free TMEM) while the other's MMAs / arrivals can still reach it
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == ALLOC_WARP) tmem_dealloc2(tmem_base, 512);
+}
+
+}  // namespace tcp
+
+// ------------------------------------------------------------------------------------------------ host side
+namespace {
+
+// Append one pair box: for each CTA (rank 0, then rank 1) 128 image rows of 128 B.
+//   n128 = true : two N = 128 K-block halves per CTA: rows [0,64) = W[n0 + 64 r + n][k0 + k], rows [64,128) the same weight
+//                 rows at k0 + 64 (K-blocks k0/64 and k0/64 + 1); kvalid counts valid columns from k0 (the rest is zero)
+//   n128 = false: one N = 256 K-block half per CTA: rows [0,128) = W[n0 + 128 r + n][k0 + k]
+// Each 64-row (or 128-row) block is a SW128 K-major tile: row n at n * 128 B, 16-byte chunk c at (c ^ (n & 7)).
+// Returns false when a weight is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
+bool append_box(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid, bool n128) {
+    const size_t base = blob.size();
+    blob.resize(base + 2 * tcp::BOX_BYTES / 2, 0);
+    bool ok = true;
+    for (int r = 0; r < 2; ++r)
+        for (int row = 0; row < 128; ++row)
+            for (int k = 0; k < 64; ++k) {
+                int n, kk;
+                if (n128) { n = n0 + 64 * r + (row & 63); kk = (row >> 6) * 64 + k; }
+                else { n = n0 + 128 * r + row; kk = k; }
+                const float v = kk < kvalid ? W[(size_t)n * ld + k0 + kk] : 0.0f;
+                const int tr = n128 ? (row & 63) : row;     // row inside its SW128 tile
+                const size_t off = (size_t)r * tcp::BOX_BYTES + (size_t)row * 128 + (size_t)((((k >> 3) ^ (tr & 7)) << 4)) +
+                                   (size_t)(k & 7) * 2;
+                uint16_t hb;
+                ok &= f32_to_f16_bits(v, &hb);
+                blob[base + off / 2] = hb;
+            }
+    return ok;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+bool tcp_model_ok(const Model& m) {
+    return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tcp::D &&
+           m.d_a == tcp::DA && m.hidden >= 256 && m.hidden <= tcp::MAX_HID && m.hidden % 128 == 0 &&
+           ((m.n_lin == 3 && m.sdim[1] == tcp::SW && m.sdim[2] == tcp::SW) || m.ranker_kind == WM_RANKER_FOREST) &&
+           m.H >= 8 && m.H <= tcp::MAX_H && m.H % 8 == 0 && m.n_types <= tcp::MAX_TYPES && m.P <= tcp::MAX_P;
+}
+
+int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
+    Model& m = ctx->m;
+    m.tcp_ok = 0;
+    if (!tcp_model_ok(m)) return WM_OK;
+    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT);
+    if ((int)L.total > ctx->smem_optin) return WM_OK;
+    auto get = [&](const char* n) -> const std::vector<float>& {
+        for (size_t i = 0; i < names.size(); ++i)
+            if (names[i] == n) return hv[i];
+        static const std::vector<float> empty;
+        return empty;
+    };
+    const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1");
+    const int hid = m.hidden, NC = hid / 128, K1 = tcp::D + tcp::DA;
+    const int F = m.phi_dim, K0 = tcp::D + F + m.H;   // scorer input [z ; phi (F <= 128 columns) ; hw]
+    const size_t n_boxes = (size_t)5 * NC + tcp::SC_BOXES;
+    std::vector<uint16_t> blob;
+    bool ok = true;   // every weight finite in fp16
+    blob.reserve(n_boxes * tcp::BOX_BYTES);
+    // the MMA warp's order (tcp::stage_boxes): a K-blocks (4, 5) of chunks 0 and 1, z K-blocks (0-3) of chunk 0, of chunk 1,
+    // GEMM2 chunk 0, then per chunk i >= 2: a, z, GEMM2 chunk i - 1; last GEMM2 chunk NC - 1
+    auto g1a = [&](int c) { ok &= append_box(blob, W1, K1, c * 128, 4 * 64, 128, true); };
+    auto g1z = [&](int c) {
+        ok &= append_box(blob, W1, K1, c * 128, 0, 128, true);
+        ok &= append_box(blob, W1, K1, c * 128, 128, 128, true);
+    };
+    auto g2 = [&](int c) {            // GEMM2 chunk c: the chunk's two hidden K-blocks x all 256 latent columns
+        ok &= append_box(blob, W2, hid, 0, c * 128, 64, false);
+        ok &= append_box(blob, W2, hid, 0, c * 128 + 64, 64, false);
+    };
+    g1a(0); g1a(1); g1z(0); g1z(1);
+    g2(0);
+    for (int i = 2; i <= NC; ++i) {
+        if (i < NC) { g1a(i); g1z(i); }
+        g2(i - 1);
+    }
+    // phi weights of scorer layer 1 as the kernel's phi K-blocks see them, [SW][128] (see wm_tc.cu tc_prepare)
+    const bool forest = m.ranker_kind == WM_RANKER_FOREST;
+    std::vector<float> Wphi((size_t)tcp::SW * 128, 0.0f);
+    if (forest) {
+    } else if (m.phi_kind == WM_PHI_STRUCT) {
+        for (int n = 0; n < tcp::SW; ++n)
+            for (int c = 0; c < F; ++c) Wphi[(size_t)n * 128 + c] = Ws0[(size_t)n * K0 + tcp::D + c];
+    } else {
+        const std::vector<float>&E = get("E"), &Wp = get("W_p"), &bpv = get("b_p");
+        for (int n = 0; n < tcp::SW; ++n) {
+            const float* wr = &Ws0[(size_t)n * K0 + tcp::D];
+            for (int c = 0; c < m.n_types; ++c) {
+                double acc = 0.0;
+                for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tcp::DA + k];
+                Wphi[(size_t)n * 128 + c] = (float)acc;
+            }
+            for (int j = 0; j < m.P; ++j) {
+                double acc = 0.0;
+                for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * m.P + j];
+                Wphi[(size_t)n * 128 + m.n_types + j] = (float)acc;
+            }
+            double acc = 0.0;
+            for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * bpv[k];
+            Wphi[(size_t)n * 128 + m.n_types + m.P] = (float)acc;
+        }
+    }
+    std::vector<float> zero1(1, 0.0f);
+    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2 K-blocks), hw + zero padding, z (4 K-blocks)
+        ok &= append_box(blob, Wphi, 128, c * 128, 0, forest ? 0 : 128, true);
+        ok &= append_box(blob, Ws0, K0, c * 128, tcp::D + F, forest ? 0 : m.H, true);
+        ok &= append_box(blob, Ws0, K0, c * 128, 0, forest ? 0 : 128, true);
+        ok &= append_box(blob, Ws0, K0, c * 128, 128, forest ? 0 : 128, true);
+    }
+    for (int c = 0; c < 4; ++c)       // scorer layer 2: K = 512 = 8 K-blocks = 4 boxes
+        for (int kb = 0; kb < 8; kb += 2) ok &= append_box(blob, Ws1, tcp::SW, c * 128, kb * 64, forest ? 0 : 128, true);
+    if (blob.size() * 2 != n_boxes * 2 * tcp::BOX_BYTES) {
+        set_error("tcp_prepare: internal weight-image size mismatch");
+        return WM_ERR_FORMAT;
+    }
+    if (!ok) return WM_OK;   // a weight beyond the fp16 range: this model stays on the fp32 kernel
+
+    void* d_blob = nullptr;
+    WM_CUDA_TRY(cudaMalloc(&d_blob, blob.size() * 2));
+    ctx->allocs.push_back(d_blob);
+    WM_CUDA_TRY(cudaMemcpy(d_blob, blob.data(), blob.size() * 2, cudaMemcpyHostToDevice));
+
+    // tensor map over the image seen as rows of 64 16-bit values (128 B); one box = 128 rows.  The image is already
+    // swizzled, so the map itself uses no swizzle.
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    WM_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
+    if (!fn || qr != cudaDriverEntryPointSuccess) {
+        set_error("tcp_prepare: cuTensorMapEncodeTiled is not available from this driver");
+        return WM_ERR_CUDA;
+    }
+    static_assert(sizeof(CUtensorMap) <= sizeof(m.tcp_tmap), "tensor map storage");
+    CUtensorMap tm;
+    const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
+    const cuuint64_t strides[1] = {128};
+    const cuuint32_t box[2] = {64, 128}, es[2] = {1, 1};
+    const CUresult r = ((EncodeTiledFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_blob, dims, strides, box, es,
+                                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("tcp_prepare: cuTensorMapEncodeTiled failed (%d)", (int)r);
+        return WM_ERR_CUDA;
+    }
+    memcpy(m.tcp_tmap, &tm, sizeof(tm));
+    if (m.phi_kind == WM_PHI_STRUCT) {
+        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_STRUCT, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_STRUCT, true>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    } else {
+        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_MEAN, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_MEAN, true>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    }
+    m.tcp_ok = 1;
+    return WM_OK;
+}
+
+int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
+    (void)ws;
+    const Model& m = ctx->m;
+    tcp::Params p;
+    p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
+    p.hw_ksteps = (m.H + 15) / 16;
+    p.ln_eps = m.ln_eps;
+    p.E = static_cast<const __nv_bfloat16*>(m.tc_E);
+    p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
+    if (m.ranker_kind == WM_RANKER_FOREST) p.bs0 = p.bs1 = p.w3 = p.bs2 = m.zeros;   // (unused scorer, zero image)
+    p.a = a;
+    p.n_tiles = (int)((a.B + tcp::TMP - 1) / tcp::TMP);
+    CUtensorMap tm;
+    memcpy(&tm, m.tcp_tmap, sizeof(tm));
+    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, m.hidden, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
+    const int max_pairs = ctx->n_sms / 2;
+    const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
+    const bool prefix_call = a.start || a.init_index || a.latents_out;
+    if (m.phi_kind == WM_PHI_STRUCT) {
+        if (prefix_call) tcp::wm_tcp_kernel<WM_PHI_STRUCT, true><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
+        else tcp::wm_tcp_kernel<WM_PHI_STRUCT, false><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
+    } else {
+        if (prefix_call) tcp::wm_tcp_kernel<WM_PHI_MEAN, true><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
+        else tcp::wm_tcp_kernel<WM_PHI_MEAN, false><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
+    }
+    WM_CUDA_TRY(cudaGetLastError());
+    ctx->launches.fetch_add(1);
+    return WM_OK;
+}
+
+}  // namespace wm

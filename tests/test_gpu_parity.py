@@ -400,14 +400,14 @@ def test_full_size_against_full_oracle(wm, n, n_sub):
 
 @pytest.mark.parametrize("n", [11, 12])
 def test_full_size_forest_against_full_oracle(wm, n):
-    """The tree-ensemble ranker (f4) at cfg 2's full batch and real density (64 of 2048).  The bar the forest can hold
-    on the bf16 path is NOT north_star's 0.95: a 1e-3 error in the terminal latent moves a candidate across a split
-    whenever its latent sits within that distance of one of the ~768 thresholds on its paths (6 levels x 128 trees),
-    which changes its score by a leaf difference, not by 1e-3 — the score is discontinuous in z.  What is asserted:
-    every candidate that provably cannot have flipped carries the oracle's score (margin-aware, _forest_parity), and
-    the top-64-of-2048 overlap stays >= 0.75 on the tcgen05 path (>= 0.95 on the fp32 path, whose latent error is 1e-6)."""
+    """The tree-ensemble ranker (f4) at cfg 2's full batch and real density (64 of 2048).  The SCORE of a forest is
+    discontinuous in z (a 1e-3 error in the terminal latent flips a branch whenever the latent sits that close to one of
+    the ~768 thresholds on a candidate's paths, and the score then moves by a leaf difference), so scores are compared
+    margin-aware (_forest_parity: every candidate that provably cannot have flipped carries the oracle's score).  The
+    RANKING still meets north_star's bar: mean top-64-of-2048 overlap >= 0.95 on both paths (measured 0.987 / 0.999 on
+    the tcgen05 path for configs 11 / 12, 1.000 on the fp32 path)."""
     cfg = gen.get_config(n)
-    res = _forest_parity(wm, cfg, gen.make_weights(cfg), gen.make_inputs(cfg), min_clear=0.9, min_safe=0.9, min_overlap=0.75)
+    res = _forest_parity(wm, cfg, gen.make_weights(cfg), gen.make_inputs(cfg), min_clear=0.9, min_safe=0.9, min_overlap=0.95)
     print(f"full-size forest parity cfg {n}: " + ", ".join(f"path {k}: compared {v[0]:.3f}, overlap {v[1]:.4f}" for k, v in res.items()))
 
 
