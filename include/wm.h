@@ -87,6 +87,9 @@ extern "C" {
 #define WM_OPT_TIMING    3      /* 1 = record CUDA events around the rollout+score kernel (K2) of every call,   */
                                 /*     read back with wm_last_kernel_ms; 0 = off (default)                      */
 
+#define WM_OPT_PAIR      4      /* d = 256 MLP+LayerNorm models: 1 = the CTA-pair form wm_tcp_kernel (256-candidate tiles,  */
+                                /*     tcgen05.mma.cta_group::2, default), 0 = wm_tc_kernel (one CTA per 128-candidate tile) */
+
 typedef struct wm_ctx wm_ctx;   /* opaque: device weights (all layouts the kernels need) + workspace pool      */
 
 typedef struct wm_info {        /* model hyper-parameters, as read from the weight-file header                 */
@@ -99,7 +102,8 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
     int32_t tc_variant;         /* tcgen05 kernel built for this model: 0 = none, 1 = wm_tc_kernel (one CTA per  */
                                 /* 128-candidate tile, d = 256), 2 = wm_tc2_kernel (CTA pair per tile, d = 512),  */
                                 /* 3 = wm_tcg_kernel (CTA pair per tile, GRU transition, d = 384),             */
-                                /* 4 = wm_tct_kernel (TransH transition, d = 256)                              */
+                                /* 4 = wm_tct_kernel (TransH transition, d = 256), 5 = wm_tcp_kernel (CTA pair  */
+                                /* per 256-candidate tile, d = 256: the default form of variant 1, WM_OPT_PAIR) */
     int32_t phi_kind;           /* WM_PHI_*: which action features G reads                                     */
     int32_t ranker_kind;        /* WM_RANKER_*                                                                 */
     int32_t n_trees, tree_depth;   /* WM_RANKER_FOREST only                                                    */

@@ -60,6 +60,8 @@ struct Model {
     void* tc_E = nullptr;      // bf16 [n_types][d_a]
     int tc_ok = 0;             // 0 = no tcgen05 path, 1 = wm_tc_kernel (one CTA per tile), 2 = wm_tc2_kernel (CTA pair), 3 = wm_tcg_kernel (CTA pair, GRU), 4 = wm_tct_kernel (TransH)
     alignas(64) unsigned char tc2_tmap[128] = {};   // CUtensorMap over tc_blob (pair kernel)
+    int tcp_ok = 0;            // 1 = wm_tcp_kernel (the CTA-pair, M = 256 form of wm_tc_kernel) is built for this model too
+    alignas(64) unsigned char tcp_tmap[128] = {};   // CUtensorMap over wm_tcp_kernel's own weight image
 };
 
 // NVTX range around an ABI call (header-only NVTX 3: a no-op unless a profiler injects itself)
@@ -105,6 +107,7 @@ struct wm_ctx {
     int opt_path = 0;     // WM_OPT_PATH
     int opt_sort = 1;     // WM_OPT_SORT
     int opt_timing = 0;   // WM_OPT_TIMING
+    int opt_pair = 1;     // WM_OPT_PAIR
     uint32_t* fault = nullptr;   // device fault word
     std::mutex mu;
     std::vector<wm::Workspace*> pool;
@@ -193,6 +196,12 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
                 const std::vector<std::string>& names);
 int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
+
+// K2 tcgen05, CTA pair with M = 256 (wm_tcp.cu): the pair form of wm_tc_kernel, same models.  Prepared after tc_prepare
+// succeeds; launch_tc dispatches to it unless WM_OPT_PAIR = 0.
+int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
+                const std::vector<std::string>& names);
+int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 
 // K2 tcgen05, CTA pair, gated (wm_tcg.cu): bf16 GRU models with d = 384 and the bucket table.  Same entry route.
 int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,

@@ -978,7 +978,7 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
     }
     m.tc_ok = 1;
-    return WM_OK;
+    return tcp_prepare(ctx, hv, names);   // the pair form (wm_tcp_kernel) of the same model, taken by default when built
 }
 
 int tc_supported(const wm_ctx* ctx) { return ctx->m.tc_ok; }
@@ -1005,6 +1005,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     if (m.tc_ok == 2) return launch_tc2(ctx, ws, a, st);
     if (m.tc_ok == 3) return launch_tcg(ctx, ws, a, st);
     if (m.tc_ok == 4) return launch_tct(ctx, ws, a, st);
+    if (m.tcp_ok && ctx->opt_pair) return launch_tcp(ctx, ws, a, st);
     tc::Params p;
     p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;

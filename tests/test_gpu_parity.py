@@ -36,18 +36,27 @@ def wm():
     return wm
 
 
+PATH_TC_SINGLE = 12     # test-only path id: tcgen05 forced, single-CTA form (WM_OPT_PAIR = 0) of a model whose default is the pair form
+
+
 def _ctx(wm, cfg, path=None):
     ctx = wm.wm_load_weights(weight_file(cfg))
-    if path is not None:
+    if path == PATH_TC_SINGLE:
+        wm.wm_set_option(ctx, wm.WM_OPT_PATH, wm.PATH_TCGEN05)
+        wm.wm_set_option(ctx, wm.WM_OPT_PAIR, 0)
+        assert wm.wm_get_info(ctx).tc_variant == 1
+    elif path is not None:
         wm.wm_set_option(ctx, wm.WM_OPT_PATH, path)
     return ctx
 
 
 def _paths(wm, cfg):
+    """Every GPU implementation of this model: the fp32 kernel, the kernel the automatic policy picks and, for the d = 256
+    MLP+LayerNorm models (default: the pair form, tc_variant 5), the single-CTA form as well."""
     ctx = wm.wm_load_weights(weight_file(cfg))
-    auto = wm.wm_get_info(ctx).path
+    info = wm.wm_get_info(ctx)
     wm.wm_free(ctx)
-    return sorted({wm.PATH_FP32, auto})
+    return sorted({wm.PATH_FP32, info.path} | ({PATH_TC_SINGLE} if info.tc_variant == 5 else set()))
 
 
 @pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9])
@@ -441,20 +450,23 @@ def test_outputs_do_not_overrun(wm, n):
         assert (hi[:pad] == -77).all() and (hi[pad + S * k:] == -77).all(), (n, path)
 
 
-@pytest.mark.parametrize("n", [2, 3, 5, 7, 9, 11, 12])
+@pytest.mark.parametrize("n", [2, 3, 4, 5, 7, 9, 11, 12])
 def test_repeatable_bitwise_with_several_tiles_per_cta(wm, n):
     """A batch large enough that every persistent CTA (or CTA pair) walks several tiles, scored three times: the
     scores must be bit-identical.  Barrier phase counters that do not survive a tile boundary, or a wait that passes
     on a stale phase, show up as run-to-run differences long before they exceed the parity tolerance."""
-    cfg = gen.get_config(n).scaled(S=10, per_subgraph=2048 if n != 5 else 2047)
+    cfg = gen.get_config(n).scaled(S=10 if n != 4 else 40, per_subgraph=2048 if n != 5 else 2047)
     b = gen.make_inputs(cfg)
-    ctx = _ctx(wm, cfg)
-    assert wm.wm_get_info(ctx).path == wm.PATH_TCGEN05
-    y0 = gpu_scores(ctx, b)
-    for _ in range(2):
-        np.testing.assert_array_equal(gpu_scores(ctx, b).view(np.uint32), y0.view(np.uint32))
-    wm.wm_free(ctx)
-    assert np.isfinite(y0).all()
+    for path in _paths(wm, cfg):
+        if path == wm.PATH_FP32:
+            continue
+        ctx = _ctx(wm, cfg, path)
+        assert wm.wm_get_info(ctx).path == wm.PATH_TCGEN05
+        y0 = gpu_scores(ctx, b)
+        for _ in range(2):
+            np.testing.assert_array_equal(gpu_scores(ctx, b).view(np.uint32), y0.view(np.uint32))
+        wm.wm_free(ctx)
+        assert np.isfinite(y0).all()
 
 
 @pytest.mark.parametrize("n", [8, 9])
@@ -486,7 +498,7 @@ def test_struct_phi_feature_readout(wm, n):
             np.testing.assert_array_equal(y, b.hw_feats[seg, 0])
 
 
-PREFIX_TC_VARIANTS = (1,)       # (the TransH kernel, variant 4, takes wm_rollout_latents only)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
+PREFIX_TC_VARIANTS = (1, 5)       # (the TransH kernel, variant 4, takes wm_rollout_latents only)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
 
 
 def _prefix_case(n, S, per):
@@ -496,7 +508,7 @@ def _prefix_case(n, S, per):
 
 def _prefix_unsupported(wm, ctx, path, call, variants=None):
     """True (after checking the error code) when `path` is a forced tcgen05 kernel without prefix-reuse support."""
-    if path != wm.PATH_TCGEN05 or wm.wm_get_info(ctx).tc_variant in (variants or PREFIX_TC_VARIANTS):
+    if path not in (wm.PATH_TCGEN05, PATH_TC_SINGLE) or wm.wm_get_info(ctx).tc_variant in (variants or PREFIX_TC_VARIANTS):
         return False
     with pytest.raises(wm.WmError) as e:
         call()
@@ -520,7 +532,7 @@ def test_rollout_latents_match_oracle(wm, n):
         out = torch.full((b.B, cfg.T_max, cfg.d), -777.0, dtype=torch.float32, device="cuda:0")
         call = lambda: wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"],
                                              dv["lengths"], out, dv["subgraph_offsets"])
-        if _prefix_unsupported(wm, ctx, path, call, variants=(1, 4)):
+        if _prefix_unsupported(wm, ctx, path, call, variants=(1, 4, 5)):
             continue
         call()
         assert wm.wm_check(ctx) == 0
@@ -571,7 +583,8 @@ def test_score_from_bank_matches_literal(wm, n):
         assert oracle.score_error(y, lit, b.subgraph_offsets) <= 2e-5, (n, path)
 
 
-def test_cfg4_prefix_reuse_full_family_structure(wm):
+@pytest.mark.parametrize("form", [None, PATH_TC_SINGLE])
+def test_cfg4_prefix_reuse_full_family_structure(wm, form):
     """cfg 4's shared-prefix structure used the way a search loop would (bench.py --prefix-reuse): one representative per
     family rolled over the copied prefix with every latent banked, every child scored from its cut.  Scores must equal the
     literal call's (fp32 rounding of nothing: the bank holds the very latent the literal rollout carries) and the top-k
@@ -580,8 +593,8 @@ def test_cfg4_prefix_reuse_full_family_structure(wm):
     cfg = gen.get_config(4).scaled(S=3, per_subgraph=1024)
     b = gen.make_inputs(cfg)
     C, T = cfg.prefix_children, cfg.T_max
-    ctx = _ctx(wm, cfg)
-    assert wm.wm_get_info(ctx).tc_variant == 1
+    ctx = _ctx(wm, cfg, form)
+    assert wm.wm_get_info(ctx).tc_variant == (1 if form == PATH_TC_SINGLE else 5)
     lit = gpu_scores(ctx, b)
     dv = to_device(b)
     cut = b.cut.reshape(-1, C)
