@@ -296,6 +296,8 @@ class Leg:
         from wm_harness import weight_file, to_device
         self.wm, self.cfg, self.batch, self.dev, self.flush = wm, cfg, batch, dev, flush
         self.ctx = wm.wm_load_weights(weight_file(cfg), dev.index or 0)
+        if os.environ.get("WM_BENCH_SINGLE_CTA"):     # A/B: the single-CTA form of the d = 256 kernel (WM_OPT_PAIR = 0)
+            wm.wm_set_option(self.ctx, wm.WM_OPT_PAIR, 0)
         self.info = wm.wm_get_info(self.ctx)
         self.dv = to_device(batch, device=dev)
         self.B, self.S, self.k = batch.B, batch.S, cfg.k

@@ -28,6 +28,7 @@
 
 #include "wm_internal.h"
 #include "wm_ptx.cuh"
+#include "wm_trace.cuh"
 
 namespace wm {
 
@@ -76,6 +77,7 @@ struct Params {
     const float *bs0, *bs1, *w3, *bs2;
     CallArgs a;
     int n_tiles;
+    unsigned long long* prof;   // developer trace buffer (wm_trace.cuh), null in a normal build
 };
 
 struct SmemLayout {
@@ -200,6 +202,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     if (warp == PROD_WARP) {
         // =============================================================== tile schedule + TMA producer
         uint32_t stage = 0, ph = 0;
+        WM_TRACE_DECL(p.prof, 1)
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
             int tile = tile_of((int)it, pair, n_pairs, p.n_tiles);
@@ -223,7 +226,9 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (lane == 0) {
                 // image row of box `b` of this CTA: boxes of the two CTAs alternate, 128 rows each
                 auto issue = [&](int nbox, int box0) {
+                    WM_TRACE(60);
                     mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
+                    WM_TRACE(61);
                     // the leader's barrier collects both CTAs' boxes of the stage
                     if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2u * (uint32_t)nbox * BOX_BYTES);
                     for (int b = 0; b < nbox; ++b)
@@ -253,9 +258,12 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
         bool pend[2] = {false, false};
         const uint32_t s_hwk = s_base + L.hwk;
+        WM_TRACE_DECL(p.prof, 0)
         auto wait_h = [&](int b) {
             if (pend[b]) {
+                WM_TRACE(10 + b);
                 mbar_wait_cluster_warp(bar(B_HREADY + b), n_h[b] & 1);
+                WM_TRACE(12 + b);
                 ++n_h[b];
                 pend[b] = false;
                 tc_fence_after();
@@ -265,13 +273,16 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint32_t b_lo = ring_lo0;
         bool ready = false;
         auto acquire_stage = [&]() {       // returns with the current stage's data landed; probes the next stage
+            WM_TRACE(20);
             if (!ready) mbar_wait_warp(bar(B_FULL + stage), ph);
+            WM_TRACE(21);
             tc_fence_after();
             const uint32_t nst = stage + 1 == NSTAGE ? 0u : stage + 1;
             ready = __all_sync(0xffffffffu, mbar_test_wait(bar(B_FULL + nst), nst == 0 ? ph ^ 1u : ph));
         };
         auto advance = [&]() {
             __syncwarp();
+            WM_TRACE(22);
             b_lo += STAGE_BYTES >> 4;
             if (++stage == NSTAGE) { stage = 0; ph ^= 1; b_lo = ring_lo0; }
         };
@@ -369,12 +380,17 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             for (int t = 0; t < nsteps; ++t) {
                 // Step boundary: the a K-blocks of chunks 0 and 1 depend only on a_{t+1} and both GEMM1 accumulators are
                 // free, so they are issued before the wait for z' (pipe drain + LayerNorm is the serial section of a step)
+                WM_TRACE(30);
                 wait_h(0);
                 wait_h(1);
+                WM_TRACE(1);
                 mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after();
+                WM_TRACE(2);
                 stage_a01();
                 if (NC == 2) commit(B_AFREE);
+                WM_TRACE(3);
                 mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after();
+                WM_TRACE(4);
                 stage_z(0); commit(B_D1FULL + 0); pend[0] = true;
                 stage_z(1); commit(B_D1FULL + 1); pend[1] = true;
                 wait_h(0);
@@ -402,6 +418,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 continue;
             }
             // ---- scorer layer 1: four 128-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0)
+            WM_TRACE(31);
 #pragma unroll 1
             for (int c = 0; c < 4; ++c) {
                 const int b = c & 1;
@@ -439,6 +456,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
         uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
         const float inv_d = 1.0f / (float)D;
+        WM_TRACE_DECL(warp == 0 ? p.prof : nullptr, 2)
         // write 32 consecutive z columns of this row: fp32 -> TMEM, fp16 -> A1 (when `to_smem`)
         auto put_z = [&](int col0, const uint32_t (&v)[32], bool to_smem) {
             tmem_st32(T_Z + lane_off + (uint32_t)col0, v);
@@ -465,7 +483,9 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         };
         // bias + GELU over this thread's 64 columns of accumulator buffer b, fp16 result to TMEM at dst_col
         auto gelu_chunk = [&](int b, const float* bias, bool bias_in_smem, uint32_t dst_col) {
+            WM_TRACE(40);
             mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+            WM_TRACE(41);
             ++n_d1[b];
             tc_fence_after();
 #pragma unroll
@@ -485,6 +505,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 tmem_st16(dst_col + lane_off + 16u * p2, o);
             }
             publish(b == 0 ? r_hready0 : r_hready1, false);
+            WM_TRACE(42);
         };
 
         for (uint32_t it = 0;; ++it) {
@@ -525,7 +546,9 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int c = 0; c < NC; ++c)
                     gelu_chunk(c & 1, s_b1 + c * 128 + 64 * hh, true, T_D1 + 128u * (c & 1) + 64u * hh);
                 // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
+                WM_TRACE(50);
                 mbar_wait(bar(B_D2FULL), n_d2 & 1);
+                WM_TRACE(51);
                 ++n_d2;
                 tc_fence_after();
                 float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
@@ -555,6 +578,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 red[hh * TM + row] = make_float2(s1, s2);
                 named_bar_sync(1 + q, 64);
                 const float2 other = red[(hh ^ 1) * TM + row];
+                WM_TRACE(52);
                 const float mean = (s1 + other.x) * inv_d;
                 const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
                 const float rstd = rsqrtf(var + p.ln_eps);
@@ -599,6 +623,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     }
                 }
                 publish(r_zready, true);
+                WM_TRACE(53);
             }
 
             if (!rank_it) continue;
@@ -651,6 +676,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) bp4[e] = __ldg(p.bp + col4 + e);
         uint32_t n_w = 0;
+        WM_TRACE_DECL(aw == 0 ? p.prof : nullptr, 3)
         // A1 destination of this lane's 4 columns (8 bytes) in row r: K-block 4 + lane/16
         auto a_dst = [&](int r) -> uint2* {
             return reinterpret_cast<uint2*>(a1 + (4 + (lane >> 4)) * KB_BYTES + sw128_off(r, (lane & 15) >> 1) +
@@ -737,6 +763,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 
             for (int t = 0; t < nsteps; ++t) {
                 // phase 1 (one row per lane): read the step's action, log2 of its parameters, phi statistics
+                WM_TRACE(70);
                 int id = -1;
                 float lp[MAX_P];
 #pragma unroll
@@ -772,7 +799,9 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                 for (int rr = 0; rr < PRE; ++rr) pk[rr] = a_row(32 * aw + rr);
                 // store only once GEMM1 of the previous step no longer reads the a-part of A1
+                WM_TRACE(71);
                 if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+                WM_TRACE(72);
                 ++n_w;
 #pragma unroll
                 for (int rr = 0; rr < PRE; ++rr) *a_dst(32 * aw + rr) = pk[rr];
@@ -784,6 +813,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 fence_proxy_async();
                 __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
                 if (lane == 0) mbar_arrive_cluster(r_aready);
+                WM_TRACE(73);
             }
 
             // ---- the phi K-blocks of the scorer's A operand, one ROW per lane (see wm_tc_kernel): psi for WM_PHI_MEAN
@@ -1024,6 +1054,7 @@ int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     if (m.ranker_kind == WM_RANKER_FOREST) p.bs0 = p.bs1 = p.w3 = p.bs2 = m.zeros;   // (unused scorer, zero image)
     p.a = a;
     p.n_tiles = (int)((a.B + tcp::TMP - 1) / tcp::TMP);
+    p.prof = trace::begin(st);
     CUtensorMap tm;
     memcpy(&tm, m.tcp_tmap, sizeof(tm));
     const tcp::SmemLayout L = tcp::smem_layout(m.n_types, m.hidden, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
@@ -1039,6 +1070,7 @@ int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     }
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
+    trace::dump(p.prof, st);
     return WM_OK;
 }
 
