@@ -227,6 +227,23 @@ __device__ __forceinline__ uint32_t gelu2_f16(float2 acc, float2 bias) {
     return pack_f16(g.x, g.y);
 }
 
+// Two GELUs (tanh form) entirely on the packed fp16x2 pipe, for accumulators that already carry their bias: one cvt, five
+// HMUL2/HFMA2 and ONE MUFU (tanh.approx.f16x2) per pair of elements instead of nine fp32x2 / MUFU instructions.  The
+// result is the fp16 MMA operand anyway; the intermediate roundings (2^-11 each) stay below the operand rounding noise
+// the tolerance already carries (S5/S14).  Saturating convert: an out-of-range pre-activation becomes 65504,
+// never an infinity (gelu(65504) = 65504 in this arithmetic; large negative inputs give exactly 0).
+__device__ __forceinline__ uint32_t gelu2_h2(float lo, float hi) {
+    const uint32_t x = pack_f16(lo, hi);
+    uint32_t x2, pin, inner, t, hx, g;
+    asm("mul.f16x2 %0, %1, %1;" : "=r"(x2) : "r"(x));
+    asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(pin) : "r"(x2), "r"(0x28912891u), "r"(0x3A623A62u));   // 0.0356774, 0.7978846
+    asm("mul.f16x2 %0, %1, %2;" : "=r"(inner) : "r"(x), "r"(pin));
+    asm("tanh.approx.f16x2 %0, %1;" : "=r"(t) : "r"(inner));
+    asm("mul.f16x2 %0, %1, %2;" : "=r"(hx) : "r"(x), "r"(0x38003800u));                               // 0.5
+    asm("fma.rn.f16x2 %0, %1, %2, %1;" : "=r"(g) : "r"(hx), "r"(t));
+    return g;
+}
+
 // UMMA shared-memory descriptor, K-major, 128B swizzle, 8-row groups 1024 B apart (SBO), version 1 (sm_100).
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
     const uint32_t lo = ((saddr >> 4) & 0x3FFFu) | (1u << 16);

@@ -17,6 +17,15 @@
 //     (`cp.async.bulk.tensor ... cta_group::2`: both halves' complete_tx land on the leader's barrier);
 //   * MMA completion is multicast to both CTAs' barriers; epilogue / action warps of both CTAs arrive on the leader's
 //     barriers (cluster-scope release).
+// What else differs from wm_tc_kernel (measured: the CUDA-core side, not the tensor pipe or its issuer, bounded both forms —
+// ~32 K warp instructions per CTA and step against 41 K issue slots in the step's 10.2 K tensor cycles):
+//   * the action embedding is never formed: a_t = E[id] + W_p log2 p + b_p is linear in the features
+//     f_t = [onehot(id) | log2 p_j | 1], so the host folds E, W_p, b_p AND b1 into GEMM1's a-columns
+//     (W1a E^T, W1a W_p, W1a b_p + b1; summed in double, then the fp16 operand rounding every weight gets) and the action
+//     warps only write f_t: one K-block of 64 feature columns instead of two K-blocks of embedding, a handful of 16-bit
+//     stores per row and step instead of 128 FMAs;
+//   * the GELU epilogue therefore needs no bias and runs on the packed fp16x2 pipe (gelu2_h2);
+//   * scorer layer 1's bias rides on a constant-1 column of the phi features the same way.
 // Warp roles per CTA (512 threads) as in wm_tc_kernel: warps 0-7 epilogue (one thread per row and column half), warps
 // 8-11 action embedding, warp 12 TMEM allocator, warp 13 tile schedule + TMA producer, warp 15 MMA issuer (leader only).
 #include <cuda.h>
@@ -42,17 +51,17 @@ constexpr int D = 256;             // latent width
 constexpr int DA = 128;            // action-embedding width
 constexpr int SW = 512;            // scorer hidden width (both hidden layers)
 constexpr int KB_BYTES = 16384;    // one A K-block: [128 rows x 64 cols] fp16, SW128 K-major
-constexpr int BOX_BYTES = 16384;   // one TMA box: 128 image rows of 128 B = this CTA's half of two N = 128 K-blocks (2 x 64
-                                   // weight rows) or of one N = 256 K-block (128 weight rows); 512 tensor cycles of MMAs
-constexpr int HALF_BYTES = 8192;   // one N = 128 K-block half: [64 weight rows x 64 cols]
-constexpr int STAGE_BYTES = 2 * BOX_BYTES;
+constexpr int HB_BYTES = 8192;     // one TMA box ("half block"): 64 image rows of 128 B = this CTA's half of one N = 128
+                                   // K-block (64 weight rows x 64 cols; 4 MMAs, 256 tensor cycles) or a quarter of one
+                                   // N = 256 K-block (two consecutive boxes = this CTA's 128 weight rows)
+constexpr int STAGE_HB = 4;        // ring stage capacity in boxes (a stage carries 1..4 of them)
+constexpr int STAGE_BYTES = STAGE_HB * HB_BYTES;
 constexpr int NSTAGE = 3;
-constexpr int A1_KB = 6;           // z: 0-3, a/phi: 4-5
+constexpr int A1_KB = 6;           // z: 0-3, action features f_t / phi features: 4-5
 constexpr int HWK_BYTES = 4096;    // hw operand: one [128 x 16] no-swizzle K-major tile per K = 16 step
 constexpr int THREADS = 512;
 constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
 constexpr int MAX_TYPES = 64, MAX_P = 8, MAX_H = 64, MAX_HID = 1024;
-constexpr int SC_BOXES = 4 * 4 + 4 * 4;   // scorer stream per CTA: layer 1 (4 chunks x (phi, hw, z, z)), layer 2 (4 x 4)
 
 enum {
     B_FULL = 0,                    // [NSTAGE] TMA (both CTAs) -> leader's MMA warp
@@ -70,33 +79,28 @@ enum {
 
 struct Params {
     int hid, nc, n_types, P, H, hw_ksteps;
+    int akb, pkb;               // K-blocks of the action features f_t (1 or 2) and of the phi features (1 or 2)
     float ln_eps;
-    const __nv_bfloat16* E;     // [n_types][128]
-    const float *WpT, *bp;      // [P][128], [128]
-    const float *b1, *b2, *gamma, *beta;
-    const float *bs0, *bs1, *w3, *bs2;
+    const float *b2, *gamma, *beta;
+    const float *bs1, *w3, *bs2;
     CallArgs a;
     int n_tiles;
     unsigned long long* prof;   // developer trace buffer (wm_trace.cuh), null in a normal build
 };
 
 struct SmemLayout {
-    uint32_t a1, hwk, ring, e_tab, lp, mx, ids, cnt, b1, b2, gamma, beta, red, bars, sched, tmem_slot, total;
+    uint32_t a1, hwk, ring, mx, cnt, b2, gamma, beta, red, bars, sched, tmem_slot, total;
 };
 
-__host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_ksteps, int phi_struct) {
+__host__ __device__ inline SmemLayout smem_layout(int n_types, int hw_ksteps, int phi_struct) {
     SmemLayout L;
     uint32_t o = 0;
     L.a1 = o; o += A1_KB * KB_BYTES;
     L.ring = o; o += NSTAGE * STAGE_BYTES;
     L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
-    L.e_tab = o; o += (uint32_t)n_types * DA * 2;
-    L.lp = o; o += TM * MAX_P * 4;
     L.mx = o; o += phi_struct ? TM * MAX_P * 4 : 0;
-    L.ids = o; o += TM * 4;
     L.cnt = o; o += TM * (uint32_t)n_types;           // u8 counts, row-major [128][n_types]
     o = (o + 15) & ~15u;
-    L.b1 = o; o += (uint32_t)hid * 4;
     L.b2 = o; o += D * 4;
     L.gamma = o; o += D * 4;
     L.beta = o; o += D * 4;
@@ -115,11 +119,17 @@ __device__ __forceinline__ int tile_of(int it, int pair, int np, int n_tiles) {
     return idx < n_tiles ? idx : -1;
 }
 
-// Ring-stage program of one rollout step, per CTA, in boxes: stage 0 = a K-blocks of chunks 0 and 1, stages 1, 2 = z
-// K-blocks of chunk 0 / chunk 1, stage 3 = GEMM2 chunk 0, then per further chunk i: a K-blocks (ONE box), z K-blocks, GEMM2
-// chunk i-1; last stage = GEMM2 chunk NC-1.  3 NC - 1 stages, 5 NC boxes.
+// Ring-stage program of one rollout step, per CTA, in boxes: stage 0 = feature K-blocks of chunks 0 and 1 (2 akb boxes),
+// stages 1, 2 = z K-blocks of chunk 0 / chunk 1 (4 boxes each), stage 3 = GEMM2 chunk 0 (4), then per further chunk i:
+// feature K-blocks (akb), z K-blocks (4), GEMM2 chunk i-1 (4); last stage = GEMM2 chunk NC-1.  3 NC - 1 stages.
 __host__ __device__ inline int step_stages(int nc) { return 3 * nc - 1; }
-__host__ __device__ inline int stage_boxes(int j, int nc) { return (j >= 4 && j < 3 * nc - 2 && (j - 4) % 3 == 0) ? 1 : 2; }
+__host__ __device__ inline int stage_boxes(int j, int nc, int akb) {
+    if (j == 0) return 2 * akb;
+    return (j >= 4 && j < 3 * nc - 2 && (j - 4) % 3 == 0) ? akb : 4;
+}
+__host__ __device__ inline int step_boxes(int nc, int akb) { return 2 * akb + 12 + (nc - 2) * (akb + 8) + 4; }
+// scorer: layer 1, per 128-column chunk: [phi features (pkb) + hw (1)], [z (4)]; layer 2, per chunk: two stages of 4
+__host__ __device__ inline int scorer_boxes(int pkb) { return 4 * (pkb + 1 + 4) + 4 * 8; }
 
 constexpr uint32_t idesc_m256(uint32_t n) { return (1u << 4) | ((n >> 3) << 17) | ((256u >> 4) << 24); }
 constexpr uint32_t ID_N128 = idesc_m256(128), ID_N256 = idesc_m256(256);
@@ -140,12 +150,11 @@ template <int PHI, bool EXT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(1024) uint8_t smem[];
-    const SmemLayout L = smem_layout(p.n_types, p.hid, p.hw_ksteps, PHI);
+    const SmemLayout L = smem_layout(p.n_types, p.hw_ksteps, PHI);
     const uint32_t s_base = smem_u32(smem);
     const uint32_t s_a1 = s_base + L.a1, s_ring = s_base + L.ring, s_bars = s_base + L.bars;
     auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
     volatile int* s_sched = reinterpret_cast<volatile int*>(smem + L.sched);   // [2][2]: tile, nsteps
-    float* s_b1 = reinterpret_cast<float*>(smem + L.b1);
     float* s_b2 = reinterpret_cast<float*>(smem + L.b2);
     float* s_gamma = reinterpret_cast<float*>(smem + L.gamma);
     float* s_beta = reinterpret_cast<float*>(smem + L.beta);
@@ -155,7 +164,8 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int NC = p.nc;
-    const int ROLL_BOXES = 5 * NC, ROLL_STAGES = step_stages(NC);
+    const int AKB = p.akb, PKB = p.pkb;
+    const int ROLL_BOXES = step_boxes(NC, AKB), ROLL_STAGES = step_stages(NC);
 
     // ---- one-time setup
     if (threadIdx.x == 0) {
@@ -174,16 +184,12 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         fence_proxy_async();
     }
     if (warp == ALLOC_WARP) tmem_alloc2(s_base + L.tmem_slot, 512);
-    for (int i = threadIdx.x; i < p.hid; i += THREADS) s_b1[i] = __ldg(p.b1 + i);
     for (int i = threadIdx.x; i < D; i += THREADS) {
         s_b2[i] = __ldg(p.b2 + i);
         s_gamma[i] = __ldg(p.gamma + i);
         s_beta[i] = __ldg(p.beta + i);
     }
     {
-        const uint32_t* src = reinterpret_cast<const uint32_t*>(p.E);
-        uint32_t* dst = reinterpret_cast<uint32_t*>(smem + L.e_tab);
-        for (int i = threadIdx.x; i < p.n_types * DA / 2; i += THREADS) dst[i] = __ldg(src + i);
         // the hw K-block is only ever written in its first columns: clear it once so unread bytes are not NaNs
         uint32_t* hwk = reinterpret_cast<uint32_t*>(smem + L.hwk);
         for (int i = threadIdx.x; i < p.hw_ksteps * HWK_BYTES / 4; i += THREADS) hwk[i] = 0u;
@@ -224,28 +230,34 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             if (tile < 0) break;
             if (lane == 0) {
-                // image row of box `b` of this CTA: boxes of the two CTAs alternate, 128 rows each
+                // image row of box `b` of this CTA: boxes of the two CTAs alternate, 64 rows each
                 auto issue = [&](int nbox, int box0) {
                     WM_TRACE(60);
                     mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
                     WM_TRACE(61);
                     // the leader's barrier collects both CTAs' boxes of the stage
-                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2u * (uint32_t)nbox * BOX_BYTES);
+                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2u * (uint32_t)nbox * HB_BYTES);
                     for (int b = 0; b < nbox; ++b)
-                        tma_load_2sm(s_ring + stage * STAGE_BYTES + b * BOX_BYTES, &tmap, 0,
-                                     128 * (2 * (box0 + b) + (int)rank), bar(B_FULL + stage));
+                        tma_load_2sm(s_ring + stage * STAGE_BYTES + b * HB_BYTES, &tmap, 0,
+                                     64 * (2 * (box0 + b) + (int)rank), bar(B_FULL + stage));
                     if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
                 };
                 for (int t = 0; t < nsteps; ++t) {
                     int box = 0;
                     for (int j = 0; j < ROLL_STAGES; ++j) {
-                        const int nb = stage_boxes(j, NC);
+                        const int nb = stage_boxes(j, NC, AKB);
                         issue(nb, box);
                         box += nb;
                     }
                 }
-                if (rank_it)
-                    for (int j = 0; j < SC_BOXES / 2; ++j) issue(2, ROLL_BOXES + 2 * j);
+                if (rank_it) {
+                    int box = ROLL_BOXES;
+                    for (int c = 0; c < 4; ++c) {
+                        issue(PKB + 1, box); box += PKB + 1;
+                        issue(4, box); box += 4;
+                    }
+                    for (int j = 0; j < 8; ++j) { issue(4, box); box += 4; }
+                }
             }
             __syncwarp();
         }
@@ -286,34 +298,37 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             b_lo += STAGE_BYTES >> 4;
             if (++stage == NSTAGE) { stage = 0; ph ^= 1; b_lo = ring_lo0; }
         };
-        // one box against two A K-blocks (N = 128: the box holds this CTA's 64-row halves of two K-blocks): 8 MMAs
-        auto box_ss = [&](uint32_t d, uint32_t a_lo0, uint32_t a_lo1, uint32_t blo, bool first) {
+        // one box (this CTA's 64-row half of an N = 128 K-block) against the A K-block at a_kb: 4 MMAs of K = 16
+        auto kb_ss = [&](uint32_t d, uint32_t a_kb, uint32_t blo, bool first) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) mma_ss2(d, desc_of(a_lo0 + 2u * j), desc_of(blo + 2u * j), ID_N128, (first && j == 0) ? 0u : 1u);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) mma_ss2(d, desc_of(a_lo1 + 2u * j), desc_of(blo + (HALF_BYTES >> 4) + 2u * j), ID_N128, 1u);
+            for (int j = 0; j < 4; ++j) mma_ss2(d, desc_of(a_kb + 2u * j), desc_of(blo + 2u * j), ID_N128, (first && j == 0) ? 0u : 1u);
         };
         const uint32_t a_lo = smem_desc_lo(s_a1);
-        constexpr uint32_t KBL = KB_BYTES >> 4, BXL = BOX_BYTES >> 4;
+        constexpr uint32_t KBL = KB_BYTES >> 4, HBL = HB_BYTES >> 4;
         auto commit = [&](int barrier) {
             if (elect_one()) mma_commit2(bar(barrier));
             __syncwarp();
         };
-        // stage: a K-blocks (4, 5) of chunk buffers 0 AND 1
+        // stage: feature K-blocks (4 ..) of chunk buffers 0 AND 1
         auto stage_a01 = [&]() {
             acquire_stage();
             if (elect_one()) {
-                box_ss(TD1, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo, true);
-                box_ss(TD1 + 128u, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo + BXL, true);
+                for (int c = 0; c < 2; ++c)
+                    for (int k = 0; k < AKB; ++k)
+                        kb_ss(TD1 + 128u * c, a_lo + (4 + k) * KBL, b_lo + (uint32_t)(c * AKB + k) * HBL, k == 0);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
         };
-        // stage of ONE box: a / phi K-blocks (4, 5) into buffer b
-        auto stage_a = [&](int b) {
+        // stage: feature / phi K-blocks (4 ..) into buffer b, nk of them; with_hw: followed by the hw tile
+        auto stage_a = [&](int b, int nk, bool with_hw) {
             acquire_stage();
             if (elect_one()) {
-                box_ss(TD1 + 128u * b, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo, true);
+                for (int k = 0; k < nk; ++k) kb_ss(TD1 + 128u * b, a_lo + (4 + k) * KBL, b_lo + (uint32_t)k * HBL, k == 0);
+                if (with_hw)
+                    for (int j = 0; j < p.hw_ksteps; ++j)
+                        mma_ss2(TD1 + 128u * b, smem_desc_nosw(s_hwk + j * HWK_BYTES), desc_of(b_lo + (uint32_t)nk * HBL + 2u * j),
+                                ID_N128, 1u);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
@@ -322,14 +337,14 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         auto stage_z = [&](int b) {
             acquire_stage();
             if (elect_one()) {
-                box_ss(TD1 + 128u * b, a_lo, a_lo + KBL, b_lo, false);
-                box_ss(TD1 + 128u * b, a_lo + 2 * KBL, a_lo + 3 * KBL, b_lo + BXL, false);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) kb_ss(TD1 + 128u * b, a_lo + k * KBL, b_lo + (uint32_t)k * HBL, false);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
         };
         // stage: GEMM2 of hidden chunk buffer b (fp16 in TMEM: K-block 0 at +0, K-block 1 at +64 columns) x all 256
-        // latent columns: each box is this CTA's 128 weight rows of one [256 x 64] B tile, 4 MMAs with N = 256
+        // latent columns: two consecutive boxes are this CTA's 128 weight rows of one [256 x 64] B tile, 4 MMAs with N = 256
         auto stage_g2 = [&](int b) {
             acquire_stage();
             if (elect_one()) {
@@ -337,18 +352,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                 for (int j = 0; j < 4; ++j) mma_ts2(TZ, hbuf + 8u * j, desc_of(b_lo + 2u * j), ID_N256, 1u);
 #pragma unroll
-                for (int j = 0; j < 4; ++j) mma_ts2(TZ, hbuf + 64u + 8u * j, desc_of(b_lo + BXL + 2u * j), ID_N256, 1u);
-                mma_commit2(bar(B_EMPTY + stage));
-            }
-            advance();
-        };
-        // scorer layer 1 stage: phi K-blocks (box 0) + the hw tile (first half of box 1; its second half is padding)
-        auto stage_phihw = [&](int b) {
-            acquire_stage();
-            if (elect_one()) {
-                box_ss(TD1 + 128u * b, a_lo + 4 * KBL, a_lo + 5 * KBL, b_lo, true);
-                for (int j = 0; j < p.hw_ksteps; ++j)
-                    mma_ss2(TD1 + 128u * b, smem_desc_nosw(s_hwk + j * HWK_BYTES), desc_of(b_lo + BXL + 2u * j), ID_N128, 1u);
+                for (int j = 0; j < 4; ++j) mma_ts2(TZ, hbuf + 64u + 8u * j, desc_of(b_lo + 2 * HBL + 2u * j), ID_N256, 1u);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
@@ -362,7 +366,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
                         mma_ts2(TD1 + 128u * b, TZ + 32u * (kb + q) + 8u * j,
-                                desc_of(b_lo + (uint32_t)q * (HALF_BYTES >> 4) + 2u * j), ID_N128, (kb == 0 && q == 0 && j == 0) ? 0u : 1u);
+                                desc_of(b_lo + (uint32_t)q * HBL + 2u * j), ID_N128, (kb == 0 && q == 0 && j == 0) ? 0u : 1u);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
@@ -401,7 +405,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     if (i < NC) {                       // GEMM1 chunk i into buffer i & 1 (its GEMM2 reader has been issued)
                         const int b = i & 1;
                         wait_h(b);
-                        stage_a(b);
+                        stage_a(b, AKB, false);
                         if (i == NC - 1) commit(B_AFREE);
                         stage_z(b);
                         commit(B_D1FULL + b);
@@ -424,7 +428,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 const int b = c & 1;
                 wait_h(b);
                 if (c == 0) { mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
-                stage_phihw(b);
+                stage_a(b, PKB, true);
                 if (c == 3) commit(B_AFREE);
                 if (c == 0) { mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
                 stage_z(b);
@@ -481,29 +485,24 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(leader_bar);
         };
-        // bias + GELU over this thread's 64 columns of accumulator buffer b, fp16 result to TMEM at dst_col
-        auto gelu_chunk = [&](int b, const float* bias, bool bias_in_smem, uint32_t dst_col) {
+        // GELU over this thread's 64 columns of accumulator buffer b (the bias is already in the accumulator: it rides on
+        // the constant-1 feature column), fp16 result to TMEM at dst_col.  Both TMEM loads are in flight before the first use.
+        auto gelu_chunk = [&](int b, uint32_t dst_col) {
             WM_TRACE(40);
             mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
             WM_TRACE(41);
             ++n_d1[b];
             tc_fence_after();
+            uint32_t v0[32], v1[32], o[16];
+            tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh, v0);
+            tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u, v1);
+            tmem_ld_wait();
 #pragma unroll
-            for (int p2 = 0; p2 < 2; ++p2) {
-                uint32_t v[32], o[16];
-                tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u * p2, v);
-                tmem_ld_wait();
-                const float4* bp_ = reinterpret_cast<const float4*>(bias + 32 * p2);
+            for (int i = 0; i < 16; ++i) o[i] = gelu2_h2(__uint_as_float(v0[2 * i]), __uint_as_float(v0[2 * i + 1]));
+            tmem_st16(dst_col + lane_off, o);
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float4 bv = bias_in_smem ? bp_[i] : __ldg(bp_ + i);
-                    o[2 * i] = gelu2_f16(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
-                                          make_float2(bv.x, bv.y));
-                    o[2 * i + 1] = gelu2_f16(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
-                                              make_float2(bv.z, bv.w));
-                }
-                tmem_st16(dst_col + lane_off + 16u * p2, o);
-            }
+            for (int i = 0; i < 16; ++i) o[i] = gelu2_h2(__uint_as_float(v1[2 * i]), __uint_as_float(v1[2 * i + 1]));
+            tmem_st16(dst_col + lane_off + 16u, o);
             publish(b == 0 ? r_hready0 : r_hready1, false);
             WM_TRACE(42);
         };
@@ -544,7 +543,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 
             for (int t = 0; t < nsteps; ++t) {
                 for (int c = 0; c < NC; ++c)
-                    gelu_chunk(c & 1, s_b1 + c * 128 + 64 * hh, true, T_D1 + 128u * (c & 1) + 64u * hh);
+                    gelu_chunk(c & 1, T_D1 + 128u * (c & 1) + 64u * hh);
                 // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
                 WM_TRACE(50);
                 mbar_wait(bar(B_D2FULL), n_d2 & 1);
@@ -629,7 +628,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (!rank_it) continue;
             // ---- scorer layer 1 -> H1 (fp16) in TMEM columns [0,256)
             for (int c = 0; c < 4; ++c)
-                gelu_chunk(c & 1, p.bs0 + c * 128 + 64 * hh, false, T_Z + 64u * c + 32u * hh);
+                gelu_chunk(c & 1, T_Z + 64u * c + 32u * hh);
             // ---- scorer layer 2 + output dot product
             float part = 0.0f;
             for (int c = 0; c < 4; ++c) {
@@ -657,30 +656,24 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
         }
     } else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
-        // =============================================================== action-embedding warps
+        // =============================================================== action-feature warps (one row per lane)
+        // Per step a row's action enters GEMM1 as the feature row f_t = [onehot(id) (NT) | log2 p_j (P) | 1] of K-block 4
+        // (and 5 when NT + P + 1 > 64): the embedding tables and biases are folded into the weights (tcp_prepare).
         const int aw = warp - ACT_WARP0;
-        const int row = 32 * aw + lane;       // row-mapped phases
-        const int col4 = 4 * lane;            // column-mapped phases: this lane's 4 embedding columns
+        const int row = 32 * aw + lane;
         uint8_t* a1 = smem + L.a1;
-        const uint8_t* s_E = smem + L.e_tab;
-        float* s_lp = reinterpret_cast<float*>(smem + L.lp);
-        int* s_ids = reinterpret_cast<int*>(smem + L.ids);
         uint8_t* s_cnt = smem + L.cnt;
         const uint32_t r_aready = mapa(bar(B_AREADY), 0);
         const int P = p.P, NT = p.n_types;
-        float wp[MAX_P][4], bp4[4];
-#pragma unroll
-        for (int j = 0; j < MAX_P; ++j)
-#pragma unroll
-            for (int e = 0; e < 4; ++e) wp[j][e] = j < P ? __ldg(p.WpT + j * DA + col4 + e) : 0.0f;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) bp4[e] = __ldg(p.bp + col4 + e);
         uint32_t n_w = 0;
         WM_TRACE_DECL(aw == 0 ? p.prof : nullptr, 3)
-        // A1 destination of this lane's 4 columns (8 bytes) in row r: K-block 4 + lane/16
-        auto a_dst = [&](int r) -> uint2* {
-            return reinterpret_cast<uint2*>(a1 + (4 + (lane >> 4)) * KB_BYTES + sw128_off(r, (lane & 15) >> 1) +
-                                            (lane & 1) * 8);
+        // 16-bit feature store: column c of this row in K-blocks 4, 5
+        auto put = [&](int c, uint32_t h16) {
+            *reinterpret_cast<uint16_t*>(a1 + (4 + (c >> 6)) * KB_BYTES + sw128_off(row, (c & 63) >> 3) + (c & 7) * 2) = (uint16_t)h16;
+        };
+        auto clear_row = [&](int nkb) {
+            for (int ch = 0; ch < 8 * nkb; ++ch)
+                *reinterpret_cast<uint4*>(a1 + (4 + (ch >> 3)) * KB_BYTES + sw128_off(row, ch & 7)) = make_uint4(0u, 0u, 0u, 0u);
         };
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
@@ -695,7 +688,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             float slp[MAX_P];   // per parameter slot: running sum of log2 p
 #pragma unroll
             for (int j = 0; j < MAX_P; ++j) slp[j] = 0.0f;
-            // structured phi: the per-slot running maximum lives in shared memory (the registers of this role are full)
+            // structured phi: the per-slot running maximum lives in shared memory
             float4* s_mx4 = reinterpret_cast<float4*>(smem + L.mx) + row * (MAX_P / 4);
             if (PHI == WM_PHI_STRUCT) s_mx4[0] = s_mx4[1] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
             // one action of this row: type id (clamped), log2 of its parameters, phi statistics
@@ -761,94 +754,70 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (EXT && p.a.start)
                 while (__any_sync(0xffffffffu, scanned < st)) scan4();
 
+            int prev_id = -1;      // the one-hot column this row has set
             for (int t = 0; t < nsteps; ++t) {
-                // phase 1 (one row per lane): read the step's action, log2 of its parameters, phi statistics
+                // read the step's action, log2 of its parameters, phi statistics — before the wait: the loads' latency hides
                 WM_TRACE(70);
                 int id = -1;
                 float lp[MAX_P];
 #pragma unroll
                 for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
                 if (st + t < len) id = take(st + t, lp);
-                s_ids[row] = id;
-                *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
-                *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
-                __syncwarp();
-                // phase 2 (4 columns per lane, loop over the warp's 32 rows): a = E[id] + W_p log2(p) + b_p.  The first
-                // PRE rows are computed into registers BEFORE the wait below, the rest after it.
-                constexpr int PRE = 16;
-                uint2 pk[PRE];
-                auto a_row = [&](int r) -> uint2 {
-                    const int idr = s_ids[r];
-                    float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-                    if (idr >= 0) {
-                        const uint2 e = *reinterpret_cast<const uint2*>(s_E + ((size_t)idr * DA + col4) * 2);
-                        a4[0] = __uint_as_float(e.x << 16) + bp4[0];
-                        a4[1] = __uint_as_float(e.x & 0xffff0000u) + bp4[1];
-                        a4[2] = __uint_as_float(e.y << 16) + bp4[2];
-                        a4[3] = __uint_as_float(e.y & 0xffff0000u) + bp4[3];
-                        const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
-                        const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
-                        const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
-#pragma unroll
-                        for (int j = 0; j < MAX_P; ++j)
-#pragma unroll
-                            for (int e2 = 0; e2 < 4; ++e2) a4[e2] = fmaf(wp[j][e2], lr[j], a4[e2]);
-                    }
-                    return make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
-                };
-#pragma unroll
-                for (int rr = 0; rr < PRE; ++rr) pk[rr] = a_row(32 * aw + rr);
-                // store only once GEMM1 of the previous step no longer reads the a-part of A1
+                // store only once GEMM1 of the previous step (or the previous tile's scorer) no longer reads K-blocks 4, 5
                 WM_TRACE(71);
                 if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
                 WM_TRACE(72);
                 ++n_w;
+                if (t == 0) {          // the K-blocks still hold the previous tile's phi features
+                    clear_row(2);
+                    put(NT + P, 0x3C00u);                      // the constant-1 column (carries W1a b_p + b1)
+                }
+                if (id >= 0) {         // a masked row keeps its last features: its result is discarded anyway (frozen row)
+                    if (prev_id >= 0 && prev_id != id) put(prev_id, 0u);
+                    put(id, 0x3C00u);
+                    prev_id = id;
 #pragma unroll
-                for (int rr = 0; rr < PRE; ++rr) *a_dst(32 * aw + rr) = pk[rr];
-#pragma unroll 4
-                for (int rr = PRE; rr < 32; ++rr) {
-                    const int r = 32 * aw + rr;
-                    *a_dst(r) = a_row(r);
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) put(NT + j, pack_f16(lp[j], 0.0f));
                 }
                 fence_proxy_async();
-                __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
+                __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(r_aready);
                 WM_TRACE(73);
             }
 
-            // ---- the phi K-blocks of the scorer's A operand, one ROW per lane (see wm_tc_kernel): psi for WM_PHI_MEAN
-            // (the host folds E, W_p, b_p into scorer layer 1), the statistics themselves for WM_PHI_STRUCT
+            // ---- the phi features of the scorer's A operand (K-blocks 4, 5), one row per lane:
+            //   WM_PHI_MEAN    phi = mean_t a_t is LINEAR in psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) | 1 (len > 0)];
+            //                  the host folds E, W_p and b_p into scorer layer 1's phi weights (tcp_prepare)
+            //   WM_PHI_STRUCT  phi = [count_c (NT) | len | sum_j (P) | mean_j (P) | max_j (P)]   (S25)
+            // followed by a constant-1 column that carries scorer layer 1's bias
             if (!rank_it) continue;
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
             {
-                auto put = [&](int c, float v) {
-                    *reinterpret_cast<uint16_t*>(a1 + (4 + (c >> 6)) * KB_BYTES + sw128_off(row, (c & 63) >> 3) +
-                                                 (c & 7) * 2) = (uint16_t)pack_f16(v, 0.0f);
-                };
-#pragma unroll
-                for (int ch = 0; ch < 16; ++ch)
-                    *reinterpret_cast<uint4*>(a1 + (4 + (ch >> 3)) * KB_BYTES + sw128_off(row, ch & 7)) =
-                        make_uint4(0u, 0u, 0u, 0u);
+                auto putf = [&](int c, float v) { put(c, pack_f16(v, 0.0f)); };
+                clear_row(2);
                 const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
                 if (PHI == WM_PHI_STRUCT) {
-                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c]);
-                    put(NT, (float)len);
+                    for (int c = 0; c < NT; ++c) putf(c, (float)s_cnt[row * NT + c]);
+                    putf(NT, (float)len);
                     const float4 m0 = s_mx4[0], m1 = s_mx4[1];
                     const float mxr[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
 #pragma unroll
                     for (int j = 0; j < MAX_P; ++j)
                         if (j < P) {
-                            put(NT + 1 + j, slp[j]);
-                            put(NT + 1 + P + j, slp[j] * inv);
-                            put(NT + 1 + 2 * P + j, mxr[j]);
+                            putf(NT + 1 + j, slp[j]);
+                            putf(NT + 1 + P + j, slp[j] * inv);
+                            putf(NT + 1 + 2 * P + j, mxr[j]);
                         }
+                    put(NT + 1 + 3 * P, 0x3C00u);
                 } else {
-                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c] * inv);
+                    for (int c = 0; c < NT; ++c) putf(c, (float)s_cnt[row * NT + c] * inv);
 #pragma unroll
                     for (int j = 0; j < MAX_P; ++j)
-                        if (j < P) put(NT + j, slp[j] * inv);
-                    put(NT + P, len > 0 ? 1.0f : 0.0f);
+                        if (j < P) putf(NT + j, slp[j] * inv);
+                    putf(NT + P, len > 0 ? 1.0f : 0.0f);
+                    put(NT + P + 1, 0x3C00u);
                 }
             }
             // hardware features of this row -> the hw operand tile (columns >= H stay zero)
@@ -882,25 +851,20 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 // ------------------------------------------------------------------------------------------------ host side
 namespace {
 
-// Append one pair box: for each CTA (rank 0, then rank 1) 128 image rows of 128 B.
-//   n128 = true : two N = 128 K-block halves per CTA: rows [0,64) = W[n0 + 64 r + n][k0 + k], rows [64,128) the same weight
-//                 rows at k0 + 64 (K-blocks k0/64 and k0/64 + 1); kvalid counts valid columns from k0 (the rest is zero)
-//   n128 = false: one N = 256 K-block half per CTA: rows [0,128) = W[n0 + 128 r + n][k0 + k]
-// Each 64-row (or 128-row) block is a SW128 K-major tile: row n at n * 128 B, 16-byte chunk c at (c ^ (n & 7)).
+// Append one box slot: for each CTA (rank 0, then rank 1) 64 image rows of 128 B = the SW128 K-major image of
+// W[row0 + rstride * r + n][k0 + k], n < 64, k < 64 (k >= kvalid reads as zero): row n at n * 128 B, 16-byte chunk c at
+// (c ^ (n & 7)).  N = 128 K-block: rstride = 64 (the CTAs hold the two halves of the 128 weight rows).  N = 256 K-block:
+// two slots, rstride = 128, row0 = 0 and 64 (two consecutive boxes of a CTA = its 128 weight rows).
 // Returns false when a weight is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
-bool append_box(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid, bool n128) {
+bool append_slot(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int row0, int rstride, int k0, int kvalid) {
     const size_t base = blob.size();
-    blob.resize(base + 2 * tcp::BOX_BYTES / 2, 0);
+    blob.resize(base + 2 * tcp::HB_BYTES / 2, 0);
     bool ok = true;
     for (int r = 0; r < 2; ++r)
-        for (int row = 0; row < 128; ++row)
+        for (int n = 0; n < 64; ++n)
             for (int k = 0; k < 64; ++k) {
-                int n, kk;
-                if (n128) { n = n0 + 64 * r + (row & 63); kk = (row >> 6) * 64 + k; }
-                else { n = n0 + 128 * r + row; kk = k; }
-                const float v = kk < kvalid ? W[(size_t)n * ld + k0 + kk] : 0.0f;
-                const int tr = n128 ? (row & 63) : row;     // row inside its SW128 tile
-                const size_t off = (size_t)r * tcp::BOX_BYTES + (size_t)row * 128 + (size_t)((((k >> 3) ^ (tr & 7)) << 4)) +
+                const float v = k < kvalid ? W[(size_t)(row0 + rstride * r + n) * ld + k0 + k] : 0.0f;
+                const size_t off = (size_t)r * tcp::HB_BYTES + (size_t)n * 128 + (size_t)((((k >> 3) ^ (n & 7)) << 4)) +
                                    (size_t)(k & 7) * 2;
                 uint16_t hb;
                 ok &= f32_to_f16_bits(v, &hb);
@@ -926,7 +890,7 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     Model& m = ctx->m;
     m.tcp_ok = 0;
     if (!tcp_model_ok(m)) return WM_OK;
-    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT);
+    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT);
     if ((int)L.total > ctx->smem_optin) return WM_OK;
     auto get = [&](const char* n) -> const std::vector<float>& {
         for (size_t i = 0; i < names.size(); ++i)
@@ -934,23 +898,71 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         static const std::vector<float> empty;
         return empty;
     };
-    const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1");
-    const int hid = m.hidden, NC = hid / 128, K1 = tcp::D + tcp::DA;
-    const int F = m.phi_dim, K0 = tcp::D + F + m.H;   // scorer input [z ; phi (F <= 128 columns) ; hw]
-    const size_t n_boxes = (size_t)5 * NC + tcp::SC_BOXES;
+    const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &b1 = get("b1"), &E = get("E"), &Wp = get("W_p"), &bpv = get("b_p");
+    const bool forest = m.ranker_kind == WM_RANKER_FOREST;
+    const int hid = m.hidden, NC = hid / 128, K1 = tcp::D + tcp::DA, NT = m.n_types, P = m.P;
+    // ---- GEMM1's a-columns folded onto the action features f = [onehot(id) (NT) | log2 p_j (P) | 1]:
+    //      W1[:, d:] (E[id] + W_p lp + b_p) + b1  =  (W1a E^T)[:, id] + (W1a W_p) lp + (W1a b_p + b1)
+    const int NF = NT + P + 1, AKB = (NF + 63) / 64;
+    std::vector<float> W1f((size_t)hid * 64 * AKB, 0.0f);
+    for (int n = 0; n < hid; ++n) {
+        const float* wr = &W1[(size_t)n * K1 + tcp::D];
+        float* out = &W1f[(size_t)n * 64 * AKB];
+        for (int c = 0; c < NT; ++c) {
+            double acc = 0.0;
+            for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tcp::DA + k];
+            out[c] = (float)acc;
+        }
+        for (int j = 0; j < P; ++j) {
+            double acc = 0.0;
+            for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * P + j];
+            out[NT + j] = (float)acc;
+        }
+        double acc = b1[n];
+        for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * bpv[k];
+        out[NT + P] = (float)acc;
+    }
+    // ---- scorer layer 1's phi columns as the kernel's phi features see them, plus the bias on a constant-1 column:
+    //      WM_PHI_STRUCT: the F columns of Ws0 as they are; WM_PHI_MEAN: folded onto psi (see the action warps)
+    const int F = m.phi_dim, K0 = tcp::D + F + m.H;   // scorer input [z ; phi ; hw]
+    const int NPSI = (m.phi_kind == WM_PHI_STRUCT ? NT + 1 + 3 * P : NT + P + 1) + 1, PKB = (NPSI + 63) / 64;
+    std::vector<float> Wphi((size_t)tcp::SW * 64 * PKB, 0.0f);
+    if (!forest) {
+        const std::vector<float>&Ws0 = get("Ws0"), &bs0 = get("bs0");
+        for (int n = 0; n < tcp::SW; ++n) {
+            const float* wr = &Ws0[(size_t)n * K0 + tcp::D];
+            float* out = &Wphi[(size_t)n * 64 * PKB];
+            if (m.phi_kind == WM_PHI_STRUCT) {
+                for (int c = 0; c < F; ++c) out[c] = wr[c];
+            } else {
+                for (int c = 0; c < NT; ++c) {
+                    double acc = 0.0;
+                    for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tcp::DA + k];
+                    out[c] = (float)acc;
+                }
+                for (int j = 0; j < P; ++j) {
+                    double acc = 0.0;
+                    for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * P + j];
+                    out[NT + j] = (float)acc;
+                }
+                double acc = 0.0;
+                for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * bpv[k];
+                out[NT + P] = (float)acc;
+            }
+            out[NPSI - 1] = bs0[n];
+        }
+    }
+    const size_t n_slots = (size_t)tcp::step_boxes(NC, AKB) + tcp::scorer_boxes(PKB);
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
-    blob.reserve(n_boxes * tcp::BOX_BYTES);
-    // the MMA warp's order (tcp::stage_boxes): a K-blocks (4, 5) of chunks 0 and 1, z K-blocks (0-3) of chunk 0, of chunk 1,
-    // GEMM2 chunk 0, then per chunk i >= 2: a, z, GEMM2 chunk i - 1; last GEMM2 chunk NC - 1
-    auto g1a = [&](int c) { ok &= append_box(blob, W1, K1, c * 128, 4 * 64, 128, true); };
-    auto g1z = [&](int c) {
-        ok &= append_box(blob, W1, K1, c * 128, 0, 128, true);
-        ok &= append_box(blob, W1, K1, c * 128, 128, 128, true);
-    };
+    blob.reserve(n_slots * tcp::HB_BYTES);
+    // the MMA warp's order (tcp::stage_boxes): feature K-blocks of chunks 0 and 1, z K-blocks (0-3) of chunk 0, of chunk 1,
+    // GEMM2 chunk 0, then per chunk i >= 2: features, z, GEMM2 chunk i - 1; last GEMM2 chunk NC - 1
+    auto g1a = [&](int c) { for (int k = 0; k < AKB; ++k) ok &= append_slot(blob, W1f, 64 * AKB, c * 128, 64, k * 64, 64); };
+    auto g1z = [&](int c) { for (int k = 0; k < 4; ++k) ok &= append_slot(blob, W1, K1, c * 128, 64, k * 64, 64); };
     auto g2 = [&](int c) {            // GEMM2 chunk c: the chunk's two hidden K-blocks x all 256 latent columns
-        ok &= append_box(blob, W2, hid, 0, c * 128, 64, false);
-        ok &= append_box(blob, W2, hid, 0, c * 128 + 64, 64, false);
+        for (int k = 0; k < 2; ++k)
+            for (int hrow = 0; hrow < 2; ++hrow) ok &= append_slot(blob, W2, hid, 64 * hrow, 128, c * 128 + k * 64, 64);
     };
     g1a(0); g1a(1); g1z(0); g1z(1);
     g2(0);
@@ -958,42 +970,24 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         if (i < NC) { g1a(i); g1z(i); }
         g2(i - 1);
     }
-    // phi weights of scorer layer 1 as the kernel's phi K-blocks see them, [SW][128] (see wm_tc.cu tc_prepare)
-    const bool forest = m.ranker_kind == WM_RANKER_FOREST;
-    std::vector<float> Wphi((size_t)tcp::SW * 128, 0.0f);
-    if (forest) {
-    } else if (m.phi_kind == WM_PHI_STRUCT) {
-        for (int n = 0; n < tcp::SW; ++n)
-            for (int c = 0; c < F; ++c) Wphi[(size_t)n * 128 + c] = Ws0[(size_t)n * K0 + tcp::D + c];
-    } else {
-        const std::vector<float>&E = get("E"), &Wp = get("W_p"), &bpv = get("b_p");
-        for (int n = 0; n < tcp::SW; ++n) {
-            const float* wr = &Ws0[(size_t)n * K0 + tcp::D];
-            for (int c = 0; c < m.n_types; ++c) {
-                double acc = 0.0;
-                for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tcp::DA + k];
-                Wphi[(size_t)n * 128 + c] = (float)acc;
+    {
+        static const std::vector<float> none;
+        const std::vector<float>&Ws0 = forest ? none : get("Ws0"), &Ws1 = forest ? none : get("Ws1");
+        const std::vector<float> zeros((size_t)tcp::SW * 64, 0.0f);
+        for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi features (PKB), hw, z (4 K-blocks)
+            for (int k = 0; k < PKB; ++k) ok &= append_slot(blob, Wphi, 64 * PKB, c * 128, 64, k * 64, 64);
+            if (forest) {
+                for (int k = 0; k < 5; ++k) ok &= append_slot(blob, zeros, 64, c * 128, 64, 0, 0);
+            } else {
+                ok &= append_slot(blob, Ws0, K0, c * 128, 64, tcp::D + F, m.H);
+                for (int k = 0; k < 4; ++k) ok &= append_slot(blob, Ws0, K0, c * 128, 64, k * 64, 64);
             }
-            for (int j = 0; j < m.P; ++j) {
-                double acc = 0.0;
-                for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * m.P + j];
-                Wphi[(size_t)n * 128 + m.n_types + j] = (float)acc;
-            }
-            double acc = 0.0;
-            for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * bpv[k];
-            Wphi[(size_t)n * 128 + m.n_types + m.P] = (float)acc;
         }
+        for (int c = 0; c < 4; ++c)       // scorer layer 2: K = 512 = 8 K-blocks
+            for (int kb = 0; kb < 8; ++kb)
+                ok &= forest ? append_slot(blob, zeros, 64, c * 128, 64, 0, 0) : append_slot(blob, Ws1, tcp::SW, c * 128, 64, kb * 64, 64);
     }
-    std::vector<float> zero1(1, 0.0f);
-    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (2 K-blocks), hw + zero padding, z (4 K-blocks)
-        ok &= append_box(blob, Wphi, 128, c * 128, 0, forest ? 0 : 128, true);
-        ok &= append_box(blob, Ws0, K0, c * 128, tcp::D + F, forest ? 0 : m.H, true);
-        ok &= append_box(blob, Ws0, K0, c * 128, 0, forest ? 0 : 128, true);
-        ok &= append_box(blob, Ws0, K0, c * 128, 128, forest ? 0 : 128, true);
-    }
-    for (int c = 0; c < 4; ++c)       // scorer layer 2: K = 512 = 8 K-blocks = 4 boxes
-        for (int kb = 0; kb < 8; kb += 2) ok &= append_box(blob, Ws1, tcp::SW, c * 128, kb * 64, forest ? 0 : 128, true);
-    if (blob.size() * 2 != n_boxes * 2 * tcp::BOX_BYTES) {
+    if (blob.size() * 2 != n_slots * 2 * tcp::HB_BYTES) {
         set_error("tcp_prepare: internal weight-image size mismatch");
         return WM_ERR_FORMAT;
     }
@@ -1017,7 +1011,7 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     CUtensorMap tm;
     const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
     const cuuint64_t strides[1] = {128};
-    const cuuint32_t box[2] = {64, 128}, es[2] = {1, 1};
+    const cuuint32_t box[2] = {64, 64}, es[2] = {1, 1};
     const CUresult r = ((EncodeTiledFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_blob, dims, strides, box, es,
                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -1038,6 +1032,8 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
     }
     m.tcp_ok = 1;
+    m.tcp_akb = AKB;
+    m.tcp_pkb = PKB;
     return WM_OK;
 }
 
@@ -1048,16 +1044,16 @@ int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;
     p.ln_eps = m.ln_eps;
-    p.E = static_cast<const __nv_bfloat16*>(m.tc_E);
-    p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
-    p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
-    if (m.ranker_kind == WM_RANKER_FOREST) p.bs0 = p.bs1 = p.w3 = p.bs2 = m.zeros;   // (unused scorer, zero image)
+    p.akb = m.tcp_akb; p.pkb = m.tcp_pkb;
+    p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
+    if (m.ranker_kind == WM_RANKER_FOREST) p.bs1 = p.w3 = p.bs2 = m.zeros;   // (unused scorer, zero image)
     p.a = a;
     p.n_tiles = (int)((a.B + tcp::TMP - 1) / tcp::TMP);
     p.prof = trace::begin(st);
     CUtensorMap tm;
     memcpy(&tm, m.tcp_tmap, sizeof(tm));
-    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, m.hidden, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
+    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
     const int max_pairs = ctx->n_sms / 2;
     const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
     const bool prefix_call = a.start || a.init_index || a.latents_out;
