@@ -79,6 +79,16 @@ __device__ __forceinline__ void mbar_wait_warp(uint32_t bar, uint32_t parity) {
             if (clock64() - t0 > 4000000000LL) __trap();
     }
 }
+// Call-free bounded wait for any thread: a function call inside a warpgroup that has raised its register count with
+// setmaxnreg keeps ptxas from budgeting that region above the launch-time count (measured: the epilogue of
+// wm_tcp_kernel stayed at 128 registers and spilled 4 KB until its waits lost their out-of-line slow path).
+__device__ __forceinline__ void mbar_wait_inline(uint32_t bar, uint32_t parity) {
+    if (!mbar_try_wait(bar, parity)) {
+        const long long t0 = clock64();
+        while (!mbar_try_wait(bar, parity))
+            if (clock64() - t0 > 4000000000LL) __trap();
+    }
+}
 __device__ __forceinline__ void fence_barrier_init() {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }

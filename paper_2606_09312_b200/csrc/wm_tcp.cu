@@ -205,6 +205,12 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     const uint32_t T_Z = tmem_base;                 // fp32 latent / GEMM2 accumulator, 256 columns
     const uint32_t T_D1 = tmem_base + 256;          // two 128-column GEMM1 accumulators
 
+    // Register hand-over between warpgroups (the kernel is launched with 128 per thread): the two epilogue warpgroups
+    // take 176 each — the LayerNorm holds a row's 128 fp32 columns in registers: ONE pass over tensor memory instead of
+    // two — the service warpgroup (allocator, producer, MMA issuer) keeps 96, the action-feature warpgroup 64.
+    // (each warpgroup executes ONE setmaxnreg instruction, at the head of its own branch: ptxas budgets the code below it)
+    if (warp >= ALLOC_WARP) {
+    reg_dealloc<96>();
     if (warp == PROD_WARP) {
         // =============================================================== tile schedule + TMA producer
         uint32_t stage = 0, ph = 0;
@@ -450,8 +456,10 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         }
         __syncwarp();
     }
-    else if (warp >= EPI_WARP0 && warp < ACT_WARP0) {
+    }
+    else if (warp < ACT_WARP0) {
         // =============================================================== epilogue warps (GELU / LayerNorm / scorer)
+        reg_alloc<176>();
         const int q = warp & 3, hh = (warp - EPI_WARP0) >> 2;
         const int row = 32 * q + lane;
         const uint32_t lane_off = (uint32_t)(32 * q) << 16;
@@ -461,21 +469,20 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
         const float inv_d = 1.0f / (float)D;
         WM_TRACE_DECL(warp == 0 ? p.prof : nullptr, 2)
-        // write 32 consecutive z columns of this row: fp32 -> TMEM, fp16 -> A1 (when `to_smem`)
-        auto put_z = [&](int col0, const uint32_t (&v)[32], bool to_smem) {
-            tmem_st32(T_Z + lane_off + (uint32_t)col0, v);
-            if (to_smem) {
-                uint8_t* kb = a1 + (col0 >> 6) * KB_BYTES;
-                const int chunk0 = (col0 & 63) >> 3;
+        // The latent lives twice: fp16 z in A1 (GEMM1's operand, the scorer's input) and fp32 z + b2 in TMEM — GEMM2
+        // accumulates W2 h onto it, so the accumulator IS LayerNorm's input z + W2 h + b2 and no pass adds b2.
+        // 32 consecutive columns of this row: z (fp32 values in v) -> fp16 -> A1
+        auto z_to_smem = [&](int col0, const uint32_t* v) {
+            uint8_t* kb = a1 + (col0 >> 6) * KB_BYTES;
+            const int chunk0 = (col0 & 63) >> 3;
 #pragma unroll
-                for (int ch = 0; ch < 4; ++ch) {
-                    uint4 o;
-                    o.x = pack_f16(__uint_as_float(v[8 * ch + 0]), __uint_as_float(v[8 * ch + 1]));
-                    o.y = pack_f16(__uint_as_float(v[8 * ch + 2]), __uint_as_float(v[8 * ch + 3]));
-                    o.z = pack_f16(__uint_as_float(v[8 * ch + 4]), __uint_as_float(v[8 * ch + 5]));
-                    o.w = pack_f16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
-                    *reinterpret_cast<uint4*>(kb + sw128_off(row, chunk0 + ch)) = o;
-                }
+            for (int ch = 0; ch < 4; ++ch) {
+                uint4 o;
+                o.x = pack_f16(__uint_as_float(v[8 * ch + 0]), __uint_as_float(v[8 * ch + 1]));
+                o.y = pack_f16(__uint_as_float(v[8 * ch + 2]), __uint_as_float(v[8 * ch + 3]));
+                o.z = pack_f16(__uint_as_float(v[8 * ch + 4]), __uint_as_float(v[8 * ch + 5]));
+                o.w = pack_f16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
+                *reinterpret_cast<uint4*>(kb + sw128_off(row, chunk0 + ch)) = o;
             }
         };
         auto publish = [&](uint32_t leader_bar, bool smem_written) {
@@ -489,7 +496,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         // the constant-1 feature column), fp16 result to TMEM at dst_col.  Both TMEM loads are in flight before the first use.
         auto gelu_chunk = [&](int b, uint32_t dst_col) {
             WM_TRACE(40);
-            mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+            mbar_wait_inline(bar(B_D1FULL + b), n_d1[b] & 1);
             WM_TRACE(41);
             ++n_d1[b];
             tc_fence_after();
@@ -509,7 +516,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
-            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            mbar_wait_inline(bar(B_SFULL + slot), (it >> 1) & 1);
             const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
@@ -537,38 +544,40 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                     for (int i = 0; i < 32; ++i) v[i] = 0u;
                 }
-                put_z(col0, v, true);
+                z_to_smem(col0, v);
+                const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float4 bb = b2v[i];
+                    v[4 * i + 0] = __float_as_uint(__uint_as_float(v[4 * i + 0]) + bb.x);
+                    v[4 * i + 1] = __float_as_uint(__uint_as_float(v[4 * i + 1]) + bb.y);
+                    v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) + bb.z);
+                    v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) + bb.w);
+                }
+                tmem_st32(T_Z + lane_off + (uint32_t)col0, reinterpret_cast<const uint32_t(&)[32]>(v));
             }
             publish(r_zready, true);
 
             for (int t = 0; t < nsteps; ++t) {
                 for (int c = 0; c < NC; ++c)
                     gelu_chunk(c & 1, T_D1 + 128u * (c & 1) + 64u * hh);
-                // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
+                // ---- LayerNorm(z + W2 h + b2) = LayerNorm(accumulator), this thread's 128 columns held in registers
                 WM_TRACE(50);
-                mbar_wait(bar(B_D2FULL), n_d2 & 1);
+                mbar_wait_inline(bar(B_D2FULL), n_d2 & 1);
                 WM_TRACE(51);
                 ++n_d2;
                 tc_fence_after();
-                float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
-#pragma unroll 1
-                for (int p4 = 0; p4 < 4; ++p4) {
-                    const int col0 = 128 * hh + 32 * p4;
-                    uint32_t v[32];
-                    tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
-                    tmem_ld_wait();
-                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
+                uint32_t v[128];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const float4 bb = b2v[i];
-                        const float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
-                                                     make_float2(bb.x, bb.y));
-                        const float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
-                                                     make_float2(bb.z, bb.w));
-                        s1v = __fadd2_rn(s1v, __fadd2_rn(x0, x1));
-                        s2v = __ffma2_rn(x0, x0, s2v);
-                        s2v = __ffma2_rn(x1, x1, s2v);
-                    }
+                for (int p4 = 0; p4 < 4; ++p4)
+                    tmem_ld32(T_Z + lane_off + (uint32_t)(128 * hh + 32 * p4), reinterpret_cast<uint32_t(&)[32]>(v[32 * p4]));
+                tmem_ld_wait();
+                float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
+#pragma unroll
+                for (int i = 0; i < 64; ++i) {
+                    const float2 x = make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+                    s1v = __fadd2_rn(s1v, x);
+                    s2v = __ffma2_rn(x, x, s2v);
                 }
                 const float s1 = s1v.x + s1v.y, s2 = s2v.x + s2v.y;
                 // exchanged through the slot of this LayerNorm's parity: the partner reads the previous LayerNorm's value
@@ -589,37 +598,42 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     else if (st + t == len - 1)
                         lat = reinterpret_cast<float4*>(p.a.latents_out + (size_t)cand * D);
                 }
-#pragma unroll 1
+                const float2 rs2 = make_float2(rstd, rstd), mr2 = make_float2(-mean * rstd, -mean * rstd);
+#pragma unroll
                 for (int p4 = 0; p4 < 4; ++p4) {
                     const int col0 = 128 * hh + 32 * p4;
-                    uint32_t v[32];
-                    tmem_ld32(T_Z + lane_off + (uint32_t)col0, v);
-                    tmem_ld_wait();
-                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
+                    uint32_t* vv = v + 32 * p4;
                     const float4* gv = reinterpret_cast<const float4*>(s_gamma + col0);
                     const float4* bev = reinterpret_cast<const float4*>(s_beta + col0);
-                    const float2 rs2 = make_float2(rstd, rstd), mr2 = make_float2(-mean * rstd, -mean * rstd);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
-                        const float4 bb = b2v[i], gg = gv[i], be = bev[i];
-                        float2 x0 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
-                                               make_float2(bb.x, bb.y));
-                        float2 x1 = __fadd2_rn(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
-                                               make_float2(bb.z, bb.w));
+                        const float4 gg = gv[i], be = bev[i];
+                        float2 x0 = make_float2(__uint_as_float(vv[4 * i]), __uint_as_float(vv[4 * i + 1]));
+                        float2 x1 = make_float2(__uint_as_float(vv[4 * i + 2]), __uint_as_float(vv[4 * i + 3]));
                         x0 = __ffma2_rn(__ffma2_rn(x0, rs2, mr2), make_float2(gg.x, gg.y), make_float2(be.x, be.y));
                         x1 = __ffma2_rn(__ffma2_rn(x1, rs2, mr2), make_float2(gg.z, gg.w), make_float2(be.z, be.w));
-                        v[4 * i] = __float_as_uint(x0.x); v[4 * i + 1] = __float_as_uint(x0.y);
-                        v[4 * i + 2] = __float_as_uint(x1.x); v[4 * i + 3] = __float_as_uint(x1.y);
+                        vv[4 * i] = __float_as_uint(x0.x); vv[4 * i + 1] = __float_as_uint(x0.y);
+                        vv[4 * i + 2] = __float_as_uint(x1.x); vv[4 * i + 3] = __float_as_uint(x1.y);
                     }
                     // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
                     // fp32 master is never read again
-                    put_z(col0, v, live);
+                    if (live) z_to_smem(col0, vv);
                     if (lat) {
 #pragma unroll
                         for (int i = 0; i < 8; ++i)
-                            lat[(col0 >> 2) + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
-                                                               __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+                            lat[(col0 >> 2) + i] = make_float4(__uint_as_float(vv[4 * i]), __uint_as_float(vv[4 * i + 1]),
+                                                               __uint_as_float(vv[4 * i + 2]), __uint_as_float(vv[4 * i + 3]));
                     }
+                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 bb = b2v[i];
+                        const float2 y0 = __fadd2_rn(make_float2(__uint_as_float(vv[4 * i]), __uint_as_float(vv[4 * i + 1])), make_float2(bb.x, bb.y));
+                        const float2 y1 = __fadd2_rn(make_float2(__uint_as_float(vv[4 * i + 2]), __uint_as_float(vv[4 * i + 3])), make_float2(bb.z, bb.w));
+                        vv[4 * i] = __float_as_uint(y0.x); vv[4 * i + 1] = __float_as_uint(y0.y);
+                        vv[4 * i + 2] = __float_as_uint(y1.x); vv[4 * i + 3] = __float_as_uint(y1.y);
+                    }
+                    tmem_st32(T_Z + lane_off + (uint32_t)col0, reinterpret_cast<const uint32_t(&)[32]>(v[32 * p4]));
                 }
                 publish(r_zready, true);
                 WM_TRACE(53);
@@ -633,7 +647,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             float part = 0.0f;
             for (int c = 0; c < 4; ++c) {
                 const int b = c & 1;
-                mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
+                mbar_wait_inline(bar(B_D1FULL + b), n_d1[b] & 1);
                 ++n_d1[b];
                 tc_fence_after();
 #pragma unroll
@@ -655,8 +669,9 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (hh == 0 && cand >= 0 && (!EXT || p.a.scores_out)) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
             named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
         }
-    } else if (warp >= ACT_WARP0 && warp < ACT_WARP0 + 4) {
+    } else {
         // =============================================================== action-feature warps (one row per lane)
+        reg_dealloc<64>();
         // Per step a row's action enters GEMM1 as the feature row f_t = [onehot(id) (NT) | log2 p_j (P) | 1] of K-block 4
         // (and 5 when NT + P + 1 > 64): the embedding tables and biases are folded into the weights (tcp_prepare).
         const int aw = warp - ACT_WARP0;
