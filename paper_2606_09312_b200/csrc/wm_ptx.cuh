@@ -340,6 +340,15 @@ __device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// The same with the default semantics (release at CTA scope), as CUTLASS's ClusterBarrier::arrive(cta_id) does.  The
+// cluster-scope release above compiles to MEMBAR.ALL.GPU + ERRBAR + CGAERRBAR in front of the arrive: measured ~1500
+// cycles per publish in wm_tcp_kernel (more than the GELU it publishes).  What the pair kernels hand over is either
+// tensor memory (completed by tcgen05.wait::st and ordered by tcgen05.fence::before_thread_sync) or the arriving CTA's
+// OWN shared memory, made visible to its own async proxy by fence.proxy.async before the arrive; the MMA the leader
+// then issues reads each CTA's operands through that CTA's own SM, so no generic-proxy data crosses CTAs.
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     asm volatile(

@@ -280,7 +280,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         auto wait_h = [&](int b) {
             if (pend[b]) {
                 WM_TRACE(10 + b);
-                mbar_wait_cluster_warp(bar(B_HREADY + b), n_h[b] & 1);
+                mbar_wait_warp(bar(B_HREADY + b), n_h[b] & 1);
                 WM_TRACE(12 + b);
                 ++n_h[b];
                 pend[b] = false;
@@ -394,12 +394,12 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 wait_h(0);
                 wait_h(1);
                 WM_TRACE(1);
-                mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after();
+                mbar_wait_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after();
                 WM_TRACE(2);
                 stage_a01();
                 if (NC == 2) commit(B_AFREE);
                 WM_TRACE(3);
-                mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after();
+                mbar_wait_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after();
                 WM_TRACE(4);
                 stage_z(0); commit(B_D1FULL + 0); pend[0] = true;
                 stage_z(1); commit(B_D1FULL + 1); pend[1] = true;
@@ -423,7 +423,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 }
             }
             if (!rank_it) {   // nothing to rank: only take the terminal latent's ZREADY so the phase count stays in step
-                mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1);
+                mbar_wait_warp(bar(B_ZREADY), n_z & 1);
                 ++n_z;
                 continue;
             }
@@ -433,10 +433,10 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             for (int c = 0; c < 4; ++c) {
                 const int b = c & 1;
                 wait_h(b);
-                if (c == 0) { mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
+                if (c == 0) { mbar_wait_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
                 stage_a(b, PKB, true);
                 if (c == 3) commit(B_AFREE);
-                if (c == 0) { mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
+                if (c == 0) { mbar_wait_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
                 stage_z(b);
                 commit(B_D1FULL + b);
                 pend[b] = true;
@@ -487,10 +487,11 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         };
         auto publish = [&](uint32_t leader_bar, bool smem_written) {
             tmem_st_wait();
+            WM_TRACE(45);
             if (smem_written) fence_proxy_async();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(leader_bar);
+            if (lane == 0) mbar_arrive_remote(leader_bar);
         };
         // GELU over this thread's 64 columns of accumulator buffer b (the bias is already in the accumulator: it rides on
         // the constant-1 feature column), fp16 result to TMEM at dst_col.  Both TMEM loads are in flight before the first use.
@@ -504,12 +505,14 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh, v0);
             tmem_ld32(T_D1 + 128u * b + lane_off + 64u * hh + 32u, v1);
             tmem_ld_wait();
+            WM_TRACE(43);
 #pragma unroll
             for (int i = 0; i < 16; ++i) o[i] = gelu2_h2(__uint_as_float(v0[2 * i]), __uint_as_float(v0[2 * i + 1]));
             tmem_st16(dst_col + lane_off, o);
 #pragma unroll
             for (int i = 0; i < 16; ++i) o[i] = gelu2_h2(__uint_as_float(v1[2 * i]), __uint_as_float(v1[2 * i + 1]));
             tmem_st16(dst_col + lane_off + 16u, o);
+            WM_TRACE(44);
             publish(b == 0 ? r_hready0 : r_hready1, false);
             WM_TRACE(42);
         };
@@ -572,6 +575,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int p4 = 0; p4 < 4; ++p4)
                     tmem_ld32(T_Z + lane_off + (uint32_t)(128 * hh + 32 * p4), reinterpret_cast<uint32_t(&)[32]>(v[32 * p4]));
                 tmem_ld_wait();
+                WM_TRACE(54);
                 float2 s1v = make_float2(0.0f, 0.0f), s2v = make_float2(0.0f, 0.0f);
 #pragma unroll
                 for (int i = 0; i < 64; ++i) {
@@ -584,6 +588,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 // from the other slot, so no second barrier is needed before the next one writes
                 float2* red = s_red + (n_d2 & 1u) * 2 * TM;
                 red[hh * TM + row] = make_float2(s1, s2);
+                WM_TRACE(55);
                 named_bar_sync(1 + q, 64);
                 const float2 other = red[(hh ^ 1) * TM + row];
                 WM_TRACE(52);
@@ -662,7 +667,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(b == 0 ? r_hready0 : r_hready1);
+                if (lane == 0) mbar_arrive_remote(b == 0 ? r_hready0 : r_hready1);
             }
             s_red[hh * TM + row] = make_float2(part, 0.0f);
             named_bar_sync(1 + q, 64);
@@ -797,7 +802,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(r_aready);
+                if (lane == 0) mbar_arrive_remote(r_aready);
                 WM_TRACE(73);
             }
 
@@ -850,7 +855,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             fence_proxy_async();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(r_aready);
+            if (lane == 0) mbar_arrive_remote(r_aready);
         }
     }
 
