@@ -247,7 +247,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         auto wait_h = [&](int b) {
             if (pend[b]) {
                 WM_TRACE(10 + b);
-                mbar_wait_cluster_warp(bar(B_HREADY + b), n_h[b] & 1);
+                mbar_wait_warp(bar(B_HREADY + b), n_h[b] & 1);
                 WM_TRACE(12 + b);
                 ++n_h[b];
                 pend[b] = false;
@@ -304,12 +304,12 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         auto gemm_a1 = [&](int b, bool first_chunk, bool last_chunk, bool with_hw) {
             wait_h(b);
             const uint32_t d = T_D1 + 128u * b;
-            if (first_chunk) { WM_TRACE(20); mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); }
+            if (first_chunk) { WM_TRACE(20); mbar_wait_warp(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); }
 #pragma unroll 1
             for (int k = 0; k < 4; ++k) stage_ss(d, s_a1 + (8 + k) * KB_BYTES, k == 0);
             if (with_hw) stage_hw(d);
             if (last_chunk) commit(B_AFREE);
-            if (first_chunk) { WM_TRACE(22); mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); }
+            if (first_chunk) { WM_TRACE(22); mbar_wait_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); }
 #pragma unroll 1
             for (int k = 0; k < 8; ++k) stage_ss(d, s_a1 + k * KB_BYTES, false);
             commit(B_D1FULL + b);
@@ -331,13 +331,13 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 // section of a step); then the z K-blocks of chunks 0 and 1.  (NC >= 2.)
                 wait_h(0);
                 wait_h(1);
-                WM_TRACE(20); mbar_wait_cluster_warp(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after();
+                WM_TRACE(20); mbar_wait_warp(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after();
 #pragma unroll 1
                 for (int b = 0; b < 2; ++b)
 #pragma unroll 1
                     for (int k = 0; k < 4; ++k) stage_ss(T_D1 + 128u * b, s_a1 + (8 + k) * KB_BYTES, k == 0);
                 if (NC == 2) commit(B_AFREE);
-                WM_TRACE(22); mbar_wait_cluster_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after();
+                WM_TRACE(22); mbar_wait_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after();
 #pragma unroll 1
                 for (int b = 0; b < 2; ++b) {
 #pragma unroll 1
@@ -430,7 +430,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             fence_proxy_async();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(leader_bar);
+            if (lane == 0) mbar_arrive_remote(leader_bar);
         };
         auto wait_d1 = [&](int b) {
             mbar_wait(bar(B_D1FULL + b), n_d1[b] & 1);
@@ -610,7 +610,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 dot32(T_D1 + 128u * b + 64u * e + 32u + lane_off, 512 + 256 * b + 64 * part + 32);
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(b == 0 ? r_hready0 : r_hready1);
+                if (lane == 0) mbar_arrive_remote(b == 0 ? r_hready0 : r_hready1);
             }
             s_red[part * TMR + row] = make_float2(acc, 0.0f);
             named_bar_sync(1 + rh, 128);
@@ -727,7 +727,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 }
                 fence_proxy_async();
                 __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
-                if (lane == 0) mbar_arrive_cluster(r_aready);
+                if (lane == 0) mbar_arrive_remote(r_aready);
             }
 
             // ---- the phi K-blocks (8-11) of the scorer's A operand.  phi = mean_t a_t = (sum_c count_c E[c] +
@@ -773,7 +773,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             fence_proxy_async();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(r_aready);
+            if (lane == 0) mbar_arrive_remote(r_aready);
         }
     }
 

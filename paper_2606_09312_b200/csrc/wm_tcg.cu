@@ -215,7 +215,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         auto wait_x = [&](int b) {       // accumulator b read by the epilogue (and that epilogue's output written)
             if ((pend >> b) & 1u) {
                 WM_TRACE(10 + b);
-                mbar_wait_cluster(bar(B_XFREE + b), (xpar >> b) & 1u);
+                mbar_wait(bar(B_XFREE + b), (xpar >> b) & 1u);
                 WM_TRACE(15);
                 xpar ^= 1u << b;
                 pend &= ~(1u << b);
@@ -274,8 +274,8 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         };
         auto a_part = [&](int b) { seg_a(b, true); };
         auto z_part = [&](int b, uint32_t zbase) { seg_z(b, zbase, false); finish(b); };
-        auto wait_a = [&]() { WM_TRACE(20); mbar_wait_cluster(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); };
-        auto wait_z = [&]() { WM_TRACE(22); mbar_wait_cluster(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); };
+        auto wait_a = [&]() { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); };
+        auto wait_z = [&]() { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); };
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
             mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
@@ -371,8 +371,8 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             tc_fence_before();
             __syncwarp();
             if (lane == 0) {
-                mbar_arrive_cluster(bar_a);
-                if (bar_b) mbar_arrive_cluster(bar_b);
+                mbar_arrive_remote(bar_a);
+                if (bar_b) mbar_arrive_remote(bar_b);
             }
         };
 
@@ -480,7 +480,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 blend(1, 1, true);
                 // both tiles of z' are written (the arrivals above already ordered the writes)
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(r_zready);
+                if (lane == 0) mbar_arrive_remote(r_zready);
             }
 
             // ---- scorer layer 1 -> h1 (fp16): tiles 0, 1 into the spare z buffer, tiles 2, 3 into the r*z buffer
@@ -526,7 +526,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(r_xfree(xb));
+                if (lane == 0) mbar_arrive_remote(r_xfree(xb));
             }
             s_red[part * TMR + row] = acc;
             named_bar_sync(1 + rh, 128);
@@ -652,7 +652,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 }
                 fence_proxy_async();
                 __syncwarp();   // also: phase 2 reads of s_idx are done before the next phase 1 overwrites
-                if (lane == 0) mbar_arrive_cluster(r_aready);
+                if (lane == 0) mbar_arrive_remote(r_aready);
             }
 
             // ---- phi = mean_t a_t (0 when len = 0)
@@ -684,7 +684,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             fence_proxy_async();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(r_aready);
+            if (lane == 0) mbar_arrive_remote(r_aready);
         }
     }
 
