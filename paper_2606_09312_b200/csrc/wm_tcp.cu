@@ -69,7 +69,8 @@ enum {
     B_D1FULL = B_EMPTY + NSTAGE,   // [2] MMA commit -> epilogue: accumulator buffer b filled
     B_HREADY = B_D1FULL + 2,       // [2] epilogue (both CTAs) -> leader MMA: buffer b read, fp16 hidden written to TMEM
     B_D2FULL = B_HREADY + 2,       // MMA commit -> epilogue: GEMM2 of the step done
-    B_ZREADY,                      // epilogue (both CTAs) -> leader MMA: z written
+    B_ZREADY,                      // epilogue (both CTAs) -> leader MMA: z K-blocks 0 and 2 written (first half of every thread's columns)
+    B_ZREADY2,                     // ... K-blocks 1 and 3 written, and the fp32 latent in TMEM
     B_AFREE,                       // MMA commit -> action warps: a-part of A1 no longer read
     B_AREADY,                      // action warps (both CTAs) -> leader MMA: a-part written
     B_SFULL,                       // [2] schedule slot filled (CTA-local)
@@ -178,6 +179,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         }
         mbar_init(bar(B_D2FULL), 1);
         mbar_init(bar(B_ZREADY), 16);
+        mbar_init(bar(B_ZREADY2), 16);
         mbar_init(bar(B_AFREE), 1);
         mbar_init(bar(B_AREADY), 8);
         fence_barrier_init();
@@ -187,7 +189,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     for (int i = threadIdx.x; i < D; i += THREADS) {
         s_b2[i] = __ldg(p.b2 + i);
         s_gamma[i] = __ldg(p.gamma + i);
-        s_beta[i] = __ldg(p.beta + i);
+        s_beta[i] = __ldg(p.beta + i) + __ldg(p.b2 + i);   // the latent is carried as u = z + b2 (see the epilogue)
     }
     {
         // the hw K-block is only ever written in its first columns: clear it once so unread bytes are not NaNs
@@ -349,6 +351,33 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             advance();
         };
+        // step boundary, stage 1: z K-blocks 0 and 2 (published first by the LayerNorm) of chunk buffers 0 and 1
+        auto stage_za = [&]() {
+            acquire_stage();
+            if (elect_one()) {
+                kb_ss(TD1, a_lo, b_lo, false);
+                kb_ss(TD1, a_lo + 2 * KBL, b_lo + HBL, false);
+                kb_ss(TD1 + 128u, a_lo, b_lo + 2 * HBL, false);
+                kb_ss(TD1 + 128u, a_lo + 2 * KBL, b_lo + 3 * HBL, false);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // step boundary, stage 2: z K-blocks 1 and 3 of chunk buffer 0 (accumulator 0 complete: published from inside the
+        // stage), then of chunk buffer 1
+        auto stage_zb = [&]() {
+            acquire_stage();
+            if (elect_one()) {
+                kb_ss(TD1, a_lo + KBL, b_lo, false);
+                kb_ss(TD1, a_lo + 3 * KBL, b_lo + HBL, false);
+                mma_commit2(bar(B_D1FULL + 0));
+                kb_ss(TD1 + 128u, a_lo + KBL, b_lo + 2 * HBL, false);
+                kb_ss(TD1 + 128u, a_lo + 3 * KBL, b_lo + 3 * HBL, false);
+                mma_commit2(bar(B_EMPTY + stage));
+                mma_commit2(bar(B_D1FULL + 1));
+            }
+            advance();
+        };
         // stage: GEMM2 of hidden chunk buffer b (fp16 in TMEM: K-block 0 at +0, K-block 1 at +64 columns) x all 256
         // latent columns: two consecutive boxes are this CTA's 128 weight rows of one [256 x 64] B tile, 4 MMAs with N = 256
         auto stage_g2 = [&](int b) {
@@ -399,10 +428,12 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 stage_a01();
                 if (NC == 2) commit(B_AFREE);
                 WM_TRACE(3);
-                mbar_wait_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after();
+                mbar_wait_warp(bar(B_ZREADY), n_z & 1); tc_fence_after();
                 WM_TRACE(4);
-                stage_z(0); commit(B_D1FULL + 0); pend[0] = true;
-                stage_z(1); commit(B_D1FULL + 1); pend[1] = true;
+                stage_za();
+                mbar_wait_warp(bar(B_ZREADY2), n_z & 1); ++n_z; tc_fence_after();
+                stage_zb();
+                pend[0] = pend[1] = true;
                 wait_h(0);
                 stage_g2(0);
                 if (NC == 1) commit(B_D2FULL);
@@ -424,6 +455,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             if (!rank_it) {   // nothing to rank: only take the terminal latent's ZREADY so the phase count stays in step
                 mbar_wait_warp(bar(B_ZREADY), n_z & 1);
+                mbar_wait_warp(bar(B_ZREADY2), n_z & 1);
                 ++n_z;
                 continue;
             }
@@ -436,7 +468,12 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 if (c == 0) { mbar_wait_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after(); }
                 stage_a(b, PKB, true);
                 if (c == 3) commit(B_AFREE);
-                if (c == 0) { mbar_wait_warp(bar(B_ZREADY), n_z & 1); ++n_z; tc_fence_after(); }
+                if (c == 0) {
+                    mbar_wait_warp(bar(B_ZREADY), n_z & 1);
+                    mbar_wait_warp(bar(B_ZREADY2), n_z & 1);
+                    ++n_z;
+                    tc_fence_after();
+                }
                 stage_z(b);
                 commit(B_D1FULL + b);
                 pend[b] = true;
@@ -465,13 +502,15 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         const uint32_t lane_off = (uint32_t)(32 * q) << 16;
         uint8_t* a1 = smem + L.a1;
         const uint32_t r_hready0 = mapa(bar(B_HREADY), 0), r_hready1 = mapa(bar(B_HREADY + 1), 0);
-        const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
+        const uint32_t r_zready = mapa(bar(B_ZREADY), 0), r_zready2 = mapa(bar(B_ZREADY2), 0);
         uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
         const float inv_d = 1.0f / (float)D;
         WM_TRACE_DECL(warp == 0 ? p.prof : nullptr, 2)
-        // The latent lives twice: fp16 z in A1 (GEMM1's operand, the scorer's input) and fp32 z + b2 in TMEM — GEMM2
-        // accumulates W2 h onto it, so the accumulator IS LayerNorm's input z + W2 h + b2 and no pass adds b2.
-        // 32 consecutive columns of this row: z (fp32 values in v) -> fp16 -> A1
+        // The latent is carried as u = z + b2, twice: fp32 in TMEM — GEMM2 accumulates W2 h onto it, so the accumulator IS
+        // LayerNorm's input z + W2 h + b2 and no pass adds b2 — and fp16 in A1 (GEMM1's operand, the scorer's input): the
+        // host subtracts W1z b2 (Ws0z b2) from the bias that rides on the constant feature column (tcp_prepare), and
+        // beta in shared memory is beta + b2, so LayerNorm's output is u directly.
+        // 32 consecutive columns of this row: u (fp32 values in v) -> fp16 -> A1
         auto z_to_smem = [&](int col0, const uint32_t* v) {
             uint8_t* kb = a1 + (col0 >> 6) * KB_BYTES;
             const int chunk0 = (col0 & 63) >> 3;
@@ -484,6 +523,12 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 o.w = pack_f16(__uint_as_float(v[8 * ch + 6]), __uint_as_float(v[8 * ch + 7]));
                 *reinterpret_cast<uint4*>(kb + sw128_off(row, chunk0 + ch)) = o;
             }
+        };
+        // first half of this thread's columns (K-block 2 hh) is in A1: GEMM1 may start on it
+        auto publish_half = [&]() {
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_remote(r_zready);
         };
         auto publish = [&](uint32_t leader_bar, bool smem_written) {
             tmem_st_wait();
@@ -547,7 +592,6 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                     for (int i = 0; i < 32; ++i) v[i] = 0u;
                 }
-                z_to_smem(col0, v);
                 const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
@@ -557,9 +601,11 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     v[4 * i + 2] = __float_as_uint(__uint_as_float(v[4 * i + 2]) + bb.z);
                     v[4 * i + 3] = __float_as_uint(__uint_as_float(v[4 * i + 3]) + bb.w);
                 }
+                z_to_smem(col0, v);
                 tmem_st32(T_Z + lane_off + (uint32_t)col0, reinterpret_cast<const uint32_t(&)[32]>(v));
+                if (p4 == 1) publish_half();
             }
-            publish(r_zready, true);
+            publish(r_zready2, true);
 
             for (int t = 0; t < nsteps; ++t) {
                 for (int c = 0; c < NC; ++c)
@@ -623,24 +669,19 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
                     // fp32 master is never read again
                     if (live) z_to_smem(col0, vv);
-                    if (lat) {
+                    if (EXT && lat) {      // the caller's latent is z = u - b2
+                        const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
 #pragma unroll
-                        for (int i = 0; i < 8; ++i)
-                            lat[(col0 >> 2) + i] = make_float4(__uint_as_float(vv[4 * i]), __uint_as_float(vv[4 * i + 1]),
-                                                               __uint_as_float(vv[4 * i + 2]), __uint_as_float(vv[4 * i + 3]));
-                    }
-                    const float4* b2v = reinterpret_cast<const float4*>(s_b2 + col0);
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const float4 bb = b2v[i];
-                        const float2 y0 = __fadd2_rn(make_float2(__uint_as_float(vv[4 * i]), __uint_as_float(vv[4 * i + 1])), make_float2(bb.x, bb.y));
-                        const float2 y1 = __fadd2_rn(make_float2(__uint_as_float(vv[4 * i + 2]), __uint_as_float(vv[4 * i + 3])), make_float2(bb.z, bb.w));
-                        vv[4 * i] = __float_as_uint(y0.x); vv[4 * i + 1] = __float_as_uint(y0.y);
-                        vv[4 * i + 2] = __float_as_uint(y1.x); vv[4 * i + 3] = __float_as_uint(y1.y);
+                        for (int i = 0; i < 8; ++i) {
+                            const float4 bb = b2v[i];
+                            lat[(col0 >> 2) + i] = make_float4(__uint_as_float(vv[4 * i]) - bb.x, __uint_as_float(vv[4 * i + 1]) - bb.y,
+                                                               __uint_as_float(vv[4 * i + 2]) - bb.z, __uint_as_float(vv[4 * i + 3]) - bb.w);
+                        }
                     }
                     tmem_st32(T_Z + lane_off + (uint32_t)col0, reinterpret_cast<const uint32_t(&)[32]>(v[32 * p4]));
+                    if (p4 == 1) publish_half();
                 }
-                publish(r_zready, true);
+                publish(r_zready2, true);
                 WM_TRACE(53);
             }
 
@@ -919,6 +960,7 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         return empty;
     };
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &b1 = get("b1"), &E = get("E"), &Wp = get("W_p"), &bpv = get("b_p");
+    const std::vector<float>& b2h = get("b2");
     const bool forest = m.ranker_kind == WM_RANKER_FOREST;
     const int hid = m.hidden, NC = hid / 128, K1 = tcp::D + tcp::DA, NT = m.n_types, P = m.P;
     // ---- GEMM1's a-columns folded onto the action features f = [onehot(id) (NT) | log2 p_j (P) | 1]:
@@ -940,6 +982,7 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         }
         double acc = b1[n];
         for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * bpv[k];
+        for (int k = 0; k < tcp::D; ++k) acc -= (double)W1[(size_t)n * K1 + k] * b2h[k];   // the z operand is u = z + b2
         out[NT + P] = (float)acc;
     }
     // ---- scorer layer 1's phi columns as the kernel's phi features see them, plus the bias on a constant-1 column:
@@ -969,7 +1012,9 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
                 for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * bpv[k];
                 out[NT + P] = (float)acc;
             }
-            out[NPSI - 1] = bs0[n];
+            double bias = bs0[n];
+            for (int k = 0; k < tcp::D; ++k) bias -= (double)Ws0[(size_t)n * K0 + k] * b2h[k];           // z_T arrives as u = z_T + b2
+            out[NPSI - 1] = (float)bias;
         }
     }
     const size_t n_slots = (size_t)tcp::step_boxes(NC, AKB) + tcp::scorer_boxes(PKB);
@@ -984,7 +1029,11 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         for (int k = 0; k < 2; ++k)
             for (int hrow = 0; hrow < 2; ++hrow) ok &= append_slot(blob, W2, hid, 64 * hrow, 128, c * 128 + k * 64, 64);
     };
-    g1a(0); g1a(1); g1z(0); g1z(1);
+    g1a(0); g1a(1);
+    // step boundary: z K-blocks 0 and 2 of chunks 0, 1 (stage_za), then K-blocks 1 and 3 (stage_zb)
+    for (int half = 0; half < 2; ++half)
+        for (int c = 0; c < 2; ++c)
+            for (int k = half; k < 4; k += 2) ok &= append_slot(blob, W1, K1, c * 128, 64, k * 64, 64);
     g2(0);
     for (int i = 2; i <= NC; ++i) {
         if (i < NC) { g1a(i); g1z(i); }
