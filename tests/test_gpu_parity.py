@@ -563,6 +563,7 @@ def test_score_from_bank_matches_literal(wm, n):
     d_start = torch.from_numpy(start).cuda(); d_index = torch.from_numpy(index).cuda()
     for path in _paths(wm, cfg):
         ctx = _ctx(wm, cfg, path)
+        variant = wm.wm_get_info(ctx).tc_variant
         lit = gpu_scores(ctx, b)
         bank = torch.zeros((cfg.S + b.B * cfg.T_max, cfg.d), dtype=torch.float32, device="cuda:0")
         bank[:cfg.S] = dv["init_states"]
@@ -580,7 +581,10 @@ def test_score_from_bank_matches_literal(wm, n):
         y = out.cpu().numpy()
         tol = 1e-4 if cfg.dtype == DTYPE_FP32 else (2e-3 if path == wm.PATH_FP32 else 2e-2)
         assert oracle.score_error(y, ref, b.subgraph_offsets) <= tol, (n, path)
-        assert oracle.score_error(y, lit, b.subgraph_offsets) <= 2e-5, (n, path)
+        # against the same path's literal scores: fp32 rounding, except on the pair kernel (tc_variant 5), which carries the
+        # latent as u = z + b2: a banked z reproduces u to one more fp32 rounding, which can move an fp16 operand by an ulp
+        same = 2e-5 if not (path == wm.PATH_TCGEN05 and variant == 5) else 2e-3
+        assert oracle.score_error(y, lit, b.subgraph_offsets) <= same, (n, path)
 
 
 @pytest.mark.parametrize("form", [None, PATH_TC_SINGLE])
@@ -612,10 +616,15 @@ def test_cfg4_prefix_reuse_full_family_structure(wm, form):
     assert wm.wm_check(ctx) == 0
     wm.wm_free(ctx)
     y = out.cpu().numpy()
-    np.testing.assert_array_equal(y.view(np.uint32), lit.view(np.uint32))
     ref = oracle_scores(cfg, gen.make_weights(cfg), b)
     assert oracle.score_error(y, ref, b.subgraph_offsets) <= TOL[False]
-    np.testing.assert_array_equal(gpu_topk(y, b.subgraph_offsets, cfg.k), gpu_topk(lit, b.subgraph_offsets, cfg.k))
+    if form == PATH_TC_SINGLE:      # the bank holds the very fp32 latent the literal rollout carries: bit-identical
+        np.testing.assert_array_equal(y.view(np.uint32), lit.view(np.uint32))
+        np.testing.assert_array_equal(gpu_topk(y, b.subgraph_offsets, cfg.k), gpu_topk(lit, b.subgraph_offsets, cfg.k))
+    else:                           # pair kernel: the latent is carried as u = z + b2, the bank holds z (one more fp32 rounding)
+        assert oracle.score_error(y, lit, b.subgraph_offsets) <= 2e-3
+        ov, _ = oracle.topk_overlap(gpu_topk(y, b.subgraph_offsets, cfg.k), gpu_topk(lit, b.subgraph_offsets, cfg.k))
+        assert ov >= 0.99, ov
 
 
 @pytest.mark.parametrize("n", [1, 2])
