@@ -18,7 +18,7 @@ SOURCES = ["wm_api.cu", "wm_bucket.cu", "wm_forest.cu", "wm_generic.cu", "wm_tc.
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
-if os.environ.get("WM_TC_PROFILE"):   # dev instrumentation of wm_tc.cu (per-role wait-cycle counters)
+if os.environ.get("WM_TC_PROFILE"):   # developer build: the trace macros of csrc/wm_trace.cuh are compiled in
     FLAGS.append("-DWM_TC_PROFILE")
 
 

@@ -28,6 +28,7 @@
 
 #include "wm_internal.h"
 #include "wm_ptx.cuh"
+#include "wm_trace.cuh"
 
 namespace wm {
 
@@ -77,7 +78,7 @@ struct Params {
     CallArgs a;
     int n_tiles;
     int* tile_counter;
-    unsigned long long* prof;   // dev instrumentation trace buffer (WM_TC_PROFILE builds), else nullptr
+    unsigned long long* prof;   // developer trace buffer (wm_trace.cuh), null in a normal build
 };
 
 struct SmemLayout {
@@ -110,22 +111,6 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
 }
 
 using namespace ptx;
-
-// Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of CTA 0 appends
-// (tag, clock) records to a trace buffer that launch_tc dumps.  Compiled out otherwise.
-#ifdef WM_TC_PROFILE
-#define WM_TRACE_DECL(role, cond)                                                                       \
-    uint2* tr_buf = p.prof ? reinterpret_cast<uint2*>(p.prof) + (role) * 8192 : nullptr;                 \
-    const bool tr_on = tr_buf != nullptr && blockIdx.x == 0 && lane == 0 && (cond);                     \
-    uint32_t tr_n = 0;
-#define WM_TRACE(tag)                                                                                   \
-    do {                                                                                                \
-        if (tr_on && tr_n < 8191) { tr_buf[1 + tr_n] = make_uint2((uint32_t)(tag), (uint32_t)clock64()); ++tr_n; tr_buf[0].x = tr_n; } \
-    } while (0)
-#else
-#define WM_TRACE_DECL(role, cond)
-#define WM_TRACE(tag) do { } while (0)
-#endif
 
 }  // namespace tc
 
@@ -245,7 +230,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
             uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
             bool pend[2] = {false, false};
             const uint32_t s_hwk = s_base + L.hwk;
-            WM_TRACE_DECL(0, true)
+            WM_TRACE_DECL(p.prof, 0)
             auto wait_h = [&](int b) {
                 if (pend[b]) {
                     WM_TRACE(10 + b);
@@ -1019,15 +1004,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.n_tiles = (int)((a.B + tc::TM - 1) / tc::TM);
     p.tile_counter = ws->counters + kTileCtrOff;
     WM_CUDA_TRY(cudaMemsetAsync(p.tile_counter, 0, sizeof(int), st));
-    p.prof = nullptr;
-    static unsigned long long* d_prof = nullptr;
-#ifdef WM_TC_PROFILE
-    if (getenv("WM_TC_PROF")) {
-        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, 3 * 8192 * 8));
-        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, 3 * 8192 * 8, st));
-        p.prof = d_prof;
-    }
-#endif
+    p.prof = trace::begin(st);
     const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
     const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
     if (m.phi_kind == WM_PHI_STRUCT) {
@@ -1039,20 +1016,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     }
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
-#ifdef WM_TC_PROFILE
-    if (p.prof) {   // dev instrumentation: dump CTA 0's per-role (tag, clock) traces to WM_TC_PROF's path
-        std::vector<uint2> h(3 * 8192);
-        WM_CUDA_TRY(cudaStreamSynchronize(st));
-        WM_CUDA_TRY(cudaMemcpy(h.data(), d_prof, h.size() * 8, cudaMemcpyDeviceToHost));
-        FILE* f = fopen(getenv("WM_TC_PROF"), "w");
-        if (f) {
-            for (int r = 0; r < 3; ++r)
-                for (uint32_t i = 0; i < h[r * 8192].x; ++i)
-                    fprintf(f, "%d %u %u\n", r, h[r * 8192 + 1 + i].x, h[r * 8192 + 1 + i].y);
-            fclose(f);
-        }
-    }
-#endif
+    trace::dump(p.prof, st);
     return WM_OK;
 }
 

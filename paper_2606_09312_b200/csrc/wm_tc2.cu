@@ -31,6 +31,7 @@
 
 #include "wm_internal.h"
 #include "wm_ptx.cuh"
+#include "wm_trace.cuh"
 
 namespace wm {
 
@@ -56,8 +57,9 @@ constexpr int THREADS = 512;
 constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 11, PROD_WARP = 13, MMA_WARP = 15;
 __device__ __forceinline__ int action_index(int warp) { return warp == 12 ? 3 : (warp >= 8 && warp <= 10) ? warp - 8 : -1; }
 constexpr int MAX_TYPES = 64, MAX_P = 8, MAX_H = 64, MAX_HID = 1024;
-constexpr int G1_STAGES = 12, G2_STAGES = 8;              // per 256-column hidden chunk
-constexpr int SC_STAGES = 4 * 13 + 2 * 32;                // scorer: layer 1 (4 x (4 phi, hw, 8 z)), layer 2 (2 rounds x 16 x 2)
+constexpr int G2_STAGES = 8;                              // per 256-column hidden chunk: GEMM2; GEMM1 takes akb + 8
+// scorer: layer 1 (4 x (pkb phi features, hw, 8 z)), layer 2 (2 rounds x 16 x 2)
+__host__ __device__ inline int sc_stages(int pkb) { return 4 * (pkb + 9) + 2 * 32; }
 
 enum {
     B_FULL = 0,                    // [NSTAGE] TMA (both CTAs) -> leader's MMA warp
@@ -76,32 +78,14 @@ enum {
 
 struct Params {
     int hid, nc, n_types, P, H, hw_ksteps;
+    int akb, pkb;               // K-blocks of the folded action features f_t (1 or 2) and of the phi features (1 or 2)
     float ln_eps;
-    const __nv_bfloat16* E;     // [n_types][256]
-    const float *WpT, *bp;      // [P][256], [256]
-    const float *b1, *b2, *gamma, *beta;
-    const float *bs0, *bs1, *w3, *bs2;
+    const float *b2, *gamma, *beta;
+    const float *bs1, *w3, *bs2;
     CallArgs a;
     int n_tiles;
-    unsigned long long* prof;   // dev instrumentation trace buffer (WM_TC_PROFILE builds), else nullptr
+    unsigned long long* prof;   // developer trace buffer (wm_trace.cuh), null in a normal build
 };
-
-// Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of the leader CTA of pair 0
-// appends (tag, clock) records to a trace buffer that launch_tc2 dumps.  Compiled out otherwise.
-#ifdef WM_TC_PROFILE
-constexpr int TRACE_CAP = 16384;
-#define WM_TRACE_DECL(role)                                                                            \
-    uint2* tr_buf = p.prof ? reinterpret_cast<uint2*>(p.prof) + (role) * TRACE_CAP : nullptr;           \
-    const bool tr_on = tr_buf != nullptr && blockIdx.x == 0 && lane == 0;                              \
-    uint32_t tr_n = 0;
-#define WM_TRACE(tag)                                                                                  \
-    do {                                                                                               \
-        if (tr_on && tr_n < TRACE_CAP - 1) { tr_buf[1 + tr_n] = make_uint2((uint32_t)(tag), (uint32_t)clock64()); ++tr_n; tr_buf[0].x = tr_n; } \
-    } while (0)
-#else
-#define WM_TRACE_DECL(role)
-#define WM_TRACE(tag) do { } while (0)
-#endif
 
 struct SmemLayout {
     uint32_t a1, hbuf, ring, hwk, lp, ids, cnt, b1, red, bars, sched, tmem_slot, total;
@@ -114,8 +98,7 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
     L.hbuf = o; o += 2 * H_KB * KB_BYTES;
     L.ring = o; o += NSTAGE * BT_BYTES;
     L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
-    L.lp = o; o += TMR * MAX_P * 4;
-    L.ids = o; o += TMR * 4;
+    L.lp = o; L.ids = o;                               // (unused since the action features are folded)
     L.cnt = o; o += TMR * (uint32_t)n_types;          // u8 counts, row-major [64][n_types]
     o = (o + 15) & ~15u;
     L.b1 = o; o += 3 * D * 4;                          // b2, gamma, beta (LayerNorm: on the critical path; b1 is __ldg)
@@ -149,7 +132,8 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int NC = p.nc;
-    const int ROLL_STAGES = NC * (G1_STAGES + G2_STAGES);
+    const int AKB = p.akb, PKB = p.pkb;
+    const int ROLL_STAGES = NC * (AKB + 8 + G2_STAGES);
 
     // ---- one-time setup
     if (threadIdx.x == 0) {
@@ -191,7 +175,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     if (warp == PROD_WARP) {
         // =============================================================== tile schedule + TMA producer
         uint32_t stage = 0, ph = 0;
-        WM_TRACE_DECL(1)
+        WM_TRACE_DECL(p.prof, 1)
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
             int tile = tile_of((int)it, pair, n_pairs, p.n_tiles);
@@ -213,7 +197,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             if (tile < 0) break;
             if (lane == 0) {
-                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + SC_STAGES;
+                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + sc_stages(PKB);
                 int src = 0;
                 for (int i = 0; i < total; ++i) {
                     if (i == roll_total) src = ROLL_STAGES;
@@ -243,7 +227,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
         bool pend[2] = {false, false};
         const uint32_t s_hwk = s_base + L.hwk;
-        WM_TRACE_DECL(0)
+        WM_TRACE_DECL(p.prof, 0)
         auto wait_h = [&](int b) {
             if (pend[b]) {
                 WM_TRACE(10 + b);
@@ -305,8 +289,9 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             wait_h(b);
             const uint32_t d = T_D1 + 128u * b;
             if (first_chunk) { WM_TRACE(20); mbar_wait_warp(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); }
+            const int nk = with_hw ? PKB : AKB;      // scorer layer 1: phi features; rollout: action features
 #pragma unroll 1
-            for (int k = 0; k < 4; ++k) stage_ss(d, s_a1 + (8 + k) * KB_BYTES, k == 0);
+            for (int k = 0; k < nk; ++k) stage_ss(d, s_a1 + (8 + k) * KB_BYTES, k == 0);
             if (with_hw) stage_hw(d);
             if (last_chunk) commit(B_AFREE);
             if (first_chunk) { WM_TRACE(22); mbar_wait_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); }
@@ -335,7 +320,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll 1
                 for (int b = 0; b < 2; ++b)
 #pragma unroll 1
-                    for (int k = 0; k < 4; ++k) stage_ss(T_D1 + 128u * b, s_a1 + (8 + k) * KB_BYTES, k == 0);
+                    for (int k = 0; k < AKB; ++k) stage_ss(T_D1 + 128u * b, s_a1 + (8 + k) * KB_BYTES, k == 0);
                 if (NC == 2) commit(B_AFREE);
                 WM_TRACE(22); mbar_wait_warp(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after();
 #pragma unroll 1
@@ -407,7 +392,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
         uint32_t n_d1[2] = {0, 0}, n_d2 = 0, n_hw[2] = {0, 0};
         const float inv_d = 1.0f / (float)D;
-        WM_TRACE_DECL(2)
+        WM_TRACE_DECL(p.prof, 2)
         // write 32 consecutive z columns of this row (N tile j, 32-column half `half` of the thread's quarter):
         // fp32 -> TMEM, fp16 -> A1 K-block 4 j + part (when `to_smem`)
         auto put_z = [&](int j, int half, const uint32_t (&v)[32], bool to_smem) {
@@ -437,38 +422,38 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             ++n_d1[b];
             tc_fence_after();
         };
-        // bias + GELU over this thread's 64 columns of accumulator b -> fp16 row of the K-block at dst (SW128)
-        auto gelu_to_smem = [&](int b, const float* bias, bool bias_in_smem, uint8_t* dst) {
+        // GELU over this thread's 64 columns of accumulator b (the bias is already in the accumulator: it rides on the
+        // constant-1 feature column) -> fp16 row of the K-block at dst (SW128).  Packed fp16x2 arithmetic (gelu2_h2).
+        auto gelu_to_smem = [&](int b, uint8_t* dst) {
+            uint32_t v0[32], v1[32];
+            tmem_ld32(T_D1 + 128u * b + 64u * e + lane_off, v0);
+            tmem_ld32(T_D1 + 128u * b + 64u * e + 32u + lane_off, v1);
+            tmem_ld_wait();
 #pragma unroll
-            for (int p2 = 0; p2 < 2; ++p2) {
-                uint32_t v[32], o[16];
-                tmem_ld32(T_D1 + 128u * b + 64u * e + 32u * p2 + lane_off, v);
-                tmem_ld_wait();
-                const float4* bp_ = reinterpret_cast<const float4*>(bias + 32 * p2);
+            for (int ch = 0; ch < 4; ++ch)
+                *reinterpret_cast<uint4*>(dst + sw128_off(row, ch)) =
+                    make_uint4(gelu2_h2(__uint_as_float(v0[8 * ch + 0]), __uint_as_float(v0[8 * ch + 1])),
+                               gelu2_h2(__uint_as_float(v0[8 * ch + 2]), __uint_as_float(v0[8 * ch + 3])),
+                               gelu2_h2(__uint_as_float(v0[8 * ch + 4]), __uint_as_float(v0[8 * ch + 5])),
+                               gelu2_h2(__uint_as_float(v0[8 * ch + 6]), __uint_as_float(v0[8 * ch + 7])));
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float4 bv = bias_in_smem ? bp_[i] : __ldg(bp_ + i);
-                    o[2 * i] = gelu2_f16(make_float2(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1])),
-                                          make_float2(bv.x, bv.y));
-                    o[2 * i + 1] = gelu2_f16(make_float2(__uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3])),
-                                              make_float2(bv.z, bv.w));
-                }
-#pragma unroll
-                for (int ch = 0; ch < 4; ++ch)
-                    *reinterpret_cast<uint4*>(dst + sw128_off(row, 4 * p2 + ch)) =
-                        make_uint4(o[4 * ch], o[4 * ch + 1], o[4 * ch + 2], o[4 * ch + 3]);
-            }
+            for (int ch = 0; ch < 4; ++ch)
+                *reinterpret_cast<uint4*>(dst + sw128_off(row, 4 + ch)) =
+                    make_uint4(gelu2_h2(__uint_as_float(v1[8 * ch + 0]), __uint_as_float(v1[8 * ch + 1])),
+                               gelu2_h2(__uint_as_float(v1[8 * ch + 2]), __uint_as_float(v1[8 * ch + 3])),
+                               gelu2_h2(__uint_as_float(v1[8 * ch + 4]), __uint_as_float(v1[8 * ch + 5])),
+                               gelu2_h2(__uint_as_float(v1[8 * ch + 6]), __uint_as_float(v1[8 * ch + 7])));
             publish(b == 0 ? r_hready0 : r_hready1, false);
         };
         // hidden chunk into hidden buffer b (waits until GEMM2 no longer reads the buffer's previous contents)
-        auto gelu_to_h = [&](int b, const float* bias, bool bias_in_smem) {
+        auto gelu_to_h = [&](int b) {
             WM_TRACE(40);
             wait_d1(b);
             WM_TRACE(41);
             mbar_wait(bar(B_HFREE + b), (n_hw[b] & 1) ^ 1);
             ++n_hw[b];
             WM_TRACE(42);
-            gelu_to_smem(b, bias, bias_in_smem, hb + (b * H_KB + part) * KB_BYTES);
+            gelu_to_smem(b, hb + (b * H_KB + part) * KB_BYTES);
             WM_TRACE(43);
         };
 
@@ -505,7 +490,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             publish(r_zready, true);
 
             for (int t = 0; t < nsteps; ++t) {
-                for (int c = 0; c < NC; ++c) gelu_to_h(c & 1, p.b1 + c * 256 + 64 * part, false);
+                for (int c = 0; c < NC; ++c) gelu_to_h(c & 1);
                 // ---- LayerNorm(z + W2 h + b2): the accumulator already holds z + W2 h
                 WM_TRACE(50);
                 mbar_wait(bar(B_D2FULL), n_d2 & 1);
@@ -578,13 +563,13 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
 
             // ---- scorer layer 1 -> h1 (fp16): chunks 0, 1 into the hidden buffers ...
-            gelu_to_h(0, p.bs0 + 64 * part, false);
-            gelu_to_h(1, p.bs0 + 256 + 64 * part, false);
+            gelu_to_h(0);
+            gelu_to_h(1);
             // ... chunks 2, 3 over A1's z K-blocks, once every layer-1 MMA (the readers of A1) has completed
             wait_d1(0);
             wait_d1(1);
-            gelu_to_smem(0, p.bs0 + 512 + 64 * part, false, a1 + part * KB_BYTES);
-            gelu_to_smem(1, p.bs0 + 768 + 64 * part, false, a1 + (4 + part) * KB_BYTES);
+            gelu_to_smem(0, a1 + part * KB_BYTES);
+            gelu_to_smem(1, a1 + (4 + part) * KB_BYTES);
             // ---- scorer layer 2 + output dot product: N tiles 0, 1 in the latent columns, 2, 3 in the accumulators
             float acc = 0.0f;
             auto dot32 = [&](uint32_t taddr, int n0) {
@@ -621,36 +606,29 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         }
     }
     else if (action_index(warp) >= 0) {
-        // =============================================================== action-embedding warps
-        // warp aw owns rows [16 aw, 16 aw + 16).  Phase 1 is row-mapped (lanes 0-15), phase 2 column-mapped (lane =
-        // 8 embedding columns = one 16-byte chunk of K-block 8 + lane / 8).
+        // =============================================================== action-feature warps
+        // warp aw owns rows [16 aw, 16 aw + 16), one row per lane 0-15 (lanes 16-31 help clearing).  Per step a row's
+        // action enters GEMM1 as the feature row f_t = [onehot(id) (NT) | log2 p_j (P) | 1] of K-block 8 (and 9 when
+        // NT + P + 1 > 64): the host folds E, W_p, b_p and b1 into GEMM1's a-columns (tc2_prepare), so the embedding
+        // a_t = E[id] + W_p log2 p + b_p is never formed.
         const int aw = action_index(warp);
         const int row = 16 * aw + (lane & 15);
         const bool row_lane = lane < 16;
-        const int col8 = 8 * lane;
         uint8_t* a1 = smem + L.a1;
-        float* s_lp = reinterpret_cast<float*>(smem + L.lp);
-        int* s_ids = reinterpret_cast<int*>(smem + L.ids);
         uint8_t* s_cnt = smem + L.cnt;
         const uint32_t r_aready = mapa(bar(B_AREADY), 0);
         const int P = p.P, NT = p.n_types;
-        float wp[MAX_P][8], bp8[8];
-#pragma unroll
-        for (int j = 0; j < MAX_P; ++j)
-#pragma unroll
-            for (int c = 0; c < 8; ++c) wp[j][c] = j < P ? __ldg(p.WpT + j * DA + col8 + c) : 0.0f;
-#pragma unroll
-        for (int c = 0; c < 8; ++c) bp8[c] = __ldg(p.bp + col8 + c);
         uint32_t n_w = 0;
-        auto a_dst = [&](int r) -> uint4* {
-            return reinterpret_cast<uint4*>(a1 + (8 + (lane >> 3)) * KB_BYTES + sw128_off(r, lane & 7));
+        // 16-bit feature store: column c of this row in K-blocks 8 ..
+        auto put = [&](int c, uint32_t h16) {
+            *reinterpret_cast<uint16_t*>(a1 + (8 + (c >> 6)) * KB_BYTES + sw128_off(row, (c & 63) >> 3) + (c & 7) * 2) = (uint16_t)h16;
         };
-        auto e_row = [&](int id, float (&o)[8]) {
-            const uint4 v = __ldg(reinterpret_cast<const uint4*>(p.E + (size_t)id * DA + col8));
-            o[0] = __uint_as_float(v.x << 16); o[1] = __uint_as_float(v.x & 0xffff0000u);
-            o[2] = __uint_as_float(v.y << 16); o[3] = __uint_as_float(v.y & 0xffff0000u);
-            o[4] = __uint_as_float(v.z << 16); o[5] = __uint_as_float(v.z & 0xffff0000u);
-            o[6] = __uint_as_float(v.w << 16); o[7] = __uint_as_float(v.w & 0xffff0000u);
+        // lanes l and l + 16 clear the row's K-blocks 8, 9 (one each)
+        auto clear_row = [&]() {
+            const int hk = 8 + (lane >> 4);
+#pragma unroll
+            for (int ch = 0; ch < 8; ++ch)
+                *reinterpret_cast<uint4*>(a1 + hk * KB_BYTES + sw128_off(row, ch)) = make_uint4(0u, 0u, 0u, 0u);
         };
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
@@ -667,97 +645,73 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             float slp[MAX_P];
 #pragma unroll
             for (int j = 0; j < MAX_P; ++j) slp[j] = 0.0f;
+            int prev_id = -1;
 
             for (int t = 0; t < nsteps; ++t) {
-                // phase 1 (one row per lane 0-15): read the step's action, log2 of its parameters, phi statistics
-                if (row_lane) {
-                    int id = -1;
-                    float lp[MAX_P];
+                // read the step's action, log2 of its parameters, phi statistics — before the wait: the loads' latency hides
+                int id = -1;
+                float lp[MAX_P];
 #pragma unroll
-                    for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
-                    if (t < len) {
-                        id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
-                        if (id < 0 || id >= NT) {
-                            atomicOr(p.a.fault, WM_FAULT_TYPE);
-                            id = id < 0 ? 0 : NT - 1;
-                        }
-                        const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
-#pragma unroll
-                        for (int j = 0; j < MAX_P; ++j) {
-                            if (j < P) {
-                                int prm = __ldg(pp + j);
-                                if (prm < 1) {
-                                    atomicOr(p.a.fault, WM_FAULT_PARAM);
-                                    prm = 1;
-                                }
-                                lp[j] = log2f((float)prm);
-                                slp[j] += lp[j];
-                            }
-                        }
-                        s_cnt[row * NT + id] += 1;
+                for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                if (row_lane && t < len) {
+                    id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
+                    if (id < 0 || id >= NT) {
+                        atomicOr(p.a.fault, WM_FAULT_TYPE);
+                        id = id < 0 ? 0 : NT - 1;
                     }
-                    s_ids[row] = id;
-                    *reinterpret_cast<float4*>(s_lp + row * MAX_P) = make_float4(lp[0], lp[1], lp[2], lp[3]);
-                    *reinterpret_cast<float4*>(s_lp + row * MAX_P + 4) = make_float4(lp[4], lp[5], lp[6], lp[7]);
+                    const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j) {
+                        if (j < P) {
+                            int prm = __ldg(pp + j);
+                            if (prm < 1) {
+                                atomicOr(p.a.fault, WM_FAULT_PARAM);
+                                prm = 1;
+                            }
+                            lp[j] = log2f((float)prm);
+                            slp[j] += lp[j];
+                        }
+                    }
+                    s_cnt[row * NT + id] += 1;
                 }
-                __syncwarp();
-                // store only once GEMM1 of the previous step no longer reads the a-part of A1
+                // store only once GEMM1 of the previous step (or the previous tile's scorer) no longer reads K-blocks 8 ..
                 if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
                 ++n_w;
-                // phase 2 (8 columns per lane, loop over the warp's 16 rows): a = E[id] + W_p log2(p) + b_p
-#pragma unroll 2
-                for (int rr = 0; rr < 16; ++rr) {
-                    const int r = 16 * aw + rr;
-                    const int idr = s_ids[r];
-                    float a8[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
-                    if (idr >= 0) {
-                        e_row(idr, a8);
+                if (t == 0) {          // the K-blocks still hold the previous tile's phi features
+                    clear_row();
+                    __syncwarp();
+                    if (row_lane) put(NT + P, 0x3C00u);        // the constant-1 column (carries W1a b_p + b1)
+                }
+                if (id >= 0) {         // a masked row keeps its last features: its result is discarded anyway (frozen row)
+                    if (prev_id >= 0 && prev_id != id) put(prev_id, 0u);
+                    put(id, 0x3C00u);
+                    prev_id = id;
 #pragma unroll
-                        for (int c = 0; c < 8; ++c) a8[c] += bp8[c];
-                        const float4 l0 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P);
-                        const float4 l1 = *reinterpret_cast<const float4*>(s_lp + r * MAX_P + 4);
-                        const float lr[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
-#pragma unroll
-                        for (int j = 0; j < MAX_P; ++j)
-#pragma unroll
-                            for (int c = 0; c < 8; ++c) a8[c] = fmaf(wp[j][c], lr[j], a8[c]);
-                    }
-                    *a_dst(r) = make_uint4(pack_f16(a8[0], a8[1]), pack_f16(a8[2], a8[3]), pack_f16(a8[4], a8[5]),
-                                           pack_f16(a8[6], a8[7]));
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) put(NT + j, pack_f16(lp[j], 0.0f));
                 }
                 fence_proxy_async();
-                __syncwarp();   // also: phase 2 reads of s_ids / s_lp are done before the next phase 1 overwrites
+                __syncwarp();
                 if (lane == 0) mbar_arrive_remote(r_aready);
             }
 
-            // ---- the phi K-blocks (8-11) of the scorer's A operand.  phi = mean_t a_t = (sum_c count_c E[c] +
-            // W_p sum_t log2 p_t) / len + b_p is LINEAR in psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) |
-            // 1 (len > 0)]: the host folds E, W_p and b_p into scorer layer 1's phi weights (tc2_prepare) and the kernel
-            // only writes psi, one row per lane: lanes l and l + 16 clear the row's four K-blocks (two each), then the row's
-            // lane stores one 16-bit value per feature (n_types + P + 1 <= 128: all in the K-blocks it cleared itself).
+            // ---- the phi features (K-blocks 8 ..) of the scorer's A operand: phi = mean_t a_t is LINEAR in
+            // psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) | 1 (len > 0)]; the host folds E, W_p and b_p into scorer
+            // layer 1's phi weights (tc2_prepare); a constant-1 column after psi carries scorer layer 1's bias
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
-            {
-                const int hk = 8 + 2 * (lane >> 4);
-#pragma unroll
-                for (int ch = 0; ch < 16; ++ch)
-                    *reinterpret_cast<uint4*>(a1 + (hk + (ch >> 3)) * KB_BYTES + sw128_off(row, ch & 7)) =
-                        make_uint4(0u, 0u, 0u, 0u);
-                if (row_lane) {
-                    auto put = [&](int c, float v) {
-                        *reinterpret_cast<uint16_t*>(a1 + (8 + (c >> 6)) * KB_BYTES + sw128_off(row, (c & 63) >> 3) +
-                                                     (c & 7) * 2) = (uint16_t)pack_f16(v, 0.0f);
-                    };
-                    const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
-                    for (int c = 0; c < NT; ++c) put(c, (float)s_cnt[row * NT + c] * inv);
-#pragma unroll
-                    for (int j = 0; j < MAX_P; ++j)
-                        if (j < P) put(NT + j, slp[j] * inv);
-                    put(NT + P, len > 0 ? 1.0f : 0.0f);
-                }
-            }
-            // hardware features of this row -> the hw operand tile (columns >= H stay zero)
+            clear_row();
+            __syncwarp();
             if (row_lane) {
+                auto putf = [&](int c, float v) { put(c, pack_f16(v, 0.0f)); };
+                const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
+                for (int c = 0; c < NT; ++c) putf(c, (float)s_cnt[row * NT + c] * inv);
+#pragma unroll
+                for (int j = 0; j < MAX_P; ++j)
+                    if (j < P) putf(NT + j, slp[j] * inv);
+                putf(NT + P, len > 0 ? 1.0f : 0.0f);
+                put(NT + P + 1, 0x3C00u);
+                // hardware features of this row -> the hw operand tile (columns >= H stay zero)
                 for (int ch = 0; ch < p.H / 8; ++ch) {
                     uint4 o = make_uint4(0u, 0u, 0u, 0u);
                     if (cand >= 0) {
@@ -841,50 +795,71 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         return empty;
     };
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1"), &E = get("E");
-    const int hid = m.hidden, NC = hid / 256, K1 = tc2::D + tc2::DA, K0 = K1 + m.H;
-    const size_t n_tiles = (size_t)NC * (tc2::G1_STAGES + tc2::G2_STAGES) + tc2::SC_STAGES;
+    const std::vector<float>&b1 = get("b1"), &bs0 = get("bs0"), &Wp = get("W_p"), &bpv = get("b_p");
+    const int hid = m.hidden, NC = hid / 256, K1 = tc2::D + tc2::DA, K0 = K1 + m.H, NT = m.n_types, P = m.P;
+    // ---- GEMM1's a-columns folded onto the action features f = [onehot(id) (NT) | log2 p_j (P) | 1]:
+    //      W1[:, d:] (E[id] + W_p lp + b_p) + b1  =  (W1a E^T)[:, id] + (W1a W_p) lp + (W1a b_p + b1)
+    const int NF = NT + P + 1, AKB = (NF + 63) / 64;
+    std::vector<float> W1f((size_t)hid * 64 * AKB, 0.0f);
+    for (int n = 0; n < hid; ++n) {
+        const float* wr = &W1[(size_t)n * K1 + tc2::D];
+        float* out = &W1f[(size_t)n * 64 * AKB];
+        for (int c = 0; c < NT; ++c) {
+            double acc = 0.0;
+            for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tc2::DA + k];
+            out[c] = (float)acc;
+        }
+        for (int j = 0; j < P; ++j) {
+            double acc = 0.0;
+            for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * P + j];
+            out[NT + j] = (float)acc;
+        }
+        double acc = b1[n];
+        for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * bpv[k];
+        out[NT + P] = (float)acc;
+    }
+    // ---- scorer layer 1's phi columns folded onto psi = [count_c / len | sum log2 p_j / len | 1 (len > 0)] (see the action
+    //      warps): Ws0_phi E^T, Ws0_phi W_p, Ws0_phi b_p, summed in double; then a constant-1 column that carries bs0
+    const int NPSI = NT + P + 2, PKB = (NPSI + 63) / 64;
+    std::vector<float> Wphi((size_t)tc2::SW * 64 * PKB, 0.0f);
+    for (int n = 0; n < tc2::SW; ++n) {
+        const float* wr = &Ws0[(size_t)n * K0 + tc2::D];
+        float* out = &Wphi[(size_t)n * 64 * PKB];
+        for (int c = 0; c < NT; ++c) {
+            double acc = 0.0;
+            for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tc2::DA + k];
+            out[c] = (float)acc;
+        }
+        for (int j = 0; j < P; ++j) {
+            double acc = 0.0;
+            for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * P + j];
+            out[NT + j] = (float)acc;
+        }
+        double acc = 0.0;
+        for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * bpv[k];
+        out[NT + P] = (float)acc;
+        out[NT + P + 1] = bs0[n];
+    }
+    const size_t n_tiles = (size_t)NC * (AKB + 8 + tc2::G2_STAGES) + tc2::sc_stages(PKB);
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
     blob.reserve(n_tiles * tc2::BT_BYTES);
-    // the MMA warp's order: a K-blocks (8-11) of chunks 0 and 1, z K-blocks (0-7) of chunks 0 and 1, G2(0), then G1(i)
-    // (a then z), G2(i-1)
-    auto g1_part = [&](int c, int k0, int k1) {
-        for (int k = k0; k < k1; ++k) ok &= append_pair_tile(blob, W1, K1, c * 256, k * 64, 64);
-    };
+    // the MMA warp's order: feature K-blocks of chunks 0 and 1, z K-blocks (0-7) of chunks 0 and 1, G2(0), then G1(i)
+    // (features then z), G2(i-1)
+    auto g1a = [&](int c) { for (int k = 0; k < AKB; ++k) ok &= append_pair_tile(blob, W1f, 64 * AKB, c * 256, k * 64, 64); };
+    auto g1z = [&](int c) { for (int k = 0; k < 8; ++k) ok &= append_pair_tile(blob, W1, K1, c * 256, k * 64, 64); };
     auto g2 = [&](int c) {            // GEMM2 chunk c: hidden K-blocks x the two 256-column N tiles of d
         for (int kb = 0; kb < 4; ++kb)
             for (int j = 0; j < 2; ++j) ok &= append_pair_tile(blob, W2, hid, j * 256, c * 256 + kb * 64, 64);
     };
-    g1_part(0, 8, 12); g1_part(1, 8, 12); g1_part(0, 0, 8); g1_part(1, 0, 8);
+    g1a(0); g1a(1); g1z(0); g1z(1);
     g2(0);
     for (int i = 2; i <= NC; ++i) {
-        if (i < NC) { g1_part(i, 8, 12); g1_part(i, 0, 8); }
+        if (i < NC) { g1a(i); g1z(i); }
         g2(i - 1);
     }
-    // phi weights of scorer layer 1 folded onto psi = [count_c / len | sum log2 p_j / len | 1] (see the action warps):
-    // Ws0_phi E^T, Ws0_phi W_p, Ws0_phi b_p, summed in double; [SW][256], columns past n_types + P + 1 zero
-    std::vector<float> Wphi((size_t)tc2::SW * 256, 0.0f);
-    {
-        const std::vector<float>&Wp = get("W_p"), &bpv = get("b_p");
-        for (int n = 0; n < tc2::SW; ++n) {
-            const float* wr = &Ws0[(size_t)n * K0 + tc2::D];
-            for (int c = 0; c < m.n_types; ++c) {
-                double acc = 0.0;
-                for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tc2::DA + k];
-                Wphi[(size_t)n * 256 + c] = (float)acc;
-            }
-            for (int j = 0; j < m.P; ++j) {
-                double acc = 0.0;
-                for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * m.P + j];
-                Wphi[(size_t)n * 256 + m.n_types + j] = (float)acc;
-            }
-            double acc = 0.0;
-            for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * bpv[k];
-            Wphi[(size_t)n * 256 + m.n_types + m.P] = (float)acc;
-        }
-    }
-    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi (4), hw (1, zero-padded to 64 columns), z (8)
-        for (int k = 0; k < 4; ++k) ok &= append_pair_tile(blob, Wphi, 256, c * 256, k * 64, 64);
+    for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi features (PKB), hw (1, zero-padded to 64 columns), z (8)
+        for (int k = 0; k < PKB; ++k) ok &= append_pair_tile(blob, Wphi, 64 * PKB, c * 256, k * 64, 64);
         ok &= append_pair_tile(blob, Ws0, K0, c * 256, K1, m.H);
         for (int k = 0; k < 8; ++k) ok &= append_pair_tile(blob, Ws0, K0, c * 256, k * 64, 64);
     }
@@ -902,12 +877,6 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     WM_CUDA_TRY(cudaMalloc(&d_blob, blob.size() * 2));
     ctx->allocs.push_back(d_blob);
     WM_CUDA_TRY(cudaMemcpy(d_blob, blob.data(), blob.size() * 2, cudaMemcpyHostToDevice));
-    std::vector<uint16_t> e16(E.size());
-    for (size_t i = 0; i < E.size(); ++i) e16[i] = f32_to_bf16(E[i]);
-    void* d_e = nullptr;
-    WM_CUDA_TRY(cudaMalloc(&d_e, e16.size() * 2 + 16));
-    ctx->allocs.push_back(d_e);
-    WM_CUDA_TRY(cudaMemcpy(d_e, e16.data(), e16.size() * 2, cudaMemcpyHostToDevice));
 
     // tensor map over the image seen as rows of 64 bf16 (128 B); one box = 128 rows = one 16 KB half tile.  The
     // image is already swizzled, so the map itself uses no swizzle.
@@ -933,7 +902,8 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     memcpy(m.tc2_tmap, &tm, sizeof(tm));
     m.tc_blob = d_blob;
     m.tc_blob_bytes = blob.size() * 2;
-    m.tc_E = d_e;
+    m.tcp_akb = AKB;      // (shared fields: a model has either the d = 256 pair kernel or this one)
+    m.tcp_pkb = PKB;
     WM_CUDA_TRY(cudaFuncSetAttribute(tc2::wm_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
     m.tc_ok = 2;
     return WM_OK;
@@ -946,21 +916,12 @@ int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.hid = m.hidden; p.nc = m.hidden / 256; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;
     p.ln_eps = m.ln_eps;
-    p.E = static_cast<const __nv_bfloat16*>(m.tc_E);
-    p.WpT = m.WpT; p.bp = m.bp; p.b1 = m.b1; p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
-    p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
+    p.akb = m.tcp_akb; p.pkb = m.tcp_pkb;
+    p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
+    p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
     p.a = a;
     p.n_tiles = (int)((a.B + tc2::TMP - 1) / tc2::TMP);
-    p.prof = nullptr;
-#ifdef WM_TC_PROFILE
-    static unsigned long long* d_prof = nullptr;
-    const size_t prof_bytes = (size_t)3 * tc2::TRACE_CAP * 8;
-    if (getenv("WM_TC_PROF")) {
-        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, prof_bytes));
-        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, prof_bytes, st));
-        p.prof = d_prof;
-    }
-#endif
+    p.prof = trace::begin(st);
     CUtensorMap tm;
     memcpy(&tm, m.tc2_tmap, sizeof(tm));
     const tc2::SmemLayout L = tc2::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
@@ -969,20 +930,7 @@ int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     tc2::wm_tc2_kernel<<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
-#ifdef WM_TC_PROFILE
-    if (p.prof) {   // dev instrumentation: dump pair 0's per-role (tag, clock) traces to WM_TC_PROF's path
-        std::vector<uint2> h((size_t)3 * tc2::TRACE_CAP);
-        WM_CUDA_TRY(cudaStreamSynchronize(st));
-        WM_CUDA_TRY(cudaMemcpy(h.data(), p.prof, h.size() * 8, cudaMemcpyDeviceToHost));
-        FILE* f = fopen(getenv("WM_TC_PROF"), "w");
-        if (f) {
-            for (int r = 0; r < 3; ++r)
-                for (uint32_t i = 0; i < h[(size_t)r * tc2::TRACE_CAP].x; ++i)
-                    fprintf(f, "%d %u %u\n", r, h[(size_t)r * tc2::TRACE_CAP + 1 + i].x, h[(size_t)r * tc2::TRACE_CAP + 1 + i].y);
-            fclose(f);
-        }
-    }
-#endif
+    trace::dump(p.prof, st);
     return WM_OK;
 }
 

@@ -27,6 +27,7 @@
 
 #include "wm_internal.h"
 #include "wm_ptx.cuh"
+#include "wm_trace.cuh"
 
 namespace wm {
 
@@ -75,25 +76,8 @@ struct Params {
     const float *bs0, *bs1, *w3, *bs2;
     CallArgs a;
     int n_tiles;
-    unsigned long long* prof;   // dev instrumentation trace buffer (WM_TC_PROFILE builds), else nullptr
+    unsigned long long* prof;   // developer trace buffer (wm_trace.cuh), null in a normal build
 };
-
-// Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of the leader CTA of pair 0
-// appends (tag, clock) records to a trace buffer that launch_tcg dumps.  Compiled out otherwise.
-#ifdef WM_TC_PROFILE
-constexpr int TRACE_CAP = 16384;
-#define WM_TRACE_DECL(role)                                                                            \
-    uint2* tr_buf = p.prof ? reinterpret_cast<uint2*>(p.prof) + (role) * TRACE_CAP : nullptr;           \
-    const bool tr_on = tr_buf != nullptr && blockIdx.x == 0 && lane == 0;                              \
-    uint32_t tr_n = 0;
-#define WM_TRACE(tag)                                                                                  \
-    do {                                                                                               \
-        if (tr_on && tr_n < TRACE_CAP - 1) { tr_buf[1 + tr_n] = make_uint2((uint32_t)(tag), (uint32_t)clock64()); ++tr_n; tr_buf[0].x = tr_n; } \
-    } while (0)
-#else
-#define WM_TRACE_DECL(role)
-#define WM_TRACE(tag) do { } while (0)
-#endif
 
 struct SmemLayout {
     uint32_t zbuf, abuf, rz, ring, hwk, idx, lens, red, bars, sched, tmem_slot, total;
@@ -211,7 +195,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint32_t n_z = 0, n_a = 0;
         uint32_t pend = 0, xpar = 0;     // per accumulator: a commit is outstanding / parity of its XFREE barrier
         const uint32_t s_hwk = s_base + L.hwk;
-        WM_TRACE_DECL(0)
+        WM_TRACE_DECL(p.prof, 0)
         auto wait_x = [&](int b) {       // accumulator b read by the epilogue (and that epilogue's output written)
             if ((pend >> b) & 1u) {
                 WM_TRACE(10 + b);
@@ -833,16 +817,7 @@ int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.bs0 = m.bs[0]; p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
     p.a = a;
     p.n_tiles = (int)((a.B + tcg::TMP - 1) / tcg::TMP);
-    p.prof = nullptr;
-#ifdef WM_TC_PROFILE
-    static unsigned long long* d_prof = nullptr;
-    const size_t prof_bytes = (size_t)tcg::TRACE_CAP * 8;
-    if (getenv("WM_TC_PROF")) {
-        if (!d_prof) WM_CUDA_TRY(cudaMalloc(&d_prof, prof_bytes));
-        WM_CUDA_TRY(cudaMemsetAsync(d_prof, 0, prof_bytes, st));
-        p.prof = d_prof;
-    }
-#endif
+    p.prof = trace::begin(st);
     CUtensorMap tm;
     memcpy(&tm, m.tc2_tmap, sizeof(tm));
     const tcg::SmemLayout L = tcg::smem_layout(p.hw_ksteps);
@@ -851,18 +826,7 @@ int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     tcg::wm_tcg_kernel<<<2 * pairs, tcg::THREADS, L.total, st>>>(p, tm);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
-#ifdef WM_TC_PROFILE
-    if (p.prof) {   // dev instrumentation: dump the leader MMA warp's (tag, clock) trace to WM_TC_PROF's path
-        std::vector<uint2> h((size_t)tcg::TRACE_CAP);
-        WM_CUDA_TRY(cudaStreamSynchronize(st));
-        WM_CUDA_TRY(cudaMemcpy(h.data(), p.prof, h.size() * 8, cudaMemcpyDeviceToHost));
-        FILE* f = fopen(getenv("WM_TC_PROF"), "w");
-        if (f) {
-            for (uint32_t i = 0; i < h[0].x; ++i) fprintf(f, "0 %u %u\n", h[1 + i].x, h[1 + i].y);
-            fclose(f);
-        }
-    }
-#endif
+    trace::dump(p.prof, st);
     return WM_OK;
 }
 

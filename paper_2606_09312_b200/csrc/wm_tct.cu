@@ -22,6 +22,7 @@
 
 #include "wm_internal.h"
 #include "wm_ptx.cuh"
+#include "wm_trace.cuh"
 
 namespace wm {
 
@@ -72,7 +73,7 @@ struct Params {
     CallArgs a;
     int n_tiles;
     int* tile_counter;
-    unsigned long long* prof;   // dev instrumentation trace buffer (WM_TC_PROFILE builds), else nullptr
+    unsigned long long* prof;   // developer trace buffer (wm_trace.cuh), null in a normal build
 };
 
 struct SmemLayout {
@@ -103,22 +104,6 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hid, int hw_k
 }
 
 using namespace ptx;
-
-// Dev instrumentation (-DWM_TC_PROFILE + WM_TC_PROF=<file>): lane 0 of one warp per role of CTA 0 appends
-// (tag, clock) records to a trace buffer that launch_tc dumps.  Compiled out otherwise.
-#ifdef WM_TC_PROFILE
-#define WM_TRACE_DECL(role, cond)                                                                       \
-    uint2* tr_buf = p.prof ? reinterpret_cast<uint2*>(p.prof) + (role) * 8192 : nullptr;                 \
-    const bool tr_on = tr_buf != nullptr && blockIdx.x == 0 && lane == 0 && (cond);                     \
-    uint32_t tr_n = 0;
-#define WM_TRACE(tag)                                                                                   \
-    do {                                                                                                \
-        if (tr_on && tr_n < 8191) { tr_buf[1 + tr_n] = make_uint2((uint32_t)(tag), (uint32_t)clock64()); ++tr_n; tr_buf[0].x = tr_n; } \
-    } while (0)
-#else
-#define WM_TRACE_DECL(role, cond)
-#define WM_TRACE(tag) do { } while (0)
-#endif
 
 }  // namespace tct
 
@@ -233,7 +218,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
             uint32_t n_z = 0, n_a = 0, n_h[2] = {0, 0};
             bool pend[2] = {false, false};
             const uint32_t s_hwk = s_base + L.hwk;
-            WM_TRACE_DECL(0, true)
+            WM_TRACE_DECL(p.prof, 0)
             auto wait_h = [&](int b) {
                 if (pend[b]) {
                     WM_TRACE(10 + b);
@@ -956,13 +941,14 @@ int launch_tct(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.n_tiles = (int)((a.B + tct::TM - 1) / tct::TM);
     p.tile_counter = ws->counters + kTileCtrOff;
     WM_CUDA_TRY(cudaMemsetAsync(p.tile_counter, 0, sizeof(int), st));
-    p.prof = nullptr;
+    p.prof = trace::begin(st);
     const tct::SmemLayout L = tct::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
     const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
     if (a.latents_out) tct::wm_tct_kernel<true><<<grid, tct::THREADS, L.total, st>>>(p);    // terminal latents only
     else tct::wm_tct_kernel<false><<<grid, tct::THREADS, L.total, st>>>(p);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
+    trace::dump(p.prof, st);
     return WM_OK;
 }
 
