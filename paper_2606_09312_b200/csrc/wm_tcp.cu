@@ -54,10 +54,13 @@ constexpr int KB_BYTES = 16384;    // one A K-block: [128 rows x 64 cols] fp16, 
 constexpr int HB_BYTES = 8192;     // one TMA box ("half block"): 64 image rows of 128 B = this CTA's half of one N = 128
                                    // K-block (64 weight rows x 64 cols; 4 MMAs, 256 tensor cycles) or a quarter of one
                                    // N = 256 K-block (two consecutive boxes = this CTA's 128 weight rows)
-constexpr int STAGE_HB = 4;        // ring stage capacity in boxes (a stage carries 1..4 of them)
-constexpr int STAGE_BYTES = STAGE_HB * HB_BYTES;
 constexpr int NSTAGE = 3;
-constexpr int A1_KB = 6;           // z: 0-3, action features f_t / phi features: 4-5
+// Two shared-memory shapes.  "wide" (akb = pkb = 1: the action and phi features fit one K-block each, e.g. cfg 2 / 4): A1 is
+// five K-blocks and a ring stage holds up to FIVE boxes (40 KB), so a later chunk's feature K-block and its four z K-blocks
+// are ONE stage (one wait, one commit, one elected region: the issuer's fixed cost per stage is ~350 cycles).  Otherwise A1
+// is six K-blocks, a stage holds four boxes and features and z are two stages.
+__host__ __device__ inline int a1_kb(bool wide) { return wide ? 5 : 6; }      // z: 0-3, features f_t / phi: 4(-5)
+__host__ __device__ inline int stage_hb(bool wide) { return wide ? 5 : 4; }
 constexpr int HWK_BYTES = 4096;    // hw operand: one [128 x 16] no-swizzle K-major tile per K = 16 step
 constexpr int THREADS = 512;
 constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
@@ -93,11 +96,12 @@ struct SmemLayout {
     uint32_t a1, hwk, ring, mx, cnt, b2, gamma, beta, red, bars, sched, tmem_slot, total;
 };
 
-__host__ __device__ inline SmemLayout smem_layout(int n_types, int hw_ksteps, int phi_struct) {
+__host__ __device__ inline SmemLayout smem_layout(int n_types, int hw_ksteps, int phi_struct, bool wide) {
     SmemLayout L;
     uint32_t o = 0;
-    L.a1 = o; o += A1_KB * KB_BYTES;
-    L.ring = o; o += NSTAGE * STAGE_BYTES;
+    L.a1 = o; o += a1_kb(wide) * KB_BYTES;
+    o = (o + 1023) & ~1023u;
+    L.ring = o; o += NSTAGE * stage_hb(wide) * HB_BYTES;
     L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
     L.mx = o; o += phi_struct ? TM * MAX_P * 4 : 0;
     L.cnt = o; o += TM * (uint32_t)n_types;           // u8 counts, row-major [128][n_types]
@@ -123,9 +127,11 @@ __device__ __forceinline__ int tile_of(int it, int pair, int np, int n_tiles) {
 // Ring-stage program of one rollout step, per CTA, in boxes: stage 0 = feature K-blocks of chunks 0 and 1 (2 akb boxes),
 // stages 1, 2 = z K-blocks of chunk 0 / chunk 1 (4 boxes each), stage 3 = GEMM2 chunk 0 (4), then per further chunk i:
 // feature K-blocks (akb), z K-blocks (4), GEMM2 chunk i-1 (4); last stage = GEMM2 chunk NC-1.  3 NC - 1 stages.
-__host__ __device__ inline int step_stages(int nc) { return 3 * nc - 1; }
-__host__ __device__ inline int stage_boxes(int j, int nc, int akb) {
+// (wide: 2 NC + 1 stages — features and z of chunk i are one stage of 5 boxes)
+__host__ __device__ inline int step_stages(int nc, bool wide) { return wide ? 2 * nc + 1 : 3 * nc - 1; }
+__host__ __device__ inline int stage_boxes(int j, int nc, int akb, bool wide) {
     if (j == 0) return 2 * akb;
+    if (wide) return (j >= 4 && j < 2 * nc && (j - 4) % 2 == 0) ? 5 : 4;
     return (j >= 4 && j < 3 * nc - 2 && (j - 4) % 3 == 0) ? akb : 4;
 }
 __host__ __device__ inline int step_boxes(int nc, int akb) { return 2 * akb + 12 + (nc - 2) * (akb + 8) + 4; }
@@ -151,7 +157,9 @@ template <int PHI, bool EXT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(1024) uint8_t smem[];
-    const SmemLayout L = smem_layout(p.n_types, p.hw_ksteps, PHI);
+    const bool WIDE = p.akb == 1 && p.pkb == 1;
+    const SmemLayout L = smem_layout(p.n_types, p.hw_ksteps, PHI, WIDE);
+    const uint32_t STAGE_BYTES = (uint32_t)stage_hb(WIDE) * HB_BYTES;
     const uint32_t s_base = smem_u32(smem);
     const uint32_t s_a1 = s_base + L.a1, s_ring = s_base + L.ring, s_bars = s_base + L.bars;
     auto bar = [&](int i) -> uint32_t { return s_bars + 8u * (uint32_t)i; };
@@ -166,7 +174,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int NC = p.nc;
     const int AKB = p.akb, PKB = p.pkb;
-    const int ROLL_BOXES = step_boxes(NC, AKB), ROLL_STAGES = step_stages(NC);
+    const int ROLL_BOXES = step_boxes(NC, AKB), ROLL_STAGES = step_stages(NC, WIDE);
 
     // ---- one-time setup
     if (threadIdx.x == 0) {
@@ -253,7 +261,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int t = 0; t < nsteps; ++t) {
                     int box = 0;
                     for (int j = 0; j < ROLL_STAGES; ++j) {
-                        const int nb = stage_boxes(j, NC, AKB);
+                        const int nb = stage_boxes(j, NC, AKB, WIDE);
                         issue(nb, box);
                         box += nb;
                     }
@@ -291,14 +299,11 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         };
         const uint32_t ring_lo0 = smem_desc_lo(s_ring);
         uint32_t b_lo = ring_lo0;
-        bool ready = false;
-        auto acquire_stage = [&]() {       // returns with the current stage's data landed; probes the next stage
+        auto acquire_stage = [&]() {       // returns with the current stage's data landed
             WM_TRACE(20);
-            if (!ready) mbar_wait_warp(bar(B_FULL + stage), ph);
+            mbar_wait_warp(bar(B_FULL + stage), ph);
             WM_TRACE(21);
             tc_fence_after();
-            const uint32_t nst = stage + 1 == NSTAGE ? 0u : stage + 1;
-            ready = __all_sync(0xffffffffu, mbar_test_wait(bar(B_FULL + nst), nst == 0 ? ph ^ 1u : ph));
         };
         auto advance = [&]() {
             __syncwarp();
@@ -337,6 +342,19 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     for (int j = 0; j < p.hw_ksteps; ++j)
                         mma_ss2(TD1 + 128u * b, smem_desc_nosw(s_hwk + j * HWK_BYTES), desc_of(b_lo + (uint32_t)nk * HBL + 2u * j),
                                 ID_N128, 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
+        // wide shape, one stage: the feature K-block then z K-blocks 0-3 into buffer b; the a-buffer is released (B_AFREE)
+        // from inside the stage when this is the step's last read of it
+        auto stage_az = [&](int b, bool last) {
+            acquire_stage();
+            if (elect_one()) {
+                kb_ss(TD1 + 128u * b, a_lo + 4 * KBL, b_lo, true);
+                if (last) mma_commit2(bar(B_AFREE));
+#pragma unroll
+                for (int k = 0; k < 4; ++k) kb_ss(TD1 + 128u * b, a_lo + k * KBL, b_lo + (uint32_t)(k + 1) * HBL, false);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
@@ -442,9 +460,13 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     if (i < NC) {                       // GEMM1 chunk i into buffer i & 1 (its GEMM2 reader has been issued)
                         const int b = i & 1;
                         wait_h(b);
-                        stage_a(b, AKB, false);
-                        if (i == NC - 1) commit(B_AFREE);
-                        stage_z(b);
+                        if (WIDE) {
+                            stage_az(b, i == NC - 1);
+                        } else {
+                            stage_a(b, AKB, false);
+                            if (i == NC - 1) commit(B_AFREE);
+                            stage_z(b);
+                        }
                         commit(B_D1FULL + b);
                         pend[b] = true;
                     }
@@ -830,7 +852,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 WM_TRACE(72);
                 ++n_w;
                 if (t == 0) {          // the K-blocks still hold the previous tile's phi features
-                    clear_row(2);
+                    clear_row(WIDE ? 1 : 2);
                     put(NT + P, 0x3C00u);                      // the constant-1 column (carries W1a b_p + b1)
                 }
                 if (id >= 0) {         // a masked row keeps its last features: its result is discarded anyway (frozen row)
@@ -857,7 +879,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             ++n_w;
             {
                 auto putf = [&](int c, float v) { put(c, pack_f16(v, 0.0f)); };
-                clear_row(2);
+                clear_row(WIDE ? 1 : 2);
                 const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
                 if (PHI == WM_PHI_STRUCT) {
                     for (int c = 0; c < NT; ++c) putf(c, (float)s_cnt[row * NT + c]);
@@ -951,8 +973,6 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     Model& m = ctx->m;
     m.tcp_ok = 0;
     if (!tcp_model_ok(m)) return WM_OK;
-    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT);
-    if ((int)L.total > ctx->smem_optin) return WM_OK;
     auto get = [&](const char* n) -> const std::vector<float>& {
         for (size_t i = 0; i < names.size(); ++i)
             if (names[i] == n) return hv[i];
@@ -1017,6 +1037,8 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
             out[NPSI - 1] = (float)bias;
         }
     }
+    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT, AKB == 1 && PKB == 1);
+    if ((int)L.total > ctx->smem_optin) return WM_OK;
     const size_t n_slots = (size_t)tcp::step_boxes(NC, AKB) + tcp::scorer_boxes(PKB);
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
@@ -1122,7 +1144,7 @@ int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.prof = trace::begin(st);
     CUtensorMap tm;
     memcpy(&tm, m.tcp_tmap, sizeof(tm));
-    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT);
+    const tcp::SmemLayout L = tcp::smem_layout(m.n_types, p.hw_ksteps, m.phi_kind == WM_PHI_STRUCT, p.akb == 1 && p.pkb == 1);
     const int max_pairs = ctx->n_sms / 2;
     const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
     const bool prefix_call = a.start || a.init_index || a.latents_out;
