@@ -395,7 +395,7 @@ int wm_get_info(const wm_ctx* ctx, wm_info* o) {
     for (int i = 0; i < 6; ++i) o->scorer_widths[i] = (i + 1 < m.n_lin) ? m.sdim[i + 1] : 0;
     o->ln_eps = m.ln_eps;
     o->path = tc_supported(ctx) ? 2 : 1;
-    o->tc_variant = tc_supported(ctx) == 1 && m.tcp_ok && ctx->opt_pair ? 5 : tc_supported(ctx);
+    o->tc_variant = tc_supported(ctx) == 1 && m.tcp_ok && (ctx->opt_pair || !m.tc1_ok) ? 5 : tc_supported(ctx);
     o->phi_kind = m.phi_kind;
     o->ranker_kind = m.ranker_kind; o->n_trees = m.n_trees; o->tree_depth = m.tree_depth;
     return WM_OK;
@@ -442,6 +442,10 @@ int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value) {
         if (value < 0 || value > 1) {
             set_error("wm_set_option: WM_OPT_PAIR takes 0 or 1");
             return WM_ERR_ARG;
+        }
+        if (value == 0 && ctx->m.tcp_ok && !ctx->m.tc1_ok) {
+            set_error("wm_set_option: this model has no single-CTA tcgen05 form (its embedding table does not fit shared memory)");
+            return WM_ERR_UNSUPPORTED;
         }
         ctx->opt_pair = value;
         return WM_OK;

@@ -60,6 +60,7 @@ struct Model {
     void* tc_E = nullptr;      // bf16 [n_types][d_a]
     int tc_ok = 0;             // 0 = no tcgen05 path, 1 = wm_tc_kernel (one CTA per tile), 2 = wm_tc2_kernel (CTA pair), 3 = wm_tcg_kernel (CTA pair, GRU), 4 = wm_tct_kernel (TransH)
     alignas(64) unsigned char tc2_tmap[128] = {};   // CUtensorMap over tc_blob (pair kernel)
+    int tc1_ok = 0;            // the single-CTA form wm_tc_kernel is built (tc_ok == 1 means: at least one of the two forms is)
     int tcp_akb = 1, tcp_pkb = 1;   // wm_tcp_kernel: K-blocks of the folded action features / phi features
     int tcp_ok = 0;            // 1 = wm_tcp_kernel (the CTA-pair, M = 256 form of wm_tc_kernel) is built for this model too
     alignas(64) unsigned char tcp_tmap[128] = {};   // CUtensorMap over wm_tcp_kernel's own weight image

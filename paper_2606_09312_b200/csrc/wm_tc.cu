@@ -868,8 +868,14 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         const int rc2 = tcg_prepare(ctx, hv, names);
         return rc2 != WM_OK || m.tc_ok ? rc2 : tct_prepare(ctx, hv, names);   // TransH models (NEXT row f1)
     }
+    // the pair form (wm_tcp_kernel) of the same model, taken by default when built; then the single-CTA form
+    {
+        const int rc = tcp_prepare(ctx, hv, names);
+        if (rc != WM_OK) return rc;
+        if (m.tcp_ok) m.tc_ok = 1;
+    }
     const tc::SmemLayout L = tc::smem_layout(m.n_types, m.hidden, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT);
-    if ((int)L.total > ctx->smem_optin) return WM_OK;
+    if ((int)L.total > ctx->smem_optin) return WM_OK;      // (e.g. many action types: the embedding table does not fit)
     auto get = [&](const char* n) -> const std::vector<float>& {
         for (size_t i = 0; i < names.size(); ++i)
             if (names[i] == n) return hv[i];
@@ -963,7 +969,8 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
     }
     m.tc_ok = 1;
-    return tcp_prepare(ctx, hv, names);   // the pair form (wm_tcp_kernel) of the same model, taken by default when built
+    m.tc1_ok = 1;
+    return WM_OK;
 }
 
 int tc_supported(const wm_ctx* ctx) { return ctx->m.tc_ok; }
@@ -990,7 +997,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     if (m.tc_ok == 2) return launch_tc2(ctx, ws, a, st);
     if (m.tc_ok == 3) return launch_tcg(ctx, ws, a, st);
     if (m.tc_ok == 4) return launch_tct(ctx, ws, a, st);
-    if (m.tcp_ok && ctx->opt_pair) return launch_tcp(ctx, ws, a, st);
+    if (m.tcp_ok && (ctx->opt_pair || !m.tc1_ok)) return launch_tcp(ctx, ws, a, st);
     tc::Params p;
     p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;

@@ -81,6 +81,33 @@ def test_config_parity_small(wm, n):
         np.testing.assert_array_equal(idx, oracle.topk_segments(y, b.subgraph_offsets, cfg.k))
 
 
+@pytest.mark.parametrize("phi", [0, 1])
+def test_many_action_types_two_feature_kblocks(wm, phi):
+    """A d = 256 model whose folded action features [onehot | log2 p | 1] and phi features need TWO K-blocks each
+    (n_types + P + 1 > 64): the non-"wide" shape of wm_tcp_kernel (six A K-blocks, four-box stages), which no BASELINE.json
+    config reaches.  Both phi kinds, every path, several tiles and a ragged tail."""
+    base = gen.get_config(2 if phi == 0 else 9)
+    cfg = replace(base.scaled(S=3, per_subgraph=250), n_types=60, P=8, name=base.name + "_nt60")
+    w = gen.make_weights(cfg)
+    b = gen.make_inputs(cfg)
+    ref = oracle_scores(cfg, w, b)
+    seen = set()
+    for path in (wm.PATH_FP32, wm.PATH_TCGEN05):
+        ctx = wm.wm_load_weights(weight_file(cfg, w))
+        wm.wm_set_option(ctx, wm.WM_OPT_PATH, path)
+        if path == wm.PATH_TCGEN05:       # (the single-CTA form keeps a 60 x 128 embedding table in shared memory: no room)
+            with pytest.raises(wm.WmError) as e:
+                wm.wm_set_option(ctx, wm.WM_OPT_PAIR, 0)
+            assert e.value.code == wm.WM_ERR_UNSUPPORTED
+        seen.add(wm.wm_get_info(ctx).tc_variant if path != wm.PATH_FP32 else 0)
+        y = gpu_scores(ctx, b)
+        np.testing.assert_array_equal(gpu_scores(ctx, b).view(np.uint32), y.view(np.uint32))
+        wm.wm_free(ctx)
+        tol = 2e-3 if path == wm.PATH_FP32 else 2e-2
+        assert oracle.score_error(y, ref, b.subgraph_offsets) <= tol, (phi, path)
+    assert seen == {0, 5}, seen
+
+
 def _edge_batch(cfg, lengths=None, S=None, per=None):
     if cfg.prefix_children:      # cfg 4: its MODEL (hidden 768: six GEMM1 chunks) on free-form batches with mixed lengths
         cfg = replace(cfg, prefix_children=0, len_dist="uniform", len_lo=0)
