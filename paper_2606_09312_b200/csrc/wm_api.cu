@@ -461,7 +461,8 @@ int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value) {
 static int run_rollout_locked(wm_ctx* ctx, Workspace* ws, CallArgs a, cudaStream_t st) {
     a.perm = nullptr;
     a.fault = ctx->fault;
-    if (ctx->opt_sort) {
+    // (a batch that fits one tile of any kernel gains nothing from the sort and pays three launches for it)
+    if (ctx->opt_sort && a.B > 256) {
         int rc = ensure_perm(ws, a.B, st);
         if (rc != WM_OK) return rc;
         rc = launch_length_bucketing(ctx, ws, a.lengths, a.start, a.B, a.T_max, st);

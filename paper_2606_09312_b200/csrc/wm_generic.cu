@@ -11,6 +11,7 @@
 #include <math_constants.h>
 
 #include "wm_internal.h"
+#include "wm_ptx.cuh"
 
 namespace wm {
 
@@ -29,9 +30,17 @@ struct GenericParams {
     const float* bs[kMaxScorerLinears];
     CallArgs a;
     int n_tiles;
+    // weights-in-shared-memory mode (wm_generic_kernel<R, true>): byte offset of the weight region in dynamic shared memory
+    // and the float offsets of W1t, W2t and the scorer matrices inside it
+    uint32_t ws_off, ws_bytes;
+    uint32_t ws_w1, ws_w2, ws_s[kMaxScorerLinears];
+    // ... and of the small tensors: E, WpT, bp, b1, b2, gamma, beta, scorer biases
+    uint32_t ws_E, ws_Wp, ws_bp, ws_b1, ws_b2, ws_g, ws_be, ws_bs[kMaxScorerLinears];
+    int split_ok;   // every linear's width <= 256: the split-K form applies (R <= 8)
 };
 
 enum { ACT_NONE = 0, ACT_GELU = 1, ACT_SIGMOID = 2, ACT_TANH = 3 };
+constexpr int kSplitThreads = 256;   // = kGenericThreads (defined below); threads that share one split-K linear
 
 __device__ __forceinline__ float gelu_erf(float x) { return 0.5f * x * (1.0f + erff(x * 0.70710678118654752440f)); }
 __device__ __forceinline__ float sigmoidf_(float x) { return 1.0f / (1.0f + expf(-x)); }
@@ -44,13 +53,14 @@ __device__ __forceinline__ float apply_act(float x) {
     return x;
 }
 
-// outT[n][r] = act(bias[n] + sum_k Wt[k][n] * inT[k][r]),  n < N, r < R.  inT/outT in shared memory.
-template <int R, int ACT>
+// outT[n][r] = act(bias[n] + sum_k Wt[k][n] * inT[k][r]),  n < N, r < R.  inT/outT in shared memory.  WS: Wt is in shared
+// memory too (staged once per CTA), read with plain loads: consecutive threads -> consecutive banks.
+template <int R, int ACT, bool WS = false>
 __device__ void linear_T(const float* __restrict__ Wt, const float* __restrict__ bias, const float* inT, int K,
                          int N, float* outT) {
     for (int n = threadIdx.x; n < N; n += blockDim.x) {
         float acc[R];
-        const float b = bias ? __ldg(bias + n) : 0.0f;
+        const float b = bias ? (WS ? bias[n] : __ldg(bias + n)) : 0.0f;
 #pragma unroll
         for (int r = 0; r < R; ++r) acc[r] = b;
         const float* wp = Wt + n;
@@ -58,7 +68,7 @@ __device__ void linear_T(const float* __restrict__ Wt, const float* __restrict__
         for (; k + 4 <= K; k += 4) {
             float w[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) w[u] = __ldg(wp + (size_t)(k + u) * N);
+            for (int u = 0; u < 4; ++u) w[u] = WS ? wp[(size_t)(k + u) * N] : __ldg(wp + (size_t)(k + u) * N);
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const float4* xv = reinterpret_cast<const float4*>(inT + (size_t)(k + u) * R);
@@ -73,7 +83,7 @@ __device__ void linear_T(const float* __restrict__ Wt, const float* __restrict__
             }
         }
         for (; k < K; ++k) {
-            const float w = __ldg(wp + (size_t)k * N);
+            const float w = WS ? wp[(size_t)k * N] : __ldg(wp + (size_t)k * N);
             const float4* xv = reinterpret_cast<const float4*>(inT + (size_t)k * R);
 #pragma unroll
             for (int q = 0; q < R / 4; ++q) {
@@ -97,6 +107,69 @@ __device__ void linear_T(const float* __restrict__ Wt, const float* __restrict__
     }
 }
 
+// Split-K form for the weights-in-shared-memory mode and small tiles (R <= 8): with N <= 128 output units only N of the
+// CTA's 256 threads would work, each on a serial chain of K dependent FMAs — the whole cost of a cfg-1-sized call.  Here
+// S = 256 / N thread groups take K / S of the reduction each, partial sums meet in `scratch` ([S][N][R] floats) and the
+// first N threads add bias and activation.  Called by all threads (two block barriers inside).
+// explicit shared-space load (the matrix pointer reaches linear_T_split as a generic pointer: without this ptxas emits LD.E)
+__device__ __forceinline__ float lds_f32(const float* p) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"((uint32_t)__cvta_generic_to_shared(p)));
+    return v;
+}
+
+template <int R, int ACT>
+__device__ void linear_T_split(const float* Wt, const float* bias, const float* inT, int K, int N, float* outT,
+                               float* scratch) {
+    const int S = N <= kSplitThreads ? kSplitThreads / N : 1;
+    const int tid = threadIdx.x;
+    const int n = tid % N, part = tid / N;
+    if (part < S) {
+        const int kc = (K + S - 1) / S, k0 = part * kc, k1 = min(K, k0 + kc);
+        float acc[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+        const float* wp = Wt + n;
+#pragma unroll 4
+        for (int k = k0; k < k1; ++k) {
+            const float w = lds_f32(wp + (size_t)k * N);
+            const float4* xv = reinterpret_cast<const float4*>(inT + (size_t)k * R);
+#pragma unroll
+            for (int q = 0; q < R / 4; ++q) {
+                const float4 x = xv[q];
+                acc[4 * q + 0] = fmaf(w, x.x, acc[4 * q + 0]);
+                acc[4 * q + 1] = fmaf(w, x.y, acc[4 * q + 1]);
+                acc[4 * q + 2] = fmaf(w, x.z, acc[4 * q + 2]);
+                acc[4 * q + 3] = fmaf(w, x.w, acc[4 * q + 3]);
+            }
+        }
+        float4* sv = reinterpret_cast<float4*>(scratch + ((size_t)part * N + n) * R);
+#pragma unroll
+        for (int q = 0; q < R / 4; ++q) sv[q] = make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
+    }
+    __syncthreads();
+    if (tid < N) {
+        float acc[R];
+        const float b = bias ? bias[tid] : 0.0f;
+#pragma unroll
+        for (int r = 0; r < R; ++r) acc[r] = b;
+        for (int s = 0; s < S; ++s) {
+            const float4* sv = reinterpret_cast<const float4*>(scratch + ((size_t)s * N + tid) * R);
+#pragma unroll
+            for (int q = 0; q < R / 4; ++q) {
+                const float4 x = sv[q];
+                acc[4 * q + 0] += x.x; acc[4 * q + 1] += x.y; acc[4 * q + 2] += x.z; acc[4 * q + 3] += x.w;
+            }
+        }
+        float4* ov = reinterpret_cast<float4*>(outT + (size_t)tid * R);
+#pragma unroll
+        for (int q = 0; q < R / 4; ++q)
+            ov[q] = make_float4(apply_act<ACT>(acc[4 * q + 0]), apply_act<ACT>(acc[4 * q + 1]), apply_act<ACT>(acc[4 * q + 2]),
+                                apply_act<ACT>(acc[4 * q + 3]));
+    }
+    __syncthreads();
+}
+
 __device__ __forceinline__ int find_segment(const int32_t* __restrict__ off, int S, int cand) {
     // largest s with off[s] <= cand (empty segments have off[s] == off[s+1]; pick the one that contains cand)
     int lo = 0, hi = S;  // invariant: off[lo] <= cand < off[hi]
@@ -108,8 +181,13 @@ __device__ __forceinline__ int find_segment(const int32_t* __restrict__ off, int
 }
 
 constexpr int kGenericThreads = 256;
+static_assert(kSplitThreads == kGenericThreads, "linear_T_split spreads K over the whole CTA");
 
-template <int R>
+// WS = true (small residual-MLP models whose W1, W2 and scorer matrices fit shared memory beside the tile, e.g. BASELINE.json
+// cfg 1: 135 KB): every CTA stages the matrices ONCE with bulk async copies (TMA engine, mbarrier complete_tx) and then
+// walks its tiles — north_star's "transition weights are staged once per CTA through TMA into shared memory", which is
+// literally possible only for models of this size.  WS = false re-reads them through the read-only path.
+template <int R, bool WS>
 __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const GenericParams p) {
     extern __shared__ __align__(16) float smem[];
     const int d = p.d, da = p.da, H = p.H, P = p.P;
@@ -138,6 +216,50 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
     const int g_of = tid / R;
     constexpr int G = kGenericThreads / R;
     const CallArgs& a = p.a;
+    const float* W1t = p.W1t;
+    const float* W2t = p.W2t;
+    const float* Wst[kMaxScorerLinears];
+    const float* bsv[kMaxScorerLinears];
+#pragma unroll
+    for (int l = 0; l < kMaxScorerLinears; ++l) { Wst[l] = p.Wst[l]; bsv[l] = p.bs[l]; }
+    const float *pE = p.E, *pWp = p.WpT, *pbp = p.bp, *pb1 = p.b1, *pb2 = p.b2, *pg = p.gamma, *pbe = p.beta;
+    if (WS) {
+        float* wreg = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(smem) + p.ws_off);
+        uint64_t* wbar = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(smem) + p.ws_off + p.ws_bytes);
+        const uint32_t bar = ptx::smem_u32(wbar);
+        if (tid == 0) {
+            ptx::mbar_init(bar, 1);
+            ptx::fence_barrier_init();
+            ptx::mbar_arrive_expect_tx(bar, p.ws_bytes);
+            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_w1), p.W1t, (uint32_t)((size_t)(p.d + p.da) * p.hidden * 4), bar);
+            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_w2), p.W2t, (uint32_t)((size_t)p.hidden * p.d * 4), bar);
+            for (int l = 0; l < p.n_lin; ++l) {
+                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_s[l]), p.Wst[l], (uint32_t)((size_t)p.sdim[l] * p.sdim[l + 1] * 4), bar);
+                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_bs[l]), p.bs[l], (uint32_t)(((size_t)p.sdim[l + 1] * 4 + 15) & ~15u), bar);
+            }
+            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_E), p.E, (uint32_t)((size_t)p.n_types * p.da * 4), bar);
+            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_Wp), p.WpT, (uint32_t)((size_t)p.P * p.da * 4), bar);
+            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_bp), p.bp, (uint32_t)((size_t)p.da * 4), bar);
+            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_b1), p.b1, (uint32_t)((size_t)p.hidden * 4), bar);
+            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_b2), p.b2, (uint32_t)((size_t)p.d * 4), bar);
+            if (p.kind == WM_KIND_MLP_LN) {
+                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_g), p.gamma, (uint32_t)((size_t)p.d * 4), bar);
+                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_be), p.beta, (uint32_t)((size_t)p.d * 4), bar);
+            }
+        }
+        __syncthreads();
+        ptx::mbar_wait(bar, 0);
+        W1t = wreg + p.ws_w1;
+        W2t = wreg + p.ws_w2;
+#pragma unroll
+        for (int l = 0; l < kMaxScorerLinears; ++l) { Wst[l] = wreg + p.ws_s[l]; bsv[l] = wreg + p.ws_bs[l]; }
+        pE = wreg + p.ws_E; pWp = wreg + p.ws_Wp; pbp = wreg + p.ws_bp; pb1 = wreg + p.ws_b1; pb2 = wreg + p.ws_b2;
+        pg = wreg + p.ws_g; pbe = wreg + p.ws_be;
+    }
+    auto ldw = [&](const float* q) -> float { return WS ? *q : __ldg(q); };
+    // split-K scratch: [256][R] floats behind the weight region's barrier (WS mode, R <= 8, every width <= 256)
+    constexpr bool SPLIT = WS && R <= 8;
+    float* scratch = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(smem) + p.ws_off + p.ws_bytes + 16);
 
     for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
         __syncthreads();
@@ -240,8 +362,8 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                 if (live_of(r)) {
                     const int id = m_id[r];
                     if (p.embed == WM_EMBED_LINEAR) {
-                        v = __ldg(p.E + (size_t)id * da + j) + __ldg(p.bp + j);
-                        for (int q = 0; q < P; ++q) v = fmaf(__ldg(p.WpT + (size_t)q * da + j), LP[r * P + q], v);
+                        v = ldw(pE + (size_t)id * da + j) + ldw(pbp + j);
+                        for (int q = 0; q < P; ++q) v = fmaf(ldw(pWp + (size_t)q * da + j), LP[r * P + q], v);
                     } else {
                         for (int q = 0; q < P; ++q) {
                             const int bk = __float_as_int(LP[r * P + q]);
@@ -308,10 +430,15 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     for (int j = g_of; j < d; j += G) X[(size_t)j * R + r_of] = V[(size_t)j * R + r_of] * rn;
                 }
             } else if (p.kind != WM_KIND_GRU) {
-                linear_T<R, ACT_GELU>(p.W1t, p.b1, X, K1, p.hidden, Hb);
-                __syncthreads();
-                linear_T<R, ACT_NONE>(p.W2t, p.b2, Hb, p.hidden, d, V);
-                __syncthreads();
+                if (SPLIT && p.split_ok) {
+                    linear_T_split<R, ACT_GELU>(W1t, pb1, X, K1, p.hidden, Hb, scratch);
+                    linear_T_split<R, ACT_NONE>(W2t, pb2, Hb, p.hidden, d, V, scratch);
+                } else {
+                    linear_T<R, ACT_GELU, WS>(W1t, pb1, X, K1, p.hidden, Hb);
+                    __syncthreads();
+                    linear_T<R, ACT_NONE, WS>(W2t, pb2, Hb, p.hidden, d, V);
+                    __syncthreads();
+                }
                 if (p.kind == WM_KIND_MLP_LN) {
                     // v = z + V; two-pass LayerNorm over the d features of each row
                     float s = 0.0f;
@@ -340,7 +467,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     if (live_row) {
                         for (int j = g_of; j < d; j += G) {
                             const float c = (V[(size_t)j * R + r_of] - mean) * rstd;
-                            X[(size_t)j * R + r_of] = fmaf(__ldg(p.gamma + j), c, __ldg(p.beta + j));
+                            X[(size_t)j * R + r_of] = fmaf(ldw(pg + j), c, ldw(pbe + j));
                         }
                     }
                 } else {
@@ -408,11 +535,16 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
         const float* in = X;
         for (int l = 0; l < p.n_lin; ++l) {
             float* out = (l & 1) ? ALT : Hb;
-            if (l + 1 < p.n_lin)
-                linear_T<R, ACT_GELU>(p.Wst[l], p.bs[l], in, p.sdim[l], p.sdim[l + 1], out);
-            else
-                linear_T<R, ACT_NONE>(p.Wst[l], p.bs[l], in, p.sdim[l], p.sdim[l + 1], out);
-            __syncthreads();
+            if (SPLIT && p.split_ok) {
+                if (l + 1 < p.n_lin) linear_T_split<R, ACT_GELU>(Wst[l], bsv[l], in, p.sdim[l], p.sdim[l + 1], out, scratch);
+                else linear_T_split<R, ACT_NONE>(Wst[l], bsv[l], in, p.sdim[l], p.sdim[l + 1], out, scratch);
+            } else {
+                if (l + 1 < p.n_lin)
+                    linear_T<R, ACT_GELU, WS>(Wst[l], bsv[l], in, p.sdim[l], p.sdim[l + 1], out);
+                else
+                    linear_T<R, ACT_NONE, WS>(Wst[l], bsv[l], in, p.sdim[l], p.sdim[l + 1], out);
+                __syncthreads();
+            }
             in = out;
         }
         // ---- a6: scatter to the original order
@@ -434,13 +566,58 @@ static size_t generic_smem_bytes(const Model& m, int R, int* maxw_out, int* alt_
     return floats * 4 + (5 * R + 4) * sizeof(int);
 }
 
-template <int R>
+template <int R, bool WS>
 static int launch_R(wm_ctx* ctx, const GenericParams& p, size_t smem, int grid, cudaStream_t st) {
-    WM_CUDA_TRY(cudaFuncSetAttribute(wm_generic_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    wm_generic_kernel<R><<<grid, kGenericThreads, smem, st>>>(p);
+    // (the attribute call costs microseconds of host time per launch — the whole budget of a cfg-1-sized call: made only
+    // when this instance needs more shared memory than it has been granted on this device)
+    static std::atomic<int> granted[16];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    dev &= 15;
+    if (granted[dev].load(std::memory_order_relaxed) < (int)smem) {
+        WM_CUDA_TRY(cudaFuncSetAttribute(wm_generic_kernel<R, WS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        granted[dev].store((int)smem, std::memory_order_relaxed);
+    }
+    wm_generic_kernel<R, WS><<<grid, kGenericThreads, smem, st>>>(p);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
     return WM_OK;
+}
+
+// Weights-in-shared-memory mode: residual-MLP models (no TransH / GRU matrices) with an MLP ranker whose W1t, W2t and
+// scorer matrices fit beside the tile; every matrix a multiple of 16 bytes (bulk-copy granularity).  Fills the ws_*
+// fields and returns the total dynamic shared memory, or 0 when the mode does not apply.
+static size_t weights_in_smem(const wm_ctx* ctx, GenericParams* p, size_t tile_bytes) {
+    const Model& m = ctx->m;
+    if ((m.kind != WM_KIND_MLP && m.kind != WM_KIND_MLP_LN) || m.ranker_kind != WM_RANKER_MLP || m.n_lin < 1 ||
+        m.embed != WM_EMBED_LINEAR)
+        return 0;
+    size_t off = 0;   // in floats
+    auto take = [&](size_t n, uint32_t* at) -> bool {
+        if ((n * 4) % 16 != 0) return false;
+        *at = (uint32_t)off;
+        off += n;
+        return true;
+    };
+    if (!take((size_t)(m.d + m.d_a) * m.hidden, &p->ws_w1) || !take((size_t)m.hidden * m.d, &p->ws_w2)) return 0;
+    for (int l = 0; l < m.n_lin; ++l) {
+        if (!take((size_t)m.sdim[l] * m.sdim[l + 1], &p->ws_s[l])) return 0;
+        p->ws_bs[l] = (uint32_t)off;            // (every device vector is allocated with 16 spare bytes: the copy is rounded up)
+        off += ((size_t)m.sdim[l + 1] + 3) & ~(size_t)3;
+    }
+    if (!take((size_t)m.n_types * m.d_a, &p->ws_E) || !take((size_t)m.P * m.d_a, &p->ws_Wp) || !take(m.d_a, &p->ws_bp) ||
+        !take(m.hidden, &p->ws_b1) || !take(m.d, &p->ws_b2))
+        return 0;
+    if (m.kind == WM_KIND_MLP_LN && (!take(m.d, &p->ws_g) || !take(m.d, &p->ws_be))) return 0;
+    bool split_ok = m.hidden <= kGenericThreads && m.d <= kGenericThreads;
+    for (int l = 1; l <= m.n_lin; ++l) split_ok &= m.sdim[l] <= kGenericThreads;
+    p->split_ok = split_ok ? 1 : 0;
+    const size_t base = (tile_bytes + 127) & ~(size_t)127;
+    const size_t total = base + off * 4 + 16 + (size_t)kGenericThreads * 8 * 4;   // + barrier + split-K scratch (R <= 8)
+    if (total > (size_t)ctx->smem_optin || off * 4 >= (1u << 20)) return 0;   // (mbarrier tx-count: < 2^20 bytes per phase)
+    p->ws_off = (uint32_t)base;
+    p->ws_bytes = (uint32_t)(off * 4);
+    return total;
 }
 
 static int pick_R(const wm_ctx* ctx, int64_t B, size_t* smem_out, int* maxw, int* alt) {
@@ -488,13 +665,27 @@ int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st) {
         return WM_ERR_UNSUPPORTED;
     }
     p.n_tiles = (int)((a.B + R - 1) / R);
-    int grid = p.n_tiles < ctx->n_sms * 4 ? p.n_tiles : ctx->n_sms * 4;
-    if (grid < 1) return WM_OK;
+    if (p.n_tiles < 1) return WM_OK;
+    p.ws_off = p.ws_bytes = p.ws_w1 = p.ws_w2 = 0;
+    p.split_ok = 0;
+    p.ws_E = p.ws_Wp = p.ws_bp = p.ws_b1 = p.ws_b2 = p.ws_g = p.ws_be = 0;
+    for (int i = 0; i < kMaxScorerLinears; ++i) p.ws_s[i] = p.ws_bs[i] = 0;
+    const size_t ws_total = weights_in_smem(ctx, &p, smem);
+    if (ws_total) {       // one CTA per SM (the weights take most of its shared memory), each walks its tiles
+        const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
+        switch (R) {
+            case 32: return launch_R<32, true>(ctx, p, ws_total, grid, st);
+            case 16: return launch_R<16, true>(ctx, p, ws_total, grid, st);
+            case 8: return launch_R<8, true>(ctx, p, ws_total, grid, st);
+            default: return launch_R<4, true>(ctx, p, ws_total, grid, st);
+        }
+    }
+    const int grid = p.n_tiles < ctx->n_sms * 4 ? p.n_tiles : ctx->n_sms * 4;
     switch (R) {
-        case 32: return launch_R<32>(ctx, p, smem, grid, st);
-        case 16: return launch_R<16>(ctx, p, smem, grid, st);
-        case 8: return launch_R<8>(ctx, p, smem, grid, st);
-        default: return launch_R<4>(ctx, p, smem, grid, st);
+        case 32: return launch_R<32, false>(ctx, p, smem, grid, st);
+        case 16: return launch_R<16, false>(ctx, p, smem, grid, st);
+        case 8: return launch_R<8, false>(ctx, p, smem, grid, st);
+        default: return launch_R<4, false>(ctx, p, smem, grid, st);
     }
 }
 
