@@ -11,7 +11,8 @@ from typing import Tuple
 KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH = 0, 1, 2, 3
 DTYPE_FP32, DTYPE_BF16 = 0, 1
 EMBED_LINEAR, EMBED_BUCKET = 0, 1
-PHI_MEAN, PHI_STRUCT = 0, 1     # action features of the ranker: mean action embedding | structured statistics (f2)
+PHI_MEAN, PHI_STRUCT, PHI_TYPED = 0, 1, 2     # action features of the ranker: mean action embedding | structured statistics
+                                              # pooled per parameter slot (f2, S25) | kept per action type (f2, S28)
 RANKER_MLP, RANKER_FOREST = 0, 1   # G: the configs' MLP | a tree ensemble, the paper's own kind of ranker (f4)
 
 
@@ -61,6 +62,8 @@ class WMConfig:
     def phi_dim(self) -> int:
         """Width of phi: d_a for the mean action embedding; per-type counts, length and per-slot sum / mean / max of
         log2 params for the structured form."""
+        if self.phi_kind == PHI_TYPED:
+            return self.n_types + 1 + 3 * self.n_types * self.P
         return self.d_a if self.phi_kind == PHI_MEAN else self.n_types + 1 + 3 * self.P
 
     @property
@@ -138,6 +141,15 @@ CONFIGS = {
                  T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
                  param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(), k=64,
                  phi_kind=PHI_STRUCT, ranker_kind=RANKER_FOREST, n_trees=128, tree_depth=6),
+    # NEXT row f2 as SURVEY.md §8(f) words it — PER-TYPE numeric statistics ("action-specific numeric attributes",
+    # PAPER.md:186; S28).  13 = cfg 1's shapes (fp32, 209 features), 14 = cfg 2's shapes and batch (609 features).
+    13: WMConfig("f2_typedphi_tiny_fp32", 13, KIND_MLP, DTYPE_FP32, EMBED_LINEAR, S=1, per_subgraph=64, T_max=8,
+                 len_dist="uniform", len_lo=0, len_hi=8, n_types=16, P=4, param_dist="uniform", param_hi=64,
+                 n_buckets=0, d=64, d_a=32, hidden=128, H=8, scorer_widths=(128,), k=8, phi_kind=PHI_TYPED),
+    14: WMConfig("f2_typedphi_evolution_round", 14, KIND_MLP_LN, DTYPE_BF16, EMBED_LINEAR, S=16, per_subgraph=2048,
+                 T_max=32, len_dist="uniform", len_lo=8, len_hi=32, n_types=32, P=6, param_dist="loguniform",
+                 param_hi=1024, n_buckets=0, d=256, d_a=128, hidden=512, H=16, scorer_widths=(512, 512), k=64,
+                 phi_kind=PHI_TYPED),
 }
 
 

@@ -19,7 +19,7 @@ from typing import Dict, List
 import numpy as np
 
 from .configs import (WMConfig, KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH, DTYPE_BF16, EMBED_LINEAR, EMBED_BUCKET,
-                      PHI_STRUCT, RANKER_FOREST)
+                      PHI_STRUCT, PHI_TYPED, RANKER_FOREST)
 
 MAGIC = b"WMW1"
 VERSION = 1
@@ -112,7 +112,7 @@ def make_weights(cfg: WMConfig) -> Dict[str, np.ndarray]:
         else:  # bias of the layer drawn just before it
             fan_in = shapes[_matrix_of(name)][1]
             t = rng.standard_normal(shp) / np.sqrt(fan_in)
-        if name == "Ws0" and cfg.phi_kind == PHI_STRUCT:
+        if name == "Ws0" and cfg.phi_kind in (PHI_STRUCT, PHI_TYPED):
             t = t * phi_column_scale(cfg)[None, :]
         t = t.astype(np.float32)
         if cfg.dtype == DTYPE_BF16:
@@ -153,6 +153,12 @@ def phi_column_scale(cfg: WMConfig) -> np.ndarray:
     sc = np.ones(cfg.scorer_in)
     o, nt, P, T = cfg.d, cfg.n_types, cfg.P, float(cfg.T_max)
     sc[o:o + nt + 1] = 1.0 / T                              # per-type counts, length
+    if cfg.phi_kind == PHI_TYPED:                           # per type: sums | means | maxima (a type occurs ~T/nt times)
+        for k in range(nt):
+            b = o + nt + 1 + 3 * P * k
+            sc[b:b + P] = 1.0 / (10.0 * max(T / nt, 1.0))
+            sc[b + P:b + 3 * P] = 0.1
+        return sc
     sc[o + nt + 1:o + nt + 1 + P] = 1.0 / (10.0 * T)        # sums of log2 params
     sc[o + nt + 1 + P:o + nt + 1 + 3 * P] = 0.1             # means, maxima
     return sc

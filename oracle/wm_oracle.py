@@ -36,7 +36,7 @@ from scipy.special import erf as _erf
 
 KIND_MLP, KIND_MLP_LN, KIND_GRU, KIND_TRANSH = 0, 1, 2, 3
 EMBED_LINEAR, EMBED_BUCKET = 0, 1
-PHI_MEAN, PHI_STRUCT = 0, 1
+PHI_MEAN, PHI_STRUCT, PHI_TYPED = 0, 1, 2
 F64 = np.float64
 
 
@@ -163,6 +163,39 @@ def phi_struct(ids, params, n_types: int) -> np.ndarray:
     return np.concatenate([counts, [float(n)], s, m, x])
 
 
+def phi_struct_typed(ids, params, n_types: int) -> np.ndarray:
+    """Structured action features with ACTION-SPECIFIC numeric attributes (phi_kind = PHI_TYPED; S28).
+
+    PAPER.md:186 lists "action counts, sequence length, and action-specific numeric attributes": slot j of one action type
+    is a different attribute from slot j of another (a split factor, an unroll depth, a thread extent ...), so the numeric
+    statistics are kept PER ACTION TYPE instead of pooled per slot as in phi_struct (S25).  Layout, in this order:
+        c_k                                    k = 0..n_types-1     (action counts)
+        len                                                         (sequence length)
+        for every type k = 0..n_types-1:
+            s_kj = sum over steps of type k of log2 p_tj,   j = 0..P-1
+            m_kj = s_kj / c_k                               (0 when the type does not occur)
+            x_kj = max over steps of type k of log2 p_tj    (0 when the type does not occur)
+    Returns float64 [n_types + 1 + 3 n_types P]."""
+    ids = np.asarray(ids).astype(np.int64).reshape(-1)
+    par = np.asarray(params)
+    n, P = ids.shape[0], par.shape[-1]
+    lp = np.log2(par.reshape(n, P).astype(F64)) if n else np.zeros((0, P), dtype=F64)
+    counts = np.zeros(n_types, dtype=F64)
+    blocks = []
+    for k in range(n_types):
+        rows = lp[ids == k]
+        counts[k] = rows.shape[0]
+        if rows.shape[0] == 0:
+            blocks.append(np.zeros(3 * P, dtype=F64))
+        else:
+            blocks.append(np.concatenate([rows.sum(axis=0), rows.sum(axis=0) / rows.shape[0], rows.max(axis=0)]))
+    return np.concatenate([counts, [float(n)]] + blocks)
+
+
+def _phi_features(phi_kind: int, ids, params, n_types: int) -> np.ndarray:
+    return phi_struct_typed(ids, params, n_types) if phi_kind == PHI_TYPED else phi_struct(ids, params, n_types)
+
+
 def forest_score(x, Tf, Tt, Tv, Tb, return_margin: bool = False):
     """Tree-ensemble ranker (NEXT row f4).  PAPER.md:190: "G is implemented as an XGBoost ranking model" — an additive
     ensemble of regression trees over the concatenated features (Eq.12); the paper prints no tree, so reading S27
@@ -281,9 +314,10 @@ def rollout_score_vec(w: Dict[str, np.ndarray], init_states, action_ids, action_
             asum[idx] += a
             z[idx] = _step(w, z[idx], a, ln_eps)       # masked rows keep z unchanged
         phi = np.where(ln[:, None] > 0, asum / np.maximum(ln, 1)[:, None], 0.0)
-        if phi_kind == PHI_STRUCT:
+        if phi_kind != PHI_MEAN:
             n_types = w["E"].shape[0] if "E" in w else w["Tbl"].shape[0] // (P * n_buckets)
-            phi = np.stack([phi_struct(ids[lo + i, :ln[i]], par[lo + i, :ln[i], :], n_types) for i in range(n)])
+            phi = np.stack([_phi_features(phi_kind, ids[lo + i, :ln[i]], par[lo + i, :ln[i], :], n_types) for i in range(n)]) \
+                if n else np.zeros((0, 0))
         scores[lo:hi] = _rank(np.concatenate([z, phi, h], axis=-1), w, nl)
         if return_latent:
             lat[lo:hi] = z
@@ -335,8 +369,8 @@ def rollout_score_from(w, bank, bank_index, start, action_ids, action_params, le
         z = bank[int(bank_index[b])][None, :].copy()
         for t in range(st, n):
             z = _step(w, z, _embed(w, ids[b:b + 1, t], par[b:b + 1, t, :], P, n_buckets), ln_eps)
-        if phi_kind == PHI_STRUCT:
-            phi = phi_struct(ids[b, :n], par[b, :n, :], n_types)
+        if phi_kind != PHI_MEAN:
+            phi = _phi_features(phi_kind, ids[b, :n], par[b, :n, :], n_types)
         elif n > 0:
             phi = _embed(w, ids[b, :n], par[b, :n, :], P, n_buckets).sum(axis=0) / n
         else:
@@ -432,6 +466,21 @@ def rollout_score_scalar(w, init_states, action_ids, action_params, lengths, hw_
                     tot[j] += l2
                     big[j] = l2 if t == 0 else max(big[j], l2)
             phi = cnt + [float(lens[b])] + tot + [v / lens[b] if lens[b] > 0 else 0.0 for v in tot] + big
+        elif phi_kind == PHI_TYPED:  # S28, by counting loops (independent of phi_struct_typed above)
+            n_types = len(W["E"]) if "E" in W else len(W["Tbl"]) // (P * n_buckets)
+            cnt = [0.0] * n_types
+            tot = [[0.0] * P for _ in range(n_types)]
+            big = [[0.0] * P for _ in range(n_types)]
+            for t in range(lens[b]):
+                k = ids[b][t]
+                for j in range(P):
+                    l2 = math.log2(par[b][t][j])
+                    tot[k][j] += l2
+                    big[k][j] = l2 if cnt[k] == 0.0 else max(big[k][j], l2)
+                cnt[k] += 1.0
+            phi = cnt + [float(lens[b])]
+            for k in range(n_types):
+                phi += tot[k] + [v / cnt[k] if cnt[k] > 0 else 0.0 for v in tot[k]] + big[k]
         x = z + phi + list(hw[s])
         if "Tf" in W:      # tree ensemble (S27), comparisons in float32
             nodes = len(W["Tf"][0])
@@ -531,7 +580,7 @@ def read_weight_file(path: str):
     if version == 3:      # version 3 = version 2 + uint32 ranker_kind, n_trees, tree_depth
         hdr["ranker_kind"], hdr["n_trees"], hdr["tree_depth"] = struct.unpack_from("<3I", raw, pos)
         pos += 12
-    phi_dim = d_a if hdr["phi_kind"] == PHI_MEAN else n_types + 1 + 3 * P
+    phi_dim = {PHI_MEAN: d_a, PHI_STRUCT: n_types + 1 + 3 * P, PHI_TYPED: n_types + 1 + 3 * n_types * P}[hdr["phi_kind"]]
     w = {}
 
     def take(name, *shape):

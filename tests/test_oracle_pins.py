@@ -132,6 +132,64 @@ def test_p16_phi_struct_hand_worked(golden):
     assert np.abs(oracle.phi_struct([0, 2, 0], par, 4) - np.array(g["phi"])).max() >= 1.0
 
 
+def test_p22_phi_typed_hand_worked(golden):
+    """NEXT row f2 as SURVEY.md words it: per-TYPE numeric statistics (S28)."""
+    g = golden("p22_phi_typed.txt")
+    ids = [1, 0, 1]; par = [[2, 8], [4, 1], [16, 2]]
+    np.testing.assert_allclose(oracle.phi_struct_typed(ids, par, 3), g["phi"], rtol=0, atol=0)
+    np.testing.assert_allclose(oracle.phi_struct_typed(ids[:1], par[:1], 3), g["phi_prefix1"], rtol=0, atol=0)
+    np.testing.assert_allclose(oracle.phi_struct_typed([], np.zeros((0, 2), dtype=np.int32), 3), g["phi_empty"], rtol=0, atol=0)
+    # the fixture discriminates: swapped parameter slots, swapped type ids, a statistic pooled over types
+    assert np.abs(oracle.phi_struct_typed(ids, [q[::-1] for q in par], 3) - np.array(g["phi"])).max() >= 1.0
+    assert np.abs(oracle.phi_struct_typed([0, 1, 0], par, 3) - np.array(g["phi"])).max() >= 1.0
+    assert len(g["phi"]) == 3 + 1 + 3 * 3 * 2
+
+
+def test_p23_phi_typed_closed_forms_and_placement():
+    """Closed forms that tie phi_struct_typed to the (pinned) pooled phi_struct and to plain numpy, and its placement in
+    the ranker's input [z_T ; phi ; h] through the scalar and vector rollouts."""
+    rng = np.random.default_rng(23)
+    NT, P, n = 5, 3, 17
+    ids = rng.integers(0, NT, n); par = rng.integers(1, 200, (n, P))
+    t = oracle.phi_struct_typed(ids, par, NT)
+    s = oracle.phi_struct(ids, par, NT)
+    lp = np.log2(par.astype(np.float64))
+    blocks = t[NT + 1:].reshape(NT, 3, P)
+    np.testing.assert_array_equal(t[:NT + 1], s[:NT + 1])                                 # counts and length are the same
+    np.testing.assert_allclose(blocks[:, 0].sum(axis=0), s[NT + 1:NT + 1 + P], rtol=1e-14)   # per-type sums add up to the pooled sums
+    np.testing.assert_allclose((t[:NT, None] * blocks[:, 1]).sum(axis=0), s[NT + 1:NT + 1 + P], rtol=1e-14)   # sum_k c_k m_k = pooled sum
+    np.testing.assert_array_equal(blocks[:, 2].max(axis=0), s[NT + 1 + 2 * P:])             # max over types of per-type maxima
+    for k in range(NT):                                                                     # each block against numpy on the type's rows
+        rows = lp[ids == k]
+        want = np.concatenate([rows.sum(0), rows.mean(0), rows.max(0)]) if len(rows) else np.zeros(3 * P)
+        np.testing.assert_allclose(blocks[k].reshape(-1), want, rtol=1e-14, atol=0)
+    # a sequence of ONE type: that type's block is the pooled statistics, every other block is zero
+    one = np.full(n, 3)
+    t1 = oracle.phi_struct_typed(one, par, NT); s1 = oracle.phi_struct(one, par, NT)
+    np.testing.assert_allclose(t1[NT + 1:].reshape(NT, 3 * P)[3], s1[NT + 1:], rtol=1e-14)
+    assert np.count_nonzero(np.delete(t1[NT + 1:].reshape(NT, 3 * P), 3, axis=0)) == 0
+    # order of the steps does not matter; concatenating sequences adds counts and sums
+    perm = rng.permutation(n)
+    np.testing.assert_allclose(oracle.phi_struct_typed(ids[perm], par[perm], NT), t, rtol=1e-14)
+    a, b = oracle.phi_struct_typed(ids[:7], par[:7], NT), oracle.phi_struct_typed(ids[7:], par[7:], NT)
+    np.testing.assert_allclose(a[:NT + 1] + b[:NT + 1], t[:NT + 1])
+    np.testing.assert_allclose(a[NT + 1:].reshape(NT, 3, P)[:, 0] + b[NT + 1:].reshape(NT, 3, P)[:, 0], blocks[:, 0], rtol=1e-14)
+    # placement: a one-linear ranker with a unit weight on one input reads exactly that feature, vector == scalar rollout
+    cfg = WMConfig(**{**gen.get_config(13).__dict__, "d": 6, "d_a": 4, "hidden": 8, "scorer_widths": (), "S": 2,
+                      "per_subgraph": 5, "n_types": 3, "P": 2})
+    w = gen.make_weights(cfg); bt = gen.make_inputs(cfg)
+    F = cfg.phi_dim
+    assert F == 3 + 1 + 18 and w["Ws0"].shape == (1, cfg.d + F + cfg.H)
+    for col in (0, 2, 3, 4, 9, 10, F - 1):
+        w1 = dict(w); w1["Ws0"] = np.zeros_like(w["Ws0"]); w1["Ws0"][0, cfg.d + col] = 1.0; w1["bs0"] = np.zeros_like(w["bs0"])
+        kw = dict(phi_kind=cfg.phi_kind)
+        yv = oracle.rollout_score_vec(w1, bt.init_states, bt.action_ids, bt.action_params, bt.lengths, bt.hw_feats, bt.subgraph_offsets, **kw)
+        ys = oracle.rollout_score_scalar(w1, bt.init_states, bt.action_ids, bt.action_params, bt.lengths, bt.hw_feats, bt.subgraph_offsets, **kw)
+        want = [oracle.phi_struct_typed(bt.action_ids[i, :bt.lengths[i]], bt.action_params[i, :bt.lengths[i]], 3)[col] for i in range(bt.B)]
+        np.testing.assert_allclose(yv, want, rtol=1e-14, atol=0)
+        np.testing.assert_allclose(ys, want, rtol=1e-13, atol=1e-13)
+
+
 def test_p17_phi_struct_closed_forms_and_placement():
     rng = np.random.default_rng(17)
     nt, P, n = 7, 3, 11
