@@ -74,6 +74,10 @@ extern "C" {
                                /* c_k = number of steps of type k, s_j / m_j / x_j = sum / mean / max over the valid   */
                                /* steps of log2 p_tj, all 0 for an empty sequence (S25).       */
                                /* n_types + 1 + 3P values; this build needs n_types + 1 + 3P <= d_a                    */
+#define WM_PHI_TYPED    2      /* phi = [c_k (n_types) | len | per type k: s_kj (P) | m_kj (P) | x_kj (P)]: the numeric  */
+                               /* statistics kept PER ACTION TYPE, over the steps of that type, 0 for a type that does   */
+                               /* not occur ("action-specific numeric attributes"; S28).         */
+                               /* n_types (1 + 3P) + 1 values, no relation to d_a; runs on the fp32 kernel              */
 
 /* wm_set_option keys */
 #define WM_RANKER_MLP    0     /* G = the configs' MLP                                                              */

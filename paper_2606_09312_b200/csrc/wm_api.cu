@@ -120,7 +120,7 @@ static int load_weights_impl(const char* path, int device, wm_ctx** ctx_out) {
         return WM_ERR_FORMAT;
     }
     uint32_t phi_kind = WM_PHI_MEAN;   // version 2 = the version-1 header followed by uint32 phi_kind
-    if (h.version >= 2 && (fread(&phi_kind, 4, 1, f) != 1 || phi_kind > WM_PHI_STRUCT)) {
+    if (h.version >= 2 && (fread(&phi_kind, 4, 1, f) != 1 || phi_kind > WM_PHI_TYPED)) {
         fclose(f);
         set_error("wm_load_weights: bad phi_kind");
         return WM_ERR_FORMAT;
@@ -168,8 +168,16 @@ static int load_weights_impl(const char* path, int device, wm_ctx** ctx_out) {
     };
     const int d = h.d, da = h.d_a, hid = h.hidden;
     // width of phi: the mean action embedding, or counts | len | per-slot sum, mean, max of log2 params (S25)
-    const int phi_dim = phi_kind == WM_PHI_MEAN ? da : (int)(h.n_types + 1 + 3 * h.P);
-    if (phi_dim > da) {   // the kernels keep phi in the rows / K-blocks of the action embedding
+    const uint64_t phi_dim64 = phi_kind == WM_PHI_MEAN ? (uint64_t)da
+                               : phi_kind == WM_PHI_STRUCT ? (uint64_t)h.n_types + 1 + 3 * (uint64_t)h.P
+                                                           : (uint64_t)h.n_types * (1 + 3 * (uint64_t)h.P) + 1;
+    if (phi_dim64 > (1u << 20)) {
+        fclose(f);
+        set_error("wm_load_weights: header field out of range (phi width)");
+        return WM_ERR_FORMAT;
+    }
+    const int phi_dim = (int)phi_dim64;
+    if (phi_kind == WM_PHI_STRUCT && phi_dim > da) {   // the kernels keep the pooled phi in the rows / K-blocks of the action embedding
         fclose(f);
         set_error("wm_load_weights: structured phi needs n_types + 1 + 3 P <= d_a in this build");
         return WM_ERR_UNSUPPORTED;

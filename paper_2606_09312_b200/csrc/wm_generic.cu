@@ -21,6 +21,8 @@ struct GenericParams {
     int sdim[kMaxScorerLinears + 1];
     int maxw;        // rows of buffer Hb
     int alt_rows;    // rows of the region that holds V, AS, Y (and the scorer's second ping-pong buffer)
+    int xa_rows;     // rows of X's middle part: max(da, phi_dim) (the step's a, then phi for the scorer)
+    int as_rows;     // rows of AS: da, or for WM_PHI_TYPED n_types + 2 n_types P (counts, per-type sums, per-type maxima)
     float ln_eps;
     const float *E, *WpT, *bp, *Tbl;
     const float *W1t, *b1, *W2t, *b2, *gamma, *beta;
@@ -192,14 +194,14 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
     extern __shared__ __align__(16) float smem[];
     const int d = p.d, da = p.da, H = p.H, P = p.P;
     const int K1 = d + da;
-    float* X = smem;                                   // [(d+da+H)][R]  rows: z | a (phi) | hw
-    float* Hb = X + (size_t)(K1 + H) * R;              // [maxw][R]
+    float* X = smem;                                   // [(d+xa_rows+H)][R]  rows: z | a (phi) | hw
+    float* Hb = X + (size_t)(d + p.xa_rows + H) * R;   // [maxw][R]
     float* ALT = Hb + (size_t)p.maxw * R;              // [alt_rows][R]: V | AS | Y   (scorer: ping-pong buffer)
     float* V = ALT;                                    // [d][R]
     float* AS = V + (size_t)d * R;                     // [da][R] running sum of a (WM_PHI_MEAN), or the running
                                                        // statistics of WM_PHI_STRUCT: counts [n_types], then per
                                                        // parameter slot sum [P] and max [P] of log2 p
-    float* Y = AS + (size_t)da * R;                    // [(d+da)][R], GRU and TransH only
+    float* Y = AS + (size_t)p.as_rows * R;             // [(d+da)][R], GRU and TransH only
     float* LP = ALT + (size_t)p.alt_rows * R;          // [R][P] log2(param) or bucket index (as int bits)
     float* RED = LP + (size_t)R * P;                   // [G][R] reduction scratch, G = threads / R
     int* meta = reinterpret_cast<int*>(RED + kGenericThreads);   // cand[R], len[R], seg[R], id[R], start[R], tile_len, tile_pre
@@ -305,7 +307,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
             }
             X[(size_t)j * R + r] = v;
         }
-        for (int e = tid; e < da * R; e += kGenericThreads) AS[e] = 0.0f;
+        for (int e = tid; e < p.as_rows * R; e += kGenericThreads) AS[e] = 0.0f;
         __syncthreads();
 
         // Iterations tq < 0 walk the prefix positions [0, start) of every row: embedding and phi statistics only, no
@@ -328,7 +330,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     }
                 }
                 m_id[tid] = id;
-                if (p.phi_kind == WM_PHI_STRUCT && live_of(tid)) AS[(size_t)id * R + tid] += 1.0f;
+                if (p.phi_kind != WM_PHI_MEAN && live_of(tid)) AS[(size_t)id * R + tid] += 1.0f;
             }
             for (int e = tid; e < R * P; e += kGenericThreads) {
                 const int r = e / P, j = e % P;
@@ -343,6 +345,14 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                         const float l2 = log2f((float)prm);
                         float* sum = AS + (size_t)(p.n_types + j) * R + r;
                         float* mx = AS + (size_t)(p.n_types + P + j) * R + r;
+                        *sum += l2;
+                        *mx = fmaxf(*mx, l2);
+                    } else if (p.phi_kind == WM_PHI_TYPED) {   // per action type (S28); the id is re-read here: m_id is
+                        int id = __ldg(a.action_ids + (size_t)m_cand[r] * a.T_max + pos_of(r));   // written by another thread
+                        id = id < 0 ? 0 : (id >= p.n_types ? p.n_types - 1 : id);
+                        const float l2 = log2f((float)prm);
+                        float* sum = AS + (size_t)(p.n_types + id * P + j) * R + r;
+                        float* mx = AS + (size_t)(p.n_types + p.n_types * P + id * P + j) * R + r;
                         *sum += l2;
                         *mx = fmaxf(*mx, l2);
                     }
@@ -514,6 +524,11 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
             float v;
             if (p.phi_kind == WM_PHI_MEAN) {
                 v = len > 0 ? AS[e] / (float)len : 0.0f;
+            } else if (p.phi_kind == WM_PHI_TYPED && j > NT) {   // per type k: sums | means | maxima (S28)
+                const int q = j - NT - 1, k = q / (3 * P), stat = (q / P) % 3, slot = q % P;
+                const float cnt = AS[(size_t)k * R + r];
+                const float sum = AS[(size_t)(NT + k * P + slot) * R + r];
+                v = stat == 0 ? sum : stat == 1 ? (cnt > 0.0f ? sum / cnt : 0.0f) : AS[(size_t)(NT + NT * P + k * P + slot) * R + r];
             } else if (j < NT) {                       // counts (S25)
                 v = AS[e];
             } else if (j == NT) {                      // length
@@ -552,16 +567,22 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
     }
 }
 
+static int generic_as_rows(const Model& m) {
+    const int typed = m.n_types + 2 * m.n_types * m.P;
+    return m.phi_kind == WM_PHI_TYPED && typed > m.d_a ? typed : m.d_a;
+}
+
 static size_t generic_smem_bytes(const Model& m, int R, int* maxw_out, int* alt_rows_out) {
     int maxw = m.d > m.hidden ? m.d : m.hidden;
     int maxsw = 1;
     for (int l = 1; l <= m.n_lin; ++l) maxsw = m.sdim[l] > maxsw ? m.sdim[l] : maxsw;
     if (maxsw > maxw) maxw = maxsw;
-    int alt = m.d + m.d_a + (m.kind == WM_KIND_GRU || m.kind == WM_KIND_TRANSH ? m.d + m.d_a : 0);
+    const int as_rows = generic_as_rows(m), xa_rows = m.phi_dim > m.d_a ? m.phi_dim : m.d_a;
+    int alt = m.d + as_rows + (m.kind == WM_KIND_GRU || m.kind == WM_KIND_TRANSH ? m.d + m.d_a : 0);
     if (maxsw > alt) alt = maxsw;
     *maxw_out = maxw;
     *alt_rows_out = alt;
-    size_t floats = (size_t)(m.d + m.d_a + m.H) * R + (size_t)maxw * R + (size_t)alt * R + (size_t)R * m.P +
+    size_t floats = (size_t)(m.d + xa_rows + m.H) * R + (size_t)maxw * R + (size_t)alt * R + (size_t)R * m.P +
                     kGenericThreads;
     return floats * 4 + (5 * R + 4) * sizeof(int);
 }
@@ -659,6 +680,8 @@ int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st) {
     for (int i = 0; i < kMaxScorerLinears; ++i) { p.Wst[i] = m.Wst[i]; p.bs[i] = m.bs[i]; }
     p.a = a;
     size_t smem = 0;
+    p.as_rows = generic_as_rows(m);
+    p.xa_rows = m.phi_dim > m.d_a ? m.phi_dim : m.d_a;
     const int R = pick_R(ctx, a.B, &smem, &p.maxw, &p.alt_rows);
     if (R == 0) {
         set_error("model too wide for the fp32 kernel's shared-memory tile");

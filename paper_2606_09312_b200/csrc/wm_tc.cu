@@ -853,7 +853,7 @@ struct TcState {
 }  // namespace
 
 static bool tc_model_ok(const Model& m) {
-    return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc::D &&
+    return m.phi_kind <= WM_PHI_STRUCT && m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc::D &&
            m.d_a == tc::DA && m.hidden >= 256 && m.hidden <= tc::MAX_HID && m.hidden % 128 == 0 &&
            ((m.n_lin == 3 && m.sdim[1] == tc::SW && m.sdim[2] == tc::SW) || m.ranker_kind == WM_RANKER_FOREST) && m.H >= 8 && m.H <= tc::MAX_H && m.H % 8 == 0 &&
            m.n_types <= tc::MAX_TYPES && m.P <= tc::MAX_P;

@@ -963,7 +963,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 }  // namespace
 
 bool tcp_model_ok(const Model& m) {
-    return m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tcp::D &&
+    return m.phi_kind <= WM_PHI_STRUCT && m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tcp::D &&
            m.d_a == tcp::DA && m.hidden >= 256 && m.hidden <= tcp::MAX_HID && m.hidden % 128 == 0 &&
            ((m.n_lin == 3 && m.sdim[1] == tcp::SW && m.sdim[2] == tcp::SW) || m.ranker_kind == WM_RANKER_FOREST) &&
            m.H >= 8 && m.H <= tcp::MAX_H && m.H % 8 == 0 && m.n_types <= tcp::MAX_TYPES && m.P <= tcp::MAX_P;

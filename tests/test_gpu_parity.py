@@ -25,7 +25,9 @@ SMALL = {1: dict(S=1, per_subgraph=64), 2: dict(S=3, per_subgraph=171), 3: dict(
          # NEXT row f1 (TransH transition): 6 = the fp32 parity case, 7 = cfg 2's shapes (bf16-valued weights)
          6: dict(S=1, per_subgraph=64), 7: dict(S=3, per_subgraph=171),
          # NEXT row f2 (structured phi): 8 = the fp32 parity case, 9 = cfg 2's shapes
-         8: dict(S=1, per_subgraph=64), 9: dict(S=3, per_subgraph=171)}
+         8: dict(S=1, per_subgraph=64), 9: dict(S=3, per_subgraph=171),
+         # NEXT row f2, per-action-type statistics (S28): 13 = the fp32 parity case, 14 = cfg 2's shapes (609 features; fp32 kernel)
+         13: dict(S=1, per_subgraph=64), 14: dict(S=3, per_subgraph=171)}
 
 
 @pytest.fixture(scope="module")
@@ -59,7 +61,7 @@ def _paths(wm, cfg):
     return sorted({wm.PATH_FP32, info.path} | ({PATH_TC_SINGLE} if info.tc_variant == 5 else set()))
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9])
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9, 13, 14])
 def test_config_parity_small(wm, n):
     cfg = gen.get_config(n).scaled(**SMALL[n])
     w = gen.make_weights(cfg)
@@ -148,7 +150,7 @@ def _edge_case(n, case):
 EDGE_CASES = ["B1", "B127", "B129", "B257", "len0", "lenmax", "one_long", "param_ends"]
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9])
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9, 13, 14])
 @pytest.mark.parametrize("case", EDGE_CASES)
 def test_edge_cases(wm, n, case):
     cfg, b = _edge_case(n, case)
@@ -447,7 +449,7 @@ def test_full_size_forest_against_full_oracle(wm, n):
     print(f"full-size forest parity cfg {n}: " + ", ".join(f"path {k}: compared {v[0]:.3f}, overlap {v[1]:.4f}" for k, v in res.items()))
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9, 10, 11, 12])
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14])
 def test_outputs_do_not_overrun(wm, n):
     """compute-sanitizer is closed on this pool: canaries instead.  The score and index buffers are sub-ranges of
     larger allocations filled with sentinels; everything outside [0, B) / [0, S*k) must come back untouched, and a
@@ -496,7 +498,7 @@ def test_repeatable_bitwise_with_several_tiles_per_cta(wm, n):
         assert np.isfinite(y0).all()
 
 
-@pytest.mark.parametrize("n", [8, 9])
+@pytest.mark.parametrize("n", [8, 9, 13])
 def test_struct_phi_feature_readout(wm, n):
     """NEXT row f2: with a first scorer layer that copies single inputs (unit-vector rows, zero bias) followed by
     identity-like layers, the fp32 kernel's score IS one entry of [z_T ; phi ; h].  Config 8 (one linear): every
@@ -507,15 +509,17 @@ def test_struct_phi_feature_readout(wm, n):
     w = gen.make_weights(cfg)
     b = gen.make_inputs(cfg)
     F = cfg.phi_dim
-    want = np.stack([oracle.phi_struct(b.action_ids[i, :b.lengths[i]], b.action_params[i, :b.lengths[i]], cfg.n_types)
+    feats = oracle.phi_struct_typed if cfg.phi_kind == 2 else oracle.phi_struct
+    want = np.stack([feats(b.action_ids[i, :b.lengths[i]], b.action_params[i, :b.lengths[i]], cfg.n_types)
                      for i in range(b.B)])
-    for col in list(range(F)) + [F]:      # F = first hardware feature: hw sits right after phi
+    cols = list(range(F)) if F <= 64 else sorted(set(range(0, F, 7)) | set(range(cfg.n_types + 1)) | {F - 1})
+    for col in cols + [F]:      # F = first hardware feature: hw sits right after phi
         w1 = dict(w)
         w1["Ws0"] = np.zeros_like(w["Ws0"]); w1["Ws0"][0, cfg.d + col] = 1.0
         w1["bs0"] = np.zeros_like(w["bs0"])
         ctx = wm.wm_load_weights(weight_file(cfg, w1))
         wm.wm_set_option(ctx, wm.WM_OPT_PATH, wm.PATH_FP32)
-        assert wm.wm_get_info(ctx).phi_kind == 1
+        assert wm.wm_get_info(ctx).phi_kind == cfg.phi_kind
         y = gpu_scores(ctx, b)
         wm.wm_free(ctx)
         if col < F:

@@ -705,9 +705,9 @@ def test_p21_topk_overlap_hand_values():
 # ---- generator / file format ----------------------------------------------------------------------------------
 
 def test_weight_file_roundtrip(tmp_path):
-    for n in (1, 2, 5, 6, 8, 9, 10):
+    for n in (1, 2, 5, 6, 8, 9, 10, 13):
         cfg = gen.get_config(n)
-        if n not in (1, 8, 10):
+        if n not in (1, 8, 10, 13):
             cfg = WMConfig(**{**cfg.__dict__, "d": 16, "d_a": 8, "hidden": 0 if n == 5 else 24,
                               "scorer_widths": (12, 10)})
         w = gen.make_weights(cfg)
