@@ -224,6 +224,17 @@ int wm_score_topk_host(wm_ctx* ctx,
                        int64_t B, int32_t S, int32_t T_max, int32_t k,
                        float* scores_out, int32_t* idx_out, void* cuda_stream);
 
+/* The same call for callers that keep the action arrays compact — type ids as uint8 (n_types <= 256, else
+ * WM_ERR_UNSUPPORTED), parameters as uint16 (values 1..65535; BASELINE.json's configs draw them from 1..1024) — which is
+ * 13 instead of 28 bytes per action on the host-to-device link (the call is PCIe-bound at evolution-round sizes): the arrays
+ * are copied as they are and widened to int32 on the device (one extra small kernel).  Padding positions may hold anything.
+ * Same results, bit for bit, as wm_score_topk_host on the widened arrays; same errors. */
+int wm_score_topk_host_compact(wm_ctx* ctx,
+                               const float* init_states, const uint8_t* action_ids, const uint16_t* action_params,
+                               const int32_t* lengths, const float* hw_feats, const int32_t* subgraph_offsets,
+                               int64_t B, int32_t S, int32_t T_max, int32_t k,
+                               float* scores_out, int32_t* idx_out, void* cuda_stream);
+
 /* With WM_OPT_TIMING = 1: synchronise `cuda_stream` and return, in *ms_out, the device time of the rollout+score
  * kernel (K2 alone: bucketing and top-k excluded) of the most recent wm_rollout_score call made on that stream.
  * bench.py's roofline leg uses it.  Errors: WM_ERR_ARG (null, timing off, or no call yet), WM_ERR_CUDA. */

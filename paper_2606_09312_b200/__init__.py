@@ -23,7 +23,7 @@ PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 # every symbol include/wm.h declares
 ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
                "wm_rollout_latents", "wm_rollout_score_from",
-               "wm_check", "wm_score_topk_host", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error")
+               "wm_check", "wm_score_topk_host", "wm_score_topk_host_compact", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error")
 
 
 class WmInfo(ctypes.Structure):
@@ -75,6 +75,8 @@ def lib() -> ctypes.CDLL:
     L.wm_check.restype = ctypes.c_int
     L.wm_score_topk_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp, vp, vp]
     L.wm_score_topk_host.restype = ctypes.c_int
+    L.wm_score_topk_host_compact.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp, vp, vp]
+    L.wm_score_topk_host_compact.restype = ctypes.c_int
     L.wm_last_kernel_ms.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_float)]
     L.wm_last_kernel_ms.restype = ctypes.c_int
     L.wm_launch_count.argtypes = [vp]
@@ -182,6 +184,19 @@ def wm_score_topk_host(ctx: int, init_states, action_ids, action_params, lengths
     _check(lib().wm_score_topk_host(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
                                     _ptr(hw_feats), _ptr(subgraph_offsets), B, S, T_max, int(k),
                                     _ptr(scores_out), _ptr(idx_out), _stream(stream)))
+
+
+def wm_score_topk_host_compact(ctx: int, init_states, action_ids_u8, action_params_u16, lengths, hw_feats, subgraph_offsets,
+                               k: int, scores_out, idx_out, stream=None) -> None:
+    """wm_score_topk_host with uint8 type ids and uint16 parameters (HOST tensors).  include/wm.h."""
+    import torch
+    assert action_ids_u8.dtype == torch.uint8 and action_params_u16.dtype in (torch.uint16, torch.int16)
+    B = int(lengths.numel())
+    T_max = int(action_ids_u8.shape[1]) if action_ids_u8.dim() == 2 else 0
+    S = int(subgraph_offsets.numel()) - 1
+    _check(lib().wm_score_topk_host_compact(ctx, _ptr(init_states), _ptr(action_ids_u8), _ptr(action_params_u16), _ptr(lengths),
+                                            _ptr(hw_feats), _ptr(subgraph_offsets), B, S, T_max, int(k),
+                                            _ptr(scores_out), _ptr(idx_out), _stream(stream)))
 
 
 def wm_last_kernel_ms(ctx: int, stream=None) -> float:

@@ -2,6 +2,7 @@
 // No arithmetic of the method lives here; see wm_bucket.cu (a0), wm_generic.cu / wm_tc.cu (a1-a6), wm_topk.cu (a7).
 #include <cstdarg>
 #include <cstdio>
+#include <algorithm>
 #include <cstring>
 #include <new>
 
@@ -670,10 +671,21 @@ static int64_t host_chunk_min() {
 }
 #define kHostChunkMin host_chunk_min()
 
-int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* action_ids,
-                       const int32_t* action_params, const int32_t* lengths, const float* hw_feats,
-                       const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
-                       float* scores_out, int32_t* idx_out, void* cuda_stream) {
+// widen the compact host encodings (uint8 type ids, uint16 parameters) to the int32 arrays the kernels read
+__global__ void wm_widen_kernel(const uint8_t* __restrict__ ids8, const uint16_t* __restrict__ par16, int32_t* __restrict__ ids,
+                                int32_t* __restrict__ par, int64_t n_ids, int64_t n_par) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_par; i += stride) par[i] = par16[i];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_ids; i += stride) ids[i] = ids8[i];
+}
+
+// Shared body of wm_score_topk_host (int32 arrays: ib = pb = 4) and wm_score_topk_host_compact (ib = 1, pb = 2: the arrays
+// are staged as they come and widened on the device by wm_widen_kernel).
+static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const void* action_ids, const void* action_params,
+                                int ib, int pb, const int32_t* lengths, const float* hw_feats,
+                                const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
+                                float* scores_out, int32_t* idx_out, void* cuda_stream) {
+    const bool compact = ib != 4;
     if (!ctx) {
         set_error("wm_score_topk_host: null ctx");
         return WM_ERR_ARG;
@@ -717,7 +729,8 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
         cs[nch] = S;
     }
     const size_t b_reb = up16((size_t)(S + 5) * 4);
-    const size_t need = b_z0 + b_hw + b_ids + b_par + b_len + b_off + b_sc + b_idx + b_reb;
+    const size_t b_ids8 = compact ? up16((size_t)B * T_max * ib) : 0, b_par16 = compact ? up16((size_t)B * T_max * m.P * pb) : 0;
+    const size_t need = b_z0 + b_hw + b_ids + b_par + b_len + b_off + b_sc + b_idx + b_reb + b_ids8 + b_par16;
     if (ws->stage_cap < need) {
         if (ws->stage) {
             WM_CUDA_TRY(cudaStreamSynchronize(st));
@@ -737,8 +750,36 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
     int32_t* doff = (int32_t*)p; p += b_off;
     float* dsc = (float*)p; p += b_sc;
     int32_t* didx = (int32_t*)p; p += b_idx;
-    int32_t* dreb = (int32_t*)p;
+    int32_t* dreb = (int32_t*)p; p += b_reb;
+    uint8_t* dids8 = (uint8_t*)p; p += b_ids8;
+    uint16_t* dpar16 = (uint16_t*)p;
     const auto H2D = cudaMemcpyHostToDevice;
+    const char* h_ids = static_cast<const char*>(action_ids);
+    const char* h_par = static_cast<const char*>(action_params);
+    // copy candidates [c0, c0 + Bc) of the action arrays on stream `cs`; compact: stage raw, widen on stream `ks`
+    // (the caller orders `ks` after the copy)
+    auto copy_actions = [&](int64_t c0, int64_t Bc, cudaStream_t cs) -> int {
+        if (Bc <= 0 || T_max <= 0) return WM_OK;
+        const size_t ni = (size_t)Bc * T_max, np_ = ni * m.P;
+        if (!compact) {
+            WM_CUDA_TRY(cudaMemcpyAsync(dids + c0 * T_max, h_ids + (size_t)c0 * T_max * 4, ni * 4, H2D, cs));
+            WM_CUDA_TRY(cudaMemcpyAsync(dpar + c0 * T_max * m.P, h_par + (size_t)c0 * T_max * m.P * 4, np_ * 4, H2D, cs));
+        } else {
+            WM_CUDA_TRY(cudaMemcpyAsync(dids8 + c0 * T_max, h_ids + (size_t)c0 * T_max, ni, H2D, cs));
+            WM_CUDA_TRY(cudaMemcpyAsync(dpar16 + c0 * T_max * m.P, h_par + (size_t)c0 * T_max * m.P * 2, np_ * 2, H2D, cs));
+        }
+        return WM_OK;
+    };
+    auto widen = [&](int64_t c0, int64_t Bc, cudaStream_t ks) -> int {
+        if (!compact || Bc <= 0 || T_max <= 0) return WM_OK;
+        const int64_t ni = Bc * T_max, np_ = ni * m.P;
+        const int grid = (int)std::min<int64_t>((np_ + 255) / 256, (int64_t)ctx->n_sms * 8);
+        wm_widen_kernel<<<grid, 256, 0, ks>>>(dids8 + c0 * T_max, dpar16 + c0 * T_max * m.P, dids + c0 * T_max,
+                                              dpar + c0 * T_max * m.P, ni, np_);
+        WM_CUDA_TRY(cudaGetLastError());
+        ctx->launches.fetch_add(1);
+        return WM_OK;
+    };
     if (nch > 1) {
         if (!ctx->hs_copy) {
             WM_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->hs_copy, cudaStreamNonBlocking));
@@ -778,15 +819,16 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
             const int64_t c0 = subgraph_offsets[s0], Bc = (int64_t)subgraph_offsets[cs[c + 1]] - c0;
             if (Bc > 0) {
                 WM_CUDA_TRY(cudaMemcpyAsync(dlen + c0, lengths + c0, (size_t)Bc * 4, H2D, cp));
-                if (T_max > 0) {
-                    WM_CUDA_TRY(cudaMemcpyAsync(dids + c0 * T_max, action_ids + c0 * T_max, (size_t)Bc * T_max * 4, H2D, cp));
-                    WM_CUDA_TRY(cudaMemcpyAsync(dpar + c0 * T_max * m.P, action_params + c0 * T_max * m.P,
-                                                (size_t)Bc * T_max * m.P * 4, H2D, cp));
-                }
+                const int rc0 = copy_actions(c0, Bc, cp);
+                if (rc0 != WM_OK) return rc0;
             }
             WM_CUDA_TRY(cudaEventRecord(ctx->hev_copy[c], cp));
             cudaStream_t ks = ctx->hs_k[c & 1];
             WM_CUDA_TRY(cudaStreamWaitEvent(ks, ctx->hev_copy[c], 0));
+            {
+                const int rc0 = widen(c0, Bc, ks);
+                if (rc0 != WM_OK) return rc0;
+            }
             if (Bc > 0) {
                 const int rc = wm_rollout_score(ctx, dz0 + (size_t)s0 * m.d, dids + c0 * T_max, dpar + c0 * T_max * m.P,
                                                 dlen + c0, dhw + (size_t)s0 * m.H, dsc + c0, dreb + reb_at[c], Bc, Sc, T_max, ks);
@@ -814,9 +856,10 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
     }
     WM_CUDA_TRY(cudaMemcpyAsync(dz0, init_states, (size_t)S * m.d * 4, H2D, st));
     if (m.H) WM_CUDA_TRY(cudaMemcpyAsync(dhw, hw_feats, (size_t)S * m.H * 4, H2D, st));
-    if (B && T_max) {
-        WM_CUDA_TRY(cudaMemcpyAsync(dids, action_ids, (size_t)B * T_max * 4, H2D, st));
-        WM_CUDA_TRY(cudaMemcpyAsync(dpar, action_params, (size_t)B * T_max * m.P * 4, H2D, st));
+    {
+        int rc0 = copy_actions(0, B, st);
+        if (rc0 == WM_OK) rc0 = widen(0, B, st);
+        if (rc0 != WM_OK) return rc0;
     }
     if (B) WM_CUDA_TRY(cudaMemcpyAsync(dlen, lengths, (size_t)B * 4, H2D, st));
     WM_CUDA_TRY(cudaMemcpyAsync(doff, subgraph_offsets, (size_t)(S + 1) * 4, H2D, st));
@@ -834,6 +877,26 @@ int wm_launch_empty(void* cuda_stream) {
     wm_empty_kernel<<<1, 32, 0, static_cast<cudaStream_t>(cuda_stream)>>>();
     WM_CUDA_TRY(cudaGetLastError());
     return WM_OK;
+}
+
+int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* action_ids,
+                       const int32_t* action_params, const int32_t* lengths, const float* hw_feats,
+                       const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
+                       float* scores_out, int32_t* idx_out, void* cuda_stream) {
+    return score_topk_host_impl(ctx, init_states, action_ids, action_params, 4, 4, lengths, hw_feats, subgraph_offsets, B, S,
+                                T_max, k, scores_out, idx_out, cuda_stream);
+}
+
+int wm_score_topk_host_compact(wm_ctx* ctx, const float* init_states, const uint8_t* action_ids,
+                               const uint16_t* action_params, const int32_t* lengths, const float* hw_feats,
+                               const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
+                               float* scores_out, int32_t* idx_out, void* cuda_stream) {
+    if (ctx && ctx->m.n_types > 256) {
+        set_error("wm_score_topk_host_compact: uint8 type ids need n_types <= 256");
+        return WM_ERR_UNSUPPORTED;
+    }
+    return score_topk_host_impl(ctx, init_states, action_ids, action_params, 1, 2, lengths, hw_feats, subgraph_offsets, B, S,
+                                T_max, k, scores_out, idx_out, cuda_stream);
 }
 
 int64_t wm_launch_count(const wm_ctx* ctx) {

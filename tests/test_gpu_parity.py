@@ -373,6 +373,17 @@ def test_host_entry_matches_device_entry(wm, n, S, per):
                           h(b.hw_feats), h(b.subgraph_offsets), cfg.k, sc, ix)
     np.testing.assert_array_equal(sc.numpy().view(np.uint32), y.view(np.uint32))
     np.testing.assert_array_equal(ix.numpy(), idx)
+    # the compact entry (uint8 type ids, uint16 parameters; padding positions hold other garbage): same bits
+    valid = np.arange(b.T_max)[None, :] < b.lengths[:, None]
+    ids8 = np.where(valid, b.action_ids, 255).astype(np.uint8)
+    par16 = np.where(valid[:, :, None], b.action_params, 65535).astype(np.uint16)
+    sc2 = torch.empty(b.B, dtype=torch.float32).pin_memory()
+    ix2 = torch.empty((b.S, cfg.k), dtype=torch.int32).pin_memory()
+    wm.wm_score_topk_host_compact(ctx, h(b.init_states), h(ids8), torch.from_numpy(par16.view(np.int16)).pin_memory(), h(b.lengths),
+                                  h(b.hw_feats), h(b.subgraph_offsets), cfg.k, sc2, ix2)
+    assert wm.wm_check(ctx) == 0
+    np.testing.assert_array_equal(sc2.numpy().view(np.uint32), y.view(np.uint32))
+    np.testing.assert_array_equal(ix2.numpy(), idx)
     wm.wm_free(ctx)
 
 
