@@ -58,6 +58,8 @@ extern "C" {
 #define WM_FAULT_TYPE   2u      /* an action type id at a valid position was outside [0, n_types) (clamped)   */
 #define WM_FAULT_PARAM  4u      /* an action parameter at a valid position was < 1 (treated as 1)             */
 #define WM_FAULT_INDEX  8u      /* wm_rollout_score_from: a bank_index was outside [0, n_bank) (clamped)      */
+#define WM_FAULT_RANGE  16u     /* tcgen05 kernels: an initial latent (init_states / bank row) had |value| > 65504, */
+                                /* the largest fp16 MMA operand; it was clamped (the fp32 kernel has no such limit) */
 
 /* values of wm_info.kind / dtype / embed (the weight-file header fields) */
 #define WM_KIND_MLP     0
@@ -129,7 +131,9 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
  *   G (forest):   Tf[n_trees, 2^depth-1] feature indices (stored as fp32), Tt[n_trees, 2^depth-1] thresholds,
  *                 Tv[n_trees, 2^depth] leaf values, Tb[1] base score
  * With dtype = bf16 every stored value is already bf16-representable (BASELINE.json cfg 2-5: "bf16 weights with
- * fp32 accumulate"); the tcgen05 kernels encode them exactly as fp16 operands (activations rounded to fp16), accumulate
+ * fp32 accumulate"); the tcgen05 kernels encode them as fp16 operands — exact for 2^-14 <= |w| <= 65504 (smaller magnitudes
+ * land on the fp16 subnormal grid, absolute change <= 3e-8; a larger one sends the model to the fp32 kernel) — with
+ * activations rounded to fp16, accumulate
  * in fp32 and keep the latent in fp32 (S14).
  * Errors: WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_UNSUPPORTED, WM_ERR_CUDA.  Synchronous. */
 int wm_load_weights(const char* path, int device, wm_ctx** ctx_out);

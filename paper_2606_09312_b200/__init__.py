@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libwm.so")
 
 WM_OK, WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_CUDA, WM_ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5
 WM_MAX_T, WM_MAX_K = 256, 1024
-WM_FAULT_LEN, WM_FAULT_TYPE, WM_FAULT_PARAM, WM_FAULT_INDEX = 1, 2, 4, 8
+WM_FAULT_LEN, WM_FAULT_TYPE, WM_FAULT_PARAM, WM_FAULT_INDEX, WM_FAULT_RANGE = 1, 2, 4, 8, 16
 WM_OPT_PATH, WM_OPT_SORT, WM_OPT_TIMING, WM_OPT_PAIR = 1, 2, 3, 4
 PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 

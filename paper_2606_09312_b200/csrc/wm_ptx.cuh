@@ -203,6 +203,13 @@ __device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
     return r;
 }
 
+// Activations enter the MMAs as fp16 with a SATURATING convert, so a caller-supplied initial latent beyond the fp16 range
+// would be silently clamped to 65504: the z_0 loads of the tcgen05 kernels report it (WM_FAULT_RANGE).  Later latents cannot
+// leave the range by themselves (LayerNorm / L2 normalisation / the GRU's convex blend bound them by the weights).
+__device__ __forceinline__ void range_check(const float4& f, uint32_t* fault) {
+    if (fmaxf(fmaxf(fabsf(f.x), fabsf(f.y)), fmaxf(fabsf(f.z), fabsf(f.w))) > 65504.0f) atomicOr(fault, WM_FAULT_RANGE);
+}
+
 // GELU, tanh form (hardware tanh.approx): |gelu_tanh - gelu_erf| <= 5e-4 abs, below the bf16 rounding of the
 // hidden activations it feeds (DESIGN.md §3 S5).  (A quintic inner polynomial fitted to the erf form, max deviation
 // 2.6e-5, was measured: no change in score error, which is dominated by operand rounding, and 4 % slower.)

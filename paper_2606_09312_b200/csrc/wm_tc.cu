@@ -475,6 +475,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tc_kernel(const Params p) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const float4 f = __ldg(src + i);
+                        range_check(f, p.a.fault);
                         v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
                         v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
                     }
@@ -984,7 +985,7 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const bool prefix_call = a.start || a.init_index || a.latents_out;   // wm_rollout_latents / wm_rollout_score_from
     // the prefix-reuse calls are built into wm_tc_kernel only (the other models take the fp32 kernel for them); the
     // TransH kernel has the latents-out piece (wm_rollout_latents; the rollout half of a forest-ranker model)
-    const bool ext_ok = m.tc_ok == 1 || (m.tc_ok == 4 && a.latents_out && !a.scores_out && !a.start && !a.init_index);
+    const bool ext_ok = m.tc_ok == 1 || m.tc_ok == 2 || (m.tc_ok == 4 && a.latents_out && !a.scores_out && !a.start && !a.init_index);
     if (prefix_call && !ext_ok && ctx->opt_path != 2) return launch_generic(ctx, a, st);
     if (!m.tc_ok || a.T_max > 255 || !aligned || (prefix_call && !ext_ok)) {
         if (ctx->opt_path == 2) {

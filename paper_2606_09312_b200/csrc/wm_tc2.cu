@@ -117,6 +117,10 @@ __device__ __forceinline__ int tile_of(int it, int pair, int np, int n_tiles) {
     return idx < n_tiles ? idx : -1;
 }
 
+// PHI = WM_PHI_MEAN | WM_PHI_STRUCT (what the action warps write into the phi K-blocks at the end of a tile); EXT = the
+// prefix-latent-reuse calls (wm_rollout_latents / wm_rollout_score_from: per-candidate start and initial-latent row,
+// latents stored), compiled out of the literal path — as in wm_tcp_kernel.
+template <int PHI, bool EXT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -171,6 +175,8 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(smem + L.tmem_slot);
     const uint32_t T_Z = tmem_base;                 // fp32 latent / GEMM2 accumulators: two 128-column N tiles
     const uint32_t T_D1 = tmem_base + 256;          // two 128-column GEMM1 accumulators (256 hidden units each)
+    // EXT calls that store latents and rank nothing skip the scorer in every role
+    const bool rank_it = !EXT || p.a.scores_out != nullptr;
 
     if (warp == PROD_WARP) {
         // =============================================================== tile schedule + TMA producer
@@ -184,7 +190,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int r = lane; r < TMP; r += 32) {
                     int cand, len, seg;
                     row_meta(p.a, (int64_t)tile * TMP + r, cand, len, seg, rank == 0);
-                    nsteps = max(nsteps, len);
+                    nsteps = max(nsteps, EXT ? len - row_start(p.a, cand, len) : len);
                 }
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) nsteps = max(nsteps, __shfl_xor_sync(0xffffffffu, nsteps, o));
@@ -197,7 +203,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             if (tile < 0) break;
             if (lane == 0) {
-                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + sc_stages(PKB);
+                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + (rank_it ? sc_stages(PKB) : 0);
                 int src = 0;
                 for (int i = 0; i < total; ++i) {
                     if (i == roll_total) src = ROLL_STAGES;
@@ -348,6 +354,11 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     gemm2(i - 1);
                 }
             }
+            if (!rank_it) {   // nothing to rank: only take the terminal latent's ZREADY so the phase count stays in step
+                mbar_wait_warp(bar(B_ZREADY), n_z & 1);
+                ++n_z;
+                continue;
+            }
             // ---- scorer layer 1: four 256-column chunks of gelu(Ws0 [z_T; phi; hw] + bs0).  Chunks 0, 1 land in the
             // hidden buffers; chunks 2, 3 are written over A1's z K-blocks once every layer-1 MMA has completed.
 #pragma unroll 1
@@ -466,18 +477,22 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (tile < 0) break;
             int cand, len, seg;
             row_meta(p.a, (int64_t)tile * TMP + TMR * (int)rank + row, cand, len, seg, false);
+            // prefix-latent reuse: the rollout covers positions [st, len) and starts from the row init_index names
+            const int st = EXT ? row_start(p.a, cand, len) : 0, rem = len - st;
+            const size_t zrow = EXT ? row_init(p.a, cand, seg) : (size_t)seg;
 
-            // ---- z_0 (the task's initial latent)
+            // ---- z_0 (the task's initial latent; or the banked latent after the first st steps)
 #pragma unroll 1
             for (int jh = 0; jh < 4; ++jh) {
                 const int j = jh >> 1, half = jh & 1;
                 const int col0 = 256 * j + 64 * part + 32 * half;
                 uint32_t v[32];
                 if (cand >= 0) {
-                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + col0);
+                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + zrow * D + col0);
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const float4 f = __ldg(src + i);
+                        range_check(f, p.a.fault);
                         v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
                         v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
                     }
@@ -530,7 +545,14 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 const float mean = s1 * inv_d;
                 const float var = fmaxf(s2 * inv_d - mean * mean, 0.0f);
                 const float rstd = rsqrtf(var + p.ln_eps);
-                const bool live = t < len;     // masked steps leave the state unchanged
+                const bool live = t < rem;     // masked steps leave the state unchanged
+                float4* lat = nullptr;     // wm_rollout_latents: z after this step (or only the terminal one: [B, d])
+                if (EXT && p.a.latents_out && live) {
+                    if (!p.a.latents_terminal)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + ((size_t)cand * p.a.T_max + st + t) * D);
+                    else if (st + t == len - 1)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + (size_t)cand * D);
+                }
 #pragma unroll 1
                 for (int jh = 0; jh < 4; ++jh) {
                     const int j = jh >> 1, half = jh & 1;
@@ -557,11 +579,18 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     // frozen rows: the fp16 copy (GEMM1 operand, scorer input) keeps the terminal latent; their
                     // fp32 master is never read again
                     put_z(j, half, v, live);
+                    if (EXT && lat) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+                            lat[(col0 >> 2) + i] = make_float4(__uint_as_float(v[4 * i]), __uint_as_float(v[4 * i + 1]),
+                                                               __uint_as_float(v[4 * i + 2]), __uint_as_float(v[4 * i + 3]));
+                    }
                 }
                 publish(r_zready, true);
                 WM_TRACE(52);
             }
 
+            if (!rank_it) continue;
             // ---- scorer layer 1 -> h1 (fp16): chunks 0, 1 into the hidden buffers ...
             gelu_to_h(0);
             gelu_to_h(1);
@@ -599,7 +628,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             s_red[part * TMR + row] = make_float2(acc, 0.0f);
             named_bar_sync(1 + rh, 128);
-            if (part == 0 && cand >= 0)
+            if (part == 0 && cand >= 0 && (!EXT || p.a.scores_out))
                 p.a.scores_out[cand] = (s_red[row].x + s_red[TMR + row].x) + (s_red[2 * TMR + row].x + s_red[3 * TMR + row].x) +
                                        __ldg(p.bs2);
             named_bar_sync(1 + rh, 128);   // s_red is reused by the next tile's first LayerNorm
@@ -642,9 +671,45 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 row_meta(p.a, (int64_t)tile * TMP + TMR * (int)rank + row, cand, len, seg, false);
                 for (int c = 0; c < NT; ++c) s_cnt[row * NT + c] = 0;
             }
-            float slp[MAX_P];
+            float slp[MAX_P], smx[MAX_P];    // per parameter slot: running sum and (WM_PHI_STRUCT) maximum of log2 p
 #pragma unroll
-            for (int j = 0; j < MAX_P; ++j) slp[j] = 0.0f;
+            for (int j = 0; j < MAX_P; ++j) slp[j] = smx[j] = 0.0f;
+            // one action of this row: type id (clamped), log2 of its parameters, phi statistics
+            auto take = [&](int pos, float (&lp)[MAX_P]) -> int {
+                int id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos);
+                if (id < 0 || id >= NT) {
+                    atomicOr(p.a.fault, WM_FAULT_TYPE);
+                    id = id < 0 ? 0 : NT - 1;
+                }
+                const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P;
+#pragma unroll
+                for (int j = 0; j < MAX_P; ++j) {
+                    if (j < P) {
+                        int prm = __ldg(pp + j);
+                        if (prm < 1) {
+                            atomicOr(p.a.fault, WM_FAULT_PARAM);
+                            prm = 1;
+                        }
+                        lp[j] = log2f((float)prm);
+                        slp[j] += lp[j];
+                        if (PHI == WM_PHI_STRUCT) smx[j] = fmaxf(smx[j], lp[j]);
+                    }
+                }
+                s_cnt[row * NT + id] += 1;
+                return id;
+            };
+            // prefix-latent reuse: positions [0, st) only feed phi; scanned in position order BEFORE the first rollout step
+            // (the running sums then see the positions in the literal call's order: bit-identical scores)
+            const int st = (EXT && row_lane) ? row_start(p.a, cand, len) : 0;
+            if (EXT && p.a.start) {
+                for (int pos = 0; pos < st; ++pos) {
+                    float lp[MAX_P];
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
+                    take(pos, lp);
+                }
+                __syncwarp();
+            }
             int prev_id = -1;
 
             for (int t = 0; t < nsteps; ++t) {
@@ -653,27 +718,7 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 float lp[MAX_P];
 #pragma unroll
                 for (int j = 0; j < MAX_P; ++j) lp[j] = 0.0f;
-                if (row_lane && t < len) {
-                    id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
-                    if (id < 0 || id >= NT) {
-                        atomicOr(p.a.fault, WM_FAULT_TYPE);
-                        id = id < 0 ? 0 : NT - 1;
-                    }
-                    const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
-#pragma unroll
-                    for (int j = 0; j < MAX_P; ++j) {
-                        if (j < P) {
-                            int prm = __ldg(pp + j);
-                            if (prm < 1) {
-                                atomicOr(p.a.fault, WM_FAULT_PARAM);
-                                prm = 1;
-                            }
-                            lp[j] = log2f((float)prm);
-                            slp[j] += lp[j];
-                        }
-                    }
-                    s_cnt[row * NT + id] += 1;
-                }
+                if (row_lane && st + t < len) id = take(st + t, lp);
                 // store only once GEMM1 of the previous step (or the previous tile's scorer) no longer reads K-blocks 8 ..
                 if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
                 ++n_w;
@@ -695,9 +740,12 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 if (lane == 0) mbar_arrive_remote(r_aready);
             }
 
-            // ---- the phi features (K-blocks 8 ..) of the scorer's A operand: phi = mean_t a_t is LINEAR in
-            // psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) | 1 (len > 0)]; the host folds E, W_p and b_p into scorer
-            // layer 1's phi weights (tc2_prepare); a constant-1 column after psi carries scorer layer 1's bias
+            // ---- the phi features (K-blocks 8 ..) of the scorer's A operand, followed by a constant-1 column that carries
+            // scorer layer 1's bias:
+            //   WM_PHI_MEAN    phi = mean_t a_t is LINEAR in psi = [count_c / len (NT) | sum_t log2 p_tj / len (P) | 1 (len > 0)];
+            //                  the host folds E, W_p and b_p into scorer layer 1's phi weights (tc2_prepare)
+            //   WM_PHI_STRUCT  phi = [count_c (NT) | len | sum_j (P) | mean_j (P) | max_j (P)]   (S25)
+            if (!rank_it) continue;
             if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
             clear_row();
@@ -705,16 +753,29 @@ wm_tc2_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (row_lane) {
                 auto putf = [&](int c, float v) { put(c, pack_f16(v, 0.0f)); };
                 const float inv = len > 0 ? 1.0f / (float)len : 0.0f;
-                for (int c = 0; c < NT; ++c) putf(c, (float)s_cnt[row * NT + c] * inv);
+                if (PHI == WM_PHI_STRUCT) {
+                    for (int c = 0; c < NT; ++c) putf(c, (float)s_cnt[row * NT + c]);
+                    putf(NT, (float)len);
 #pragma unroll
-                for (int j = 0; j < MAX_P; ++j)
-                    if (j < P) putf(NT + j, slp[j] * inv);
-                putf(NT + P, len > 0 ? 1.0f : 0.0f);
-                put(NT + P + 1, 0x3C00u);
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) {
+                            putf(NT + 1 + j, slp[j]);
+                            putf(NT + 1 + P + j, slp[j] * inv);
+                            putf(NT + 1 + 2 * P + j, smx[j]);
+                        }
+                    put(NT + 1 + 3 * P, 0x3C00u);
+                } else {
+                    for (int c = 0; c < NT; ++c) putf(c, (float)s_cnt[row * NT + c] * inv);
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) putf(NT + j, slp[j] * inv);
+                    putf(NT + P, len > 0 ? 1.0f : 0.0f);
+                    put(NT + P + 1, 0x3C00u);
+                }
                 // hardware features of this row -> the hw operand tile (columns >= H stay zero)
                 for (int ch = 0; ch < p.H / 8; ++ch) {
                     uint4 o = make_uint4(0u, 0u, 0u, 0u);
-                    if (cand >= 0) {
+                    if (cand >= 0 && (!EXT || p.a.hw_feats)) {
                         const float4* src = reinterpret_cast<const float4*>(p.a.hw_feats + (size_t)seg * p.H + 8 * ch);
                         const float4 f0 = __ldg(src), f1 = __ldg(src + 1);
                         o.x = pack_f16(f0.x, f0.y); o.y = pack_f16(f0.z, f0.w);
@@ -777,7 +838,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 }  // namespace
 
 bool tc2_model_ok(const Model& m) {
-    return m.kind == WM_KIND_MLP_LN && m.phi_kind == WM_PHI_MEAN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc2::D &&
+    return m.kind == WM_KIND_MLP_LN && m.phi_kind <= WM_PHI_STRUCT && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tc2::D &&
            m.d_a == tc2::DA && m.hidden >= 512 && m.hidden <= tc2::MAX_HID && m.hidden % 256 == 0 && m.n_lin == 3 &&
            m.sdim[1] == tc2::SW && m.sdim[2] == tc2::SW && m.H >= 8 && m.H <= tc2::MAX_H && m.H % 8 == 0 &&
            m.n_types <= tc2::MAX_TYPES && m.P <= tc2::MAX_P;
@@ -796,7 +857,7 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     };
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1"), &E = get("E");
     const std::vector<float>&b1 = get("b1"), &bs0 = get("bs0"), &Wp = get("W_p"), &bpv = get("b_p");
-    const int hid = m.hidden, NC = hid / 256, K1 = tc2::D + tc2::DA, K0 = K1 + m.H, NT = m.n_types, P = m.P;
+    const int hid = m.hidden, NC = hid / 256, K1 = tc2::D + tc2::DA, K0 = tc2::D + m.phi_dim + m.H, NT = m.n_types, P = m.P;
     // ---- GEMM1's a-columns folded onto the action features f = [onehot(id) (NT) | log2 p_j (P) | 1]:
     //      W1[:, d:] (E[id] + W_p lp + b_p) + b1  =  (W1a E^T)[:, id] + (W1a W_p) lp + (W1a b_p + b1)
     const int NF = NT + P + 1, AKB = (NF + 63) / 64;
@@ -820,11 +881,17 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     }
     // ---- scorer layer 1's phi columns folded onto psi = [count_c / len | sum log2 p_j / len | 1 (len > 0)] (see the action
     //      warps): Ws0_phi E^T, Ws0_phi W_p, Ws0_phi b_p, summed in double; then a constant-1 column that carries bs0
-    const int NPSI = NT + P + 2, PKB = (NPSI + 63) / 64;
+    const bool pstruct = m.phi_kind == WM_PHI_STRUCT;
+    const int NPSI = (pstruct ? NT + 1 + 3 * P : NT + P + 1) + 1, PKB = (NPSI + 63) / 64;
     std::vector<float> Wphi((size_t)tc2::SW * 64 * PKB, 0.0f);
     for (int n = 0; n < tc2::SW; ++n) {
         const float* wr = &Ws0[(size_t)n * K0 + tc2::D];
         float* out = &Wphi[(size_t)n * 64 * PKB];
+        if (pstruct) {           // the structured statistics enter as they are (S25)
+            for (int c = 0; c < m.phi_dim; ++c) out[c] = wr[c];
+            out[NPSI - 1] = bs0[n];
+            continue;
+        }
         for (int c = 0; c < NT; ++c) {
             double acc = 0.0;
             for (int k = 0; k < tc2::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tc2::DA + k];
@@ -860,7 +927,7 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     }
     for (int c = 0; c < 4; ++c) {     // scorer layer 1: phi features (PKB), hw (1, zero-padded to 64 columns), z (8)
         for (int k = 0; k < PKB; ++k) ok &= append_pair_tile(blob, Wphi, 64 * PKB, c * 256, k * 64, 64);
-        ok &= append_pair_tile(blob, Ws0, K0, c * 256, K1, m.H);
+        ok &= append_pair_tile(blob, Ws0, K0, c * 256, tc2::D + m.phi_dim, m.H);
         for (int k = 0; k < 8; ++k) ok &= append_pair_tile(blob, Ws0, K0, c * 256, k * 64, 64);
     }
     for (int round = 0; round < 2; ++round)   // scorer layer 2: two rounds of two N tiles over all 16 K-blocks
@@ -904,7 +971,13 @@ int tc2_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     m.tc_blob_bytes = blob.size() * 2;
     m.tcp_akb = AKB;      // (shared fields: a model has either the d = 256 pair kernel or this one)
     m.tcp_pkb = PKB;
-    WM_CUDA_TRY(cudaFuncSetAttribute(tc2::wm_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    if (pstruct) {
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc2::wm_tc2_kernel<WM_PHI_STRUCT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc2::wm_tc2_kernel<WM_PHI_STRUCT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    } else {
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc2::wm_tc2_kernel<WM_PHI_MEAN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+        WM_CUDA_TRY(cudaFuncSetAttribute(tc2::wm_tc2_kernel<WM_PHI_MEAN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    }
     m.tc_ok = 2;
     return WM_OK;
 }
@@ -927,7 +1000,14 @@ int launch_tc2(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const tc2::SmemLayout L = tc2::smem_layout(m.n_types, m.hidden, p.hw_ksteps);
     const int max_pairs = ctx->n_sms / 2;
     const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
-    tc2::wm_tc2_kernel<<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
+    const bool prefix_call = a.start || a.init_index || a.latents_out;
+    if (m.phi_kind == WM_PHI_STRUCT) {
+        if (prefix_call) tc2::wm_tc2_kernel<WM_PHI_STRUCT, true><<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
+        else tc2::wm_tc2_kernel<WM_PHI_STRUCT, false><<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
+    } else {
+        if (prefix_call) tc2::wm_tc2_kernel<WM_PHI_MEAN, true><<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
+        else tc2::wm_tc2_kernel<WM_PHI_MEAN, false><<<2 * pairs, tc2::THREADS, L.total, st>>>(p, tm);
+    }
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
     trace::dump(p.prof, st);

@@ -478,6 +478,7 @@ __global__ void __launch_bounds__(THREADS, 1) wm_tct_kernel(const Params p) {
 #pragma unroll
                         for (int i = 0; i < 8; ++i) {
                             const float4 f = __ldg(src + i);
+                        range_check(f, p.a.fault);
                             v[4 * i + 0] = __float_as_uint(f.x); v[4 * i + 1] = __float_as_uint(f.y);
                             v[4 * i + 2] = __float_as_uint(f.z); v[4 * i + 3] = __float_as_uint(f.w);
                         }

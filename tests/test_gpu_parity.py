@@ -110,6 +110,23 @@ def test_many_action_types_two_feature_kblocks(wm, phi):
     assert seen == {0, 5}, seen
 
 
+def test_struct_phi_on_the_d512_pair_kernel(wm):
+    """NEXT row f2 (pooled structured phi, S25) on a d = 512 model: wm_tc2_kernel<WM_PHI_STRUCT> (74 phi features + the
+    constant column: two phi K-blocks), against the oracle and the fp32 kernel; several tiles and a ragged tail."""
+    cfg = replace(gen.get_config(3).scaled(S=3, per_subgraph=139), phi_kind=1, name="cfg3_structphi")
+    w = gen.make_weights(cfg)
+    b = gen.make_inputs(cfg)
+    ref = oracle_scores(cfg, w, b)
+    for path in (wm.PATH_FP32, wm.PATH_TCGEN05):
+        ctx = wm.wm_load_weights(weight_file(cfg, w))
+        wm.wm_set_option(ctx, wm.WM_OPT_PATH, path)
+        info = wm.wm_get_info(ctx)
+        assert info.phi_kind == 1 and (path == wm.PATH_FP32 or info.tc_variant == 2)
+        y = gpu_scores(ctx, b)
+        wm.wm_free(ctx)
+        assert oracle.score_error(y, ref, b.subgraph_offsets) <= (2e-3 if path == wm.PATH_FP32 else 2e-2), path
+
+
 def _edge_batch(cfg, lengths=None, S=None, per=None):
     if cfg.prefix_children:      # cfg 4: its MODEL (hidden 768: six GEMM1 chunks) on free-form batches with mixed lengths
         cfg = replace(cfg, prefix_children=0, len_dist="uniform", len_lo=0)
@@ -258,6 +275,26 @@ def test_fault_word(wm):
     assert wm.wm_check(ctx) == 0
     assert torch.isfinite(out).all()
     wm.wm_free(ctx)
+
+
+@pytest.mark.parametrize("n", [2, 3, 5, 7])
+def test_fault_range_on_initial_latent(wm, n):
+    """An initial latent beyond the fp16 operand range is clamped by the tcgen05 kernels' saturating convert: the call
+    reports WM_FAULT_RANGE (and stays finite); the fp32 kernel has no such limit and reports nothing."""
+    cfg = gen.get_config(n).scaled(S=2, per_subgraph=40)
+    b = gen.make_inputs(cfg)
+    b.init_states = b.init_states.copy()
+    b.init_states[1, 3] = 1.0e5
+    for path, want in ((wm.PATH_TCGEN05, wm.WM_FAULT_RANGE), (wm.PATH_FP32, 0)):
+        import torch
+        ctx = _ctx(wm, cfg, path)
+        dv = to_device(b)
+        out = torch.empty(b.B, dtype=torch.float32, device="cuda:0")
+        wm.wm_rollout_score(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"], dv["hw_feats"], out,
+                            dv["subgraph_offsets"])
+        assert wm.wm_check(ctx) == want, (n, path)
+        assert torch.isfinite(out).all()
+        wm.wm_free(ctx)
 
 
 def test_two_streams_share_one_ctx(wm):
@@ -540,7 +577,7 @@ def test_struct_phi_feature_readout(wm, n):
             np.testing.assert_array_equal(y, b.hw_feats[seg, 0])
 
 
-PREFIX_TC_VARIANTS = (1, 5)       # (the TransH kernel, variant 4, takes wm_rollout_latents only)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
+PREFIX_TC_VARIANTS = (1, 2, 5)       # (the TransH kernel, variant 4, takes wm_rollout_latents only)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
 
 
 def _prefix_case(n, S, per):
@@ -574,7 +611,7 @@ def test_rollout_latents_match_oracle(wm, n):
         out = torch.full((b.B, cfg.T_max, cfg.d), -777.0, dtype=torch.float32, device="cuda:0")
         call = lambda: wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"],
                                              dv["lengths"], out, dv["subgraph_offsets"])
-        if _prefix_unsupported(wm, ctx, path, call, variants=(1, 4, 5)):
+        if _prefix_unsupported(wm, ctx, path, call, variants=(1, 2, 4, 5)):
             continue
         call()
         assert wm.wm_check(ctx) == 0
