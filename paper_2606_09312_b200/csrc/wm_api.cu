@@ -404,7 +404,7 @@ int wm_get_info(const wm_ctx* ctx, wm_info* o) {
     for (int i = 0; i < 6; ++i) o->scorer_widths[i] = (i + 1 < m.n_lin) ? m.sdim[i + 1] : 0;
     o->ln_eps = m.ln_eps;
     o->path = tc_supported(ctx) ? 2 : 1;
-    o->tc_variant = tc_supported(ctx) == 1 && m.tcp_ok && (ctx->opt_pair || !m.tc1_ok) ? 5 : tc_supported(ctx);
+    o->tc_variant = (tc_supported(ctx) == 1 || tc_supported(ctx) == 4) && m.tcp_ok && (ctx->opt_pair || !m.tc1_ok) ? 5 : tc_supported(ctx);
     o->phi_kind = m.phi_kind;
     o->ranker_kind = m.ranker_kind; o->n_trees = m.n_trees; o->tree_depth = m.tree_depth;
     return WM_OK;

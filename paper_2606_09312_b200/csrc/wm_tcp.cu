@@ -74,6 +74,7 @@ enum {
     B_D2FULL = B_HREADY + 2,       // MMA commit -> epilogue: GEMM2 of the step done
     B_ZREADY,                      // epilogue (both CTAs) -> leader MMA: z K-blocks 0 and 2 written (first half of every thread's columns)
     B_ZREADY2,                     // ... K-blocks 1 and 3 written, and the fp32 latent in TMEM
+    B_UFULL,                       // TransH step: MMA commit -> epilogue: u = W_w a of the next step is in the GEMM1 accumulators
     B_AFREE,                       // MMA commit -> action warps: a-part of A1 no longer read
     B_AREADY,                      // action warps (both CTAs) -> leader MMA: a-part written
     B_SFULL,                       // [2] schedule slot filled (CTA-local)
@@ -109,7 +110,7 @@ __host__ __device__ inline SmemLayout smem_layout(int n_types, int hw_ksteps, in
     L.b2 = o; o += D * 4;
     L.gamma = o; o += D * 4;
     L.beta = o; o += D * 4;
-    L.red = o; o += 4 * TM * 8;                        // [2 (LayerNorm parity)][2 column halves][128 rows] float2
+    L.red = o; o += 4 * TM * 16;                       // [2 (parity)][2 column halves][128 rows] float4 (LayerNorm uses .x, .y)
     L.bars = o; o += B_COUNT * 8;
     L.sched = o; o += 2 * 8;
     L.tmem_slot = o; o += 16;
@@ -135,6 +136,14 @@ __host__ __device__ inline int stage_boxes(int j, int nc, int akb, bool wide) {
     return (j >= 4 && j < 3 * nc - 2 && (j - 4) % 3 == 0) ? akb : 4;
 }
 __host__ __device__ inline int step_boxes(int nc, int akb) { return 2 * akb + 12 + (nc - 2) * (akb + 8) + 4; }
+// TransH step (STEP_TRANSH): three feature stages first — u = W_w a (N = 256: 2 akb boxes), the translation W_d a onto the
+// latent (2 akb), the feature K-blocks of chunks 0 and 1 (2 akb) — then z K-blocks of chunk 0, of chunk 1 (4 each), GEMM2
+// chunk 0 and the rest as above.
+__host__ __device__ inline int th_step_stages(int nc, bool wide) { return step_stages(nc, wide) + 2; }
+__host__ __device__ inline int th_stage_boxes(int j, int nc, int akb, bool wide) {
+    return j < 3 ? 2 * akb : stage_boxes(j - 2, nc, akb, wide);
+}
+__host__ __device__ inline int th_step_boxes(int nc, int akb) { return step_boxes(nc, akb) + 4 * akb; }
 // scorer: layer 1, per 128-column chunk: [phi features (pkb) + hw (1)], [z (4)]; layer 2, per chunk: two stages of 4
 __host__ __device__ inline int scorer_boxes(int pkb) { return 4 * (pkb + 1 + 4) + 4 * 8; }
 
@@ -153,9 +162,18 @@ __device__ __forceinline__ void mma_ts2(uint32_t d_tmem, uint32_t a_tmem, uint64
 // PHI / EXT as in wm_tc_kernel: PHI = WM_PHI_MEAN | WM_PHI_STRUCT (what the action warps write into the phi K-blocks);
 // EXT = the prefix-latent-reuse calls (per-candidate start and initial-latent row, latents stored), compiled out of
 // the literal path.
-template <int PHI, bool EXT>
+// STEP = STEP_MLP_LN: z' = LayerNorm(z + W2 gelu(W1 [z; a] + b1) + b2) (BASELINE.json cfg 2 / 4).
+// STEP = STEP_TRANSH (NEXT row f1, S24): u = W_w a; z_perp = z - (u.z) u / (|u|^2 + eps);
+//   x = z_perp + W_d a; v = x + W2 gelu(W1 [x; a] + b1) + b2; z' = v / sqrt(|v|^2 + eps).  On this skeleton: u = W_w a is one
+//   more N = 256 GEMM on the feature K-block into the (then free) GEMM1 accumulators; ONE boundary epilogue per step
+//   normalises the previous step's v (held in registers) and projects it for the next action; the translation W_d a (with b2
+//   on the constant feature column) is accumulated onto the latent by the tensor core, and GEMM1 consumes z_perp with
+//   W1a' = W1a + W1z W_d folded on the host, so x is never formed by a thread.
+constexpr int STEP_MLP_LN = 0, STEP_TRANSH = 1;
+template <int PHI, bool EXT, int STEP>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
+    constexpr bool TH = STEP == STEP_TRANSH;
     extern __shared__ __align__(1024) uint8_t smem[];
     const bool WIDE = p.akb == 1 && p.pkb == 1;
     const SmemLayout L = smem_layout(p.n_types, p.hw_ksteps, PHI, WIDE);
@@ -167,14 +185,15 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     float* s_b2 = reinterpret_cast<float*>(smem + L.b2);
     float* s_gamma = reinterpret_cast<float*>(smem + L.gamma);
     float* s_beta = reinterpret_cast<float*>(smem + L.beta);
-    float2* s_red = reinterpret_cast<float2*>(smem + L.red);                  // [2][2][128]
+    float4* s_red = reinterpret_cast<float4*>(smem + L.red);                  // [2][2][128]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
     const int NC = p.nc;
     const int AKB = p.akb, PKB = p.pkb;
-    const int ROLL_BOXES = step_boxes(NC, AKB), ROLL_STAGES = step_stages(NC, WIDE);
+    const int ROLL_BOXES = TH ? th_step_boxes(NC, AKB) : step_boxes(NC, AKB);
+    const int ROLL_STAGES = TH ? th_step_stages(NC, WIDE) : step_stages(NC, WIDE);
 
     // ---- one-time setup
     if (threadIdx.x == 0) {
@@ -188,6 +207,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         mbar_init(bar(B_D2FULL), 1);
         mbar_init(bar(B_ZREADY), 16);
         mbar_init(bar(B_ZREADY2), 16);
+        mbar_init(bar(B_UFULL), 1);
         mbar_init(bar(B_AFREE), 1);
         mbar_init(bar(B_AREADY), 8);
         fence_barrier_init();
@@ -196,8 +216,8 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     if (warp == ALLOC_WARP) tmem_alloc2(s_base + L.tmem_slot, 512);
     for (int i = threadIdx.x; i < D; i += THREADS) {
         s_b2[i] = __ldg(p.b2 + i);
-        s_gamma[i] = __ldg(p.gamma + i);
-        s_beta[i] = __ldg(p.beta + i) + __ldg(p.b2 + i);   // the latent is carried as u = z + b2 (see the epilogue)
+        s_gamma[i] = TH ? 1.0f : __ldg(p.gamma + i);
+        s_beta[i] = TH ? 0.0f : __ldg(p.beta + i) + __ldg(p.b2 + i);   // the latent is carried as u = z + b2 (see the epilogue)
     }
     {
         // the hw K-block is only ever written in its first columns: clear it once so unread bytes are not NaNs
@@ -261,7 +281,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int t = 0; t < nsteps; ++t) {
                     int box = 0;
                     for (int j = 0; j < ROLL_STAGES; ++j) {
-                        const int nb = stage_boxes(j, NC, AKB, WIDE);
+                        const int nb = TH ? th_stage_boxes(j, NC, AKB, WIDE) : stage_boxes(j, NC, AKB, WIDE);
                         issue(nb, box);
                         box += nb;
                     }
@@ -396,6 +416,21 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             advance();
         };
+        // TransH: one stage of N = 256 MMAs of the feature K-blocks (4 ..) against a [256 x 64 akb] weight tile (two boxes per
+        // K-block = this CTA's 128 weight rows) into the 256-column tile d: u = W_w' f (d = both GEMM1 accumulators, fresh) or
+        // the translation W_d' f accumulated onto the latent
+        auto stage_f256 = [&](uint32_t d, bool fresh) {
+            acquire_stage();
+            if (elect_one()) {
+                for (int k = 0; k < AKB; ++k)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        mma_ss2(d, desc_of(a_lo + (4 + k) * KBL + 2u * j), desc_of(b_lo + (uint32_t)(2 * k) * HBL + 2u * j), ID_N256,
+                                (fresh && k == 0 && j == 0) ? 0u : 1u);
+                mma_commit2(bar(B_EMPTY + stage));
+            }
+            advance();
+        };
         // stage: GEMM2 of hidden chunk buffer b (fp16 in TMEM: K-block 0 at +0, K-block 1 at +64 columns) x all 256
         // latent columns: two consecutive boxes are this CTA's 128 weight rows of one [256 x 64] B tile, 4 MMAs with N = 256
         auto stage_g2 = [&](int b) {
@@ -443,14 +478,25 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 WM_TRACE(1);
                 mbar_wait_warp(bar(B_AREADY), n_a & 1); ++n_a; tc_fence_after();
                 WM_TRACE(2);
-                stage_a01();
-                if (NC == 2) commit(B_AFREE);
-                WM_TRACE(3);
-                mbar_wait_warp(bar(B_ZREADY), n_z & 1); tc_fence_after();
-                WM_TRACE(4);
-                stage_za();
-                mbar_wait_warp(bar(B_ZREADY2), n_z & 1); ++n_z; tc_fence_after();
-                stage_zb();
+                if (TH) {
+                    stage_f256(TD1, true);                 // u = W_w a into both (free) GEMM1 accumulators
+                    commit(B_UFULL);
+                    mbar_wait_warp(bar(B_ZREADY2), n_z & 1); ++n_z; tc_fence_after();   // boundary done: z_perp written, u read
+                    stage_f256(TZ, false);                 // x = z_perp + W_d a (+ b2), accumulated onto the latent
+                    stage_a01();
+                    if (NC == 2) commit(B_AFREE);
+                    stage_z(0); commit(B_D1FULL + 0);
+                    stage_z(1); commit(B_D1FULL + 1);
+                } else {
+                    stage_a01();
+                    if (NC == 2) commit(B_AFREE);
+                    WM_TRACE(3);
+                    mbar_wait_warp(bar(B_ZREADY), n_z & 1); tc_fence_after();
+                    WM_TRACE(4);
+                    stage_za();
+                    mbar_wait_warp(bar(B_ZREADY2), n_z & 1); ++n_z; tc_fence_after();
+                    stage_zb();
+                }
                 pend[0] = pend[1] = true;
                 wait_h(0);
                 stage_g2(0);
@@ -476,7 +522,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 }
             }
             if (!rank_it) {   // nothing to rank: only take the terminal latent's ZREADY so the phase count stays in step
-                mbar_wait_warp(bar(B_ZREADY), n_z & 1);
+                if (!TH) mbar_wait_warp(bar(B_ZREADY), n_z & 1);
                 mbar_wait_warp(bar(B_ZREADY2), n_z & 1);
                 ++n_z;
                 continue;
@@ -491,7 +537,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 stage_a(b, PKB, true);
                 if (c == 3) commit(B_AFREE);
                 if (c == 0) {
-                    mbar_wait_warp(bar(B_ZREADY), n_z & 1);
+                    if (!TH) mbar_wait_warp(bar(B_ZREADY), n_z & 1);
                     mbar_wait_warp(bar(B_ZREADY2), n_z & 1);
                     ++n_z;
                     tc_fence_after();
@@ -525,7 +571,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint8_t* a1 = smem + L.a1;
         const uint32_t r_hready0 = mapa(bar(B_HREADY), 0), r_hready1 = mapa(bar(B_HREADY + 1), 0);
         const uint32_t r_zready = mapa(bar(B_ZREADY), 0), r_zready2 = mapa(bar(B_ZREADY2), 0);
-        uint32_t n_d1[2] = {0, 0}, n_d2 = 0;
+        uint32_t n_d1[2] = {0, 0}, n_d2 = 0, n_u = 0, n_b = 0;
         const float inv_d = 1.0f / (float)D;
         WM_TRACE_DECL(warp == 0 ? p.prof : nullptr, 2)
         // The latent is carried as u = z + b2, twice: fp32 in TMEM — GEMM2 accumulates W2 h onto it, so the accumulator IS
@@ -597,6 +643,112 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             const int st = EXT ? row_start(p.a, cand, len) : 0, rem = len - st;
             const size_t zrow = EXT ? row_init(p.a, cand, seg) : (size_t)seg;
 
+            if (TH) {
+            // ---- TransH: boundary t = 0 .. nsteps.  Boundary t normalises the result of step t - 1 (t = 0: takes z_0 as it
+            // is) and, when a step t follows, projects it onto the hyperplane of action t: ONE epilogue per step boundary.
+            constexpr float kEps = 1e-12f;
+#pragma unroll 1
+            for (int t = 0; t <= nsteps; ++t) {
+                const bool has_u = t < nsteps;
+                uint32_t v[128];
+                if (t > 0) {
+                    mbar_wait_inline(bar(B_D2FULL), n_d2 & 1);
+                    ++n_d2;
+                    tc_fence_after();
+#pragma unroll
+                    for (int p4 = 0; p4 < 4; ++p4)
+                        tmem_ld32(T_Z + lane_off + (uint32_t)(128 * hh + 32 * p4), reinterpret_cast<uint32_t(&)[32]>(v[32 * p4]));
+                } else {
+#pragma unroll
+                    for (int p4 = 0; p4 < 4; ++p4) {
+                        if (cand >= 0) {
+                            const float4* src = reinterpret_cast<const float4*>(p.a.init_states + zrow * D + 128 * hh + 32 * p4);
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) {
+                                const float4 f = __ldg(src + i);
+                                range_check(f, p.a.fault);
+                                v[32 * p4 + 4 * i + 0] = __float_as_uint(f.x); v[32 * p4 + 4 * i + 1] = __float_as_uint(f.y);
+                                v[32 * p4 + 4 * i + 2] = __float_as_uint(f.z); v[32 * p4 + 4 * i + 3] = __float_as_uint(f.w);
+                            }
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) v[32 * p4 + i] = 0u;
+                        }
+                    }
+                }
+                if (has_u) {
+                    mbar_wait_inline(bar(B_UFULL), n_u & 1);
+                    ++n_u;
+                    tc_fence_after();
+                }
+                tmem_ld_wait();
+                // pass 1: |v|^2, |u|^2, u.v over this thread's 128 columns (u streamed from the GEMM1 accumulators)
+                float2 svv = make_float2(0.0f, 0.0f), suu = make_float2(0.0f, 0.0f), suv = make_float2(0.0f, 0.0f);
+#pragma unroll
+                for (int i = 0; i < 64; ++i) {
+                    const float2 x = make_float2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+                    svv = __ffma2_rn(x, x, svv);
+                }
+                if (has_u) {
+#pragma unroll
+                    for (int p4 = 0; p4 < 4; ++p4) {
+                        uint32_t u[32];
+                        tmem_ld32(T_D1 + lane_off + (uint32_t)(128 * hh + 32 * p4), u);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) {
+                            const float2 uu = make_float2(__uint_as_float(u[2 * i]), __uint_as_float(u[2 * i + 1]));
+                            const float2 x = make_float2(__uint_as_float(v[32 * p4 + 2 * i]), __uint_as_float(v[32 * p4 + 2 * i + 1]));
+                            suu = __ffma2_rn(uu, uu, suu);
+                            suv = __ffma2_rn(uu, x, suv);
+                        }
+                    }
+                }
+                float4* red = s_red + (n_b & 1u) * 2 * TM;      // (parity slots as in the LayerNorm: one barrier per exchange)
+                ++n_b;
+                red[hh * TM + row] = make_float4(svv.x + svv.y, suu.x + suu.y, suv.x + suv.y, 0.0f);
+                named_bar_sync(1 + q, 64);
+                const float4 other = red[(hh ^ 1) * TM + row];
+                const float vv = svv.x + svv.y + other.x, uu2 = suu.x + suu.y + other.y, uv = suv.x + suv.y + other.z;
+                const float rn = t > 0 ? rsqrtf(vv + kEps) : 1.0f;        // z' = v / sqrt(|v|^2 + eps); boundary 0 keeps z_0
+                const bool live = t < rem;                                 // a step t follows for this row
+                const bool done_now = t == rem;                            // z' is this row's terminal latent
+                const float c = (has_u && live) ? uv * rn / (uu2 + kEps) : 0.0f;   // (w.z') w = (u.z') u / (|u|^2 + eps)
+                float4* lat = nullptr;     // wm_rollout_latents: z after step t - 1 (or only the terminal one: [B, d])
+                if (EXT && p.a.latents_out && t > 0 && t - 1 < rem) {
+                    if (!p.a.latents_terminal)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + ((size_t)cand * p.a.T_max + st + t - 1) * D);
+                    else if (done_now)
+                        lat = reinterpret_cast<float4*>(p.a.latents_out + (size_t)cand * D);
+                }
+                const float2 rn2 = make_float2(rn, rn), mc2 = make_float2(-c, -c);
+#pragma unroll
+                for (int p4 = 0; p4 < 4; ++p4) {
+                    const int col0 = 128 * hh + 32 * p4;
+                    uint32_t* vv32 = v + 32 * p4;
+                    uint32_t u[32];
+                    if (has_u) {
+                        tmem_ld32(T_D1 + lane_off + (uint32_t)col0, u);
+                        tmem_ld_wait();
+                    }
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        float2 x = __fmul2_rn(make_float2(__uint_as_float(vv32[2 * i]), __uint_as_float(vv32[2 * i + 1])), rn2);   // z'
+                        if (EXT && lat) reinterpret_cast<float2*>(lat)[(col0 >> 1) + i] = x;
+                        if (done_now) { vv32[2 * i] = __float_as_uint(x.x); vv32[2 * i + 1] = __float_as_uint(x.y); }
+                        if (has_u) x = __ffma2_rn(make_float2(__uint_as_float(u[2 * i]), __uint_as_float(u[2 * i + 1])), mc2, x);   // z_perp
+                        if (!done_now) { vv32[2 * i] = __float_as_uint(x.x); vv32[2 * i + 1] = __float_as_uint(x.y); }
+                    }
+                    // live rows: z_perp -> fp16 operand; a row that has just finished: its terminal z' (and it is frozen);
+                    // rows that finished earlier keep theirs.  The fp32 copy is written for every row (it stays bounded).
+                    if (live || done_now) z_to_smem(col0, vv32);
+                    tmem_st32(T_Z + lane_off + (uint32_t)col0, reinterpret_cast<const uint32_t(&)[32]>(v[32 * p4]));
+                }
+                publish(r_zready2, true);
+                if (has_u)
+                    for (int cc = 0; cc < NC; ++cc) gelu_chunk(cc & 1, T_D1 + 128u * (cc & 1) + 64u * hh);
+            }
+            } else {
             // ---- z_0 (the task's initial latent; or the banked latent after the first st steps)
 #pragma unroll 1
             for (int p4 = 0; p4 < 4; ++p4) {
@@ -655,11 +807,11 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 const float s1 = s1v.x + s1v.y, s2 = s2v.x + s2v.y;
                 // exchanged through the slot of this LayerNorm's parity: the partner reads the previous LayerNorm's value
                 // from the other slot, so no second barrier is needed before the next one writes
-                float2* red = s_red + (n_d2 & 1u) * 2 * TM;
-                red[hh * TM + row] = make_float2(s1, s2);
+                float4* red = s_red + (n_d2 & 1u) * 2 * TM;
+                red[hh * TM + row] = make_float4(s1, s2, 0.0f, 0.0f);
                 WM_TRACE(55);
                 named_bar_sync(1 + q, 64);
-                const float2 other = red[(hh ^ 1) * TM + row];
+                const float4 other = red[(hh ^ 1) * TM + row];
                 WM_TRACE(52);
                 const float mean = (s1 + other.x) * inv_d;
                 const float var = fmaxf((s2 + other.y) * inv_d - mean * mean, 0.0f);
@@ -708,6 +860,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 WM_TRACE(53);
             }
 
+            }
             if (!rank_it) continue;
             // ---- scorer layer 1 -> H1 (fp16) in TMEM columns [0,256)
             for (int c = 0; c < 4; ++c)
@@ -733,7 +886,7 @@ wm_tcp_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(b == 0 ? r_hready0 : r_hready1);
             }
-            s_red[hh * TM + row] = make_float2(part, 0.0f);
+            s_red[hh * TM + row] = make_float4(part, 0.0f, 0.0f, 0.0f);
             named_bar_sync(1 + q, 64);
             if (hh == 0 && cand >= 0 && (!EXT || p.a.scores_out)) p.a.scores_out[cand] = part + s_red[TM + row].x + __ldg(p.bs2);
             named_bar_sync(1 + q, 64);   // s_red is reused by the next tile's first LayerNorm
@@ -964,7 +1117,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 }  // namespace
 
 bool tcp_model_ok(const Model& m) {
-    return m.phi_kind <= WM_PHI_STRUCT && m.kind == WM_KIND_MLP_LN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tcp::D &&
+    return m.phi_kind <= WM_PHI_STRUCT && (m.kind == WM_KIND_MLP_LN || m.kind == WM_KIND_TRANSH) && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tcp::D &&
            m.d_a == tcp::DA && m.hidden >= 256 && m.hidden <= tcp::MAX_HID && m.hidden % 128 == 0 &&
            ((m.n_lin == 3 && m.sdim[1] == tcp::SW && m.sdim[2] == tcp::SW) || m.ranker_kind == WM_RANKER_FOREST) &&
            m.H >= 8 && m.H <= tcp::MAX_H && m.H % 8 == 0 && m.n_types <= tcp::MAX_TYPES && m.P <= tcp::MAX_P;
@@ -982,29 +1135,57 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     };
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &b1 = get("b1"), &E = get("E"), &Wp = get("W_p"), &bpv = get("b_p");
     const std::vector<float>& b2h = get("b2");
-    const bool forest = m.ranker_kind == WM_RANKER_FOREST;
+    const bool forest = m.ranker_kind == WM_RANKER_FOREST, transh = m.kind == WM_KIND_TRANSH;
     const int hid = m.hidden, NC = hid / 128, K1 = tcp::D + tcp::DA, NT = m.n_types, P = m.P;
-    // ---- GEMM1's a-columns folded onto the action features f = [onehot(id) (NT) | log2 p_j (P) | 1]:
-    //      W1[:, d:] (E[id] + W_p lp + b_p) + b1  =  (W1a E^T)[:, id] + (W1a W_p) lp + (W1a b_p + b1)
+    // ---- A matrix that multiplies the action embedding, folded onto the action features f = [onehot(id) (NT) | log2 p_j (P) | 1]:
+    //      M (E[id] + W_p lp + b_p) + bias  =  (M E^T)[:, id] + (M W_p) lp + (M b_p + bias); products summed in double
     const int NF = NT + P + 1, AKB = (NF + 63) / 64;
-    std::vector<float> W1f((size_t)hid * 64 * AKB, 0.0f);
-    for (int n = 0; n < hid; ++n) {
-        const float* wr = &W1[(size_t)n * K1 + tcp::D];
-        float* out = &W1f[(size_t)n * 64 * AKB];
-        for (int c = 0; c < NT; ++c) {
-            double acc = 0.0;
-            for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * E[(size_t)c * tcp::DA + k];
-            out[c] = (float)acc;
+    auto fold = [&](const double* M, int rows, const double* bias) {     // M [rows][d_a], row-major
+        std::vector<float> out((size_t)rows * 64 * AKB, 0.0f);
+        for (int n = 0; n < rows; ++n) {
+            const double* wr = M + (size_t)n * tcp::DA;
+            float* o = &out[(size_t)n * 64 * AKB];
+            for (int c = 0; c < NT; ++c) {
+                double acc = 0.0;
+                for (int k = 0; k < tcp::DA; ++k) acc += wr[k] * E[(size_t)c * tcp::DA + k];
+                o[c] = (float)acc;
+            }
+            for (int j = 0; j < P; ++j) {
+                double acc = 0.0;
+                for (int k = 0; k < tcp::DA; ++k) acc += wr[k] * Wp[(size_t)k * P + j];
+                o[NT + j] = (float)acc;
+            }
+            double acc = bias ? bias[n] : 0.0;
+            for (int k = 0; k < tcp::DA; ++k) acc += wr[k] * bpv[k];
+            o[NT + P] = (float)acc;
         }
-        for (int j = 0; j < P; ++j) {
-            double acc = 0.0;
-            for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * Wp[(size_t)k * P + j];
-            out[NT + j] = (float)acc;
+        return out;
+    };
+    // GEMM1's a-columns (+ b1 on the constant column).  MLP+LN: the z operand is u = z + b2, so W1z b2 comes off the bias.
+    // TransH: W1 [x ; a] with x = z_perp + W_d a  =  W1z z_perp + (W1a + W1z W_d) a: the translation is folded in as well.
+    std::vector<double> W1a((size_t)hid * tcp::DA), b1f(hid);
+    std::vector<float> W1f, Uf, Df;
+    {
+        const std::vector<float>* Wd = transh ? &get("W_d") : nullptr;
+        for (int n = 0; n < hid; ++n) {
+            for (int j = 0; j < tcp::DA; ++j) {
+                double acc = W1[(size_t)n * K1 + tcp::D + j];
+                if (transh)
+                    for (int k = 0; k < tcp::D; ++k) acc += (double)W1[(size_t)n * K1 + k] * (double)(*Wd)[(size_t)k * tcp::DA + j];
+                W1a[(size_t)n * tcp::DA + j] = acc;
+            }
+            double bb = b1[n];
+            if (!transh)
+                for (int k = 0; k < tcp::D; ++k) bb -= (double)W1[(size_t)n * K1 + k] * b2h[k];
+            b1f[n] = bb;
         }
-        double acc = b1[n];
-        for (int k = 0; k < tcp::DA; ++k) acc += (double)wr[k] * bpv[k];
-        for (int k = 0; k < tcp::D; ++k) acc -= (double)W1[(size_t)n * K1 + k] * b2h[k];   // the z operand is u = z + b2
-        out[NT + P] = (float)acc;
+        W1f = fold(W1a.data(), hid, b1f.data());
+        if (transh) {     // u = W_w a and the translation W_d a (+ b2: the accumulator then is v = x + W2 h + b2)
+            const std::vector<float>& Ww = get("W_w");
+            std::vector<double> Mw(Ww.begin(), Ww.end()), Md(Wd->begin(), Wd->end()), b2d(b2h.begin(), b2h.end());
+            Uf = fold(Mw.data(), tcp::D, nullptr);
+            Df = fold(Md.data(), tcp::D, b2d.data());
+        }
     }
     // ---- scorer layer 1's phi columns as the kernel's phi features see them, plus the bias on a constant-1 column:
     //      WM_PHI_STRUCT: the F columns of Ws0 as they are; WM_PHI_MEAN: folded onto psi (see the action warps)
@@ -1034,13 +1215,14 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
                 out[NT + P] = (float)acc;
             }
             double bias = bs0[n];
-            for (int k = 0; k < tcp::D; ++k) bias -= (double)Ws0[(size_t)n * K0 + k] * b2h[k];           // z_T arrives as u = z_T + b2
+            if (!transh)
+                for (int k = 0; k < tcp::D; ++k) bias -= (double)Ws0[(size_t)n * K0 + k] * b2h[k];       // z_T arrives as u = z_T + b2
             out[NPSI - 1] = (float)bias;
         }
     }
     const tcp::SmemLayout L = tcp::smem_layout(m.n_types, (m.H + 15) / 16, m.phi_kind == WM_PHI_STRUCT, AKB == 1 && PKB == 1);
     if ((int)L.total > ctx->smem_optin) return WM_OK;
-    const size_t n_slots = (size_t)tcp::step_boxes(NC, AKB) + tcp::scorer_boxes(PKB);
+    const size_t n_slots = (size_t)(transh ? tcp::th_step_boxes(NC, AKB) : tcp::step_boxes(NC, AKB)) + tcp::scorer_boxes(PKB);
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
     blob.reserve(n_slots * tcp::HB_BYTES);
@@ -1052,11 +1234,19 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         for (int k = 0; k < 2; ++k)
             for (int hrow = 0; hrow < 2; ++hrow) ok &= append_slot(blob, W2, hid, 64 * hrow, 128, c * 128 + k * 64, 64);
     };
-    g1a(0); g1a(1);
-    // step boundary: z K-blocks 0 and 2 of chunks 0, 1 (stage_za), then K-blocks 1 and 3 (stage_zb)
-    for (int half = 0; half < 2; ++half)
-        for (int c = 0; c < 2; ++c)
-            for (int k = half; k < 4; k += 2) ok &= append_slot(blob, W1, K1, c * 128, 64, k * 64, 64);
+    if (transh) {
+        // u = W_w' f, then the translation W_d' f: N = 256, two slots per feature K-block (weight rows 0-63 / 128-191, 64-127 / 192-255)
+        for (const std::vector<float>* M : {&Uf, &Df})
+            for (int k = 0; k < AKB; ++k)
+                for (int hrow = 0; hrow < 2; ++hrow) ok &= append_slot(blob, *M, 64 * AKB, 64 * hrow, 128, k * 64, 64);
+        g1a(0); g1a(1); g1z(0); g1z(1);
+    } else {
+        g1a(0); g1a(1);
+        // step boundary: z K-blocks 0 and 2 of chunks 0, 1 (stage_za), then K-blocks 1 and 3 (stage_zb)
+        for (int half = 0; half < 2; ++half)
+            for (int c = 0; c < 2; ++c)
+                for (int k = half; k < 4; k += 2) ok &= append_slot(blob, W1, K1, c * 128, 64, k * 64, 64);
+    }
     g2(0);
     for (int i = 2; i <= NC; ++i) {
         if (i < NC) { g1a(i); g1z(i); }
@@ -1112,16 +1302,14 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
         return WM_ERR_CUDA;
     }
     memcpy(m.tcp_tmap, &tm, sizeof(tm));
-    if (m.phi_kind == WM_PHI_STRUCT) {
-        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_STRUCT, false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
-        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_STRUCT, true>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
-    } else {
-        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_MEAN, false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
-        WM_CUDA_TRY(cudaFuncSetAttribute(tcp::wm_tcp_kernel<WM_PHI_MEAN, true>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    {
+        const void* fns[8] = {(const void*)tcp::wm_tcp_kernel<WM_PHI_MEAN, false, tcp::STEP_MLP_LN>, (const void*)tcp::wm_tcp_kernel<WM_PHI_MEAN, true, tcp::STEP_MLP_LN>,
+                              (const void*)tcp::wm_tcp_kernel<WM_PHI_STRUCT, false, tcp::STEP_MLP_LN>, (const void*)tcp::wm_tcp_kernel<WM_PHI_STRUCT, true, tcp::STEP_MLP_LN>,
+                              (const void*)tcp::wm_tcp_kernel<WM_PHI_MEAN, false, tcp::STEP_TRANSH>, (const void*)tcp::wm_tcp_kernel<WM_PHI_MEAN, true, tcp::STEP_TRANSH>,
+                              (const void*)tcp::wm_tcp_kernel<WM_PHI_STRUCT, false, tcp::STEP_TRANSH>, (const void*)tcp::wm_tcp_kernel<WM_PHI_STRUCT, true, tcp::STEP_TRANSH>};
+        const int base = (transh ? 4 : 0) + (m.phi_kind == WM_PHI_STRUCT ? 2 : 0);
+        for (int e = 0; e < 2; ++e)
+            WM_CUDA_TRY(cudaFuncSetAttribute(fns[base + e], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
     }
     m.tcp_ok = 1;
     m.tcp_akb = AKB;
@@ -1149,13 +1337,17 @@ int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const int max_pairs = ctx->n_sms / 2;
     const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
     const bool prefix_call = a.start || a.init_index || a.latents_out;
-    if (m.phi_kind == WM_PHI_STRUCT) {
-        if (prefix_call) tcp::wm_tcp_kernel<WM_PHI_STRUCT, true><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
-        else tcp::wm_tcp_kernel<WM_PHI_STRUCT, false><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
+    const bool ps = m.phi_kind == WM_PHI_STRUCT;
+    const dim3 grid(2 * pairs), block(tcp::THREADS);
+#define WM_TCP_LAUNCH(PHI_, EXT_, STEP_) tcp::wm_tcp_kernel<PHI_, EXT_, STEP_><<<grid, block, L.total, st>>>(p, tm)
+    if (m.kind == WM_KIND_TRANSH) {
+        if (ps) { if (prefix_call) WM_TCP_LAUNCH(WM_PHI_STRUCT, true, tcp::STEP_TRANSH); else WM_TCP_LAUNCH(WM_PHI_STRUCT, false, tcp::STEP_TRANSH); }
+        else { if (prefix_call) WM_TCP_LAUNCH(WM_PHI_MEAN, true, tcp::STEP_TRANSH); else WM_TCP_LAUNCH(WM_PHI_MEAN, false, tcp::STEP_TRANSH); }
     } else {
-        if (prefix_call) tcp::wm_tcp_kernel<WM_PHI_MEAN, true><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
-        else tcp::wm_tcp_kernel<WM_PHI_MEAN, false><<<2 * pairs, tcp::THREADS, L.total, st>>>(p, tm);
+        if (ps) { if (prefix_call) WM_TCP_LAUNCH(WM_PHI_STRUCT, true, tcp::STEP_MLP_LN); else WM_TCP_LAUNCH(WM_PHI_STRUCT, false, tcp::STEP_MLP_LN); }
+        else { if (prefix_call) WM_TCP_LAUNCH(WM_PHI_MEAN, true, tcp::STEP_MLP_LN); else WM_TCP_LAUNCH(WM_PHI_MEAN, false, tcp::STEP_MLP_LN); }
     }
+#undef WM_TCP_LAUNCH
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
     trace::dump(p.prof, st);
