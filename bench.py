@@ -49,7 +49,7 @@ import gen
 
 METRIC = "candidates_scored_per_sec"
 UNIT = "candidates/s"
-KERNELS = {1: "wm_tc_kernel", 2: "wm_tc2_kernel", 3: "wm_tcg_kernel", 4: "wm_tct_kernel", 5: "wm_tcp_kernel"}
+KERNELS = {1: "wm_tc_kernel", 2: "wm_tc2_kernel", 3: "wm_tcg_kernel", 5: "wm_tcp_kernel"}
 
 
 def _kernel_name(info) -> str:

@@ -108,8 +108,8 @@ typedef struct wm_info {        /* model hyper-parameters, as read from the weig
     int32_t tc_variant;         /* tcgen05 kernel built for this model: 0 = none, 1 = wm_tc_kernel (one CTA per  */
                                 /* 128-candidate tile, d = 256), 2 = wm_tc2_kernel (CTA pair per tile, d = 512),  */
                                 /* 3 = wm_tcg_kernel (CTA pair per tile, GRU transition, d = 384),             */
-                                /* 4 = wm_tct_kernel (TransH transition, d = 256), 5 = wm_tcp_kernel (CTA pair  */
-                                /* per 256-candidate tile, d = 256: the default form of variant 1, WM_OPT_PAIR) */
+                                /* 5 = wm_tcp_kernel (CTA pair per 256-candidate tile, d = 256: MLP+LayerNorm   */
+                                /* and TransH steps; the default form of variant 1, WM_OPT_PAIR)               */
     int32_t phi_kind;           /* WM_PHI_*: which action features G reads                                     */
     int32_t ranker_kind;        /* WM_RANKER_*                                                                 */
     int32_t n_trees, tree_depth;   /* WM_RANKER_FOREST only                                                    */

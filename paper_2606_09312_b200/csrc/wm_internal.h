@@ -58,7 +58,7 @@ struct Model {
     void* tc_blob = nullptr;
     size_t tc_blob_bytes = 0;
     void* tc_E = nullptr;      // bf16 [n_types][d_a]
-    int tc_ok = 0;             // 0 = no tcgen05 path, 1 = wm_tc_kernel (one CTA per tile), 2 = wm_tc2_kernel (CTA pair), 3 = wm_tcg_kernel (CTA pair, GRU), 4 = wm_tct_kernel (TransH)
+    int tc_ok = 0;             // 0 = no tcgen05 path, 1 = wm_tc_kernel (one CTA per tile), 2 = wm_tc2_kernel (CTA pair), 3 = wm_tcg_kernel (CTA pair, GRU), 4 = TransH model on wm_tcp_kernel (no single-CTA form)
     alignas(64) unsigned char tc2_tmap[128] = {};   // CUtensorMap over tc_blob (pair kernel)
     int tc1_ok = 0;            // the single-CTA form wm_tc_kernel is built (tc_ok == 1 means: at least one of the two forms is)
     int tcp_akb = 1, tcp_pkb = 1;   // wm_tcp_kernel: K-blocks of the folded action features / phi features
@@ -209,11 +209,6 @@ int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
                 const std::vector<std::string>& names);
 int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
-
-// K2 tcgen05, TransH (wm_tct.cu): bf16 TransH models with d = 256 (NEXT row f1).  Same entry route.
-int tct_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
-                const std::vector<std::string>& names);
-int launch_tct(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 
 // K4 (wm_forest.cu): tree-ensemble ranker over [z_T ; structured phi ; h] (NEXT row f4)
 int launch_forest(wm_ctx* ctx, const float* zT, const CallArgs& a, float* scores_out, cudaStream_t st);

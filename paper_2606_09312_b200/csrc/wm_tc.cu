@@ -868,10 +868,7 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         if (rc != WM_OK || m.tc_ok) return rc;
         const int rc2 = tcg_prepare(ctx, hv, names);
         if (rc2 != WM_OK || m.tc_ok) return rc2;
-        // TransH models (NEXT row f1): the single-CTA kernel wm_tct_kernel and the TransH step of the pair kernel
-        const int rc3 = tct_prepare(ctx, hv, names);
-        if (rc3 != WM_OK) return rc3;
-        m.tc1_ok = m.tc_ok == 4;
+        // TransH models (NEXT row f1): the TransH step of the pair kernel (tc_ok 4: no single-CTA form)
         if (m.kind == WM_KIND_TRANSH) {
             const int rc4 = tcp_prepare(ctx, hv, names);
             if (rc4 != WM_OK) return rc4;
@@ -993,15 +990,13 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const bool aligned = ((uintptr_t)a.init_states % 16 == 0) && ((uintptr_t)a.hw_feats % 16 == 0) &&
                          ((uintptr_t)a.latents_out % 16 == 0);
     const bool prefix_call = a.start || a.init_index || a.latents_out;   // wm_rollout_latents / wm_rollout_score_from
-    // the prefix-reuse calls are built into wm_tc_kernel only (the other models take the fp32 kernel for them); the
-    // TransH kernel has the latents-out piece (wm_rollout_latents; the rollout half of a forest-ranker model)
     const bool use_pair = m.tcp_ok && (ctx->opt_pair || !m.tc1_ok);      // d = 256 models: the pair kernel takes the call
-    const bool ext_ok = m.tc_ok == 1 || m.tc_ok == 2 || (m.tc_ok == 4 && (use_pair || (a.latents_out && !a.scores_out && !a.start && !a.init_index)));
+    const bool ext_ok = m.tc_ok == 1 || m.tc_ok == 2 || m.tc_ok == 4;      // (the GRU kernel does not take the prefix-reuse calls)
     if (prefix_call && !ext_ok && ctx->opt_path != 2) return launch_generic(ctx, a, st);
     if (!m.tc_ok || a.T_max > 255 || !aligned || (prefix_call && !ext_ok)) {
         if (ctx->opt_path == 2) {
             set_error("tcgen05 path: needs T_max <= 255, 16-byte aligned init_states / hw_feats (and, for "
-                      "wm_rollout_latents / wm_rollout_score_from, a d = 256 MLP+LayerNorm model)");
+                      "wm_rollout_latents / wm_rollout_score_from, an MLP+LayerNorm or TransH model)");
             return WM_ERR_UNSUPPORTED;
         }
         return launch_generic(ctx, a, st);
@@ -1009,7 +1004,6 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     if (m.tc_ok == 2) return launch_tc2(ctx, ws, a, st);
     if (m.tc_ok == 3) return launch_tcg(ctx, ws, a, st);
     if (use_pair) return launch_tcp(ctx, ws, a, st);
-    if (m.tc_ok == 4) return launch_tct(ctx, ws, a, st);
     tc::Params p;
     p.hid = m.hidden; p.nc = m.hidden / 128; p.n_types = m.n_types; p.P = m.P; p.H = m.H;
     p.hw_ksteps = (m.H + 15) / 16;
