@@ -12,9 +12,13 @@
 //     R_0 -> X2, R_1 -> X1, G_0 -> X0, H_0 -> X2, H_1 -> X1, G_1 -> X0
 // (H_j needs all of r*z, i.e. both R epilogues; G_1 reuses G_0's accumulator once blend_0 has read it), while the
 // epilogue warps turn R_j into the fp16 operand r*z (shared memory) and (G_j, H_j) into z' (fp32 -> TMEM, fp16 ->
-// the OTHER of two z operand buffers: G_1 still reads the old z while z'_0 is written).  Everything else — weight
-// ring fed by TMA into both CTAs with completion on the leader's barrier, multicast commits, cluster-scope arrivals,
-// static serpentine tile schedule, scorer on the same machinery — is as in wm_tc2.cu.
+// shared memory: z'_0 goes to the OTHER of two buffers of K-blocks 0-2, because G_1 still reads the old z while z'_0 is
+// written; z'_1 overwrites K-blocks 3-5 in place, G_1 having completed before blend_1 starts).  z'_0 and z'_1 are
+// published separately, so R_0 of step t+1 runs its first five K-blocks (z'_0 and a_{t+1}) under blend_1 of step t.
+// A ring stage is TWO [192 x 64] weight tiles (8 MMAs per wait / commit: the issuing warp, not the tensor pipe, was
+// the limiter with one tile per stage).  Everything else — weight ring fed by TMA into both CTAs with completion on
+// the leader's barrier, multicast commits, remote arrivals, static serpentine tile schedule, scorer on the same
+// machinery — is as in wm_tc2.cu.
 // Warp roles per CTA (512 threads): warps 0-7 epilogue (q = warp % 4: rows 32 (q & 1) + lane, N half q / 2; e = warp / 4:
 // 48-column half of the 96-column buffer), warps 8-11 action embedding (bucket-table gather), warp 12 TMEM allocator,
 // warp 13 tile schedule + TMA producer, warp 15 MMA issuer (leader CTA only).
@@ -43,17 +47,20 @@ constexpr int SW = 768;            // scorer hidden width (both hidden layers)
 constexpr int NT = 192;            // MMA N (columns per tile)
 constexpr int XC = NT / 2;         // TMEM columns per tile and CTA
 constexpr int KB_BYTES = 8192;     // one A K-block: [64 rows x 64 cols] fp16, SW128 K-major
-constexpr int BT_BYTES = 12288;    // one B half tile: [96 weight rows x 64 cols] fp16, SW128 K-major (= ring stage)
-constexpr int NSTAGE = 4;
+constexpr int BT_BYTES = 12288;    // one B half tile: [96 weight rows x 64 cols] fp16, SW128 K-major
+constexpr int STG_BYTES = 2 * BT_BYTES;   // a ring stage: two half tiles per CTA
+constexpr int NSTAGE = 3;
 constexpr int Z_KB = 6, A_KB = 2;  // K-blocks of the z part / the a (phi) part of an operand
+constexpr int ZH_KB = Z_KB / 2;    // K-blocks of one 192-column latent tile
+constexpr int ZH_BYTES = ZH_KB * KB_BYTES;
 constexpr int ZB_BYTES = Z_KB * KB_BYTES;
 constexpr int HWK_BYTES = 2048;    // hw operand: one [64 x 16] no-swizzle K-major tile per K = 16 step
 constexpr int THREADS = 512;
 constexpr int EPI_WARP0 = 0, ACT_WARP0 = 8, ALLOC_WARP = 12, PROD_WARP = 13, MMA_WARP = 15;
 constexpr int MAX_P = 8, MAX_H = 64, MAX_BUCKETS = 64;
-constexpr int TILE_STAGES = A_KB + Z_KB;                  // ring stages of one N tile of the rollout
+constexpr int TILE_STAGES = (A_KB + Z_KB) / 2;            // ring stages of one N tile of the rollout
 constexpr int ROLL_STAGES = 6 * TILE_STAGES;              // per step
-constexpr int SC_STAGES = 4 * (A_KB + 1 + Z_KB) + 2 * 24; // scorer: layer 1 (4 x (2 phi, hw, 6 z)), layer 2 (2 rounds x 12 x 2)
+constexpr int SC_STAGES = 4 * (1 + 1 + Z_KB / 2) + 2 * 12; // scorer: layer 1 (4 x (phi pair, hw, 3 z pairs)), layer 2 (2 rounds x 12)
 constexpr uint32_t IDESC_G = idesc_pair(NT);
 constexpr int NXB = 5;             // accumulators: X0, X1, X2 and, in the scorer, the two (dead) latent tiles
 
@@ -62,8 +69,8 @@ enum {
     B_EMPTY = B_FULL + NSTAGE,     // [NSTAGE] MMA commit (multicast) -> each CTA's producer
     B_XFULL = B_EMPTY + NSTAGE,    // [NXB] MMA commit -> epilogue: accumulator b filled
     B_XFREE = B_XFULL + NXB,       // [NXB] epilogue (both CTAs) -> leader MMA: accumulator b read, its output written
-    B_ZREADY = B_XFREE + NXB,      // epilogue (both CTAs) -> leader MMA: z' (both tiles) written
-    B_AFREE,                       // MMA commit -> action warps: a-part no longer read
+    B_ZREADY = B_XFREE + NXB,      // [2] epilogue (both CTAs) -> leader MMA: z' tile 0 / tile 1 written
+    B_AFREE = B_ZREADY + 2,                       // MMA commit -> action warps: a-part no longer read
     B_AREADY,                      // action warps (both CTAs) -> leader MMA: a-part written
     B_SFULL,                       // [2] schedule slot filled (CTA-local)
     B_SEMPTY = B_SFULL + 2,        // [2] schedule slot consumed (CTA-local)
@@ -86,10 +93,10 @@ struct SmemLayout {
 __host__ __device__ inline SmemLayout smem_layout(int hw_ksteps) {
     SmemLayout L;
     uint32_t o = 0;
-    L.zbuf = o; o += 2 * ZB_BYTES;                     // two fp16 z operand buffers (6 K-blocks each)
+    L.zbuf = o; o += 3 * ZH_BYTES;                     // fp16 z operand: K-blocks 0-2 twice (double-buffered), then 3-5
     L.abuf = o; o += A_KB * KB_BYTES;                  // fp16 a_t / phi
     L.rz = o; o += ZB_BYTES;                           // fp16 r*z
-    L.ring = o; o += NSTAGE * BT_BYTES;
+    L.ring = o; o += NSTAGE * STG_BYTES;
     L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
     L.idx = o; o += TMR * MAX_P * 4;                   // table row of every parameter slot of the step
     L.lens = o; o += TMR * 4;
@@ -127,6 +134,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         for (int i = 0; i < NXB; ++i) { mbar_init(bar(B_XFULL + i), 1); mbar_init(bar(B_XFREE + i), 16); }
         for (int i = 0; i < 2; ++i) { mbar_init(bar(B_SFULL + i), 1); mbar_init(bar(B_SEMPTY + i), 13); }
         mbar_init(bar(B_ZREADY), 16);
+        mbar_init(bar(B_ZREADY + 1), 16);
         mbar_init(bar(B_AFREE), 1);
         mbar_init(bar(B_AREADY), 8);
         fence_barrier_init();
@@ -149,6 +157,10 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     // TMEM column base of accumulator b (3, 4 = the latent tiles, free once the rollout of a tile is over)
     auto xcol = [&](int b) -> uint32_t { return b < 3 ? T_X + (uint32_t)(XC * b) : T_Z + (uint32_t)(XC * (b - 3)); };
 
+    // Register hand-over (setmaxnreg works per warpgroup of four warps): the two epilogue warpgroups give up 16
+    // registers per thread, the action warpgroup (8-11) takes them: it holds a whole step's 16 embedded rows per warp in
+    // registers while the a-buffer is still being read, so that only the stores stand between the buffer's release and
+    // the next step's first a K-block.
     if (warp == PROD_WARP) {
         // =============================================================== tile schedule + TMA producer
         uint32_t stage = 0, ph = 0;
@@ -179,9 +191,9 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     if (i == roll_total) src = ROLL_STAGES;
                     else if (i < roll_total && src == ROLL_STAGES) src = 0;
                     mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
-                    // the leader's barrier collects both halves of the [192 x 64] tile
-                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2 * BT_BYTES);
-                    tma_load_2sm(s_ring + stage * BT_BYTES, &tmap, 0, XC * (2 * src + (int)rank), bar(B_FULL + stage));
+                    // the leader's barrier collects both CTAs' halves of the stage's two [192 x 64] tiles
+                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2 * STG_BYTES);
+                    tma_load_2sm(s_ring + stage * STG_BYTES, &tmap, 0, 2 * XC * (2 * src + (int)rank), bar(B_FULL + stage));
                     ++src;
                     if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
                 }
@@ -217,20 +229,34 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             WM_TRACE(3);
             if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
         };
-        // one ring stage = one [192 x 64] B tile against the [64(+64) x 64] A K-block at a_tile: 4 MMAs of K = 16
-        auto stage_ss = [&](uint32_t d_tmem, uint32_t a_tile, bool first) {
-            wait_full();
-            const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + stage * BT_BYTES);
-            if (elect_one()) {
+        // A ring stage holds two [192 x 64] B tiles; each goes against one [64(+64) x 64] A K-block: 4 MMAs of K = 16.
+        // tile_mma is called by the elected lane only.
+        auto tile_mma = [&](uint32_t d_tmem, uint32_t a_tile, int i, bool first) {
+            const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + stage * STG_BYTES + i * BT_BYTES);
 #pragma unroll
-                for (int j = 0; j < 4; ++j) mma_ss2(d_tmem, a0 + 2u * j, b0 + 2u * j, IDESC_G, (first && j == 0) ? 0u : 1u);
+            for (int j = 0; j < 4; ++j) mma_ss2(d_tmem, a0 + 2u * j, b0 + 2u * j, IDESC_G, (first && j == 0) ? 0u : 1u);
+        };
+        auto stage_end = [&]() {
+            if (elect_one()) mma_commit2(bar(B_EMPTY + stage));
+            advance();
+        };
+        // both tiles of the stage in one go: (accumulator, A K-block) x 2
+        auto stage2 = [&](uint32_t d0, uint32_t a_tile0, bool first0, uint32_t d1, uint32_t a_tile1, bool first1) {
+            wait_full();
+            if (elect_one()) {
+                tile_mma(d0, a_tile0, 0, first0);
+                tile_mma(d1, a_tile1, 1, first1);
                 mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
         };
-        auto stage_hw = [&](uint32_t d_tmem) {
+        auto half = [&](uint32_t d, uint32_t a_tile, int i, bool first) {     // one tile of an open stage
+            if (elect_one()) tile_mma(d, a_tile, i, first);
+            __syncwarp();
+        };
+        auto stage_hw = [&](uint32_t d_tmem) {       // the stage's second tile is padding
             wait_full();
-            const uint64_t b0 = smem_desc(s_ring + stage * BT_BYTES);
+            const uint64_t b0 = smem_desc(s_ring + stage * STG_BYTES);
             if (elect_one()) {
                 for (int j = 0; j < p.hw_ksteps; ++j)
                     mma_ss2(d_tmem, smem_desc_nosw(s_hwk + j * HWK_BYTES), b0 + 2u * j, IDESC_G, 1u);
@@ -242,24 +268,27 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (elect_one()) mma_commit2(bar(barrier));
             __syncwarp();
         };
-        // A tile = its a (or phi) K-blocks and its z (or r*z, h1) K-blocks, in either order; `first` marks the segment
-        // that starts the accumulation
-        auto seg_a = [&](int b, bool first) {
-            stage_ss(xcol(b), s_a, first);
-            stage_ss(xcol(b), s_a + KB_BYTES, false);
-        };
-        auto seg_z = [&](int b, uint32_t zbase, bool first) {
-#pragma unroll 1
-            for (int k = 0; k < Z_KB; ++k) stage_ss(xcol(b), zbase + k * KB_BYTES, first && k == 0);
-        };
         auto finish = [&](int b) {
             commit(B_XFULL + b);
             pend |= 1u << b;
         };
-        auto a_part = [&](int b) { seg_a(b, true); };
-        auto z_part = [&](int b, uint32_t zbase) { seg_z(b, zbase, false); finish(b); };
+        // the a (or phi) K-block pair; `first` starts the accumulation
+        auto seg_a = [&](int b, bool first) { stage2(xcol(b), s_a, first, xcol(b), s_a + KB_BYTES, false); };
+        // six z-like K-blocks as three stages: K-blocks 0-2 at lo, 3-5 at hi
+        auto seg_z = [&](int b, uint32_t lo, uint32_t hi, bool first) {
+            stage2(xcol(b), lo, first, xcol(b), lo + KB_BYTES, false);
+            stage2(xcol(b), lo + 2 * KB_BYTES, false, xcol(b), hi, false);
+            stage2(xcol(b), hi + KB_BYTES, false, xcol(b), hi + 2 * KB_BYTES, false);
+        };
         auto wait_a = [&]() { WM_TRACE(20); mbar_wait(bar(B_AREADY), n_a & 1); WM_TRACE(21); ++n_a; tc_fence_after(); };
-        auto wait_z = [&]() { WM_TRACE(22); mbar_wait(bar(B_ZREADY), n_z & 1); WM_TRACE(23); ++n_z; tc_fence_after(); };
+        auto wait_z = [&](int j) {
+            WM_TRACE(22 + 2 * j);
+            mbar_wait(bar(B_ZREADY + j), (n_z >> j) & 1);
+            WM_TRACE(23 + 2 * j);
+            n_z ^= 1u << j;
+            tc_fence_after();
+        };
+        const uint32_t s_zhi = s_z + 2 * ZH_BYTES, s_rzhi = s_rz + ZH_BYTES;
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
             mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
@@ -270,36 +299,44 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (rank != 0) continue;
 #pragma unroll 1
             for (int t = 0; t < nsteps; ++t) {
-                const uint32_t zc = s_z + (uint32_t)(t & 1) * ZB_BYTES;     // fp16 z_t
-                // the first three tiles take their z K-blocks first and their a K-blocks last: a_{t+1} is written only
-                // after G_1 of step t has released the a-buffer, and its gather latency hides under these z stages
-                wait_x(2); wait_z(); seg_z(2, zc, true); wait_a(); seg_a(2, false); finish(2);   // R_0 -> X2
-                wait_x(1); seg_z(1, zc, true); seg_a(1, false); finish(1);                       // R_1 -> X1
-                wait_x(0); seg_z(0, zc, true); seg_a(0, false); finish(0);                       // G_0 -> X0
+                WM_TRACE(30);
+                const uint32_t zlo = s_z + (uint32_t)(t & 1) * ZH_BYTES;    // fp16 z_t, K-blocks 0-2 (3-5 are at s_zhi)
+                // R_0 -> X2 starts on z'_0 (tile 0 of the previous blend) and a_t while blend_1 of step t-1 is still
+                // running: K-blocks z0 z1 | z2 a0 | a1 z3 | z4 z5
+                wait_x(2); wait_z(0);
+                stage2(xcol(2), zlo, true, xcol(2), zlo + KB_BYTES, false);
+                wait_full(); half(xcol(2), zlo + 2 * KB_BYTES, 0, false); wait_a(); half(xcol(2), s_a, 1, false); stage_end();
+                wait_full(); half(xcol(2), s_a + KB_BYTES, 0, false); wait_z(1); half(xcol(2), s_zhi, 1, false); stage_end();
+                stage2(xcol(2), s_zhi + KB_BYTES, false, xcol(2), s_zhi + 2 * KB_BYTES, false);
+                finish(2);
+                wait_x(1); seg_z(1, zlo, s_zhi, true); seg_a(1, false); finish(1);               // R_1 -> X1
+                wait_x(0); seg_z(0, zlo, s_zhi, true); seg_a(0, false); finish(0);               // G_0 -> X0
                 wait_x(2); wait_x(1);                                       // r*z complete, X2 / X1 read
-                a_part(2); z_part(2, s_rz);                                 // H_0 -> X2
-                a_part(1); z_part(1, s_rz);                                 // H_1 -> X1
+                seg_a(2, true); seg_z(2, s_rz, s_rzhi, false); finish(2);   // H_0 -> X2
+                seg_a(1, true); seg_z(1, s_rz, s_rzhi, false); finish(1);   // H_1 -> X1
                 wait_x(0);                                                  // blend_0 has read G_0
-                a_part(0); commit(B_AFREE); z_part(0, zc);                  // G_1 -> X0 (still the OLD z)
+                seg_a(0, true); commit(B_AFREE); seg_z(0, zlo, s_zhi, false); finish(0);   // G_1 -> X0 (still the OLD z)
             }
             // ---- scorer layer 1: four 192-column tiles of gelu(Ws0 [z_T; phi; hw] + bs0) into X2, X1, X0 and latent
-            // tile 0; their fp16 outputs h1 go to the spare z buffer (tiles 0, 1) and the r*z buffer (tiles 2, 3)
-            const uint32_t zc = s_z + (uint32_t)(nsteps & 1) * ZB_BYTES;    // z_T
-            const uint32_t h1a = s_z + (uint32_t)((nsteps & 1) ^ 1) * ZB_BYTES, h1b = s_rz;
+            // tile 0; their fp16 outputs h1 go to the spare z K-blocks (tile 0), the r*z buffer (tiles 1, 2) and, once
+            // every layer-1 MMA has completed, over z_T's K-blocks 3-5 (tile 3)
+            const uint32_t zlo = s_z + (uint32_t)(nsteps & 1) * ZH_BYTES;   // z_T, K-blocks 0-2
+            const uint32_t h1_0 = s_z + (uint32_t)((nsteps & 1) ^ 1) * ZH_BYTES;
             const int l1buf[4] = {2, 1, 0, 3};
 #pragma unroll
             for (int n = 0; n < 4; ++n) {
                 const int b = l1buf[n];
                 wait_x(b);
                 if (n == 0) wait_a();
-                a_part(b);
+                seg_a(b, true);
                 stage_hw(xcol(b));
                 if (n == 3) commit(B_AFREE);
-                if (n == 0) wait_z();
-                z_part(b, zc);
+                if (n == 0) { wait_z(0); wait_z(1); }
+                seg_z(b, zlo, s_zhi, false);
+                finish(b);
             }
             // ---- scorer layer 2, K = 768 as the four h1 tiles (3 K-blocks each), N = 768 in two rounds of two
-            // 192-column tiles: round 0 into latent tile 1 and X2, round 1 into X1 and X0
+            // 192-column tiles (a stage = one K-block of both): round 0 into latent tile 1 and X2, round 1 into X1 and X0
 #pragma unroll
             for (int round = 0; round < 2; ++round) {
                 const int b0 = round == 0 ? 4 : 1, b1 = round == 0 ? 2 : 0;
@@ -307,12 +344,11 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll 1
                 for (int kc = 0; kc < 4; ++kc) {
                     if (round == 0) wait_x(kc == 0 ? 2 : kc == 1 ? 1 : kc == 2 ? 0 : 3);   // h1 tile kc written
-                    const uint32_t a_base = (kc < 2 ? h1a : h1b) + (uint32_t)((kc & 1) * 3) * KB_BYTES;
+                    const uint32_t a_base = kc == 0 ? h1_0 : kc == 1 ? s_rz : kc == 2 ? s_rzhi : s_zhi;
 #pragma unroll 1
-                    for (int kb = 0; kb < 3; ++kb) {
-                        stage_ss(xcol(b0), a_base + kb * KB_BYTES, kc == 0 && kb == 0);
-                        stage_ss(xcol(b1), a_base + kb * KB_BYTES, kc == 0 && kb == 0);
-                    }
+                    for (int kb = 0; kb < 3; ++kb)
+                        stage2(xcol(b0), a_base + kb * KB_BYTES, kc == 0 && kb == 0, xcol(b1), a_base + kb * KB_BYTES,
+                               kc == 0 && kb == 0);
                 }
                 commit(B_XFULL + b0);
                 commit(B_XFULL + b1);
@@ -323,6 +359,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     }
     else if (warp >= EPI_WARP0 && warp < ACT_WARP0) {
         // =============================================================== epilogue warps (gates / blend / scorer)
+        reg_dealloc<112>();
         const int q = warp & 3, e = (warp - EPI_WARP0) >> 2;
         const int rh = q & 1, nh = q >> 1;
         const int row = 32 * rh + lane;                 // row of this CTA's 64
@@ -334,14 +371,15 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         uint8_t* rzb = smem + L.rz;
         const uint32_t r_xfree0 = mapa(bar(B_XFREE), 0);      // leader's XFREE[b] = r_xfree0 + 8 b
         auto r_xfree = [&](int b) -> uint32_t { return r_xfree0 + 8u * (uint32_t)b; };
-        const uint32_t r_zready = mapa(bar(B_ZREADY), 0);
+        const uint32_t r_zready = mapa(bar(B_ZREADY), 0);      // tile 0; tile 1 at + 8
+        uint8_t* zhi = zb + 2 * ZH_BYTES;                      // fp16 z K-blocks 3-5 (latent tile 1)
         uint32_t fpar = 0;                              // parity of every XFULL barrier
         auto wait_full = [&](int b) {
             mbar_wait(bar(B_XFULL + b), (fpar >> b) & 1u);
             fpar ^= 1u << b;
             tc_fence_after();
         };
-        // 16 fp16 values of this row at column m0 (multiple of 16) of a 384-wide operand buffer (6 K-blocks)
+        // 16 fp16 values of this row at column m0 (multiple of 16) of a 192-wide operand region (3 K-blocks)
         auto put16 = [&](uint8_t* buf, int m0, const uint32_t (&o)[8]) {
             uint8_t* kb = buf + (m0 >> 6) * KB_BYTES;
             const int ch = (m0 & 63) >> 3;
@@ -349,7 +387,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             *reinterpret_cast<uint4*>(kb + sw128_off(row, ch + 1)) = make_uint4(o[4], o[5], o[6], o[7]);
         };
         // arrive on up to two leader barriers after this warp's TMEM / shared-memory writes are visible
-        auto publish = [&](uint32_t bar_a, uint32_t bar_b, bool tmem_written) {
+        auto publish = [&](uint32_t bar_a, uint32_t bar_b, uint32_t bar_c, bool tmem_written) {
             if (tmem_written) tmem_st_wait();
             fence_proxy_async();
             tc_fence_before();
@@ -357,6 +395,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (lane == 0) {
                 mbar_arrive_remote(bar_a);
                 if (bar_b) mbar_arrive_remote(bar_b);
+                if (bar_c) mbar_arrive_remote(bar_c);
             }
         };
 
@@ -392,12 +431,12 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) o[i] = pack_f16(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
                 tmem_st16(T_Z + (uint32_t)(XC * j) + tcol + 16u * s, v);
-                put16(zb, m0, o);
+                put16(j == 0 ? zb : zhi, cb + 16 * s, o);
             }
-            publish(r_zready, 0u, true);
+            publish(r_zready, r_zready + 8u, 0u, true);
 
             for (int t = 0; t < nsteps; ++t) {
-                uint8_t* znext = zb + ((t & 1) ^ 1) * ZB_BYTES;
+                uint8_t* znext = zb + ((t & 1) ^ 1) * ZH_BYTES;     // z'_0 (K-blocks 0-2); z'_1 overwrites zhi
                 const bool live = t < len;     // masked steps leave the state unchanged
                 // ---- r = sigma(R_j), fp16 r*z -> the r*z operand buffer (R_0 in X2, R_1 in X1)
 #pragma unroll 1
@@ -414,9 +453,9 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                         for (int i = 0; i < 8; ++i)
                             o[i] = pack_f16(sigmoid_fast(__uint_as_float(x[2 * i])) * __uint_as_float(z[2 * i]),
                                             sigmoid_fast(__uint_as_float(x[2 * i + 1])) * __uint_as_float(z[2 * i + 1]));
-                        put16(rzb, NT * j + cb + 16 * s, o);
+                        put16(rzb + j * ZH_BYTES, cb + 16 * s, o);
                     }
-                    publish(r_xfree(xb), 0u, false);
+                    publish(r_xfree(xb), 0u, 0u, false);
                 }
                 // ---- z'_j = z + g (tanh(H_j) - z) = (1 - g) z + g h,  g = sigma(G_j)  (G_j in X0; H_0 in X2, H_1 in X1).
                 // The blend is bound by the special-function unit (sigma and tanh: 2 of 16 per clock and SM for each of
@@ -441,9 +480,10 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                         for (int i = 0; i < 8; ++i) o[i] = pack_f16(__uint_as_float(z[2 * i]), __uint_as_float(z[2 * i + 1]));
                         tmem_st16(T_Z + (uint32_t)(XC * j) + tcol + 16u * s, z);
-                        put16(znext, NT * j + cb + 16 * s, o);
+                        put16(j == 0 ? znext : zhi, cb + 16 * s, o);
                     }
-                    publish(r_xfree(0), r_xfree(xh), true);
+                    // tile j of z' is written: X0 and the H accumulator are free, R_0 of the next step may read z'_j
+                    publish(r_xfree(0), r_xfree(xh), r_zready + 8u * (uint32_t)j, true);
                 };
                 wait_full(0);      // G_0
                 wait_full(2);      // H_0
@@ -463,13 +503,11 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 tmem_st_wait();
                 wait_full(0);      // G_1
                 blend(1, 1, true);
-                // both tiles of z' are written (the arrivals above already ordered the writes)
-                __syncwarp();
-                if (lane == 0) mbar_arrive_remote(r_zready);
             }
 
-            // ---- scorer layer 1 -> h1 (fp16): tiles 0, 1 into the spare z buffer, tiles 2, 3 into the r*z buffer
-            uint8_t* h1a = zb + ((nsteps & 1) ^ 1) * ZB_BYTES;
+            // ---- scorer layer 1 -> h1 (fp16): tile 0 into the spare z K-blocks, tiles 1, 2 into the r*z buffer, tile 3
+            // over z_T's K-blocks 3-5 (its accumulator is the last of layer 1: every MMA that reads z_T has completed)
+            uint8_t* h1_0 = zb + ((nsteps & 1) ^ 1) * ZH_BYTES;
 #pragma unroll 1
             for (int n = 0; n < 4; ++n) {
                 const int xb = n == 0 ? 2 : n == 1 ? 1 : n == 2 ? 0 : 3;
@@ -489,9 +527,9 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                         o[2 * i + 1] = gelu2_f16(make_float2(__uint_as_float(x[4 * i + 2]), __uint_as_float(x[4 * i + 3])),
                                                  make_float2(bv.z, bv.w));
                     }
-                    put16(n < 2 ? h1a : rzb, (n & 1) * NT + cb + 16 * s, o);
+                    put16(n == 0 ? h1_0 : n == 1 ? rzb : n == 2 ? rzb + ZH_BYTES : zhi, cb + 16 * s, o);
                 }
-                publish(r_xfree(xb), 0u, false);
+                publish(r_xfree(xb), 0u, 0u, false);
             }
             // ---- scorer layer 2 + output dot product: N tiles 0..3 arrive in latent tile 1, X2, X1, X0
             float acc = 0.0f;
@@ -525,6 +563,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         // =============================================================== action-embedding warps
         // warp aw owns rows [16 aw, 16 aw + 16).  Phase 1 is row-mapped (lanes 0-15: table row of every parameter
         // slot), phase 2 column-mapped (lane = 4 embedding columns: gather P table rows per candidate row and add).
+        reg_alloc<160>();
         const int aw = warp - ACT_WARP0;
         const int row = 16 * aw + (lane & 15);
         const bool row_lane = lane < 16;
@@ -538,28 +577,9 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         auto a_dst = [&](int r) -> uint2* {
             return reinterpret_cast<uint2*>(ab + (lane >> 4) * KB_BYTES + sw128_off(r, (lane & 15) >> 1) + (lane & 1) * 8);
         };
-        // a (4 columns of this lane) of row r of the step whose slot rows are in s_idx; false when the row is masked
-        auto embed_row = [&](int r, float (&a4)[4]) -> bool {
-            const int4 i0 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P);
-            const int4 i1 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P + 4);
-            a4[0] = a4[1] = a4[2] = a4[3] = 0.0f;
-            if (i0.x < 0) return false;
-            const int ix[8] = {i0.x, i0.y, i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
-#pragma unroll
-            for (int j = 0; j < MAX_P; ++j) {
-                if (j < P) {
-                    const uint2 v = __ldg(reinterpret_cast<const uint2*>(p.Tbl + (size_t)ix[j] * DA + col4));
-                    a4[0] += __uint_as_float(v.x << 16);
-                    a4[1] += __uint_as_float(v.x & 0xffff0000u);
-                    a4[2] += __uint_as_float(v.y << 16);
-                    a4[3] += __uint_as_float(v.y & 0xffff0000u);
-                }
-            }
-            return true;
-        };
         for (uint32_t it = 0;; ++it) {
             const uint32_t slot = it & 1;
-            mbar_wait(bar(B_SFULL + slot), (it >> 1) & 1);
+            mbar_wait_inline(bar(B_SFULL + slot), (it >> 1) & 1);
             const int tile = s_sched[slot * 2 + 0], nsteps = s_sched[slot * 2 + 1];
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(B_SEMPTY + slot));
@@ -569,24 +589,35 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             float phi[16][4];
 #pragma unroll
             for (int rr = 0; rr < 16; ++rr) phi[rr][0] = phi[rr][1] = phi[rr][2] = phi[rr][3] = 0.0f;
+            // the action of step t of this lane's row, fetched one step ahead (the arrays stream from HBM)
+            int id_n = 0, prm_n[MAX_P];
+            auto fetch = [&](int t) {
+                if (row_lane && t < len) {
+                    id_n = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
+                    const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
+#pragma unroll
+                    for (int j = 0; j < MAX_P; ++j)
+                        if (j < P) prm_n[j] = __ldg(pp + j);
+                }
+            };
+            fetch(0);
 
             for (int t = 0; t < nsteps; ++t) {
-                // phase 1: table row of every parameter slot: (id P + j) n_b + bucket(p_j)
+                // phase 1 (row-mapped): table row of every parameter slot: (id P + j) n_b + bucket(p_j)
                 if (row_lane) {
                     int ix[MAX_P];
 #pragma unroll
                     for (int j = 0; j < MAX_P; ++j) ix[j] = 0;
                     if (t < len) {
-                        int id = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
+                        int id = id_n;
                         if (id < 0 || id >= p.n_types) {
                             atomicOr(p.a.fault, WM_FAULT_TYPE);
                             id = id < 0 ? 0 : p.n_types - 1;
                         }
-                        const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
 #pragma unroll
                         for (int j = 0; j < MAX_P; ++j) {
                             if (j < P) {
-                                int prm = __ldg(pp + j);
+                                int prm = prm_n[j];
                                 if (prm < 1) {
                                     atomicOr(p.a.fault, WM_FAULT_PARAM);
                                     prm = 1;
@@ -607,34 +638,48 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     *reinterpret_cast<int4*>(s_idx + row * MAX_P + 4) = make_int4(ix[4], ix[5], ix[6], ix[7]);
                 }
                 __syncwarp();
-                // phase 2: the first PRE rows are gathered and summed in registers BEFORE the a-part is free (the table rows
-                // come from L2; that latency sits between the a-buffer's release and the next step's first MMAs), the
-                // rest after.  PRE = 12 / 16 and a setmaxnreg hand-over of registers to these warps were measured:
-                // both spill under the kernel's 128-register cap and are slower (715 vs 794 TFLOP/s).
-                constexpr int PRE = 8;
-                uint2 pk[PRE];
+                fetch(t + 1);
+                // phase 2 (column-mapped, lane = 4 embedding columns): all 16 rows are gathered from the table (L2) and
+                // summed in registers BEFORE the a-buffer is free, two rows' loads in flight at a time
+                uint2 pk[16];
 #pragma unroll
-                for (int rr = 0; rr < PRE; ++rr) {
-                    float a4[4];
-                    if (embed_row(16 * aw + rr, a4)) {
+                for (int g = 0; g < 8; ++g) {
+                    uint2 v[2][MAX_P];
+                    bool on[2];
 #pragma unroll
-                        for (int c = 0; c < 4; ++c) phi[rr][c] += a4[c];
+                    for (int q = 0; q < 2; ++q) {
+                        const int r = 16 * aw + 2 * g + q;
+                        const int4 i0 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P);
+                        const int4 i1 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P + 4);
+                        on[q] = i0.x >= 0;
+                        const int ix[8] = {i0.x, i0.y, i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
+#pragma unroll
+                        for (int j = 0; j < MAX_P; ++j)
+                            if (j < P && on[q]) v[q][j] = __ldg(reinterpret_cast<const uint2*>(p.Tbl + (size_t)ix[j] * DA + col4));
                     }
-                    pk[rr] = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        float a4[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+                        if (on[q]) {
+#pragma unroll
+                            for (int j = 0; j < MAX_P; ++j) {
+                                if (j < P) {
+                                    a4[0] += __uint_as_float(v[q][j].x << 16);
+                                    a4[1] += __uint_as_float(v[q][j].x & 0xffff0000u);
+                                    a4[2] += __uint_as_float(v[q][j].y << 16);
+                                    a4[3] += __uint_as_float(v[q][j].y & 0xffff0000u);
+                                }
+                            }
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) phi[2 * g + q][c] += a4[c];
+                        }
+                        pk[2 * g + q] = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
+                    }
                 }
-                if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+                if (n_w > 0) mbar_wait_inline(bar(B_AFREE), (n_w - 1) & 1);
                 ++n_w;
 #pragma unroll
-                for (int rr = 0; rr < PRE; ++rr) *a_dst(16 * aw + rr) = pk[rr];
-#pragma unroll
-                for (int rr = PRE; rr < 16; ++rr) {
-                    float a4[4];
-                    if (embed_row(16 * aw + rr, a4)) {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) phi[rr][c] += a4[c];
-                    }
-                    *a_dst(16 * aw + rr) = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
-                }
+                for (int rr = 0; rr < 16; ++rr) *a_dst(16 * aw + rr) = pk[rr];
                 fence_proxy_async();
                 __syncwarp();   // also: phase 2 reads of s_idx are done before the next phase 1 overwrites
                 if (lane == 0) mbar_arrive_remote(r_aready);
@@ -643,7 +688,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             // ---- phi = mean_t a_t (0 when len = 0)
             if (row_lane) s_lens[row] = len;
             __syncwarp();
-            if (n_w > 0) mbar_wait(bar(B_AFREE), (n_w - 1) & 1);
+            if (n_w > 0) mbar_wait_inline(bar(B_AFREE), (n_w - 1) & 1);
             ++n_w;
 #pragma unroll
             for (int rr = 0; rr < 16; ++rr) {
@@ -692,23 +737,34 @@ uint16_t f32_to_bf16(float f) {
     return (uint16_t)(u >> 16);
 }
 
-// Append the [192 x 64] pair tile W[n0 + n][k0 + k] (k < kvalid, else 0) as two 12 KB halves (weight rows 0-95 for the
-// leader CTA, 96-191 for its peer), each in the SW128 K-major shared-memory image, fp16.  Returns false when a weight
-// is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
-bool append_pair_tile(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld, int n0, int k0, int kvalid) {
+// One [192 x 64] weight tile W[n0 + n][k0 + k] (k < kvalid, else 0); W == nullptr is padding.
+struct Box {
+    const std::vector<float>* W;
+    int ld, n0, k0, kvalid;
+};
+
+// Append one ring stage = two tiles.  Image of a stage: the leader CTA's 24 KB (weight rows 0-95 of tile A, then of tile
+// B), then its peer's (rows 96-191 of A, of B); every 12 KB half tile in the SW128 K-major shared-memory image, fp16.
+// Returns false when a weight is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
+bool append_stage(std::vector<uint16_t>& blob, const Box& A, const Box& B) {
     const size_t base = blob.size();
-    blob.resize(base + 2 * tcg::BT_BYTES / 2, 0);
+    blob.resize(base + 2 * tcg::STG_BYTES / 2, 0);
     bool ok = true;
-    for (int n = 0; n < tcg::NT; ++n)
-        for (int k = 0; k < 64; ++k) {
-            const float v = k < kvalid ? W[(size_t)(n0 + n) * ld + k0 + k] : 0.0f;
-            const int nn = n % tcg::XC;
-            const size_t off = (size_t)(n / tcg::XC) * tcg::BT_BYTES + (size_t)nn * 128 +
-                               (size_t)((((k >> 3) ^ (nn & 7)) << 4)) + (size_t)(k & 7) * 2;
-            uint16_t hb;
-            ok &= f32_to_f16_bits(v, &hb);
-            blob[base + off / 2] = hb;
-        }
+    const Box* bx[2] = {&A, &B};
+    for (int i = 0; i < 2; ++i) {
+        if (!bx[i]->W) continue;
+        const std::vector<float>& W = *bx[i]->W;
+        for (int n = 0; n < tcg::NT; ++n)
+            for (int k = 0; k < 64; ++k) {
+                const float v = k < bx[i]->kvalid ? W[(size_t)(bx[i]->n0 + n) * bx[i]->ld + bx[i]->k0 + k] : 0.0f;
+                const int nn = n % tcg::XC;
+                const size_t off = (size_t)(n / tcg::XC) * tcg::STG_BYTES + (size_t)i * tcg::BT_BYTES + (size_t)nn * 128 +
+                                   (size_t)((((k >> 3) ^ (nn & 7)) << 4)) + (size_t)(k & 7) * 2;
+                uint16_t hb;
+                ok &= f32_to_f16_bits(v, &hb);
+                blob[base + off / 2] = hb;
+            }
+    }
     return ok;
 }
 
@@ -739,29 +795,34 @@ int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     const std::vector<float>&Wg = get("W_g"), &Wr = get("W_r"), &Wh = get("W_h"), &Ws0 = get("Ws0"), &Ws1 = get("Ws1");
     const std::vector<float>& Tbl = get("Tbl");
     const int K1 = tcg::D + tcg::DA, K0 = K1 + m.H;
-    const size_t n_tiles = (size_t)tcg::ROLL_STAGES + tcg::SC_STAGES;
+    const size_t n_stages = (size_t)tcg::ROLL_STAGES + tcg::SC_STAGES;
     std::vector<uint16_t> blob;
     bool ok = true;   // every weight finite in fp16
-    blob.reserve(n_tiles * tcg::BT_BYTES);
-    auto roll_tile = [&](const std::vector<float>& W, int j, bool a_first) {   // K-blocks a (6, 7) and z / r*z (0-5)
-        if (a_first)
-            for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
-        for (int k = 0; k < tcg::Z_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
-        if (!a_first)
-            for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, W, K1, j * tcg::NT, k * 64, 64);
+    blob.reserve(n_stages * tcg::STG_BYTES);
+    // K-block k of the rollout operand [z ; a]: 0-5 = z (or r*z), 6, 7 = a
+    auto rb = [&](const std::vector<float>& W, int j, int k) { return Box{&W, K1, j * tcg::NT, k * 64, 64}; };
+    auto st = [&](const Box& A, const Box& B) { ok &= append_stage(blob, A, B); };
+    // the MMA warp's order (wm_tcg_kernel): R_0 interleaves a between z'_0 and z'_1; R_1, G_0 take z first; H_0, H_1,
+    // G_1 take a first
+    st(rb(Wr, 0, 0), rb(Wr, 0, 1)); st(rb(Wr, 0, 2), rb(Wr, 0, 6)); st(rb(Wr, 0, 7), rb(Wr, 0, 3)); st(rb(Wr, 0, 4), rb(Wr, 0, 5));
+    auto roll_tile = [&](const std::vector<float>& W, int j, bool a_first) {
+        if (a_first) st(rb(W, j, 6), rb(W, j, 7));
+        for (int k = 0; k < tcg::Z_KB; k += 2) st(rb(W, j, k), rb(W, j, k + 1));
+        if (!a_first) st(rb(W, j, 6), rb(W, j, 7));
     };
-    // the MMA warp's order: R_0, R_1, G_0 (z K-blocks first), H_0, H_1, G_1 (a K-blocks first)
-    roll_tile(Wr, 0, false); roll_tile(Wr, 1, false); roll_tile(Wg, 0, false);
+    roll_tile(Wr, 1, false); roll_tile(Wg, 0, false);
     roll_tile(Wh, 0, true); roll_tile(Wh, 1, true); roll_tile(Wg, 1, true);
-    for (int n = 0; n < 4; ++n) {     // scorer layer 1: phi (2), hw (1, zero-padded to 64 columns), z (6)
-        for (int k = tcg::Z_KB; k < tcg::Z_KB + tcg::A_KB; ++k) ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, k * 64, 64);
-        ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, K1, m.H);
-        for (int k = 0; k < tcg::Z_KB; ++k) ok &= append_pair_tile(blob, Ws0, K0, n * tcg::NT, k * 64, 64);
+    const Box pad{nullptr, 0, 0, 0, 0};
+    for (int n = 0; n < 4; ++n) {     // scorer layer 1: phi pair, hw (zero-padded to 64 columns) + padding, three z pairs
+        auto sb = [&](int k0, int kvalid) { return Box{&Ws0, K0, n * tcg::NT, k0, kvalid}; };
+        st(sb(tcg::D, 64), sb(tcg::D + 64, 64));
+        st(sb(K1, m.H), pad);
+        for (int k = 0; k < tcg::Z_KB; k += 2) st(sb(k * 64, 64), sb((k + 1) * 64, 64));
     }
     for (int round = 0; round < 2; ++round)   // scorer layer 2: two rounds of two N tiles over all 12 K-blocks
         for (int kb = 0; kb < 12; ++kb)
-            for (int jj = 0; jj < 2; ++jj) ok &= append_pair_tile(blob, Ws1, tcg::SW, (2 * round + jj) * tcg::NT, kb * 64, 64);
-    if (blob.size() * 2 != n_tiles * 2 * tcg::BT_BYTES) {
+            st(Box{&Ws1, tcg::SW, (2 * round) * tcg::NT, kb * 64, 64}, Box{&Ws1, tcg::SW, (2 * round + 1) * tcg::NT, kb * 64, 64});
+    if (blob.size() * 2 != n_stages * 2 * tcg::STG_BYTES) {
         set_error("tcg_prepare: internal weight-image size mismatch");
         return WM_ERR_FORMAT;
     }
@@ -778,7 +839,7 @@ int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     ctx->allocs.push_back(d_t);
     WM_CUDA_TRY(cudaMemcpy(d_t, t16.data(), t16.size() * 2, cudaMemcpyHostToDevice));
 
-    // tensor map over the image seen as rows of 64 fp16 (128 B); one box = 96 rows = one 12 KB half tile.  The
+    // tensor map over the image seen as rows of 64 fp16 (128 B); one box = 192 rows = one CTA's 24 KB of a stage.  The
     // image is already swizzled, so the map itself uses no swizzle.
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qr;
@@ -791,7 +852,7 @@ int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     CUtensorMap tm;
     const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
     const cuuint64_t strides[1] = {128};
-    const cuuint32_t box[2] = {64, (cuuint32_t)tcg::XC}, es[2] = {1, 1};
+    const cuuint32_t box[2] = {64, (cuuint32_t)(2 * tcg::XC)}, es[2] = {1, 1};
     const CUresult r = ((EncodeTiledFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, d_blob, dims, strides, box, es,
                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
