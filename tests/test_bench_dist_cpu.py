@@ -110,10 +110,11 @@ def test_gpus_flag_relaunches_under_torchrun():
 
 def test_ncu_traffic_reads_the_newest_profile(tmp_path, monkeypatch):
     import bench
-    b, src = bench.ncu_traffic(5, "wm_tcg_kernel")                     # (round 1's capture: the only one for this kernel)
-    assert b == 3450484000 + 61085952 and src == "profiles/r1_tcg_v1.md"
-    b3, src3 = bench.ncu_traffic(3, "wm_tc2_kernel")                   # two captures name this pair: the newer file wins
-    assert src3 > "profiles/r1_tc2_v4.md" and b3 > 0
+    b, src = bench.ncu_traffic(2, "wm_tc_kernel")                      # (round 1's capture: the only one for this kernel)
+    assert b == 23908352 and src == "profiles/r1_tc_v8.md"
+    for n, kern, r1 in ((3, "wm_tc2_kernel", "profiles/r1_tc2_v4.md"), (5, "wm_tcg_kernel", "profiles/r1_tcg_v1.md")):
+        b3, src3 = bench.ncu_traffic(n, kern)                          # two captures name this pair: the newer file wins
+        assert src3 > r1 and b3 > 0
     assert bench.ncu_traffic(99, "wm_tc_kernel") == (None, None)
     (tmp_path / "profiles").mkdir()
     (tmp_path / "profiles" / "r1_x.md").write_text("<!-- traffic: config=2 kernel=k dram_bytes_per_launch=10 -->")
