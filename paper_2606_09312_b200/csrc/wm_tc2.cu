@@ -46,8 +46,8 @@ constexpr int DA = 256;            // action-embedding width
 constexpr int SW = 1024;           // scorer hidden width (both hidden layers)
 constexpr int KB_BYTES = 8192;     // one A K-block: [64 rows x 64 cols] fp16, SW128 K-major
 constexpr int BT_BYTES = 16384;    // one B half tile: [128 weight rows x 64 cols] fp16, SW128 K-major (= ring stage)
-constexpr int NSTAGE = 3;
-constexpr int A1_KB = 12;          // z: 0-7, a/phi: 8-11
+constexpr int NSTAGE = 4;            // ring depth: the stand-alone issue loop reaches 66 % of the pipe with 3 stages, 85 % with 4
+constexpr int A1_KB = 10;          // z: 0-7, action / phi features: 8-9 (akb, pkb <= 2)
 constexpr int H_KB = 4;            // K-blocks of one hidden chunk buffer (256 columns)
 constexpr int HWK_BYTES = 2048;    // hw operand: one [64 x 16] no-swizzle K-major tile per K = 16 step
 constexpr int THREADS = 512;
