@@ -991,12 +991,12 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
                          ((uintptr_t)a.latents_out % 16 == 0);
     const bool prefix_call = a.start || a.init_index || a.latents_out;   // wm_rollout_latents / wm_rollout_score_from
     const bool use_pair = m.tcp_ok && (ctx->opt_pair || !m.tc1_ok);      // d = 256 models: the pair kernel takes the call
-    const bool ext_ok = m.tc_ok == 1 || m.tc_ok == 2 || m.tc_ok == 4;      // (the GRU kernel does not take the prefix-reuse calls)
+    const bool ext_ok = m.tc_ok >= 1 && m.tc_ok <= 4;                      // every tcgen05 kernel takes the prefix-reuse calls
     if (prefix_call && !ext_ok && ctx->opt_path != 2) return launch_generic(ctx, a, st);
     if (!m.tc_ok || a.T_max > 255 || !aligned || (prefix_call && !ext_ok)) {
         if (ctx->opt_path == 2) {
             set_error("tcgen05 path: needs T_max <= 255, 16-byte aligned init_states / hw_feats (and, for "
-                      "wm_rollout_latents / wm_rollout_score_from, an MLP+LayerNorm or TransH model)");
+                      "wm_rollout_latents / wm_rollout_score_from, a 16-byte aligned latents_out)");
             return WM_ERR_UNSUPPORTED;
         }
         return launch_generic(ctx, a, st);

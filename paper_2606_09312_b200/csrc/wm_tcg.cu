@@ -113,6 +113,10 @@ __device__ __forceinline__ int tile_of(int it, int pair, int np, int n_tiles) {
     return idx < n_tiles ? idx : -1;
 }
 
+// EXT = the prefix-latent reuse calls (S26; as in wm_tcp_kernel / wm_tc2_kernel): a per-candidate first position
+// `start` (the rollout covers [start, len), phi still sees [0, len)), the initial latent from a bank row, z' stored to
+// latents_out, and no scorer when scores_out is null.  Compiled out of the literal instance.
+template <bool EXT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -127,6 +131,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();          // 0 = leader (issues the MMAs)
     const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+    const bool rank_it = !EXT || p.a.scores_out != nullptr;   // EXT calls that only store latents skip the scorer in every role
 
     // ---- one-time setup
     if (threadIdx.x == 0) {
@@ -172,7 +177,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int r = lane; r < TMP; r += 32) {
                     int cand, len, seg;
                     row_meta(p.a, (int64_t)tile * TMP + r, cand, len, seg, rank == 0);
-                    nsteps = max(nsteps, len);
+                    nsteps = max(nsteps, EXT ? len - row_start(p.a, cand, len) : len);
                 }
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) nsteps = max(nsteps, __shfl_xor_sync(0xffffffffu, nsteps, o));
@@ -185,7 +190,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             }
             if (tile < 0) break;
             if (lane == 0) {
-                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + SC_STAGES;
+                const int roll_total = nsteps * ROLL_STAGES, total = roll_total + (rank_it ? SC_STAGES : 0);
                 int src = 0;
                 for (int i = 0; i < total; ++i) {
                     if (i == roll_total) src = ROLL_STAGES;
@@ -317,6 +322,11 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 wait_x(0);                                                  // blend_0 has read G_0
                 seg_a(0, true); commit(B_AFREE); seg_z(0, zlo, s_zhi, false); finish(0);   // G_1 -> X0 (still the OLD z)
             }
+            if (!rank_it) {     // no scorer: take the last z' phases so that the barrier parities stay in step
+                wait_z(0);
+                wait_z(1);
+                continue;
+            }
             // ---- scorer layer 1: four 192-column tiles of gelu(Ws0 [z_T; phi; hw] + bs0) into X2, X1, X0 and latent
             // tile 0; their fp16 outputs h1 go to the spare z K-blocks (tile 0), the r*z buffer (tiles 1, 2) and, once
             // every layer-1 MMA has completed, over z_T's K-blocks 3-5 (tile 3)
@@ -408,15 +418,19 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (tile < 0) break;
             int cand, len, seg;
             row_meta(p.a, (int64_t)tile * TMP + TMR * (int)rank + row, cand, len, seg, false);
+            // prefix-latent reuse: the rollout covers positions [st, len) and starts from the row init_index names
+            const int st = EXT ? row_start(p.a, cand, len) : 0, rem = len - st;
+            const size_t zrow = EXT ? row_init(p.a, cand, seg) : (size_t)seg;
 
-            // ---- z_0 (the task's initial latent) -> fp32 TMEM + fp16 buffer 0
+            // ---- z_0 (the task's initial latent, or the banked latent after the first st steps) -> fp32
+            // TMEM + fp16 buffer 0
 #pragma unroll 1
             for (int js = 0; js < 6; ++js) {
                 const int j = js / 3, s = js % 3;
                 const int m0 = NT * j + cb + 16 * s;
                 uint32_t v[16], o[8];
                 if (cand >= 0) {
-                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + (size_t)seg * D + m0);
+                    const float4* src = reinterpret_cast<const float4*>(p.a.init_states + zrow * D + m0);
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         const float4 f = __ldg(src + i);
@@ -437,7 +451,12 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 
             for (int t = 0; t < nsteps; ++t) {
                 uint8_t* znext = zb + ((t & 1) ^ 1) * ZH_BYTES;     // z'_0 (K-blocks 0-2); z'_1 overwrites zhi
-                const bool live = t < len;     // masked steps leave the state unchanged
+                const bool live = t < rem;     // masked steps leave the state unchanged
+                float* lat = nullptr;          // wm_rollout_latents: z after this step (or only the terminal one: [B, d])
+                if (EXT && p.a.latents_out && live) {
+                    if (!p.a.latents_terminal) lat = p.a.latents_out + ((size_t)cand * p.a.T_max + st + t) * D;
+                    else if (st + t == len - 1) lat = p.a.latents_out + (size_t)cand * D;
+                }
                 // ---- r = sigma(R_j), fp16 r*z -> the r*z operand buffer (R_0 in X2, R_1 in X1)
 #pragma unroll 1
                 for (int j = 0; j < 2; ++j) {
@@ -481,6 +500,13 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                         for (int i = 0; i < 8; ++i) o[i] = pack_f16(__uint_as_float(z[2 * i]), __uint_as_float(z[2 * i + 1]));
                         tmem_st16(T_Z + (uint32_t)(XC * j) + tcol + 16u * s, z);
                         put16(j == 0 ? znext : zhi, cb + 16 * s, o);
+                        if (EXT && lat) {
+                            float4* dst = reinterpret_cast<float4*>(lat + NT * j + cb + 16 * s);
+#pragma unroll
+                            for (int i = 0; i < 4; ++i)
+                                dst[i] = make_float4(__uint_as_float(z[4 * i]), __uint_as_float(z[4 * i + 1]),
+                                                     __uint_as_float(z[4 * i + 2]), __uint_as_float(z[4 * i + 3]));
+                        }
                     }
                     // tile j of z' is written: X0 and the H accumulator are free, R_0 of the next step may read z'_j
                     publish(r_xfree(0), r_xfree(xh), r_zready + 8u * (uint32_t)j, true);
@@ -505,6 +531,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 blend(1, 1, true);
             }
 
+            if (!rank_it) continue;
             // ---- scorer layer 1 -> h1 (fp16): tile 0 into the spare z K-blocks, tiles 1, 2 into the r*z buffer, tile 3
             // over z_T's K-blocks 3-5 (its accumulator is the last of layer 1: every MMA that reads z_T has completed)
             uint8_t* h1_0 = zb + ((nsteps & 1) ^ 1) * ZH_BYTES;
@@ -589,26 +616,25 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             float phi[16][4];
 #pragma unroll
             for (int rr = 0; rr < 16; ++rr) phi[rr][0] = phi[rr][1] = phi[rr][2] = phi[rr][3] = 0.0f;
-            // the action of step t of this lane's row, fetched one step ahead (the arrays stream from HBM)
+            // the action at position `pos` of this lane's row, fetched one step ahead (the arrays stream from HBM)
             int id_n = 0, prm_n[MAX_P];
-            auto fetch = [&](int t) {
-                if (row_lane && t < len) {
-                    id_n = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + t);
-                    const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + t) * P;
+            auto fetch = [&](int pos) {
+                if (row_lane && pos < len) {
+                    id_n = __ldg(p.a.action_ids + (size_t)cand * p.a.T_max + pos);
+                    const int32_t* pp = p.a.action_params + ((size_t)cand * p.a.T_max + pos) * P;
 #pragma unroll
                     for (int j = 0; j < MAX_P; ++j)
                         if (j < P) prm_n[j] = __ldg(pp + j);
                 }
             };
-            fetch(0);
-
-            for (int t = 0; t < nsteps; ++t) {
-                // phase 1 (row-mapped): table row of every parameter slot: (id P + j) n_b + bucket(p_j)
+            // phase 1 (row-mapped): table row of every parameter slot of the fetched action: (id P + j) n_b + bucket(p_j);
+            // -1 in slot 0 marks a row with no action at this position
+            auto index_rows = [&](bool valid) {
                 if (row_lane) {
                     int ix[MAX_P];
 #pragma unroll
                     for (int j = 0; j < MAX_P; ++j) ix[j] = 0;
-                    if (t < len) {
+                    if (valid) {
                         int id = id_n;
                         if (id < 0 || id >= p.n_types) {
                             atomicOr(p.a.fault, WM_FAULT_TYPE);
@@ -638,10 +664,10 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     *reinterpret_cast<int4*>(s_idx + row * MAX_P + 4) = make_int4(ix[4], ix[5], ix[6], ix[7]);
                 }
                 __syncwarp();
-                fetch(t + 1);
-                // phase 2 (column-mapped, lane = 4 embedding columns): all 16 rows are gathered from the table (L2) and
-                // summed in registers BEFORE the a-buffer is free, two rows' loads in flight at a time
-                uint2 pk[16];
+            };
+            // phase 2 (column-mapped, lane = 4 embedding columns): the warp's 16 rows are gathered from the table (L2) and
+            // summed in registers, two rows' loads in flight at a time; phi accumulates, pk takes the fp16 operand
+            auto gather = [&](uint2 (&pk)[16]) {
 #pragma unroll
                 for (int g = 0; g < 8; ++g) {
                     uint2 v[2][MAX_P];
@@ -676,6 +702,32 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                         pk[2 * g + q] = make_uint2(pack_f16(a4[0], a4[1]), pack_f16(a4[2], a4[3]));
                     }
                 }
+            };
+            // prefix-latent reuse: positions [0, st) only feed phi; scanned in position order BEFORE the first rollout step
+            // (the running sums then see the positions in the literal call's order: bit-identical phi)
+            const int st = (EXT && row_lane) ? row_start(p.a, cand, len) : 0;
+            if (EXT && p.a.start) {
+                int st_max = st;
+#pragma unroll
+                for (int o = 8; o > 0; o >>= 1) st_max = max(st_max, __shfl_xor_sync(0xffffffffu, st_max, o));
+                st_max = __shfl_sync(0xffffffffu, st_max, 0);
+                for (int pos = 0; pos < st_max; ++pos) {
+                    uint2 pk[16];
+                    fetch(pos);
+                    index_rows(pos < st);
+                    gather(pk);
+                    __syncwarp();   // phase 2 reads of s_idx are done before the next phase 1 overwrites
+                }
+            }
+            fetch(st);
+
+            for (int t = 0; t < nsteps; ++t) {
+                index_rows(st + t < len);
+                fetch(st + t + 1);
+                // all 16 rows are gathered BEFORE the a-buffer is free: only the stores stand between its release and the
+                // next step's a K-blocks
+                uint2 pk[16];
+                gather(pk);
                 if (n_w > 0) mbar_wait_inline(bar(B_AFREE), (n_w - 1) & 1);
                 ++n_w;
 #pragma unroll
@@ -684,6 +736,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 __syncwarp();   // also: phase 2 reads of s_idx are done before the next phase 1 overwrites
                 if (lane == 0) mbar_arrive_remote(r_aready);
             }
+            if (!rank_it) continue;
 
             // ---- phi = mean_t a_t (0 when len = 0)
             if (row_lane) s_lens[row] = len;
@@ -864,7 +917,8 @@ int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     m.tc_blob = d_blob;
     m.tc_blob_bytes = blob.size() * 2;
     m.tc_E = d_t;
-    WM_CUDA_TRY(cudaFuncSetAttribute(tcg::wm_tcg_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    WM_CUDA_TRY(cudaFuncSetAttribute(tcg::wm_tcg_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
+    WM_CUDA_TRY(cudaFuncSetAttribute(tcg::wm_tcg_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total));
     m.tc_ok = 3;
     return WM_OK;
 }
@@ -885,7 +939,8 @@ int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const tcg::SmemLayout L = tcg::smem_layout(p.hw_ksteps);
     const int max_pairs = ctx->n_sms / 2;
     const int pairs = p.n_tiles < max_pairs ? p.n_tiles : max_pairs;
-    tcg::wm_tcg_kernel<<<2 * pairs, tcg::THREADS, L.total, st>>>(p, tm);
+    if (a.start || a.init_index || a.latents_out) tcg::wm_tcg_kernel<true><<<2 * pairs, tcg::THREADS, L.total, st>>>(p, tm);
+    else tcg::wm_tcg_kernel<false><<<2 * pairs, tcg::THREADS, L.total, st>>>(p, tm);
     WM_CUDA_TRY(cudaGetLastError());
     ctx->launches.fetch_add(1);
     trace::dump(p.prof, st);

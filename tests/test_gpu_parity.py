@@ -584,7 +584,7 @@ def test_struct_phi_feature_readout(wm, n):
             np.testing.assert_array_equal(y, b.hw_feats[seg, 0])
 
 
-PREFIX_TC_VARIANTS = (1, 2, 5)       # (the TransH kernel, variant 4, takes wm_rollout_latents only)    # tcgen05 kernels that take the prefix-reuse calls; the others answer WM_ERR_UNSUPPORTED
+PREFIX_TC_VARIANTS = (1, 2, 3, 5)    # tcgen05 kernels that take the prefix-reuse calls (every one: single-CTA d = 256, d = 512 pair, GRU pair, d = 256 pair)
 
 
 def _prefix_case(n, S, per):
@@ -618,7 +618,7 @@ def test_rollout_latents_match_oracle(wm, n):
         out = torch.full((b.B, cfg.T_max, cfg.d), -777.0, dtype=torch.float32, device="cuda:0")
         call = lambda: wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"],
                                              dv["lengths"], out, dv["subgraph_offsets"])
-        if _prefix_unsupported(wm, ctx, path, call, variants=(1, 2, 4, 5)):
+        if _prefix_unsupported(wm, ctx, path, call, variants=(1, 2, 3, 4, 5)):
             continue
         call()
         assert wm.wm_check(ctx) == 0
