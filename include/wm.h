@@ -168,6 +168,26 @@ int wm_rollout_score(wm_ctx* ctx,
                      const int32_t* lengths, const float* hw_feats, float* scores_out,
                      const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream);
 
+/* wm_rollout_score for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc).  Same arguments, same scores_out (PAPER.md:215 / :162 Eq.8 / :188 Eq.12, as above).  The
+ * call's scratch — the length-sorted permutation of K1 (a0), its histogram / cursor counters and the tile counter of
+ * the single-CTA tcgen05 kernel — lives in ONE file-scope device array of the library, sized for WM_STATIC_MAX_B
+ * candidates (1 MB + 2 KB; every GPU that loads the library holds it until the process exits) instead of the
+ * per-stream workspace wm_rollout_score grows with cudaMalloc.  The entry calls no cudaMalloc / cudaFree / event or
+ * stream creation (the first launch of a kernel in a process may still load its module: call once before capturing).
+ * Every call on a device shares the array, in every context and on every stream: the counters are cleared at the
+ * start of each call (on the stream), the permutation is rewritten; two calls whose kernels can OVERLAP on the GPU
+ * (different streams without an event between them) race on it — serialise them on one stream.  Host threads are
+ * serialised by the library while they enqueue.
+ * Errors: those of wm_rollout_score; WM_ERR_ARG when B > WM_STATIC_MAX_B (the message names the limit);
+ * WM_ERR_UNSUPPORTED for WM_RANKER_FOREST models (they need a [B, d] latent buffer) and while WM_OPT_TIMING is on
+ * (it creates events). */
+#define WM_STATIC_MAX_B 262144
+int wm_rollout_score_static(wm_ctx* ctx,
+                            const float* init_states, const int32_t* action_ids, const int32_t* action_params,
+                            const int32_t* lengths, const float* hw_feats, float* scores_out,
+                            const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream);
+
 /* Prefix-latent reuse (SURVEY.md §8(b) extension and NEXT row f3; the online loop of PAPER.md:215 scores, round after
  * round, candidates that share long action prefixes with survivors of earlier rounds).  Two calls:
  *

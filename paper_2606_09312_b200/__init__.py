@@ -18,11 +18,12 @@ WM_OK, WM_ERR_ARG, WM_ERR_IO, WM_ERR_FORMAT, WM_ERR_CUDA, WM_ERR_UNSUPPORTED = 0
 WM_MAX_T, WM_MAX_K = 256, 1024
 WM_FAULT_LEN, WM_FAULT_TYPE, WM_FAULT_PARAM, WM_FAULT_INDEX, WM_FAULT_RANGE = 1, 2, 4, 8, 16
 WM_OPT_PATH, WM_OPT_SORT, WM_OPT_TIMING, WM_OPT_PAIR = 1, 2, 3, 4
+WM_STATIC_MAX_B = 262144   # wm_rollout_score_static: candidates the static scratch holds
 PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 
 # every symbol include/wm.h declares
 ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
-               "wm_rollout_latents", "wm_rollout_score_from",
+               "wm_rollout_latents", "wm_rollout_score_from", "wm_rollout_score_static",
                "wm_check", "wm_score_topk_host", "wm_score_topk_host_compact", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error")
 
 
@@ -65,6 +66,8 @@ def lib() -> ctypes.CDLL:
     L.wm_set_option.restype = ctypes.c_int
     L.wm_rollout_score.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, vp]
     L.wm_rollout_score.restype = ctypes.c_int
+    L.wm_rollout_score_static.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, vp]
+    L.wm_rollout_score_static.restype = ctypes.c_int
     L.wm_rollout_latents.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, vp]
     L.wm_rollout_score_from.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i64, vp]
     L.wm_rollout_latents.restype = ctypes.c_int
@@ -141,6 +144,18 @@ def wm_rollout_score(ctx: int, init_states, action_ids, action_params, lengths, 
     _check(lib().wm_rollout_score(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
                                   _ptr(hw_feats), _ptr(scores_out), _ptr(subgraph_offsets), B, S, T_max,
                                   _stream(stream)))
+
+
+def wm_rollout_score_static(ctx: int, init_states, action_ids, action_params, lengths, hw_feats, scores_out,
+                            subgraph_offsets=None, stream=None) -> None:
+    """wm_rollout_score without any allocation: the call's scratch is a static device array of the library, shared by
+    every call on the device (B <= WM_STATIC_MAX_B; calls that overlap on the GPU race).  include/wm.h."""
+    B = int(lengths.numel())
+    T_max = int(action_ids.shape[1]) if action_ids is not None and action_ids.dim() == 2 else 0
+    S = int(subgraph_offsets.numel()) - 1 if subgraph_offsets is not None else 0
+    _check(lib().wm_rollout_score_static(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
+                                         _ptr(hw_feats), _ptr(scores_out), _ptr(subgraph_offsets), B, S, T_max,
+                                         _stream(stream)))
 
 
 def wm_rollout_latents(ctx: int, init_states, action_ids, action_params, lengths, latents_out,

@@ -562,6 +562,73 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
     return run_rollout(ctx, a, st, "wm_rollout_score");
 }
 
+// ---- wm_rollout_score_static: the allocation-free entry (include/wm.h).  Its scratch is this file-scope device array:
+// [kCounterInts] counters (histogram, cursors, tile counter) followed by the permutation of up to WM_STATIC_MAX_B
+// candidates.  In host code the NAME of a __device__ array is a host-side stand-in, not a device address: the address the
+// kernels get comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr int kStaticPermOff = (kCounterInts + 63) / 64 * 64;   // keeps the permutation 256-byte aligned
+static __device__ __align__(256) int32_t g_static_scratch[kStaticPermOff + WM_STATIC_MAX_B];
+static std::mutex g_static_mu;                 // one call at a time enqueues on the shared scratch
+static int32_t* g_static_ptr[64] = {};         // per device: the array's device address
+
+int wm_rollout_score_static(wm_ctx* ctx, const float* init_states, const int32_t* action_ids,
+                            const int32_t* action_params, const int32_t* lengths, const float* hw_feats,
+                            float* scores_out, const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max,
+                            void* cuda_stream) {
+    if (!ctx) {
+        set_error("wm_rollout_score_static: null ctx");
+        return WM_ERR_ARG;
+    }
+    if (!sizes_ok("wm_rollout_score_static", B, S, T_max)) return WM_ERR_ARG;
+    if (B > WM_STATIC_MAX_B) {
+        set_error("wm_rollout_score_static: B = %lld exceeds the static scratch (WM_STATIC_MAX_B = %d candidates); "
+                  "use wm_rollout_score",
+                  (long long)B, (int)WM_STATIC_MAX_B);
+        return WM_ERR_ARG;
+    }
+    if (ctx->m.ranker_kind == WM_RANKER_FOREST || ctx->opt_timing) {
+        set_error("wm_rollout_score_static: not available for WM_RANKER_FOREST models or with WM_OPT_TIMING on");
+        return WM_ERR_UNSUPPORTED;
+    }
+    if (B == 0) return WM_OK;
+    if (!init_states || !lengths || !scores_out || (ctx->m.H > 0 && !hw_feats) ||
+        (T_max > 0 && (!action_ids || !action_params)) || (subgraph_offsets && S < 1)) {
+        set_error("wm_rollout_score_static: null pointer (or S < 1 with offsets) for a non-empty batch");
+        return WM_ERR_ARG;
+    }
+    if (ctx->device < 0 || ctx->device >= 64) {
+        set_error("wm_rollout_score_static: device ordinal %d out of range", ctx->device);
+        return WM_ERR_ARG;
+    }
+    WM_CUDA_TRY(cudaSetDevice(ctx->device));
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[ctx->device]) {
+        int32_t* ptr = nullptr;
+        WM_CUDA_TRY(cudaGetSymbolAddress((void**)&ptr, g_static_scratch));
+        g_static_ptr[ctx->device] = ptr;
+    }
+    nvtx::Range nr("wm_rollout_score_static");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Workspace ws;                    // a view of the static array: nothing in it is owned, grown or freed
+    ws.stream = st;
+    ws.counters = g_static_ptr[ctx->device];
+    ws.perm = g_static_ptr[ctx->device] + kStaticPermOff;
+    ws.perm_cap = WM_STATIC_MAX_B;
+    CallArgs a = {};
+    a.init_states = init_states; a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
+    a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets;
+    a.B = B; a.S = S; a.T_max = T_max;
+    a.fault = ctx->fault;
+    // the steps of run_rollout_locked without its growing / event-creating branches: K1 clears the counters it starts
+    // from (cudaMemsetAsync on the stream) and rewrites the permutation; the single-CTA kernel clears its tile counter
+    if (ctx->opt_sort && B > 256) {
+        const int rc = launch_length_bucketing(ctx, &ws, a.lengths, nullptr, a.B, a.T_max, st);
+        if (rc != WM_OK) return rc;
+        a.perm = ws.perm;
+    }
+    return pick_path(ctx) == 2 ? launch_tc(ctx, &ws, a, st) : launch_generic(ctx, a, st);
+}
+
 int wm_rollout_latents(wm_ctx* ctx, const float* init_states, const int32_t* action_ids, const int32_t* action_params,
                        const int32_t* lengths, const int32_t* subgraph_offsets, float* latents_out, int64_t B,
                        int32_t S, int32_t T_max, void* cuda_stream) {
