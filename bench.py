@@ -147,17 +147,27 @@ class ClockSampler:
         bits = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
         get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
             getattr(pynvml, "nvmlDeviceGetCurrentClocksThrottleReasons")
+        # two pollers: NVML's power and reasons queries take several ms each, the clock query about one; a single loop over
+        # all three saw ONE sample of a 10 ms timed region
+        def slow():
+            while not self.stop_flag:
+                try:
+                    self.power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                    r = int(get_reasons(h))
+                    for name, bit in bits.items():
+                        if r & bit:
+                            self.reasons.add(name)
+                except Exception:     # noqa: BLE001
+                    pass
+                time.sleep(self.period)
+        self.thread2 = threading.Thread(target=slow, daemon=True)
+        self.thread2.start()
         while not self.stop_flag:
             try:
                 self.sm.append(float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
-                self.power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
-                r = int(get_reasons(h))
-                for name, bit in bits.items():
-                    if r & bit:
-                        self.reasons.add(name)
             except Exception:     # noqa: BLE001
                 pass
-            time.sleep(self.period)
+            time.sleep(self.period / 4)
 
     def _read_cli(self):
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
@@ -182,13 +192,15 @@ class ClockSampler:
         self.stop_flag = True
         if self.thread is not None:
             self.thread.join(1.0)
+        if getattr(self, "thread2", None) is not None:
+            self.thread2.join(1.0)
         sm = sorted(self.sm)
         # "under load" = the upper half of the samples (the sampler also sees the idle gaps between steps)
         load = sm[len(sm) // 2:] if sm else []
         return {"sm_mhz": float(np.median(load)) if load else None, "sm_min_mhz": sm[0] if sm else None,
                 "sm_max_mhz": self.mx, "power_w_max": max(self.power) if self.power else None,
                 "reasons": sorted(self.reasons), "samples": len(sm),
-                "source": "nvml poll 2 ms" if self.nvml else "nvidia-smi -lms 20"}
+                "source": "nvml poll (clock 0.5 ms, power / reasons 2 ms between queries)" if self.nvml else "nvidia-smi -lms 20"}
 
 
 def cpu_baseline(cfg, n_subgraphs: int):
