@@ -559,6 +559,43 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
         const int rc = run_rollout_locked(ctx, ws, r, st);
         return rc != WM_OK ? rc : launch_forest(ctx, ws->zt, a, scores_out, st);
     }
+    if (ctx->m.phi_kind == WM_PHI_TYPED && pick_path(ctx) == 2 && B <= 0x7fffffffLL / ctx->m.d &&
+        (uintptr_t)init_states % 16 == 0 && T_max > 0 && T_max <= 255) {
+        // per-type phi (S28) on a model the pair kernel can roll: 609 running statistics per row do not fit beside a
+        // 256-row tile, so K2 (tcgen05) stores the terminal latents [B, d] and the fp32 kernel takes them as per-candidate
+        // initial latents with start = len: it walks every position for phi only (no transition step) and runs the scorer
+        WM_CUDA_TRY(cudaSetDevice(ctx->device));
+        Workspace* ws = acquire_ws(ctx, st);
+        if (!ws) {
+            set_error("wm_rollout_score: cannot allocate workspace");
+            return WM_ERR_CUDA;
+        }
+        std::lock_guard<std::mutex> lk(ws->mu);
+        nvtx::Range nr("wm_rollout_score");
+        const size_t need = (size_t)B * ctx->m.d;
+        if (ws->zt_cap < need) {
+            if (ws->zt) {
+                WM_CUDA_TRY(cudaStreamSynchronize(st));
+                WM_CUDA_TRY(cudaFree(ws->zt));
+                ws->zt = nullptr;
+                ws->zt_cap = 0;
+            }
+            WM_CUDA_TRY(cudaMalloc(&ws->zt, (need + need / 4 + 1024) * sizeof(float)));
+            ws->zt_cap = need + need / 4 + 1024;
+        }
+        CallArgs r = a;
+        r.scores_out = nullptr; r.latents_out = ws->zt; r.latents_terminal = true;
+        int rc = run_rollout_locked(ctx, ws, r, st);
+        if (rc != WM_OK) return rc;
+        CallArgs sc = a;
+        sc.fault = ctx->fault;
+        sc.perm = (ctx->opt_sort && a.B > 256) ? ws->perm : nullptr;   // K1's order by length serves both passes
+        sc.cand_latents = ws->zt;     // (rows of length 0 stored no latent: they keep init_states, their z_T = z_0)
+        sc.start = a.lengths;
+        rc = launch_generic(ctx, sc, st);
+        if (rc == WM_OK && ctx->opt_timing && ws->ev1) WM_CUDA_TRY(cudaEventRecord(ws->ev1, st));
+        return rc;
+    }
     return run_rollout(ctx, a, st, "wm_rollout_score");
 }
 

@@ -303,7 +303,8 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
                     }
                     zrow = (size_t)bi;
                 }
-                v = __ldg(a.init_states + zrow * d + j);
+                v = (a.cand_latents && m_len[r] > 0) ? __ldg(a.cand_latents + (size_t)m_cand[r] * d + j)
+                                                     : __ldg(a.init_states + zrow * d + j);
             }
             X[(size_t)j * R + r] = v;
         }

@@ -155,6 +155,8 @@ struct CallArgs {
     int64_t n_init;             // rows of init_states when init_index is used (indices are clamped to it)
     float* latents_out;         // [B, T_max, d] z after step t+1 at [b][t] for start <= t < len; scores_out may be null
     bool latents_terminal;      // latents_out is [B, d]: only the latent after the LAST step (t = len - 1) is stored
+    const float* cand_latents;  // [B, d] (fp32 kernel only): a candidate with len > 0 starts from its own row of this array
+                                // instead of its init_states row (the second pass of a WM_PHI_TYPED model, wm_api.cu)
 };
 
 // Quarter-octave bucket floor(4 log2 p) of a parameter p >= 1, exact for every int32 p (S10): with

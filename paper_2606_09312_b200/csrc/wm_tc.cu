@@ -868,8 +868,9 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
         if (rc != WM_OK || m.tc_ok) return rc;
         const int rc2 = tcg_prepare(ctx, hv, names);
         if (rc2 != WM_OK || m.tc_ok) return rc2;
-        // TransH models (NEXT row f1): the TransH step of the pair kernel (tc_ok 4: no single-CTA form)
-        if (m.kind == WM_KIND_TRANSH) {
+        // TransH models (NEXT row f1): the TransH step of the pair kernel (tc_ok 4: no single-CTA form); models with the
+        // per-type phi (S28): the pair kernel for the rollout, the fp32 kernel for phi + scorer (wm_rollout_score)
+        if (m.kind == WM_KIND_TRANSH || m.phi_kind == WM_PHI_TYPED) {
             const int rc4 = tcp_prepare(ctx, hv, names);
             if (rc4 != WM_OK) return rc4;
             if (m.tcp_ok) m.tc_ok = 4;
@@ -993,6 +994,15 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const bool use_pair = m.tcp_ok && (ctx->opt_pair || !m.tc1_ok);      // d = 256 models: the pair kernel takes the call
     const bool ext_ok = m.tc_ok >= 1 && m.tc_ok <= 4;                      // every tcgen05 kernel takes the prefix-reuse calls
     if (prefix_call && !ext_ok && ctx->opt_path != 2) return launch_generic(ctx, a, st);
+    // per-type phi: the tcgen05 kernels hold no scorer for it; a call that wants scores from them (wm_rollout_score_from,
+    // wm_rollout_score_static; wm_rollout_score splits the call itself) runs on the fp32 kernel
+    if (m.phi_kind == WM_PHI_TYPED && a.scores_out) {
+        if (ctx->opt_path == 2) {
+            set_error("tcgen05 path: a WM_PHI_TYPED model is scored by wm_rollout_score only");
+            return WM_ERR_UNSUPPORTED;
+        }
+        return launch_generic(ctx, a, st);
+    }
     if (!m.tc_ok || a.T_max > 255 || !aligned || (prefix_call && !ext_ok)) {
         if (ctx->opt_path == 2) {
             set_error("tcgen05 path: needs T_max <= 255, 16-byte aligned init_states / hw_feats (and, for "

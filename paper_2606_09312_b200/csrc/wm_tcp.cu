@@ -1117,9 +1117,11 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 }  // namespace
 
 bool tcp_model_ok(const Model& m) {
-    return m.phi_kind <= WM_PHI_STRUCT && (m.kind == WM_KIND_MLP_LN || m.kind == WM_KIND_TRANSH) && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tcp::D &&
+    // per-type phi (WM_PHI_TYPED, S28): this kernel rolls such a model and hands the terminal latents to the fp32 kernel, which
+    // builds phi and runs the scorer (wm_api.cu): no scorer shape to match, as for the forest ranker
+    return m.phi_kind <= WM_PHI_TYPED && (m.kind == WM_KIND_MLP_LN || m.kind == WM_KIND_TRANSH) && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_LINEAR && m.d == tcp::D &&
            m.d_a == tcp::DA && m.hidden >= 256 && m.hidden <= tcp::MAX_HID && m.hidden % 128 == 0 &&
-           ((m.n_lin == 3 && m.sdim[1] == tcp::SW && m.sdim[2] == tcp::SW) || m.ranker_kind == WM_RANKER_FOREST) &&
+           ((m.n_lin == 3 && m.sdim[1] == tcp::SW && m.sdim[2] == tcp::SW) || m.ranker_kind == WM_RANKER_FOREST || m.phi_kind == WM_PHI_TYPED) &&
            m.H >= 8 && m.H <= tcp::MAX_H && m.H % 8 == 0 && m.n_types <= tcp::MAX_TYPES && m.P <= tcp::MAX_P;
 }
 
@@ -1135,7 +1137,8 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     };
     const std::vector<float>&W1 = get("W1"), &W2 = get("W2"), &b1 = get("b1"), &E = get("E"), &Wp = get("W_p"), &bpv = get("b_p");
     const std::vector<float>& b2h = get("b2");
-    const bool forest = m.ranker_kind == WM_RANKER_FOREST, transh = m.kind == WM_KIND_TRANSH;
+    // `forest` = the kernel's MLP scorer is never run for this model (zero image): forest ranker, or per-type phi
+    const bool forest = m.ranker_kind == WM_RANKER_FOREST || m.phi_kind == WM_PHI_TYPED, transh = m.kind == WM_KIND_TRANSH;
     const int hid = m.hidden, NC = hid / 128, K1 = tcp::D + tcp::DA, NT = m.n_types, P = m.P;
     // ---- A matrix that multiplies the action embedding, folded onto the action features f = [onehot(id) (NT) | log2 p_j (P) | 1]:
     //      M (E[id] + W_p lp + b_p) + bias  =  (M E^T)[:, id] + (M W_p) lp + (M b_p + bias); products summed in double
@@ -1327,7 +1330,7 @@ int launch_tcp(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     p.akb = m.tcp_akb; p.pkb = m.tcp_pkb;
     p.b2 = m.b2; p.gamma = m.gamma; p.beta = m.beta;
     p.bs1 = m.bs[1]; p.w3 = m.Wst[2]; p.bs2 = m.bs[2];
-    if (m.ranker_kind == WM_RANKER_FOREST) p.bs1 = p.w3 = p.bs2 = m.zeros;   // (unused scorer, zero image)
+    if (m.ranker_kind == WM_RANKER_FOREST || m.phi_kind == WM_PHI_TYPED) p.bs1 = p.w3 = p.bs2 = m.zeros;   // (unused scorer, zero image)
     p.a = a;
     p.n_tiles = (int)((a.B + tcp::TMP - 1) / tcp::TMP);
     p.prof = trace::begin(st);

@@ -673,6 +673,49 @@ def test_score_from_bank_matches_literal(wm, n):
         assert oracle.score_error(y, lit, b.subgraph_offsets) <= same, (n, path)
 
 
+def test_typed_phi_model_splits_the_call_and_keeps_prefix_reuse(wm):
+    """A WM_PHI_TYPED model with cfg 2's shapes (config 14): wm_rollout_score rolls on the pair kernel (tc_variant 5) and
+    ranks on the fp32 kernel from the terminal latents (rows of length 0 keep z_0); wm_rollout_score_from, which the
+    tcgen05 kernels cannot rank for this phi, runs on the fp32 kernel under the automatic policy and is refused
+    (WM_ERR_UNSUPPORTED) when the tcgen05 path is forced."""
+    import torch
+    cfg = gen.get_config(14).scaled(S=3, per_subgraph=300)
+    w, b = gen.make_weights(cfg), gen.make_inputs(cfg)
+    b.lengths[:7] = 0                                   # zero-length rows in the first tile and ...
+    b.lengths[-3:] = 0                                  # ... in the ragged last one
+    ref = oracle_scores(cfg, w, b)
+    ctx = _ctx(wm, cfg)
+    info = wm.wm_get_info(ctx)
+    assert info.path == 2 and info.tc_variant == 5 and info.phi_kind == 2
+    n0 = wm.wm_launch_count(ctx)
+    y = gpu_scores(ctx, b)
+    assert wm.wm_launch_count(ctx) - n0 == 4            # K1 (two launches), the pair kernel, the fp32 phi + scorer pass
+    assert oracle.score_error(y, ref, b.subgraph_offsets) <= TOL[False]
+    ov, _ = oracle.topk_overlap(gpu_topk(y, b.subgraph_offsets, cfg.k), oracle.topk_segments(ref, b.subgraph_offsets, cfg.k))
+    assert ov >= 0.95
+    # prefix reuse: bank every latent, score from random cuts
+    dv = to_device(b)
+    bank = torch.zeros((cfg.S + b.B * cfg.T_max, cfg.d), dtype=torch.float32, device="cuda:0")
+    bank[:cfg.S] = dv["init_states"]
+    wm.wm_rollout_latents(ctx, dv["init_states"], dv["action_ids"], dv["action_params"], dv["lengths"],
+                          bank[cfg.S:].view(b.B, cfg.T_max, cfg.d), dv["subgraph_offsets"])
+    rng = np.random.default_rng(77)
+    st = np.minimum(rng.integers(0, cfg.T_max + 1, b.B), b.lengths).astype(np.int32)
+    seg = np.repeat(np.arange(cfg.S), cfg.per_subgraph)
+    index = np.where(st == 0, seg, cfg.S + np.arange(b.B) * cfg.T_max + st - 1).astype(np.int32)
+    out = torch.full((b.B,), float("nan"), dtype=torch.float32, device="cuda:0")
+    args = (bank, torch.from_numpy(index).cuda(), torch.from_numpy(st).cuda(), dv["action_ids"], dv["action_params"],
+            dv["lengths"], dv["hw_feats"], out, dv["subgraph_offsets"])
+    wm.wm_rollout_score_from(ctx, *args)
+    assert wm.wm_check(ctx) == 0
+    assert oracle.score_error(out.cpu().numpy(), ref, b.subgraph_offsets) <= TOL[False]
+    wm.wm_set_option(ctx, wm.WM_OPT_PATH, wm.PATH_TCGEN05)
+    with pytest.raises(wm.WmError) as e:
+        wm.wm_rollout_score_from(ctx, *args)
+    assert e.value.code == wm.WM_ERR_UNSUPPORTED
+    wm.wm_free(ctx)
+
+
 @pytest.mark.parametrize("form", [None, PATH_TC_SINGLE])
 def test_cfg4_prefix_reuse_full_family_structure(wm, form):
     """cfg 4's shared-prefix structure used the way a search loop would (bench.py --prefix-reuse): one representative per
