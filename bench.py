@@ -57,6 +57,8 @@ def _kernel_name(info) -> str:
     if info.path == 2 and info.phi_kind == 2:
         # per-type phi: the pair kernel rolls, the fp32 kernel builds phi and ranks; the second pass dominates the step
         return "wm_generic_kernel"
+    if info.path != 2 and info.kind in (0, 1) and info.embed == 0 and info.phi_kind == 0 and info.dtype == 0 and info.d <= 256:
+        return "wm_small_kernel (<= 592 candidates) / wm_generic_kernel"     # csrc/wm_generic.cu: small_call_ok
     return KERNELS.get(info.tc_variant, "wm_tc_kernel") if info.path == 2 else "wm_generic_kernel"
 
 

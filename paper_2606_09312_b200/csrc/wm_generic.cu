@@ -182,6 +182,27 @@ __device__ __forceinline__ int find_segment(const int32_t* __restrict__ off, int
     return lo;
 }
 
+// Weights-in-shared-memory modes: one thread issues the bulk async copies (TMA engine) of every matrix and vector the
+// residual-MLP step and the scorer read; `bar` (initialised, count 1) completes when all of them have landed.
+__device__ __forceinline__ void stage_weights(const GenericParams& p, float* wreg, uint32_t bar) {
+    ptx::mbar_arrive_expect_tx(bar, p.ws_bytes);
+    ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_w1), p.W1t, (uint32_t)((size_t)(p.d + p.da) * p.hidden * 4), bar);
+    ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_w2), p.W2t, (uint32_t)((size_t)p.hidden * p.d * 4), bar);
+    for (int l = 0; l < p.n_lin; ++l) {
+        ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_s[l]), p.Wst[l], (uint32_t)((size_t)p.sdim[l] * p.sdim[l + 1] * 4), bar);
+        ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_bs[l]), p.bs[l], (uint32_t)(((size_t)p.sdim[l + 1] * 4 + 15) & ~15u), bar);
+    }
+    ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_E), p.E, (uint32_t)((size_t)p.n_types * p.da * 4), bar);
+    ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_Wp), p.WpT, (uint32_t)((size_t)p.P * p.da * 4), bar);
+    ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_bp), p.bp, (uint32_t)((size_t)p.da * 4), bar);
+    ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_b1), p.b1, (uint32_t)((size_t)p.hidden * 4), bar);
+    ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_b2), p.b2, (uint32_t)((size_t)p.d * 4), bar);
+    if (p.kind == WM_KIND_MLP_LN) {
+        ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_g), p.gamma, (uint32_t)((size_t)p.d * 4), bar);
+        ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_be), p.beta, (uint32_t)((size_t)p.d * 4), bar);
+    }
+}
+
 constexpr int kGenericThreads = 256;
 static_assert(kSplitThreads == kGenericThreads, "linear_T_split spreads K over the whole CTA");
 
@@ -232,22 +253,7 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
         if (tid == 0) {
             ptx::mbar_init(bar, 1);
             ptx::fence_barrier_init();
-            ptx::mbar_arrive_expect_tx(bar, p.ws_bytes);
-            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_w1), p.W1t, (uint32_t)((size_t)(p.d + p.da) * p.hidden * 4), bar);
-            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_w2), p.W2t, (uint32_t)((size_t)p.hidden * p.d * 4), bar);
-            for (int l = 0; l < p.n_lin; ++l) {
-                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_s[l]), p.Wst[l], (uint32_t)((size_t)p.sdim[l] * p.sdim[l + 1] * 4), bar);
-                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_bs[l]), p.bs[l], (uint32_t)(((size_t)p.sdim[l + 1] * 4 + 15) & ~15u), bar);
-            }
-            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_E), p.E, (uint32_t)((size_t)p.n_types * p.da * 4), bar);
-            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_Wp), p.WpT, (uint32_t)((size_t)p.P * p.da * 4), bar);
-            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_bp), p.bp, (uint32_t)((size_t)p.da * 4), bar);
-            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_b1), p.b1, (uint32_t)((size_t)p.hidden * 4), bar);
-            ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_b2), p.b2, (uint32_t)((size_t)p.d * 4), bar);
-            if (p.kind == WM_KIND_MLP_LN) {
-                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_g), p.gamma, (uint32_t)((size_t)p.d * 4), bar);
-                ptx::bulk_g2s(ptx::smem_u32(wreg + p.ws_be), p.beta, (uint32_t)((size_t)p.d * 4), bar);
-            }
+            stage_weights(p, wreg, bar);
         }
         __syncthreads();
         ptx::mbar_wait(bar, 0);
@@ -568,6 +574,237 @@ __global__ void __launch_bounds__(kGenericThreads) wm_generic_kernel(const Gener
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// K2-small: ONE CTA (four warps) PER CANDIDATE, for search-round-sized calls of a small residual-MLP model (BASELINE.json
+// cfg 1: 64 candidates, T_max 8; PAPER.md:21 works with 64-trial budgets).  Such a call is bound by the LATENCY of its
+// serial chain (T_max steps x two matrix-vector products), not by throughput: in wm_generic_kernel<4, true> a step costs
+// about eight block barriers and ~8 K cycles on 16 of the 148 SMs.  Here every candidate gets an SM of its own: the
+// weights are staged once per CTA by bulk async copies (as in the WS mode above); a matrix-vector product is split over
+// the four warps by K (one warp per scheduler, each streams a quarter of the matrix from shared memory: a lone warp is
+// bound by the latency of its own loads, measured 2.3 us per step for both products), a lane owns the output units
+// [NPL lane, NPL lane + NPL) so that a weight row is one conflict-free vector load per lane, inputs are float4
+// broadcasts; the four partial sums meet in shared memory.  Four 128-thread barriers per step.
+constexpr int kSmallWarps = 4;
+constexpr int kSmallMaxB = 592;     // four candidates per SM; beyond that the tiled kernel's reuse of a weight read over R rows wins
+constexpr int kSmallMaxW = 256;     // widest layer: 8 output units per lane
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// part[n] = sum over k in [k0, k1) of Wt[k][n] in[k] for the N = 32 NPL output units; Wt ([K][N]), in, part in shared
+// memory, 16-byte aligned; k0, k1 multiples of 4.  Two accumulator sets (even / odd k) halve the dependent-FMA chain.
+template <int NPL>
+__device__ __forceinline__ void warp_partial_n(const float* Wt, const float* in, int k0, int k1, float* part, int lane) {
+    constexpr int N = 32 * NPL;
+    float acc[2][NPL];
+#pragma unroll
+    for (int i = 0; i < NPL; ++i) acc[0][i] = acc[1][i] = 0.0f;
+    const float* wl = Wt + NPL * lane;
+#pragma unroll 2
+    for (int k = k0; k < k1; k += 4) {
+        const float4 x = *reinterpret_cast<const float4*>(in + k);
+        const float xv[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            float w[NPL];
+            const float* r = wl + (size_t)(k + u) * N;
+            if (NPL == 1) {
+                w[0] = r[0];
+            } else if (NPL == 2) {
+                const float2 t = *reinterpret_cast<const float2*>(r);
+                w[0] = t.x; w[1] = t.y;
+            } else {
+#pragma unroll
+                for (int q = 0; q < NPL / 4; ++q) {
+                    const float4 t = *reinterpret_cast<const float4*>(r + 4 * q);
+                    w[4 * q] = t.x; w[4 * q + 1] = t.y; w[4 * q + 2] = t.z; w[4 * q + 3] = t.w;
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < NPL; ++i) acc[u & 1][i] = fmaf(w[i], xv[u], acc[u & 1][i]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < NPL; ++i) part[NPL * lane + i] = acc[0][i] + acc[1][i];
+}
+
+// The CTA's product out = act(bias + Wt^T in) for N in {32, 64, 128, 256}: warp w takes the w-th quarter of K (in groups of
+// four rows) into part[w][.]; after a barrier thread n (and n + 128) adds the four partial sums and the bias.  Called by all
+// 128 threads; ends with a barrier (out is complete, part is free again).
+template <int ACT>
+__device__ __forceinline__ void cta_linear(const float* Wt, const float* bias, const float* in, int K, int N, float* out,
+                                           float* part, int maxw, int warp, int lane) {
+    const int groups = K >> 2, g0 = (groups * warp) / kSmallWarps, g1 = (groups * (warp + 1)) / kSmallWarps;
+    float* mine = part + (size_t)warp * maxw;
+    switch (N) {
+        case 32: warp_partial_n<1>(Wt, in, 4 * g0, 4 * g1, mine, lane); break;
+        case 64: warp_partial_n<2>(Wt, in, 4 * g0, 4 * g1, mine, lane); break;
+        case 128: warp_partial_n<4>(Wt, in, 4 * g0, 4 * g1, mine, lane); break;
+        default: warp_partial_n<8>(Wt, in, 4 * g0, 4 * g1, mine, lane); break;
+    }
+    __syncthreads();
+    for (int n = threadIdx.x; n < N; n += kSmallWarps * 32)
+        out[n] = apply_act<ACT>((part[n] + part[maxw + n]) + (part[2 * maxw + n] + part[3 * maxw + n]) + bias[n]);
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kSmallWarps * 32) wm_small_kernel(const GenericParams p) {
+    extern __shared__ __align__(16) float smem[];
+    const int d = p.d, da = p.da, H = p.H, P = p.P, K1 = d + da;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // weight region first (ws_off = 0), its barrier, then xs [d | da | H] (4-float aligned), hb, yb [maxw], part [4][maxw]
+    float* wreg = smem;
+    uint64_t* wbar = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(smem) + p.ws_bytes);
+    const int xs_len = (d + da + H + 3) & ~3;
+    float* xs = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(smem) + p.ws_bytes + 16);
+    float* hb = xs + xs_len;
+    float* yb = hb + p.maxw;
+    float* part = yb + p.maxw;
+    const uint32_t bar = ptx::smem_u32(wbar);
+    if (tid == 0) {
+        ptx::mbar_init(bar, 1);
+        ptx::fence_barrier_init();
+        stage_weights(p, wreg, bar);
+    }
+    __syncthreads();
+    const CallArgs& a = p.a;
+    const float *W1t = wreg + p.ws_w1, *W2t = wreg + p.ws_w2, *pE = wreg + p.ws_E, *pWp = wreg + p.ws_Wp,
+                *pbp = wreg + p.ws_bp, *pb1 = wreg + p.ws_b1, *pb2 = wreg + p.ws_b2, *pg = wreg + p.ws_g, *pbe = wreg + p.ws_be;
+    const int dj = (d + 31) >> 5, aj = (da + 31) >> 5;
+    bool staged = false;
+    for (int64_t i = blockIdx.x; i < a.B; i += gridDim.x) {
+        const int cand = a.perm ? __ldg(a.perm + i) : (int)i;
+        int len = __ldg(a.lengths + cand);
+        if (len < 0 || len > a.T_max) {
+            if (tid == 0) atomicOr(a.fault, WM_FAULT_LEN);
+            len = len < 0 ? 0 : a.T_max;
+        }
+        const int seg = a.offsets ? find_segment(a.offsets, a.S, cand) : cand;
+        // z_0 and the hardware features (the loads fly while the weights land)
+        for (int n = tid; n < d; n += kSmallWarps * 32) xs[n] = __ldg(a.init_states + (size_t)seg * d + n);
+        for (int n = tid; n < H; n += kSmallWarps * 32) xs[K1 + n] = __ldg(a.hw_feats + (size_t)seg * H + n);
+        float phi[8];      // warp 1: running sum of the embedding columns lane, lane + 32, ...
+#pragma unroll
+        for (int j = 0; j < 8; ++j) phi[j] = 0.0f;
+        if (!staged) {
+            ptx::mbar_wait(bar, 0);
+            staged = true;
+        }
+        // warp 1 writes a_t = E[id] + W_p log2 p + b_p (a1) into xs[d ..): `fetch` issues the step's global loads (a product
+        // earlier than `embed` needs them), `embed` runs beside warp 0's latent update
+        int id_n = 0, prm_n = 1;
+        auto fetch = [&](int t) {
+            id_n = __ldg(a.action_ids + (size_t)cand * a.T_max + t);
+            if (lane < P) prm_n = __ldg(a.action_params + ((size_t)cand * a.T_max + t) * P + lane);
+        };
+        auto embed = [&]() {
+            int id = id_n;
+            if (id < 0 || id >= p.n_types) {
+                if (lane == 0) atomicOr(a.fault, WM_FAULT_TYPE);
+                id = id < 0 ? 0 : p.n_types - 1;
+            }
+            float lp = 0.0f;
+            if (lane < P) {
+                int prm = prm_n;
+                if (prm < 1) {
+                    atomicOr(a.fault, WM_FAULT_PARAM);
+                    prm = 1;
+                }
+                lp = log2f((float)prm);
+            }
+            float lq[8];       // log2 p_q of this step, q < P <= 8
+#pragma unroll
+            for (int q = 0; q < 8; ++q) lq[q] = __shfl_sync(0xffffffffu, lp, q);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int n = lane + 32 * j;
+                if (j < aj && n < da) {
+                    float v = pE[(size_t)id * da + n] + pbp[n];
+#pragma unroll
+                    for (int q = 0; q < 8; ++q)
+                        if (q < P) v = fmaf(pWp[(size_t)q * da + n], lq[q], v);
+                    xs[d + n] = v;
+                    phi[j] += v;     // a4: running sum for phi
+                }
+            }
+        };
+        if (warp == 1 && len > 0) {
+            fetch(0);
+            embed();
+        }
+        __syncthreads();
+        for (int t = 0; t < len; ++t) {
+            // ---- a2: z' = z + W2 gelu(W1 [z; a] + b1) + b2 (, LayerNorm)
+            cta_linear<ACT_GELU>(W1t, pb1, xs, K1, p.hidden, hb, part, p.maxw, warp, lane);
+            if (warp == 1 && t + 1 < len) fetch(t + 1);
+            cta_linear<ACT_NONE>(W2t, pb2, hb, p.hidden, d, yb, part, p.maxw, warp, lane);
+            if (warp == 1) {        // (the a-part of xs was last read by the first product of this step)
+                if (t + 1 < len) embed();
+            } else if (warp == 0) {
+                float v[8];
+                float s = 0.0f;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int n = lane + 32 * j;
+                    v[j] = (j < dj && n < d) ? xs[n] + yb[n] : 0.0f;
+                    s += v[j];
+                }
+                if (p.kind == WM_KIND_MLP_LN) {     // two-pass LayerNorm, as in wm_generic_kernel
+                    const float mean = warp_sum(s) / (float)d;
+                    float q = 0.0f;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int n = lane + 32 * j;
+                        const float c = (j < dj && n < d) ? v[j] - mean : 0.0f;
+                        q = fmaf(c, c, q);
+                    }
+                    const float rstd = 1.0f / sqrtf(warp_sum(q) / (float)d + p.ln_eps);
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int n = lane + 32 * j;
+                        if (j < dj && n < d) xs[n] = fmaf(pg[n], (v[j] - mean) * rstd, pbe[n]);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int n = lane + 32 * j;
+                        if (j < dj && n < d) xs[n] = v[j];
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        // ---- a4/a5: x = [z_T ; phi ; hw], scorer MLP; a6: the score goes to the candidate's slot
+        if (warp == 1) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int n = lane + 32 * j;
+                if (j < aj && n < da) xs[d + n] = len > 0 ? phi[j] / (float)len : 0.0f;
+            }
+        }
+        __syncthreads();
+        const float* in = xs;
+        for (int l = 0; l + 1 < p.n_lin; ++l) {
+            float* out = (l & 1) ? yb : hb;
+            cta_linear<ACT_GELU>(wreg + p.ws_s[l], wreg + p.ws_bs[l], in, p.sdim[l], p.sdim[l + 1], out, part, p.maxw, warp, lane);
+            in = out;
+        }
+        if (warp == 0) {      // the output unit: lanes split K, then a warp reduction
+            const int l = p.n_lin - 1;
+            const float* Ws = wreg + p.ws_s[l];
+            float acc = 0.0f;
+            for (int k = lane; k < p.sdim[l]; k += 32) acc = fmaf(Ws[k], in[k], acc);
+            acc = warp_sum(acc);
+            if (lane == 0) a.scores_out[cand] = acc + wreg[p.ws_bs[l]];
+        }
+        __syncthreads();      // xs / hb / yb are rewritten by the next candidate
+    }
+    if (!staged) ptx::mbar_wait(bar, 0);     // (a CTA without a candidate may not leave before its copies have landed)
+}
+
 static int generic_as_rows(const Model& m) {
     const int typed = m.n_types + 2 * m.n_types * m.P;
     return m.phi_kind == WM_PHI_TYPED && typed > m.d_a ? typed : m.d_a;
@@ -642,6 +879,45 @@ static size_t weights_in_smem(const wm_ctx* ctx, GenericParams* p, size_t tile_b
     return total;
 }
 
+// K2-small takes the call when it is small and plain: a model of the weights-in-shared-memory class (checked by the
+// caller), mean-embedding phi, every layer at most kSmallMaxW wide and a multiple of 4 (float4 broadcasts), no
+// prefix-reuse arguments, at most kSmallMaxB candidates.
+static size_t small_smem_bytes(const Model& m, const GenericParams& p) {
+    const int xs_len = (m.d + m.d_a + m.H + 3) & ~3;
+    return (size_t)p.ws_bytes + 16 + (size_t)(xs_len + (2 + kSmallWarps) * p.maxw) * 4;
+}
+
+static bool small_call_ok(const wm_ctx* ctx, const CallArgs& a, const GenericParams& p) {
+    const Model& m = ctx->m;
+    if (small_smem_bytes(m, p) > (size_t)ctx->smem_optin) return false;
+    if (a.B > kSmallMaxB || !a.scores_out || a.start || a.init_index || a.latents_out || a.cand_latents) return false;
+    if (m.phi_kind != WM_PHI_MEAN || m.P > 8) return false;
+    auto w32 = [](int n) { return n == 32 || n == 64 || n == 128 || n == 256; };    // widths warp_linear_n is built for
+    bool ok = w32(m.d) && w32(m.hidden) && m.d_a <= kSmallMaxW && (m.d + m.d_a) % 4 == 0 && p.maxw % 4 == 0 &&
+              m.sdim[m.n_lin] == 1 && m.sdim[0] % 4 == 0 && m.sdim[0] <= 4 * kSmallMaxW;
+    for (int l = 1; l < m.n_lin; ++l) ok &= w32(m.sdim[l]);
+    return ok;
+}
+
+static int launch_small(wm_ctx* ctx, GenericParams p, cudaStream_t st) {
+    const Model& m = ctx->m;
+    p.ws_off = 0;
+    const size_t smem = small_smem_bytes(m, p);
+    static std::atomic<int> granted[16];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    dev &= 15;
+    if (granted[dev].load(std::memory_order_relaxed) < (int)smem) {
+        WM_CUDA_TRY(cudaFuncSetAttribute(wm_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        granted[dev].store((int)smem, std::memory_order_relaxed);
+    }
+    const int grid = (int)(p.a.B < ctx->n_sms ? p.a.B : ctx->n_sms);     // one candidate per CTA, one CTA per SM
+    wm_small_kernel<<<grid, kSmallWarps * 32, smem, st>>>(p);
+    WM_CUDA_TRY(cudaGetLastError());
+    ctx->launches.fetch_add(1);
+    return WM_OK;
+}
+
 static int pick_R(const wm_ctx* ctx, int64_t B, size_t* smem_out, int* maxw, int* alt) {
     // Largest tile that fits shared memory; small batches take smaller tiles so the (latency-bound) work
     // spreads over the SMs.
@@ -695,6 +971,7 @@ int launch_generic(wm_ctx* ctx, const CallArgs& a, cudaStream_t st) {
     p.ws_E = p.ws_Wp = p.ws_bp = p.ws_b1 = p.ws_b2 = p.ws_g = p.ws_be = 0;
     for (int i = 0; i < kMaxScorerLinears; ++i) p.ws_s[i] = p.ws_bs[i] = 0;
     const size_t ws_total = weights_in_smem(ctx, &p, smem);
+    if (ws_total && small_call_ok(ctx, a, p)) return launch_small(ctx, p, st);
     if (ws_total) {       // one CTA per SM (the weights take most of its shared memory), each walks its tiles
         const int grid = p.n_tiles < ctx->n_sms ? p.n_tiles : ctx->n_sms;
         switch (R) {
