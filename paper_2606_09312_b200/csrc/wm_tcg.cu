@@ -15,8 +15,8 @@
 // shared memory: z'_0 goes to the OTHER of two buffers of K-blocks 0-2, because G_1 still reads the old z while z'_0 is
 // written; z'_1 overwrites K-blocks 3-5 in place, G_1 having completed before blend_1 starts).  z'_0 and z'_1 are
 // published separately, so R_0 of step t+1 runs its first five K-blocks (z'_0 and a_{t+1}) under blend_1 of step t.
-// A stage is TWO [192 x 64] weight tiles (8 MMAs per wait / commit: the issuing warp, not the tensor pipe, was the
-// limiter with one tile per stage) taken from a ring of seven one-tile slots (3.5 stages in flight).  Everything else — weight ring fed by TMA into both CTAs with completion on
+// A ring stage is TWO [192 x 64] weight tiles (8 MMAs per wait / commit: the issuing warp, not the tensor pipe, was
+// the limiter with one tile per stage).  Everything else — weight ring fed by TMA into both CTAs with completion on
 // the leader's barrier, multicast commits, remote arrivals, static serpentine tile schedule, scorer on the same
 // machinery — is as in wm_tc2.cu.
 // Warp roles per CTA (512 threads): warps 0-7 epilogue (q = warp % 4: rows 32 (q & 1) + lane, N half q / 2; e = warp / 4:
@@ -49,9 +49,7 @@ constexpr int XC = NT / 2;         // TMEM columns per tile and CTA
 constexpr int KB_BYTES = 8192;     // one A K-block: [64 rows x 64 cols] fp16, SW128 K-major
 constexpr int BT_BYTES = 12288;    // one B half tile: [96 weight rows x 64 cols] fp16, SW128 K-major
 constexpr int STG_BYTES = 2 * BT_BYTES;   // a ring stage: two half tiles per CTA
-constexpr int NSLOT = 7;            // ring slots of ONE tile (12 KB per CTA): 3.5 stages.  Stand-alone, the ring + issue loop
-                                    // reaches 82 % of the pipe with 3 stages of two tiles and 99.9 % with 4; shared memory has
-                                    // room for 7 tiles, so slots are per tile and a stage takes the next two (wrapping)
+constexpr int NSTAGE = 3;
 constexpr int Z_KB = 6, A_KB = 2;  // K-blocks of the z part / the a (phi) part of an operand
 constexpr int ZH_KB = Z_KB / 2;    // K-blocks of one 192-column latent tile
 constexpr int ZH_BYTES = ZH_KB * KB_BYTES;
@@ -67,9 +65,9 @@ constexpr uint32_t IDESC_G = idesc_pair(NT);
 constexpr int NXB = 5;             // accumulators: X0, X1, X2 and, in the scorer, the two (dead) latent tiles
 
 enum {
-    B_FULL = 0,                    // [NSLOT] TMA (both CTAs) -> leader's MMA warp
-    B_EMPTY = B_FULL + NSLOT,      // [NSLOT] MMA commit (multicast) -> each CTA's producer
-    B_XFULL = B_EMPTY + NSLOT,    // [NXB] MMA commit -> epilogue: accumulator b filled
+    B_FULL = 0,                    // [NSTAGE] TMA (both CTAs) -> leader's MMA warp
+    B_EMPTY = B_FULL + NSTAGE,     // [NSTAGE] MMA commit (multicast) -> each CTA's producer
+    B_XFULL = B_EMPTY + NSTAGE,    // [NXB] MMA commit -> epilogue: accumulator b filled
     B_XFREE = B_XFULL + NXB,       // [NXB] epilogue (both CTAs) -> leader MMA: accumulator b read, its output written
     B_ZREADY = B_XFREE + NXB,      // [2] epilogue (both CTAs) -> leader MMA: z' tile 0 / tile 1 written
     B_AFREE = B_ZREADY + 2,                       // MMA commit -> action warps: a-part no longer read
@@ -98,9 +96,9 @@ __host__ __device__ inline SmemLayout smem_layout(int hw_ksteps) {
     L.zbuf = o; o += 3 * ZH_BYTES;                     // fp16 z operand: K-blocks 0-2 twice (double-buffered), then 3-5
     L.abuf = o; o += A_KB * KB_BYTES;                  // fp16 a_t / phi
     L.rz = o; o += ZB_BYTES;                           // fp16 r*z
-    L.ring = o; o += NSLOT * BT_BYTES;
+    L.ring = o; o += NSTAGE * STG_BYTES;
     L.hwk = o; o += (uint32_t)hw_ksteps * HWK_BYTES;
-    L.idx = o; o += TMR * MAX_P * 2;                   // table row (16 bits) of every parameter slot of the step
+    L.idx = o; o += TMR * MAX_P * 4;                   // table row of every parameter slot of the step
     L.lens = o; o += TMR * 4;
     L.red = o; o += 4 * TMR * 4;                       // [4 column parts][64 rows] float
     L.bars = o; o += B_COUNT * 8;
@@ -137,7 +135,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 
     // ---- one-time setup
     if (threadIdx.x == 0) {
-        for (int i = 0; i < NSLOT; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 1); }
+        for (int i = 0; i < NSTAGE; ++i) { mbar_init(bar(B_FULL + i), 1); mbar_init(bar(B_EMPTY + i), 1); }
         for (int i = 0; i < NXB; ++i) { mbar_init(bar(B_XFULL + i), 1); mbar_init(bar(B_XFREE + i), 16); }
         for (int i = 0; i < 2; ++i) { mbar_init(bar(B_SFULL + i), 1); mbar_init(bar(B_SEMPTY + i), 13); }
         mbar_init(bar(B_ZREADY), 16);
@@ -197,15 +195,12 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 for (int i = 0; i < total; ++i) {
                     if (i == roll_total) src = ROLL_STAGES;
                     else if (i < roll_total && src == ROLL_STAGES) src = 0;
-#pragma unroll
-                    for (int j = 0; j < 2; ++j) {      // the stage's two tiles, a slot each
-                        mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
-                        // the leader's barrier collects both CTAs' halves of the [192 x 64] tile
-                        if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2 * BT_BYTES);
-                        tma_load_2sm(s_ring + stage * BT_BYTES, &tmap, 0, XC * (2 * (2 * src + j) + (int)rank), bar(B_FULL + stage));
-                        if (++stage == NSLOT) { stage = 0; ph ^= 1; }
-                    }
+                    mbar_wait(bar(B_EMPTY + stage), ph ^ 1);
+                    // the leader's barrier collects both CTAs' halves of the stage's two [192 x 64] tiles
+                    if (rank == 0) mbar_arrive_expect_tx(bar(B_FULL + stage), 2 * STG_BYTES);
+                    tma_load_2sm(s_ring + stage * STG_BYTES, &tmap, 0, 2 * XC * (2 * src + (int)rank), bar(B_FULL + stage));
                     ++src;
+                    if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
                 }
             }
             __syncwarp();
@@ -228,34 +223,26 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                 tc_fence_after();
             }
         };
-        // `stage`, `ph`: slot and phase of the current stage's FIRST tile; its second tile is in the next slot
-        auto slot2 = [&]() -> uint32_t { return stage + 1 == NSLOT ? 0u : stage + 1; };
         auto wait_full = [&]() {
             WM_TRACE(1);
             mbar_wait(bar(B_FULL + stage), ph);
-            mbar_wait(bar(B_FULL + slot2()), stage + 1 == NSLOT ? ph ^ 1u : ph);
             WM_TRACE(2);
             tc_fence_after();
         };
         auto advance = [&]() {
             __syncwarp();
             WM_TRACE(3);
-            stage += 2;
-            if (stage >= NSLOT) { stage -= NSLOT; ph ^= 1; }
-        };
-        auto commit_empty = [&]() {      // (elected lane) both slots of the stage go back to the producers
-            mma_commit2(bar(B_EMPTY + stage));
-            mma_commit2(bar(B_EMPTY + slot2()));
+            if (++stage == NSTAGE) { stage = 0; ph ^= 1; }
         };
         // A ring stage holds two [192 x 64] B tiles; each goes against one [64(+64) x 64] A K-block: 4 MMAs of K = 16.
         // tile_mma is called by the elected lane only.
         auto tile_mma = [&](uint32_t d_tmem, uint32_t a_tile, int i, bool first) {
-            const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + (i == 0 ? stage : slot2()) * BT_BYTES);
+            const uint64_t a0 = smem_desc(a_tile), b0 = smem_desc(s_ring + stage * STG_BYTES + i * BT_BYTES);
 #pragma unroll
             for (int j = 0; j < 4; ++j) mma_ss2(d_tmem, a0 + 2u * j, b0 + 2u * j, IDESC_G, (first && j == 0) ? 0u : 1u);
         };
         auto stage_end = [&]() {
-            if (elect_one()) commit_empty();
+            if (elect_one()) mma_commit2(bar(B_EMPTY + stage));
             advance();
         };
         // both tiles of the stage in one go: (accumulator, A K-block) x 2
@@ -264,7 +251,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
             if (elect_one()) {
                 tile_mma(d0, a_tile0, 0, first0);
                 tile_mma(d1, a_tile1, 1, first1);
-                commit_empty();
+                mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
         };
@@ -274,11 +261,11 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         };
         auto stage_hw = [&](uint32_t d_tmem) {       // the stage's second tile is padding
             wait_full();
-            const uint64_t b0 = smem_desc(s_ring + stage * BT_BYTES);
+            const uint64_t b0 = smem_desc(s_ring + stage * STG_BYTES);
             if (elect_one()) {
                 for (int j = 0; j < p.hw_ksteps; ++j)
                     mma_ss2(d_tmem, smem_desc_nosw(s_hwk + j * HWK_BYTES), b0 + 2u * j, IDESC_G, 1u);
-                commit_empty();
+                mma_commit2(bar(B_EMPTY + stage));
             }
             advance();
         };
@@ -609,7 +596,7 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
         const bool row_lane = lane < 16;
         const int col4 = 4 * lane;
         uint8_t* ab = smem + L.abuf;
-        uint16_t* s_idx = reinterpret_cast<uint16_t*>(smem + L.idx);      // 0xFFFF in slot 0: no action at this position
+        int* s_idx = reinterpret_cast<int*>(smem + L.idx);
         int* s_lens = reinterpret_cast<int*>(smem + L.lens);
         const uint32_t r_aready = mapa(bar(B_AREADY), 0);
         const int P = p.P, NB = p.n_buckets;
@@ -673,9 +660,8 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
                     } else {
                         ix[0] = -1;
                     }
-                    *reinterpret_cast<uint4*>(s_idx + row * MAX_P) =
-                        make_uint4((uint32_t)(ix[0] & 0xffff) | ((uint32_t)ix[1] << 16), (uint32_t)ix[2] | ((uint32_t)ix[3] << 16),
-                                   (uint32_t)ix[4] | ((uint32_t)ix[5] << 16), (uint32_t)ix[6] | ((uint32_t)ix[7] << 16));
+                    *reinterpret_cast<int4*>(s_idx + row * MAX_P) = make_int4(ix[0], ix[1], ix[2], ix[3]);
+                    *reinterpret_cast<int4*>(s_idx + row * MAX_P + 4) = make_int4(ix[4], ix[5], ix[6], ix[7]);
                 }
                 __syncwarp();
             };
@@ -689,10 +675,10 @@ wm_tcg_kernel(const Params p, const __grid_constant__ CUtensorMap tmap) {
 #pragma unroll
                     for (int q = 0; q < 2; ++q) {
                         const int r = 16 * aw + 2 * g + q;
-                        const uint4 iv = *reinterpret_cast<const uint4*>(s_idx + r * MAX_P);
-                        on[q] = (iv.x & 0xffffu) != 0xffffu;
-                        const int ix[8] = {(int)(iv.x & 0xffffu), (int)(iv.x >> 16), (int)(iv.y & 0xffffu), (int)(iv.y >> 16),
-                                           (int)(iv.z & 0xffffu), (int)(iv.z >> 16), (int)(iv.w & 0xffffu), (int)(iv.w >> 16)};
+                        const int4 i0 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P);
+                        const int4 i1 = *reinterpret_cast<const int4*>(s_idx + r * MAX_P + 4);
+                        on[q] = i0.x >= 0;
+                        const int ix[8] = {i0.x, i0.y, i0.z, i0.w, i1.x, i1.y, i1.z, i1.w};
 #pragma unroll
                         for (int j = 0; j < MAX_P; ++j)
                             if (j < P && on[q]) v[q][j] = __ldg(reinterpret_cast<const uint2*>(p.Tbl + (size_t)ix[j] * DA + col4));
@@ -810,8 +796,8 @@ struct Box {
     int ld, n0, k0, kvalid;
 };
 
-// Append one stage = two tiles.  Image of a tile: the leader CTA's 12 KB (weight rows 0-95), then its peer's (rows 96-191),
-// each half in the SW128 K-major shared-memory image, fp16; tile B follows tile A.
+// Append one ring stage = two tiles.  Image of a stage: the leader CTA's 24 KB (weight rows 0-95 of tile A, then of tile
+// B), then its peer's (rows 96-191 of A, of B); every 12 KB half tile in the SW128 K-major shared-memory image, fp16.
 // Returns false when a weight is not finite in fp16 (|w| > 65504): the model then stays on the fp32 kernel.
 bool append_stage(std::vector<uint16_t>& blob, const Box& A, const Box& B) {
     const size_t base = blob.size();
@@ -825,7 +811,7 @@ bool append_stage(std::vector<uint16_t>& blob, const Box& A, const Box& B) {
             for (int k = 0; k < 64; ++k) {
                 const float v = k < bx[i]->kvalid ? W[(size_t)(bx[i]->n0 + n) * bx[i]->ld + bx[i]->k0 + k] : 0.0f;
                 const int nn = n % tcg::XC;
-                const size_t off = (size_t)i * tcg::STG_BYTES + (size_t)(n / tcg::XC) * tcg::BT_BYTES + (size_t)nn * 128 +
+                const size_t off = (size_t)(n / tcg::XC) * tcg::STG_BYTES + (size_t)i * tcg::BT_BYTES + (size_t)nn * 128 +
                                    (size_t)((((k >> 3) ^ (nn & 7)) << 4)) + (size_t)(k & 7) * 2;
                 uint16_t hb;
                 ok &= f32_to_f16_bits(v, &hb);
@@ -845,7 +831,7 @@ bool tcg_model_ok(const Model& m) {
     return m.kind == WM_KIND_GRU && m.phi_kind == WM_PHI_MEAN && m.dtype == WM_DTYPE_BF16 && m.embed == WM_EMBED_BUCKET && m.d == tcg::D &&
            m.d_a == tcg::DA && m.n_lin == 3 && m.sdim[1] == tcg::SW && m.sdim[2] == tcg::SW && m.H >= 8 &&
            m.H <= tcg::MAX_H && m.H % 8 == 0 && m.P >= 1 && m.P <= tcg::MAX_P && m.n_buckets >= 1 &&
-           m.n_buckets <= tcg::MAX_BUCKETS && (long long)m.n_types * m.P * m.n_buckets < 65535;   // (16-bit table rows in shared memory)
+           m.n_buckets <= tcg::MAX_BUCKETS;
 }
 
 int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
@@ -906,7 +892,7 @@ int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     ctx->allocs.push_back(d_t);
     WM_CUDA_TRY(cudaMemcpy(d_t, t16.data(), t16.size() * 2, cudaMemcpyHostToDevice));
 
-    // tensor map over the image seen as rows of 64 fp16 (128 B); one box = 96 rows = one CTA's 12 KB half of a tile.  The
+    // tensor map over the image seen as rows of 64 fp16 (128 B); one box = 192 rows = one CTA's 24 KB of a stage.  The
     // image is already swizzled, so the map itself uses no swizzle.
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qr;
@@ -919,7 +905,7 @@ int tcg_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     CUtensorMap tm;
     const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
     const cuuint64_t strides[1] = {128};
-    const cuuint32_t box[2] = {64, (cuuint32_t)tcg::XC}, es[2] = {1, 1};
+    const cuuint32_t box[2] = {64, (cuuint32_t)(2 * tcg::XC)}, es[2] = {1, 1};
     const CUresult r = ((EncodeTiledFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, d_blob, dims, strides, box, es,
                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
