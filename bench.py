@@ -55,8 +55,8 @@ KERNELS = {1: "wm_tc_kernel", 2: "wm_tc2_kernel", 3: "wm_tcg_kernel", 5: "wm_tcp
 def _kernel_name(info) -> str:
     """The rollout+score kernel (K2) the library runs for this model, by its CUDA name."""
     if info.path == 2 and info.phi_kind == 2:
-        # per-type phi: the pair kernel rolls, the fp32 kernel builds phi and ranks; the second pass dominates the step
-        return "wm_generic_kernel"
+        # per-type phi: the pair kernel rolls, wm_typed_x_kernel writes the scorer's input rows, wm_tsc_kernel ranks
+        return "wm_tcp_kernel + wm_tsc_kernel"
     if info.path != 2 and info.kind in (0, 1) and info.embed == 0 and info.phi_kind == 0 and info.dtype == 0 and info.d <= 256:
         return "wm_small_kernel (<= 592 candidates) / wm_generic_kernel"     # csrc/wm_generic.cu: small_call_ok
     return KERNELS.get(info.tc_variant, "wm_tc_kernel") if info.path == 2 else "wm_generic_kernel"
@@ -381,7 +381,7 @@ class Leg:
             # cfg 1: 12 MFLOP / 10 KB, launch-latency-bound; report the achieved HBM GB/s as north_star asks
             roof = {"bound": "hbm", "achieved": bytes_in / (k_ms * 1e-3) / 1e9, "peak": pk["hbm"], "unit": "GB/s",
                     "traffic": None, "note": "latency-bound tiny config; neither roofline applies"}
-        elif info.path == 2 and info.phi_kind != 2:
+        elif info.path == 2:
             tr, src = ncu_traffic(cfg.number, _kernel_name(info))
             roof = {"bound": "tensor", "achieved": achieved, "peak": pk["bf16"], "unit": "TFLOP/s",
                     "traffic": tr, "traffic_source": src, "frac_of_sustained_peak": achieved / pk["bf16_sustained"],
@@ -392,13 +392,6 @@ class Leg:
             alu_peak = 148 * 128 * 2 * (pk.get("sm_max_mhz", 1965.0) * 1e6) / 1e12
             roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "traffic": None,
                     "traffic_source": None, "note": "fp32 FFMA peak derived from unit counts and the SM clock"}
-            if info.path == 2:
-                # per-type phi: two launches (pair kernel: rollout; fp32 kernel: phi + scorer).  The line describes the
-                # fp32 pass, the larger one: its FLOPs are the scorer's, its time is at most the measured total
-                flops = float(self.B) * cfg.flops_scorer()
-                roof["achieved"] = flops / (k_ms * 1e-3) / 1e12
-                roof["note"] += ("; split call: rollout on wm_tcp_kernel + phi / scorer on wm_generic_kernel, kernel_ms is "
-                                 "their sum, achieved = scorer FLOPs / kernel_ms (a lower bound for the fp32 pass)")
         roof["frac"] = roof["achieved"] / roof["peak"]
         roof.update({"kernel": _kernel_name(info), "kernel_ms": k_ms,
                      "peak_source": pk["source"] + " (burst: kernel timed alone)",

@@ -79,8 +79,9 @@ extern "C" {
 #define WM_PHI_TYPED    2      /* phi = [c_k (n_types) | len | per type k: s_kj (P) | m_kj (P) | x_kj (P)]: the numeric  */
                                /* statistics kept PER ACTION TYPE, over the steps of that type, 0 for a type that does   */
                                /* not occur ("action-specific numeric attributes"; S28).         */
-                               /* n_types (1 + 3P) + 1 values, no relation to d_a; phi and the scorer run on the fp32   */
-                               /* kernel (wm_rollout_score rolls on the tcgen05 pair kernel first where the model fits)  */
+                               /* n_types (1 + 3P) + 1 values, no relation to d_a.  wm_rollout_score of a model the pair   */
+                               /* kernel can roll (d = 256, scorer 512 / 512) is rollout + input rows + a tcgen05 ranking   */
+                               /* MLP (three launches); other shapes run on the fp32 kernel                                */
 
 /* wm_set_option keys */
 #define WM_RANKER_MLP    0     /* G = the configs' MLP                                                              */

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libwm.so")
-SOURCES = ["wm_api.cu", "wm_bucket.cu", "wm_forest.cu", "wm_generic.cu", "wm_tc.cu", "wm_tcp.cu", "wm_tc2.cu", "wm_tcg.cu", "wm_topk.cu"]
+SOURCES = ["wm_api.cu", "wm_bucket.cu", "wm_forest.cu", "wm_generic.cu", "wm_tc.cu", "wm_tcp.cu", "wm_tc2.cu", "wm_tcg.cu", "wm_tsc.cu", "wm_topk.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC]

@@ -360,6 +360,7 @@ void wm_free(wm_ctx* ctx) {
         if (w->counters) cudaFree(w->counters);
         if (w->stage) cudaFree(w->stage);
         if (w->zt) cudaFree(w->zt);
+        if (w->xbuf) cudaFree(w->xbuf);
         if (w->ev0) cudaEventDestroy(w->ev0);
         if (w->ev1) cudaEventDestroy(w->ev1);
         delete w;
@@ -587,6 +588,25 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
         r.scores_out = nullptr; r.latents_out = ws->zt; r.latents_terminal = true;
         int rc = run_rollout_locked(ctx, ws, r, st);
         if (rc != WM_OK) return rc;
+        if (ctx->m.tsc_ok) {
+            // the ranking MLP on tcgen05: wm_typed_x_kernel writes the fp16 rows [z_T | phi | 1 | h], wm_tsc_kernel ranks them
+            const size_t xneed = tsc_x_bytes(ctx, B);
+            if (ws->xbuf_cap < xneed) {
+                if (ws->xbuf) {
+                    WM_CUDA_TRY(cudaStreamSynchronize(st));
+                    WM_CUDA_TRY(cudaFree(ws->xbuf));
+                    ws->xbuf = nullptr;
+                    ws->xbuf_cap = 0;
+                }
+                WM_CUDA_TRY(cudaMalloc(&ws->xbuf, xneed + xneed / 4 + 4096));
+                ws->xbuf_cap = xneed + xneed / 4 + 4096;
+            }
+            CallArgs xa = a;
+            xa.fault = ctx->fault;
+            rc = launch_tsc(ctx, ws->zt, ws->xbuf, xa, scores_out, st);
+            if (rc == WM_OK && ctx->opt_timing && ws->ev1) WM_CUDA_TRY(cudaEventRecord(ws->ev1, st));
+            return rc;
+        }
         CallArgs sc = a;
         sc.fault = ctx->fault;
         sc.perm = (ctx->opt_sort && a.B > 256) ? ws->perm : nullptr;   // K1's order by length serves both passes

@@ -64,6 +64,10 @@ struct Model {
     int tcp_akb = 1, tcp_pkb = 1;   // wm_tcp_kernel: K-blocks of the folded action features / phi features
     int tcp_ok = 0;            // 1 = wm_tcp_kernel (the CTA-pair, M = 256 form of wm_tc_kernel) is built for this model too
     alignas(64) unsigned char tcp_tmap[128] = {};   // CUtensorMap over wm_tcp_kernel's own weight image
+    int tsc_ok = 0;            // 1 = wm_tsc_kernel (tcgen05 ranking MLP over a precomputed input row: WM_PHI_TYPED models)
+    int tsc_nkb = 0;           // K-blocks of its input row [z_T | phi | 1 | h]
+    void* tsc_blob = nullptr;  // its weight image
+    alignas(64) unsigned char tsc_tmap[128] = {};   // CUtensorMap over tsc_blob
 };
 
 // NVTX range around an ABI call (header-only NVTX 3: a no-op unless a profiler injects itself)
@@ -89,6 +93,9 @@ struct Workspace {
     // terminal latents [B, d] handed from K2 to the forest kernel (WM_RANKER_FOREST)
     float* zt = nullptr;
     size_t zt_cap = 0;
+    // fp16 input rows of the tcgen05 ranking MLP (wm_tsc.cu; WM_PHI_TYPED models)
+    void* xbuf = nullptr;
+    size_t xbuf_cap = 0;
     // WM_OPT_TIMING
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool timed = false;
@@ -214,6 +221,14 @@ int launch_tcg(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st);
 
 // K4 (wm_forest.cu): tree-ensemble ranker over [z_T ; structured phi ; h] (NEXT row f4)
 int launch_forest(wm_ctx* ctx, const float* zT, const CallArgs& a, float* scores_out, cudaStream_t st);
+
+// wm_tsc.cu: the ranking MLP on tcgen05 for WM_PHI_TYPED models the pair kernel can roll (d = 256, scorer 512 / 512).
+// tsc_prepare builds the weight image at load time (m.tsc_ok); launch_tsc turns the terminal latents zT [B, d] and the
+// action arrays into the fp16 input rows X (caller-provided, tsc_x_bytes(B) bytes) and ranks them: two launches.
+int tsc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& host_tensors_by_name_order,
+                const std::vector<std::string>& names);
+size_t tsc_x_bytes(const wm_ctx* ctx, int64_t B);
+int launch_tsc(wm_ctx* ctx, const float* zT, void* X, const CallArgs& a, float* scores_out, cudaStream_t st);
 
 // K3 (wm_topk.cu)
 int64_t topk_launches();

@@ -874,6 +874,10 @@ int tc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std
             const int rc4 = tcp_prepare(ctx, hv, names);
             if (rc4 != WM_OK) return rc4;
             if (m.tcp_ok) m.tc_ok = 4;
+            if (m.tcp_ok && m.phi_kind == WM_PHI_TYPED) {      // ... and the tcgen05 ranking MLP over [z_T | phi | h] rows
+                const int rc5 = tsc_prepare(ctx, hv, names);
+                if (rc5 != WM_OK) return rc5;
+            }
         }
         return WM_OK;
     }

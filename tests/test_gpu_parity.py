@@ -674,8 +674,9 @@ def test_score_from_bank_matches_literal(wm, n):
 
 
 def test_typed_phi_model_splits_the_call_and_keeps_prefix_reuse(wm):
-    """A WM_PHI_TYPED model with cfg 2's shapes (config 14): wm_rollout_score rolls on the pair kernel (tc_variant 5) and
-    ranks on the fp32 kernel from the terminal latents (rows of length 0 keep z_0); wm_rollout_score_from, which the
+    """A WM_PHI_TYPED model with cfg 2's shapes (config 14): wm_rollout_score rolls on the pair kernel (tc_variant 5), writes
+    the scorer's fp16 input rows [z_T | phi | 1 | h] and ranks them on the tcgen05 ranking-MLP kernel (rows of length 0 keep
+    z_0; the batch's last tile is ragged: rows past B read as zero and are not written); wm_rollout_score_from, which the
     tcgen05 kernels cannot rank for this phi, runs on the fp32 kernel under the automatic policy and is refused
     (WM_ERR_UNSUPPORTED) when the tcgen05 path is forced."""
     import torch
@@ -689,7 +690,7 @@ def test_typed_phi_model_splits_the_call_and_keeps_prefix_reuse(wm):
     assert info.path == 2 and info.tc_variant == 5 and info.phi_kind == 2
     n0 = wm.wm_launch_count(ctx)
     y = gpu_scores(ctx, b)
-    assert wm.wm_launch_count(ctx) - n0 == 4            # K1 (two launches), the pair kernel, the fp32 phi + scorer pass
+    assert wm.wm_launch_count(ctx) - n0 == 5            # K1 (two launches), the pair kernel, wm_typed_x_kernel, wm_tsc_kernel
     assert oracle.score_error(y, ref, b.subgraph_offsets) <= TOL[False]
     ov, _ = oracle.topk_overlap(gpu_topk(y, b.subgraph_offsets, cfg.k), oracle.topk_segments(ref, b.subgraph_offsets, cfg.k))
     assert ov >= 0.95
