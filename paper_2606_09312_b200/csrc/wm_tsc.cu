@@ -341,10 +341,15 @@ __global__ void __launch_bounds__(kXWarps * 32) wm_typed_x_kernel(const XParams 
                     int id = __ldg(p.ids + (size_t)c * p.T_max + t0 + lane);
                     ids[lane] = id < 0 ? 0 : (id >= NT ? NT - 1 : id);
                 }
-                const int32_t* pp = p.params + ((size_t)c * p.T_max + t0) * P;
-                for (int e = lane; e < nt * P; e += 32) {
-                    const int prm = __ldg(pp + e);
-                    l2s[(e / P) * 8 + e % P] = log2f((float)(prm < 1 ? 1 : prm));
+                if (lane < nt) {      // lane = step of the chunk: its P parameters -> log2 p (MUFU.LG2, 2 ulp in fp32: the features
+                                      // are stored as fp16, 11 bits)
+                    const int32_t* pp = p.params + ((size_t)c * p.T_max + t0 + lane) * P;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j)
+                        if (j < P) {
+                            const int prm = __ldg(pp + j);
+                            l2s[lane * 8 + j] = __log2f((float)(prm < 1 ? 1 : prm));
+                        }
                 }
                 __syncwarp();
                 for (int t = 0; t < nt; ++t) {
