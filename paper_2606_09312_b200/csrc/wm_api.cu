@@ -514,6 +514,70 @@ static bool sizes_ok(const char* who, int64_t B, int32_t S, int32_t T_max) {
     return true;
 }
 
+// Per-type phi (S28) on a model the pair kernel can roll: 609 running statistics per row do not fit beside a 256-row tile,
+// so the call is split.  K2 (tcgen05, EXT instance) rolls the candidates — from z_0, or from a bank row and a start
+// position for wm_rollout_score_from — and stores the terminal latents [B, d]; then either the tcgen05 ranking MLP
+// (wm_typed_x_kernel writes the fp16 rows [z_T | phi | 1 | h], wm_tsc_kernel ranks them) or, where that kernel is not
+// built for the model, the fp32 kernel with the latents as per-candidate initial latents and start = len (it walks every
+// position for phi only).  A prefix call takes the split only with the tcgen05 ranking MLP (the fp32 kernel runs such a
+// call whole).
+static bool typed_split_applies(const wm_ctx* ctx, const CallArgs& a, bool prefix_call) {
+    return ctx->m.phi_kind == WM_PHI_TYPED && ctx->m.ranker_kind == WM_RANKER_MLP && pick_path(ctx) == 2 &&
+           a.B <= 0x7fffffffLL / ctx->m.d && (uintptr_t)a.init_states % 16 == 0 && a.T_max > 0 && a.T_max <= 255 &&
+           (!prefix_call || ctx->m.tsc_ok);
+}
+
+static int typed_split_score(wm_ctx* ctx, const CallArgs& a, cudaStream_t st, const char* who) {
+    WM_CUDA_TRY(cudaSetDevice(ctx->device));
+    Workspace* ws = acquire_ws(ctx, st);
+    if (!ws) {
+        set_error("%s: cannot allocate workspace", who);
+        return WM_ERR_CUDA;
+    }
+    std::lock_guard<std::mutex> lk(ws->mu);
+    nvtx::Range nr(who);
+    const size_t need = (size_t)a.B * ctx->m.d;
+    if (ws->zt_cap < need) {
+        if (ws->zt) {
+            WM_CUDA_TRY(cudaStreamSynchronize(st));
+            WM_CUDA_TRY(cudaFree(ws->zt));
+            ws->zt = nullptr;
+            ws->zt_cap = 0;
+        }
+        WM_CUDA_TRY(cudaMalloc(&ws->zt, (need + need / 4 + 1024) * sizeof(float)));
+        ws->zt_cap = need + need / 4 + 1024;
+    }
+    CallArgs r = a;
+    r.scores_out = nullptr; r.latents_out = ws->zt; r.latents_terminal = true;
+    int rc = run_rollout_locked(ctx, ws, r, st);
+    if (rc != WM_OK) return rc;
+    if (ctx->m.tsc_ok) {
+        const size_t xneed = tsc_x_bytes(ctx, a.B);
+        if (ws->xbuf_cap < xneed) {
+            if (ws->xbuf) {
+                WM_CUDA_TRY(cudaStreamSynchronize(st));
+                WM_CUDA_TRY(cudaFree(ws->xbuf));
+                ws->xbuf = nullptr;
+                ws->xbuf_cap = 0;
+            }
+            WM_CUDA_TRY(cudaMalloc(&ws->xbuf, xneed + xneed / 4 + 4096));
+            ws->xbuf_cap = xneed + xneed / 4 + 4096;
+        }
+        CallArgs xa = a;
+        xa.fault = ctx->fault;
+        rc = launch_tsc(ctx, ws->zt, ws->xbuf, xa, a.scores_out, st);
+    } else {
+        CallArgs sc = a;
+        sc.fault = ctx->fault;
+        sc.perm = (ctx->opt_sort && a.B > 256) ? ws->perm : nullptr;   // K1's order by length serves both passes
+        sc.cand_latents = ws->zt;     // (rows of length 0 stored no latent: they keep init_states, their z_T = z_0)
+        sc.start = a.lengths;
+        rc = launch_generic(ctx, sc, st);
+    }
+    if (rc == WM_OK && ctx->opt_timing && ws->ev1) WM_CUDA_TRY(cudaEventRecord(ws->ev1, st));
+    return rc;
+}
+
 int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* action_ids, const int32_t* action_params,
                      const int32_t* lengths, const float* hw_feats, float* scores_out,
                      const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, void* cuda_stream) {
@@ -560,62 +624,7 @@ int wm_rollout_score(wm_ctx* ctx, const float* init_states, const int32_t* actio
         const int rc = run_rollout_locked(ctx, ws, r, st);
         return rc != WM_OK ? rc : launch_forest(ctx, ws->zt, a, scores_out, st);
     }
-    if (ctx->m.phi_kind == WM_PHI_TYPED && pick_path(ctx) == 2 && B <= 0x7fffffffLL / ctx->m.d &&
-        (uintptr_t)init_states % 16 == 0 && T_max > 0 && T_max <= 255) {
-        // per-type phi (S28) on a model the pair kernel can roll: 609 running statistics per row do not fit beside a
-        // 256-row tile, so K2 (tcgen05) stores the terminal latents [B, d] and the fp32 kernel takes them as per-candidate
-        // initial latents with start = len: it walks every position for phi only (no transition step) and runs the scorer
-        WM_CUDA_TRY(cudaSetDevice(ctx->device));
-        Workspace* ws = acquire_ws(ctx, st);
-        if (!ws) {
-            set_error("wm_rollout_score: cannot allocate workspace");
-            return WM_ERR_CUDA;
-        }
-        std::lock_guard<std::mutex> lk(ws->mu);
-        nvtx::Range nr("wm_rollout_score");
-        const size_t need = (size_t)B * ctx->m.d;
-        if (ws->zt_cap < need) {
-            if (ws->zt) {
-                WM_CUDA_TRY(cudaStreamSynchronize(st));
-                WM_CUDA_TRY(cudaFree(ws->zt));
-                ws->zt = nullptr;
-                ws->zt_cap = 0;
-            }
-            WM_CUDA_TRY(cudaMalloc(&ws->zt, (need + need / 4 + 1024) * sizeof(float)));
-            ws->zt_cap = need + need / 4 + 1024;
-        }
-        CallArgs r = a;
-        r.scores_out = nullptr; r.latents_out = ws->zt; r.latents_terminal = true;
-        int rc = run_rollout_locked(ctx, ws, r, st);
-        if (rc != WM_OK) return rc;
-        if (ctx->m.tsc_ok) {
-            // the ranking MLP on tcgen05: wm_typed_x_kernel writes the fp16 rows [z_T | phi | 1 | h], wm_tsc_kernel ranks them
-            const size_t xneed = tsc_x_bytes(ctx, B);
-            if (ws->xbuf_cap < xneed) {
-                if (ws->xbuf) {
-                    WM_CUDA_TRY(cudaStreamSynchronize(st));
-                    WM_CUDA_TRY(cudaFree(ws->xbuf));
-                    ws->xbuf = nullptr;
-                    ws->xbuf_cap = 0;
-                }
-                WM_CUDA_TRY(cudaMalloc(&ws->xbuf, xneed + xneed / 4 + 4096));
-                ws->xbuf_cap = xneed + xneed / 4 + 4096;
-            }
-            CallArgs xa = a;
-            xa.fault = ctx->fault;
-            rc = launch_tsc(ctx, ws->zt, ws->xbuf, xa, scores_out, st);
-            if (rc == WM_OK && ctx->opt_timing && ws->ev1) WM_CUDA_TRY(cudaEventRecord(ws->ev1, st));
-            return rc;
-        }
-        CallArgs sc = a;
-        sc.fault = ctx->fault;
-        sc.perm = (ctx->opt_sort && a.B > 256) ? ws->perm : nullptr;   // K1's order by length serves both passes
-        sc.cand_latents = ws->zt;     // (rows of length 0 stored no latent: they keep init_states, their z_T = z_0)
-        sc.start = a.lengths;
-        rc = launch_generic(ctx, sc, st);
-        if (rc == WM_OK && ctx->opt_timing && ws->ev1) WM_CUDA_TRY(cudaEventRecord(ws->ev1, st));
-        return rc;
-    }
+    if (typed_split_applies(ctx, a, false)) return typed_split_score(ctx, a, st, "wm_rollout_score");
     return run_rollout(ctx, a, st, "wm_rollout_score");
 }
 
@@ -730,6 +739,8 @@ int wm_rollout_score_from(wm_ctx* ctx, const float* bank, const int32_t* bank_in
     a.action_ids = action_ids; a.action_params = action_params; a.lengths = lengths;
     a.hw_feats = hw_feats; a.scores_out = scores_out; a.offsets = subgraph_offsets;
     a.B = B; a.S = S; a.T_max = T_max;
+    if (typed_split_applies(ctx, a, true))
+        return typed_split_score(ctx, a, static_cast<cudaStream_t>(cuda_stream), "wm_rollout_score_from");
     return run_rollout(ctx, a, static_cast<cudaStream_t>(cuda_stream), "wm_rollout_score_from");
 }
 

@@ -998,8 +998,9 @@ int launch_tc(wm_ctx* ctx, Workspace* ws, const CallArgs& a, cudaStream_t st) {
     const bool use_pair = m.tcp_ok && (ctx->opt_pair || !m.tc1_ok);      // d = 256 models: the pair kernel takes the call
     const bool ext_ok = m.tc_ok >= 1 && m.tc_ok <= 4;                      // every tcgen05 kernel takes the prefix-reuse calls
     if (prefix_call && !ext_ok && ctx->opt_path != 2) return launch_generic(ctx, a, st);
-    // per-type phi: the tcgen05 kernels hold no scorer for it; a call that wants scores from them (wm_rollout_score_from,
-    // wm_rollout_score_static; wm_rollout_score splits the call itself) runs on the fp32 kernel
+    // per-type phi: the rollout kernels hold no scorer for it (wm_rollout_score / wm_rollout_score_from split the call
+    // themselves, wm_api.cu); a call that still wants scores from them (wm_rollout_score_static; a prefix call of a model
+    // without the tcgen05 ranking MLP) runs on the fp32 kernel
     if (m.phi_kind == WM_PHI_TYPED && a.scores_out) {
         if (ctx->opt_path == 2) {
             set_error("tcgen05 path: a WM_PHI_TYPED model is scored by wm_rollout_score only");

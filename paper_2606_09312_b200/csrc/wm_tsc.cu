@@ -284,9 +284,11 @@ wm_tsc_kernel(const Params p, const __grid_constant__ CUtensorMap tmap_x, const 
 // type k and scans the candidate's steps in order (every lane reads the same id / parameters: broadcast loads), so every
 // sum has ONE order whatever the launch.  z_T is the terminal latent K2 stored (the task's z_0 for an empty sequence).
 struct XParams {
-    const float* zT;            // [B, d] (rows of candidates with len = 0 are not read)
-    const float* init_states;   // [S, d] ([B, d] without offsets)
+    const float* zT;            // [B, d] terminal latents of the candidates that rolled at least one step
+    const float* init_states;   // [S, d] ([B, d] without offsets); the bank [n_init, d] of a prefix-reuse call
     const int32_t *ids, *params, *lengths, *offsets;
+    const int32_t *start, *init_index;   // prefix-reuse call (else null): first rolled position, bank row
+    int64_t n_init;
     const float* hw;
     __half* X;                  // [B, 64 nkb]
     int64_t B;
@@ -314,7 +316,15 @@ __global__ void __launch_bounds__(kXWarps * 32) wm_typed_x_kernel(const XParams 
             seg = lo;
         }
         __half* x = p.X + (size_t)c * ld;
-        const float* z = len > 0 ? p.zT + (size_t)c * D : p.init_states + (size_t)seg * D;
+        // z_T: the stored terminal latent, or — when no step was rolled (empty sequence; start = len) — the latent the rollout
+        // would have started from
+        const bool rolled = len > 0 && (!p.start || clamp_start(__ldg(p.start + c), len) < len);
+        size_t zrow = (size_t)seg;
+        if (p.init_index) {
+            long long bi = __ldg(p.init_index + c);      // (K2 has reported an index outside the bank)
+            zrow = (size_t)(bi < 0 ? 0 : (bi >= p.n_init ? p.n_init - 1 : bi));
+        }
+        const float* z = rolled ? p.zT + (size_t)c * D : p.init_states + zrow * D;
         for (int j = 2 * lane; j < D; j += 64) {
             const float2 v = __ldg(reinterpret_cast<const float2*>(z + j));
             *reinterpret_cast<uint32_t*>(x + j) = pack_f16(v.x, v.y);
@@ -493,6 +503,7 @@ int launch_tsc(wm_ctx* ctx, const float* zT, void* X, const CallArgs& a, float* 
     tsc::XParams xp;
     xp.zT = zT; xp.init_states = a.init_states; xp.ids = a.action_ids; xp.params = a.action_params; xp.lengths = a.lengths;
     xp.offsets = a.offsets; xp.hw = a.hw_feats; xp.X = static_cast<__half*>(X);
+    xp.start = a.start; xp.init_index = a.init_index; xp.n_init = a.n_init;
     xp.B = a.B; xp.S = a.S; xp.T_max = a.T_max; xp.n_types = m.n_types; xp.P = m.P; xp.H = m.H; xp.nkb = NKB;
     xp.phi_dim = m.phi_dim; xp.fault = a.fault;
     const int64_t xb = (a.B + tsc::kXWarps - 1) / tsc::kXWarps;

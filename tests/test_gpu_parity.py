@@ -676,9 +676,8 @@ def test_score_from_bank_matches_literal(wm, n):
 def test_typed_phi_model_splits_the_call_and_keeps_prefix_reuse(wm):
     """A WM_PHI_TYPED model with cfg 2's shapes (config 14): wm_rollout_score rolls on the pair kernel (tc_variant 5), writes
     the scorer's fp16 input rows [z_T | phi | 1 | h] and ranks them on the tcgen05 ranking-MLP kernel (rows of length 0 keep
-    z_0; the batch's last tile is ragged: rows past B read as zero and are not written); wm_rollout_score_from, which the
-    tcgen05 kernels cannot rank for this phi, runs on the fp32 kernel under the automatic policy and is refused
-    (WM_ERR_UNSUPPORTED) when the tcgen05 path is forced."""
+    z_0; the batch's last tile is ragged: rows past B read as zero and are not written); wm_rollout_score_from takes the same
+    split with the rollout started from the bank rows, including candidates whose start is their length."""
     import torch
     cfg = gen.get_config(14).scaled(S=3, per_subgraph=300)
     w, b = gen.make_weights(cfg), gen.make_inputs(cfg)
@@ -707,13 +706,20 @@ def test_typed_phi_model_splits_the_call_and_keeps_prefix_reuse(wm):
     out = torch.full((b.B,), float("nan"), dtype=torch.float32, device="cuda:0")
     args = (bank, torch.from_numpy(index).cuda(), torch.from_numpy(st).cuda(), dv["action_ids"], dv["action_params"],
             dv["lengths"], dv["hw_feats"], out, dv["subgraph_offsets"])
+    n1 = wm.wm_launch_count(ctx)
     wm.wm_rollout_score_from(ctx, *args)
     assert wm.wm_check(ctx) == 0
-    assert oracle.score_error(out.cpu().numpy(), ref, b.subgraph_offsets) <= TOL[False]
-    wm.wm_set_option(ctx, wm.WM_OPT_PATH, wm.PATH_TCGEN05)
-    with pytest.raises(wm.WmError) as e:
-        wm.wm_rollout_score_from(ctx, *args)
-    assert e.value.code == wm.WM_ERR_UNSUPPORTED
+    assert wm.wm_launch_count(ctx) - n1 == 5            # the same split: the rollout starts from the bank rows
+    y_from = out.cpu().numpy()
+    assert oracle.score_error(y_from, ref, b.subgraph_offsets) <= TOL[False]
+    assert oracle.score_error(y_from, y, b.subgraph_offsets) <= 2e-3      # (pair kernel: u = z + b2, see test_score_from_bank)
+    # candidates that roll nothing (start = len, and the empty ones) are ranked on their bank row
+    st_all = torch.from_numpy(b.lengths.astype(np.int32)).cuda()
+    idx_all = torch.from_numpy(np.where(b.lengths == 0, seg, cfg.S + np.arange(b.B) * cfg.T_max + b.lengths - 1).astype(np.int32)).cuda()
+    out2 = torch.full((b.B,), float("nan"), dtype=torch.float32, device="cuda:0")
+    wm.wm_rollout_score_from(ctx, bank, idx_all, st_all, *args[3:7], out2, args[8])
+    assert wm.wm_check(ctx) == 0
+    assert oracle.score_error(out2.cpu().numpy(), ref, b.subgraph_offsets) <= TOL[False]
     wm.wm_free(ctx)
 
 
