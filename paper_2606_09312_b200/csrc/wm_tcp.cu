@@ -37,6 +37,7 @@
 
 #include "wm_internal.h"
 #include "wm_ptx.cuh"
+#include "wm_tmap.h"
 #include "wm_trace.cuh"
 
 namespace wm {
@@ -1110,10 +1111,6 @@ bool append_slot(std::vector<uint16_t>& blob, const std::vector<float>& W, int l
     return ok;
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
 }  // namespace
 
 bool tcp_model_ok(const Model& m) {
@@ -1285,24 +1282,11 @@ int tcp_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
 
     // tensor map over the image seen as rows of 64 16-bit values (128 B); one box = 128 rows.  The image is already
     // swizzled, so the map itself uses no swizzle.
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qr;
-    WM_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr));
-    if (!fn || qr != cudaDriverEntryPointSuccess) {
-        set_error("tcp_prepare: cuTensorMapEncodeTiled is not available from this driver");
-        return WM_ERR_CUDA;
-    }
     static_assert(sizeof(CUtensorMap) <= sizeof(m.tcp_tmap), "tensor map storage");
     CUtensorMap tm;
-    const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
-    const cuuint64_t strides[1] = {128};
-    const cuuint32_t box[2] = {64, 64}, es[2] = {1, 1};
-    const CUresult r = ((EncodeTiledFn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, d_blob, dims, strides, box, es,
-                                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-        set_error("tcp_prepare: cuTensorMapEncodeTiled failed (%d)", (int)r);
-        return WM_ERR_CUDA;
+    {
+        const int rc = encode_tmap_2d(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, d_blob, 64, blob.size() * 2 / 128, 128, 64, 64, false, "tcp_prepare");
+        if (rc != WM_OK) return rc;
     }
     memcpy(m.tcp_tmap, &tm, sizeof(tm));
     {

@@ -24,6 +24,7 @@
 
 #include "wm_internal.h"
 #include "wm_ptx.cuh"
+#include "wm_tmap.h"
 
 namespace wm {
 
@@ -421,19 +422,6 @@ bool append_box(std::vector<uint16_t>& blob, const std::vector<float>& W, int ld
     return ok;
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn() {
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qr;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess ||
-        qr != cudaDriverEntryPointSuccess)
-        return nullptr;
-    return (EncodeTiledFn)fn;
-}
-
 }  // namespace
 
 int tsc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const std::vector<std::string>& names) {
@@ -469,8 +457,6 @@ int tsc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     for (int c = 0; c < 4; ++c)               // layer 2: per chunk the eight K-blocks of H1
         for (int kb = 0; kb < 8; ++kb) ok &= append_box(blob, Ws1, tsc::SW, c * 128, kb * 64);
     if (!ok) return WM_OK;   // a weight beyond the fp16 range: the fp32 kernel ranks this model
-    EncodeTiledFn enc = encode_fn();
-    if (!enc) return WM_OK;
     void* d_blob = nullptr;
     WM_CUDA_TRY(cudaMalloc(&d_blob, blob.size() * 2));
     ctx->allocs.push_back(d_blob);
@@ -478,14 +464,9 @@ int tsc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     // the image seen as rows of 64 16-bit values (128 B); one box = 64 rows; already swizzled: the map uses no swizzle
     static_assert(sizeof(CUtensorMap) <= sizeof(m.tsc_tmap), "tensor map storage");
     CUtensorMap tm;
-    const cuuint64_t dims[2] = {64, (cuuint64_t)(blob.size() * 2 / 128)};
-    const cuuint64_t strides[1] = {128};
-    const cuuint32_t box[2] = {64, 64}, es[2] = {1, 1};
-    const CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, d_blob, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-        set_error("tsc_prepare: cuTensorMapEncodeTiled failed (%d)", (int)r);
-        return WM_ERR_CUDA;
+    {
+        const int rc = encode_tmap_2d(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, d_blob, 64, blob.size() * 2 / 128, 128, 64, 64, false, "tsc_prepare");
+        if (rc != WM_OK) return rc;
     }
     memcpy(m.tsc_tmap, &tm, sizeof(tm));
     WM_CUDA_TRY(cudaFuncSetAttribute(tsc::wm_tsc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsc::SMEM_TOTAL));
@@ -512,20 +493,11 @@ int launch_tsc(wm_ctx* ctx, const float* zT, void* X, const CallArgs& a, float* 
     WM_CUDA_TRY(cudaGetLastError());
     // tensor map over X: rows of 64 nkb fp16, one box = this CTA's 128 rows of one K-block, 128-byte swizzle = the SW128
     // K-major operand layout; rows past B read as zero
-    EncodeTiledFn enc = encode_fn();
-    if (!enc) {
-        set_error("launch_tsc: cuTensorMapEncodeTiled is not available from this driver");
-        return WM_ERR_CUDA;
-    }
     CUtensorMap tx, tw;
-    const cuuint64_t dims[2] = {(cuuint64_t)(64 * NKB), (cuuint64_t)a.B};
-    const cuuint64_t strides[1] = {(cuuint64_t)(64 * NKB) * sizeof(__half)};
-    const cuuint32_t box[2] = {64, (cuuint32_t)tsc::TM}, es[2] = {1, 1};
-    const CUresult r = enc(&tx, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, X, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                           CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-        set_error("launch_tsc: cuTensorMapEncodeTiled failed (%d)", (int)r);
-        return WM_ERR_CUDA;
+    {
+        const int rc = encode_tmap_2d(&tx, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, X, (uint64_t)(64 * NKB), (uint64_t)a.B,
+                                      (uint64_t)(64 * NKB) * sizeof(__half), 64, (uint32_t)tsc::TM, true, "launch_tsc");
+        if (rc != WM_OK) return rc;
     }
     memcpy(&tw, m.tsc_tmap, sizeof(tw));
     tsc::Params p;
