@@ -146,6 +146,13 @@ void wm_free(wm_ctx* ctx);
 /* Copy the model description out of a context. */
 int wm_get_info(const wm_ctx* ctx, wm_info* info_out);
 
+/* Why this model runs where it runs.  "" when a tcgen05 kernel takes it (wm_info.path = 2); otherwise one sentence that
+ * names the first property that keeps it on the fp32 CUDA-core kernel (wm_info.path = 1, typically 50-80 x slower on the
+ * bf16 configurations of BASELINE.json: a latent width no tcgen05 kernel is built for, a scorer of another shape, a weight
+ * beyond the fp16 range, ...), so that a caller one notch off a supported shape is told instead of silently slowed down.
+ * The string is owned by the context.  NULL ctx: "". */
+const char* wm_path_reason(const wm_ctx* ctx);
+
 /* Set a WM_OPT_* option; returns WM_ERR_ARG for an unknown key or value, WM_ERR_UNSUPPORTED when the forced
  * path cannot run this model. */
 int wm_set_option(wm_ctx* ctx, int32_t key, int32_t value);

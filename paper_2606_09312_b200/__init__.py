@@ -24,7 +24,7 @@ PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 # every symbol include/wm.h declares
 ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
                "wm_rollout_latents", "wm_rollout_score_from", "wm_rollout_score_static",
-               "wm_check", "wm_score_topk_host", "wm_score_topk_host_compact", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error")
+               "wm_check", "wm_score_topk_host", "wm_score_topk_host_compact", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error", "wm_path_reason")
 
 
 class WmInfo(ctypes.Structure):
@@ -86,6 +86,8 @@ def lib() -> ctypes.CDLL:
     L.wm_launch_count.restype = i64
     L.wm_launch_empty.argtypes = [vp]
     L.wm_launch_empty.restype = ctypes.c_int
+    L.wm_path_reason.argtypes = [vp]
+    L.wm_path_reason.restype = ctypes.c_char_p
     L.wm_last_error.argtypes = []
     L.wm_last_error.restype = ctypes.c_char_p
     _lib = L
@@ -218,6 +220,11 @@ def wm_last_kernel_ms(ctx: int, stream=None) -> float:
     ms = ctypes.c_float()
     _check(lib().wm_last_kernel_ms(ctx, _stream(stream), ctypes.byref(ms)))
     return float(ms.value)
+
+
+def wm_path_reason(ctx: int) -> str:
+    """Why the model is on the fp32 kernel ("" when a tcgen05 kernel takes it).  include/wm.h."""
+    return lib().wm_path_reason(ctx).decode()
 
 
 def wm_launch_count(ctx: Optional[int]) -> int:

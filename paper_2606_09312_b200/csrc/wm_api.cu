@@ -339,6 +339,34 @@ static int load_weights_impl(const char* path, int device, wm_ctx** ctx_out) {
         }
         rc = tc_prepare(ctx, hv, names);
     }
+    if (rc == WM_OK && !tc_supported(ctx)) {
+        // wm_path_reason: the first property that keeps the model off the tcgen05 kernels
+        const Model& m = ctx->m;
+        char buf[400];
+        const bool mlp_ln = m.kind == WM_KIND_MLP_LN, transh = m.kind == WM_KIND_TRANSH, gru = m.kind == WM_KIND_GRU;
+        if (m.dtype != WM_DTYPE_BF16)
+            snprintf(buf, sizeof buf, "fp32 weights: the tcgen05 kernels take bf16-valued weights (an fp32 model needs fp32 products for its 1e-4 tolerance)");
+        else if (m.kind == WM_KIND_MLP)
+            snprintf(buf, sizeof buf, "residual MLP without LayerNorm: the tcgen05 kernels are built for MLP+LayerNorm, TransH and GRU transitions");
+        else if ((mlp_ln && m.d != 256 && m.d != 512) || (transh && m.d != 256) || (gru && m.d != 384))
+            snprintf(buf, sizeof buf, "latent width d = %d: the tcgen05 kernels are built for d = 256 (MLP+LayerNorm, TransH), 512 (MLP+LayerNorm) and 384 (GRU)", m.d);
+        else if ((m.d == 256 && m.d_a != 128) || (m.d == 512 && m.d_a != 256) || (m.d == 384 && m.d_a != 128))
+            snprintf(buf, sizeof buf, "action-embedding width d_a = %d: the d = %d tcgen05 kernel is built for d_a = %d", m.d_a, m.d, m.d == 512 ? 256 : 128);
+        else if ((gru && m.embed != WM_EMBED_BUCKET) || (!gru && m.embed != WM_EMBED_LINEAR))
+            snprintf(buf, sizeof buf, "action embedding kind %d: the GRU kernel takes the bucketed table, the others the linear embedding", m.embed);
+        else if (m.ranker_kind == WM_RANKER_MLP && m.phi_kind != WM_PHI_TYPED &&
+                 (m.n_lin != 3 || m.sdim[1] != m.sdim[2] || m.sdim[1] != (m.d == 256 ? 512 : m.d == 512 ? 1024 : 768)))
+            snprintf(buf, sizeof buf, "scorer shape: the d = %d tcgen05 kernel is built for two hidden layers of %d units", m.d, m.d == 256 ? 512 : m.d == 512 ? 1024 : 768);
+        else if (m.H < 8 || m.H > 64 || m.H % 8 != 0)
+            snprintf(buf, sizeof buf, "hardware-feature width H = %d: the tcgen05 kernels take 8 <= H <= 64, a multiple of 8", m.H);
+        else if (!gru && (m.hidden % (m.d == 512 ? 256 : 128) != 0 || m.hidden < (m.d == 512 ? 512 : 256) || m.hidden > 1024))
+            snprintf(buf, sizeof buf, "hidden width %d: the d = %d tcgen05 kernel takes a multiple of %d up to 1024", m.hidden, m.d, m.d == 512 ? 256 : 128);
+        else if (m.phi_kind != WM_PHI_MEAN && (gru || (m.phi_kind == WM_PHI_TYPED && m.d != 256)))
+            snprintf(buf, sizeof buf, "phi kind %d with this transition: structured phi runs on the d = 256 / 512 kernels, per-type phi on the d = 256 one", m.phi_kind);
+        else
+            snprintf(buf, sizeof buf, "outside the tcgen05 kernels' limits (action types, parameter slots, buckets, shared memory) or a weight beyond the fp16 range (|w| > 65504)");
+        ctx->path_reason = buf;
+    }
     if (rc == WM_OK && !generic_supported(ctx) && !tc_supported(ctx)) {
         set_error("wm_load_weights: no kernel in this build handles this model (too wide for shared memory)");
         rc = WM_ERR_UNSUPPORTED;
@@ -393,6 +421,8 @@ int wm_load_weights(const char* path, int device, wm_ctx** ctx_out) {
         return WM_ERR_IO;
     }
 }
+
+const char* wm_path_reason(const wm_ctx* ctx) { return ctx ? ctx->path_reason.c_str() : ""; }
 
 int wm_get_info(const wm_ctx* ctx, wm_info* o) {
     if (!ctx || !o) {

@@ -122,6 +122,7 @@ struct wm_ctx {
     std::vector<wm::Workspace*> pool;
     std::vector<void*> allocs;   // every device allocation owned by the ctx (weights)
     std::atomic<int64_t> launches{0};
+    std::string path_reason;     // wm_path_reason(): why the model is on the fp32 kernel ("" on a tcgen05 kernel)
     // wm_score_topk_host pipelines a call by chunks of whole subgraphs: a copy stream, two compute streams, events and
     // a pinned staging buffer for the per-chunk (rebased) offsets; created on first use
     std::mutex host_mu;

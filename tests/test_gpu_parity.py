@@ -673,6 +673,27 @@ def test_score_from_bank_matches_literal(wm, n):
         assert oracle.score_error(y, lit, b.subgraph_offsets) <= same, (n, path)
 
 
+def test_path_reason_names_what_keeps_a_model_on_the_fp32_kernel(wm):
+    """wm_path_reason: "" for a model a tcgen05 kernel takes; for a model one notch off a supported shape (d = 320; a scorer of
+    768 units; fp32 weights) a sentence that names the property — the fallback is 50-80 x slower and must not be silent."""
+    for n in (2, 3, 5, 7, 14):
+        ctx = wm.wm_load_weights(weight_file(gen.get_config(n).scaled(S=1, per_subgraph=64)))
+        assert wm.wm_get_info(ctx).path == 2 and wm.wm_path_reason(ctx) == ""
+        wm.wm_free(ctx)
+    base = gen.get_config(2).scaled(S=1, per_subgraph=64)
+    for cfg, word in ((replace(base, d=320, name="cfg2_d320"), "d = 320"),
+                      (replace(base, scorer_widths=(768, 768), name="cfg2_s768"), "scorer"),
+                      (gen.get_config(1), "fp32")):
+        b = gen.make_inputs(cfg)
+        ctx = wm.wm_load_weights(weight_file(cfg))
+        assert wm.wm_get_info(ctx).path == 1
+        assert word in wm.wm_path_reason(ctx), wm.wm_path_reason(ctx)
+        y = gpu_scores(ctx, b)                               # ... and the fp32 kernel still ranks it within its tolerance
+        tol = 1e-4 if cfg.dtype == DTYPE_FP32 else 2e-3
+        assert oracle.score_error(y, oracle_scores(cfg, gen.make_weights(cfg), b), b.subgraph_offsets) <= tol
+        wm.wm_free(ctx)
+
+
 def test_typed_phi_model_splits_the_call_and_keeps_prefix_reuse(wm):
     """A WM_PHI_TYPED model with cfg 2's shapes (config 14): wm_rollout_score rolls on the pair kernel (tc_variant 5), writes
     the scorer's fp16 input rows [z_T | phi | 1 | h] and ranks them on the tcgen05 ranking-MLP kernel (rows of length 0 keep
