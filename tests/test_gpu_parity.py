@@ -460,8 +460,9 @@ def test_full_size_sampled(wm, n):
 
 
 # (config, subgraphs the oracle recomputes in full): cfg 2 and cfg 3 whole; cfg 4 / cfg 5 the first whole subgraph of the
-# full 2,097,152-candidate launch (16,384 candidates = 0.5 / 0.8 TFLOP of float64 numpy); 7 and 9 are cfg 2's batch
-FULL_ORACLE = [(2, 16), (3, 64), (4, 1), (5, 1), (7, 16), (9, 16)]
+# full 2,097,152-candidate launch (16,384 candidates = 0.5 / 0.8 TFLOP of float64 numpy); 7, 9 and 14 are cfg 2's batch
+# (14: the per-type phi through wm_typed_x_kernel + wm_tsc_kernel)
+FULL_ORACLE = [(2, 16), (3, 64), (4, 1), (5, 1), (7, 16), (9, 16), (14, 16)]
 
 
 @pytest.mark.parametrize("n,n_sub", FULL_ORACLE)
