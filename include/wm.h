@@ -216,9 +216,9 @@ int wm_rollout_score_static(wm_ctx* ctx,
  * tcgen05 kernels keep the latent in fp32 between steps, so a bank written by wm_rollout_latents reproduces them).
  * Candidates are bucketed by their remaining steps lengths[b] - start[b].
  * Errors: as wm_rollout_score; WM_ERR_ARG also for a null bank / bank_index / start / latents_out or n_bank < 1;
- * WM_ERR_UNSUPPORTED for wm_rollout_score_from on a WM_RANKER_FOREST model, and when the tcgen05 path is forced
- * (WM_OPT_PATH = 2) on a model whose tcgen05 kernel does not take these calls (the d = 256 MLP+LayerNorm kernel takes both, the
- * TransH kernel wm_rollout_latents; under the automatic policy the other models run them on the fp32 kernel). */
+ * WM_ERR_UNSUPPORTED for wm_rollout_score_from on a WM_RANKER_FOREST model.  Every tcgen05 kernel takes both calls (its EXT
+ * instance); a call whose latents_out is not 16-byte aligned runs on the fp32 kernel (WM_ERR_UNSUPPORTED when the tcgen05
+ * path is forced with WM_OPT_PATH = 2). */
 int wm_rollout_latents(wm_ctx* ctx,
                        const float* init_states, const int32_t* action_ids, const int32_t* action_params,
                        const int32_t* lengths, const int32_t* subgraph_offsets, float* latents_out,
