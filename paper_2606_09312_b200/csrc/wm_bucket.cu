@@ -104,12 +104,96 @@ __global__ void __launch_bounds__(kBucketThreads) wm_len_scatter_kernel(const in
     }
 }
 
+// Both steps in ONE launch for batches whose CTAs are all resident at once (grid <= number of SMs; cfg 2 / 3: 8 / 16
+// CTAs): every CTA adds its histogram to the global one, the CTAs meet at a counter (bounded spin; co-residency makes it
+// safe), then each takes its ranges and places its candidates as wm_len_scatter_kernel does.  The lengths are read once and
+// one launch (of three in an evolution-round-sized call) goes away.  `hist` is read back through L2 (__ldcg): it was written
+// by other CTAs' atomics during this launch.
+__global__ void __launch_bounds__(kBucketThreads) wm_len_sort_kernel(const int32_t* __restrict__ lengths,
+                                                                     const int32_t* __restrict__ start, int64_t B,
+                                                                     int T_max, int32_t* hist, int32_t* cursor,
+                                                                     int32_t* arrived, int32_t* __restrict__ perm) {
+    __shared__ int s_cnt[WM_MAX_T + 1];    // this CTA's histogram, then its running cursor inside each bin
+    __shared__ int s_base[WM_MAX_T + 1];   // global start of the CTA's range in each bin
+    for (int i = threadIdx.x; i <= T_max; i += blockDim.x) s_cnt[i] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * (kBucketThreads * kBucketItems);
+    int my_len[kBucketItems];
+#pragma unroll
+    for (int it = 0; it < kBucketItems; ++it) {
+        const int64_t i = base + (int64_t)it * kBucketThreads + threadIdx.x;
+        my_len[it] = -1;
+        if (i < B) {
+            my_len[it] = steps_of(lengths, start, i, T_max);
+            atomicAdd(&s_cnt[my_len[it]], 1);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= T_max; i += blockDim.x)
+        if (s_cnt[i]) atomicAdd(&hist[i], s_cnt[i]);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        atomicAdd(arrived, 1);
+        const long long t0 = clock64();
+        while (atomicAdd(arrived, 0) < (int)gridDim.x)
+            if (clock64() - t0 > 4000000000LL) __trap();      // (a CTA that is not resident would never arrive)
+        __threadfence();
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const int nb = T_max + 1;
+        const int per = (nb + 31) / 32;
+        const int lane = threadIdx.x;
+        int sum = 0;
+        for (int q = 0; q < per; ++q) {
+            const int bin = T_max - (lane * per + q);
+            if (bin >= 0) sum += __ldcg(hist + bin);
+        }
+        int incl = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        int run = incl - sum;
+        for (int q = 0; q < per; ++q) {
+            const int bin = T_max - (lane * per + q);
+            if (bin >= 0) {
+                int mine = 0;
+                const int c = s_cnt[bin];
+                if (c) mine = atomicAdd(&cursor[bin], c);
+                s_base[bin] = run + mine;
+                run += __ldcg(hist + bin);
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= T_max; i += blockDim.x) s_cnt[i] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < kBucketItems; ++it) {
+        if (my_len[it] >= 0) {
+            const int64_t i = base + (int64_t)it * kBucketThreads + threadIdx.x;
+            const int pos = s_base[my_len[it]] + atomicAdd(&s_cnt[my_len[it]], 1);
+            perm[pos] = (int32_t)i;
+        }
+    }
+}
+
 int launch_length_bucketing(wm_ctx* ctx, Workspace* ws, const int32_t* lengths, const int32_t* start, int64_t B,
                             int T_max, cudaStream_t st) {
     if (B <= 0) return WM_OK;
     WM_CUDA_TRY(cudaMemsetAsync(ws->counters, 0, sizeof(int32_t) * kCounterInts, st));
     const int64_t per_cta = (int64_t)kBucketThreads * kBucketItems;
     const int grid = (int)((B + per_cta - 1) / per_cta);
+    if (grid <= ctx->n_sms) {      // every CTA resident at once: one launch (the counters' memset above clears the meeting word too)
+        wm_len_sort_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, start, B, T_max, ws->counters + kHistOff,
+                                                            ws->counters + kCursorOff, ws->counters + kTileCtrOff + 1, ws->perm);
+        WM_CUDA_TRY(cudaGetLastError());
+        ctx->launches.fetch_add(1);
+        return WM_OK;
+    }
     wm_len_hist_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, start, B, T_max, ws->counters + kHistOff);
     WM_CUDA_TRY(cudaGetLastError());
     wm_len_scatter_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, start, B, T_max, ws->counters + kHistOff,
