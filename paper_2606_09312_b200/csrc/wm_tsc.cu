@@ -5,7 +5,7 @@
 // PAPER.md:122 Eq.3 / :188 Eq.12 — y = G([z_T ; phi ; h]) with G = Linear -> GELU -> Linear -> GELU -> Linear(-> 1).
 // wm_rollout_score of such a model is three launches after K1: wm_tcp_kernel<., EXT> rolls the candidates and stores the
 // terminal latents; wm_typed_x_kernel (below) writes the scorer input X = [z_T | phi | 1 | 0.. | h | 0..] as fp16 rows
-// (phi in a fixed order per row: lane k owns action type k and scans the steps, no atomics); this kernel is the scorer of
+// (phi in a fixed order per row: the steps of one action type are summed in step order by one lane, no atomics); this kernel is the scorer of
 // wm_tcp_kernel with the A operand streamed from X instead of being written by the epilogue / action warps.
 //
 // A cluster of two CTAs owns a tile of 256 consecutive candidates (128 rows each).  Layer 1 runs as two passes of two
@@ -281,9 +281,8 @@ wm_tsc_kernel(const Params p, const __grid_constant__ CUtensorMap tmap_x, const 
 }
 
 // X row of a candidate: [z_T (256) | phi (n_types (1 + 3P) + 1) | 1 | 0.. to a K-block | h (H) | 0.. to a K-block], fp16.
-// One warp per candidate.  phi (S28) = [c_k | len | per type k: s_kj | m_kj | x_kj]: lane k (k, k + 32, ...) owns action
-// type k and scans the candidate's steps in order (every lane reads the same id / parameters: broadcast loads), so every
-// sum has ONE order whatever the launch.  z_T is the terminal latent K2 stored (the task's z_0 for an empty sequence).
+// One warp per candidate.  phi (S28) = [c_k | len | per type k: s_kj | m_kj | x_kj]; the steps of one type are summed in step
+// order by one lane (see the loop), so every sum has ONE order whatever the launch.  z_T is the terminal latent K2 stored (the task's z_0 for an empty sequence).
 struct XParams {
     const float* zT;            // [B, d] terminal latents of the candidates that rolled at least one step
     const float* init_states;   // [S, d] ([B, d] without offsets); the bank [n_init, d] of a prefix-reuse call
@@ -298,10 +297,10 @@ struct XParams {
 };
 
 constexpr int kXWarps = 8;
+constexpr int kXTypes = 64, kXAcc = 17;     // most action types; accumulator floats per type (odd: conflict-free)
 
 __global__ void __launch_bounds__(kXWarps * 32) wm_typed_x_kernel(const XParams p) {
-    __shared__ __align__(16) float s_l2[kXWarps * 32 * 8];      // per warp: log2 p of a chunk of 32 steps, 8 slots each
-    __shared__ int s_id[kXWarps * 32];
+    __shared__ float s_acc[kXWarps * kXTypes * kXAcc];          // per warp and action type: count, sum[8], max[8]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int NT = p.n_types, P = p.P, ld = 64 * p.nkb;
     for (int64_t c = (int64_t)blockIdx.x * kXWarps + warp; c < p.B; c += (int64_t)gridDim.x * kXWarps) {
@@ -331,64 +330,83 @@ __global__ void __launch_bounds__(kXWarps * 32) wm_typed_x_kernel(const XParams 
             *reinterpret_cast<uint32_t*>(x + j) = pack_f16(v.x, v.y);
         }
         // everything behind z_T starts as zero (padding columns must not hold NaNs: their weights are zero, 0 * NaN is not)
-        for (int j = D + 2 * lane; j < ld; j += 64) *reinterpret_cast<uint32_t*>(x + j) = 0u;
+        for (int j = D + 8 * lane; j < ld; j += 256) *reinterpret_cast<uint4*>(x + j) = make_uint4(0u, 0u, 0u, 0u);   // (rows are 16-byte aligned)
         __syncwarp();
         __half* phi = x + D;
-        // Steps in chunks of 32: the warp first turns the chunk's (step, slot) parameters into log2 p with coalesced loads
-        // (one value per lane and pass), then every lane walks the chunk's steps for its own type, branch-free (a step of
-        // another type adds 0 / keeps the max): the sums see the steps in order, whatever the launch.
-        float* l2s = s_l2 + warp * (32 * 8);
-        int* ids = s_id + warp * 32;
-        for (int k0 = 0; k0 < NT; k0 += 32) {
-            const int k = k0 + lane;
+        // Steps in chunks of 32, one step per lane: the lane turns its step's parameters into log2 p; the lanes of one action
+        // type find each other (match.any), the group's first lane collects the others' values in step order (one shuffle
+        // per slot and round, as many rounds as the most frequent type has steps) and adds the chunk's partial to the
+        // type's accumulators in shared memory.  One order per sum, whatever the launch; a type that does not occur keeps
+        // the zeros the row was filled with.
+        float* acc = s_acc + warp * (kXTypes * kXAcc);
+        for (int e = lane; e < NT * kXAcc; e += 32) acc[e] = 0.0f;
+        __syncwarp();
+        for (int t0 = 0; t0 < len; t0 += 32) {
+            const int nt = min(32, len - t0);
+            const bool valid = lane < nt;
+            int id = -1 - lane;            // lanes without a step: groups of their own, ignored
+            float l2[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) l2[j] = 0.0f;
+            if (valid) {
+                id = __ldg(p.ids + (size_t)c * p.T_max + t0 + lane);
+                id = id < 0 ? 0 : (id >= NT ? NT - 1 : id);
+                const int32_t* pp = p.params + ((size_t)c * p.T_max + t0 + lane) * P;
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    if (j < P) {      // MUFU.LG2 (2 ulp in fp32): the features are stored as fp16, 11 bits
+                        const int prm = __ldg(pp + j);
+                        l2[j] = __log2f((float)(prm < 1 ? 1 : prm));
+                    }
+            }
+            const uint32_t mask = __match_any_sync(0xffffffffu, id);
+            const int leader = __ffs(mask) - 1, cnt = __popc(mask);
+            const int rounds = __reduce_max_sync(0xffffffffu, valid ? cnt : 1);
             float sum[8], mx[8];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) sum[j] = mx[j] = 0.0f;
-            int cnt = 0;
-            for (int t0 = 0; t0 < len; t0 += 32) {
-                const int nt = min(32, len - t0);
-                __syncwarp();
-                if (lane < nt) {
-                    int id = __ldg(p.ids + (size_t)c * p.T_max + t0 + lane);
-                    ids[lane] = id < 0 ? 0 : (id >= NT ? NT - 1 : id);
-                }
-                if (lane < nt) {      // lane = step of the chunk: its P parameters -> log2 p (MUFU.LG2, 2 ulp in fp32: the features
-                                      // are stored as fp16, 11 bits)
-                    const int32_t* pp = p.params + ((size_t)c * p.T_max + t0 + lane) * P;
+            for (int j = 0; j < 8; ++j) sum[j] = mx[j] = l2[j];       // the group's first step is the leader's own
+            for (int r = 1; r < rounds; ++r) {
+                const uint32_t src = __fns(mask, 0, r + 1);           // lane of the group's r-th later step (none: > 31)
+                const bool take = lane == leader && src < 32u;
 #pragma unroll
-                    for (int j = 0; j < 8; ++j)
-                        if (j < P) {
-                            const int prm = __ldg(pp + j);
-                            l2s[lane * 8 + j] = __log2f((float)(prm < 1 ? 1 : prm));
+                for (int j = 0; j < 8; ++j)
+                    if (j < P) {
+                        const float v = __shfl_sync(0xffffffffu, l2[j], (int)(src & 31u));
+                        if (take) {
+                            sum[j] += v;
+                            mx[j] = fmaxf(mx[j], v);                  // (log2 p >= 0)
                         }
-                }
-                __syncwarp();
-                for (int t = 0; t < nt; ++t) {
-                    const bool mine = ids[t] == k;
-                    cnt += mine ? 1 : 0;
-                    const float4 a0 = *reinterpret_cast<const float4*>(l2s + 8 * t), a1 = *reinterpret_cast<const float4*>(l2s + 8 * t + 4);
-                    const float v[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-#pragma unroll
-                    for (int j = 0; j < 8; ++j)
-                        if (j < P) {
-                            sum[j] += mine ? v[j] : 0.0f;
-                            mx[j] = fmaxf(mx[j], mine ? v[j] : 0.0f);      // (log2 p >= 0)
-                        }
-                }
+                    }
             }
-            if (k < NT) {
-                phi[k] = __float2half_rn((float)cnt);
-                const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
+            if (valid && lane == leader) {
+                float* a = acc + id * kXAcc;
+                a[0] += (float)cnt;
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    if (j < P) {
+                        a[1 + j] += sum[j];
+                        a[9 + j] = fmaxf(a[9 + j], mx[j]);
+                    }
+            }
+            __syncwarp();
+        }
+        for (int k = lane; k < NT; k += 32) {
+            const float* a = acc + k * kXAcc;
+            const float cntf = a[0];
+            if (cntf > 0.0f) {
+                phi[k] = __float2half_rn(cntf);
+                const float inv = 1.0f / cntf;
                 __half* q = phi + NT + 1 + k * 3 * P;
 #pragma unroll
                 for (int j = 0; j < 8; ++j)
                     if (j < P) {
-                        q[j] = __float2half_rn(sum[j]);
-                        q[P + j] = __float2half_rn(sum[j] * inv);
-                        q[2 * P + j] = __float2half_rn(mx[j]);
+                        q[j] = __float2half_rn(a[1 + j]);
+                        q[P + j] = __float2half_rn(a[1 + j] * inv);
+                        q[2 * P + j] = __float2half_rn(a[9 + j]);
                     }
             }
         }
+        __syncwarp();      // acc is cleared for the warp's next candidate
         if (lane == 0) {
             phi[NT] = __float2half_rn((float)len);
             phi[p.phi_dim] = __float2half_rn(1.0f);        // the constant column that carries bs0
@@ -428,7 +446,7 @@ int tsc_prepare(wm_ctx* ctx, const std::vector<std::vector<float>>& hv, const st
     Model& m = ctx->m;
     m.tsc_ok = 0;
     if (m.phi_kind != WM_PHI_TYPED || m.ranker_kind != WM_RANKER_MLP || !m.tcp_ok || m.d != tsc::D || m.n_lin != 3 ||
-        m.sdim[1] != tsc::SW || m.sdim[2] != tsc::SW || m.sdim[3] != 1 || m.H < 1 || m.H > 64 || m.P > 8 ||
+        m.sdim[1] != tsc::SW || m.sdim[2] != tsc::SW || m.sdim[3] != 1 || m.H < 1 || m.H > 64 || m.P > 8 || m.n_types > tsc::kXTypes ||
         (int)tsc::SMEM_TOTAL > ctx->smem_optin)
         return WM_OK;
     const int F = m.phi_dim, PKB = (F + 1 + 63) / 64, NKB = 4 + PKB + 1, KX = 64 * NKB, K0 = tsc::D + F + m.H;
