@@ -190,7 +190,8 @@ int wm_rollout_score(wm_ctx* ctx,
  * serialised by the library while they enqueue.
  * Errors: those of wm_rollout_score; WM_ERR_ARG when B > WM_STATIC_MAX_B (the message names the limit);
  * WM_ERR_UNSUPPORTED for WM_RANKER_FOREST models (they need a [B, d] latent buffer) and while WM_OPT_TIMING is on
- * (it creates events). */
+ * (it creates events).  A WM_PHI_TYPED model runs this entry on the fp32 kernel (wm_rollout_score's split of such a call
+ * needs two buffers of the batch's size). */
 #define WM_STATIC_MAX_B 262144
 int wm_rollout_score_static(wm_ctx* ctx,
                             const float* init_states, const int32_t* action_ids, const int32_t* action_params,

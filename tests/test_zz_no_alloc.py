@@ -66,6 +66,22 @@ def test_static_entry_matches_rollout_score_twice_in_a_row(wm, n, single):
     wm.wm_free(ctx)
 
 
+def test_static_entry_on_a_per_type_phi_model(wm):
+    """A WM_PHI_TYPED model: wm_rollout_score splits the call over three kernels and two workspace buffers it allocates; the
+    allocation-free entry cannot, and runs the whole call on the fp32 kernel instead (no tcgen05 rollout kernel holds a
+    scorer for this phi) — slower, and within the fp32 kernel's tolerance of the oracle."""
+    cfg = gen.get_config(14).scaled(S=2, per_subgraph=300)
+    w, b = gen.make_weights(cfg), gen.make_inputs(cfg)
+    ctx = wm.wm_load_weights(weight_file(cfg))
+    assert wm.wm_get_info(ctx).path == 2
+    ref = oracle_scores(cfg, w, b)
+    for _ in range(2):
+        y = _static_scores(wm, ctx, b)
+        assert oracle.score_error(y, ref, b.subgraph_offsets) <= 2e-3
+    assert oracle.score_error(gpu_scores(ctx, b), ref, b.subgraph_offsets) <= 2e-2      # the split call, for comparison
+    wm.wm_free(ctx)
+
+
 def test_static_entry_rejects_what_it_cannot_hold(wm):
     """B beyond WM_STATIC_MAX_B: WM_ERR_ARG and a message that names the limit (checked before any pointer is read);
     the forest ranker and WM_OPT_TIMING: WM_ERR_UNSUPPORTED; B = 0: no-op."""
