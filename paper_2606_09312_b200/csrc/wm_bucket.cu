@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(kBucketThreads) wm_len_scatter_kernel(const in
     }
 }
 
-// Both steps in ONE launch for batches whose CTAs are all resident at once (grid <= number of SMs; cfg 2 / 3: 8 / 16
+// Both steps in ONE launch for batches whose CTAs are all resident at once (grid <= 32; cfg 2 / 3: 8 / 16
 // CTAs): every CTA adds its histogram to the global one, the CTAs meet at a counter (bounded spin; co-residency makes it
 // safe), then each takes its ranges and places its candidates as wm_len_scatter_kernel does.  The lengths are read once and
 // one launch (of three in an evolution-round-sized call) goes away.  `hist` is read back through L2 (__ldcg): it was written
@@ -187,7 +187,11 @@ int launch_length_bucketing(wm_ctx* ctx, Workspace* ws, const int32_t* lengths, 
     WM_CUDA_TRY(cudaMemsetAsync(ws->counters, 0, sizeof(int32_t) * kCounterInts, st));
     const int64_t per_cta = (int64_t)kBucketThreads * kBucketItems;
     const int grid = (int)((B + per_cta - 1) / per_cta);
-    if (grid <= ctx->n_sms) {      // every CTA resident at once: one launch (the counters' memset above clears the meeting word too)
+    // one launch while every CTA is certainly resident at once: at most kSortMaxCtas CTAs of 512 threads (an SM holds four,
+    // so even a dozen such sorts on other streams, or a persistent kernel that leaves a fifth of the SMs, cannot starve the
+    // meeting); the counters' memset above clears the meeting word too
+    constexpr int kSortMaxCtas = 32;     // 131,072 candidates: cfg 2 (8 CTAs), cfg 3 (16), every search-round-sized call
+    if (grid <= kSortMaxCtas && grid <= ctx->n_sms) {
         wm_len_sort_kernel<<<grid, kBucketThreads, 0, st>>>(lengths, start, B, T_max, ws->counters + kHistOff,
                                                             ws->counters + kCursorOff, ws->counters + kTileCtrOff + 1, ws->perm);
         WM_CUDA_TRY(cudaGetLastError());
