@@ -674,6 +674,22 @@ def test_score_from_bank_matches_literal(wm, n):
         assert oracle.score_error(y, lit, b.subgraph_offsets) <= same, (n, path)
 
 
+def test_typed_phi_many_tiles_per_pair_against_the_fp32_kernel(wm):
+    """The tcgen05 ranking MLP (wm_tsc_kernel) with many tiles per CTA pair and a ragged tail: 205,100 candidates = 802 tiles of
+    256 on 74 pairs (its ring and accumulator barriers run through > 400 phases per pair), against the fp32 kernel — the
+    second, independent GPU implementation — on every candidate."""
+    cfg = gen.get_config(14).scaled(S=100, per_subgraph=2051)
+    b = gen.make_inputs(cfg)
+    ctx = _ctx(wm, cfg)
+    assert wm.wm_get_info(ctx).path == 2
+    y_tc = gpu_scores(ctx, b)
+    wm.wm_set_option(ctx, wm.WM_OPT_PATH, wm.PATH_FP32)
+    y_fp = gpu_scores(ctx, b)
+    wm.wm_free(ctx)
+    assert np.isfinite(y_tc).all()
+    assert oracle.score_error(y_tc, y_fp, b.subgraph_offsets) <= TOL[False]
+
+
 def test_path_reason_names_what_keeps_a_model_on_the_fp32_kernel(wm):
     """wm_path_reason: "" for a model a tcgen05 kernel takes; for a model one notch off a supported shape (d = 320; a scorer of
     768 units; fp32 weights) a sentence that names the property — the fallback is 50-80 x slower and must not be silent."""
