@@ -10,7 +10,8 @@ over one seeded synthetic batch of the workload config (default: BASELINE.json c
 
 `value`      : candidates/s, inputs resident in HBM, CUDA-event time per step, max over ranks, L2 flushed between steps.
 `e2e`        : the same metric through the C-ABI entry that takes HOST (pinned) buffers: H2D of the step's inputs and
-               D2H of scores + top-k indices inside the timed region.
+               D2H of scores + top-k indices inside the timed region.  The entry is wm_score_topk_host_compact (padded
+               uint8 / uint16 arrays); `e2e_ragged` (the valid steps only) and `e2e_int32` (padded int32) beside it.
 `roofline`   : rollout+score kernel (K2) alone: literal FLOPs of the batch / its CUDA-event time (WM_OPT_TIMING).
 `sustained`  : (N = 1) the headline config's wm_rollout_score launched back to back for >= 2 s with no flush in between —
                the online loop of PAPER.md:215 calls the evaluator round after round — with the clocks seen, against the
@@ -597,6 +598,11 @@ def run_ours(args, cfg):
     if compact:
         hb["ids8"] = pin(np.where(valid, batch.action_ids, 0).astype(np.uint8))
         hb["par16"] = torch.from_numpy(np.where(valid[:, :, None], batch.action_params, 1).astype(np.uint16).view(np.int16)).pin_memory()
+        # ... and ragged (a search loop holds sequences of different lengths as they are: the valid steps only, packed
+        # candidate after candidate; include/wm.h wm_score_topk_host_ragged): no padding crosses PCIe
+        hb["so"] = pin(np.concatenate([[0], np.cumsum(batch.lengths)]).astype(np.int32))
+        hb["sid8"] = pin(batch.action_ids[valid].astype(np.uint8))
+        hb["spar16"] = torch.from_numpy(np.ascontiguousarray(batch.action_params[valid]).astype(np.uint16).view(np.int16)).pin_memory()
 
     def e2e_step_int32():
         wm.wm_score_topk_host(ctx, hb["z0"], hb["ids"], hb["par"], hb["ln"], hb["hw"], hb["off"], k, h_scores, h_idx)
@@ -604,25 +610,45 @@ def run_ours(args, cfg):
     def e2e_step_compact():
         wm.wm_score_topk_host_compact(ctx, hb["z0"], hb["ids8"], hb["par16"], hb["ln"], hb["hw"], hb["off"], k, h_scores, h_idx)
 
-    def time_e2e(fn):
-        for _ in range(3):
+    def e2e_step_ragged():
+        wm.wm_score_topk_host_ragged(ctx, hb["z0"], hb["sid8"], hb["spar16"], hb["so"], hb["hw"], hb["off"], batch.T_max, k,
+                                     h_scores, h_idx)
+
+    def time_e2e_all(fns):
+        """K synchronous calls of every entry, one entry after the other (alternating between the entries was measured: each
+        has its own pinned buffers, 52 MB in all, and on these boxes — a VM behind an IOMMU — a call that follows a call on
+        OTHER buffers is 0.2-0.3 ms slower than one that repeats its own); seconds per call of each entry, max over ranks."""
+        for fn in fns:
             fn()
+            np.testing.assert_array_equal(h_idx.numpy(), idx.cpu().numpy())   # same answer through every entry
+        total = [0.0] * len(fns)
+        left = [args.steps] * len(fns)
+        block = args.steps
         barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            fn()          # synchronous: returns after the D2H copies
+        while any(left):
+            for i, fn in enumerate(fns):
+                n = min(block, left[i])
+                if n == 0:
+                    continue
+                for _ in range(3):
+                    fn()          # warm-up of this entry's block
+                t0 = time.perf_counter()
+                for _ in range(n):
+                    fn()          # synchronous: returns after the D2H copies
+                total[i] += time.perf_counter() - t0
+                left[i] -= n
         torch.cuda.synchronize()
-        secs = reduce_max((time.perf_counter() - t0) / args.steps, dist, dev)
-        np.testing.assert_array_equal(h_idx.numpy(), idx.cpu().numpy())   # same answer through every entry
-        return secs
+        return [reduce_max(t / args.steps, dist, dev) for t in total]
 
     nbytes = lambda names: sum(int(hb[n].numel() * hb[n].element_size()) for n in names)
-    e2e32_s = time_e2e(e2e_step_int32)
     h2d32 = nbytes(("z0", "ids", "par", "ln", "hw", "off"))
+    e2er_s = h2dr = None
     if compact:
-        e2e_s = time_e2e(e2e_step_compact)
+        e2e32_s, e2e_s, e2er_s = time_e2e_all([e2e_step_int32, e2e_step_compact, e2e_step_ragged])
         h2d = nbytes(("z0", "ids8", "par16", "ln", "hw", "off"))
+        h2dr = nbytes(("z0", "sid8", "spar16", "so", "hw", "off"))
     else:
+        (e2e32_s,) = time_e2e_all([e2e_step_int32])
         e2e_s, h2d = e2e32_s, h2d32
     d2h = int(h_scores.numel() * 4 + h_idx.numel() * 4)
     del hb, h_scores, h_idx
@@ -653,6 +679,10 @@ def run_ours(args, cfg):
            "e2e_int32": {"value": cands_all / e2e32_s, "unit": UNIT, "h2d_bytes_per_step": h2d32, "d2h_bytes_per_step": d2h,
                          "ms_per_step": e2e32_s * 1e3, "entry": "wm_score_topk_host (int32)"},
            "roofline": roof}
+    if e2er_s is not None:
+        out["e2e_ragged"] = {"value": cands_all / e2er_s, "unit": UNIT, "h2d_bytes_per_step": h2dr, "d2h_bytes_per_step": d2h,
+                             "ms_per_step": e2er_s * 1e3,
+                             "entry": "wm_score_topk_host_ragged (valid steps only: uint8 ids, uint16 params, int32 step offsets)"}
     if sustained is not None:
         out["sustained"] = sustained
     if prefix is not None:

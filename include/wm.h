@@ -269,6 +269,18 @@ int wm_score_topk_host_compact(wm_ctx* ctx,
                                int64_t B, int32_t S, int32_t T_max, int32_t k,
                                float* scores_out, int32_t* idx_out, void* cuda_stream);
 
+/* The same with the VALID steps only (candidates of one search round have very different lengths; at cfg 2 the
+ * padded arrays are 37 % padding).  step_offsets [B + 1] int32 (host): candidate b's steps are rows
+ * [step_offsets[b], step_offsets[b + 1]) of step_ids [N] uint8 and step_params [N, P] uint16, N = step_offsets[B],
+ * step_offsets[0] = 0; its length is the difference (a length above T_max raises WM_FAULT_LEN and is clamped).  The packed
+ * arrays are staged as they are and expanded on the device.  Results are bit-identical to wm_score_topk_host on the padded
+ * form of the same candidates.  Errors: as wm_score_topk_host_compact; WM_ERR_ARG for inconsistent step_offsets. */
+int wm_score_topk_host_ragged(wm_ctx* ctx,
+                              const float* init_states, const uint8_t* step_ids, const uint16_t* step_params,
+                              const int32_t* step_offsets, const float* hw_feats, const int32_t* subgraph_offsets,
+                              int64_t B, int32_t S, int32_t T_max, int32_t k,
+                              float* scores_out, int32_t* idx_out, void* cuda_stream);
+
 /* With WM_OPT_TIMING = 1: synchronise `cuda_stream` and return, in *ms_out, the device time of the rollout+score
  * kernel (K2 alone: bucketing and top-k excluded) of the most recent wm_rollout_score call made on that stream.
  * bench.py's roofline leg uses it.  Errors: WM_ERR_ARG (null, timing off, or no call yet), WM_ERR_CUDA. */

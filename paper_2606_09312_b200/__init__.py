@@ -24,7 +24,7 @@ PATH_AUTO, PATH_FP32, PATH_TCGEN05 = 0, 1, 2
 # every symbol include/wm.h declares
 ABI_SYMBOLS = ("wm_load_weights", "wm_free", "wm_get_info", "wm_set_option", "wm_rollout_score", "wm_topk",
                "wm_rollout_latents", "wm_rollout_score_from", "wm_rollout_score_static",
-               "wm_check", "wm_score_topk_host", "wm_score_topk_host_compact", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error", "wm_path_reason")
+               "wm_check", "wm_score_topk_host", "wm_score_topk_host_compact", "wm_score_topk_host_ragged", "wm_last_kernel_ms", "wm_launch_count", "wm_launch_empty", "wm_last_error", "wm_path_reason")
 
 
 class WmInfo(ctypes.Structure):
@@ -79,6 +79,8 @@ def lib() -> ctypes.CDLL:
     L.wm_score_topk_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp, vp, vp]
     L.wm_score_topk_host.restype = ctypes.c_int
     L.wm_score_topk_host_compact.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp, vp, vp]
+    L.wm_score_topk_host_ragged.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i32, i32, i32, vp, vp, vp]
+    L.wm_score_topk_host_ragged.restype = ctypes.c_int
     L.wm_score_topk_host_compact.restype = ctypes.c_int
     L.wm_last_kernel_ms.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_float)]
     L.wm_last_kernel_ms.restype = ctypes.c_int
@@ -158,6 +160,19 @@ def wm_rollout_score_static(ctx: int, init_states, action_ids, action_params, le
     _check(lib().wm_rollout_score_static(ctx, _ptr(init_states), _ptr(action_ids), _ptr(action_params), _ptr(lengths),
                                          _ptr(hw_feats), _ptr(scores_out), _ptr(subgraph_offsets), B, S, T_max,
                                          _stream(stream)))
+
+
+def wm_score_topk_host_ragged(ctx: int, init_states, step_ids_u8, step_params_u16, step_offsets, hw_feats, subgraph_offsets,
+                              T_max: int, k: int, scores_out, idx_out, stream=None) -> None:
+    """wm_score_topk_host on the valid steps only (HOST tensors): step_ids [N] uint8, step_params [N, P] uint16,
+    step_offsets [B + 1] int32.  include/wm.h."""
+    import torch
+    assert step_ids_u8.dtype == torch.uint8 and step_params_u16.dtype in (torch.uint16, torch.int16)
+    B = int(step_offsets.numel()) - 1
+    S = int(subgraph_offsets.numel()) - 1
+    _check(lib().wm_score_topk_host_ragged(ctx, _ptr(init_states), _ptr(step_ids_u8), _ptr(step_params_u16), _ptr(step_offsets),
+                                           _ptr(hw_feats), _ptr(subgraph_offsets), B, S, int(T_max), int(k),
+                                           _ptr(scores_out), _ptr(idx_out), _stream(stream)))
 
 
 def wm_rollout_latents(ctx: int, init_states, action_ids, action_params, lengths, latents_out,

@@ -844,21 +844,48 @@ __global__ void wm_widen_kernel(const uint8_t* __restrict__ ids8, const uint16_t
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_ids; i += stride) ids[i] = ids8[i];
 }
 
-// Shared body of wm_score_topk_host (int32 arrays: ib = pb = 4) and wm_score_topk_host_compact (ib = 1, pb = 2: the arrays
-// are staged as they come and widened on the device by wm_widen_kernel).
+// Ragged entry: the VALID steps only, packed candidate after candidate (ids8 [N], par16 [N, P], so [B + 1] = first step of
+// every candidate, all indexed from the call's first step) -> the padded int32 arrays the kernels read and the lengths.
+// Positions past a candidate's length are left as they are: no kernel reads them.  A length outside [0, T_max] is stored as
+// it is (K2 clamps it and raises WM_FAULT_LEN) and clamped here.
+__global__ void wm_expand_kernel(const uint8_t* __restrict__ ids8, const uint16_t* __restrict__ par16,
+                                 const int32_t* __restrict__ so, int32_t* __restrict__ ids, int32_t* __restrict__ par,
+                                 int32_t* __restrict__ lens, int64_t c0, int64_t Bc, int T_max, int P) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, n = Bc * T_max;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += stride) {
+        const int64_t b = c0 + e / T_max;
+        const int t = (int)(e % T_max);
+        const int first = so[b], len = so[b + 1] - first;
+        if (t == 0) lens[b] = len;
+        if (t < len) {
+            const int64_t src = (int64_t)first + t, dst = b * T_max + t;
+            ids[dst] = ids8[src];
+            for (int j = 0; j < P; ++j) par[dst * P + j] = par16[src * P + j];
+        }
+    }
+}
+
+// Shared body of wm_score_topk_host (int32 arrays: ib = pb = 4), wm_score_topk_host_compact (ib = 1, pb = 2: the arrays
+// are staged as they come and widened on the device by wm_widen_kernel) and wm_score_topk_host_ragged (ib = 1, pb = 2,
+// step_offsets non-null: valid steps only, expanded on the device by wm_expand_kernel).
 static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const void* action_ids, const void* action_params,
-                                int ib, int pb, const int32_t* lengths, const float* hw_feats,
+                                int ib, int pb, const int32_t* lengths, const int32_t* step_offsets, const float* hw_feats,
                                 const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
                                 float* scores_out, int32_t* idx_out, void* cuda_stream) {
-    const bool compact = ib != 4;
+    const bool compact = ib != 4, ragged = step_offsets != nullptr;
     if (!ctx) {
         set_error("wm_score_topk_host: null ctx");
         return WM_ERR_ARG;
     }
     if (B < 0 || B > 0x7fffffffLL || S < 1 || T_max < 0 || T_max > WM_MAX_T || k <= 0 || k > WM_MAX_K ||
-        !subgraph_offsets || !idx_out || !init_states || !lengths || (ctx->m.H > 0 && !hw_feats) ||
+        !subgraph_offsets || !idx_out || !init_states || (!lengths && !ragged) || (ctx->m.H > 0 && !hw_feats) ||
         (B > 0 && T_max > 0 && (!action_ids || !action_params))) {
         set_error("wm_score_topk_host: bad argument");
+        return WM_ERR_ARG;
+    }
+    const int64_t n_steps = ragged ? (B > 0 ? (int64_t)step_offsets[B] - step_offsets[0] : 0) : 0;
+    if (ragged && B > 0 && (step_offsets[0] != 0 || n_steps < 0 || n_steps > B * (int64_t)T_max)) {
+        set_error("wm_score_topk_host_ragged: step_offsets must start at 0 and end at the number of valid steps (<= B * T_max)");
         return WM_ERR_ARG;
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -894,8 +921,10 @@ static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const voi
         cs[nch] = S;
     }
     const size_t b_reb = up16((size_t)(S + 5) * 4);
-    const size_t b_ids8 = compact ? up16((size_t)B * T_max * ib) : 0, b_par16 = compact ? up16((size_t)B * T_max * m.P * pb) : 0;
-    const size_t need = b_z0 + b_hw + b_ids + b_par + b_len + b_off + b_sc + b_idx + b_reb + b_ids8 + b_par16;
+    const size_t n_raw = ragged ? (size_t)n_steps : (size_t)B * T_max;      // staged 8- / 16-bit elements (per slot)
+    const size_t b_ids8 = compact ? up16(n_raw * ib) : 0, b_par16 = compact ? up16(n_raw * m.P * pb) : 0;
+    const size_t b_so = ragged ? up16((size_t)(B + 1) * 4) : 0;
+    const size_t need = b_z0 + b_hw + b_ids + b_par + b_len + b_off + b_sc + b_idx + b_reb + b_ids8 + b_par16 + b_so;
     if (ws->stage_cap < need) {
         if (ws->stage) {
             WM_CUDA_TRY(cudaStreamSynchronize(st));
@@ -917,7 +946,8 @@ static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const voi
     int32_t* didx = (int32_t*)p; p += b_idx;
     int32_t* dreb = (int32_t*)p; p += b_reb;
     uint8_t* dids8 = (uint8_t*)p; p += b_ids8;
-    uint16_t* dpar16 = (uint16_t*)p;
+    uint16_t* dpar16 = (uint16_t*)p; p += b_par16;
+    int32_t* dso = (int32_t*)p;
     const auto H2D = cudaMemcpyHostToDevice;
     const char* h_ids = static_cast<const char*>(action_ids);
     const char* h_par = static_cast<const char*>(action_params);
@@ -926,7 +956,14 @@ static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const voi
     auto copy_actions = [&](int64_t c0, int64_t Bc, cudaStream_t cs) -> int {
         if (Bc <= 0 || T_max <= 0) return WM_OK;
         const size_t ni = (size_t)Bc * T_max, np_ = ni * m.P;
-        if (!compact) {
+        if (ragged) {      // the candidates' valid steps are one contiguous run of the packed arrays
+            const size_t n0 = (size_t)step_offsets[c0], n1 = (size_t)step_offsets[c0 + Bc];
+            WM_CUDA_TRY(cudaMemcpyAsync(dso + c0, step_offsets + c0, (size_t)(Bc + 1) * 4, H2D, cs));
+            if (n1 > n0) {
+                WM_CUDA_TRY(cudaMemcpyAsync(dids8 + n0, h_ids + n0, n1 - n0, H2D, cs));
+                WM_CUDA_TRY(cudaMemcpyAsync(dpar16 + n0 * m.P, h_par + n0 * m.P * 2, (n1 - n0) * m.P * 2, H2D, cs));
+            }
+        } else if (!compact) {
             WM_CUDA_TRY(cudaMemcpyAsync(dids + c0 * T_max, h_ids + (size_t)c0 * T_max * 4, ni * 4, H2D, cs));
             WM_CUDA_TRY(cudaMemcpyAsync(dpar + c0 * T_max * m.P, h_par + (size_t)c0 * T_max * m.P * 4, np_ * 4, H2D, cs));
         } else {
@@ -936,9 +973,16 @@ static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const voi
         return WM_OK;
     };
     auto widen = [&](int64_t c0, int64_t Bc, cudaStream_t ks) -> int {
+        if (ragged && Bc > 0 && T_max <= 0) WM_CUDA_TRY(cudaMemsetAsync(dlen + c0, 0, (size_t)Bc * 4, ks));   // (no step can exist)
         if (!compact || Bc <= 0 || T_max <= 0) return WM_OK;
         const int64_t ni = Bc * T_max, np_ = ni * m.P;
         const int grid = (int)std::min<int64_t>((np_ + 255) / 256, (int64_t)ctx->n_sms * 8);
+        if (ragged) {
+            wm_expand_kernel<<<grid, 256, 0, ks>>>(dids8, dpar16, dso, dids, dpar, dlen, c0, Bc, T_max, m.P);
+            WM_CUDA_TRY(cudaGetLastError());
+            ctx->launches.fetch_add(1);
+            return WM_OK;
+        }
         wm_widen_kernel<<<grid, 256, 0, ks>>>(dids8 + c0 * T_max, dpar16 + c0 * T_max * m.P, dids + c0 * T_max,
                                               dpar + c0 * T_max * m.P, ni, np_);
         WM_CUDA_TRY(cudaGetLastError());
@@ -983,7 +1027,7 @@ static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const voi
             const int s0 = cs[c], Sc = cs[c + 1] - cs[c];
             const int64_t c0 = subgraph_offsets[s0], Bc = (int64_t)subgraph_offsets[cs[c + 1]] - c0;
             if (Bc > 0) {
-                WM_CUDA_TRY(cudaMemcpyAsync(dlen + c0, lengths + c0, (size_t)Bc * 4, H2D, cp));
+                if (!ragged) WM_CUDA_TRY(cudaMemcpyAsync(dlen + c0, lengths + c0, (size_t)Bc * 4, H2D, cp));
                 const int rc0 = copy_actions(c0, Bc, cp);
                 if (rc0 != WM_OK) return rc0;
             }
@@ -1026,7 +1070,7 @@ static int score_topk_host_impl(wm_ctx* ctx, const float* init_states, const voi
         if (rc0 == WM_OK) rc0 = widen(0, B, st);
         if (rc0 != WM_OK) return rc0;
     }
-    if (B) WM_CUDA_TRY(cudaMemcpyAsync(dlen, lengths, (size_t)B * 4, H2D, st));
+    if (B && !ragged) WM_CUDA_TRY(cudaMemcpyAsync(dlen, lengths, (size_t)B * 4, H2D, st));
     WM_CUDA_TRY(cudaMemcpyAsync(doff, subgraph_offsets, (size_t)(S + 1) * 4, H2D, st));
     int rc = wm_rollout_score(ctx, dz0, dids, dpar, dlen, dhw, dsc, doff, B, S, T_max, cuda_stream);
     if (rc != WM_OK) return rc;
@@ -1048,7 +1092,7 @@ int wm_score_topk_host(wm_ctx* ctx, const float* init_states, const int32_t* act
                        const int32_t* action_params, const int32_t* lengths, const float* hw_feats,
                        const int32_t* subgraph_offsets, int64_t B, int32_t S, int32_t T_max, int32_t k,
                        float* scores_out, int32_t* idx_out, void* cuda_stream) {
-    return score_topk_host_impl(ctx, init_states, action_ids, action_params, 4, 4, lengths, hw_feats, subgraph_offsets, B, S,
+    return score_topk_host_impl(ctx, init_states, action_ids, action_params, 4, 4, lengths, nullptr, hw_feats, subgraph_offsets, B, S,
                                 T_max, k, scores_out, idx_out, cuda_stream);
 }
 
@@ -1060,8 +1104,23 @@ int wm_score_topk_host_compact(wm_ctx* ctx, const float* init_states, const uint
         set_error("wm_score_topk_host_compact: uint8 type ids need n_types <= 256");
         return WM_ERR_UNSUPPORTED;
     }
-    return score_topk_host_impl(ctx, init_states, action_ids, action_params, 1, 2, lengths, hw_feats, subgraph_offsets, B, S,
+    return score_topk_host_impl(ctx, init_states, action_ids, action_params, 1, 2, lengths, nullptr, hw_feats, subgraph_offsets, B, S,
                                 T_max, k, scores_out, idx_out, cuda_stream);
+}
+
+int wm_score_topk_host_ragged(wm_ctx* ctx, const float* init_states, const uint8_t* step_ids, const uint16_t* step_params,
+                              const int32_t* step_offsets, const float* hw_feats, const int32_t* subgraph_offsets, int64_t B,
+                              int32_t S, int32_t T_max, int32_t k, float* scores_out, int32_t* idx_out, void* cuda_stream) {
+    if (ctx && ctx->m.n_types > 256) {
+        set_error("wm_score_topk_host_ragged: uint8 type ids need n_types <= 256");
+        return WM_ERR_UNSUPPORTED;
+    }
+    if (!step_offsets) {
+        set_error("wm_score_topk_host_ragged: null step_offsets");
+        return WM_ERR_ARG;
+    }
+    return score_topk_host_impl(ctx, init_states, step_ids, step_params, 1, 2, nullptr, step_offsets, hw_feats, subgraph_offsets,
+                                B, S, T_max, k, scores_out, idx_out, cuda_stream);
 }
 
 int64_t wm_launch_count(const wm_ctx* ctx) {

@@ -428,6 +428,18 @@ def test_host_entry_matches_device_entry(wm, n, S, per):
     assert wm.wm_check(ctx) == 0
     np.testing.assert_array_equal(sc2.numpy().view(np.uint32), y.view(np.uint32))
     np.testing.assert_array_equal(ix2.numpy(), idx)
+    # the ragged entry (valid steps only, packed candidate after candidate): same bits again
+    so = np.concatenate([[0], np.cumsum(b.lengths)]).astype(np.int32)
+    step_ids = b.action_ids[valid].astype(np.uint8)                         # row-major: candidate after candidate
+    step_par = b.action_params[valid].astype(np.uint16)                     # [N, P]
+    assert step_ids.shape[0] == so[-1] and step_par.shape == (so[-1], b.action_params.shape[2])
+    sc3 = torch.empty(b.B, dtype=torch.float32).pin_memory()
+    ix3 = torch.empty((b.S, cfg.k), dtype=torch.int32).pin_memory()
+    wm.wm_score_topk_host_ragged(ctx, h(b.init_states), h(step_ids), torch.from_numpy(step_par.view(np.int16)).pin_memory(), h(so),
+                                 h(b.hw_feats), h(b.subgraph_offsets), b.T_max, cfg.k, sc3, ix3)
+    assert wm.wm_check(ctx) == 0
+    np.testing.assert_array_equal(sc3.numpy().view(np.uint32), y.view(np.uint32))
+    np.testing.assert_array_equal(ix3.numpy(), idx)
     wm.wm_free(ctx)
 
 
